@@ -1,0 +1,75 @@
+"""Test-only helpers that are independent of BOTH the oracle and the CUDA path: dense numpy
+restatements of the paper's definitions, used to pin the oracle."""
+import itertools
+
+import numpy as np
+
+
+def dense_adj(n, rp, ci, wt=None):
+    """A in N_0^{n x n}; duplicate entries add."""
+    A = np.zeros((n, n), dtype=np.int64)
+    for i in range(n):
+        for e in range(rp[i], rp[i + 1]):
+            A[i, ci[e]] += 1 if wt is None else int(wt[e])
+    return A
+
+
+def indicator(colors):
+    colors = np.asarray(colors)
+    k = int(colors.max()) + 1 if colors.size else 0
+    S = np.zeros((colors.size, k), dtype=np.int64)
+    S[np.arange(colors.size), colors] = 1
+    return S
+
+
+def stable_dense(A, colors):
+    """Def. 1 (L47-L49) literally: rows of A.S are equal inside every block."""
+    AS = A @ indicator(colors)
+    colors = np.asarray(colors)
+    for b in np.unique(colors):
+        rows = AS[colors == b]
+        if not (rows == rows[0]).all():
+            return False
+    return True
+
+
+def set_partitions(n):
+    """All set partitions of range(n) as restricted-growth strings."""
+    def rec(prefix, mx):
+        if len(prefix) == n:
+            yield tuple(prefix)
+            return
+        for v in range(mx + 2):
+            yield from rec(prefix + [v], max(mx, v))
+    if n == 0:
+        yield ()
+        return
+    yield from rec([0], 0)
+
+
+def refines(fine, coarse):
+    """every block of `fine` lies inside one block of `coarse` (Def. 2)."""
+    fine, coarse = np.asarray(fine), np.asarray(coarse)
+    m = {}
+    for f, c in zip(fine.tolist(), coarse.tolist()):
+        if m.setdefault(f, c) != c:
+            return False
+    return True
+
+
+def brute_force_coarsest(A, init):
+    """Def. 3 (L57) + L94 by exhaustion: among all partitions that refine `init` and are stable, the one with
+    the fewest blocks; asserts it is unique and that every other stable refinement of init refines it."""
+    n = A.shape[0]
+    stable = [p for p in set_partitions(n) if refines(p, init) and stable_dense(A, p)]
+    assert stable, "the discrete partition is always stable"
+    kmin = min(max(p) + 1 for p in stable)
+    best = [p for p in stable if max(p) + 1 == kmin]
+    assert len(best) == 1
+    for p in stable:
+        assert refines(p, best[0])
+    return np.array(best[0], dtype=np.int32)  # restricted growth string == first-occurrence numbering
+
+
+def same_partition(a, b):
+    return refines(a, b) and refines(b, a)
