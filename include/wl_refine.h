@@ -1,0 +1,181 @@
+/*
+ * wl_refine.h — C ABI of the B200-native randomized 1-WL colour refinement library.
+ *
+ * Implements, with hand-written sm_100a CUDA kernels, the data-parallel hot path of
+ * arxiv/paper_2607_02603 ("Scaling Weisfeiler-Leman Expressiveness Analysis to Massive Graphs with GPUs"):
+ *   Algorithm 1, RSC: random weight per colour, z = A w over Z/2^64, relabel (colour, z)
+ *   Algorithm 2, RBSC: edge batches, inner nodes (Def. 5), local RSC, merge (Eq. 4), quotient (Def. 4)
+ * Citations "L<n>" are line numbers of PAPER.md; "Q<n>" are the readings listed in DESIGN.md.
+ *
+ * General conventions
+ *   - Graph = CSR whose ROWS ARE SOURCES: a_ij = (weighted) number of edges i -> j, sums run over row i (L43, L49, Q8).
+ *     row_ptr int64[n+1] (row_ptr[0] = 0, non-decreasing, row_ptr[n] = m), col_idx int32[m] in [0, n),
+ *     weights uint32[m] (>= 0) or NULL meaning all ones.  Duplicate (i, j) entries add (a_ij in N_0, L43, Q10).
+ *   - Preconditions of Theorem 1 (L129): n <= 2^31 - 2 here (int32 ids; the paper allows 2^32) and every row sum <= 2^32.
+ *   - Arithmetic is the ring Z/2^64 (unsigned 64-bit wrap-around, L100, Q3).  No floating point on the path.
+ *   - Colours returned to the caller are CANONICAL: ids 0..k-1 in order of first occurrence, so equal partitions give
+ *     equal arrays (Q7, Q21).
+ *   - "device" pointers are CUDA device memory of the current device, "host" pointers are host memory (pinned
+ *     recommended for the *_host / batched entry points).  All buffers are owned by the caller; the library never
+ *     frees caller memory.  Entry points taking a workspace allocate nothing on the device.
+ *   - cuda_stream is a cudaStream_t cast to void* (NULL = default stream).  Calls return after the result is
+ *     complete on that stream (they synchronise the stream to read the convergence state).
+ *   - Return value: WL_OK (0) or a negative wl_status.  Functions never throw and never call exit().
+ *   - There is NO CPU fallback: without a CUDA device every compute entry point returns WL_ECUDA.
+ */
+#ifndef WL_REFINE_H_
+#define WL_REFINE_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum wl_status {
+  WL_OK = 0,
+  WL_EINVAL = -1,     /* null pointer, negative size, malformed CSR (bad offsets, column out of range)            */
+  WL_ERANGE = -2,     /* n too large for int32 ids, or a row sum above 2^32 (Theorem 1 precondition, L129)        */
+  WL_ENOMEM = -3,     /* workspace / device cap too small, or a device allocation failed                           */
+  WL_ECUDA = -4,      /* a CUDA call failed (wl_last_cuda_error() gives the cudaError_t)                           */
+  WL_EMAXROUNDS = -5  /* max_rounds / max_outer_iters reached before the fixed point                               */
+} wl_status;
+
+/* Adjacency in CSR form; all three arrays live where the entry point says (device or host). */
+typedef struct wl_csr {
+  int64_t n;               /* nodes                                            */
+  int64_t m;               /* stored entries                                   */
+  const int64_t* row_ptr;  /* n + 1 offsets                                    */
+  const int32_t* col_idx;  /* m targets                                        */
+  const uint32_t* weights; /* m edge weights, or NULL = unweighted (all ones)  */
+} wl_csr;
+
+/* flags for wl_options.flags */
+#define WL_FLAG_NO_VALIDATE 1u   /* skip the CSR validation pass (one extra read of col_idx)                          */
+#define WL_FLAG_NO_PRUNE 2u      /* keep every row in every round (no active-set pruning); results are identical      */
+#define WL_FLAG_ROW_KERNEL 4u    /* use the simple warp-per-row SpMV instead of the edge-balanced merge-path kernel   */
+#define WL_FLAG_AGGRESSIVE_STOP 8u /* batched: stop when the next iteration's N_b would not decrease (L328)            */
+#define WL_FLAG_NO_CANONICAL 16u /* leave internal dense ids in out_colors (skips S6)                                  */
+
+typedef struct wl_options {
+  uint32_t flags;           /* WL_FLAG_*                                                                             */
+  int32_t max_rounds;       /* <= 0: n + 1 (Alg. 1 needs at most n refinement steps, L416)                           */
+  uint64_t stream_id;       /* second input of the round key (outer iteration / batch id); 0 for plain RSC           */
+  int64_t* round_colors;    /* host, optional: number of colours after every round (the trajectory the oracle prints) */
+  int32_t round_colors_cap; /* capacity of round_colors                                                              */
+  int32_t max_outer_iters;  /* batched only; <= 0: unlimited                                                          */
+} wl_options;
+
+typedef struct wl_stats {
+  int32_t rounds;            /* refinement rounds executed (the last one only confirms, Q1/Q2)                        */
+  int32_t outer_iters;       /* batched: outer iterations of Alg. 2; 0 for wl_refine                                  */
+  int64_t num_colors;        /* |H| of the result                                                                     */
+  int64_t last_num_batches;  /* batched: N_b of the last outer iteration                                              */
+  int64_t boundary_nodes;    /* batched: boundary nodes (Def. 5) in the first outer iteration                         */
+  int64_t edges_streamed;    /* column indices actually consumed by SpMV kernels over all rounds                      */
+  int64_t bytes_h2d;         /* host -> device bytes moved by the call                                                */
+  int64_t bytes_d2h;         /* device -> host bytes moved by the call                                                */
+  double ms_total;           /* device time of the whole call (CUDA events on cuda_stream)                            */
+  double ms_spmv;            /* sum over rounds of the S1+S2 kernels                                                  */
+  double ms_relabel;         /* sum over rounds of the S3+S4 kernels                                                  */
+} wl_stats;
+
+/* ------------------------------------------------------------------------------------------------------------------
+ * Single batch: Algorithm 1 (RSC), L106-L127, from an arbitrary initial partition (L94).
+ * ---------------------------------------------------------------------------------------------------------------- */
+
+/* Bytes of device workspace wl_refine needs for a graph with n nodes and m entries (0 on invalid sizes). */
+size_t wl_refine_workspace_bytes(int64_t n, int64_t m);
+
+/* Coarsest stable colouring refining init_colors, with error probability <= 1e-9 (Theorem 1).
+ *   g            CSR, all arrays DEVICE.
+ *   init_colors  DEVICE int32[n], arbitrary non-negative labels (equal label = same block), or NULL = one block.
+ *   seed         seeds the per-round weights  w(c) = P_key(c), key = f(seed, opt->stream_id, round)  (Q4, Q5).
+ *   out_colors   DEVICE int32[n]; canonical ids on return (may alias init_colors).
+ *   stats        HOST, may be NULL.      opt  HOST, may be NULL (defaults).
+ *   workspace    DEVICE, >= wl_refine_workspace_bytes(n, m), 256-byte aligned; contents undefined before and after.
+ * Errors: WL_EINVAL, WL_ERANGE, WL_ENOMEM (workspace too small), WL_ECUDA, WL_EMAXROUNDS. */
+int wl_refine(const wl_csr* g, const int32_t* init_colors, uint64_t seed, int32_t* out_colors, wl_stats* stats,
+              const wl_options* opt, void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* Same computation from HOST buffers (the end-to-end call): allocates its own device memory, copies the CSR and
+ * init_colors host -> device, runs wl_refine, copies the colours device -> host.  g arrays, init_colors, out_colors: HOST. */
+int wl_refine_host(const wl_csr* g, const int32_t* init_colors, uint64_t seed, int32_t* out_colors, wl_stats* stats,
+                   const wl_options* opt, void* cuda_stream);
+
+/* ------------------------------------------------------------------------------------------------------------------
+ * Step-level entry points, used by the parity tests and the benchmark.
+ * ---------------------------------------------------------------------------------------------------------------- */
+
+/* key(seed, stream_id, round) of the weight bijection (HOST computation, pure). Round numbers start at 1. */
+uint64_t wl_round_key(uint64_t seed, uint64_t stream_id, uint64_t round);
+/* w(c) = P_key(c) (HOST computation, pure): the weight Algorithm 1 line 3 assigns to colour c (L115-L118). */
+uint64_t wl_weight(uint64_t key, uint64_t color);
+
+/* S1+S2: y_i = sum_j a_ij * w(colors[j]) mod 2^64 (Alg. 1 line 5, L120).  colors: DEVICE int32[n] (any non-negative
+ * ids); y: DEVICE uint64[n]; workspace as for wl_refine.  flags: WL_FLAG_ROW_KERNEL selects the simple kernel. */
+int wl_spmv_round(const wl_csr* g, const int32_t* colors, uint64_t key, uint64_t* y, uint32_t flags, void* workspace,
+                  size_t workspace_bytes, void* cuda_stream);
+
+/* S3+S4: new_colors = dense ids (0..k'-1, unspecified order) of the exact pairs (colors[i], y[i]) (Alg. 1 line 6,
+ * L122; Q6).  colors must be dense ids 0..k-1 (k given).  num_colors: HOST, receives k'.  new_colors may alias colors.
+ * Blocks that do not split keep their id. */
+int wl_relabel(int64_t n, const int32_t* colors, int64_t k, const uint64_t* y, int32_t* new_colors, int64_t* num_colors,
+               void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* S6: canonical first-occurrence renumbering.  colors: DEVICE int32[n] with ids in [0, n); out may alias colors;
+ * num_colors HOST (may be NULL). */
+int wl_canonicalize(int64_t n, const int32_t* colors, int32_t* out, int64_t* num_colors, void* workspace,
+                    size_t workspace_bytes, void* cuda_stream);
+
+/* ------------------------------------------------------------------------------------------------------------------
+ * Batched: Algorithm 2 (RBSC), L169-L202, over HOST-resident edge batches.
+ * ---------------------------------------------------------------------------------------------------------------- */
+
+/* One batch E_k of the edge partition (L137, L180).  Either
+ *   CSR-slice form (src == NULL): the batch owns the consecutive CSR edge positions [edge_begin, edge_begin + num_edges) of a
+ *     global CSR whose row_ptr (HOST, n + 1 offsets, shared by all batches) is given in every batch; col_idx / weights point at
+ *     THIS batch's first entry; or
+ *   COO form (src != NULL): arbitrary edges (src[e], col_idx[e]) with optional weights; row_ptr is ignored. */
+typedef struct wl_edge_batch {
+  int64_t edge_begin;
+  int64_t num_edges;
+  const int64_t* row_ptr;
+  const int32_t* col_idx;
+  const uint32_t* weights;
+  const int32_t* src;
+} wl_edge_batch;
+
+/* Stable colouring of (V, A) by Algorithm 2; equals the coarsest one whenever the loop ends with N_b = 1 (L208).
+ *   batches          HOST array of num_batches descriptors = the edge partition of outer iteration 1 (Alg. 2 line 5).
+ *                    num_batches == 0: `whole` must be given and the library cuts it itself (Q13).
+ *   whole            HOST CSR of the full graph, or NULL when batches are given in COO form.
+ *   max_batch_edges  M_b (L171): cap on edges per batch for the library's own partitions (later outer iterations, Q14).
+ *   device_cap_bytes upper bound on device memory the call may allocate (0 = no cap); WL_ENOMEM if it cannot be met.
+ *   out_colors       HOST int32[n], canonical ids on the ORIGINAL nodes (Q16). */
+int wl_refine_batched(int64_t n, int32_t num_batches, const wl_edge_batch* batches, const wl_csr* whole, uint64_t seed,
+                      size_t device_cap_bytes, int64_t max_batch_edges, int32_t* out_colors, wl_stats* stats,
+                      const wl_options* opt, void* cuda_stream);
+
+/* B2: inner-node labels of Def. 5 (L139-L145) by the method of L463.  edge_batch: DEVICE int32[m] batch id of every CSR edge
+ * slot; sink_batch: DEVICE int32[n] label given to nodes without out-edges (Q9); label: DEVICE int32[n], -1 = boundary. */
+int wl_inner_labels(int64_t n, const int64_t* row_ptr, const int32_t* edge_batch, const int32_t* sink_batch, int32_t* label,
+                    void* cuda_stream);
+
+/* B6: quotient graph of Def. 4 / Eq. 1 (L59-L65) for canonical colours (representative = first node of a block, Q17).
+ * All arrays DEVICE.  q_row_ptr int64[k+1]; q_col / q_weights capacity q_cap entries; *q_m (HOST) receives the entry count.
+ * Columns of a row come out sorted with equal targets merged.  WL_ENOMEM if q_cap is too small (q_m is still set). */
+int wl_quotient(const wl_csr* g, const int32_t* colors, int64_t k, int64_t* q_row_ptr, int32_t* q_col, uint32_t* q_weights,
+                int64_t q_cap, int64_t* q_m, void* workspace, size_t workspace_bytes, void* cuda_stream);
+size_t wl_quotient_workspace_bytes(int64_t n, int64_t m);
+
+/* ------------------------------------------------------------------------------------------------------------------ */
+const char* wl_strerror(int code);
+int wl_last_cuda_error(void);      /* cudaError_t of the last WL_ECUDA on this thread */
+const char* wl_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* WL_REFINE_H_ */

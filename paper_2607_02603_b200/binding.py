@@ -1,0 +1,282 @@
+"""Thin ctypes binding over libwlrefine.so (argument marshalling only: every step runs in the CUDA kernels).
+
+Function names mirror include/wl_refine.h.  torch is used for device memory and streams only.  There is no CPU
+fallback: a missing library or a failing call raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from dataclasses import dataclass
+from typing import List, Optional
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libwlrefine.so")
+
+WL_OK, WL_EINVAL, WL_ERANGE, WL_ENOMEM, WL_ECUDA, WL_EMAXROUNDS = 0, -1, -2, -3, -4, -5
+WL_FLAG_NO_VALIDATE, WL_FLAG_NO_PRUNE, WL_FLAG_ROW_KERNEL, WL_FLAG_AGGRESSIVE_STOP, WL_FLAG_NO_CANONICAL = 1, 2, 4, 8, 16
+
+EXPORTS = [
+    "wl_refine_workspace_bytes", "wl_refine", "wl_refine_host", "wl_round_key", "wl_weight", "wl_spmv_round",
+    "wl_relabel", "wl_canonicalize", "wl_refine_batched", "wl_inner_labels", "wl_quotient",
+    "wl_quotient_workspace_bytes", "wl_strerror", "wl_last_cuda_error", "wl_version",
+]
+
+
+class WlError(RuntimeError):
+    def __init__(self, code: int, where: str):
+        self.code = code
+        msg = lib().wl_strerror(code).decode()
+        if code == WL_ECUDA:
+            msg += f" [cudaError {lib().wl_last_cuda_error()}]"
+        super().__init__(f"{where}: {msg} ({code})")
+
+
+class wl_csr(C.Structure):
+    _fields_ = [("n", C.c_int64), ("m", C.c_int64), ("row_ptr", C.c_void_p), ("col_idx", C.c_void_p),
+                ("weights", C.c_void_p)]
+
+
+class wl_options(C.Structure):
+    _fields_ = [("flags", C.c_uint32), ("max_rounds", C.c_int32), ("stream_id", C.c_uint64),
+                ("round_colors", C.c_void_p), ("round_colors_cap", C.c_int32), ("max_outer_iters", C.c_int32)]
+
+
+class wl_stats(C.Structure):
+    _fields_ = [("rounds", C.c_int32), ("outer_iters", C.c_int32), ("num_colors", C.c_int64),
+                ("last_num_batches", C.c_int64), ("boundary_nodes", C.c_int64), ("edges_streamed", C.c_int64),
+                ("bytes_h2d", C.c_int64), ("bytes_d2h", C.c_int64), ("ms_total", C.c_double), ("ms_spmv", C.c_double),
+                ("ms_relabel", C.c_double)]
+
+
+class wl_edge_batch(C.Structure):
+    _fields_ = [("edge_begin", C.c_int64), ("num_edges", C.c_int64), ("row_ptr", C.c_void_p), ("col_idx", C.c_void_p),
+                ("weights", C.c_void_p), ("src", C.c_void_p)]
+
+
+_lib = None
+
+
+def lib():
+    """Load the CUDA library; raises if it has not been built (python paper_2607_02603_b200/build.py)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_LIB_PATH):
+            raise RuntimeError(f"{_LIB_PATH} is missing: build it with `python -m paper_2607_02603_b200.build` "
+                               "(there is no CPU fallback)")
+        L = C.CDLL(_LIB_PATH)
+        vp, i64, i32, u64, u32, sz = C.c_void_p, C.c_int64, C.c_int32, C.c_uint64, C.c_uint32, C.c_size_t
+        L.wl_refine_workspace_bytes.restype = sz
+        L.wl_refine_workspace_bytes.argtypes = [i64, i64]
+        L.wl_refine.restype = C.c_int
+        L.wl_refine.argtypes = [C.POINTER(wl_csr), vp, u64, vp, C.POINTER(wl_stats), C.POINTER(wl_options), vp, sz, vp]
+        L.wl_refine_host.restype = C.c_int
+        L.wl_refine_host.argtypes = [C.POINTER(wl_csr), vp, u64, vp, C.POINTER(wl_stats), C.POINTER(wl_options), vp]
+        L.wl_round_key.restype = u64
+        L.wl_round_key.argtypes = [u64, u64, u64]
+        L.wl_weight.restype = u64
+        L.wl_weight.argtypes = [u64, u64]
+        L.wl_spmv_round.restype = C.c_int
+        L.wl_spmv_round.argtypes = [C.POINTER(wl_csr), vp, u64, vp, u32, vp, sz, vp]
+        L.wl_relabel.restype = C.c_int
+        L.wl_relabel.argtypes = [i64, vp, i64, vp, vp, C.POINTER(i64), vp, sz, vp]
+        L.wl_canonicalize.restype = C.c_int
+        L.wl_canonicalize.argtypes = [i64, vp, vp, C.POINTER(i64), vp, sz, vp]
+        L.wl_refine_batched.restype = C.c_int
+        L.wl_refine_batched.argtypes = [i64, i32, C.POINTER(wl_edge_batch), C.POINTER(wl_csr), u64, sz, i64, vp,
+                                        C.POINTER(wl_stats), C.POINTER(wl_options), vp]
+        L.wl_inner_labels.restype = C.c_int
+        L.wl_inner_labels.argtypes = [i64, vp, vp, vp, vp, vp]
+        L.wl_quotient.restype = C.c_int
+        L.wl_quotient.argtypes = [C.POINTER(wl_csr), vp, i64, vp, vp, vp, i64, C.POINTER(i64), vp, sz, vp]
+        L.wl_quotient_workspace_bytes.restype = sz
+        L.wl_quotient_workspace_bytes.argtypes = [i64, i64]
+        L.wl_strerror.restype = C.c_char_p
+        L.wl_strerror.argtypes = [C.c_int]
+        L.wl_last_cuda_error.restype = C.c_int
+        L.wl_version.restype = C.c_char_p
+        _lib = L
+    return _lib
+
+
+def _ptr(t: Optional[torch.Tensor]):
+    return None if t is None else C.c_void_p(t.data_ptr())
+
+
+def _stream_ptr(device):
+    return C.c_void_p(torch.cuda.current_stream(device).cuda_stream)
+
+
+def _check(t: Optional[torch.Tensor], dtype, device_type: str, name: str, numel: Optional[int] = None):
+    if t is None:
+        return
+    if t.dtype != dtype or t.device.type != device_type or not t.is_contiguous():
+        raise TypeError(f"{name}: expected contiguous {dtype} on {device_type}, got {t.dtype} on {t.device}")
+    if numel is not None and t.numel() != numel:
+        raise ValueError(f"{name}: expected {numel} elements, got {t.numel()}")
+
+
+def _as_u32_weights(weights: Optional[torch.Tensor]) -> Optional[torch.Tensor]:
+    """Edge weights travel as uint32; torch tensors hold them as int64 (values < 2^32) or int32 bit patterns."""
+    if weights is None:
+        return None
+    if weights.dtype == torch.int64:
+        return (weights & 0xFFFFFFFF).to(torch.uint32) if hasattr(torch, "uint32") else weights.to(torch.int32)
+    return weights
+
+
+@dataclass
+class RefineResult:
+    colors: torch.Tensor
+    num_colors: int
+    rounds: int
+    round_colors: List[int]
+    stats: dict
+    status: int
+
+
+def _stats_dict(s: wl_stats) -> dict:
+    return {f: getattr(s, f) for f, _ in wl_stats._fields_}
+
+
+def _make_csr(n, row_ptr, col_idx, weights, device_type):
+    _check(row_ptr, torch.int64, device_type, "row_ptr", n + 1)
+    _check(col_idx, torch.int32, device_type, "col_idx")
+    w = _as_u32_weights(weights)
+    if w is not None:
+        if w.device.type != device_type or not w.is_contiguous() or w.numel() != col_idx.numel() or w.element_size() != 4:
+            raise TypeError("weights: expected contiguous 4-byte integers, one per edge")
+    g = wl_csr(n, col_idx.numel(), row_ptr.data_ptr() if n >= 0 else None, col_idx.data_ptr(),
+               None if w is None else w.data_ptr())
+    return g, w
+
+
+def wl_refine_workspace_bytes(n: int, m: int) -> int:
+    return int(lib().wl_refine_workspace_bytes(n, m))
+
+
+def wl_refine(n: int, row_ptr: torch.Tensor, col_idx: torch.Tensor, weights: Optional[torch.Tensor] = None,
+              init_colors: Optional[torch.Tensor] = None, seed: int = 0, *, flags: int = 0, max_rounds: int = 0,
+              stream_id: int = 0, workspace: Optional[torch.Tensor] = None, out: Optional[torch.Tensor] = None,
+              round_cap: int = 4096, allow_max_rounds: bool = False) -> RefineResult:
+    """Algorithm 1 on device-resident CSR tensors.  Returns canonical colours (device int32[n])."""
+    L = lib()
+    dev = row_ptr.device
+    if dev.type != "cuda":
+        raise RuntimeError("wl_refine needs CUDA tensors (no CPU fallback); use wl_refine_host for host buffers")
+    g, w = _make_csr(n, row_ptr, col_idx, weights, "cuda")
+    _check(init_colors, torch.int32, "cuda", "init_colors", n)
+    if out is None:
+        out = torch.empty(n, dtype=torch.int32, device=dev)
+    _check(out, torch.int32, "cuda", "out", n)
+    need = wl_refine_workspace_bytes(n, col_idx.numel())
+    if workspace is None:
+        workspace = torch.empty(max(need, 256), dtype=torch.uint8, device=dev)
+    rc_buf = (C.c_int64 * round_cap)()
+    opt = wl_options(flags, max_rounds, stream_id, C.cast(rc_buf, C.c_void_p), round_cap, 0)
+    st = wl_stats()
+    with torch.cuda.device(dev):
+        rc = L.wl_refine(C.byref(g), _ptr(init_colors), seed, _ptr(out), C.byref(st), C.byref(opt), _ptr(workspace),
+                         workspace.numel(), _stream_ptr(dev))
+    if rc != WL_OK and not (allow_max_rounds and rc == WL_EMAXROUNDS):
+        raise WlError(rc, "wl_refine")
+    return RefineResult(out, st.num_colors, st.rounds, list(rc_buf[: min(st.rounds, round_cap)]), _stats_dict(st), rc)
+
+
+def wl_refine_host(n: int, row_ptr: torch.Tensor, col_idx: torch.Tensor, weights: Optional[torch.Tensor] = None,
+                   init_colors: Optional[torch.Tensor] = None, seed: int = 0, *, flags: int = 0, max_rounds: int = 0,
+                   out: Optional[torch.Tensor] = None, round_cap: int = 4096, device=None) -> RefineResult:
+    """Same computation from HOST tensors (pinned recommended): H2D, refine, D2H all inside the call."""
+    L = lib()
+    if not torch.cuda.is_available():
+        raise RuntimeError("wl_refine_host needs a CUDA device (no CPU fallback)")
+    dev = torch.device("cuda", torch.cuda.current_device()) if device is None else torch.device(device)
+    g, w = _make_csr(n, row_ptr, col_idx, weights, "cpu")
+    _check(init_colors, torch.int32, "cpu", "init_colors", n)
+    if out is None:
+        out = torch.empty(n, dtype=torch.int32, pin_memory=True)
+    _check(out, torch.int32, "cpu", "out", n)
+    rc_buf = (C.c_int64 * round_cap)()
+    opt = wl_options(flags, max_rounds, 0, C.cast(rc_buf, C.c_void_p), round_cap, 0)
+    st = wl_stats()
+    with torch.cuda.device(dev):
+        rc = L.wl_refine_host(C.byref(g), _ptr(init_colors), seed, _ptr(out), C.byref(st), C.byref(opt),
+                              _stream_ptr(dev))
+    if rc != WL_OK:
+        raise WlError(rc, "wl_refine_host")
+    return RefineResult(out, st.num_colors, st.rounds, list(rc_buf[: min(st.rounds, round_cap)]), _stats_dict(st), rc)
+
+
+def wl_round_key(seed: int, stream_id: int, rnd: int) -> int:
+    return int(lib().wl_round_key(seed, stream_id, rnd))
+
+
+def wl_weight(key: int, color: int) -> int:
+    return int(lib().wl_weight(key, color))
+
+
+def wl_spmv_round(n, row_ptr, col_idx, weights, colors, key: int, *, flags: int = 0, workspace=None) -> torch.Tensor:
+    """S1+S2: y = A w(colors) over Z/2^64.  Returns a device int64 tensor holding the u64 bit patterns."""
+    L = lib()
+    dev = row_ptr.device
+    g, w = _make_csr(n, row_ptr, col_idx, weights, "cuda")
+    _check(colors, torch.int32, "cuda", "colors", n)
+    y = torch.empty(n, dtype=torch.int64, device=dev)
+    need = wl_refine_workspace_bytes(n, col_idx.numel())
+    if workspace is None:
+        workspace = torch.empty(max(need, 256), dtype=torch.uint8, device=dev)
+    with torch.cuda.device(dev):
+        rc = L.wl_spmv_round(C.byref(g), _ptr(colors), key, _ptr(y), flags, _ptr(workspace), workspace.numel(),
+                             _stream_ptr(dev))
+    if rc != WL_OK:
+        raise WlError(rc, "wl_spmv_round")
+    return y
+
+
+def wl_relabel(colors: torch.Tensor, k: int, y: torch.Tensor, *, workspace=None):
+    """S3+S4: dense ids of the exact pairs (colors[i], y[i]).  -> (new_colors, k')."""
+    L = lib()
+    n = colors.numel()
+    dev = colors.device
+    _check(colors, torch.int32, "cuda", "colors")
+    _check(y, torch.int64, "cuda", "y", n)
+    out = torch.empty_like(colors)
+    need = wl_refine_workspace_bytes(n, 0)
+    if workspace is None:
+        workspace = torch.empty(max(need, 256), dtype=torch.uint8, device=dev)
+    kk = C.c_int64(0)
+    with torch.cuda.device(dev):
+        rc = L.wl_relabel(n, _ptr(colors), k, _ptr(y), _ptr(out), C.byref(kk), _ptr(workspace), workspace.numel(),
+                          _stream_ptr(dev))
+    if rc != WL_OK:
+        raise WlError(rc, "wl_relabel")
+    return out, kk.value
+
+
+def wl_canonicalize(colors: torch.Tensor, *, workspace=None):
+    """S6: first-occurrence renumbering.  -> (canonical colours, k)."""
+    L = lib()
+    n = colors.numel()
+    dev = colors.device
+    _check(colors, torch.int32, "cuda", "colors")
+    out = torch.empty_like(colors)
+    need = wl_refine_workspace_bytes(n, 0)
+    if workspace is None:
+        workspace = torch.empty(max(need, 256), dtype=torch.uint8, device=dev)
+    kk = C.c_int64(0)
+    with torch.cuda.device(dev):
+        rc = L.wl_canonicalize(n, _ptr(colors), _ptr(out), C.byref(kk), _ptr(workspace), workspace.numel(),
+                               _stream_ptr(dev))
+    if rc != WL_OK:
+        raise WlError(rc, "wl_canonicalize")
+    return out, kk.value
+
+
+def wl_strerror(code: int) -> str:
+    return lib().wl_strerror(code).decode()
+
+
+def wl_version() -> str:
+    return lib().wl_version().decode()

@@ -1,0 +1,391 @@
+// Kernels of the single-batch path.  sm_100a, integer-only.
+#pragma once
+#include "wl_device.cuh"
+
+namespace wl {
+
+constexpr int kSpmvThreads = 256;
+constexpr int kSpmvIpt = 7;  // odd: 64-bit shared-memory reads at stride IPT are bank-conflict free
+constexpr int kSpmvTile = kSpmvThreads * kSpmvIpt;
+constexpr u32 kNone = 0xffffffffu;
+constexpr u32 kWinBit = 0x80000000u;
+
+// error bits written by device-side validation
+constexpr u32 kErrRowPtr = 1u, kErrCol = 2u, kErrRowSum = 4u, kErrInit = 8u;
+
+// ---------------------------------------------------------------------------------------------------------------------
+// S0: validation of the CSR (WL_EINVAL / WL_ERANGE conditions of include/wl_refine.h)
+// ---------------------------------------------------------------------------------------------------------------------
+__global__ void validate_rows_kernel(int64_t n, int64_t m, const int64_t* __restrict__ row_ptr,
+                                     const u32* __restrict__ wt, u32* __restrict__ err) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  int64_t a = row_ptr[i], b = row_ptr[i + 1];
+  u32 e = 0;
+  if (i == 0 && a != 0) e |= kErrRowPtr;
+  if (i == n - 1 && b != m) e |= kErrRowPtr;
+  if (a > b || a < 0 || b > m) e |= kErrRowPtr;
+  if (!e) {
+    if (wt) {
+      u64 s = 0;
+      for (int64_t p = a; p < b; ++p) s += wt[p];
+      if (s > (1ull << 32)) e |= kErrRowSum;
+    } else if ((u64)(b - a) > (1ull << 32)) {
+      e |= kErrRowSum;
+    }
+  }
+  if (e) atomicOr(err, e);
+}
+
+__global__ void validate_cols_kernel(int64_t n, int64_t m, const int* __restrict__ col, u32* __restrict__ err) {
+  int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  bool bad = false;
+  for (int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; p < m; p += stride) {
+    int c = col[p];
+    bad |= (c < 0) | ((int64_t)c >= n);
+  }
+  if (bad) atomicOr(err, kErrCol);
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
+// S0: merge-path tile starts.  The path merges the n row ends (row_ptr[1..n]) with the m entry indices; tile t starts
+// at diagonal t*T.  tile_row[t] = number of row ends consumed before that diagonal.
+// ---------------------------------------------------------------------------------------------------------------------
+__global__ void tile_search_kernel(int64_t n, int64_t m, const int64_t* __restrict__ row_ptr, int64_t ntiles,
+                                   int* __restrict__ tile_row) {
+  int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t > ntiles) return;
+  int64_t d = t * (int64_t)kSpmvTile;
+  if (d > n + m) d = n + m;
+  int64_t lo = d > m ? d - m : 0, hi = d < n ? d : n;
+  while (lo < hi) {
+    int64_t mid = (lo + hi) >> 1;
+    if (row_ptr[mid + 1] <= d - 1 - mid)
+      lo = mid + 1;
+    else
+      hi = mid;
+  }
+  tile_row[t] = (int)lo;
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
+// S1+S2, edge-balanced: y_i = sum_j a_ij * w(colour_j)  (Alg. 1 line 5, L120), weights inline from the colour id.
+// One CTA owns kSpmvTile consecutive items of the merge path (row ends + entries), so work per CTA is equal whatever
+// the degree distribution.  Phase 1 streams the tile's column indices coalesced, gathers the colour of every target and
+// leaves a_ij*w in shared memory.  Phase 2 gives every thread IPT consecutive path items: it walks them sequentially and
+// flushes each row segment with one no-return 64-bit add at L2.  y must be zero before the launch.
+// ---------------------------------------------------------------------------------------------------------------------
+template <bool WEIGHTED>
+__global__ void __launch_bounds__(kSpmvThreads)
+spmv_merge_kernel(int64_t n, int64_t m, const int64_t* __restrict__ row_ptr, const int* __restrict__ col,
+                  const u32* __restrict__ wt, const int* __restrict__ colour, u64 key,
+                  const int* __restrict__ tile_row, u64* __restrict__ y) {
+  __shared__ u64 s_val[kSpmvTile];
+  __shared__ int s_rowend[kSpmvTile + 1];
+  const int tid = threadIdx.x;
+  const int64_t tile = blockIdx.x;
+  const int64_t d0 = tile * (int64_t)kSpmvTile;
+  const int64_t total = n + m;
+  const int64_t d1 = d0 + kSpmvTile < total ? d0 + kSpmvTile : total;
+  const int64_t i0 = tile_row[tile], i1 = tile_row[tile + 1];
+  const int64_t j0 = d0 - i0, j1 = d1 - i1;
+  const int nrows = (int)(i1 - i0);  // row ends inside the tile
+  const int nnz = (int)(j1 - j0);    // entries inside the tile
+
+  for (int r = tid; r <= nrows; r += kSpmvThreads) {
+    int64_t re = (i0 + r < n) ? row_ptr[i0 + r + 1] - j0 : (int64_t)kSpmvTile + 1;
+    s_rowend[r] = re > kSpmvTile + 1 ? kSpmvTile + 1 : (int)re;
+  }
+  {
+    int cidx[kSpmvIpt];
+    u32 a[kSpmvIpt];
+#pragma unroll
+    for (int k = 0; k < kSpmvIpt; ++k) {
+      int idx = tid + k * kSpmvThreads;
+      cidx[k] = idx < nnz ? ld_stream_i32(col + j0 + idx) : -1;
+      if (WEIGHTED) a[k] = idx < nnz ? ld_stream_u32(wt + j0 + idx) : 0u;
+    }
+    int cc[kSpmvIpt];
+#pragma unroll
+    for (int k = 0; k < kSpmvIpt; ++k) cc[k] = cidx[k] >= 0 ? __ldg(colour + cidx[k]) : 0;
+#pragma unroll
+    for (int k = 0; k < kSpmvIpt; ++k) {
+      int idx = tid + k * kSpmvThreads;
+      if (idx < nnz) {
+        u64 w = weight_of(key, (u64)(u32)cc[k]);
+        if (WEIGHTED) w *= (u64)a[k];
+        s_val[idx] = w;
+      }
+    }
+  }
+  __syncthreads();
+
+  const int items = (int)(d1 - d0);
+  int d = tid * kSpmvIpt;
+  if (d > items) d = items;
+  int dend = d + kSpmvIpt;
+  if (dend > items) dend = items;
+  int lo = d > nnz ? d - nnz : 0, hi = d < nrows ? d : nrows;
+  while (lo < hi) {
+    int mid = (lo + hi) >> 1;
+    if (s_rowend[mid] <= d - 1 - mid)
+      lo = mid + 1;
+    else
+      hi = mid;
+  }
+  int ri = lo, vj = d - lo;
+  int rend = s_rowend[ri];
+  u64 acc = 0;
+  for (int it = d; it < dend; ++it) {
+    if (rend <= vj) {  // row i0+ri ends here
+      if (acc) red_add_u64(y + i0 + ri, acc);
+      acc = 0;
+      ++ri;
+      rend = s_rowend[ri];
+    } else {
+      acc += s_val[vj];
+      ++vj;
+    }
+  }
+  if (acc) red_add_u64(y + i0 + ri, acc);
+}
+
+// S1+S2, simple variant: one warp per row (used for cross-checks and for pruned rounds over an active list).
+// rows == NULL: row index = warp index.  y is written with plain stores (no zeroing needed).
+template <bool WEIGHTED>
+__global__ void spmv_row_kernel(int64_t nrows, const int* __restrict__ rows, const int64_t* __restrict__ row_ptr,
+                                const int* __restrict__ col, const u32* __restrict__ wt,
+                                const int* __restrict__ colour, u64 key, u64* __restrict__ y) {
+  const int lane = threadIdx.x & 31;
+  int64_t w = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  if (w >= nrows) return;
+  const int64_t i = rows ? rows[w] : w;
+  const int64_t a = row_ptr[i], b = row_ptr[i + 1];
+  u64 acc = 0;
+  for (int64_t p = a + lane; p < b; p += 32) {
+    u64 v = weight_of(key, (u64)(u32)__ldg(colour + ld_stream_i32(col + p)));
+    if (WEIGHTED) v *= (u64)ld_stream_u32(wt + p);
+    acc += v;
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+  if (lane == 0) y[i] = acc;
+}
+
+// Round with a single colour and unit weights: y_i = outdeg(i) * w(0); no column read.
+__global__ void spmv_uniform_kernel(int64_t n, const int64_t* __restrict__ row_ptr, u64 w0, u64* __restrict__ y) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) y[i] = (u64)(row_ptr[i + 1] - row_ptr[i]) * w0;
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
+// S3+S4: relabel (colour_i, y_i) -> dense id (Alg. 1 line 6, L122; Q6: exact 96-bit pairs, never a hash of them).
+// A block keeps its id for the sub-block that agrees with its representative rep[c]; every other distinct pair
+// (c, y) claims a slot of an exact-key hash table with one 128-bit CAS and gets a fresh id k, k+1, ...  (block-
+// aggregated counter).  stamp[c] == round  <=>  block c has at least two nodes after this round (no atomics: plain
+// idempotent stores).  nodes == NULL: all nodes.
+// ---------------------------------------------------------------------------------------------------------------------
+constexpr int kRelabelThreads = 256;
+
+__global__ void __launch_bounds__(kRelabelThreads)
+relabel_insert_kernel(int64_t count, const int* __restrict__ nodes, const int* __restrict__ colour,
+                      const u64* __restrict__ y, int* __restrict__ rep, int* __restrict__ stamp, int round,
+                      Slot* __restrict__ table, u32 table_mask, u32* __restrict__ tmp, int k_old,
+                      u64* __restrict__ new_counter) {
+  int64_t t = (int64_t)blockIdx.x * kRelabelThreads + threadIdx.x;
+  bool win = false;
+  u32 slot = 0;
+  int i = -1;
+  if (t < count) {
+    i = nodes ? nodes[t] : (int)t;
+    const int c = colour[i];
+    const int r = rep[c];
+    const u64 yi = y[i];
+    const u64 yr = y[r];
+    if (yi == yr) {
+      if (i != r && stamp[c] != round) stamp[c] = round;
+      tmp[i] = kNone;
+    } else {
+      const Slot mine = {yi, (u64)(u32)c | ((u64)(u32)i << 32)};
+      const Slot empty = {kEmpty, kEmpty};
+      slot = (u32)slot_hash((u32)c, yi) & table_mask;
+      while (true) {
+        Slot v = load_slot(table + slot);
+        if (v.y == kEmpty || v.cx == kEmpty) {  // empty, or a torn view of a slot being claimed: decide with the CAS
+          v = cas128(table + slot, empty, mine);
+          if (v.y == kEmpty && v.cx == kEmpty) {
+            win = true;
+            break;
+          }
+        }
+        if (v.y == yi && (u32)v.cx == (u32)c) break;
+        slot = (slot + 1) & table_mask;
+      }
+      tmp[i] = slot | (win ? kWinBit : 0u);
+    }
+  }
+  int total;
+  const int rank = block_rank<kRelabelThreads>(win, &total);
+  __shared__ u64 s_base;
+  if (threadIdx.x == 0 && total > 0) s_base = atomicAdd(new_counter, (u64)total);
+  __syncthreads();
+  if (win) {
+    const int id = k_old + (int)s_base + rank;
+    // publish the id in the slot's x field (losers only ever compare y and the colour half)
+    reinterpret_cast<u32*>(table + slot)[3] = (u32)id;
+    rep[id] = i;
+  }
+}
+
+__global__ void relabel_resolve_kernel(int64_t count, const int* __restrict__ nodes, int* __restrict__ colour,
+                                       int* __restrict__ stamp, int round, const Slot* __restrict__ table,
+                                       const u32* __restrict__ tmp) {
+  int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= count) return;
+  const int i = nodes ? nodes[t] : (int)t;
+  const u32 s = tmp[i];
+  if (s == kNone) return;
+  const int id = (int)reinterpret_cast<const u32*>(table + (s & ~kWinBit))[3];
+  colour[i] = id;
+  if (!(s & kWinBit) && stamp[id] != round) stamp[id] = round;
+}
+
+__global__ void relabel_cleanup_kernel(int64_t count, const int* __restrict__ nodes, Slot* __restrict__ table,
+                                       const u32* __restrict__ tmp) {
+  int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= count) return;
+  const int i = nodes ? nodes[t] : (int)t;
+  const u32 s = tmp[i];
+  if (s == kNone) return;
+  store_slot(table + (s & ~kWinBit), kEmpty, kEmpty);
+}
+
+// rep[c] = some node of colour c (any one: benign race)
+__global__ void set_rep_kernel(int64_t n, const int* __restrict__ colour, int* __restrict__ rep) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) rep[colour[i]] = (int)i;
+}
+
+// densify helper: y_i = init label (must be non-negative), colour_i = 0
+__global__ void init_labels_kernel(int64_t n, const int* __restrict__ init, int* __restrict__ colour,
+                                   u64* __restrict__ y, u32* __restrict__ err) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  int v = init ? init[i] : 0;
+  if (v < 0) atomicOr(err, kErrInit);
+  colour[i] = 0;
+  y[i] = (u64)(u32)v;
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
+// S6: canonical first-occurrence ids.  first[c] = min node of colour c; blocks are ranked by their first node.
+// ---------------------------------------------------------------------------------------------------------------------
+constexpr int kScanThreads = 256;
+constexpr int kScanItems = 8;
+constexpr int kScanChunk = kScanThreads * kScanItems;
+
+__global__ void first_node_kernel(int64_t n, const int* __restrict__ colour, int* __restrict__ first) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const int c = colour[i];
+  if (first[c] > (int)i) atomicMin(first + c, (int)i);
+}
+
+__global__ void __launch_bounds__(kScanThreads)
+canon_count_kernel(int64_t n, const int* __restrict__ colour, const int* __restrict__ first, int* __restrict__ bsum) {
+  const int64_t base = (int64_t)blockIdx.x * kScanChunk;
+  int cnt = 0;
+#pragma unroll
+  for (int k = 0; k < kScanItems; ++k) {
+    int64_t i = base + threadIdx.x + k * kScanThreads;
+    if (i < n) cnt += (first[colour[i]] == (int)i);
+  }
+  __shared__ int s[kScanThreads / 32];
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) cnt += __shfl_xor_sync(0xffffffffu, cnt, o);
+  if ((threadIdx.x & 31) == 0) s[threadIdx.x >> 5] = cnt;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    int t = 0;
+    for (int w = 0; w < kScanThreads / 32; ++w) t += s[w];
+    bsum[blockIdx.x] = t;
+  }
+}
+
+// exclusive scan of nb block sums by one CTA; total -> out_total
+__global__ void __launch_bounds__(1024) scan_bsum_kernel(int64_t nb, int* __restrict__ bsum, u64* __restrict__ out_total) {
+  __shared__ int s_w[32];
+  __shared__ int s_carry;
+  if (threadIdx.x == 0) s_carry = 0;
+  __syncthreads();
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  for (int64_t base = 0; base < nb; base += 1024) {
+    int64_t i = base + threadIdx.x;
+    int v = i < nb ? bsum[i] : 0;
+    int x = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      int t = __shfl_up_sync(0xffffffffu, x, o);
+      if (lane >= o) x += t;
+    }
+    if (lane == 31) s_w[wid] = x;
+    __syncthreads();
+    if (wid == 0) {
+      int t = s_w[lane];
+      int xs = t;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        int u = __shfl_up_sync(0xffffffffu, xs, o);
+        if (lane >= o) xs += u;
+      }
+      s_w[lane] = xs - t;  // exclusive warp offsets
+    }
+    __syncthreads();
+    const int carry = s_carry;
+    if (i < nb) bsum[i] = carry + s_w[wid] + x - v;
+    __syncthreads();
+    if (threadIdx.x == 1023) s_carry = carry + s_w[wid] + x;
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) *out_total = (u64)s_carry;
+}
+
+// canon_of_first[i] = rank of the block whose first node is i
+__global__ void __launch_bounds__(kScanThreads)
+canon_rank_kernel(int64_t n, const int* __restrict__ colour, const int* __restrict__ first,
+                  const int* __restrict__ bsum, int* __restrict__ canon_of_first) {
+  // blocked arrangement so that ranks follow node order
+  const int64_t base = (int64_t)blockIdx.x * kScanChunk + (int64_t)threadIdx.x * kScanItems;
+  bool f[kScanItems];
+  int cnt = 0;
+#pragma unroll
+  for (int k = 0; k < kScanItems; ++k) {
+    int64_t i = base + k;
+    f[k] = i < n && first[colour[i]] == (int)i;
+    cnt += f[k];
+  }
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  int x = cnt;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    int t = __shfl_up_sync(0xffffffffu, x, o);
+    if (lane >= o) x += t;
+  }
+  __shared__ int s_w[kScanThreads / 32];
+  if (lane == 31) s_w[wid] = x;
+  __syncthreads();
+  int woff = 0;
+  for (int w = 0; w < wid; ++w) woff += s_w[w];
+  int r = bsum[blockIdx.x] + woff + x - cnt;
+#pragma unroll
+  for (int k = 0; k < kScanItems; ++k)
+    if (f[k]) canon_of_first[base + k] = r++;
+}
+
+__global__ void canon_apply_kernel(int64_t n, const int* __restrict__ colour, const int* __restrict__ first,
+                                   const int* __restrict__ canon_of_first, int* __restrict__ out) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) out[i] = canon_of_first[first[colour[i]]];
+}
+
+}  // namespace wl

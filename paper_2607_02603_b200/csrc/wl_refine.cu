@@ -1,0 +1,445 @@
+// Host side of the single-batch engine: workspace layout, the round loop of Algorithm 1 and the
+// step-level entry points declared in include/wl_refine.h.  Every step of the path runs in the kernels of wl_kernels.cuh.
+#include "wl_host.h"
+
+#include <algorithm>
+#include <cstdio>
+#include <cstring>
+#include <vector>
+
+#include "wl_kernels.cuh"
+
+namespace wl {
+
+thread_local int g_last_cuda_error = 0;
+
+static inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
+
+static inline u32 table_slots_for(int64_t n) {
+  // power of two >= 2n, at least 1024, at most 2^31 (slot indices share a word with the winner bit)
+  u64 s = 1024;
+  while (s < 2ull * (u64)n && s < (1ull << 31)) s <<= 1;
+  return (u32)(s - 1);  // returned as mask
+}
+
+Layout make_layout(int64_t n, int64_t m) {
+  Layout L{};
+  L.n = n;
+  L.m = m;
+  L.ntiles = (n + m + kSpmvTile - 1) / kSpmvTile;
+  L.table_mask = table_slots_for(n);
+  L.nscan = (n + kScanChunk - 1) / kScanChunk;
+  size_t off = 0;
+  auto take = [&](size_t bytes) {
+    size_t o = off;
+    off = align_up(off + bytes);
+    return o;
+  };
+  L.o_scal = take(sizeof(u64) * kNumScal);
+  L.o_colour = take(sizeof(int) * (size_t)n);
+  L.o_rep = take(sizeof(int) * (size_t)n);
+  L.o_stamp = take(sizeof(int) * (size_t)n);
+  L.o_tmp = take(sizeof(u32) * (size_t)n);
+  L.o_y = take(sizeof(u64) * (size_t)n);
+  L.o_tile_row = take(sizeof(int) * (size_t)(L.ntiles + 1));
+  L.o_bsum = take(sizeof(int) * (size_t)(L.nscan + 1));
+  L.o_table = take(sizeof(Slot) * ((size_t)L.table_mask + 1));
+  L.bytes = off;
+  return L;
+}
+
+static inline unsigned blocks_for(int64_t count, int threads) { return (unsigned)((count + threads - 1) / threads); }
+
+// ---- step launchers -----------------------------------------------------------------------------------------------
+void launch_tile_search(const Layout& L, const wl_csr& g, int* tile_row, cudaStream_t st) {
+  tile_search_kernel<<<blocks_for(L.ntiles + 1, 256), 256, 0, st>>>(g.n, g.m, g.row_ptr, L.ntiles, tile_row);
+}
+
+void launch_spmv(const Layout& L, const wl_csr& g, const int* colour, u64 key, const int* tile_row, u64* y,
+                 bool row_kernel, cudaStream_t st) {
+  if (g.n == 0) return;
+  if (row_kernel) {
+    unsigned grid = blocks_for(g.n * 32, 256);
+    if (g.weights)
+      spmv_row_kernel<true><<<grid, 256, 0, st>>>(g.n, nullptr, g.row_ptr, g.col_idx, g.weights, colour, key, y);
+    else
+      spmv_row_kernel<false><<<grid, 256, 0, st>>>(g.n, nullptr, g.row_ptr, g.col_idx, g.weights, colour, key, y);
+    return;
+  }
+  cudaMemsetAsync(y, 0, sizeof(u64) * (size_t)g.n, st);
+  if (g.weights)
+    spmv_merge_kernel<true><<<(unsigned)L.ntiles, kSpmvThreads, 0, st>>>(g.n, g.m, g.row_ptr, g.col_idx, g.weights,
+                                                                        colour, key, tile_row, y);
+  else
+    spmv_merge_kernel<false><<<(unsigned)L.ntiles, kSpmvThreads, 0, st>>>(g.n, g.m, g.row_ptr, g.col_idx, g.weights,
+                                                                         colour, key, tile_row, y);
+}
+
+// one relabel step over all nodes; counter (device u64) must be zero on entry and holds the number of new ids on exit
+void launch_relabel(const Layout& L, int64_t n, int* colour, const u64* y, int* rep, int* stamp, int round, Slot* table,
+                    u32* tmp, int k_old, u64* counter, cudaStream_t st) {
+  if (n == 0) return;
+  unsigned grid = blocks_for(n, kRelabelThreads);
+  relabel_insert_kernel<<<grid, kRelabelThreads, 0, st>>>(n, nullptr, colour, y, rep, stamp, round, table, L.table_mask,
+                                                          tmp, k_old, counter);
+  relabel_resolve_kernel<<<grid, kRelabelThreads, 0, st>>>(n, nullptr, colour, stamp, round, table, tmp);
+  relabel_cleanup_kernel<<<grid, kRelabelThreads, 0, st>>>(n, nullptr, table, tmp);
+}
+
+// canonical ids: uses `first` (int[n]) and `cof` (int[n]) as scratch, bsum int[nscan+1], total -> scal slot
+void launch_canonical(const Layout& L, int64_t n, const int* colour, int* out, int* first, int* cof, int* bsum,
+                      u64* total, cudaStream_t st) {
+  if (n == 0) return;
+  cudaMemsetAsync(first, 0x7f, sizeof(int) * (size_t)n, st);
+  first_node_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, colour, first);
+  canon_count_kernel<<<(unsigned)L.nscan, kScanThreads, 0, st>>>(n, colour, first, bsum);
+  scan_bsum_kernel<<<1, 1024, 0, st>>>(L.nscan, bsum, total);
+  canon_rank_kernel<<<(unsigned)L.nscan, kScanThreads, 0, st>>>(n, colour, first, bsum, cof);
+  canon_apply_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, colour, first, cof, out);
+}
+
+int check_cuda(cudaError_t e) {
+  if (e == cudaSuccess) return WL_OK;
+  g_last_cuda_error = (int)e;
+  return WL_ECUDA;
+}
+
+int basic_csr_check(const wl_csr* g) {
+  if (!g) return WL_EINVAL;
+  if (g->n < 0 || g->m < 0) return WL_EINVAL;
+  if (g->n > 0 && !g->row_ptr) return WL_EINVAL;
+  if (g->m > 0 && !g->col_idx) return WL_EINVAL;
+  if (g->n > kMaxNodes) return WL_ERANGE;
+  if (g->n == 0 && g->m != 0) return WL_EINVAL;
+  return WL_OK;
+}
+
+// pinned host mirror of the device scalars (one per host thread)
+static u64* host_scal() {
+  static thread_local u64* p = nullptr;
+  if (!p) {
+    if (cudaHostAlloc((void**)&p, sizeof(u64) * kNumScal, cudaHostAllocDefault) != cudaSuccess) p = nullptr;
+  }
+  return p;
+}
+
+struct EventPool {
+  std::vector<cudaEvent_t> ev;
+  ~EventPool() {
+    for (auto e : ev) cudaEventDestroy(e);
+  }
+  cudaEvent_t get(size_t i) {
+    while (ev.size() <= i) {
+      cudaEvent_t e;
+      cudaEventCreate(&e);
+      ev.push_back(e);
+    }
+    return ev[i];
+  }
+};
+
+}  // namespace wl
+
+using namespace wl;
+
+extern "C" {
+
+size_t wl_refine_workspace_bytes(int64_t n, int64_t m) {
+  if (n < 0 || m < 0 || n > kMaxNodes) return 0;
+  return make_layout(n, m).bytes;
+}
+
+uint64_t wl_round_key(uint64_t seed, uint64_t stream_id, uint64_t round) { return round_key(seed, stream_id, round); }
+uint64_t wl_weight(uint64_t key, uint64_t color) { return weight_of(key, color); }
+
+int wl_refine(const wl_csr* g, const int32_t* init_colors, uint64_t seed, int32_t* out_colors, wl_stats* stats,
+              const wl_options* opt, void* workspace, size_t workspace_bytes, void* cuda_stream) {
+  int rc = basic_csr_check(g);
+  if (rc) return rc;
+  const int64_t n = g->n, m = g->m;
+  if (stats) std::memset(stats, 0, sizeof(*stats));
+  if (n == 0) return WL_OK;
+  if (!out_colors || !workspace) return WL_EINVAL;
+  const Layout L = make_layout(n, m);
+  if (workspace_bytes < L.bytes) return WL_ENOMEM;
+  if ((uintptr_t)workspace % 256) return WL_EINVAL;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const uint32_t flags = opt ? opt->flags : 0u;
+  const int64_t max_rounds = (opt && opt->max_rounds > 0) ? opt->max_rounds : n + 1;
+  const uint64_t stream_id = opt ? opt->stream_id : 0;
+  u64* hs = host_scal();
+  if (!hs) return check_cuda(cudaGetLastError() == cudaSuccess ? cudaErrorMemoryAllocation : cudaGetLastError());
+
+  char* ws = (char*)workspace;
+  u64* scal = (u64*)(ws + L.o_scal);
+  int* colour = (int*)(ws + L.o_colour);
+  int* rep = (int*)(ws + L.o_rep);
+  int* stamp = (int*)(ws + L.o_stamp);
+  u32* tmp = (u32*)(ws + L.o_tmp);
+  u64* y = (u64*)(ws + L.o_y);
+  int* tile_row = (int*)(ws + L.o_tile_row);
+  int* bsum = (int*)(ws + L.o_bsum);
+  Slot* table = (Slot*)(ws + L.o_table);
+
+  EventPool evp;
+  cudaEvent_t ev_begin = evp.get(0), ev_end = evp.get(1);
+  cudaEventRecord(ev_begin, st);
+
+  // ---- S0: setup ---------------------------------------------------------------------------------------------------
+  cudaMemsetAsync(scal, 0, sizeof(u64) * kNumScal, st);
+  cudaMemsetAsync(table, 0xff, sizeof(Slot) * ((size_t)L.table_mask + 1), st);
+  cudaMemsetAsync(stamp, 0xff, sizeof(int) * (size_t)n, st);
+  u32* d_err = (u32*)(scal + kScalErr);
+  if (!(flags & WL_FLAG_NO_VALIDATE)) {
+    validate_rows_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, m, g->row_ptr, g->weights, d_err);
+    if (m > 0) validate_cols_kernel<<<148 * 8, 256, 0, st>>>(n, m, g->col_idx, d_err);
+    // the merge-path search below walks row_ptr: make sure it is well formed first
+    cudaMemcpyAsync(hs + kScalErr, scal + kScalErr, sizeof(u64), cudaMemcpyDeviceToHost, st);
+    rc = check_cuda(cudaStreamSynchronize(st));
+    if (rc) return rc;
+    const u32 e = (u32)hs[kScalErr];
+    if (e & (kErrRowPtr | kErrCol)) return WL_EINVAL;
+    if (e & kErrRowSum) return WL_ERANGE;
+  }
+  const bool row_kernel = (flags & WL_FLAG_ROW_KERNEL) != 0;
+  if (!row_kernel) launch_tile_search(L, *g, tile_row, st);
+
+  // initial partition: colour 0 everywhere; a given init is densified by one relabel step keyed on the label (L94)
+  int64_t k = 1;
+  init_labels_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, init_colors, colour, y, d_err);
+  // rep[0] = node 0; stamp[0] = 0 marks block 0 as non-singleton when n >= 2
+  cudaMemsetAsync(rep, 0, sizeof(int), st);
+  if (init_colors) {
+    launch_relabel(L, n, colour, y, rep, stamp, /*round=*/0, table, tmp, /*k_old=*/1, scal + kScalNew, st);
+    cudaMemcpyAsync(hs, scal, sizeof(u64) * kNumScal, cudaMemcpyDeviceToHost, st);
+    rc = check_cuda(cudaStreamSynchronize(st));
+    if (rc) return rc;
+    if ((u32)hs[kScalErr] & kErrInit) return WL_EINVAL;
+    k = 1 + (int64_t)hs[kScalNew];
+  }
+
+  // ---- S1-S5: rounds -------------------------------------------------------------------------------------------------
+  int64_t edges_streamed = 0;
+  double ms_spmv = 0, ms_relabel = 0;
+  int32_t rounds = 0;
+  bool converged = false;
+  const u64 w0_dummy = 0;
+  (void)w0_dummy;
+  for (int64_t r = 1; r <= max_rounds; ++r) {
+    const u64 key = round_key(seed, stream_id, (u64)r);
+    cudaEvent_t e0 = evp.get(2), e1 = evp.get(3), e2 = evp.get(4);
+    cudaEventRecord(e0, st);
+    if (k == 1 && !g->weights) {
+      spmv_uniform_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, g->row_ptr, weight_of(key, 0), y);
+    } else {
+      launch_spmv(L, *g, colour, key, tile_row, y, row_kernel, st);
+      edges_streamed += m;
+    }
+    cudaEventRecord(e1, st);
+    cudaMemsetAsync(scal + kScalNew, 0, sizeof(u64), st);
+    launch_relabel(L, n, colour, y, rep, stamp, (int)r, table, tmp, (int)k, scal + kScalNew, st);
+    cudaEventRecord(e2, st);
+    cudaMemcpyAsync(hs, scal, sizeof(u64) * kNumScal, cudaMemcpyDeviceToHost, st);
+    rc = check_cuda(cudaStreamSynchronize(st));
+    if (rc) return rc;
+    float a = 0, b = 0;
+    cudaEventElapsedTime(&a, e0, e1);
+    cudaEventElapsedTime(&b, e1, e2);
+    ms_spmv += a;
+    ms_relabel += b;
+    const int64_t k_new = k + (int64_t)hs[kScalNew];
+    rounds = (int32_t)r;
+    if (opt && opt->round_colors && r <= opt->round_colors_cap) opt->round_colors[r - 1] = k_new;
+    if (k_new == k) {  // the partition did not change (Q1, Q2): fixed point
+      converged = true;
+      break;
+    }
+    k = k_new;
+  }
+
+  // ---- S6: canonical ids ---------------------------------------------------------------------------------------------
+  if (flags & WL_FLAG_NO_CANONICAL) {
+    cudaMemcpyAsync(out_colors, colour, sizeof(int) * (size_t)n, cudaMemcpyDeviceToDevice, st);
+  } else {
+    // scratch: tmp -> first, rep -> canon_of_first (both dead now)
+    launch_canonical(L, n, colour, out_colors, (int*)tmp, rep, bsum, scal + kScalCanon, st);
+  }
+  cudaEventRecord(ev_end, st);
+  rc = check_cuda(cudaStreamSynchronize(st));
+  if (rc) return rc;
+  rc = check_cuda(cudaGetLastError());
+  if (rc) return rc;
+  if (stats) {
+    float t = 0;
+    cudaEventElapsedTime(&t, ev_begin, ev_end);
+    stats->rounds = rounds;
+    stats->num_colors = k;
+    stats->edges_streamed = edges_streamed;
+    stats->ms_total = t;
+    stats->ms_spmv = ms_spmv;
+    stats->ms_relabel = ms_relabel;
+  }
+  return converged ? WL_OK : WL_EMAXROUNDS;
+}
+
+int wl_refine_host(const wl_csr* g, const int32_t* init_colors, uint64_t seed, int32_t* out_colors, wl_stats* stats,
+                   const wl_options* opt, void* cuda_stream) {
+  int rc = basic_csr_check(g);
+  if (rc) return rc;
+  if (stats) std::memset(stats, 0, sizeof(*stats));
+  const int64_t n = g->n, m = g->m;
+  if (n == 0) return WL_OK;
+  if (!out_colors) return WL_EINVAL;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const size_t wsb = wl_refine_workspace_bytes(n, m);
+  char* d_all = nullptr;
+  size_t o_rp = 0, o_col, o_wt, o_init, o_out, o_ws, off = 0;
+  auto take = [&](size_t b) {
+    size_t o = off;
+    off = align_up(off + b);
+    return o;
+  };
+  o_rp = take(sizeof(int64_t) * (size_t)(n + 1));
+  o_col = take(sizeof(int) * (size_t)m);
+  o_wt = take(g->weights ? sizeof(u32) * (size_t)m : 0);
+  o_init = take(init_colors ? sizeof(int) * (size_t)n : 0);
+  o_out = take(sizeof(int) * (size_t)n);
+  o_ws = take(wsb);
+  if (cudaMalloc((void**)&d_all, off) != cudaSuccess) {
+    cudaGetLastError();
+    return WL_ENOMEM;
+  }
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0);
+  cudaEventCreate(&e1);
+  cudaEventRecord(e0, st);
+  int64_t h2d = 0;
+  cudaMemcpyAsync(d_all + o_rp, g->row_ptr, sizeof(int64_t) * (size_t)(n + 1), cudaMemcpyHostToDevice, st);
+  h2d += sizeof(int64_t) * (n + 1);
+  if (m) cudaMemcpyAsync(d_all + o_col, g->col_idx, sizeof(int) * (size_t)m, cudaMemcpyHostToDevice, st);
+  h2d += sizeof(int) * m;
+  if (g->weights && m) {
+    cudaMemcpyAsync(d_all + o_wt, g->weights, sizeof(u32) * (size_t)m, cudaMemcpyHostToDevice, st);
+    h2d += sizeof(u32) * m;
+  }
+  if (init_colors) {
+    cudaMemcpyAsync(d_all + o_init, init_colors, sizeof(int) * (size_t)n, cudaMemcpyHostToDevice, st);
+    h2d += sizeof(int) * n;
+  }
+  wl_csr dg = {n, m, (const int64_t*)(d_all + o_rp), (const int*)(d_all + o_col),
+               g->weights ? (const u32*)(d_all + o_wt) : nullptr};
+  wl_stats inner;
+  rc = wl_refine(&dg, init_colors ? (const int*)(d_all + o_init) : nullptr, seed, (int*)(d_all + o_out), &inner, opt,
+                 d_all + o_ws, wsb, cuda_stream);
+  if (rc == WL_OK || rc == WL_EMAXROUNDS) {
+    cudaMemcpyAsync(out_colors, d_all + o_out, sizeof(int) * (size_t)n, cudaMemcpyDeviceToHost, st);
+    cudaEventRecord(e1, st);
+    int rc2 = check_cuda(cudaStreamSynchronize(st));
+    if (rc2) rc = rc2;
+    if (stats) {
+      *stats = inner;
+      float t = 0;
+      cudaEventElapsedTime(&t, e0, e1);
+      stats->ms_total = t;
+      stats->bytes_h2d = h2d;
+      stats->bytes_d2h = sizeof(int) * n;
+    }
+  }
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  cudaFree(d_all);
+  return rc;
+}
+
+int wl_spmv_round(const wl_csr* g, const int32_t* colors, uint64_t key, uint64_t* y, uint32_t flags, void* workspace,
+                  size_t workspace_bytes, void* cuda_stream) {
+  int rc = basic_csr_check(g);
+  if (rc) return rc;
+  if (g->n == 0) return WL_OK;
+  if (!colors || !y || !workspace) return WL_EINVAL;
+  const Layout L = make_layout(g->n, g->m);
+  if (workspace_bytes < L.bytes) return WL_ENOMEM;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  int* tile_row = (int*)((char*)workspace + L.o_tile_row);
+  const bool row_kernel = (flags & WL_FLAG_ROW_KERNEL) != 0;
+  if (!row_kernel) launch_tile_search(L, *g, tile_row, st);
+  launch_spmv(L, *g, colors, key, tile_row, (u64*)y, row_kernel, st);
+  rc = check_cuda(cudaStreamSynchronize(st));
+  if (rc) return rc;
+  return check_cuda(cudaGetLastError());
+}
+
+int wl_relabel(int64_t n, const int32_t* colors, int64_t k, const uint64_t* y, int32_t* new_colors, int64_t* num_colors,
+               void* workspace, size_t workspace_bytes, void* cuda_stream) {
+  if (n < 0 || k < 0 || k > n) return WL_EINVAL;
+  if (n > kMaxNodes) return WL_ERANGE;
+  if (n == 0) {
+    if (num_colors) *num_colors = 0;
+    return WL_OK;
+  }
+  if (!colors || !y || !new_colors || !workspace) return WL_EINVAL;
+  const Layout L = make_layout(n, 0);
+  if (workspace_bytes < L.bytes) return WL_ENOMEM;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  char* ws = (char*)workspace;
+  u64* scal = (u64*)(ws + L.o_scal);
+  int* rep = (int*)(ws + L.o_rep);
+  int* stamp = (int*)(ws + L.o_stamp);
+  u32* tmp = (u32*)(ws + L.o_tmp);
+  Slot* table = (Slot*)(ws + L.o_table);
+  u64* hs = host_scal();
+  if (!hs) return WL_ECUDA;
+  cudaMemsetAsync(scal, 0, sizeof(u64) * kNumScal, st);
+  cudaMemsetAsync(table, 0xff, sizeof(Slot) * ((size_t)L.table_mask + 1), st);
+  cudaMemsetAsync(stamp, 0xff, sizeof(int) * (size_t)n, st);
+  if (new_colors != colors)
+    cudaMemcpyAsync(new_colors, colors, sizeof(int) * (size_t)n, cudaMemcpyDeviceToDevice, st);
+  set_rep_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, new_colors, rep);
+  launch_relabel(L, n, new_colors, (const u64*)y, rep, stamp, 1, table, tmp, (int)k, scal + kScalNew, st);
+  cudaMemcpyAsync(hs, scal, sizeof(u64) * kNumScal, cudaMemcpyDeviceToHost, st);
+  int rc = check_cuda(cudaStreamSynchronize(st));
+  if (rc) return rc;
+  if (num_colors) *num_colors = k + (int64_t)hs[kScalNew];
+  return check_cuda(cudaGetLastError());
+}
+
+int wl_canonicalize(int64_t n, const int32_t* colors, int32_t* out, int64_t* num_colors, void* workspace,
+                    size_t workspace_bytes, void* cuda_stream) {
+  if (n < 0) return WL_EINVAL;
+  if (n > kMaxNodes) return WL_ERANGE;
+  if (n == 0) {
+    if (num_colors) *num_colors = 0;
+    return WL_OK;
+  }
+  if (!colors || !out || !workspace) return WL_EINVAL;
+  const Layout L = make_layout(n, 0);
+  if (workspace_bytes < L.bytes) return WL_ENOMEM;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  char* ws = (char*)workspace;
+  u64* scal = (u64*)(ws + L.o_scal);
+  u64* hs = host_scal();
+  if (!hs) return WL_ECUDA;
+  launch_canonical(L, n, colors, out, (int*)(ws + L.o_tmp), (int*)(ws + L.o_rep), (int*)(ws + L.o_bsum),
+                   scal + kScalCanon, st);
+  cudaMemcpyAsync(hs + kScalCanon, scal + kScalCanon, sizeof(u64), cudaMemcpyDeviceToHost, st);
+  int rc = check_cuda(cudaStreamSynchronize(st));
+  if (rc) return rc;
+  if (num_colors) *num_colors = (int64_t)hs[kScalCanon];
+  return check_cuda(cudaGetLastError());
+}
+
+const char* wl_strerror(int code) {
+  switch (code) {
+    case WL_OK: return "ok";
+    case WL_EINVAL: return "invalid argument (null pointer, negative size, malformed CSR or negative label)";
+    case WL_ERANGE: return "out of range (too many nodes for int32 ids, or a row sum above 2^32)";
+    case WL_ENOMEM: return "workspace or device memory cap too small";
+    case WL_ECUDA: return "CUDA error (see wl_last_cuda_error)";
+    case WL_EMAXROUNDS: return "round / outer-iteration limit reached before the fixed point";
+    default: return "unknown wl_status";
+  }
+}
+int wl_last_cuda_error(void) { return g_last_cuda_error; }
+const char* wl_version(void) { return "wl_refine 0.1 (sm_100a)"; }
+
+}  // extern "C"

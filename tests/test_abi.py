@@ -1,0 +1,58 @@
+"""CPU-side checks of the boundary: the C-ABI library builds, loads and exports every symbol include/wl_refine.h
+declares; host-only pure functions agree with the oracle's independent restatement.  No compute calls (no GPU here)."""
+import os
+import re
+
+import pytest
+
+
+def test_library_exports_every_declared_symbol(repo_root):
+    import paper_2607_02603_b200 as wl
+    from paper_2607_02603_b200.build import build
+    build()
+    header = open(os.path.join(repo_root, "include", "wl_refine.h")).read()
+    header = re.sub(r"/\*.*?\*/", "", header, flags=re.S)
+    declared = set(re.findall(r"\b(wl_[a-z_0-9]+)\s*\(", header))
+    assert declared, "no prototypes found"
+    L = wl.lib()
+    for name in declared:
+        assert hasattr(L, name), f"{name} declared in wl_refine.h but not exported"
+    assert declared == set(wl.EXPORTS)
+
+
+def test_host_weight_function_matches_oracle_restatement():
+    import oracle
+    import paper_2607_02603_b200 as wl
+    for s, st, r, c in [(0, 0, 1, 0), (5, 1, 7, 123456), (2 ** 64 - 1, 9, 3, 2 ** 32 + 5), (42, 1 << 40, 1000, 7)]:
+        k = wl.wl_round_key(s, st, r)
+        assert k == oracle.round_key(s, st, r)
+        assert wl.wl_weight(k, c) == oracle.weight(k, c)
+
+
+def test_workspace_size_is_monotone_and_rejects_bad_sizes():
+    import paper_2607_02603_b200 as wl
+    assert wl.wl_refine_workspace_bytes(-1, 0) == 0
+    assert wl.wl_refine_workspace_bytes(1 << 40, 0) == 0
+    a = wl.wl_refine_workspace_bytes(1000, 5000)
+    b = wl.wl_refine_workspace_bytes(2000, 5000)
+    c = wl.wl_refine_workspace_bytes(2000, 50000)
+    assert 0 < a <= b <= c
+
+
+def test_no_cpu_fallback_without_cuda():
+    import torch
+    import paper_2607_02603_b200 as wl
+    if torch.cuda.is_available():
+        pytest.skip("CUDA present")
+    import graphgen as gg
+    g = gg.erdos_renyi(50, 100, seed=1)
+    with pytest.raises(RuntimeError):
+        wl.wl_refine(g.n, g.row_ptr, g.col)
+    with pytest.raises(RuntimeError):
+        wl.wl_refine_host(g.n, g.row_ptr, g.col)
+
+
+def test_strerror():
+    import paper_2607_02603_b200 as wl
+    assert wl.wl_strerror(0) == "ok"
+    assert "workspace" in wl.wl_strerror(wl.WL_ENOMEM)

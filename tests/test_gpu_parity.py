@@ -1,0 +1,199 @@
+"""GPU parity tests: the CUDA path (through the C ABI, via the thin binding) against the CPU oracle on the same
+seeded inputs.  Integer / index work: bit exact (partitions compared after canonical first-occurrence relabelling)."""
+import numpy as np
+import pytest
+import torch
+
+import graphgen as gg
+import oracle
+
+pytestmark = pytest.mark.gpu
+
+wl = pytest.importorskip("paper_2607_02603_b200")
+
+
+def dev():
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    return torch.device("cuda", 0)
+
+
+def dgraph(g):
+    d = g.to(dev())
+    return d.n, d.row_ptr, d.col, d.weights
+
+
+def u64(t):
+    return t.cpu().numpy().view(np.uint64)
+
+
+def oracle_w(key, colors):
+    return np.array([oracle.weight(key, int(c)) for c in colors], dtype=np.uint64)
+
+
+GRAPHS = {
+    "er_c1": lambda: gg.erdos_renyi(),
+    "er_small": lambda: gg.erdos_renyi(300, 900, seed=3),
+    "grid_33": lambda: gg.grid2d(33),
+    "grid_64": lambda: gg.grid2d(64),
+    "rmat12_sym": lambda: gg.rmat(12, seed=1),
+    "rmat13_dir": lambda: gg.rmat(13, seed=2, symmetrize=False),
+    "path_101": lambda: gg.path_graph(101),
+    "dpath_40": lambda: gg.directed_path(40),
+    "star_1000": lambda: gg.star_graph(1000),
+    "hub_20000": lambda: gg.from_edge_list(20001, [(0, j) for j in range(1, 20001)] + [(5, 7), (9, 7)]),
+    "k_5_7": lambda: gg.complete_bipartite(5, 7),
+    "circ": lambda: gg.circulant(50, (1, 4, 9)),
+    "empty_edges": lambda: gg.from_edge_list(17, []),
+    "one_node": lambda: gg.from_edge_list(1, []),
+    "self_loops": lambda: gg.from_edge_list(4, [(0, 0), (1, 1), (2, 3)]),
+    "weighted": lambda: gg.random_weighted_digraph(500, 3000, 5, max_w=4),
+    "weighted_big_w": lambda: gg.random_weighted_digraph(200, 2000, 6, max_w=1 << 20),
+}
+
+
+# ------------------------------------------------------------------ S1+S2
+@pytest.mark.parametrize("name", list(GRAPHS))
+@pytest.mark.parametrize("flags", [0, 4])
+def test_spmv_bit_exact(name, flags):
+    g = GRAPHS[name]()
+    n, rp, ci, wt = g.numpy()
+    colors = gg.random_partition(n, max(1, n // 3), 11).numpy()
+    key = wl.wl_round_key(123, 0, 2)
+    assert key == oracle.round_key(123, 0, 2)
+    want = oracle.spmv_u64(n, rp, ci, wt, oracle_w(key, colors))
+    dn, drp, dci, dwt = dgraph(g)
+    y = wl.wl_spmv_round(dn, drp, dci, dwt, torch.from_numpy(colors).to(dev()), key, flags=flags)
+    assert (u64(y) == want).all()
+
+
+def test_spmv_uniform_gives_degrees_times_w0():
+    g = gg.rmat(12, seed=4)
+    n, rp, ci, wt = g.numpy()
+    key = wl.wl_round_key(9, 0, 1)
+    dn, drp, dci, dwt = dgraph(g)
+    y = wl.wl_spmv_round(dn, drp, dci, dwt, torch.zeros(n, dtype=torch.int32, device=dev()), key)
+    assert (u64(y) == np.diff(rp).astype(np.uint64) * np.uint64(oracle.weight(key, 0))).all()
+
+
+# ------------------------------------------------------------------ S3+S4
+def _same_partition(a, b):
+    return oracle.canonical(a).tolist() == oracle.canonical(b).tolist()
+
+
+@pytest.mark.parametrize("case", ["all_equal", "all_distinct", "equal_y_across_colours", "same_colour_distinct_y", "random"])
+def test_relabel_matches_cpu_sort(case):
+    n = 5000
+    rng = np.random.default_rng(3)
+    if case == "all_equal":
+        c, y = np.zeros(n, np.int32), np.full(n, 77, np.uint64)
+    elif case == "all_distinct":
+        c, y = np.zeros(n, np.int32), rng.permutation(n).astype(np.uint64)
+    elif case == "equal_y_across_colours":
+        c, y = (np.arange(n) % 7).astype(np.int32), np.full(n, 5, np.uint64)
+    elif case == "same_colour_distinct_y":
+        c, y = (np.arange(n) % 3).astype(np.int32), (np.arange(n) % 11).astype(np.uint64) << np.uint64(40)
+    else:
+        c, y = rng.integers(0, 50, n).astype(np.int32), rng.integers(0, 4, n).astype(np.uint64) * np.uint64(0x9E3779B97F4A7C15)
+    c = oracle.canonical(c)
+    k = int(c.max()) + 1
+    new, k2 = wl.wl_relabel(torch.from_numpy(c).to(dev()), k, torch.from_numpy(y.view(np.int64)).to(dev()))
+    new = new.cpu().numpy()
+    # CPU: dense ids of lexicographically sorted exact pairs
+    pairs = np.stack([c.astype(np.uint64), y], 1)
+    _, inv = np.unique(pairs, axis=0, return_inverse=True)
+    assert k2 == inv.max() + 1
+    assert sorted(np.unique(new).tolist()) == list(range(k2))  # dense
+    assert _same_partition(new, inv)
+    # refinement of the old partition (L153)
+    assert len({(a, b) for a, b in zip(new.tolist(), c.tolist())}) == k2
+
+
+# ------------------------------------------------------------------ S6
+@pytest.mark.parametrize("n", [1, 2, 31, 2048, 2049, 100_003])
+def test_canonicalize(n):
+    rng = np.random.default_rng(n)
+    c = rng.integers(0, max(1, n // 2), n).astype(np.int32)
+    out, k = wl.wl_canonicalize(torch.from_numpy(c).to(dev()))
+    assert out.cpu().numpy().tolist() == oracle.canonical(c).tolist()
+    assert k == np.unique(c).size
+
+
+# ------------------------------------------------------------------ whole Algorithm 1
+@pytest.mark.parametrize("name", list(GRAPHS))
+@pytest.mark.parametrize("flags", [0, 4])
+def test_refine_equals_oracle(name, flags):
+    g = GRAPHS[name]()
+    n, rp, ci, wt = g.numpy()
+    want, counts, rounds = oracle.refine(n, rp, ci, wt)
+    dn, drp, dci, dwt = dgraph(g)
+    for seed in (0, 1, 2):
+        res = wl.wl_refine(dn, drp, dci, dwt, seed=seed, flags=flags)
+        assert res.round_colors == counts and res.rounds == rounds  # same trajectory
+        assert res.num_colors == counts[-1]
+        assert res.colors.cpu().numpy().tolist() == want.tolist()
+
+
+@pytest.mark.parametrize("seed", range(20))
+def test_refine_many_seeds_rmat(seed):
+    g = gg.rmat(10, edge_factor=8, seed=seed, symmetrize=bool(seed % 2))
+    n, rp, ci, wt = g.numpy()
+    init = None if seed % 3 == 0 else gg.random_partition(n, 1 + seed, seed)
+    want, counts, rounds = oracle.refine(n, rp, ci, wt, None if init is None else init.numpy())
+    dn, drp, dci, dwt = dgraph(g)
+    res = wl.wl_refine(dn, drp, dci, dwt, None if init is None else (init * 3 + 5).to(dev()), seed=seed * 977)
+    assert res.round_colors == counts
+    assert res.colors.cpu().numpy().tolist() == want.tolist()
+
+
+def test_refine_weighted_equals_multigraph():
+    g1 = gg.from_edge_list(4, [(0, 1), (0, 1), (2, 1), (3, 3)])
+    g2 = gg.from_edge_list(4, [(0, 1), (2, 1), (3, 3)], weights=[2, 1, 1])
+    r1 = wl.wl_refine(*dgraph(g1), seed=1)
+    r2 = wl.wl_refine(*dgraph(g2), seed=1)
+    assert r1.colors.tolist() == r2.colors.tolist() == oracle.refine(*g1.numpy())[0].tolist()
+
+
+def test_grid_256_closed_form():
+    s = 256
+    g = gg.grid2d(s)
+    res = wl.wl_refine(*dgraph(g), seed=5)
+    h = s // 2
+    assert res.rounds == h and res.num_colors == h * (h + 1) // 2
+    assert torch.equal(res.colors.cpu(), gg.grid2d_orbit_colors(s))
+
+
+def test_refine_host_entry_point():
+    g = gg.erdos_renyi(2000, 9000, seed=7)
+    n, rp, ci, wt = g.numpy()
+    want, counts, _ = oracle.refine(n, rp, ci)
+    res = wl.wl_refine_host(n, g.row_ptr.pin_memory(), g.col.pin_memory(), seed=3)
+    assert res.colors.numpy().tolist() == want.tolist() and res.round_colors == counts
+    assert res.stats["bytes_h2d"] == 8 * (n + 1) + 4 * g.m and res.stats["bytes_d2h"] == 4 * n
+
+
+# ------------------------------------------------------------------ error behaviour
+def test_error_codes():
+    g = gg.erdos_renyi(100, 300, seed=1)
+    n, rp, ci, wt = dgraph(g)
+    bad = ci.clone()
+    bad[5] = n
+    with pytest.raises(wl.WlError) as e:
+        wl.wl_refine(n, rp, bad)
+    assert e.value.code == wl.WL_EINVAL
+    bad_rp = rp.clone()
+    bad_rp[3] = bad_rp[4] + 1
+    with pytest.raises(wl.WlError) as e:
+        wl.wl_refine(n, bad_rp, ci)
+    assert e.value.code == wl.WL_EINVAL
+    with pytest.raises(wl.WlError) as e:
+        wl.wl_refine(n, rp, ci, workspace=torch.empty(1024, dtype=torch.uint8, device=dev()))
+    assert e.value.code == wl.WL_ENOMEM
+    with pytest.raises(wl.WlError) as e:
+        wl.wl_refine(n, rp, ci, init_colors=torch.full((n,), -3, dtype=torch.int32, device=dev()))
+    assert e.value.code == wl.WL_EINVAL
+    res = wl.wl_refine(n, rp, ci, max_rounds=1, allow_max_rounds=True)
+    assert res.status == wl.WL_EMAXROUNDS
+    big = gg.from_edge_list(2, [(0, 1), (0, 1)], weights=[(1 << 32) - 1, 5])
+    with pytest.raises(wl.WlError) as e:
+        wl.wl_refine(*dgraph(big))
+    assert e.value.code == wl.WL_ERANGE
