@@ -1,0 +1,292 @@
+#!/usr/bin/env python
+"""Benchmark of the hot path: one "step" = one complete randomized 1-WL refinement (all S0-S6 rows of SURVEY.md §8(a),
+Algorithm 1 of PAPER.md L106-L127, run to its fixed point) of the headline synthetic graph, BASELINE.json configs[3]:
+R-MAT scale 27, edge factor 16, (a,b,c,d) = (.57,.19,.19,.05), seed 2, symmetrised, deduplicated, CSR resident in HBM.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--scale S] [--impl reference]
+
+Prints ONE JSON line (see the task contract).  `value` = column indices consumed per second over the whole call
+(GEdges/s); `e2e` = the same through wl_refine_host (pinned host CSR -> device, colours -> host inside the timed region);
+`roofline` = the SpMV kernel (dominant) against the measured HBM copy bandwidth; `cpu_baseline` = the CPU oracle on a
+bounded sample.  With N > 1 (torchrun) every rank refines its own replica of the graph: the path does not shard
+without a collective per round, so scaling is weak / replicas only.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+RMAT_SEEDS = {22: 1, 27: 2, 30: 3}  # BASELINE.json configs[2..4]
+ORACLE_SAMPLE_SCALE = 21           # bounded sample of the same recipe for the CPU oracle (about 10-30 s)
+HBM_FALLBACK_GBS = 6650.0          # /opt/skills/guides/B200_PROFILING.md fallback
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return json.load(open(p)), "measured"
+        except Exception:
+            pass
+    return {"hbm_gbs": HBM_FALLBACK_GBS}, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for l in self.lines:
+            f = [x.strip() for x in l.split(",")]
+            if len(f) < 8:
+                continue
+            try:
+                sm.append(float(f[0]))
+                mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for name, v in zip(names, f[4:8]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def oracle_sample(scale: int):
+    """The CPU oracle, as it stands, on a bounded sample of the workload: the same R-MAT recipe at a smaller scale."""
+    import graphgen as gg
+    import oracle
+    try:
+        import torch
+        gen_dev = "cuda" if torch.cuda.is_available() else "cpu"
+    except Exception:
+        gen_dev = "cpu"
+    g = gg.rmat(scale, seed=RMAT_SEEDS[27], device=gen_dev)  # input generation only; the oracle runs on the host cores
+    n, rp, ci, wt = g.numpy()
+    t0 = time.perf_counter()
+    _, counts, rounds = oracle.refine(n, rp, ci, wt)
+    dt = time.perf_counter() - t0
+    cores = int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1))
+    return {"value": g.m * rounds / dt / 1e9, "unit": "GEdges/s", "cores": cores, "kind": "oracle",
+            "sample": f"R-MAT scale {scale} (n={n}, m={g.m}), same recipe and seed as the workload, {rounds} rounds of "
+                      f"signature-sort refinement in {dt:.2f} s (signatures built with OpenMP, sort on one core)",
+            "seconds": dt, "rounds": rounds, "m": g.m}
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores, on this arm's metric / unit / config."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    times, last = [], None
+    for i in range(args.warmup + args.steps):
+        last = oracle_sample(args.oracle_scale)
+        if i >= args.warmup:
+            times.append(last["seconds"])
+    ms = 1e3 * sum(times) / len(times)
+    value = last["m"] * last["rounds"] / (ms / 1e3) / 1e9
+    cb = {k: last[k] for k in ("unit", "cores", "kind", "sample")}
+    cb["value"] = value
+    line = {"impl": "reference", "metric": "refine_gedges_per_s", "value": value, "unit": "GEdges/s",
+            "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u64", "data": "synthetic",
+            "config": workload_config(args.scale, None, None), "cpu_baseline": cb,
+            "e2e": {"value": value, "unit": "GEdges/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+def workload_config(scale, n, m):
+    return {"workload": f"R-MAT scale {scale}, edge factor 16, (a,b,c,d)=(0.57,0.19,0.19,0.05), seed "
+                        f"{RMAT_SEEDS.get(scale, 2)}, symmetrised, deduplicated, uniform initial colour "
+                        f"(BASELINE.json configs[{ {22: 2, 27: 3}.get(scale, 3)}])",
+            "n": n, "m": m, "step": "wl_refine to the fixed point (all rounds, S0-S6)",
+            "l2": "inputs (CSR >= 0.5 GB, 17 GB at scale 27) exceed the 126 MB L2; no flush needed between steps"}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--scale", type=int, default=27)
+    ap.add_argument("--impl", default="ours")
+    ap.add_argument("--oracle-scale", type=int, default=ORACLE_SAMPLE_SCALE)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--flags", type=int, default=0, help="WL_FLAG_* bits passed to wl_refine")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 0)
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import graphgen as gg
+    import paper_2607_02603_b200 as wl
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    dev = torch.device("cuda", local_rank)
+    torch.cuda.set_device(dev)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    # ---- synthetic input, generated on the device (not timed) --------------------------------------------------------
+    seed = RMAT_SEEDS.get(args.scale, 2)
+    g = gg.rmat(args.scale, seed=seed, device=dev, chunk=1 << 28)
+    torch.cuda.empty_cache()
+    n, m = g.n, g.m
+    ws = torch.empty(wl.wl_refine_workspace_bytes(n, m), dtype=torch.uint8, device=dev)
+    out = torch.empty(n, dtype=torch.int32, device=dev)
+
+    def step(i):
+        return wl.wl_refine(n, g.row_ptr, g.col, None, seed=1000 + i, flags=args.flags, workspace=ws, out=out)
+
+    for i in range(max(args.warmup, 3)):
+        res = step(i)
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    barrier()
+    launches0 = wl.wl_kernel_launches()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record()
+    results = []
+    for i in range(args.steps):
+        results.append(step(100 + i))
+    ev1.record()
+    barrier()
+    launches = wl.wl_kernel_launches() - launches0
+    clocks = sampler.stop() if rank == 0 else None
+    ms_total = ev0.elapsed_time(ev1)
+    t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_total = float(t.item())
+    ms_per_step = ms_total / args.steps
+    edges_per_step = results[-1].stats["edges_streamed"]
+    value = world * edges_per_step / (ms_per_step / 1e3) / 1e9
+
+    # ---- roofline of the dominant kernel (S1+S2 SpMV), from the library's own CUDA events on the launch stream --------
+    peaks, peak_kind = measured_peaks()
+    spmv_ms = sum(r.stats["ms_spmv_kernel"] for r in results)
+    spmv_launches = sum(r.stats["spmv_launches"] for r in results)
+    alg_bytes = sum(r.stats["spmv_alg_bytes"] for r in results)  # (4+G) per streamed entry + 16 per row, DESIGN.md
+    spmv_edges = sum(r.stats["edges_streamed"] for r in results)
+    roofline = None
+    if spmv_launches:
+        achieved = alg_bytes / (spmv_ms / 1e3) / 1e9
+        roofline = {"bound": "hbm", "kernel": "spmv_merge_kernel" if args.flags & 4 else "spmv_rows32_kernel(+spmv_hub_kernel)",
+                    "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": achieved / peaks["hbm_gbs"],
+                    "peak_kind": f"{peak_kind} copy bandwidth", "algorithmic_bytes_per_launch": alg_bytes / spmv_launches,
+                    "avg_launch_ms": spmv_ms / spmv_launches, "launches_timed": spmv_launches,
+                    "gedges_per_s_in_kernel": spmv_edges / (spmv_ms / 1e3) / 1e9, "traffic": None,
+                    "share_of_step": spmv_ms / ms_total}
+
+    # ---- end to end through the host-buffer entry point ---------------------------------------------------------------
+    e2e = None
+    if not args.no_e2e:
+        h_rp = torch.empty(n + 1, dtype=torch.int64, pin_memory=True)
+        h_col = torch.empty(m, dtype=torch.int32, pin_memory=True)
+        h_out = torch.empty(n, dtype=torch.int32, pin_memory=True)
+        h_rp.copy_(g.row_ptr)
+        h_col.copy_(g.col)
+        torch.cuda.synchronize(dev)
+        e_steps = max(1, min(args.steps, 3))
+        wl.wl_refine_host(n, h_rp, h_col, seed=5, flags=args.flags, out=h_out)  # warm-up
+        barrier()
+        t0 = time.perf_counter()
+        for i in range(e_steps):
+            r = wl.wl_refine_host(n, h_rp, h_col, seed=200 + i, flags=args.flags, out=h_out)
+        torch.cuda.synchronize(dev)
+        dt = time.perf_counter() - t0
+        tt = torch.tensor([dt], dtype=torch.float64, device=dev)
+        if dist is not None:
+            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        dt = float(tt.item())
+        e2e = {"value": world * r.stats["edges_streamed"] * e_steps / dt / 1e9, "unit": "GEdges/s",
+               "h2d_bytes_per_step": r.stats["bytes_h2d"], "d2h_bytes_per_step": r.stats["bytes_d2h"],
+               "seconds_per_step": dt / e_steps, "steps": e_steps, "api": "wl_refine_host (pinned host CSR)"}
+        same = bool((h_out.to(dev) == out).all().item())
+        e2e["matches_device_path"] = same
+        del h_rp, h_col, h_out
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return 0
+
+    cpu_baseline = None
+    if not args.no_cpu_baseline and world == 1:
+        cb = oracle_sample(args.oracle_scale)
+        cpu_baseline = {k: cb[k] for k in ("value", "unit", "cores", "kind", "sample")}
+
+    last = results[-1]
+    line = {
+        "metric": "refine_gedges_per_s", "value": value, "unit": "GEdges/s", "n_gpus": world, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "u64", "data": "synthetic", "config": workload_config(args.scale, n, m),
+        "rounds": last.rounds, "num_colors": last.num_colors, "round_colors": last.round_colors,
+        "edges_streamed_per_step": edges_per_step,
+        "effective_gedges_per_s": world * m * last.rounds / (ms_per_step / 1e3) / 1e9,
+        "seconds_to_stable_coloring": ms_per_step / 1e3,
+        "phase_ms": {"spmv": last.stats["ms_spmv"], "relabel": last.stats["ms_relabel"], "total": last.stats["ms_total"]},
+        "roofline": roofline, "cpu_baseline": cpu_baseline, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
+    }
+    print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -54,8 +54,11 @@ typedef struct wl_csr {
 /* flags for wl_options.flags */
 #define WL_FLAG_NO_VALIDATE 1u   /* skip the CSR validation pass (one extra read of col_idx)                          */
 #define WL_FLAG_NO_PRUNE 2u      /* keep every row in every round (no active-set pruning); results are identical      */
-#define WL_FLAG_ROW_KERNEL 4u    /* use the simple warp-per-row SpMV instead of the edge-balanced merge-path kernel   */
+#define WL_FLAG_MERGE_KERNEL 4u  /* use the merge-path (edge-balanced, shared-memory staged) SpMV instead of the default
+                                    warp-per-row + hub-chunk kernels; implies no pruning                               */
 #define WL_FLAG_AGGRESSIVE_STOP 8u /* batched: stop when the next iteration's N_b would not decrease (L328)            */
+#define WL_FLAG_NARROW_COLORS 32u /* wl_spmv_round only: all colour ids are < 65536, gather them as 16-bit (wl_refine
+                                    switches by itself while k <= 65536)                                              */
 #define WL_FLAG_NO_CANONICAL 16u /* leave internal dense ids in out_colors (skips S6)                                  */
 
 typedef struct wl_options {
@@ -79,6 +82,11 @@ typedef struct wl_stats {
   double ms_total;           /* device time of the whole call (CUDA events on cuda_stream)                            */
   double ms_spmv;            /* sum over rounds of the S1+S2 kernels                                                  */
   double ms_relabel;         /* sum over rounds of the S3+S4 kernels                                                  */
+  int32_t spmv_launches;     /* rounds whose S1+S2 kernels streamed column indices (all rows or an active row list)   */
+  int32_t kernel_launches;   /* kernels launched by the call                                                          */
+  double ms_spmv_kernel;     /* device time of those S1+S2 kernels alone (CUDA events on cuda_stream)                 */
+  int64_t spmv_alg_bytes;    /* algorithmic bytes of those launches: (4+G) per streamed entry (G = 2 or 4 bytes of
+                                gathered colour id) + 16 per processed row (offsets + y)        */
 } wl_stats;
 
 /* ------------------------------------------------------------------------------------------------------------------
@@ -114,7 +122,7 @@ uint64_t wl_round_key(uint64_t seed, uint64_t stream_id, uint64_t round);
 uint64_t wl_weight(uint64_t key, uint64_t color);
 
 /* S1+S2: y_i = sum_j a_ij * w(colors[j]) mod 2^64 (Alg. 1 line 5, L120).  colors: DEVICE int32[n] (any non-negative
- * ids); y: DEVICE uint64[n]; workspace as for wl_refine.  flags: WL_FLAG_ROW_KERNEL selects the simple kernel. */
+ * ids); y: DEVICE uint64[n]; workspace as for wl_refine.  flags: WL_FLAG_MERGE_KERNEL selects the merge-path kernel. */
 int wl_spmv_round(const wl_csr* g, const int32_t* colors, uint64_t key, uint64_t* y, uint32_t flags, void* workspace,
                   size_t workspace_bytes, void* cuda_stream);
 
@@ -174,6 +182,7 @@ size_t wl_quotient_workspace_bytes(int64_t n, int64_t m);
 const char* wl_strerror(int code);
 int wl_last_cuda_error(void);      /* cudaError_t of the last WL_ECUDA on this thread */
 const char* wl_version(void);
+int64_t wl_kernel_launches(void);  /* kernels launched by this library on the calling thread since it was loaded */
 
 #ifdef __cplusplus
 }

@@ -16,12 +16,13 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "libwlrefine.so")
 
 WL_OK, WL_EINVAL, WL_ERANGE, WL_ENOMEM, WL_ECUDA, WL_EMAXROUNDS = 0, -1, -2, -3, -4, -5
-WL_FLAG_NO_VALIDATE, WL_FLAG_NO_PRUNE, WL_FLAG_ROW_KERNEL, WL_FLAG_AGGRESSIVE_STOP, WL_FLAG_NO_CANONICAL = 1, 2, 4, 8, 16
+WL_FLAG_NO_VALIDATE, WL_FLAG_NO_PRUNE, WL_FLAG_MERGE_KERNEL, WL_FLAG_AGGRESSIVE_STOP, WL_FLAG_NO_CANONICAL = 1, 2, 4, 8, 16
+WL_FLAG_NARROW_COLORS = 32
 
 EXPORTS = [
     "wl_refine_workspace_bytes", "wl_refine", "wl_refine_host", "wl_round_key", "wl_weight", "wl_spmv_round",
     "wl_relabel", "wl_canonicalize", "wl_refine_batched", "wl_inner_labels", "wl_quotient",
-    "wl_quotient_workspace_bytes", "wl_strerror", "wl_last_cuda_error", "wl_version",
+    "wl_quotient_workspace_bytes", "wl_strerror", "wl_last_cuda_error", "wl_version", "wl_kernel_launches",
 ]
 
 
@@ -48,7 +49,8 @@ class wl_stats(C.Structure):
     _fields_ = [("rounds", C.c_int32), ("outer_iters", C.c_int32), ("num_colors", C.c_int64),
                 ("last_num_batches", C.c_int64), ("boundary_nodes", C.c_int64), ("edges_streamed", C.c_int64),
                 ("bytes_h2d", C.c_int64), ("bytes_d2h", C.c_int64), ("ms_total", C.c_double), ("ms_spmv", C.c_double),
-                ("ms_relabel", C.c_double)]
+                ("ms_relabel", C.c_double), ("spmv_launches", C.c_int32), ("kernel_launches", C.c_int32),
+                ("ms_spmv_kernel", C.c_double), ("spmv_alg_bytes", C.c_int64)]
 
 
 class wl_edge_batch(C.Structure):
@@ -97,6 +99,7 @@ def lib():
         L.wl_strerror.argtypes = [C.c_int]
         L.wl_last_cuda_error.restype = C.c_int
         L.wl_version.restype = C.c_char_p
+        L.wl_kernel_launches.restype = C.c_int64
         _lib = L
     return _lib
 
@@ -276,6 +279,10 @@ def wl_canonicalize(colors: torch.Tensor, *, workspace=None):
 
 def wl_strerror(code: int) -> str:
     return lib().wl_strerror(code).decode()
+
+
+def wl_kernel_launches() -> int:
+    return int(lib().wl_kernel_launches())
 
 
 def wl_version() -> str:

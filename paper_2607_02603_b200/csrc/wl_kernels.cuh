@@ -150,26 +150,181 @@ spmv_merge_kernel(int64_t n, int64_t m, const int64_t* __restrict__ row_ptr, con
   if (acc) red_add_u64(y + i0 + ri, acc);
 }
 
-// S1+S2, simple variant: one warp per row (used for cross-checks and for pruned rounds over an active list).
-// rows == NULL: row index = warp index.  y is written with plain stores (no zeroing needed).
-template <bool WEIGHTED>
-__global__ void spmv_row_kernel(int64_t nrows, const int* __restrict__ rows, const int64_t* __restrict__ row_ptr,
-                                const int* __restrict__ col, const u32* __restrict__ wt,
-                                const int* __restrict__ colour, u64 key, u64* __restrict__ y) {
+// S1+S2, default kernel: one warp owns 32 consecutive rows (or 32 entries of the active row list).
+//   * rows with at most kSmallRow entries are summed by their own lane (thread per row, no shuffles, up to kSmallRow
+//     independent gathers in flight per lane);
+//   * longer rows are processed one after the other by the whole warp (coalesced column loads, four gathers in flight
+//     per lane, butterfly reduction);
+//   * rows longer than hub_threshold are left to spmv_hub_kernel (y = 0 here).
+// Everything accumulates in registers: the divergent gathers and shared-memory traffic share the LSU pipe, and staging
+// through shared memory (spmv_merge_kernel) more than doubled the time on B200 (profiles/).
+// CT = int or unsigned short (narrow colour ids while k <= 65536: the gathered array is half the size and a 32-byte
+// sector holds 16 nodes; measured 267 vs 125 G gathers/s on the scale-27 access pattern).
+constexpr int kSmallRow = 8;
+
+template <bool WEIGHTED, typename CT>
+__global__ void __launch_bounds__(256)
+spmv_rows32_kernel(int64_t nrows, const int* __restrict__ rows, const int64_t* __restrict__ row_ptr,
+                   const int* __restrict__ col, const u32* __restrict__ wt, const CT* __restrict__ colour, u64 key,
+                   u64* __restrict__ y, int64_t hub_threshold) {
   const int lane = threadIdx.x & 31;
-  int64_t w = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-  if (w >= nrows) return;
-  const int64_t i = rows ? rows[w] : w;
-  const int64_t a = row_ptr[i], b = row_ptr[i + 1];
+  const int64_t base = (((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5) << 5;
+  if (base >= nrows) return;
+  const int64_t idx = base + lane;
+  const bool valid = idx < nrows;
+  int64_t i = 0, a = 0, b = 0;
+  if (valid) {
+    i = rows ? (int64_t)rows[idx] : idx;
+    a = row_ptr[i];
+    b = row_ptr[i + 1];
+  }
+  const int64_t d = b - a;
+  const bool small = d <= kSmallRow;
   u64 acc = 0;
-  for (int64_t p = a + lane; p < b; p += 32) {
-    u64 v = weight_of(key, (u64)(u32)__ldg(colour + ld_stream_i32(col + p)));
+  {
+    const int dd = small ? (int)d : 0;
+    int cidx[kSmallRow];
+#pragma unroll
+    for (int t = 0; t < kSmallRow; ++t) cidx[t] = t < dd ? __ldg(col + a + t) : -1;
+#pragma unroll
+    for (int t = 0; t < kSmallRow; ++t) {
+      if (cidx[t] >= 0) {
+        u64 v = weight_of(key, (u64)__ldg(colour + cidx[t]));
+        if (WEIGHTED) v *= (u64)__ldg(wt + a + t);
+        acc += v;
+      }
+    }
+  }
+  unsigned big = __ballot_sync(0xffffffffu, valid && !small && d <= hub_threshold);
+  while (big) {
+    const int src = __ffs(big) - 1;
+    big &= big - 1;
+    const int64_t ra = __shfl_sync(0xffffffffu, a, src), rb = __shfl_sync(0xffffffffu, b, src);
+    u64 s = 0;
+    int64_t p = ra + lane;
+    for (; p + 96 < rb; p += 128) {  // four independent gathers in flight per lane
+      const int c0 = ld_stream_i32(col + p), c1 = ld_stream_i32(col + p + 32), c2 = ld_stream_i32(col + p + 64),
+                c3 = ld_stream_i32(col + p + 96);
+      u64 v0 = weight_of(key, (u64)__ldg(colour + c0)), v1 = weight_of(key, (u64)__ldg(colour + c1)),
+          v2 = weight_of(key, (u64)__ldg(colour + c2)), v3 = weight_of(key, (u64)__ldg(colour + c3));
+      if (WEIGHTED) {
+        v0 *= (u64)ld_stream_u32(wt + p);
+        v1 *= (u64)ld_stream_u32(wt + p + 32);
+        v2 *= (u64)ld_stream_u32(wt + p + 64);
+        v3 *= (u64)ld_stream_u32(wt + p + 96);
+      }
+      s += (v0 + v1) + (v2 + v3);
+    }
+    for (; p < rb; p += 32) {
+      u64 v = weight_of(key, (u64)__ldg(colour + ld_stream_i32(col + p)));
+      if (WEIGHTED) v *= (u64)ld_stream_u32(wt + p);
+      s += v;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    if (lane == src) acc = s;
+  }
+  if (valid) y[i] = acc;
+}
+
+// Hub rows (degree > hub_threshold) are cut into chunks of kHubChunk entries, one CTA each; partial sums meet in y
+// through one no-return 64-bit add per CTA (exact under any order: sums in Z/2^64).
+constexpr int kHubChunk = 4096;
+constexpr int kHubThreads = 256;
+
+__global__ void hub_collect_kernel(int64_t n, const int64_t* __restrict__ row_ptr, int64_t hub_threshold,
+                                   int2* __restrict__ chunks, u64* __restrict__ counter) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const int64_t d = row_ptr[i + 1] - row_ptr[i];
+  if (d <= hub_threshold) return;
+  const int nc = (int)((d + kHubChunk - 1) / kHubChunk);
+  const u64 base = atomicAdd(counter, (u64)nc);
+  for (int c = 0; c < nc; ++c) chunks[base + c] = make_int2((int)i, c);
+}
+
+// active == NULL: every hub row; else only rows whose block is still splittable (stamp[colour[row]] == live_stamp)
+template <bool WEIGHTED, typename CT>
+__global__ void __launch_bounds__(kHubThreads)
+spmv_hub_kernel(const int2* __restrict__ chunks, const int64_t* __restrict__ row_ptr, const int* __restrict__ col,
+                const u32* __restrict__ wt, const CT* __restrict__ colour, u64 key, u64* __restrict__ y,
+                const int* __restrict__ colour32, const int* __restrict__ stamp, int live_stamp) {
+  const int2 ch = chunks[blockIdx.x];
+  const int64_t row = ch.x;
+  if (stamp && stamp[colour32[row]] != live_stamp) return;
+  const int64_t a = row_ptr[row] + (int64_t)ch.y * kHubChunk;
+  int64_t b = a + kHubChunk;
+  const int64_t rend = row_ptr[row + 1];
+  if (b > rend) b = rend;
+  u64 acc = 0;
+#pragma unroll 4
+  for (int64_t p = a + threadIdx.x; p < b; p += kHubThreads) {
+    u64 v = weight_of(key, (u64)__ldg(colour + ld_stream_i32(col + p)));
     if (WEIGHTED) v *= (u64)ld_stream_u32(wt + p);
     acc += v;
   }
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
-  if (lane == 0) y[i] = acc;
+  __shared__ u64 s[kHubThreads / 32];
+  if ((threadIdx.x & 31) == 0) s[threadIdx.x >> 5] = acc;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    u64 t = 0;
+#pragma unroll
+    for (int w = 0; w < kHubThreads / 32; ++w) t += s[w];
+    if (t) red_add_u64(y + row, t);
+  }
+}
+
+// narrow copy of the colour ids for rounds with k <= 65536
+__global__ void narrow_kernel(int64_t n, const int* __restrict__ colour, unsigned short* __restrict__ colour16) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) colour16[i] = (unsigned short)colour[i];
+}
+
+// Active-set pruning (SURVEY.md §8(d) option 6): a node whose block is a singleton can never split again and keeps its
+// id, so its row needs neither y nor a relabel.  next = nodes of `nodes` (NULL: all) whose block still has >= 2 members
+// after round `round`; counters[0] += |next|, counters[1] += sum of their out-degrees.  Rows without out-edges are
+// dropped as soon as their block's representative has none either (their y is 0 in every round).
+__global__ void __launch_bounds__(256)
+compact_active_kernel(int64_t count, const int* __restrict__ nodes, const int* __restrict__ colour,
+                      const int* __restrict__ stamp, const int* __restrict__ rep, int round,
+                      const int64_t* __restrict__ row_ptr, int* __restrict__ next, u64* __restrict__ counters) {
+  int64_t t = (int64_t)blockIdx.x * 256 + threadIdx.x;
+  bool keep = false;
+  int i = 0;
+  u64 deg = 0;
+  if (t < count) {
+    i = nodes ? nodes[t] : (int)t;
+    const int c = colour[i];
+    keep = stamp[c] == round;
+    if (keep) {
+      deg = (u64)(row_ptr[i + 1] - row_ptr[i]);
+      if (deg == 0) {
+        // y_i = 0 in every round.  If the block's representative has no out-edge either, every member with an
+        // out-edge is compared against y[rep] = 0 and leaves on its own; the edgeless members never need another look.
+        const int r = rep[c];
+        keep = row_ptr[r + 1] != row_ptr[r];
+      }
+    }
+  }
+  int total;
+  const int rank = block_rank<256>(keep, &total);
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) deg += __shfl_xor_sync(0xffffffffu, deg, o);
+  __shared__ u64 s_deg[8];
+  __shared__ u64 s_base;
+  if ((threadIdx.x & 31) == 0) s_deg[threadIdx.x >> 5] = deg;
+  __syncthreads();
+  if (threadIdx.x == 0 && total > 0) {
+    u64 d = 0;
+#pragma unroll
+    for (int w = 0; w < 8; ++w) d += s_deg[w];
+    s_base = atomicAdd(counters, (u64)total);
+    atomicAdd(counters + 1, d);
+  }
+  __syncthreads();
+  if (keep) next[s_base + rank] = i;
 }
 
 // Round with a single colour and unit weights: y_i = outdeg(i) * w(0); no column read.

@@ -4,6 +4,7 @@
 
 #include <algorithm>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <vector>
 
@@ -12,6 +13,7 @@
 namespace wl {
 
 thread_local int g_last_cuda_error = 0;
+thread_local int64_t g_launches = 0;
 
 static inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
@@ -44,6 +46,11 @@ Layout make_layout(int64_t n, int64_t m) {
   L.o_tile_row = take(sizeof(int) * (size_t)(L.ntiles + 1));
   L.o_bsum = take(sizeof(int) * (size_t)(L.nscan + 1));
   L.o_table = take(sizeof(Slot) * ((size_t)L.table_mask + 1));
+  L.o_colour16 = take(sizeof(unsigned short) * (size_t)n);
+  L.o_act0 = take(sizeof(int) * (size_t)n);
+  L.o_act1 = take(sizeof(int) * (size_t)n);
+  L.hub_cap = m / kHubChunk + m / (kHubThreshold + 1) + 1;
+  L.o_hub = take(sizeof(int2) * (size_t)L.hub_cap);
   L.bytes = off;
   return L;
 }
@@ -52,38 +59,66 @@ static inline unsigned blocks_for(int64_t count, int threads) { return (unsigned
 
 // ---- step launchers -----------------------------------------------------------------------------------------------
 void launch_tile_search(const Layout& L, const wl_csr& g, int* tile_row, cudaStream_t st) {
-  tile_search_kernel<<<blocks_for(L.ntiles + 1, 256), 256, 0, st>>>(g.n, g.m, g.row_ptr, L.ntiles, tile_row);
+  ++g_launches; tile_search_kernel<<<blocks_for(L.ntiles + 1, 256), 256, 0, st>>>(g.n, g.m, g.row_ptr, L.ntiles, tile_row);
 }
 
-void launch_spmv(const Layout& L, const wl_csr& g, const int* colour, u64 key, const int* tile_row, u64* y,
-                 bool row_kernel, cudaStream_t st) {
-  if (g.n == 0) return;
-  if (row_kernel) {
-    unsigned grid = blocks_for(g.n * 32, 256);
-    if (g.weights)
-      spmv_row_kernel<true><<<grid, 256, 0, st>>>(g.n, nullptr, g.row_ptr, g.col_idx, g.weights, colour, key, y);
-    else
-      spmv_row_kernel<false><<<grid, 256, 0, st>>>(g.n, nullptr, g.row_ptr, g.col_idx, g.weights, colour, key, y);
+// S1+S2 over all rows or an active row list.  merge: the merge-path kernel (all rows; y must be zero before it).
+// Otherwise warp-per-row over `rows` (NULL: all) followed by the hub-chunk kernel.  narrow: gather 16-bit colour ids.
+struct SpmvArgs {
+  const int* rows;       // active row list or NULL
+  int64_t nrows;         // rows to process (n when rows == NULL)
+  const int* colour;     // int32 colours
+  const unsigned short* colour16;  // valid when narrow
+  bool narrow;
+  const int2* hub_chunks;
+  int64_t num_hub_chunks;
+  const int* stamp;      // hub activity test (NULL: all hubs)
+  int live_stamp;
+};
+
+template <bool W, typename CT>
+static void launch_row_hub(const wl_csr& g, const SpmvArgs& a, const CT* colour, u64 key, u64* y, cudaStream_t st) {
+  unsigned grid = blocks_for(a.nrows, 256);
+  ++g_launches; spmv_rows32_kernel<W, CT><<<grid, 256, 0, st>>>(a.nrows, a.rows, g.row_ptr, g.col_idx, g.weights, colour, key, y, kHubThreshold);
+  if (a.num_hub_chunks > 0) {
+    ++g_launches; spmv_hub_kernel<W, CT><<<(unsigned)a.num_hub_chunks, kHubThreads, 0, st>>>(a.hub_chunks, g.row_ptr, g.col_idx, g.weights, colour, key, y, a.colour, a.stamp, a.live_stamp);
+  }
+}
+
+void launch_spmv(const Layout& L, const wl_csr& g, const SpmvArgs& a, u64 key, const int* tile_row, u64* y, bool merge,
+                 cudaStream_t st) {
+  if (g.n == 0 || a.nrows == 0) return;
+  if (merge) {
+    if (g.weights) {
+      ++g_launches; spmv_merge_kernel<true><<<(unsigned)L.ntiles, kSpmvThreads, 0, st>>>(g.n, g.m, g.row_ptr, g.col_idx, g.weights, a.colour, key, tile_row, y);
+    } else {
+      ++g_launches; spmv_merge_kernel<false><<<(unsigned)L.ntiles, kSpmvThreads, 0, st>>>(g.n, g.m, g.row_ptr, g.col_idx, g.weights, a.colour, key, tile_row, y);
+    }
     return;
   }
-  cudaMemsetAsync(y, 0, sizeof(u64) * (size_t)g.n, st);
-  if (g.weights)
-    spmv_merge_kernel<true><<<(unsigned)L.ntiles, kSpmvThreads, 0, st>>>(g.n, g.m, g.row_ptr, g.col_idx, g.weights,
-                                                                        colour, key, tile_row, y);
-  else
-    spmv_merge_kernel<false><<<(unsigned)L.ntiles, kSpmvThreads, 0, st>>>(g.n, g.m, g.row_ptr, g.col_idx, g.weights,
-                                                                         colour, key, tile_row, y);
+  if (g.weights) {
+    if (a.narrow) launch_row_hub<true, unsigned short>(g, a, a.colour16, key, y, st);
+    else launch_row_hub<true, int>(g, a, a.colour, key, y, st);
+  } else {
+    if (a.narrow) launch_row_hub<false, unsigned short>(g, a, a.colour16, key, y, st);
+    else launch_row_hub<false, int>(g, a, a.colour, key, y, st);
+  }
+}
+
+// hub chunk list (rows with degree > kHubThreshold); *counter (device u64) must be zero
+void launch_hub_collect(const Layout& L, const wl_csr& g, int2* chunks, u64* counter, cudaStream_t st) {
+  if (g.n == 0) return;
+  ++g_launches; hub_collect_kernel<<<blocks_for(g.n, 256), 256, 0, st>>>(g.n, g.row_ptr, kHubThreshold, chunks, counter);
 }
 
 // one relabel step over all nodes; counter (device u64) must be zero on entry and holds the number of new ids on exit
-void launch_relabel(const Layout& L, int64_t n, int* colour, const u64* y, int* rep, int* stamp, int round, Slot* table,
-                    u32* tmp, int k_old, u64* counter, cudaStream_t st) {
-  if (n == 0) return;
-  unsigned grid = blocks_for(n, kRelabelThreads);
-  relabel_insert_kernel<<<grid, kRelabelThreads, 0, st>>>(n, nullptr, colour, y, rep, stamp, round, table, L.table_mask,
-                                                          tmp, k_old, counter);
-  relabel_resolve_kernel<<<grid, kRelabelThreads, 0, st>>>(n, nullptr, colour, stamp, round, table, tmp);
-  relabel_cleanup_kernel<<<grid, kRelabelThreads, 0, st>>>(n, nullptr, table, tmp);
+void launch_relabel(const Layout& L, int64_t count, const int* nodes, int* colour, const u64* y, int* rep, int* stamp,
+                    int round, Slot* table, u32* tmp, int k_old, u64* counter, cudaStream_t st) {
+  if (count == 0) return;
+  unsigned grid = blocks_for(count, kRelabelThreads);
+  ++g_launches; relabel_insert_kernel<<<grid, kRelabelThreads, 0, st>>>(count, nodes, colour, y, rep, stamp, round, table, L.table_mask, tmp, k_old, counter);
+  ++g_launches; relabel_resolve_kernel<<<grid, kRelabelThreads, 0, st>>>(count, nodes, colour, stamp, round, table, tmp);
+  ++g_launches; relabel_cleanup_kernel<<<grid, kRelabelThreads, 0, st>>>(count, nodes, table, tmp);
 }
 
 // canonical ids: uses `first` (int[n]) and `cof` (int[n]) as scratch, bsum int[nscan+1], total -> scal slot
@@ -91,11 +126,11 @@ void launch_canonical(const Layout& L, int64_t n, const int* colour, int* out, i
                       u64* total, cudaStream_t st) {
   if (n == 0) return;
   cudaMemsetAsync(first, 0x7f, sizeof(int) * (size_t)n, st);
-  first_node_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, colour, first);
-  canon_count_kernel<<<(unsigned)L.nscan, kScanThreads, 0, st>>>(n, colour, first, bsum);
-  scan_bsum_kernel<<<1, 1024, 0, st>>>(L.nscan, bsum, total);
-  canon_rank_kernel<<<(unsigned)L.nscan, kScanThreads, 0, st>>>(n, colour, first, bsum, cof);
-  canon_apply_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, colour, first, cof, out);
+  ++g_launches; first_node_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, colour, first);
+  ++g_launches; canon_count_kernel<<<(unsigned)L.nscan, kScanThreads, 0, st>>>(n, colour, first, bsum);
+  ++g_launches; scan_bsum_kernel<<<1, 1024, 0, st>>>(L.nscan, bsum, total);
+  ++g_launches; canon_rank_kernel<<<(unsigned)L.nscan, kScanThreads, 0, st>>>(n, colour, first, bsum, cof);
+  ++g_launches; canon_apply_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, colour, first, cof, out);
 }
 
 int check_cuda(cudaError_t e) {
@@ -181,6 +216,7 @@ int wl_refine(const wl_csr* g, const int32_t* init_colors, uint64_t seed, int32_
   int* bsum = (int*)(ws + L.o_bsum);
   Slot* table = (Slot*)(ws + L.o_table);
 
+  const int64_t launches_at_entry = g_launches;
   EventPool evp;
   cudaEvent_t ev_begin = evp.get(0), ev_end = evp.get(1);
   cudaEventRecord(ev_begin, st);
@@ -191,8 +227,8 @@ int wl_refine(const wl_csr* g, const int32_t* init_colors, uint64_t seed, int32_
   cudaMemsetAsync(stamp, 0xff, sizeof(int) * (size_t)n, st);
   u32* d_err = (u32*)(scal + kScalErr);
   if (!(flags & WL_FLAG_NO_VALIDATE)) {
-    validate_rows_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, m, g->row_ptr, g->weights, d_err);
-    if (m > 0) validate_cols_kernel<<<148 * 8, 256, 0, st>>>(n, m, g->col_idx, d_err);
+    ++g_launches; validate_rows_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, m, g->row_ptr, g->weights, d_err);
+    if (m > 0) { ++g_launches; validate_cols_kernel<<<148 * 8, 256, 0, st>>>(n, m, g->col_idx, d_err); }
     // the merge-path search below walks row_ptr: make sure it is well formed first
     cudaMemcpyAsync(hs + kScalErr, scal + kScalErr, sizeof(u64), cudaMemcpyDeviceToHost, st);
     rc = check_cuda(cudaStreamSynchronize(st));
@@ -201,60 +237,114 @@ int wl_refine(const wl_csr* g, const int32_t* init_colors, uint64_t seed, int32_
     if (e & (kErrRowPtr | kErrCol)) return WL_EINVAL;
     if (e & kErrRowSum) return WL_ERANGE;
   }
-  const bool row_kernel = (flags & WL_FLAG_ROW_KERNEL) != 0;
-  if (!row_kernel) launch_tile_search(L, *g, tile_row, st);
+  const bool merge = (flags & WL_FLAG_MERGE_KERNEL) != 0;
+  const bool prune = !merge && !(flags & WL_FLAG_NO_PRUNE);
+  unsigned short* colour16 = (unsigned short*)(ws + L.o_colour16);
+  int* act[2] = {(int*)(ws + L.o_act0), (int*)(ws + L.o_act1)};
+  int2* hub_chunks = (int2*)(ws + L.o_hub);
+  if (merge) launch_tile_search(L, *g, tile_row, st);
+  else launch_hub_collect(L, *g, hub_chunks, scal + kScalHub, st);
 
   // initial partition: colour 0 everywhere; a given init is densified by one relabel step keyed on the label (L94)
   int64_t k = 1;
-  init_labels_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, init_colors, colour, y, d_err);
-  // rep[0] = node 0; stamp[0] = 0 marks block 0 as non-singleton when n >= 2
+  ++g_launches; init_labels_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, init_colors, colour, y, d_err);
+  // rep[0] = node 0; stamp[0] = 0 marks block 0 as non-singleton (n >= 2)
   cudaMemsetAsync(rep, 0, sizeof(int), st);
-  if (init_colors) {
-    launch_relabel(L, n, colour, y, rep, stamp, /*round=*/0, table, tmp, /*k_old=*/1, scal + kScalNew, st);
-    cudaMemcpyAsync(hs, scal, sizeof(u64) * kNumScal, cudaMemcpyDeviceToHost, st);
-    rc = check_cuda(cudaStreamSynchronize(st));
-    if (rc) return rc;
-    if ((u32)hs[kScalErr] & kErrInit) return WL_EINVAL;
-    k = 1 + (int64_t)hs[kScalNew];
-  }
+  cudaMemsetAsync(stamp, 0, sizeof(int), st);
+  if (init_colors)
+    launch_relabel(L, n, nullptr, colour, y, rep, stamp, /*round=*/0, table, tmp, /*k_old=*/1, scal + kScalNew, st);
+  cudaMemcpyAsync(hs, scal, sizeof(u64) * kNumScal, cudaMemcpyDeviceToHost, st);
+  rc = check_cuda(cudaStreamSynchronize(st));
+  if (rc) return rc;
+  if ((u32)hs[kScalErr] & kErrInit) return WL_EINVAL;
+  k = 1 + (int64_t)hs[kScalNew];
+  const int64_t num_hub_chunks = merge ? 0 : (int64_t)hs[kScalHub];
 
   // ---- S1-S5: rounds -------------------------------------------------------------------------------------------------
-  int64_t edges_streamed = 0;
-  double ms_spmv = 0, ms_relabel = 0;
-  int32_t rounds = 0;
+  int64_t edges_streamed = 0, spmv_alg_bytes = 0;
+  double ms_spmv = 0, ms_relabel = 0, ms_spmv_kernel = 0;
+  int32_t rounds = 0, spmv_launches = 0;
   bool converged = false;
-  const u64 w0_dummy = 0;
-  (void)w0_dummy;
+  const bool debug = std::getenv("WL_DEBUG") != nullptr;
+  const double list_frac = std::getenv("WL_LIST_FRAC") ? std::atof(std::getenv("WL_LIST_FRAC")) : 0.75;
+  const int* cur_list = nullptr;  // NULL: every node is active
+  int64_t n_active = n, active_edges = m;
+  int cur = 0;
   for (int64_t r = 1; r <= max_rounds; ++r) {
     const u64 key = round_key(seed, stream_id, (u64)r);
-    cudaEvent_t e0 = evp.get(2), e1 = evp.get(3), e2 = evp.get(4);
+    cudaEvent_t e0 = evp.get(2), e1 = evp.get(3), e2 = evp.get(4), ek0 = evp.get(5), ek1 = evp.get(6);
     cudaEventRecord(e0, st);
+    bool full_spmv = false;
     if (k == 1 && !g->weights) {
-      spmv_uniform_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, g->row_ptr, weight_of(key, 0), y);
+      ++g_launches; spmv_uniform_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, g->row_ptr, weight_of(key, 0), y);
     } else {
-      launch_spmv(L, *g, colour, key, tile_row, y, row_kernel, st);
-      edges_streamed += m;
+      const bool narrow = !merge && k <= 65536;
+      if (narrow) { ++g_launches; narrow_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, colour, colour16); }
+      if (merge) cudaMemsetAsync(y, 0, sizeof(u64) * (size_t)n, st);
+      SpmvArgs a{cur_list, n_active, colour, colour16, narrow, hub_chunks, num_hub_chunks,
+                 cur_list ? stamp : nullptr, (int)r - 1};
+      cudaEventRecord(ek0, st);
+      launch_spmv(L, *g, a, key, tile_row, y, merge, st);
+      cudaEventRecord(ek1, st);
+      edges_streamed += active_edges;
+      spmv_alg_bytes += (int64_t)(4 + (narrow ? 2 : 4) + (g->weights ? 4 : 0)) * active_edges + 16 * n_active;
+      full_spmv = true;
     }
     cudaEventRecord(e1, st);
     cudaMemsetAsync(scal + kScalNew, 0, sizeof(u64), st);
-    launch_relabel(L, n, colour, y, rep, stamp, (int)r, table, tmp, (int)k, scal + kScalNew, st);
+    launch_relabel(L, n_active, cur_list, colour, y, rep, stamp, (int)r, table, tmp, (int)k, scal + kScalNew, st);
+    if (prune) {
+      cudaMemsetAsync(scal + kScalActive, 0, 2 * sizeof(u64), st);
+      ++g_launches; compact_active_kernel<<<blocks_for(n_active, 256), 256, 0, st>>>(n_active, cur_list, colour, stamp, rep, (int)r, g->row_ptr, act[cur], scal + kScalActive);
+    }
     cudaEventRecord(e2, st);
     cudaMemcpyAsync(hs, scal, sizeof(u64) * kNumScal, cudaMemcpyDeviceToHost, st);
     rc = check_cuda(cudaStreamSynchronize(st));
     if (rc) return rc;
-    float a = 0, b = 0;
-    cudaEventElapsedTime(&a, e0, e1);
-    cudaEventElapsedTime(&b, e1, e2);
-    ms_spmv += a;
-    ms_relabel += b;
+    float ta = 0, tb = 0;
+    cudaEventElapsedTime(&ta, e0, e1);
+    cudaEventElapsedTime(&tb, e1, e2);
+    ms_spmv += ta;
+    ms_relabel += tb;
+    if (full_spmv) {
+      float tc = 0;
+      cudaEventElapsedTime(&tc, ek0, ek1);
+      ms_spmv_kernel += tc;
+      ++spmv_launches;
+    }
     const int64_t k_new = k + (int64_t)hs[kScalNew];
     rounds = (int32_t)r;
+    if (debug)
+      std::fprintf(stderr, "[wl_refine] round %lld: k %lld -> %lld, rows %lld, edges %lld, spmv %.3f ms, relabel %.3f ms\n",
+                   (long long)r, (long long)k, (long long)k_new, (long long)n_active, (long long)active_edges, ta, tb);
     if (opt && opt->round_colors && r <= opt->round_colors_cap) opt->round_colors[r - 1] = k_new;
     if (k_new == k) {  // the partition did not change (Q1, Q2): fixed point
       converged = true;
       break;
     }
     k = k_new;
+    if (prune) {
+      n_active = (int64_t)hs[kScalActive];
+      active_edges = (int64_t)hs[kScalActiveDeg];
+      if ((double)n_active < list_frac * (double)n) {
+        cur_list = act[cur];
+        cur ^= 1;
+      } else {  // nearly everything is still active: keep the list-free kernels
+        cur_list = nullptr;
+        n_active = n;
+        active_edges = m;
+      }
+      if (n_active == 0) {
+        // every block is a singleton: the next round cannot change anything and only confirms (same trajectory as
+        // the un-pruned algorithm)
+        if (r + 1 <= max_rounds) {
+          rounds = (int32_t)(r + 1);
+          if (opt && opt->round_colors && r + 1 <= opt->round_colors_cap) opt->round_colors[r] = k;
+          converged = true;
+        }
+        break;
+      }
+    }
   }
 
   // ---- S6: canonical ids ---------------------------------------------------------------------------------------------
@@ -278,6 +368,10 @@ int wl_refine(const wl_csr* g, const int32_t* init_colors, uint64_t seed, int32_
     stats->ms_total = t;
     stats->ms_spmv = ms_spmv;
     stats->ms_relabel = ms_relabel;
+    stats->ms_spmv_kernel = ms_spmv_kernel;
+    stats->spmv_launches = spmv_launches;
+    stats->spmv_alg_bytes = spmv_alg_bytes;
+    stats->kernel_launches = (int32_t)(g_launches - launches_at_entry);
   }
   return converged ? WL_OK : WL_EMAXROUNDS;
 }
@@ -360,10 +454,27 @@ int wl_spmv_round(const wl_csr* g, const int32_t* colors, uint64_t key, uint64_t
   const Layout L = make_layout(g->n, g->m);
   if (workspace_bytes < L.bytes) return WL_ENOMEM;
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  int* tile_row = (int*)((char*)workspace + L.o_tile_row);
-  const bool row_kernel = (flags & WL_FLAG_ROW_KERNEL) != 0;
-  if (!row_kernel) launch_tile_search(L, *g, tile_row, st);
-  launch_spmv(L, *g, colors, key, tile_row, (u64*)y, row_kernel, st);
+  char* ws = (char*)workspace;
+  int* tile_row = (int*)(ws + L.o_tile_row);
+  u64* scal = (u64*)(ws + L.o_scal);
+  const bool merge = (flags & WL_FLAG_MERGE_KERNEL) != 0;
+  const bool narrow = !merge && (flags & WL_FLAG_NARROW_COLORS) != 0;
+  SpmvArgs a{nullptr, g->n, colors, (unsigned short*)(ws + L.o_colour16), narrow, (int2*)(ws + L.o_hub), 0, nullptr, 0};
+  if (merge) {
+    launch_tile_search(L, *g, tile_row, st);
+    cudaMemsetAsync(y, 0, sizeof(u64) * (size_t)g->n, st);
+  } else {
+    u64* hs = host_scal();
+    if (!hs) return WL_ECUDA;
+    cudaMemsetAsync(scal, 0, sizeof(u64) * kNumScal, st);
+    launch_hub_collect(L, *g, (int2*)(ws + L.o_hub), scal + kScalHub, st);
+    cudaMemcpyAsync(hs, scal, sizeof(u64) * kNumScal, cudaMemcpyDeviceToHost, st);
+    rc = check_cuda(cudaStreamSynchronize(st));
+    if (rc) return rc;
+    a.num_hub_chunks = (int64_t)hs[kScalHub];
+    if (narrow) { ++g_launches; narrow_kernel<<<blocks_for(g->n, 256), 256, 0, st>>>(g->n, colors, (unsigned short*)(ws + L.o_colour16)); }
+  }
+  launch_spmv(L, *g, a, key, tile_row, (u64*)y, merge, st);
   rc = check_cuda(cudaStreamSynchronize(st));
   if (rc) return rc;
   return check_cuda(cudaGetLastError());
@@ -394,8 +505,8 @@ int wl_relabel(int64_t n, const int32_t* colors, int64_t k, const uint64_t* y, i
   cudaMemsetAsync(stamp, 0xff, sizeof(int) * (size_t)n, st);
   if (new_colors != colors)
     cudaMemcpyAsync(new_colors, colors, sizeof(int) * (size_t)n, cudaMemcpyDeviceToDevice, st);
-  set_rep_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, new_colors, rep);
-  launch_relabel(L, n, new_colors, (const u64*)y, rep, stamp, 1, table, tmp, (int)k, scal + kScalNew, st);
+  ++g_launches; set_rep_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, new_colors, rep);
+  launch_relabel(L, n, nullptr, new_colors, (const u64*)y, rep, stamp, 1, table, tmp, (int)k, scal + kScalNew, st);
   cudaMemcpyAsync(hs, scal, sizeof(u64) * kNumScal, cudaMemcpyDeviceToHost, st);
   int rc = check_cuda(cudaStreamSynchronize(st));
   if (rc) return rc;
@@ -440,6 +551,7 @@ const char* wl_strerror(int code) {
   }
 }
 int wl_last_cuda_error(void) { return g_last_cuda_error; }
+int64_t wl_kernel_launches(void) { return g_launches; }
 const char* wl_version(void) { return "wl_refine 0.1 (sm_100a)"; }
 
 }  // extern "C"

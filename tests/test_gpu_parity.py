@@ -41,6 +41,10 @@ GRAPHS = {
     "dpath_40": lambda: gg.directed_path(40),
     "star_1000": lambda: gg.star_graph(1000),
     "hub_20000": lambda: gg.from_edge_list(20001, [(0, j) for j in range(1, 20001)] + [(5, 7), (9, 7)]),
+    # two twin hubs (degree 10000 > the hub-chunk threshold) that stay in one block over many rounds, plus a directed
+    # path among their targets so that refinement takes a few hundred rounds with the hubs still active
+    "twin_hubs": lambda: gg.from_edge_list(10302, [(h, j) for h in (0, 1) for j in range(2, 10002)]
+                                           + [(j, j + 1) for j in range(10002, 10301)] + [(2, 10002), (3, 10002)]),
     "k_5_7": lambda: gg.complete_bipartite(5, 7),
     "circ": lambda: gg.circulant(50, (1, 4, 9)),
     "empty_edges": lambda: gg.from_edge_list(17, []),
@@ -53,11 +57,11 @@ GRAPHS = {
 
 # ------------------------------------------------------------------ S1+S2
 @pytest.mark.parametrize("name", list(GRAPHS))
-@pytest.mark.parametrize("flags", [0, 4])
+@pytest.mark.parametrize("flags", [0, 4, 32])
 def test_spmv_bit_exact(name, flags):
     g = GRAPHS[name]()
     n, rp, ci, wt = g.numpy()
-    colors = gg.random_partition(n, max(1, n // 3), 11).numpy()
+    colors = gg.random_partition(n, max(1, min(n // 3, 60000)), 11).numpy()
     key = wl.wl_round_key(123, 0, 2)
     assert key == oracle.round_key(123, 0, 2)
     want = oracle.spmv_u64(n, rp, ci, wt, oracle_w(key, colors))
@@ -120,7 +124,7 @@ def test_canonicalize(n):
 
 # ------------------------------------------------------------------ whole Algorithm 1
 @pytest.mark.parametrize("name", list(GRAPHS))
-@pytest.mark.parametrize("flags", [0, 4])
+@pytest.mark.parametrize("flags", [0, 2, 4])
 def test_refine_equals_oracle(name, flags):
     g = GRAPHS[name]()
     n, rp, ci, wt = g.numpy()
