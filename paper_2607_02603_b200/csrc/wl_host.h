@@ -24,6 +24,33 @@ struct Layout {
 };
 Layout make_layout(int64_t n, int64_t m);
 
+struct CoreResult {
+  int64_t k, edges_streamed, spmv_alg_bytes;
+  int32_t rounds, spmv_launches, kernel_launches;
+  double ms_spmv, ms_relabel, ms_spmv_kernel;
+  int* colour;  // dense ids, inside the workspace
+};
+int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, const wl_options* opt, bool ranged, int lo,
+                int hi, int64_t n_targets, int64_t edge_first, void* workspace, const Layout& L, cudaStream_t st,
+                CoreResult* res);
+void launch_canonical(const Layout& L, int64_t n, const int* colour, int* out, int* first, int* cof, int* bsum, u64* total,
+                      cudaStream_t st);
+u64* host_scal();
+static inline unsigned blocks_for(int64_t count, int threads) { return (unsigned)((count + threads - 1) / threads); }
+static inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
+
+struct EventPool {
+  cudaEvent_t ev[8];
+  int n = 0;
+  ~EventPool() {
+    for (int i = 0; i < n; ++i) cudaEventDestroy(ev[i]);
+  }
+  cudaEvent_t get(int i) {
+    while (n <= i) cudaEventCreate(&ev[n++]);
+    return ev[i];
+  }
+};
+
 extern thread_local int g_last_cuda_error;
 extern thread_local int64_t g_launches;
 int check_cuda(cudaError_t e);

@@ -16,31 +16,36 @@ constexpr u32 kErrRowPtr = 1u, kErrCol = 2u, kErrRowSum = 4u, kErrInit = 8u;
 // ---------------------------------------------------------------------------------------------------------------------
 // S0: validation of the CSR (WL_EINVAL / WL_ERANGE conditions of include/wl_refine.h)
 // ---------------------------------------------------------------------------------------------------------------------
-__global__ void validate_rows_kernel(int64_t n, int64_t m, const int64_t* __restrict__ row_ptr,
-                                     const u32* __restrict__ wt, u32* __restrict__ err) {
+// Offsets may start anywhere (a batch slice indexes the batch's column buffer through a shifted pointer): the caller
+// says which first / last offset it expects (0 and m for a whole graph).
+__global__ void validate_rows_kernel(int64_t n, const int64_t* __restrict__ row_ptr, const u32* __restrict__ wt,
+                                     int64_t expect_first, int64_t expect_last, u32* __restrict__ err) {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
   int64_t a = row_ptr[i], b = row_ptr[i + 1];
   u32 e = 0;
-  if (i == 0 && a != 0) e |= kErrRowPtr;
-  if (i == n - 1 && b != m) e |= kErrRowPtr;
-  if (a > b || a < 0 || b > m) e |= kErrRowPtr;
+  if (i == 0 && a != expect_first) e |= kErrRowPtr;
+  if (i == n - 1 && b != expect_last) e |= kErrRowPtr;
+  if (a > b || a < expect_first || b > expect_last) e |= kErrRowPtr;
   if (!e) {
     if (wt) {
       u64 s = 0;
       for (int64_t p = a; p < b; ++p) s += wt[p];
-      if (s > (1ull << 32)) e |= kErrRowSum;
-    } else if ((u64)(b - a) > (1ull << 32)) {
+      if (s >= (1ull << 32)) e |= kErrRowSum;  // quotient weights are row-sum bounded and travel as uint32
+    } else if ((u64)(b - a) >= (1ull << 32)) {
       e |= kErrRowSum;
     }
   }
   if (e) atomicOr(err, e);
 }
 
-__global__ void validate_cols_kernel(int64_t n, int64_t m, const int* __restrict__ col, u32* __restrict__ err) {
+// every stored target must be a node id in [0, n_targets); entries [begin, m) of col are checked
+__global__ void validate_cols_kernel(int64_t n_targets, int64_t begin, int64_t m, const int* __restrict__ col,
+                                     u32* __restrict__ err) {
+  const int64_t n = n_targets;
   int64_t stride = (int64_t)gridDim.x * blockDim.x;
   bool bad = false;
-  for (int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; p < m; p += stride) {
+  for (int64_t p = begin + (int64_t)blockIdx.x * blockDim.x + threadIdx.x; p < m; p += stride) {
     int c = col[p];
     bad |= (c < 0) | ((int64_t)c >= n);
   }
@@ -150,6 +155,18 @@ spmv_merge_kernel(int64_t n, int64_t m, const int64_t* __restrict__ row_ptr, con
   if (acc) red_add_u64(y + i0 + ri, acc);
 }
 
+// Colour id of target node j.  Plain RSC: the dense id colour[j].  Batched local RSC (RANGED): nodes of V_k = [lo, hi)
+// carry dense ids (< 2^32) in colour[j - lo]; every other node is an implicit singleton of H_k^0 (Eq. 3) whose id
+// is 2^32 + j, a domain disjoint from the dense ids, so all weights stay pairwise distinct.
+template <bool RANGED, typename CT>
+__device__ __forceinline__ u64 colour_id(const CT* __restrict__ colour, int j, int lo, int hi) {
+  if (RANGED) {
+    if (j >= lo && j < hi) return (u64)__ldg(colour + (j - lo));
+    return (1ull << 32) + (u64)(u32)j;
+  }
+  return (u64)__ldg(colour + j);
+}
+
 // S1+S2, default kernel: one warp owns 32 consecutive rows (or 32 entries of the active row list).
 //   * rows with at most kSmallRow entries are summed by their own lane (thread per row, no shuffles, up to kSmallRow
 //     independent gathers in flight per lane);
@@ -162,11 +179,11 @@ spmv_merge_kernel(int64_t n, int64_t m, const int64_t* __restrict__ row_ptr, con
 // sector holds 16 nodes; measured 267 vs 125 G gathers/s on the scale-27 access pattern).
 constexpr int kSmallRow = 8;
 
-template <bool WEIGHTED, typename CT>
+template <bool WEIGHTED, typename CT, bool RANGED>
 __global__ void __launch_bounds__(256)
 spmv_rows32_kernel(int64_t nrows, const int* __restrict__ rows, const int64_t* __restrict__ row_ptr,
                    const int* __restrict__ col, const u32* __restrict__ wt, const CT* __restrict__ colour, u64 key,
-                   u64* __restrict__ y, int64_t hub_threshold) {
+                   u64* __restrict__ y, int64_t hub_threshold, int lo, int hi) {
   const int lane = threadIdx.x & 31;
   const int64_t base = (((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5) << 5;
   if (base >= nrows) return;
@@ -189,7 +206,7 @@ spmv_rows32_kernel(int64_t nrows, const int* __restrict__ rows, const int64_t* _
 #pragma unroll
     for (int t = 0; t < kSmallRow; ++t) {
       if (cidx[t] >= 0) {
-        u64 v = weight_of(key, (u64)__ldg(colour + cidx[t]));
+        u64 v = weight_of(key, colour_id<RANGED>(colour, cidx[t], lo, hi));
         if (WEIGHTED) v *= (u64)__ldg(wt + a + t);
         acc += v;
       }
@@ -205,8 +222,10 @@ spmv_rows32_kernel(int64_t nrows, const int* __restrict__ rows, const int64_t* _
     for (; p + 96 < rb; p += 128) {  // four independent gathers in flight per lane
       const int c0 = ld_stream_i32(col + p), c1 = ld_stream_i32(col + p + 32), c2 = ld_stream_i32(col + p + 64),
                 c3 = ld_stream_i32(col + p + 96);
-      u64 v0 = weight_of(key, (u64)__ldg(colour + c0)), v1 = weight_of(key, (u64)__ldg(colour + c1)),
-          v2 = weight_of(key, (u64)__ldg(colour + c2)), v3 = weight_of(key, (u64)__ldg(colour + c3));
+      u64 v0 = weight_of(key, colour_id<RANGED>(colour, c0, lo, hi)),
+          v1 = weight_of(key, colour_id<RANGED>(colour, c1, lo, hi)),
+          v2 = weight_of(key, colour_id<RANGED>(colour, c2, lo, hi)),
+          v3 = weight_of(key, colour_id<RANGED>(colour, c3, lo, hi));
       if (WEIGHTED) {
         v0 *= (u64)ld_stream_u32(wt + p);
         v1 *= (u64)ld_stream_u32(wt + p + 32);
@@ -216,7 +235,7 @@ spmv_rows32_kernel(int64_t nrows, const int* __restrict__ rows, const int64_t* _
       s += (v0 + v1) + (v2 + v3);
     }
     for (; p < rb; p += 32) {
-      u64 v = weight_of(key, (u64)__ldg(colour + ld_stream_i32(col + p)));
+      u64 v = weight_of(key, colour_id<RANGED>(colour, ld_stream_i32(col + p), lo, hi));
       if (WEIGHTED) v *= (u64)ld_stream_u32(wt + p);
       s += v;
     }
@@ -244,11 +263,11 @@ __global__ void hub_collect_kernel(int64_t n, const int64_t* __restrict__ row_pt
 }
 
 // active == NULL: every hub row; else only rows whose block is still splittable (stamp[colour[row]] == live_stamp)
-template <bool WEIGHTED, typename CT>
+template <bool WEIGHTED, typename CT, bool RANGED>
 __global__ void __launch_bounds__(kHubThreads)
 spmv_hub_kernel(const int2* __restrict__ chunks, const int64_t* __restrict__ row_ptr, const int* __restrict__ col,
                 const u32* __restrict__ wt, const CT* __restrict__ colour, u64 key, u64* __restrict__ y,
-                const int* __restrict__ colour32, const int* __restrict__ stamp, int live_stamp) {
+                const int* __restrict__ colour32, const int* __restrict__ stamp, int live_stamp, int lo, int hi) {
   const int2 ch = chunks[blockIdx.x];
   const int64_t row = ch.x;
   if (stamp && stamp[colour32[row]] != live_stamp) return;
@@ -259,7 +278,7 @@ spmv_hub_kernel(const int2* __restrict__ chunks, const int64_t* __restrict__ row
   u64 acc = 0;
 #pragma unroll 4
   for (int64_t p = a + threadIdx.x; p < b; p += kHubThreads) {
-    u64 v = weight_of(key, (u64)__ldg(colour + ld_stream_i32(col + p)));
+    u64 v = weight_of(key, colour_id<RANGED>(colour, ld_stream_i32(col + p), lo, hi));
     if (WEIGHTED) v *= (u64)ld_stream_u32(wt + p);
     acc += v;
   }

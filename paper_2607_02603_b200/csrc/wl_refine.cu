@@ -15,7 +15,7 @@ namespace wl {
 thread_local int g_last_cuda_error = 0;
 thread_local int64_t g_launches = 0;
 
-static inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
+
 
 static inline u32 table_slots_for(int64_t n) {
   // power of two >= 2n, at least 1024, at most 2^31 (slot indices share a word with the winner bit)
@@ -55,7 +55,7 @@ Layout make_layout(int64_t n, int64_t m) {
   return L;
 }
 
-static inline unsigned blocks_for(int64_t count, int threads) { return (unsigned)((count + threads - 1) / threads); }
+
 
 // ---- step launchers -----------------------------------------------------------------------------------------------
 void launch_tile_search(const Layout& L, const wl_csr& g, int* tile_row, cudaStream_t st) {
@@ -74,15 +74,22 @@ struct SpmvArgs {
   int64_t num_hub_chunks;
   const int* stamp;      // hub activity test (NULL: all hubs)
   int live_stamp;
+  bool ranged;           // batched local RSC: targets outside [lo, hi) are implicit singletons
+  int lo, hi;
 };
 
+template <bool W, typename CT, bool R>
+static void launch_row_hub2(const wl_csr& g, const SpmvArgs& a, const CT* colour, u64 key, u64* y, cudaStream_t st) {
+  unsigned grid = blocks_for(a.nrows, 256);
+  ++g_launches; spmv_rows32_kernel<W, CT, R><<<grid, 256, 0, st>>>(a.nrows, a.rows, g.row_ptr, g.col_idx, g.weights, colour, key, y, kHubThreshold, a.lo, a.hi);
+  if (a.num_hub_chunks > 0) {
+    ++g_launches; spmv_hub_kernel<W, CT, R><<<(unsigned)a.num_hub_chunks, kHubThreads, 0, st>>>(a.hub_chunks, g.row_ptr, g.col_idx, g.weights, colour, key, y, a.colour, a.stamp, a.live_stamp, a.lo, a.hi);
+  }
+}
 template <bool W, typename CT>
 static void launch_row_hub(const wl_csr& g, const SpmvArgs& a, const CT* colour, u64 key, u64* y, cudaStream_t st) {
-  unsigned grid = blocks_for(a.nrows, 256);
-  ++g_launches; spmv_rows32_kernel<W, CT><<<grid, 256, 0, st>>>(a.nrows, a.rows, g.row_ptr, g.col_idx, g.weights, colour, key, y, kHubThreshold);
-  if (a.num_hub_chunks > 0) {
-    ++g_launches; spmv_hub_kernel<W, CT><<<(unsigned)a.num_hub_chunks, kHubThreads, 0, st>>>(a.hub_chunks, g.row_ptr, g.col_idx, g.weights, colour, key, y, a.colour, a.stamp, a.live_stamp);
-  }
+  if (a.ranged) launch_row_hub2<W, CT, true>(g, a, colour, key, y, st);
+  else launch_row_hub2<W, CT, false>(g, a, colour, key, y, st);
 }
 
 void launch_spmv(const Layout& L, const wl_csr& g, const SpmvArgs& a, u64 key, const int* tile_row, u64* y, bool merge,
@@ -150,28 +157,13 @@ int basic_csr_check(const wl_csr* g) {
 }
 
 // pinned host mirror of the device scalars (one per host thread)
-static u64* host_scal() {
+u64* host_scal() {
   static thread_local u64* p = nullptr;
   if (!p) {
     if (cudaHostAlloc((void**)&p, sizeof(u64) * kNumScal, cudaHostAllocDefault) != cudaSuccess) p = nullptr;
   }
   return p;
 }
-
-struct EventPool {
-  std::vector<cudaEvent_t> ev;
-  ~EventPool() {
-    for (auto e : ev) cudaEventDestroy(e);
-  }
-  cudaEvent_t get(size_t i) {
-    while (ev.size() <= i) {
-      cudaEvent_t e;
-      cudaEventCreate(&e);
-      ev.push_back(e);
-    }
-    return ev[i];
-  }
-};
 
 }  // namespace wl
 
@@ -187,23 +179,23 @@ size_t wl_refine_workspace_bytes(int64_t n, int64_t m) {
 uint64_t wl_round_key(uint64_t seed, uint64_t stream_id, uint64_t round) { return round_key(seed, stream_id, round); }
 uint64_t wl_weight(uint64_t key, uint64_t color) { return weight_of(key, color); }
 
-int wl_refine(const wl_csr* g, const int32_t* init_colors, uint64_t seed, int32_t* out_colors, wl_stats* stats,
-              const wl_options* opt, void* workspace, size_t workspace_bytes, void* cuda_stream) {
-  int rc = basic_csr_check(g);
-  if (rc) return rc;
+}  // extern "C"
+
+namespace wl {
+
+// Algorithm 1 (L106-L127) on the rows of `g` (local nodes 0..g.n-1).  ranged: batched local RSC, targets outside [lo, hi)
+// are implicit singletons and targets inside map to local node j - lo (Eq. 3).  On success the dense (non canonical)
+// colours are in the workspace's colour array and *k_out is their number.  Synchronises `st` once per round.
+int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, const wl_options* opt, bool ranged, int lo,
+                int hi, int64_t n_targets, int64_t edge_first, void* workspace, const Layout& L, cudaStream_t st,
+                CoreResult* res) {
   const int64_t n = g->n, m = g->m;
-  if (stats) std::memset(stats, 0, sizeof(*stats));
-  if (n == 0) return WL_OK;
-  if (!out_colors || !workspace) return WL_EINVAL;
-  const Layout L = make_layout(n, m);
-  if (workspace_bytes < L.bytes) return WL_ENOMEM;
-  if ((uintptr_t)workspace % 256) return WL_EINVAL;
-  cudaStream_t st = (cudaStream_t)cuda_stream;
+  int rc = WL_OK;
   const uint32_t flags = opt ? opt->flags : 0u;
   const int64_t max_rounds = (opt && opt->max_rounds > 0) ? opt->max_rounds : n + 1;
   const uint64_t stream_id = opt ? opt->stream_id : 0;
   u64* hs = host_scal();
-  if (!hs) return check_cuda(cudaGetLastError() == cudaSuccess ? cudaErrorMemoryAllocation : cudaGetLastError());
+  if (!hs) return check_cuda(cudaErrorMemoryAllocation);
 
   char* ws = (char*)workspace;
   u64* scal = (u64*)(ws + L.o_scal);
@@ -213,13 +205,9 @@ int wl_refine(const wl_csr* g, const int32_t* init_colors, uint64_t seed, int32_
   u32* tmp = (u32*)(ws + L.o_tmp);
   u64* y = (u64*)(ws + L.o_y);
   int* tile_row = (int*)(ws + L.o_tile_row);
-  int* bsum = (int*)(ws + L.o_bsum);
   Slot* table = (Slot*)(ws + L.o_table);
-
   const int64_t launches_at_entry = g_launches;
   EventPool evp;
-  cudaEvent_t ev_begin = evp.get(0), ev_end = evp.get(1);
-  cudaEventRecord(ev_begin, st);
 
   // ---- S0: setup ---------------------------------------------------------------------------------------------------
   cudaMemsetAsync(scal, 0, sizeof(u64) * kNumScal, st);
@@ -227,9 +215,9 @@ int wl_refine(const wl_csr* g, const int32_t* init_colors, uint64_t seed, int32_
   cudaMemsetAsync(stamp, 0xff, sizeof(int) * (size_t)n, st);
   u32* d_err = (u32*)(scal + kScalErr);
   if (!(flags & WL_FLAG_NO_VALIDATE)) {
-    ++g_launches; validate_rows_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, m, g->row_ptr, g->weights, d_err);
-    if (m > 0) { ++g_launches; validate_cols_kernel<<<148 * 8, 256, 0, st>>>(n, m, g->col_idx, d_err); }
-    // the merge-path search below walks row_ptr: make sure it is well formed first
+    ++g_launches; validate_rows_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, g->row_ptr, g->weights, edge_first, edge_first + m, d_err);
+    if (m > 0) { ++g_launches; validate_cols_kernel<<<148 * 8, 256, 0, st>>>(n_targets, edge_first, edge_first + m, g->col_idx, d_err); }
+    // the kernels below walk row_ptr: make sure it is well formed first
     cudaMemcpyAsync(hs + kScalErr, scal + kScalErr, sizeof(u64), cudaMemcpyDeviceToHost, st);
     rc = check_cuda(cudaStreamSynchronize(st));
     if (rc) return rc;
@@ -237,7 +225,7 @@ int wl_refine(const wl_csr* g, const int32_t* init_colors, uint64_t seed, int32_
     if (e & (kErrRowPtr | kErrCol)) return WL_EINVAL;
     if (e & kErrRowSum) return WL_ERANGE;
   }
-  const bool merge = (flags & WL_FLAG_MERGE_KERNEL) != 0;
+  const bool merge = (flags & WL_FLAG_MERGE_KERNEL) != 0 && !ranged;
   const bool prune = !merge && !(flags & WL_FLAG_NO_PRUNE);
   unsigned short* colour16 = (unsigned short*)(ws + L.o_colour16);
   int* act[2] = {(int*)(ws + L.o_act0), (int*)(ws + L.o_act1)};
@@ -248,7 +236,7 @@ int wl_refine(const wl_csr* g, const int32_t* init_colors, uint64_t seed, int32_
   // initial partition: colour 0 everywhere; a given init is densified by one relabel step keyed on the label (L94)
   int64_t k = 1;
   ++g_launches; init_labels_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, init_colors, colour, y, d_err);
-  // rep[0] = node 0; stamp[0] = 0 marks block 0 as non-singleton (n >= 2)
+  // rep[0] = node 0; stamp[0] = 0 marks block 0 as non-singleton
   cudaMemsetAsync(rep, 0, sizeof(int), st);
   cudaMemsetAsync(stamp, 0, sizeof(int), st);
   if (init_colors)
@@ -275,14 +263,14 @@ int wl_refine(const wl_csr* g, const int32_t* init_colors, uint64_t seed, int32_
     cudaEvent_t e0 = evp.get(2), e1 = evp.get(3), e2 = evp.get(4), ek0 = evp.get(5), ek1 = evp.get(6);
     cudaEventRecord(e0, st);
     bool full_spmv = false;
-    if (k == 1 && !g->weights) {
+    if (k == 1 && !g->weights && !ranged) {
       ++g_launches; spmv_uniform_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, g->row_ptr, weight_of(key, 0), y);
     } else {
       const bool narrow = !merge && k <= 65536;
       if (narrow) { ++g_launches; narrow_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, colour, colour16); }
       if (merge) cudaMemsetAsync(y, 0, sizeof(u64) * (size_t)n, st);
       SpmvArgs a{cur_list, n_active, colour, colour16, narrow, hub_chunks, num_hub_chunks,
-                 cur_list ? stamp : nullptr, (int)r - 1};
+                 cur_list ? stamp : nullptr, (int)r - 1, ranged, lo, hi};
       cudaEventRecord(ek0, st);
       launch_spmv(L, *g, a, key, tile_row, y, merge, st);
       cudaEventRecord(ek1, st);
@@ -335,8 +323,8 @@ int wl_refine(const wl_csr* g, const int32_t* init_colors, uint64_t seed, int32_
         active_edges = m;
       }
       if (n_active == 0) {
-        // every block is a singleton: the next round cannot change anything and only confirms (same trajectory as
-        // the un-pruned algorithm)
+        // every block is a singleton (or can never split again): the next round cannot change anything and only
+        // confirms (same trajectory as the un-pruned algorithm)
         if (r + 1 <= max_rounds) {
           rounds = (int32_t)(r + 1);
           if (opt && opt->round_colors && r + 1 <= opt->round_colors_cap) opt->round_colors[r] = k;
@@ -346,13 +334,51 @@ int wl_refine(const wl_csr* g, const int32_t* init_colors, uint64_t seed, int32_
       }
     }
   }
+  res->k = k;
+  res->rounds = rounds;
+  res->edges_streamed = edges_streamed;
+  res->spmv_alg_bytes = spmv_alg_bytes;
+  res->ms_spmv = ms_spmv;
+  res->ms_relabel = ms_relabel;
+  res->ms_spmv_kernel = ms_spmv_kernel;
+  res->spmv_launches = spmv_launches;
+  res->kernel_launches = (int32_t)(g_launches - launches_at_entry);
+  res->colour = colour;
+  return converged ? WL_OK : WL_EMAXROUNDS;
+}
 
+}  // namespace wl
+
+extern "C" {
+
+int wl_refine(const wl_csr* g, const int32_t* init_colors, uint64_t seed, int32_t* out_colors, wl_stats* stats,
+              const wl_options* opt, void* workspace, size_t workspace_bytes, void* cuda_stream) {
+  int rc = basic_csr_check(g);
+  if (rc) return rc;
+  const int64_t n = g->n, m = g->m;
+  if (stats) std::memset(stats, 0, sizeof(*stats));
+  if (n == 0) return WL_OK;
+  if (!out_colors || !workspace) return WL_EINVAL;
+  const Layout L = make_layout(n, m);
+  if (workspace_bytes < L.bytes) return WL_ENOMEM;
+  if ((uintptr_t)workspace % 256) return WL_EINVAL;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const uint32_t flags = opt ? opt->flags : 0u;
+  const int64_t launches_at_entry = g_launches;
+  EventPool evp;
+  cudaEvent_t ev_begin = evp.get(0), ev_end = evp.get(1);
+  cudaEventRecord(ev_begin, st);
+  CoreResult cr{};
+  const int core_rc = refine_core(g, init_colors, seed, opt, /*ranged=*/false, 0, 0, n, /*edge_first=*/0, workspace, L, st, &cr);
+  if (core_rc != WL_OK && core_rc != WL_EMAXROUNDS) return core_rc;
+  char* ws = (char*)workspace;
   // ---- S6: canonical ids ---------------------------------------------------------------------------------------------
   if (flags & WL_FLAG_NO_CANONICAL) {
-    cudaMemcpyAsync(out_colors, colour, sizeof(int) * (size_t)n, cudaMemcpyDeviceToDevice, st);
+    cudaMemcpyAsync(out_colors, cr.colour, sizeof(int) * (size_t)n, cudaMemcpyDeviceToDevice, st);
   } else {
     // scratch: tmp -> first, rep -> canon_of_first (both dead now)
-    launch_canonical(L, n, colour, out_colors, (int*)tmp, rep, bsum, scal + kScalCanon, st);
+    launch_canonical(L, n, cr.colour, out_colors, (int*)(ws + L.o_tmp), (int*)(ws + L.o_rep), (int*)(ws + L.o_bsum),
+                     (u64*)(ws + L.o_scal) + kScalCanon, st);
   }
   cudaEventRecord(ev_end, st);
   rc = check_cuda(cudaStreamSynchronize(st));
@@ -362,18 +388,18 @@ int wl_refine(const wl_csr* g, const int32_t* init_colors, uint64_t seed, int32_
   if (stats) {
     float t = 0;
     cudaEventElapsedTime(&t, ev_begin, ev_end);
-    stats->rounds = rounds;
-    stats->num_colors = k;
-    stats->edges_streamed = edges_streamed;
+    stats->rounds = cr.rounds;
+    stats->num_colors = cr.k;
+    stats->edges_streamed = cr.edges_streamed;
     stats->ms_total = t;
-    stats->ms_spmv = ms_spmv;
-    stats->ms_relabel = ms_relabel;
-    stats->ms_spmv_kernel = ms_spmv_kernel;
-    stats->spmv_launches = spmv_launches;
-    stats->spmv_alg_bytes = spmv_alg_bytes;
+    stats->ms_spmv = cr.ms_spmv;
+    stats->ms_relabel = cr.ms_relabel;
+    stats->ms_spmv_kernel = cr.ms_spmv_kernel;
+    stats->spmv_launches = cr.spmv_launches;
+    stats->spmv_alg_bytes = cr.spmv_alg_bytes;
     stats->kernel_launches = (int32_t)(g_launches - launches_at_entry);
   }
-  return converged ? WL_OK : WL_EMAXROUNDS;
+  return core_rc;
 }
 
 int wl_refine_host(const wl_csr* g, const int32_t* init_colors, uint64_t seed, int32_t* out_colors, wl_stats* stats,
@@ -459,7 +485,8 @@ int wl_spmv_round(const wl_csr* g, const int32_t* colors, uint64_t key, uint64_t
   u64* scal = (u64*)(ws + L.o_scal);
   const bool merge = (flags & WL_FLAG_MERGE_KERNEL) != 0;
   const bool narrow = !merge && (flags & WL_FLAG_NARROW_COLORS) != 0;
-  SpmvArgs a{nullptr, g->n, colors, (unsigned short*)(ws + L.o_colour16), narrow, (int2*)(ws + L.o_hub), 0, nullptr, 0};
+  SpmvArgs a{nullptr, g->n, colors, (unsigned short*)(ws + L.o_colour16), narrow, (int2*)(ws + L.o_hub), 0, nullptr, 0,
+             false, 0, 0};
   if (merge) {
     launch_tile_search(L, *g, tile_row, st);
     cudaMemsetAsync(y, 0, sizeof(u64) * (size_t)g->n, st);
