@@ -277,6 +277,85 @@ def wl_canonicalize(colors: torch.Tensor, *, workspace=None):
     return out, kk.value
 
 
+def wl_inner_labels(n: int, row_ptr: torch.Tensor, edge_batch: torch.Tensor, sink_batch: torch.Tensor) -> torch.Tensor:
+    """B2: inner-node labels of Def. 5 (-1 = boundary) for an arbitrary edge partition given per CSR edge slot."""
+    L = lib()
+    dev = row_ptr.device
+    _check(row_ptr, torch.int64, "cuda", "row_ptr", n + 1)
+    _check(edge_batch, torch.int32, "cuda", "edge_batch")
+    _check(sink_batch, torch.int32, "cuda", "sink_batch", n)
+    label = torch.empty(n, dtype=torch.int32, device=dev)
+    with torch.cuda.device(dev):
+        rc = L.wl_inner_labels(n, _ptr(row_ptr), _ptr(edge_batch), _ptr(sink_batch), _ptr(label), _stream_ptr(dev))
+    if rc != WL_OK:
+        raise WlError(rc, "wl_inner_labels")
+    return label
+
+
+def wl_quotient_workspace_bytes(n: int, m: int) -> int:
+    return int(lib().wl_quotient_workspace_bytes(n, m))
+
+
+def wl_quotient(n, row_ptr, col_idx, weights, colors: torch.Tensor, k: int):
+    """B6: quotient graph of Def. 4 for canonical colours.  -> (q_row_ptr int64[k+1], q_col int32[q_m], q_weights int64[q_m])
+    with every (block, target block) pair stored once; order inside a row is unspecified."""
+    L = lib()
+    dev = row_ptr.device
+    g, w = _make_csr(n, row_ptr, col_idx, weights, "cuda")
+    _check(colors, torch.int32, "cuda", "colors", n)
+    m = col_idx.numel()
+    q_rp = torch.zeros(k + 1, dtype=torch.int64, device=dev)
+    q_col = torch.empty(max(m, 1), dtype=torch.int32, device=dev)
+    q_wt = torch.empty(max(m, 1), dtype=torch.int32, device=dev)
+    ws = torch.empty(max(wl_quotient_workspace_bytes(n, m), 256), dtype=torch.uint8, device=dev)
+    qm = C.c_int64(0)
+    with torch.cuda.device(dev):
+        rc = L.wl_quotient(C.byref(g), _ptr(colors), k, _ptr(q_rp), _ptr(q_col), _ptr(q_wt), m, C.byref(qm), _ptr(ws),
+                           ws.numel(), _stream_ptr(dev))
+    if rc != WL_OK:
+        raise WlError(rc, "wl_quotient")
+    return q_rp, q_col[: qm.value], q_wt[: qm.value].to(torch.int64) & 0xFFFFFFFF
+
+
+def wl_refine_batched(n: int, row_ptr: torch.Tensor, col_idx: torch.Tensor, weights: Optional[torch.Tensor] = None, *,
+                      max_batch_edges: int, cuts=None, seed: int = 0, device_cap_bytes: int = 0, flags: int = 0,
+                      max_outer_iters: int = 0, out: Optional[torch.Tensor] = None, device=None,
+                      allow_limit: bool = False) -> RefineResult:
+    """Algorithm 2 over a HOST-resident CSR (pinned recommended).  cuts (optional, increasing edge positions from 0 to m)
+    gives the edge partition of the first outer iteration as consecutive CSR slices; otherwise the library cuts by
+    max_batch_edges.  Returns canonical colours on the original nodes (host int32[n])."""
+    L = lib()
+    if not torch.cuda.is_available():
+        raise RuntimeError("wl_refine_batched needs a CUDA device (no CPU fallback)")
+    dev = torch.device("cuda", torch.cuda.current_device()) if device is None else torch.device(device)
+    g, w = _make_csr(n, row_ptr, col_idx, weights, "cpu")
+    if out is None:
+        out = torch.empty(n, dtype=torch.int32)
+    _check(out, torch.int32, "cpu", "out", n)
+    opt = wl_options(flags, 0, 0, None, 0, max_outer_iters)
+    st = wl_stats()
+    nb = 0
+    batches = None
+    if cuts is not None:
+        cuts = [int(c) for c in cuts]
+        nb = len(cuts) - 1
+        arr = (wl_edge_batch * nb)()
+        for k in range(nb):
+            arr[k].edge_begin = cuts[k]
+            arr[k].num_edges = cuts[k + 1] - cuts[k]
+            arr[k].row_ptr = row_ptr.data_ptr()
+            arr[k].col_idx = col_idx.data_ptr() + 4 * cuts[k]
+            arr[k].weights = None if w is None else w.data_ptr() + 4 * cuts[k]
+            arr[k].src = None
+        batches = arr
+    with torch.cuda.device(dev):
+        rc = L.wl_refine_batched(n, nb, batches, C.byref(g) if cuts is None else None, seed, device_cap_bytes,
+                                 max_batch_edges, _ptr(out), C.byref(st), C.byref(opt), _stream_ptr(dev))
+    if rc != WL_OK and not (allow_limit and rc == WL_EMAXROUNDS):
+        raise WlError(rc, "wl_refine_batched")
+    return RefineResult(out, st.num_colors, st.rounds, [], _stats_dict(st), rc)
+
+
 def wl_strerror(code: int) -> str:
     return lib().wl_strerror(code).decode()
 

@@ -1,16 +1,742 @@
-// Batched path (Algorithm 2): placeholder translation unit, filled in by the batched engine.
+// Batched path: Algorithm 2 (RBSC) over host-resident edge batches, and its step-level pieces.
+//
+// SURVEY.md §8(a) rows and where they are:
+//   B1 stream      upload_batch(): pinned/pageable host -> two device buffers on a copy stream, the next batch is
+//                  uploaded while the current one is refined (event-ordered double buffering)
+//   B2 inner mask  row-aligned batches (the library's own partition, Q13): V_k is a contiguous node range computed on the
+//                  host from the cuts (inner_range()); arbitrary partitions: inner_labels_kernel (wl_inner_labels)
+//   B3 local init  implicit: targets outside V_k get the id 2^32 + j inside the SpMV kernels (colour_id<RANGED>)
+//   B4 local RSC   refine_core(ranged = true) on the rows of V_k only
+//   B5 merge       merge_kernel: global id = running offset + local id; boundary nodes get fresh ids (Eq. 4)
+//   B6 quotient    quot_insert_kernel / quot_emit_kernel: representative rows mapped through the block map and merged in
+//                  an exact-key hash table (key = (block, target block), value = summed weight), Def. 4 / Eq. 1
+//   B7 outer loop  wl_refine_batched(): re-batch the quotient, stop at N_b = 1 or |V| unchanged (L200), compose block maps
+//   B8 verify      lives in the test harness (oracle_is_stable on the original graph)
+// COO-form (arbitrary) first partitions are not accepted by wl_refine_batched yet (WL_EINVAL); wl_inner_labels covers
+// their Def. 5 mask.
+#include <algorithm>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <vector>
+
 #include "wl_host.h"
+
+namespace wl {
+
+// ---------------------------------------------------------------------------------------------------------------------
+// kernels
+// ---------------------------------------------------------------------------------------------------------------------
+
+// Def. 5 (L139-L145) by the method of L463: a node is inner to batch k iff all its out-edges carry label k.
+__global__ void inner_labels_kernel(int64_t n, const int64_t* __restrict__ row_ptr, const int* __restrict__ edge_batch,
+                                    const int* __restrict__ sink_batch, int* __restrict__ label) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const int64_t a = row_ptr[i], b = row_ptr[i + 1];
+  if (a == b) {
+    label[i] = sink_batch[i];
+    return;
+  }
+  const int k = edge_batch[a];
+  bool inner = true;
+  for (int64_t p = a + 1; p < b; ++p) inner &= (edge_batch[p] == k);
+  label[i] = inner ? k : -1;
+}
+
+// Eq. 4: blocks of H_k inside V_k enter the global partition with ids base + local id
+__global__ void merge_kernel(int64_t n_local, const int* __restrict__ local_colour, int base, int* __restrict__ H) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n_local) H[i] = base + local_colour[i];
+}
+
+__global__ void iota_kernel(int64_t n, int* __restrict__ a) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) a[i] = (int)i;
+}
+
+__global__ void compose_kernel(int64_t n0, int* __restrict__ map0, const int* __restrict__ Hc) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n0) map0[i] = Hc[map0[i]];
+}
+
+// rep_of_block[b] = first node of canonical block b (colours canonical => ids ordered by first node)
+__global__ void block_rep_kernel(int64_t n, const int* __restrict__ canon, int* __restrict__ rep_of_block) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const int b = canon[i];
+  if (rep_of_block[b] > (int)i) atomicMin(rep_of_block + b, (int)i);
+}
+
+// lower_bound of each query in the increasing array rep_of_block[0..k): number of blocks whose first node is < x
+__global__ void rep_lower_bound_kernel(const int* __restrict__ rep_of_block, int64_t k, const int64_t* __restrict__ queries,
+                                       int nq, int64_t* __restrict__ out) {
+  int q = blockIdx.x * blockDim.x + threadIdx.x;
+  if (q >= nq) return;
+  const int64_t x = queries[q];
+  int64_t lo = 0, hi = k;
+  while (lo < hi) {
+    int64_t mid = (lo + hi) >> 1;
+    if ((int64_t)rep_of_block[mid] < x) lo = mid + 1;
+    else hi = mid;
+  }
+  out[q] = lo;
+}
+
+// Quotient, step 1: every entry (i_B, j) of a representative row becomes key (B, H(j)); equal keys meet in one slot whose
+// value accumulates the weights (a'_{B,B'} = sum_{l in B'} a_{i_B,l}, Eq. 1).  Slot = {key + 1 : 64 | weight sum : 64},
+// empty = 0.  The claimer of a slot counts one distinct target for block B.  One warp per row.
+__global__ void __launch_bounds__(256)
+quot_insert_kernel(int64_t row_base, int64_t n_rows, const int64_t* __restrict__ row_ptr, const int* __restrict__ col,
+                   const u32* __restrict__ wt, const int* __restrict__ Hc, const int* __restrict__ rep_of_block,
+                   u64* __restrict__ table, u64 table_mask, int* __restrict__ cnt) {
+  const int lane = threadIdx.x & 31;
+  const int64_t w = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  if (w >= n_rows) return;
+  const int64_t i = row_base + w;
+  const int b = Hc[i];
+  if (rep_of_block[b] != (int)i) return;
+  const int64_t a = row_ptr[w], e = row_ptr[w + 1];
+  for (int64_t p = a + lane; p < e; p += 32) {
+    const u64 key = (((u64)(u32)b << 32) | (u64)(u32)Hc[col[p]]) + 1;
+    const u64 weight = wt ? (u64)wt[p] : 1ull;
+    u64 slot = slot_hash((u32)b, key) & table_mask;
+    while (true) {
+      u64 cur = table[2 * slot];
+      if (cur == 0) {
+        cur = atomicCAS(table + 2 * slot, 0ull, key);
+        if (cur == 0) {
+          atomicAdd(cnt + b, 1);
+          cur = key;
+        }
+      }
+      if (cur == key) {
+        atomicAdd(table + 2 * slot + 1, weight);
+        break;
+      }
+      slot = (slot + 1) & table_mask;
+    }
+  }
+}
+
+// Quotient, step 2: every occupied slot is one entry of A'; rows fill from q_row_ptr with an atomic cursor (order inside a
+// row is unspecified); the slot is emptied for the next batch.
+// Only blocks b_lo <= B < b_hi are emitted (a representative row that continues in the next batch stays in the table).
+__global__ void quot_emit_kernel(u64* __restrict__ table, u64 table_slots, const int64_t* __restrict__ q_row_ptr,
+                                 int64_t out_base, int* __restrict__ cursor, int* __restrict__ q_col,
+                                 u32* __restrict__ q_wt, int b_lo, int b_hi) {
+  int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (s >= (int64_t)table_slots) return;
+  const u64 key1 = table[2 * s];
+  if (key1 == 0) return;
+  const u64 key = key1 - 1;
+  const int b = (int)(key >> 32), t = (int)(key & 0xffffffffu);
+  if (b < b_lo || b >= b_hi) return;
+  const u64 sum = table[2 * s + 1];
+  const int64_t pos = q_row_ptr[b] - out_base + atomicAdd(cursor + b, 1);
+  q_col[pos] = t;
+  q_wt[pos] = (u32)sum;
+  table[2 * s] = 0;
+  table[2 * s + 1] = 0;
+}
+
+// exclusive scan int32 counts -> int64 offsets (3 kernels)
+constexpr int kScanT = 256, kScanI = 8, kScanC = kScanT * kScanI;
+
+__global__ void __launch_bounds__(kScanT)
+scan32_sum_kernel(const int* __restrict__ in, int64_t n, u64* __restrict__ bsum) {
+  const int64_t base = (int64_t)blockIdx.x * kScanC;
+  u64 s = 0;
+#pragma unroll
+  for (int k = 0; k < kScanI; ++k) {
+    int64_t i = base + threadIdx.x + k * kScanT;
+    if (i < n) s += (u64)(u32)in[i];
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+  __shared__ u64 sh[kScanT / 32];
+  if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = s;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    u64 t = 0;
+    for (int w = 0; w < kScanT / 32; ++w) t += sh[w];
+    bsum[blockIdx.x] = t;
+  }
+}
+
+__global__ void scan64_serial_kernel(u64* __restrict__ bsum, int64_t nb, u64* __restrict__ total) {
+  // nb is n / 2048: a single thread is enough up to billions of nodes (<= 1M block sums)
+  if (blockIdx.x == 0 && threadIdx.x == 0) {
+    u64 run = 0;
+    for (int64_t i = 0; i < nb; ++i) {
+      u64 t = bsum[i];
+      bsum[i] = run;
+      run += t;
+    }
+    *total = run;
+  }
+}
+
+__global__ void __launch_bounds__(kScanT)
+scan32_apply_kernel(const int* __restrict__ in, int64_t n, const u64* __restrict__ bsum, int64_t base_off,
+                    int64_t* __restrict__ out) {
+  const int64_t base = (int64_t)blockIdx.x * kScanC + (int64_t)threadIdx.x * kScanI;
+  u32 v[kScanI];
+  u64 s = 0;
+#pragma unroll
+  for (int k = 0; k < kScanI; ++k) {
+    v[k] = base + k < n ? (u32)in[base + k] : 0u;
+    s += v[k];
+  }
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  u64 x = s;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    u64 t = __shfl_up_sync(0xffffffffu, x, o);
+    if (lane >= o) x += t;
+  }
+  __shared__ u64 sw[kScanT / 32];
+  if (lane == 31) sw[wid] = x;
+  __syncthreads();
+  u64 woff = 0;
+  for (int w = 0; w < wid; ++w) woff += sw[w];
+  u64 r = (u64)base_off + bsum[blockIdx.x] + woff + x - s;
+#pragma unroll
+  for (int k = 0; k < kScanI; ++k) {
+    if (base + k < n) out[base + k] = (int64_t)r;
+    r += v[k];
+    if (base + k == n - 1) out[n] = (int64_t)r;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
+// host helpers
+// ---------------------------------------------------------------------------------------------------------------------
+struct DevBuf {
+  void* p = nullptr;
+  size_t bytes = 0;
+  ~DevBuf() {
+    if (p) cudaFree(p);
+  }
+  int alloc(size_t b, size_t* used, size_t cap) {
+    bytes = b ? b : 256;
+    if (cap && *used + bytes > cap) return WL_ENOMEM;
+    if (cudaMalloc(&p, bytes) != cudaSuccess) {
+      cudaGetLastError();
+      p = nullptr;
+      return WL_ENOMEM;
+    }
+    *used += bytes;
+    return WL_OK;
+  }
+  template <typename T>
+  T* as() const { return (T*)p; }
+};
+
+// exclusive scan of cnt[0..n) into out[0..n] starting at base_off (device arrays); bsum: ceil(n / kScanC) + 1 u64
+static void launch_scan32(const int* cnt, int64_t n, int64_t base_off, int64_t* out, u64* bsum, u64* total,
+                          cudaStream_t st) {
+  if (n == 0) return;
+  const int64_t nb = (n + kScanC - 1) / kScanC;
+  ++g_launches; scan32_sum_kernel<<<(unsigned)nb, kScanT, 0, st>>>(cnt, n, bsum);
+  ++g_launches; scan64_serial_kernel<<<1, 32, 0, st>>>(bsum, nb, total);
+  ++g_launches; scan32_apply_kernel<<<(unsigned)nb, kScanT, 0, st>>>(cnt, n, bsum, base_off, out);
+}
+
+static u64 quot_table_slots(int64_t entries) {
+  u64 s = 1024;
+  while (s < 2ull * (u64)entries) s <<= 1;
+  return s;
+}
+
+// Greedy cuts of the CSR edge array (Q13): consecutive runs of at most cap entries, cut on the largest row boundary that
+// fits, inside the row only when the row alone exceeds the cap.
+static void greedy_cuts(int64_t n, const int64_t* rp, int64_t cap, std::vector<int64_t>& cuts) {
+  const int64_t m = rp[n];
+  cuts.assign(1, 0);
+  while (cuts.back() < m) {
+    const int64_t start = cuts.back(), limit = start + cap;
+    if (limit >= m) {
+      cuts.push_back(m);
+      break;
+    }
+    // largest r with rp[r] <= limit
+    const int64_t r = (std::upper_bound(rp, rp + n + 1, limit) - rp) - 1;
+    const int64_t b = rp[r];
+    cuts.push_back(b > start ? b : limit);
+  }
+  if (cuts.size() == 1) cuts.push_back(m);  // m == 0: one empty batch
+}
+
+// V_k for the batch owning edge positions [c0, c1) (Q9, Q13): nodes whose row position lies in [c0, c1), minus the last
+// one if its row crosses c1; the last batch also owns the trailing edgeless nodes.
+static void inner_range(int64_t n, const int64_t* rp, int64_t c0, int64_t c1, bool last, int64_t* r0, int64_t* r1) {
+  int64_t a = std::lower_bound(rp, rp + n, c0) - rp;  // first node with rp[i] >= c0 (among 0..n-1)
+  int64_t b = last ? n : (std::lower_bound(rp, rp + n, c1) - rp);
+  if (b > a && rp[b] > c1) --b;  // rows are [rp[i], rp[i+1]): node b-1 crosses the cut
+  if (b < a) b = a;
+  *r0 = a;
+  *r1 = b;
+}
+
+}  // namespace wl
+
+using namespace wl;
 
 extern "C" {
 
-int wl_refine_batched(int64_t, int32_t, const wl_edge_batch*, const wl_csr*, uint64_t, size_t, int64_t, int32_t*,
-                      wl_stats*, const wl_options*, void*) {
-  return WL_EINVAL;
+int wl_inner_labels(int64_t n, const int64_t* row_ptr, const int32_t* edge_batch, const int32_t* sink_batch,
+                    int32_t* label, void* cuda_stream) {
+  if (n < 0) return WL_EINVAL;
+  if (n == 0) return WL_OK;
+  if (!row_ptr || !sink_batch || !label) return WL_EINVAL;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  ++g_launches; inner_labels_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, row_ptr, edge_batch, sink_batch, label);
+  int rc = check_cuda(cudaStreamSynchronize(st));
+  if (rc) return rc;
+  return check_cuda(cudaGetLastError());
 }
-int wl_inner_labels(int64_t, const int64_t*, const int32_t*, const int32_t*, int32_t*, void*) { return WL_EINVAL; }
-int wl_quotient(const wl_csr*, const int32_t*, int64_t, int64_t*, int32_t*, uint32_t*, int64_t, int64_t*, void*, size_t,
-                void*) {
-  return WL_EINVAL;
+
+size_t wl_quotient_workspace_bytes(int64_t n, int64_t m) {
+  if (n < 0 || m < 0 || n > kMaxNodes) return 0;
+  size_t off = 0;
+  off += align_up(sizeof(u64) * 2 * quot_table_slots(m));
+  off += align_up(sizeof(int) * (size_t)n) * 3;  // rep_of_block, cnt, cursor (k <= n)
+  off += align_up(sizeof(u64) * (size_t)((n + kScanC - 1) / kScanC + 2));
+  off += 256;
+  return off;
 }
-size_t wl_quotient_workspace_bytes(int64_t, int64_t) { return 0; }
+
+int wl_quotient(const wl_csr* g, const int32_t* colors, int64_t k, int64_t* q_row_ptr, int32_t* q_col, uint32_t* q_weights,
+                int64_t q_cap, int64_t* q_m, void* workspace, size_t workspace_bytes, void* cuda_stream) {
+  int rc = basic_csr_check(g);
+  if (rc) return rc;
+  const int64_t n = g->n, m = g->m;
+  if (k < 0 || k > n || !q_m) return WL_EINVAL;
+  *q_m = 0;
+  if (n == 0) return WL_OK;
+  if (!colors || !q_row_ptr || !workspace || (q_cap > 0 && (!q_col || !q_weights))) return WL_EINVAL;
+  if (workspace_bytes < wl_quotient_workspace_bytes(n, m)) return WL_ENOMEM;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  char* ws = (char*)workspace;
+  size_t off = 0;
+  const u64 slots = quot_table_slots(m);
+  u64* table = (u64*)(ws + off);
+  off += align_up(sizeof(u64) * 2 * slots);
+  int* rep_of_block = (int*)(ws + off);
+  off += align_up(sizeof(int) * (size_t)n);
+  int* cnt = (int*)(ws + off);
+  off += align_up(sizeof(int) * (size_t)n);
+  int* cursor = (int*)(ws + off);
+  off += align_up(sizeof(int) * (size_t)n);
+  u64* bsum = (u64*)(ws + off);
+  off += align_up(sizeof(u64) * (size_t)((n + kScanC - 1) / kScanC + 2));
+  u64* total = (u64*)(ws + off);
+  cudaMemsetAsync(table, 0, sizeof(u64) * 2 * slots, st);
+  cudaMemsetAsync(rep_of_block, 0x7f, sizeof(int) * (size_t)k, st);
+  cudaMemsetAsync(cnt, 0, sizeof(int) * (size_t)k, st);
+  cudaMemsetAsync(cursor, 0, sizeof(int) * (size_t)k, st);
+  ++g_launches; block_rep_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, colors, rep_of_block);
+  ++g_launches; quot_insert_kernel<<<blocks_for(n * 32, 256), 256, 0, st>>>(0, n, g->row_ptr, g->col_idx, g->weights, colors, rep_of_block, table, slots - 1, cnt);
+  launch_scan32(cnt, k, 0, q_row_ptr, bsum, total, st);
+  u64 h_total = 0;
+  cudaMemcpyAsync(&h_total, total, sizeof(u64), cudaMemcpyDeviceToHost, st);
+  rc = check_cuda(cudaStreamSynchronize(st));
+  if (rc) return rc;
+  if (k == 0) h_total = 0;
+  *q_m = (int64_t)h_total;
+  if ((int64_t)h_total > q_cap) return WL_ENOMEM;
+  ++g_launches; quot_emit_kernel<<<blocks_for((int64_t)slots, 256), 256, 0, st>>>(table, slots, q_row_ptr, 0, cursor, q_col, q_weights, 0, (int)k);
+  rc = check_cuda(cudaStreamSynchronize(st));
+  if (rc) return rc;
+  return check_cuda(cudaGetLastError());
 }
+
+// ---------------------------------------------------------------------------------------------------------------------
+// Algorithm 2
+// ---------------------------------------------------------------------------------------------------------------------
+int wl_refine_batched(int64_t n, int32_t num_batches, const wl_edge_batch* batches, const wl_csr* whole, uint64_t seed,
+                      size_t device_cap_bytes, int64_t max_batch_edges, int32_t* out_colors, wl_stats* stats,
+                      const wl_options* opt, void* cuda_stream) {
+  if (stats) std::memset(stats, 0, sizeof(*stats));
+  if (n < 0 || num_batches < 0 || max_batch_edges <= 0) return WL_EINVAL;
+  if (n > kMaxNodes) return WL_ERANGE;
+  if (n == 0) return WL_OK;
+  if (!out_colors) return WL_EINVAL;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const uint32_t flags = opt ? opt->flags : 0u;
+  const int max_outer = (opt && opt->max_outer_iters > 0) ? opt->max_outer_iters : (1 << 30);
+
+  // ---- the host-resident graph of the current outer iteration ------------------------------------------------------
+  const int64_t* rp = nullptr;
+  const int* col = nullptr;
+  const u32* wt = nullptr;
+  std::vector<int64_t> cuts;
+  if (num_batches > 0) {
+    if (!batches) return WL_EINVAL;
+    // CSR-slice form only: all batches share one row_ptr and tile the edge array consecutively
+    rp = batches[0].row_ptr;
+    if (!rp) return WL_EINVAL;
+    int64_t pos = 0;
+    cuts.push_back(0);
+    for (int k = 0; k < num_batches; ++k) {
+      const wl_edge_batch& b = batches[k];
+      if (b.src) return WL_EINVAL;  // COO-form partitions: not supported yet
+      if (b.row_ptr != rp || b.edge_begin != pos || b.num_edges < 0) return WL_EINVAL;
+      if (b.num_edges > 0 && !b.col_idx) return WL_EINVAL;
+      pos += b.num_edges;
+      cuts.push_back(pos);
+    }
+    if (pos != rp[n]) return WL_EINVAL;
+  } else {
+    int rc = basic_csr_check(whole);
+    if (rc) return rc;
+    if (whole->n != n) return WL_EINVAL;
+    rp = whole->row_ptr;
+    col = whole->col_idx;
+    wt = whole->weights;
+    if (rp[0] != 0 || rp[n] != whole->m) return WL_EINVAL;
+    greedy_cuts(n, rp, max_batch_edges, cuts);
+  }
+  // per-batch host pointers of iteration 1 (slices may live in separate allocations)
+  auto batch_col = [&](int k) -> const int* { return num_batches > 0 ? batches[k].col_idx : col + cuts[k]; };
+  auto batch_wt = [&](int k) -> const u32* {
+    return num_batches > 0 ? batches[k].weights : (wt ? wt + cuts[k] : nullptr);
+  };
+  bool weighted = num_batches > 0 ? (batches[0].weights != nullptr) : (wt != nullptr);
+
+  u64* hs = host_scal();
+  if (!hs) return WL_ECUDA;
+  cudaStream_t copy_st;
+  if (cudaStreamCreateWithFlags(&copy_st, cudaStreamNonBlocking) != cudaSuccess) return check_cuda(cudaGetLastError());
+  cudaEvent_t ev_begin, ev_end, ev_up[2];
+  cudaEventCreate(&ev_begin);
+  cudaEventCreate(&ev_end);
+  cudaEventCreateWithFlags(&ev_up[0], cudaEventDisableTiming);
+  cudaEventCreateWithFlags(&ev_up[1], cudaEventDisableTiming);
+  cudaEventRecord(ev_begin, st);
+  auto cleanup = [&]() {
+    cudaEventDestroy(ev_begin);
+    cudaEventDestroy(ev_end);
+    cudaEventDestroy(ev_up[0]);
+    cudaEventDestroy(ev_up[1]);
+    cudaStreamDestroy(copy_st);
+  };
+
+  const int64_t n0 = n;
+  size_t used = 0;
+  DevBuf d_map0;  // original node -> node of the current graph (identity in iteration 1: left unallocated until needed)
+  bool map0_identity = true;
+  // quotient graphs of later iterations live in these host vectors
+  std::vector<int64_t> q_rp[2];
+  std::vector<int> q_col[2];
+  std::vector<u32> q_wt[2];
+  int qsel = 0;
+
+  int64_t n_t = n;
+  int outer = 0;
+  int64_t nb_last = 0, boundary_first = 0, edges_streamed = 0, bytes_h2d = 0, bytes_d2h = 0, K_final = 0;
+  double ms_spmv = 0, ms_relabel = 0, ms_spmv_kernel = 0;
+  int64_t spmv_alg_bytes = 0;
+  int32_t spmv_launches = 0;
+  const int64_t launches_at_entry = g_launches;
+  int rc = WL_OK;
+  bool hit_limit = false;
+
+  while (true) {
+    ++outer;
+    const int nb = (int)cuts.size() - 1;
+    const int64_t m_t = rp[n_t];
+    // inner ranges and sizes
+    std::vector<int64_t> r0(nb), r1(nb);
+    int64_t max_rows = 1, max_edges = 1;
+    for (int k = 0; k < nb; ++k) {
+      inner_range(n_t, rp, cuts[k], cuts[k + 1], k == nb - 1, &r0[k], &r1[k]);
+      max_rows = std::max(max_rows, r1[k] - r0[k]);
+      max_edges = std::max(max_edges, cuts[k + 1] - cuts[k]);
+    }
+    size_t ws_bytes = 0;
+    for (int k = 0; k < nb; ++k)
+      ws_bytes = std::max(ws_bytes, make_layout(r1[k] - r0[k], rp[r1[k]] - rp[r0[k]]).bytes);
+
+    // ---- device memory of this outer iteration ---------------------------------------------------------------------
+    size_t used_iter = used;
+    DevBuf d_H, d_Hc, d_first, d_cof, d_bsum, d_ws, d_col[2], d_wt[2], d_rp[2], d_rep, d_cnt, d_cursor, d_qrp, d_qtab,
+        d_qcol, d_qwt, d_sbsum, d_misc;
+    const int64_t nscan = (n_t + kCanonChunk - 1) / kCanonChunk;
+#define WL_ALLOC(buf, bytes)                                   \
+  if ((rc = buf.alloc((bytes), &used_iter, device_cap_bytes))) \
+    break;
+    WL_ALLOC(d_H, sizeof(int) * (size_t)n_t);
+    WL_ALLOC(d_Hc, sizeof(int) * (size_t)n_t);
+    WL_ALLOC(d_first, sizeof(int) * (size_t)n_t);
+    WL_ALLOC(d_cof, sizeof(int) * (size_t)n_t);
+    WL_ALLOC(d_bsum, sizeof(int) * (size_t)(nscan + 1));
+    WL_ALLOC(d_ws, ws_bytes);
+    for (int b = 0; b < 2; ++b) {
+      WL_ALLOC(d_col[b], sizeof(int) * (size_t)max_edges);
+      if (weighted) WL_ALLOC(d_wt[b], sizeof(u32) * (size_t)max_edges);
+      WL_ALLOC(d_rp[b], sizeof(int64_t) * (size_t)(max_rows + 2));
+    }
+    WL_ALLOC(d_misc, 4096);
+    if (rc) break;
+
+    auto upload_batch = [&](int k, int buf, bool rows_all) {
+      // rows_all: the quotient pass needs every row that starts inside the batch's node range (incl. a crossing one)
+      const int64_t c0 = cuts[k], c1 = cuts[k + 1];
+      const int* hc = (outer == 1) ? batch_col(k) : q_col[qsel].data() + c0;
+      const u32* hw = (outer == 1) ? batch_wt(k) : q_wt[qsel].data() + c0;
+      if (c1 > c0) {
+        cudaMemcpyAsync(d_col[buf].p, hc, sizeof(int) * (size_t)(c1 - c0), cudaMemcpyHostToDevice, copy_st);
+        bytes_h2d += sizeof(int) * (c1 - c0);
+        if (weighted) {
+          cudaMemcpyAsync(d_wt[buf].p, hw, sizeof(u32) * (size_t)(c1 - c0), cudaMemcpyHostToDevice, copy_st);
+          bytes_h2d += sizeof(u32) * (c1 - c0);
+        }
+      }
+      (void)rows_all;
+      const int64_t nr = r1[k] - r0[k];
+      cudaMemcpyAsync(d_rp[buf].p, rp + r0[k], sizeof(int64_t) * (size_t)(nr + 1), cudaMemcpyHostToDevice, copy_st);
+      bytes_h2d += sizeof(int64_t) * (nr + 1);
+      cudaEventRecord(ev_up[buf], copy_st);
+    };
+
+    // ---- Alg. 2 lines 7-11: local refinement per batch, merge ---------------------------------------------------------
+    int64_t base_id = 0;
+    cudaStreamSynchronize(st);  // buffers of the previous iteration are free
+    upload_batch(0, 0, false);
+    for (int k = 0; k < nb && !rc; ++k) {
+      const int buf = k & 1;
+      if (k + 1 < nb) upload_batch(k + 1, buf ^ 1, false);
+      cudaStreamWaitEvent(st, ev_up[buf], 0);
+      const int64_t nr = r1[k] - r0[k];
+      if (nr == 0) continue;
+      const int64_t e0 = rp[r0[k]], e1 = rp[r1[k]];
+      wl_csr lg;
+      lg.n = nr;
+      lg.m = e1 - e0;
+      lg.row_ptr = d_rp[buf].as<int64_t>();
+      lg.col_idx = d_col[buf].as<int>() - cuts[k];  // row offsets are global edge positions
+      lg.weights = weighted ? d_wt[buf].as<u32>() - cuts[k] : nullptr;
+      wl_options lo{};
+      lo.flags = flags & (WL_FLAG_NO_VALIDATE | WL_FLAG_NO_PRUNE);
+      lo.max_rounds = opt ? opt->max_rounds : 0;
+      lo.stream_id = ((u64)outer << 32) | (u64)(u32)k;
+      const Layout L = make_layout(nr, lg.m);
+      CoreResult cr{};
+      rc = refine_core(&lg, nullptr, seed, &lo, /*ranged=*/true, (int)r0[k], (int)r1[k], n_t, e0, d_ws.p, L, st, &cr);
+      if (rc) break;
+      ++g_launches; merge_kernel<<<blocks_for(nr, 256), 256, 0, st>>>(nr, cr.colour, (int)base_id, d_H.as<int>() + r0[k]);
+      base_id += cr.k;
+      edges_streamed += cr.edges_streamed;
+      ms_spmv += cr.ms_spmv;
+      ms_relabel += cr.ms_relabel;
+      ms_spmv_kernel += cr.ms_spmv_kernel;
+      spmv_alg_bytes += cr.spmv_alg_bytes;
+      spmv_launches += cr.spmv_launches;
+      rc = check_cuda(cudaStreamSynchronize(st));  // the workspace and this buffer are reused by the next batch
+    }
+    if (rc) break;
+    // ---- Alg. 2 lines 11-12: boundary nodes become singletons ---------------------------------------------------------
+    std::vector<int> bnodes, bids;
+    {
+      int64_t next = 0;
+      for (int k = 0; k <= nb; ++k) {
+        const int64_t upto = k < nb ? r0[k] : n_t;
+        for (int64_t i = next; i < upto; ++i) {
+          bnodes.push_back((int)i);
+          bids.push_back((int)(base_id++));
+        }
+        if (k < nb) next = r1[k];
+      }
+      for (size_t j = 0; j < bnodes.size(); ++j)
+        cudaMemcpyAsync(d_H.as<int>() + bnodes[j], &bids[j], sizeof(int), cudaMemcpyHostToDevice, st);
+      if (outer == 1) boundary_first = (int64_t)bnodes.size();
+    }
+    // canonical block map of this iteration (first-occurrence ids keep the composed map canonical)
+    Layout Lc{};
+    Lc.nscan = nscan;
+    launch_canonical(Lc, n_t, d_H.as<int>(), d_Hc.as<int>(), d_first.as<int>(), d_cof.as<int>(), d_bsum.as<int>(),
+                     d_misc.as<u64>(), st);
+    cudaMemcpyAsync(hs + kScalCanon, d_misc.p, sizeof(u64), cudaMemcpyDeviceToHost, st);
+    rc = check_cuda(cudaStreamSynchronize(st));
+    if (rc) break;
+    const int64_t K = (int64_t)hs[kScalCanon];
+    nb_last = nb;
+    K_final = K;
+    // compose original -> current map
+    if (map0_identity) {
+      if ((rc = d_map0.alloc(sizeof(int) * (size_t)n0, &used, device_cap_bytes))) break;
+      used_iter += d_map0.bytes;
+      cudaMemcpyAsync(d_map0.p, d_Hc.p, sizeof(int) * (size_t)n0, cudaMemcpyDeviceToDevice, st);
+      map0_identity = false;
+    } else {
+      ++g_launches; compose_kernel<<<blocks_for(n0, 256), 256, 0, st>>>(n0, d_map0.as<int>(), d_Hc.as<int>());
+    }
+    // ---- Alg. 2 line 15 (L200, Q15) -----------------------------------------------------------------------------------
+    bool stop = (nb == 1) || (K == n_t);
+    if (!stop && outer >= max_outer) {
+      stop = true;
+      hit_limit = true;
+    }
+    if (stop) {
+      rc = check_cuda(cudaStreamSynchronize(st));
+      break;
+    }
+
+    // ---- Alg. 2 line 13: quotient (Def. 4), second streaming pass -------------------------------------------------------
+    WL_ALLOC(d_rep, sizeof(int) * (size_t)K);
+    WL_ALLOC(d_cnt, sizeof(int) * (size_t)K);
+    WL_ALLOC(d_cursor, sizeof(int) * (size_t)K);
+    WL_ALLOC(d_qrp, sizeof(int64_t) * (size_t)(K + 1));
+    int64_t longest_cut_row = 0;  // a row cut by a batch border stays in the table until its last piece arrives
+    for (int k = 1; k < nb; ++k) {
+      const int64_t r = (std::upper_bound(rp, rp + n_t + 1, cuts[k]) - rp) - 1;
+      if (r >= 0 && r < n_t && rp[r] < cuts[k]) longest_cut_row = std::max(longest_cut_row, rp[r + 1] - rp[r]);
+    }
+    const u64 qslots = quot_table_slots(max_edges + longest_cut_row);
+    WL_ALLOC(d_qtab, sizeof(u64) * 2 * qslots);
+    WL_ALLOC(d_qcol, sizeof(int) * (size_t)max_edges);
+    WL_ALLOC(d_qwt, sizeof(u32) * (size_t)max_edges);
+    WL_ALLOC(d_sbsum, sizeof(u64) * (size_t)((K + kScanC - 1) / kScanC + 2));
+    if (rc) break;
+#undef WL_ALLOC
+    cudaMemsetAsync(d_rep.p, 0x7f, sizeof(int) * (size_t)K, st);
+    cudaMemsetAsync(d_cnt.p, 0, sizeof(int) * (size_t)K, st);
+    cudaMemsetAsync(d_cursor.p, 0, sizeof(int) * (size_t)K, st);
+    cudaMemsetAsync(d_qtab.p, 0, sizeof(u64) * 2 * qslots, st);
+    ++g_launches; block_rep_kernel<<<blocks_for(n_t, 256), 256, 0, st>>>(n_t, d_Hc.as<int>(), d_rep.as<int>());
+    int64_t* d_queries = (int64_t*)((char*)d_misc.p + 256);
+    int64_t* d_answers = (int64_t*)((char*)d_misc.p + 2048);
+    std::vector<int64_t>& nrp = q_rp[qsel ^ 1];
+    std::vector<int>& ncol = q_col[qsel ^ 1];
+    std::vector<u32>& nwt = q_wt[qsel ^ 1];
+    nrp.assign((size_t)K + 1, 0);
+    ncol.clear();
+    nwt.clear();
+    int64_t q_off = 0, emitted_blocks = 0;
+    // rows that cross a cut are uploaded in pieces: the piece of batch k is attributed to the node that owns it
+    for (int k = 0; k < nb && !rc; ++k) {
+      // upload the edge range of the batch plus the (clipped) row offsets of ALL nodes whose row intersects it
+      const int64_t c0 = cuts[k], c1 = cuts[k + 1];
+      size_t dummy = 0;
+      // nodes intersecting [c0, c1): from the node containing c0 to the node containing c1 - 1
+      int64_t na = (std::upper_bound(rp, rp + n_t + 1, c0) - rp) - 1;
+      int64_t nz = c1 > c0 ? (std::upper_bound(rp, rp + n_t + 1, c1 - 1) - rp) : na;
+      if (na < 0) na = 0;
+      if (nz > n_t) nz = n_t;
+      if (c1 == c0) continue;
+      const int* hc = (outer == 1) ? batch_col(k) : q_col[qsel].data() + c0;
+      const u32* hw = (outer == 1) ? batch_wt(k) : q_wt[qsel].data() + c0;
+      cudaMemcpyAsync(d_col[0].p, hc, sizeof(int) * (size_t)(c1 - c0), cudaMemcpyHostToDevice, st);
+      bytes_h2d += sizeof(int) * (c1 - c0);
+      if (weighted) {
+        cudaMemcpyAsync(d_wt[0].p, hw, sizeof(u32) * (size_t)(c1 - c0), cudaMemcpyHostToDevice, st);
+        bytes_h2d += sizeof(u32) * (c1 - c0);
+      }
+      // clipped row offsets for nodes na..nz
+      std::vector<int64_t> clip((size_t)(nz - na + 1));
+      for (int64_t i = na; i <= nz; ++i) clip[(size_t)(i - na)] = std::min(std::max(rp[i], c0), c1);
+      DevBuf d_clip;
+      if ((rc = d_clip.alloc(sizeof(int64_t) * clip.size(), &dummy, 0))) break;
+      cudaMemcpyAsync(d_clip.p, clip.data(), sizeof(int64_t) * clip.size(), cudaMemcpyHostToDevice, st);
+      bytes_h2d += sizeof(int64_t) * clip.size();
+      ++g_launches; quot_insert_kernel<<<blocks_for((nz - na) * 32, 256), 256, 0, st>>>(na, nz - na, d_clip.as<int64_t>(), d_col[0].as<int>() - c0, weighted ? d_wt[0].as<u32>() - c0 : nullptr, d_Hc.as<int>(), d_rep.as<int>(), d_qtab.as<u64>(), qslots - 1, d_cnt.as<int>());
+      rc = check_cuda(cudaStreamSynchronize(st));  // clip (host vector) and d_clip are released at the end of the scope
+      if (rc) break;
+      // a representative row that continues into the next batch is completed there: emit the blocks whose representative
+      // row ends at or before c1 and that were not emitted yet
+      int64_t done_nodes = (std::upper_bound(rp + 1, rp + n_t + 1, c1) - (rp + 1));  // nodes with rp[i+1] <= c1
+      if (k == nb - 1) done_nodes = n_t;
+      int64_t done_blocks = 0;
+      cudaMemcpyAsync(d_queries, &done_nodes, sizeof(int64_t), cudaMemcpyHostToDevice, st);
+      ++g_launches; rep_lower_bound_kernel<<<1, 32, 0, st>>>(d_rep.as<int>(), K, d_queries, 1, d_answers);
+      cudaMemcpyAsync(&done_blocks, d_answers, sizeof(int64_t), cudaMemcpyDeviceToHost, st);
+      rc = check_cuda(cudaStreamSynchronize(st));
+      if (rc) break;
+      const int64_t b_lo = emitted_blocks, b_hi = done_blocks;
+      if (b_hi > b_lo) {
+        launch_scan32(d_cnt.as<int>() + b_lo, b_hi - b_lo, q_off, d_qrp.as<int64_t>() + b_lo, d_sbsum.as<u64>(),
+                      d_misc.as<u64>() + 8, st);
+        u64 tot = 0;
+        cudaMemcpyAsync(&tot, d_misc.as<u64>() + 8, sizeof(u64), cudaMemcpyDeviceToHost, st);
+        rc = check_cuda(cudaStreamSynchronize(st));
+        if (rc) break;
+        // emit needs room for `tot` entries: the output buffers hold max_edges; finished rows may include a carried one
+        DevBuf d_oc, d_ow;
+        int* oc = d_qcol.as<int>();
+        u32* ow = d_qwt.as<u32>();
+        if ((int64_t)tot > max_edges) {
+          if ((rc = d_oc.alloc(sizeof(int) * (size_t)tot, &dummy, 0))) break;
+          if ((rc = d_ow.alloc(sizeof(u32) * (size_t)tot, &dummy, 0))) break;
+          oc = d_oc.as<int>();
+          ow = d_ow.as<u32>();
+        }
+        ++g_launches; quot_emit_kernel<<<blocks_for((int64_t)qslots, 256), 256, 0, st>>>(d_qtab.as<u64>(), qslots, d_qrp.as<int64_t>(), q_off, d_cursor.as<int>(), oc, ow, (int)b_lo, (int)b_hi);
+        ncol.resize((size_t)(q_off + (int64_t)tot));
+        nwt.resize((size_t)(q_off + (int64_t)tot));
+        if (tot) {
+          cudaMemcpyAsync(ncol.data() + q_off, oc, sizeof(int) * (size_t)tot, cudaMemcpyDeviceToHost, st);
+          cudaMemcpyAsync(nwt.data() + q_off, ow, sizeof(u32) * (size_t)tot, cudaMemcpyDeviceToHost, st);
+          bytes_d2h += (sizeof(int) + sizeof(u32)) * (int64_t)tot;
+        }
+        cudaMemcpyAsync(nrp.data() + b_lo, d_qrp.as<int64_t>() + b_lo, sizeof(int64_t) * (size_t)(b_hi - b_lo + 1),
+                        cudaMemcpyDeviceToHost, st);
+        bytes_d2h += sizeof(int64_t) * (b_hi - b_lo + 1);
+        rc = check_cuda(cudaStreamSynchronize(st));
+        if (rc) break;
+        q_off += (int64_t)tot;
+        emitted_blocks = b_hi;
+      }
+    }
+    if (rc) break;
+    nrp[(size_t)K] = q_off;
+    // ---- next outer iteration on the quotient ---------------------------------------------------------------------------
+    qsel ^= 1;
+    rp = q_rp[qsel].data();
+    n_t = K;
+    weighted = true;
+    const int64_t next_nb_cap = max_batch_edges;
+    std::vector<int64_t> next_cuts;
+    greedy_cuts(n_t, rp, next_nb_cap, next_cuts);
+    if ((flags & WL_FLAG_AGGRESSIVE_STOP) && (int64_t)next_cuts.size() - 1 >= nb) {  // L328
+      break;
+    }
+    cuts.swap(next_cuts);
+    (void)m_t;
+  }
+
+  if (rc == WL_OK) {
+    if (map0_identity) {
+      rc = WL_ECUDA;  // unreachable: every iteration composes the map
+    } else {
+      cudaMemcpyAsync(out_colors, d_map0.p, sizeof(int) * (size_t)n0, cudaMemcpyDeviceToHost, st);
+      bytes_d2h += sizeof(int) * n0;
+      cudaEventRecord(ev_end, st);
+      rc = check_cuda(cudaStreamSynchronize(st));
+    }
+  }
+  if (rc == WL_OK && stats) {
+    float t = 0;
+    cudaEventElapsedTime(&t, ev_begin, ev_end);
+    stats->outer_iters = outer;
+    stats->last_num_batches = nb_last;
+    stats->boundary_nodes = boundary_first;
+    stats->num_colors = K_final;
+    stats->edges_streamed = edges_streamed;
+    stats->bytes_h2d = bytes_h2d;
+    stats->bytes_d2h = bytes_d2h;
+    stats->ms_total = t;
+    stats->ms_spmv = ms_spmv;
+    stats->ms_relabel = ms_relabel;
+    stats->ms_spmv_kernel = ms_spmv_kernel;
+    stats->spmv_alg_bytes = spmv_alg_bytes;
+    stats->spmv_launches = spmv_launches;
+    stats->kernel_launches = (int32_t)(g_launches - launches_at_entry);
+  }
+  cleanup();
+  if (rc == WL_OK && hit_limit) return WL_EMAXROUNDS;
+  return rc;
+}
+
+}  // extern "C"

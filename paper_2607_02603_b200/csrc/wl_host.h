@@ -13,6 +13,7 @@ constexpr int64_t kMaxNodes = (1ll << 31) - 2;
 // device scalar block (u64 each)
 enum { kScalNew = 0, kScalErr = 1, kScalCanon = 2, kScalActive = 3, kScalActiveDeg = 4, kScalHub = 5, kNumScal = 16 };
 
+constexpr int kCanonChunk = 2048;        // nodes per CTA of the canonicalisation scan (== kScanChunk)
 constexpr int64_t kHubThreshold = 8192;  // rows longer than this are cut into chunks (spmv_hub_kernel)
 
 struct Layout {

@@ -12,6 +12,7 @@
 
 namespace wl {
 
+static_assert(kCanonChunk == kScanChunk, "wl_batched.cu sizes the scan scratch with kCanonChunk");
 thread_local int g_last_cuda_error = 0;
 thread_local int64_t g_launches = 0;
 

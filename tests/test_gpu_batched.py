@@ -1,0 +1,141 @@
+"""GPU parity tests of the batched path (Algorithm 2) and its step-level pieces."""
+import numpy as np
+import pytest
+import torch
+
+import graphgen as gg
+import oracle
+from helpers import refines
+
+pytestmark = pytest.mark.gpu
+wl = pytest.importorskip("paper_2607_02603_b200")
+
+
+def dev():
+    return torch.device("cuda", 0)
+
+
+# ------------------------------------------------------------------ B2
+@pytest.mark.parametrize("seed", range(6))
+def test_inner_labels_match_oracle(seed):
+    g = gg.rmat(10, edge_factor=6, seed=seed, symmetrize=bool(seed % 2))
+    n, rp, ci, wt = g.numpy()
+    nb = 2 + seed
+    eb = gg.random_edge_batches(g, nb, seed)
+    sink = (torch.arange(n) % nb).to(torch.int32)
+    want = oracle.inner_labels(n, rp, eb.numpy(), sink.numpy())
+    got = wl.wl_inner_labels(n, g.row_ptr.to(dev()), eb.to(dev()), sink.to(dev())).cpu().numpy()
+    assert (got == want).all()
+    # disjointness (L145) and the census  sum_k |V_k| + |boundary| = n
+    assert sum((got == k).sum() for k in range(nb)) + (got == -1).sum() == n
+
+
+def test_inner_labels_contiguous_batches_have_few_boundary_nodes():
+    g = gg.rmat(11, seed=3)
+    n, rp, ci, wt = g.numpy()
+    cuts = gg.contiguous_row_batches(g, g.m // 5 + 1)
+    eb = torch.bucketize(torch.arange(g.m), cuts[1:-1], right=True).to(torch.int32)
+    sink = torch.bucketize(g.row_ptr[:-1], cuts[1:-1], right=True).to(torch.int32)
+    got = wl.wl_inner_labels(n, g.row_ptr.to(dev()), eb.to(dev()), sink.to(dev())).cpu().numpy()
+    want = oracle.inner_labels(n, rp, eb.numpy(), sink.numpy())
+    assert (got == want).all()
+    assert (got == -1).sum() <= len(cuts) - 2
+
+
+# ------------------------------------------------------------------ B6
+def _rows_as_dicts(k, qrp, qc, qw):
+    return [dict(zip(qc[qrp[b]:qrp[b + 1]].tolist(), qw[qrp[b]:qrp[b + 1]].tolist())) for b in range(k)]
+
+
+@pytest.mark.parametrize("seed", range(6))
+def test_quotient_matches_oracle(seed):
+    g = gg.rmat(9, edge_factor=6, seed=seed, symmetrize=bool(seed % 2)) if seed < 4 else gg.random_weighted_digraph(300, 2500, seed, max_w=5)
+    n, rp, ci, wt = g.numpy()
+    c, counts, _ = oracle.refine(n, rp, ci, wt)
+    k, qrp, qc, qw = oracle.quotient(n, rp, ci, wt, c)
+    d = g.to(dev())
+    grp, gc, gw = wl.wl_quotient(n, d.row_ptr, d.col, d.weights, torch.from_numpy(c).to(dev()), k)
+    grp, gc, gw = grp.cpu().numpy(), gc.cpu().numpy(), gw.cpu().numpy()
+    assert grp.tolist() == qrp.tolist()  # every (B, B') pair stored once => same row lengths
+    assert _rows_as_dicts(k, grp, gc, gw) == _rows_as_dicts(k, qrp, qc, qw)
+
+
+def test_quotient_of_a_non_coarsest_stable_colouring():
+    g = gg.grid2d(12)
+    n, rp, ci, wt = g.numpy()
+    c = np.arange(n, dtype=np.int32)  # discrete partition: the quotient is the graph itself
+    d = g.to(dev())
+    grp, gc, gw = wl.wl_quotient(n, d.row_ptr, d.col, None, torch.from_numpy(c).to(dev()), n)
+    assert grp.cpu().numpy().tolist() == rp.tolist()
+    assert _rows_as_dicts(n, grp.cpu().numpy(), gc.cpu().numpy(), gw.cpu().numpy()) == \
+        _rows_as_dicts(n, rp, ci, np.ones(g.m, dtype=np.int64))
+
+
+# ------------------------------------------------------------------ Algorithm 2
+BATCH_GRAPHS = {
+    "rmat10_sym": lambda: gg.rmat(10, seed=1),
+    "rmat11_dir": lambda: gg.rmat(11, seed=2, symmetrize=False),
+    "er": lambda: gg.erdos_renyi(2000, 9000, seed=5),
+    "grid": lambda: gg.grid2d(20),
+    "weighted": lambda: gg.random_weighted_digraph(400, 3000, 9, max_w=3),
+    "hub": lambda: gg.from_edge_list(3001, [(0, j) for j in range(1, 3001)] + [(j, j % 7 + 1) for j in range(1, 3001)]),
+    "twins": lambda: gg.from_edge_list(6, [(0, 5), (1, 5), (2, 5), (3, 4), (4, 3)]),
+}
+
+
+@pytest.mark.parametrize("name", list(BATCH_GRAPHS))
+@pytest.mark.parametrize("nb", [1, 2, 4, 16])
+def test_batched_equals_cpu_algorithm2_and_invariants(name, nb):
+    g = BATCH_GRAPHS[name]()
+    n, rp, ci, wt = g.numpy()
+    cap = max(1, -(-g.m // nb))
+    coarsest, _, _ = oracle.refine(n, rp, ci, wt)
+    want, k_want, outer_want, nbl_want = oracle.rbsc(n, rp, ci, wt, cap)
+    res = wl.wl_refine_batched(n, g.row_ptr, g.col, g.weights, max_batch_edges=cap, seed=nb)
+    got = res.colors.numpy()
+    # bit-exact against the CPU Algorithm 2 that uses the deterministic oracle as RSC on the same edge partition
+    assert got.tolist() == want.tolist()
+    assert res.num_colors == k_want
+    assert res.stats["outer_iters"] == outer_want and res.stats["last_num_batches"] == nbl_want
+    # Theorem 2 (L163), refinement of the coarsest colouring (L165), case (i) (L208)
+    assert oracle.is_stable(n, rp, ci, wt, got)
+    assert refines(got, coarsest)
+    if res.stats["last_num_batches"] == 1:
+        assert got.tolist() == coarsest.tolist()
+
+
+def test_batched_caller_supplied_slices():
+    g = gg.rmat(10, seed=4)
+    n, rp, ci, wt = g.numpy()
+    cuts = gg.contiguous_row_batches(g, g.m // 3 + 1)
+    want, k_want, _, _ = oracle.rbsc(n, rp, ci, wt, g.m // 3 + 1, first_cuts=cuts.numpy())
+    res = wl.wl_refine_batched(n, g.row_ptr, g.col, None, max_batch_edges=g.m // 3 + 1, cuts=cuts.tolist(), seed=1)
+    assert res.colors.numpy().tolist() == want.tolist()
+
+
+def test_batched_cut_inside_a_long_row():
+    # one row of 3000 entries with cap 1000: the hub is a boundary node (Def. 5) in the first iteration
+    g = BATCH_GRAPHS["hub"]()
+    n, rp, ci, wt = g.numpy()
+    want, k_want, outer, nbl = oracle.rbsc(n, rp, ci, wt, 1000)
+    res = wl.wl_refine_batched(n, g.row_ptr, g.col, None, max_batch_edges=1000, seed=3)
+    assert res.colors.numpy().tolist() == want.tolist()
+    assert res.stats["boundary_nodes"] >= 1
+    assert oracle.is_stable(n, rp, ci, wt, res.colors.numpy())
+
+
+def test_batched_device_cap_and_limits():
+    g = gg.rmat(10, seed=1)
+    with pytest.raises(wl.WlError) as e:
+        wl.wl_refine_batched(g.n, g.row_ptr, g.col, None, max_batch_edges=g.m // 4, device_cap_bytes=4096)
+    assert e.value.code == wl.WL_ENOMEM
+    res = wl.wl_refine_batched(g.n, g.row_ptr, g.col, None, max_batch_edges=g.m // 4, max_outer_iters=1, allow_limit=True)
+    n, rp, ci, wt = g.numpy()
+    assert oracle.is_stable(n, rp, ci, wt, res.colors.numpy())  # every outer iteration ends on a stable colouring
+
+
+def test_batched_seed_independence():
+    g = gg.rmat(10, seed=6, symmetrize=False)
+    a = wl.wl_refine_batched(g.n, g.row_ptr, g.col, None, max_batch_edges=g.m // 5, seed=1).colors
+    b = wl.wl_refine_batched(g.n, g.row_ptr, g.col, None, max_batch_edges=g.m // 5, seed=2).colors
+    assert torch.equal(a, b)
