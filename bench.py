@@ -135,6 +135,21 @@ def run_reference(args):
     return 0
 
 
+def aggregate_over_ranks(dist, local_ms: float, units_per_rank: float, device=None):
+    """Max-over-ranks time and whole-job throughput for N independent replicas (weak scaling, no data-path collective).
+    dist = torch.distributed (initialised) or None for a single process.  Returns (ms_max, total_units_per_second)."""
+    import torch
+    world = 1
+    t = torch.tensor([local_ms], dtype=torch.float64, device=device)
+    u = torch.tensor([units_per_rank], dtype=torch.float64, device=device)
+    if dist is not None:
+        world = dist.get_world_size()
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    ms = float(t.item())
+    return ms, float(u.item()) / (ms / 1e3), world
+
+
 def workload_config(scale, n, m):
     return {"workload": f"R-MAT scale {scale}, edge factor 16, (a,b,c,d)=(0.57,0.19,0.19,0.05), seed "
                         f"{RMAT_SEEDS.get(scale, 2)}, symmetrised, deduplicated, uniform initial colour "
@@ -207,14 +222,10 @@ def main():
     barrier()
     launches = wl.wl_kernel_launches() - launches0
     clocks = sampler.stop() if rank == 0 else None
-    ms_total = ev0.elapsed_time(ev1)
-    t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
-    if dist is not None:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_total = float(t.item())
-    ms_per_step = ms_total / args.steps
     edges_per_step = results[-1].stats["edges_streamed"]
-    value = world * edges_per_step / (ms_per_step / 1e3) / 1e9
+    ms_total, edges_per_s, _ = aggregate_over_ranks(dist, ev0.elapsed_time(ev1), edges_per_step * args.steps, dev)
+    ms_per_step = ms_total / args.steps
+    value = edges_per_s / 1e9
 
     # ---- roofline of the dominant kernel (S1+S2 SpMV), from the library's own CUDA events on the launch stream --------
     peaks, peak_kind = measured_peaks()

@@ -59,6 +59,8 @@ typedef struct wl_csr {
 #define WL_FLAG_AGGRESSIVE_STOP 8u /* batched: stop when the next iteration's N_b would not decrease (L328)            */
 #define WL_FLAG_NARROW_COLORS 32u /* wl_spmv_round only: all colour ids are < 65536, gather them as 16-bit (wl_refine
                                     switches by itself while k <= 65536)                                              */
+#define WL_FLAG_SYNC_EVERY_ROUND 64u /* never queue several rounds without a host synchronisation (default: after round 6
+                                       the device keeps the colour count and the host looks once per window, S5)       */
 #define WL_FLAG_NO_CANONICAL 16u /* leave internal dense ids in out_colors (skips S6)                                  */
 
 typedef struct wl_options {

@@ -364,10 +364,12 @@ constexpr int kRelabelThreads = 256;
 __global__ void __launch_bounds__(kRelabelThreads)
 relabel_insert_kernel(int64_t count, const int* __restrict__ nodes, const int* __restrict__ colour,
                       const u64* __restrict__ y, int* __restrict__ rep, int* __restrict__ stamp, int round,
-                      Slot* __restrict__ table, u32 table_mask, u32* __restrict__ tmp, int k_old,
-                      u64* __restrict__ new_counter) {
+                      Slot* __restrict__ table, u32 table_mask, u32* __restrict__ tmp,
+                      const u64* __restrict__ k_ptr, u64* __restrict__ new_counter,
+                      u64* __restrict__ changed_counter) {
+  const int k_old = (int)*k_ptr;  // device-resident colour count: rounds can be queued without a host round trip
   int64_t t = (int64_t)blockIdx.x * kRelabelThreads + threadIdx.x;
-  bool win = false;
+  bool win = false, changed = false;
   u32 slot = 0;
   int i = -1;
   if (t < count) {
@@ -396,8 +398,11 @@ relabel_insert_kernel(int64_t count, const int* __restrict__ nodes, const int* _
         slot = (slot + 1) & table_mask;
       }
       tmp[i] = slot | (win ? kWinBit : 0u);
+      changed = true;
     }
   }
+  const int n_changed = __syncthreads_count(changed);
+  if (threadIdx.x == 0 && n_changed) atomicAdd(changed_counter, (u64)n_changed);
   int total;
   const int rank = block_rank<kRelabelThreads>(win, &total);
   __shared__ u64 s_base;
@@ -425,13 +430,28 @@ __global__ void relabel_resolve_kernel(int64_t count, const int* __restrict__ no
 }
 
 __global__ void relabel_cleanup_kernel(int64_t count, const int* __restrict__ nodes, Slot* __restrict__ table,
-                                       const u32* __restrict__ tmp) {
+                                       const u32* __restrict__ tmp, const u64* __restrict__ changed_prev) {
+  if (*changed_prev == 0) return;  // nothing was inserted by the previous step
   int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= count) return;
   const int i = nodes ? nodes[t] : (int)t;
   const u32 s = tmp[i];
   if (s == kNone) return;
   store_slot(table + (s & ~kWinBit), kEmpty, kEmpty);
+}
+
+// End of a round (S4): k += new ids; the count is logged for the host; counters are re-armed for the next round.
+// scal layout: see wl_host.h (kScalK, kScalNew, kScalChanged, kScalChangedPrev).
+__global__ void advance_round_kernel(u64* __restrict__ scal, int i_k, int i_new, int i_changed, int i_changed_prev,
+                                     u64* __restrict__ log, int log_slot) {
+  if (blockIdx.x == 0 && threadIdx.x == 0) {
+    const u64 k = scal[i_k] + scal[i_new];
+    scal[i_k] = k;
+    scal[i_new] = 0;
+    scal[i_changed_prev] = scal[i_changed];
+    scal[i_changed] = 0;
+    if (log) log[log_slot] = k;
+  }
 }
 
 // rep[c] = some node of colour c (any one: benign race)

@@ -120,13 +120,37 @@ void launch_hub_collect(const Layout& L, const wl_csr& g, int2* chunks, u64* cou
 }
 
 // one relabel step over all nodes; counter (device u64) must be zero on entry and holds the number of new ids on exit
-void launch_relabel(const Layout& L, int64_t count, const int* nodes, int* colour, const u64* y, int* rep, int* stamp,
-                    int round, Slot* table, u32* tmp, int k_old, u64* counter, cudaStream_t st) {
-  if (count == 0) return;
-  unsigned grid = blocks_for(count, kRelabelThreads);
-  ++g_launches; relabel_insert_kernel<<<grid, kRelabelThreads, 0, st>>>(count, nodes, colour, y, rep, stamp, round, table, L.table_mask, tmp, k_old, counter);
-  ++g_launches; relabel_resolve_kernel<<<grid, kRelabelThreads, 0, st>>>(count, nodes, colour, stamp, round, table, tmp);
-  ++g_launches; relabel_cleanup_kernel<<<grid, kRelabelThreads, 0, st>>>(count, nodes, table, tmp);
+// The table must be empty in slots [0, table_mask]; it is left dirty (clean_table() before the next use).
+// scal[kScalNew] / scal[kScalChanged] (zero on entry) receive the number of new ids / of nodes that changed colour.
+// Ends with advance_round_kernel: scal[kScalK] += new ids (logged to log[log_slot] if log != NULL), scal[kScalChangedPrev] =
+// nodes that changed colour in this step.
+void launch_relabel(u32 table_mask, int64_t count, const int* nodes, int* colour, const u64* y, int* rep, int* stamp,
+                    int round, Slot* table, u32* tmp, u64* scal, u64* log, int log_slot, cudaStream_t st) {
+  if (count > 0) {
+    unsigned grid = blocks_for(count, kRelabelThreads);
+    ++g_launches; relabel_insert_kernel<<<grid, kRelabelThreads, 0, st>>>(count, nodes, colour, y, rep, stamp, round, table, table_mask, tmp, scal + kScalK, scal + kScalNew, scal + kScalChanged);
+    ++g_launches; relabel_resolve_kernel<<<grid, kRelabelThreads, 0, st>>>(count, nodes, colour, stamp, round, table, tmp);
+  }
+  ++g_launches; advance_round_kernel<<<1, 32, 0, st>>>(scal, kScalK, kScalNew, kScalChanged, kScalChangedPrev, log, log_slot);
+}
+
+// Re-empty the slots the previous relabel step touched: a memset of the slot range when many nodes changed colour,
+// else a pass over that step's node list (tmp[i] holds the slot of a node that changed).
+// changed < 0: the host does not know how many nodes changed (queued rounds): the kernel decides on the device.
+void clean_table(Slot* table, u32 table_mask, int64_t changed, int64_t count, const int* nodes, const u32* tmp,
+                 const u64* scal, cudaStream_t st) {
+  if (changed == 0 || count == 0) return;
+  if (changed > 0 && (changed * 4 >= (int64_t)table_mask + 1 || changed * 2 >= count)) {
+    cudaMemsetAsync(table, 0xff, sizeof(Slot) * ((size_t)table_mask + 1), st);
+  } else {
+    ++g_launches; relabel_cleanup_kernel<<<blocks_for(count, kRelabelThreads), kRelabelThreads, 0, st>>>(count, nodes, table, tmp, scal + kScalChangedPrev);
+  }
+}
+
+static u32 round_table_mask(const Layout& L, int64_t n_active) {
+  u64 s = 1024;
+  while (s < 2ull * (u64)n_active && s < (u64)L.table_mask + 1) s <<= 1;
+  return (u32)(s - 1);
 }
 
 // canonical ids: uses `first` (int[n]) and `cof` (int[n]) as scratch, bsum int[nscan+1], total -> scal slot
@@ -215,6 +239,10 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
   cudaMemsetAsync(table, 0xff, sizeof(Slot) * ((size_t)L.table_mask + 1), st);
   cudaMemsetAsync(stamp, 0xff, sizeof(int) * (size_t)n, st);
   u32* d_err = (u32*)(scal + kScalErr);
+  // state of the previous relabel step, for the deferred table clean-up
+  int64_t prev_changed = 0, prev_count = 0;
+  const int* prev_list = nullptr;
+  u32 prev_mask = 0;
   if (!(flags & WL_FLAG_NO_VALIDATE)) {
     ++g_launches; validate_rows_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, g->row_ptr, g->weights, edge_first, edge_first + m, d_err);
     if (m > 0) { ++g_launches; validate_cols_kernel<<<148 * 8, 256, 0, st>>>(n_targets, edge_first, edge_first + m, g->col_idx, d_err); }
@@ -240,13 +268,20 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
   // rep[0] = node 0; stamp[0] = 0 marks block 0 as non-singleton
   cudaMemsetAsync(rep, 0, sizeof(int), st);
   cudaMemsetAsync(stamp, 0, sizeof(int), st);
+  const u64 one = 1;
+  cudaMemcpyAsync(scal + kScalK, &one, sizeof(u64), cudaMemcpyHostToDevice, st);
   if (init_colors)
-    launch_relabel(L, n, nullptr, colour, y, rep, stamp, /*round=*/0, table, tmp, /*k_old=*/1, scal + kScalNew, st);
+    launch_relabel(L.table_mask, n, nullptr, colour, y, rep, stamp, /*round=*/0, table, tmp, scal, nullptr, 0, st);
   cudaMemcpyAsync(hs, scal, sizeof(u64) * kNumScal, cudaMemcpyDeviceToHost, st);
   rc = check_cuda(cudaStreamSynchronize(st));
   if (rc) return rc;
   if ((u32)hs[kScalErr] & kErrInit) return WL_EINVAL;
-  k = 1 + (int64_t)hs[kScalNew];
+  k = (int64_t)hs[kScalK];
+  if (init_colors) {
+    prev_changed = (int64_t)hs[kScalChangedPrev];
+    prev_count = n;
+    prev_mask = L.table_mask;
+  }
   const int64_t num_hub_chunks = merge ? 0 : (int64_t)hs[kScalHub];
 
   // ---- S1-S5: rounds -------------------------------------------------------------------------------------------------
@@ -256,18 +291,19 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
   bool converged = false;
   const bool debug = std::getenv("WL_DEBUG") != nullptr;
   const double list_frac = std::getenv("WL_LIST_FRAC") ? std::atof(std::getenv("WL_LIST_FRAC")) : 0.75;
+  const bool no_runahead = (flags & WL_FLAG_SYNC_EVERY_ROUND) != 0;
+  constexpr int64_t kSyncRounds = 6;
   const int* cur_list = nullptr;  // NULL: every node is active
-  int64_t n_active = n, active_edges = m;
+  int64_t n_active = n, active_edges = m, pending_new = 0;
   int cur = 0;
-  for (int64_t r = 1; r <= max_rounds; ++r) {
+  // One refinement round queued on the stream (S1-S4); no host decision inside.
+  auto queue_round = [&](int64_t r, bool narrow, int64_t changed_hint, u64* log, int log_slot, cudaEvent_t ek0,
+                         cudaEvent_t ek1) -> bool {
     const u64 key = round_key(seed, stream_id, (u64)r);
-    cudaEvent_t e0 = evp.get(2), e1 = evp.get(3), e2 = evp.get(4), ek0 = evp.get(5), ek1 = evp.get(6);
-    cudaEventRecord(e0, st);
-    bool full_spmv = false;
-    if (k == 1 && !g->weights && !ranged) {
+    bool streamed = false;
+    if (k == 1 && !g->weights && !ranged && r == 1) {
       ++g_launches; spmv_uniform_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, g->row_ptr, weight_of(key, 0), y);
     } else {
-      const bool narrow = !merge && k <= 65536;
       if (narrow) { ++g_launches; narrow_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, colour, colour16); }
       if (merge) cudaMemsetAsync(y, 0, sizeof(u64) * (size_t)n, st);
       SpmvArgs a{cur_list, n_active, colour, colour16, narrow, hub_chunks, num_hub_chunks,
@@ -277,62 +313,100 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
       cudaEventRecord(ek1, st);
       edges_streamed += active_edges;
       spmv_alg_bytes += (int64_t)(4 + (narrow ? 2 : 4) + (g->weights ? 4 : 0)) * active_edges + 16 * n_active;
-      full_spmv = true;
+      streamed = true;
     }
-    cudaEventRecord(e1, st);
-    cudaMemsetAsync(scal + kScalNew, 0, sizeof(u64), st);
-    launch_relabel(L, n_active, cur_list, colour, y, rep, stamp, (int)r, table, tmp, (int)k, scal + kScalNew, st);
-    if (prune) {
-      cudaMemsetAsync(scal + kScalActive, 0, 2 * sizeof(u64), st);
-      ++g_launches; compact_active_kernel<<<blocks_for(n_active, 256), 256, 0, st>>>(n_active, cur_list, colour, stamp, rep, (int)r, g->row_ptr, act[cur], scal + kScalActive);
+    clean_table(table, prev_mask, changed_hint, prev_count, prev_list, tmp, scal, st);
+    const u32 mask_r = round_table_mask(L, n_active);
+    launch_relabel(mask_r, n_active, cur_list, colour, y, rep, stamp, (int)r, table, tmp, scal, log, log_slot, st);
+    prev_count = n_active;
+    prev_list = cur_list;
+    prev_mask = mask_r;
+    return streamed;
+  };
+  auto queue_compaction = [&](int64_t r) {
+    cudaMemsetAsync(scal + kScalActive, 0, 2 * sizeof(u64), st);
+    ++g_launches; compact_active_kernel<<<blocks_for(n_active, 256), 256, 0, st>>>(n_active, cur_list, colour, stamp, rep, (int)r, g->row_ptr, act[cur], scal + kScalActive);
+  };
+  // host side of a compaction whose counters have been read back; returns true when nothing is left to refine
+  auto adopt_compaction = [&]() -> bool {
+    pending_new = 0;
+    n_active = (int64_t)hs[kScalActive];
+    active_edges = (int64_t)hs[kScalActiveDeg];
+    if ((double)n_active < list_frac * (double)n) {
+      cur_list = act[cur];
+      cur ^= 1;
+    } else {  // nearly everything is still active: keep the list-free kernels
+      cur_list = nullptr;
+      n_active = n;
+      active_edges = m;
     }
+    return n_active == 0;
+  };
+  auto log_round = [&](int64_t r, int64_t k_new) {
+    if (opt && opt->round_colors && r <= opt->round_colors_cap) opt->round_colors[r - 1] = k_new;
+  };
+
+  int64_t r = 1;
+  while (r <= max_rounds && !converged) {
+    // Rounds 1..kSyncRounds: one host synchronisation per round (the host picks kernels from k and the active count).
+    // Deep-round regime (S5): up to kRunAhead rounds are queued back to back; the device keeps k, logs it per round,
+    // and the host looks at the log once per window.  A round after the fixed point changes nothing, so running past
+    // it is harmless; `rounds` and the trajectory stop at the first repeated count exactly as in the per-round mode.
+    const bool window = !no_runahead && r > kSyncRounds;
+    const int R = window ? (int)std::min<int64_t>(kRunAhead, max_rounds - r + 1) : 1;
+    cudaEvent_t e0 = evp.get(2), e2 = evp.get(4);
+    cudaEventRecord(e0, st);
+    bool streamed[kRunAhead];
+    const bool narrow = !merge && (window ? n <= 65536 : k <= 65536);
+    for (int j = 0; j < R; ++j) {
+      // prev_changed is the host's knowledge of how many nodes the previous step moved (-1: queued, unknown)
+      streamed[j] = queue_round(r + j, narrow, prev_changed, scal + kScalLog, j, evp.get(8 + 2 * j), evp.get(9 + 2 * j));
+      prev_changed = -1;
+    }
+    const int64_t r_last = r + R - 1;
+    const bool compact_now = prune && (window || r <= 2 || pending_new * 16 >= n_active);
+    if (compact_now) queue_compaction(r_last);
     cudaEventRecord(e2, st);
     cudaMemcpyAsync(hs, scal, sizeof(u64) * kNumScal, cudaMemcpyDeviceToHost, st);
     rc = check_cuda(cudaStreamSynchronize(st));
     if (rc) return rc;
-    float ta = 0, tb = 0;
-    cudaEventElapsedTime(&ta, e0, e1);
-    cudaEventElapsedTime(&tb, e1, e2);
-    ms_spmv += ta;
-    ms_relabel += tb;
-    if (full_spmv) {
-      float tc = 0;
-      cudaEventElapsedTime(&tc, ek0, ek1);
-      ms_spmv_kernel += tc;
-      ++spmv_launches;
+    float t_all = 0, t_spmv = 0;
+    cudaEventElapsedTime(&t_all, e0, e2);
+    for (int j = 0; j < R; ++j)
+      if (streamed[j]) {
+        float tc = 0;
+        cudaEventElapsedTime(&tc, evp.get(8 + 2 * j), evp.get(9 + 2 * j));
+        t_spmv += tc;
+        ++spmv_launches;
+      }
+    ms_spmv_kernel += t_spmv;
+    ms_spmv += t_spmv;
+    ms_relabel += t_all - t_spmv;
+    prev_changed = (int64_t)hs[kScalChangedPrev];
+    for (int j = 0; j < R && !converged; ++j) {
+      const int64_t k_new = (int64_t)hs[kScalLog + j];
+      rounds = (int32_t)(r + j);
+      log_round(r + j, k_new);
+      if (debug)
+        std::fprintf(stderr, "[wl_refine] round %lld: k %lld -> %lld, rows %lld, edges %lld%s\n", (long long)(r + j),
+                     (long long)k, (long long)k_new, (long long)n_active, (long long)active_edges,
+                     window ? " (queued)" : "");
+      if (k_new == k) converged = true;  // the partition did not change (Q1, Q2): fixed point
+      pending_new += k_new - k;
+      k = k_new;
     }
-    const int64_t k_new = k + (int64_t)hs[kScalNew];
-    rounds = (int32_t)r;
-    if (debug)
-      std::fprintf(stderr, "[wl_refine] round %lld: k %lld -> %lld, rows %lld, edges %lld, spmv %.3f ms, relabel %.3f ms\n",
-                   (long long)r, (long long)k, (long long)k_new, (long long)n_active, (long long)active_edges, ta, tb);
-    if (opt && opt->round_colors && r <= opt->round_colors_cap) opt->round_colors[r - 1] = k_new;
-    if (k_new == k) {  // the partition did not change (Q1, Q2): fixed point
-      converged = true;
+    if (debug) std::fprintf(stderr, "[wl_refine]   %d round(s): spmv %.3f ms, rest %.3f ms\n", R, t_spmv, t_all - t_spmv);
+    r += R;
+    if (converged) break;
+    if (compact_now && adopt_compaction()) {
+      // every block is a singleton (or can never split again): the next round cannot change anything and only
+      // confirms (same trajectory as the un-pruned algorithm)
+      if (r <= max_rounds) {
+        rounds = (int32_t)r;
+        log_round(r, k);
+        converged = true;
+      }
       break;
-    }
-    k = k_new;
-    if (prune) {
-      n_active = (int64_t)hs[kScalActive];
-      active_edges = (int64_t)hs[kScalActiveDeg];
-      if ((double)n_active < list_frac * (double)n) {
-        cur_list = act[cur];
-        cur ^= 1;
-      } else {  // nearly everything is still active: keep the list-free kernels
-        cur_list = nullptr;
-        n_active = n;
-        active_edges = m;
-      }
-      if (n_active == 0) {
-        // every block is a singleton (or can never split again): the next round cannot change anything and only
-        // confirms (same trajectory as the un-pruned algorithm)
-        if (r + 1 <= max_rounds) {
-          rounds = (int32_t)(r + 1);
-          if (opt && opt->round_colors && r + 1 <= opt->round_colors_cap) opt->round_colors[r] = k;
-          converged = true;
-        }
-        break;
-      }
     }
   }
   res->k = k;
@@ -534,11 +608,13 @@ int wl_relabel(int64_t n, const int32_t* colors, int64_t k, const uint64_t* y, i
   if (new_colors != colors)
     cudaMemcpyAsync(new_colors, colors, sizeof(int) * (size_t)n, cudaMemcpyDeviceToDevice, st);
   ++g_launches; set_rep_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, new_colors, rep);
-  launch_relabel(L, n, nullptr, new_colors, (const u64*)y, rep, stamp, 1, table, tmp, (int)k, scal + kScalNew, st);
+  const u64 k_u64 = (u64)k;
+  cudaMemcpyAsync(scal + kScalK, &k_u64, sizeof(u64), cudaMemcpyHostToDevice, st);
+  launch_relabel(L.table_mask, n, nullptr, new_colors, (const u64*)y, rep, stamp, 1, table, tmp, scal, nullptr, 0, st);
   cudaMemcpyAsync(hs, scal, sizeof(u64) * kNumScal, cudaMemcpyDeviceToHost, st);
   int rc = check_cuda(cudaStreamSynchronize(st));
   if (rc) return rc;
-  if (num_colors) *num_colors = k + (int64_t)hs[kScalNew];
+  if (num_colors) *num_colors = (int64_t)hs[kScalK];
   return check_cuda(cudaGetLastError());
 }
 

@@ -124,7 +124,7 @@ def test_canonicalize(n):
 
 # ------------------------------------------------------------------ whole Algorithm 1
 @pytest.mark.parametrize("name", list(GRAPHS))
-@pytest.mark.parametrize("flags", [0, 2, 4])
+@pytest.mark.parametrize("flags", [0, 2, 4, 64])
 def test_refine_equals_oracle(name, flags):
     g = GRAPHS[name]()
     n, rp, ci, wt = g.numpy()
