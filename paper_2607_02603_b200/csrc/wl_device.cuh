@@ -9,6 +9,22 @@ namespace wl {
 typedef unsigned long long u64;
 typedef unsigned int u32;
 
+// device scalar block (u64 each): counters the kernels keep between launches; kScalLog.. = colour count per queued round
+enum {
+  kScalNew = 0,        // new ids handed out by the running relabel step
+  kScalErr = 1,        // validation error bits
+  kScalCanon = 2,      // number of blocks found by the canonicalisation
+  kScalActive = 3,     // rows kept by the last compaction
+  kScalActiveDeg = 4,  // their out-degree sum
+  kScalHub = 5,        // hub chunks
+  kScalActiveHub = 6,  // hub rows kept by the last compaction
+  kScalK = 7,          // current number of colours
+  kScalTicket = 8,     // CTAs that finished relabel_finish_kernel
+  kScalErrAux = 9,     // validation error bits written on the side stream
+  kScalLog = 16,
+  kNumScal = 64
+};
+
 // ---- weight bijection (readings Q4/Q5; Alg. 1 lines 3-4) -------------------------------
 // mix is a bijection of Z/2^64: xor-shifts and odd multipliers are invertible.  M1/M2/G are
 // floor(frac(sqrt 2) 2^64)|1, floor(frac(sqrt 3) 2^64)|1, floor(frac(golden ratio) 2^64)|1.

@@ -10,9 +10,6 @@ namespace wl {
 
 constexpr int64_t kMaxNodes = (1ll << 31) - 2;
 
-// device scalar block (u64 each)
-enum { kScalNew = 0, kScalErr = 1, kScalCanon = 2, kScalActive = 3, kScalActiveDeg = 4, kScalHub = 5, kScalChanged = 6, kScalK = 7, kScalChangedPrev = 8, kScalLog = 16, kNumScal = 64 };
-
 constexpr int kRunAhead = kNumScal - kScalLog;  // rounds queued per host synchronisation in the deep-round regime
 constexpr int kCanonChunk = 2048;        // nodes per CTA of the canonicalisation scan (== kScanChunk)
 constexpr int64_t kHubThreshold = 8192;  // rows longer than this are cut into chunks (spmv_hub_kernel)

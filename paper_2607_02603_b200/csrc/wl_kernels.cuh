@@ -295,7 +295,7 @@ spmv_hub_kernel(const int2* __restrict__ chunks, const int64_t* __restrict__ row
   }
 }
 
-// narrow copy of the colour ids for rounds with k <= 65536
+// narrow copy of caller-supplied colour ids (wl_spmv_round with WL_FLAG_NARROW_COLORS; wl_refine keeps its own mirror)
 __global__ void narrow_kernel(int64_t n, const int* __restrict__ colour, unsigned short* __restrict__ colour16) {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i < n) colour16[i] = (unsigned short)colour[i];
@@ -308,7 +308,8 @@ __global__ void narrow_kernel(int64_t n, const int* __restrict__ colour, unsigne
 __global__ void __launch_bounds__(256)
 compact_active_kernel(int64_t count, const int* __restrict__ nodes, const int* __restrict__ colour,
                       const int* __restrict__ stamp, const int* __restrict__ rep, int round,
-                      const int64_t* __restrict__ row_ptr, int* __restrict__ next, u64* __restrict__ counters) {
+                      const int64_t* __restrict__ row_ptr, int64_t hub_threshold, int* __restrict__ next,
+                      u64* __restrict__ counters, u64* __restrict__ hub_counter) {
   int64_t t = (int64_t)blockIdx.x * 256 + threadIdx.x;
   bool keep = false;
   int i = 0;
@@ -319,6 +320,7 @@ compact_active_kernel(int64_t count, const int* __restrict__ nodes, const int* _
     keep = stamp[c] == round;
     if (keep) {
       deg = (u64)(row_ptr[i + 1] - row_ptr[i]);
+      if ((int64_t)deg > hub_threshold) atomicAdd(hub_counter, 1ull);  // rare: hubs still in a splittable block
       if (deg == 0) {
         // y_i = 0 in every round.  If the block's representative has no out-edge either, every member with an
         // out-edge is compared against y[rep] = 0 and leaves on its own; the edgeless members never need another look.
@@ -356,21 +358,37 @@ __global__ void spmv_uniform_kernel(int64_t n, const int64_t* __restrict__ row_p
 // S3+S4: relabel (colour_i, y_i) -> dense id (Alg. 1 line 6, L122; Q6: exact 96-bit pairs, never a hash of them).
 // A block keeps its id for the sub-block that agrees with its representative rep[c]; every other distinct pair
 // (c, y) claims a slot of an exact-key hash table with one 128-bit CAS and gets a fresh id k, k+1, ...  (block-
-// aggregated counter).  stamp[c] == round  <=>  block c has at least two nodes after this round (no atomics: plain
-// idempotent stores).  nodes == NULL: all nodes.
+// aggregated counter, S4).  One kernel per round:
+//   phase 1  every thread compares with its representative and, if different, finds or claims the slot of its key
+//            (no thread waits on another one here); a claimed slot carries the id kPending;
+//   phase 2  the winners of the CTA take consecutive ids, publish them in the slot, become the representative of the
+//            new colour and record the slot in slot_of[id] (relabel_finish_kernel re-empties exactly those slots);
+//   phase 3  a node that found its key claimed by somebody else reads the id from the slot; if it is still pending it
+//            polls.  The winner publishes without waiting on anything but its own CTA's phase 1, so the poll ends.
+// stamp[c] == round  <=>  block c has at least two nodes after this round (no atomics: plain idempotent stores).
+// colour16 (optional) mirrors the ids as 16 bits while k <= 65536 (narrow gathers in the SpMV).  nodes == NULL: all nodes.
 // ---------------------------------------------------------------------------------------------------------------------
 constexpr int kRelabelThreads = 256;
+constexpr u32 kPending = 0xffffffffu;
+
+__device__ __forceinline__ u32 ld_slot_id(const Slot* p) {
+  u32 v;
+  asm volatile("ld.global.relaxed.gpu.u32 %0, [%1];" : "=r"(v) : "l"(reinterpret_cast<const u32*>(p) + 3) : "memory");
+  return v;
+}
+__device__ __forceinline__ void st_slot_id(Slot* p, u32 id) {
+  asm volatile("st.global.relaxed.gpu.u32 [%0], %1;" ::"l"(reinterpret_cast<u32*>(p) + 3), "r"(id) : "memory");
+}
 
 __global__ void __launch_bounds__(kRelabelThreads)
-relabel_insert_kernel(int64_t count, const int* __restrict__ nodes, const int* __restrict__ colour,
-                      const u64* __restrict__ y, int* __restrict__ rep, int* __restrict__ stamp, int round,
-                      Slot* __restrict__ table, u32 table_mask, u32* __restrict__ tmp,
-                      const u64* __restrict__ k_ptr, u64* __restrict__ new_counter,
-                      u64* __restrict__ changed_counter) {
+relabel_kernel(int64_t count, const int* __restrict__ nodes, int* __restrict__ colour,
+               unsigned short* __restrict__ colour16, const u64* __restrict__ y, int* __restrict__ rep,
+               int* __restrict__ stamp, int round, Slot* __restrict__ table, u32 table_mask,
+               u32* __restrict__ slot_of, const u64* __restrict__ k_ptr, u64* __restrict__ new_counter) {
   const int k_old = (int)*k_ptr;  // device-resident colour count: rounds can be queued without a host round trip
   int64_t t = (int64_t)blockIdx.x * kRelabelThreads + threadIdx.x;
-  bool win = false, changed = false;
-  u32 slot = 0;
+  bool win = false, lose = false;
+  u32 slot = 0, id = kPending;
   int i = -1;
   if (t < count) {
     i = nodes ? nodes[t] : (int)t;
@@ -380,9 +398,8 @@ relabel_insert_kernel(int64_t count, const int* __restrict__ nodes, const int* _
     const u64 yr = y[r];
     if (yi == yr) {
       if (i != r && stamp[c] != round) stamp[c] = round;
-      tmp[i] = kNone;
     } else {
-      const Slot mine = {yi, (u64)(u32)c | ((u64)(u32)i << 32)};
+      const Slot mine = {yi, (u64)(u32)c | ((u64)kPending << 32)};
       const Slot empty = {kEmpty, kEmpty};
       slot = (u32)slot_hash((u32)c, yi) & table_mask;
       while (true) {
@@ -394,63 +411,55 @@ relabel_insert_kernel(int64_t count, const int* __restrict__ nodes, const int* _
             break;
           }
         }
-        if (v.y == yi && (u32)v.cx == (u32)c) break;
+        if (v.y == yi && (u32)v.cx == (u32)c) {
+          lose = true;
+          id = (u32)(v.cx >> 32);
+          break;
+        }
         slot = (slot + 1) & table_mask;
       }
-      tmp[i] = slot | (win ? kWinBit : 0u);
-      changed = true;
     }
   }
-  const int n_changed = __syncthreads_count(changed);
-  if (threadIdx.x == 0 && n_changed) atomicAdd(changed_counter, (u64)n_changed);
   int total;
   const int rank = block_rank<kRelabelThreads>(win, &total);
   __shared__ u64 s_base;
   if (threadIdx.x == 0 && total > 0) s_base = atomicAdd(new_counter, (u64)total);
   __syncthreads();
   if (win) {
-    const int id = k_old + (int)s_base + rank;
-    // publish the id in the slot's x field (losers only ever compare y and the colour half)
-    reinterpret_cast<u32*>(table + slot)[3] = (u32)id;
+    id = (u32)(k_old + (int)s_base + rank);
+    st_slot_id(table + slot, id);
     rep[id] = i;
+    slot_of[id] = slot;
+  } else if (lose) {
+    while (id == kPending) id = ld_slot_id(table + slot);
+    if (stamp[id] != round) stamp[id] = round;
+  }
+  if (win || lose) {
+    colour[i] = (int)id;
+    if (colour16) colour16[i] = (unsigned short)id;
   }
 }
 
-__global__ void relabel_resolve_kernel(int64_t count, const int* __restrict__ nodes, int* __restrict__ colour,
-                                       int* __restrict__ stamp, int round, const Slot* __restrict__ table,
-                                       const u32* __restrict__ tmp) {
-  int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (t >= count) return;
-  const int i = nodes ? nodes[t] : (int)t;
-  const u32 s = tmp[i];
-  if (s == kNone) return;
-  const int id = (int)reinterpret_cast<const u32*>(table + (s & ~kWinBit))[3];
-  colour[i] = id;
-  if (!(s & kWinBit) && stamp[id] != round) stamp[id] = round;
-}
-
-__global__ void relabel_cleanup_kernel(int64_t count, const int* __restrict__ nodes, Slot* __restrict__ table,
-                                       const u32* __restrict__ tmp, const u64* __restrict__ changed_prev) {
-  if (*changed_prev == 0) return;  // nothing was inserted by the previous step
-  int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (t >= count) return;
-  const int i = nodes ? nodes[t] : (int)t;
-  const u32 s = tmp[i];
-  if (s == kNone) return;
-  store_slot(table + (s & ~kWinBit), kEmpty, kEmpty);
-}
-
-// End of a round (S4): k += new ids; the count is logged for the host; counters are re-armed for the next round.
-// scal layout: see wl_host.h (kScalK, kScalNew, kScalChanged, kScalChangedPrev).
-__global__ void advance_round_kernel(u64* __restrict__ scal, int i_k, int i_new, int i_changed, int i_changed_prev,
-                                     u64* __restrict__ log, int log_slot) {
-  if (blockIdx.x == 0 && threadIdx.x == 0) {
-    const u64 k = scal[i_k] + scal[i_new];
-    scal[i_k] = k;
-    scal[i_new] = 0;
-    scal[i_changed_prev] = scal[i_changed];
-    scal[i_changed] = 0;
-    if (log) log[log_slot] = k;
+// End of a round (S4): the slots claimed by this round's new ids are emptied again (the table is empty between
+// rounds), then the last CTA to finish does k += new ids, logs k for the host and re-arms the counter.
+// scal layout: see wl_host.h.
+__global__ void __launch_bounds__(256)
+relabel_finish_kernel(Slot* __restrict__ table, const u32* __restrict__ slot_of, u64* __restrict__ scal,
+                      u64* __restrict__ log, int log_slot) {
+  const u64 k_old = scal[kScalK], n_new = scal[kScalNew];
+  const u64 stride = (u64)gridDim.x * blockDim.x;
+  for (u64 j = (u64)blockIdx.x * blockDim.x + threadIdx.x; j < n_new; j += stride)
+    store_slot(table + slot_of[k_old + j], kEmpty, kEmpty);
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    __threadfence();
+    const u64 ticket = atomicAdd(scal + kScalTicket, 1ull);
+    if (ticket == (u64)gridDim.x - 1) {  // every other CTA has read k_old / n_new before taking its ticket
+      scal[kScalK] = k_old + n_new;
+      scal[kScalNew] = 0;
+      scal[kScalTicket] = 0;
+      if (log) log[log_slot] = k_old + n_new;
+    }
   }
 }
 
@@ -462,12 +471,14 @@ __global__ void set_rep_kernel(int64_t n, const int* __restrict__ colour, int* _
 
 // densify helper: y_i = init label (must be non-negative), colour_i = 0
 __global__ void init_labels_kernel(int64_t n, const int* __restrict__ init, int* __restrict__ colour,
-                                   u64* __restrict__ y, u32* __restrict__ err) {
+                                   unsigned short* __restrict__ colour16, u64* __restrict__ y,
+                                   u32* __restrict__ err) {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
   int v = init ? init[i] : 0;
   if (v < 0) atomicOr(err, kErrInit);
   colour[i] = 0;
+  colour16[i] = 0;
   y[i] = (u64)(u32)v;
 }
 
@@ -544,19 +555,23 @@ __global__ void __launch_bounds__(1024) scan_bsum_kernel(int64_t nb, int* __rest
   if (threadIdx.x == 0) *out_total = (u64)s_carry;
 }
 
-// canon_of_first[i] = rank of the block whose first node is i
+// cid[c] = rank of block c among the blocks ordered by their first node
 __global__ void __launch_bounds__(kScanThreads)
 canon_rank_kernel(int64_t n, const int* __restrict__ colour, const int* __restrict__ first,
-                  const int* __restrict__ bsum, int* __restrict__ canon_of_first) {
+                  const int* __restrict__ bsum, int* __restrict__ cid) {
   // blocked arrangement so that ranks follow node order
   const int64_t base = (int64_t)blockIdx.x * kScanChunk + (int64_t)threadIdx.x * kScanItems;
-  bool f[kScanItems];
+  int f[kScanItems];  // colour of node base + k if it is the first node of its block, else -1
   int cnt = 0;
 #pragma unroll
   for (int k = 0; k < kScanItems; ++k) {
     int64_t i = base + k;
-    f[k] = i < n && first[colour[i]] == (int)i;
-    cnt += f[k];
+    f[k] = -1;
+    if (i < n) {
+      const int c = colour[i];
+      if (first[c] == (int)i) f[k] = c;
+    }
+    cnt += f[k] >= 0;
   }
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   int x = cnt;
@@ -573,13 +588,13 @@ canon_rank_kernel(int64_t n, const int* __restrict__ colour, const int* __restri
   int r = bsum[blockIdx.x] + woff + x - cnt;
 #pragma unroll
   for (int k = 0; k < kScanItems; ++k)
-    if (f[k]) canon_of_first[base + k] = r++;
+    if (f[k] >= 0) cid[f[k]] = r++;
 }
 
-__global__ void canon_apply_kernel(int64_t n, const int* __restrict__ colour, const int* __restrict__ first,
-                                   const int* __restrict__ canon_of_first, int* __restrict__ out) {
+__global__ void canon_apply_kernel(int64_t n, const int* __restrict__ colour, const int* __restrict__ cid,
+                                   int* __restrict__ out) {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i < n) out[i] = canon_of_first[first[colour[i]]];
+  if (i < n) out[i] = cid[colour[i]];
 }
 
 }  // namespace wl

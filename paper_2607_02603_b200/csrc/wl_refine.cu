@@ -119,32 +119,19 @@ void launch_hub_collect(const Layout& L, const wl_csr& g, int2* chunks, u64* cou
   ++g_launches; hub_collect_kernel<<<blocks_for(g.n, 256), 256, 0, st>>>(g.n, g.row_ptr, kHubThreshold, chunks, counter);
 }
 
-// one relabel step over all nodes; counter (device u64) must be zero on entry and holds the number of new ids on exit
-// The table must be empty in slots [0, table_mask]; it is left dirty (clean_table() before the next use).
-// scal[kScalNew] / scal[kScalChanged] (zero on entry) receive the number of new ids / of nodes that changed colour.
-// Ends with advance_round_kernel: scal[kScalK] += new ids (logged to log[log_slot] if log != NULL), scal[kScalChangedPrev] =
-// nodes that changed colour in this step.
-void launch_relabel(u32 table_mask, int64_t count, const int* nodes, int* colour, const u64* y, int* rep, int* stamp,
-                    int round, Slot* table, u32* tmp, u64* scal, u64* log, int log_slot, cudaStream_t st) {
+// One relabel step (S3+S4) over `nodes` (NULL: all): scal[kScalK] is the current colour count, scal[kScalNew] must be
+// zero; on completion scal[kScalK] has grown by the number of new ids (logged to log[log_slot] if log != NULL), the slots
+// [0, table_mask] of the table are empty again and colour16 (may be NULL) mirrors the new ids as 16 bits.
+// finish_items: upper bound of new ids known to the host (sizes the clean-up grid), <= 0: unknown.
+void launch_relabel(u32 table_mask, int64_t count, const int* nodes, int* colour, unsigned short* colour16, const u64* y,
+                    int* rep, int* stamp, int round, Slot* table, u32* slot_of, u64* scal, u64* log, int log_slot,
+                    cudaStream_t st) {
   if (count > 0) {
     unsigned grid = blocks_for(count, kRelabelThreads);
-    ++g_launches; relabel_insert_kernel<<<grid, kRelabelThreads, 0, st>>>(count, nodes, colour, y, rep, stamp, round, table, table_mask, tmp, scal + kScalK, scal + kScalNew, scal + kScalChanged);
-    ++g_launches; relabel_resolve_kernel<<<grid, kRelabelThreads, 0, st>>>(count, nodes, colour, stamp, round, table, tmp);
+    ++g_launches; relabel_kernel<<<grid, kRelabelThreads, 0, st>>>(count, nodes, colour, colour16, y, rep, stamp, round, table, table_mask, slot_of, scal + kScalK, scal + kScalNew);
   }
-  ++g_launches; advance_round_kernel<<<1, 32, 0, st>>>(scal, kScalK, kScalNew, kScalChanged, kScalChangedPrev, log, log_slot);
-}
-
-// Re-empty the slots the previous relabel step touched: a memset of the slot range when many nodes changed colour,
-// else a pass over that step's node list (tmp[i] holds the slot of a node that changed).
-// changed < 0: the host does not know how many nodes changed (queued rounds): the kernel decides on the device.
-void clean_table(Slot* table, u32 table_mask, int64_t changed, int64_t count, const int* nodes, const u32* tmp,
-                 const u64* scal, cudaStream_t st) {
-  if (changed == 0 || count == 0) return;
-  if (changed > 0 && (changed * 4 >= (int64_t)table_mask + 1 || changed * 2 >= count)) {
-    cudaMemsetAsync(table, 0xff, sizeof(Slot) * ((size_t)table_mask + 1), st);
-  } else {
-    ++g_launches; relabel_cleanup_kernel<<<blocks_for(count, kRelabelThreads), kRelabelThreads, 0, st>>>(count, nodes, table, tmp, scal + kScalChangedPrev);
-  }
+  const unsigned fgrid = (unsigned)std::max<int64_t>(1, std::min<int64_t>(blocks_for(count, 256), 148 * 8));
+  ++g_launches; relabel_finish_kernel<<<fgrid, 256, 0, st>>>(table, slot_of, scal, log, log_slot);
 }
 
 static u32 round_table_mask(const Layout& L, int64_t n_active) {
@@ -153,16 +140,16 @@ static u32 round_table_mask(const Layout& L, int64_t n_active) {
   return (u32)(s - 1);
 }
 
-// canonical ids: uses `first` (int[n]) and `cof` (int[n]) as scratch, bsum int[nscan+1], total -> scal slot
-void launch_canonical(const Layout& L, int64_t n, const int* colour, int* out, int* first, int* cof, int* bsum,
+// canonical ids: uses `first` (int[n], first node per colour) and `cid` (int[n], canonical id per colour) as scratch, bsum int[nscan+1], total -> scal slot
+void launch_canonical(const Layout& L, int64_t n, const int* colour, int* out, int* first, int* cid, int* bsum,
                       u64* total, cudaStream_t st) {
   if (n == 0) return;
   cudaMemsetAsync(first, 0x7f, sizeof(int) * (size_t)n, st);
   ++g_launches; first_node_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, colour, first);
   ++g_launches; canon_count_kernel<<<(unsigned)L.nscan, kScanThreads, 0, st>>>(n, colour, first, bsum);
   ++g_launches; scan_bsum_kernel<<<1, 1024, 0, st>>>(L.nscan, bsum, total);
-  ++g_launches; canon_rank_kernel<<<(unsigned)L.nscan, kScanThreads, 0, st>>>(n, colour, first, bsum, cof);
-  ++g_launches; canon_apply_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, colour, first, cof, out);
+  ++g_launches; canon_rank_kernel<<<(unsigned)L.nscan, kScanThreads, 0, st>>>(n, colour, first, bsum, cid);
+  ++g_launches; canon_apply_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, colour, cid, out);
 }
 
 int check_cuda(cudaError_t e) {
@@ -185,7 +172,7 @@ int basic_csr_check(const wl_csr* g) {
 u64* host_scal() {
   static thread_local u64* p = nullptr;
   if (!p) {
-    if (cudaHostAlloc((void**)&p, sizeof(u64) * kNumScal, cudaHostAllocDefault) != cudaSuccess) p = nullptr;
+    if (cudaHostAlloc((void**)&p, sizeof(u64) * (kNumScal + 8), cudaHostAllocDefault) != cudaSuccess) p = nullptr;
   }
   return p;
 }
@@ -208,6 +195,25 @@ uint64_t wl_weight(uint64_t key, uint64_t color) { return weight_of(key, color);
 
 namespace wl {
 
+// Side stream of refine_core: the column validation pass and the bulk of the table memset run next to round 1 when
+// that round reads neither (uniform start: y = outdeg * w(0), at most sqrt(2m) distinct keys).
+struct AuxStream {
+  cudaStream_t s = nullptr;
+  cudaEvent_t fork = nullptr, join = nullptr;
+  bool pending = false;
+  int init() {
+    if (cudaStreamCreateWithFlags(&s, cudaStreamNonBlocking) != cudaSuccess) return WL_ECUDA;
+    cudaEventCreateWithFlags(&fork, cudaEventDisableTiming);
+    cudaEventCreateWithFlags(&join, cudaEventDisableTiming);
+    return WL_OK;
+  }
+  ~AuxStream() {
+    if (fork) cudaEventDestroy(fork);
+    if (join) cudaEventDestroy(join);
+    if (s) cudaStreamDestroy(s);
+  }
+};
+
 // Algorithm 1 (L106-L127) on the rows of `g` (local nodes 0..g.n-1).  ranged: batched local RSC, targets outside [lo, hi)
 // are implicit singletons and targets inside map to local node j - lo (Eq. 3).  On success the dense (non canonical)
 // colours are in the workspace's colour array and *k_out is their number.  Synchronises `st` once per round.
@@ -227,62 +233,83 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
   int* colour = (int*)(ws + L.o_colour);
   int* rep = (int*)(ws + L.o_rep);
   int* stamp = (int*)(ws + L.o_stamp);
-  u32* tmp = (u32*)(ws + L.o_tmp);
+  u32* slot_of = (u32*)(ws + L.o_tmp);
   u64* y = (u64*)(ws + L.o_y);
   int* tile_row = (int*)(ws + L.o_tile_row);
   Slot* table = (Slot*)(ws + L.o_table);
+  unsigned short* colour16 = (unsigned short*)(ws + L.o_colour16);
+  int* act[2] = {(int*)(ws + L.o_act0), (int*)(ws + L.o_act1)};
+  int2* hub_chunks = (int2*)(ws + L.o_hub);
   const int64_t launches_at_entry = g_launches;
   EventPool evp;
+  const bool merge = (flags & WL_FLAG_MERGE_KERNEL) != 0 && !ranged;
+  const bool prune = !merge && !(flags & WL_FLAG_NO_PRUNE);
+  const bool validate = !(flags & WL_FLAG_NO_VALIDATE);
 
   // ---- S0: setup ---------------------------------------------------------------------------------------------------
   cudaMemsetAsync(scal, 0, sizeof(u64) * kNumScal, st);
-  cudaMemsetAsync(table, 0xff, sizeof(Slot) * ((size_t)L.table_mask + 1), st);
-  cudaMemsetAsync(stamp, 0xff, sizeof(int) * (size_t)n, st);
   u32* d_err = (u32*)(scal + kScalErr);
-  // state of the previous relabel step, for the deferred table clean-up
-  int64_t prev_changed = 0, prev_count = 0;
-  const int* prev_list = nullptr;
-  u32 prev_mask = 0;
-  if (!(flags & WL_FLAG_NO_VALIDATE)) {
-    ++g_launches; validate_rows_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, g->row_ptr, g->weights, edge_first, edge_first + m, d_err);
-    if (m > 0) { ++g_launches; validate_cols_kernel<<<148 * 8, 256, 0, st>>>(n_targets, edge_first, edge_first + m, g->col_idx, d_err); }
+  if (validate) {
     // the kernels below walk row_ptr: make sure it is well formed first
+    ++g_launches; validate_rows_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, g->row_ptr, g->weights, edge_first, edge_first + m, d_err);
     cudaMemcpyAsync(hs + kScalErr, scal + kScalErr, sizeof(u64), cudaMemcpyDeviceToHost, st);
     rc = check_cuda(cudaStreamSynchronize(st));
     if (rc) return rc;
     const u32 e = (u32)hs[kScalErr];
-    if (e & (kErrRowPtr | kErrCol)) return WL_EINVAL;
+    if (e & kErrRowPtr) return WL_EINVAL;
     if (e & kErrRowSum) return WL_ERANGE;
   }
-  const bool merge = (flags & WL_FLAG_MERGE_KERNEL) != 0 && !ranged;
-  const bool prune = !merge && !(flags & WL_FLAG_NO_PRUNE);
-  unsigned short* colour16 = (unsigned short*)(ws + L.o_colour16);
-  int* act[2] = {(int*)(ws + L.o_act0), (int*)(ws + L.o_act1)};
-  int2* hub_chunks = (int2*)(ws + L.o_hub);
+  // Round 1 from a uniform start with unit weights is y = outdeg * w(0): no column is read and at most sqrt(2m) + 1
+  // distinct keys exist (distinct degrees d_1 < d_2 < ... sum to at most m), so it runs in a small prefix of the table
+  // while the side stream validates the columns and empties the rest of the table.
+  const bool uniform_start = !init_colors && !g->weights && !ranged && !merge;
+  u64 prefix_slots = (u64)L.table_mask + 1;
+  if (uniform_start) {
+    u64 keys = 2;
+    while (keys * keys < 2ull * (u64)m + 4) keys <<= 1;  // power of two >= sqrt(2m)
+    u64 want = std::max<u64>(1024, 4 * keys);
+    if (want < prefix_slots) prefix_slots = want;
+  }
+  const bool overlap = uniform_start && prefix_slots < (u64)L.table_mask + 1 && n >= (1 << 16);
+  AuxStream aux;
+  cudaMemsetAsync(table, 0xff, sizeof(Slot) * (overlap ? prefix_slots : (u64)L.table_mask + 1), st);
+  cudaMemsetAsync(stamp, 0xff, sizeof(int) * (size_t)n, st);
+  if (overlap) {
+    if ((rc = aux.init())) return check_cuda(cudaGetLastError());
+    cudaEventRecord(aux.fork, st);
+    cudaStreamWaitEvent(aux.s, aux.fork, 0);
+    cudaMemsetAsync(table + prefix_slots, 0xff, sizeof(Slot) * ((u64)L.table_mask + 1 - prefix_slots), aux.s);
+    if (validate && m > 0) { ++g_launches; validate_cols_kernel<<<148 * 8, 256, 0, aux.s>>>(n_targets, edge_first, edge_first + m, g->col_idx, (u32*)(scal + kScalErrAux)); }
+    cudaMemcpyAsync(hs + kNumScal, scal + kScalErrAux, sizeof(u64), cudaMemcpyDeviceToHost, aux.s);
+    cudaEventRecord(aux.join, aux.s);
+    aux.pending = true;
+  } else if (validate && m > 0) {
+    ++g_launches; validate_cols_kernel<<<148 * 8, 256, 0, st>>>(n_targets, edge_first, edge_first + m, g->col_idx, d_err);
+  }
   if (merge) launch_tile_search(L, *g, tile_row, st);
   else launch_hub_collect(L, *g, hub_chunks, scal + kScalHub, st);
 
   // initial partition: colour 0 everywhere; a given init is densified by one relabel step keyed on the label (L94)
   int64_t k = 1;
-  ++g_launches; init_labels_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, init_colors, colour, y, d_err);
+  ++g_launches; init_labels_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, init_colors, colour, colour16, y, d_err);
   // rep[0] = node 0; stamp[0] = 0 marks block 0 as non-singleton
   cudaMemsetAsync(rep, 0, sizeof(int), st);
   cudaMemsetAsync(stamp, 0, sizeof(int), st);
   const u64 one = 1;
   cudaMemcpyAsync(scal + kScalK, &one, sizeof(u64), cudaMemcpyHostToDevice, st);
   if (init_colors)
-    launch_relabel(L.table_mask, n, nullptr, colour, y, rep, stamp, /*round=*/0, table, tmp, scal, nullptr, 0, st);
+    launch_relabel(L.table_mask, n, nullptr, colour, colour16, y, rep, stamp, /*round=*/0, table, slot_of, scal, nullptr, 0, st);
   cudaMemcpyAsync(hs, scal, sizeof(u64) * kNumScal, cudaMemcpyDeviceToHost, st);
   rc = check_cuda(cudaStreamSynchronize(st));
   if (rc) return rc;
-  if ((u32)hs[kScalErr] & kErrInit) return WL_EINVAL;
-  k = (int64_t)hs[kScalK];
-  if (init_colors) {
-    prev_changed = (int64_t)hs[kScalChangedPrev];
-    prev_count = n;
-    prev_mask = L.table_mask;
+  {
+    const u32 e = (u32)hs[kScalErr];
+    if (e & kErrCol) return WL_EINVAL;
+    if (e & kErrInit) return WL_EINVAL;
   }
+  k = (int64_t)hs[kScalK];
   const int64_t num_hub_chunks = merge ? 0 : (int64_t)hs[kScalHub];
+  int64_t active_hubs = num_hub_chunks;  // > 0: some hub row may still be in a splittable block
 
   // ---- S1-S5: rounds -------------------------------------------------------------------------------------------------
   int64_t edges_streamed = 0, spmv_alg_bytes = 0;
@@ -296,17 +323,27 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
   const int* cur_list = nullptr;  // NULL: every node is active
   int64_t n_active = n, active_edges = m, pending_new = 0;
   int cur = 0;
+  // the side stream's work must be complete (and its verdict known) before a kernel reads a column or the whole table
+  auto join_aux = [&]() -> int {
+    if (!aux.pending) return WL_OK;
+    aux.pending = false;
+    int rc2 = check_cuda(cudaStreamSynchronize(aux.s));
+    if (rc2) return rc2;
+    if ((u32)hs[kNumScal] & kErrCol) return WL_EINVAL;
+    return WL_OK;
+  };
   // One refinement round queued on the stream (S1-S4); no host decision inside.
-  auto queue_round = [&](int64_t r, bool narrow, int64_t changed_hint, u64* log, int log_slot, cudaEvent_t ek0,
+  auto queue_round = [&](int64_t r, bool narrow, bool mirror, u64* log, int log_slot, cudaEvent_t ek0,
                          cudaEvent_t ek1) -> bool {
     const u64 key = round_key(seed, stream_id, (u64)r);
     bool streamed = false;
-    if (k == 1 && !g->weights && !ranged && r == 1) {
+    u32 mask_r = round_table_mask(L, n_active);
+    if (k == 1 && uniform_start && r == 1) {
       ++g_launches; spmv_uniform_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, g->row_ptr, weight_of(key, 0), y);
+      if (aux.pending) mask_r = (u32)(prefix_slots - 1);
     } else {
-      if (narrow) { ++g_launches; narrow_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, colour, colour16); }
       if (merge) cudaMemsetAsync(y, 0, sizeof(u64) * (size_t)n, st);
-      SpmvArgs a{cur_list, n_active, colour, colour16, narrow, hub_chunks, num_hub_chunks,
+      SpmvArgs a{cur_list, n_active, colour, colour16, narrow, hub_chunks, active_hubs > 0 ? num_hub_chunks : 0,
                  cur_list ? stamp : nullptr, (int)r - 1, ranged, lo, hi};
       cudaEventRecord(ek0, st);
       launch_spmv(L, *g, a, key, tile_row, y, merge, st);
@@ -315,23 +352,21 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
       spmv_alg_bytes += (int64_t)(4 + (narrow ? 2 : 4) + (g->weights ? 4 : 0)) * active_edges + 16 * n_active;
       streamed = true;
     }
-    clean_table(table, prev_mask, changed_hint, prev_count, prev_list, tmp, scal, st);
-    const u32 mask_r = round_table_mask(L, n_active);
-    launch_relabel(mask_r, n_active, cur_list, colour, y, rep, stamp, (int)r, table, tmp, scal, log, log_slot, st);
-    prev_count = n_active;
-    prev_list = cur_list;
-    prev_mask = mask_r;
+    launch_relabel(mask_r, n_active, cur_list, colour, mirror ? colour16 : nullptr, y, rep, stamp, (int)r, table, slot_of,
+                   scal, log, log_slot, st);
     return streamed;
   };
   auto queue_compaction = [&](int64_t r) {
     cudaMemsetAsync(scal + kScalActive, 0, 2 * sizeof(u64), st);
-    ++g_launches; compact_active_kernel<<<blocks_for(n_active, 256), 256, 0, st>>>(n_active, cur_list, colour, stamp, rep, (int)r, g->row_ptr, act[cur], scal + kScalActive);
+    cudaMemsetAsync(scal + kScalActiveHub, 0, sizeof(u64), st);
+    ++g_launches; compact_active_kernel<<<blocks_for(n_active, 256), 256, 0, st>>>(n_active, cur_list, colour, stamp, rep, (int)r, g->row_ptr, kHubThreshold, act[cur], scal + kScalActive, scal + kScalActiveHub);
   };
   // host side of a compaction whose counters have been read back; returns true when nothing is left to refine
   auto adopt_compaction = [&]() -> bool {
     pending_new = 0;
     n_active = (int64_t)hs[kScalActive];
     active_edges = (int64_t)hs[kScalActiveDeg];
+    active_hubs = (int64_t)hs[kScalActiveHub];
     if ((double)n_active < list_frac * (double)n) {
       cur_list = act[cur];
       cur ^= 1;
@@ -339,6 +374,7 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
       cur_list = nullptr;
       n_active = n;
       active_edges = m;
+      active_hubs = num_hub_chunks;
     }
     return n_active == 0;
   };
@@ -354,15 +390,14 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
     // it is harmless; `rounds` and the trajectory stop at the first repeated count exactly as in the per-round mode.
     const bool window = !no_runahead && r > kSyncRounds;
     const int R = window ? (int)std::min<int64_t>(kRunAhead, max_rounds - r + 1) : 1;
+    if (!(k == 1 && uniform_start && r == 1) && (rc = join_aux())) return rc;
     cudaEvent_t e0 = evp.get(2), e2 = evp.get(4);
     cudaEventRecord(e0, st);
     bool streamed[kRunAhead];
+    // 16-bit ids: gathered while k <= 65536; the mirror is kept up to date by the relabel kernel as long as that holds
     const bool narrow = !merge && (window ? n <= 65536 : k <= 65536);
-    for (int j = 0; j < R; ++j) {
-      // prev_changed is the host's knowledge of how many nodes the previous step moved (-1: queued, unknown)
-      streamed[j] = queue_round(r + j, narrow, prev_changed, scal + kScalLog, j, evp.get(8 + 2 * j), evp.get(9 + 2 * j));
-      prev_changed = -1;
-    }
+    for (int j = 0; j < R; ++j)
+      streamed[j] = queue_round(r + j, narrow, narrow, scal + kScalLog, j, evp.get(8 + 2 * j), evp.get(9 + 2 * j));
     const int64_t r_last = r + R - 1;
     const bool compact_now = prune && (window || r <= 2 || pending_new * 16 >= n_active);
     if (compact_now) queue_compaction(r_last);
@@ -382,7 +417,6 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
     ms_spmv_kernel += t_spmv;
     ms_spmv += t_spmv;
     ms_relabel += t_all - t_spmv;
-    prev_changed = (int64_t)hs[kScalChangedPrev];
     for (int j = 0; j < R && !converged; ++j) {
       const int64_t k_new = (int64_t)hs[kScalLog + j];
       rounds = (int32_t)(r + j);
@@ -409,6 +443,7 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
       break;
     }
   }
+  if ((rc = join_aux())) return rc;
   res->k = k;
   res->rounds = rounds;
   res->edges_streamed = edges_streamed;
@@ -451,7 +486,7 @@ int wl_refine(const wl_csr* g, const int32_t* init_colors, uint64_t seed, int32_
   if (flags & WL_FLAG_NO_CANONICAL) {
     cudaMemcpyAsync(out_colors, cr.colour, sizeof(int) * (size_t)n, cudaMemcpyDeviceToDevice, st);
   } else {
-    // scratch: tmp -> first, rep -> canon_of_first (both dead now)
+    // scratch: tmp -> first node per colour, rep -> canonical id per colour (both dead now)
     launch_canonical(L, n, cr.colour, out_colors, (int*)(ws + L.o_tmp), (int*)(ws + L.o_rep), (int*)(ws + L.o_bsum),
                      (u64*)(ws + L.o_scal) + kScalCanon, st);
   }
@@ -598,7 +633,7 @@ int wl_relabel(int64_t n, const int32_t* colors, int64_t k, const uint64_t* y, i
   u64* scal = (u64*)(ws + L.o_scal);
   int* rep = (int*)(ws + L.o_rep);
   int* stamp = (int*)(ws + L.o_stamp);
-  u32* tmp = (u32*)(ws + L.o_tmp);
+  u32* slot_of = (u32*)(ws + L.o_tmp);
   Slot* table = (Slot*)(ws + L.o_table);
   u64* hs = host_scal();
   if (!hs) return WL_ECUDA;
@@ -610,7 +645,7 @@ int wl_relabel(int64_t n, const int32_t* colors, int64_t k, const uint64_t* y, i
   ++g_launches; set_rep_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, new_colors, rep);
   const u64 k_u64 = (u64)k;
   cudaMemcpyAsync(scal + kScalK, &k_u64, sizeof(u64), cudaMemcpyHostToDevice, st);
-  launch_relabel(L.table_mask, n, nullptr, new_colors, (const u64*)y, rep, stamp, 1, table, tmp, scal, nullptr, 0, st);
+  launch_relabel(L.table_mask, n, nullptr, new_colors, nullptr, (const u64*)y, rep, stamp, 1, table, slot_of, scal, nullptr, 0, st);
   cudaMemcpyAsync(hs, scal, sizeof(u64) * kNumScal, cudaMemcpyDeviceToHost, st);
   int rc = check_cuda(cudaStreamSynchronize(st));
   if (rc) return rc;
