@@ -440,16 +440,19 @@ relabel_kernel(int64_t count, const int* __restrict__ nodes, int* __restrict__ c
   }
 }
 
-// End of a round (S4): the slots claimed by this round's new ids are emptied again (the table is empty between
-// rounds), then the last CTA to finish does k += new ids, logs k for the host and re-arms the counter.
-// scal layout: see wl_host.h.
+// End of a round (S4): if `clean`, the slots claimed by this round's new ids are emptied again (the table is empty
+// between rounds; with clean == 0 the host does it once it knows how many ids there were: relabel_clean_kernel or a
+// memset), then the last CTA to finish does k += new ids, logs k for the host and re-arms the counter.
+// scal layout: see wl_device.cuh.
 __global__ void __launch_bounds__(256)
 relabel_finish_kernel(Slot* __restrict__ table, const u32* __restrict__ slot_of, u64* __restrict__ scal,
-                      u64* __restrict__ log, int log_slot) {
+                      u64* __restrict__ log, int log_slot, int clean) {
   const u64 k_old = scal[kScalK], n_new = scal[kScalNew];
-  const u64 stride = (u64)gridDim.x * blockDim.x;
-  for (u64 j = (u64)blockIdx.x * blockDim.x + threadIdx.x; j < n_new; j += stride)
-    store_slot(table + slot_of[k_old + j], kEmpty, kEmpty);
+  if (clean) {
+    const u64 stride = (u64)gridDim.x * blockDim.x;
+    for (u64 j = (u64)blockIdx.x * blockDim.x + threadIdx.x; j < n_new; j += stride)
+      store_slot(table + slot_of[k_old + j], kEmpty, kEmpty);
+  }
   __syncthreads();
   if (threadIdx.x == 0) {
     __threadfence();
@@ -461,6 +464,13 @@ relabel_finish_kernel(Slot* __restrict__ table, const u32* __restrict__ slot_of,
       if (log) log[log_slot] = k_old + n_new;
     }
   }
+}
+
+// empties the slots of the ids [first_id, first_id + count)
+__global__ void relabel_clean_kernel(Slot* __restrict__ table, const u32* __restrict__ slot_of, int64_t first_id,
+                                     int64_t count) {
+  int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (j < count) store_slot(table + slot_of[first_id + j], kEmpty, kEmpty);
 }
 
 // rep[c] = some node of colour c (any one: benign race)

@@ -122,16 +122,28 @@ void launch_hub_collect(const Layout& L, const wl_csr& g, int2* chunks, u64* cou
 // One relabel step (S3+S4) over `nodes` (NULL: all): scal[kScalK] is the current colour count, scal[kScalNew] must be
 // zero; on completion scal[kScalK] has grown by the number of new ids (logged to log[log_slot] if log != NULL), the slots
 // [0, table_mask] of the table are empty again and colour16 (may be NULL) mirrors the new ids as 16 bits.
-// finish_items: upper bound of new ids known to the host (sizes the clean-up grid), <= 0: unknown.
+// clean == false: the claimed slots stay (the caller empties them with clean_table once it knows the new colour count).
 void launch_relabel(u32 table_mask, int64_t count, const int* nodes, int* colour, unsigned short* colour16, const u64* y,
                     int* rep, int* stamp, int round, Slot* table, u32* slot_of, u64* scal, u64* log, int log_slot,
-                    cudaStream_t st) {
+                    bool clean, cudaStream_t st) {
   if (count > 0) {
     unsigned grid = blocks_for(count, kRelabelThreads);
     ++g_launches; relabel_kernel<<<grid, kRelabelThreads, 0, st>>>(count, nodes, colour, colour16, y, rep, stamp, round, table, table_mask, slot_of, scal + kScalK, scal + kScalNew);
   }
-  const unsigned fgrid = (unsigned)std::max<int64_t>(1, std::min<int64_t>(blocks_for(count, 256), 148 * 8));
-  ++g_launches; relabel_finish_kernel<<<fgrid, 256, 0, st>>>(table, slot_of, scal, log, log_slot);
+  const unsigned fgrid = clean ? (unsigned)std::max<int64_t>(1, std::min<int64_t>(blocks_for(count, 256), 148 * 8)) : 1u;
+  ++g_launches; relabel_finish_kernel<<<fgrid, 256, 0, st>>>(table, slot_of, scal, log, log_slot, clean ? 1 : 0);
+}
+
+// Re-empty the slots claimed by the ids [first_id, first_id + count) of a relabel step run with clean == false:
+// one scattered 16-byte store per id, or a memset of the slot range when that is cheaper (measured on B200: a scattered
+// store costs about as much as 16 slots of memset).
+void clean_table(Slot* table, u32 table_mask, const u32* slot_of, int64_t first_id, int64_t count, cudaStream_t st) {
+  if (count <= 0) return;
+  if (count * 16 >= (int64_t)table_mask + 1) {
+    cudaMemsetAsync(table, 0xff, sizeof(Slot) * ((size_t)table_mask + 1), st);
+  } else {
+    ++g_launches; relabel_clean_kernel<<<blocks_for(count, 256), 256, 0, st>>>(table, slot_of, first_id, count);
+  }
 }
 
 static u32 round_table_mask(const Layout& L, int64_t n_active) {
@@ -298,7 +310,7 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
   const u64 one = 1;
   cudaMemcpyAsync(scal + kScalK, &one, sizeof(u64), cudaMemcpyHostToDevice, st);
   if (init_colors)
-    launch_relabel(L.table_mask, n, nullptr, colour, colour16, y, rep, stamp, /*round=*/0, table, slot_of, scal, nullptr, 0, st);
+    launch_relabel(L.table_mask, n, nullptr, colour, colour16, y, rep, stamp, /*round=*/0, table, slot_of, scal, nullptr, 0, /*clean=*/false, st);
   cudaMemcpyAsync(hs, scal, sizeof(u64) * kNumScal, cudaMemcpyDeviceToHost, st);
   rc = check_cuda(cudaStreamSynchronize(st));
   if (rc) return rc;
@@ -308,6 +320,9 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
     if (e & kErrInit) return WL_EINVAL;
   }
   k = (int64_t)hs[kScalK];
+  // slots still claimed by the previous relabel step (emptied before the next one, when the host knows their number)
+  int64_t dirty_first = 1, dirty_count = init_colors ? k - 1 : 0;
+  u32 dirty_mask = L.table_mask;
   const int64_t num_hub_chunks = merge ? 0 : (int64_t)hs[kScalHub];
   int64_t active_hubs = num_hub_chunks;  // > 0: some hub row may still be in a splittable block
 
@@ -333,7 +348,7 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
     return WL_OK;
   };
   // One refinement round queued on the stream (S1-S4); no host decision inside.
-  auto queue_round = [&](int64_t r, bool narrow, bool mirror, u64* log, int log_slot, cudaEvent_t ek0,
+  auto queue_round = [&](int64_t r, bool narrow, bool mirror, bool clean, u64* log, int log_slot, cudaEvent_t ek0,
                          cudaEvent_t ek1) -> bool {
     const u64 key = round_key(seed, stream_id, (u64)r);
     bool streamed = false;
@@ -352,8 +367,11 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
       spmv_alg_bytes += (int64_t)(4 + (narrow ? 2 : 4) + (g->weights ? 4 : 0)) * active_edges + 16 * n_active;
       streamed = true;
     }
+    clean_table(table, dirty_mask, slot_of, dirty_first, dirty_count, st);
+    dirty_count = 0;
+    dirty_mask = mask_r;
     launch_relabel(mask_r, n_active, cur_list, colour, mirror ? colour16 : nullptr, y, rep, stamp, (int)r, table, slot_of,
-                   scal, log, log_slot, st);
+                   scal, log, log_slot, clean, st);
     return streamed;
   };
   auto queue_compaction = [&](int64_t r) {
@@ -397,7 +415,7 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
     // 16-bit ids: gathered while k <= 65536; the mirror is kept up to date by the relabel kernel as long as that holds
     const bool narrow = !merge && (window ? n <= 65536 : k <= 65536);
     for (int j = 0; j < R; ++j)
-      streamed[j] = queue_round(r + j, narrow, narrow, scal + kScalLog, j, evp.get(8 + 2 * j), evp.get(9 + 2 * j));
+      streamed[j] = queue_round(r + j, narrow, narrow, /*clean=*/window, scal + kScalLog, j, evp.get(8 + 2 * j), evp.get(9 + 2 * j));
     const int64_t r_last = r + R - 1;
     const bool compact_now = prune && (window || r <= 2 || pending_new * 16 >= n_active);
     if (compact_now) queue_compaction(r_last);
@@ -426,6 +444,10 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
                      (long long)k, (long long)k_new, (long long)n_active, (long long)active_edges,
                      window ? " (queued)" : "");
       if (k_new == k) converged = true;  // the partition did not change (Q1, Q2): fixed point
+      if (!window) {
+        dirty_first = k;
+        dirty_count = k_new - k;
+      }
       pending_new += k_new - k;
       k = k_new;
     }
@@ -645,7 +667,7 @@ int wl_relabel(int64_t n, const int32_t* colors, int64_t k, const uint64_t* y, i
   ++g_launches; set_rep_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, new_colors, rep);
   const u64 k_u64 = (u64)k;
   cudaMemcpyAsync(scal + kScalK, &k_u64, sizeof(u64), cudaMemcpyHostToDevice, st);
-  launch_relabel(L.table_mask, n, nullptr, new_colors, nullptr, (const u64*)y, rep, stamp, 1, table, slot_of, scal, nullptr, 0, st);
+  launch_relabel(L.table_mask, n, nullptr, new_colors, nullptr, (const u64*)y, rep, stamp, 1, table, slot_of, scal, nullptr, 0, /*clean=*/false, st);
   cudaMemcpyAsync(hs, scal, sizeof(u64) * kNumScal, cudaMemcpyDeviceToHost, st);
   int rc = check_cuda(cudaStreamSynchronize(st));
   if (rc) return rc;
