@@ -161,7 +161,7 @@ def workload_config(scale, n, m):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--scale", type=int, default=27)
     ap.add_argument("--impl", default="ours")
@@ -206,11 +206,19 @@ def main():
     def step(i):
         return wl.wl_refine(n, g.row_ptr, g.col, None, seed=1000 + i, flags=args.flags, workspace=ws, out=out)
 
-    for i in range(max(args.warmup, 3)):
-        res = step(i)
+    # nvidia-smi is started BEFORE the warm-up so that its start-up (NVML initialisation takes driver locks for a few
+    # hundred ms and would stretch the host round trips of the first timed steps) is over when the timed region begins;
+    # it keeps sampling every 200 ms during the timed region.
     sampler = ClockSampler(local_rank)
     if rank == 0:
         sampler.start()
+        t_wait = time.perf_counter()
+        while not sampler.lines and time.perf_counter() - t_wait < 10.0:
+            time.sleep(0.05)
+    for i in range(max(args.warmup, 3)):
+        res = step(i)
+    if rank == 0:
+        sampler.lines.clear()
     barrier()
     launches0 = wl.wl_kernel_launches()
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)

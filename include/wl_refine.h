@@ -61,6 +61,9 @@ typedef struct wl_csr {
                                     switches by itself while k <= 65536)                                              */
 #define WL_FLAG_SYNC_EVERY_ROUND 64u /* never queue several rounds without a host synchronisation (default: after round 6
                                        the device keeps the colour count and the host looks once per window, S5)       */
+#define WL_FLAG_EDGE_BALANCED 128u /* use the edge-balanced SpMV kernel (one warp per 2048 consecutive entries, all rows) in
+                                      every round instead of the row kernels; results are identical (measured slower on the
+                                      headline graph, kept for extreme degree skew)                          */
 #define WL_FLAG_NO_CANONICAL 16u /* leave internal dense ids in out_colors (skips S6)                                  */
 
 typedef struct wl_options {

@@ -19,6 +19,7 @@ WL_OK, WL_EINVAL, WL_ERANGE, WL_ENOMEM, WL_ECUDA, WL_EMAXROUNDS = 0, -1, -2, -3,
 WL_FLAG_NO_VALIDATE, WL_FLAG_NO_PRUNE, WL_FLAG_MERGE_KERNEL, WL_FLAG_AGGRESSIVE_STOP, WL_FLAG_NO_CANONICAL = 1, 2, 4, 8, 16
 WL_FLAG_NARROW_COLORS = 32
 WL_FLAG_SYNC_EVERY_ROUND = 64
+WL_FLAG_EDGE_BALANCED = 128
 
 EXPORTS = [
     "wl_refine_workspace_bytes", "wl_refine", "wl_refine_host", "wl_round_key", "wl_weight", "wl_spmv_round",

@@ -519,7 +519,7 @@ int wl_refine_batched(int64_t n, int32_t num_batches, const wl_edge_batch* batch
       lg.col_idx = d_col[buf].as<int>() - cuts[k];  // row offsets are global edge positions
       lg.weights = weighted ? d_wt[buf].as<u32>() - cuts[k] : nullptr;
       wl_options lo{};
-      lo.flags = flags & (WL_FLAG_NO_VALIDATE | WL_FLAG_NO_PRUNE);
+      lo.flags = flags & (WL_FLAG_NO_VALIDATE | WL_FLAG_NO_PRUNE | WL_FLAG_EDGE_BALANCED);
       lo.max_rounds = opt ? opt->max_rounds : 0;
       lo.stream_id = ((u64)outer << 32) | (u64)(u32)k;
       const Layout L = make_layout(nr, lg.m);

@@ -8,6 +8,8 @@ constexpr int kSpmvThreads = 256;
 constexpr int kSpmvIpt = 7;  // odd: 64-bit shared-memory reads at stride IPT are bank-conflict free
 constexpr int kSpmvTile = kSpmvThreads * kSpmvIpt;
 constexpr u32 kNone = 0xffffffffu;
+constexpr int kHubChunk = 4096;  // entries per CTA of spmv_hub_kernel
+constexpr int kHubThreads = 256;
 constexpr u32 kWinBit = 0x80000000u;
 
 // error bits written by device-side validation
@@ -34,6 +36,37 @@ __global__ void validate_rows_kernel(int64_t n, const int64_t* __restrict__ row_
       if (s >= (1ull << 32)) e |= kErrRowSum;  // quotient weights are row-sum bounded and travel as uint32
     } else if ((u64)(b - a) >= (1ull << 32)) {
       e |= kErrRowSum;
+    }
+  }
+  if (e) atomicOr(err, e);
+}
+
+// S0 for a uniform start with unit weights, one pass over row_ptr: the offsets are validated (as validate_rows_kernel),
+// every node gets colour 0, y_i = outdeg(i) * w0 is round 1's product (R2: with one colour no column needs to be read)
+// and the rows longer than hub_threshold are cut into chunks (as hub_collect_kernel).
+__global__ void s0_uniform_kernel(int64_t n, const int64_t* __restrict__ row_ptr, int64_t expect_first, int64_t expect_last,
+                                  u64 w0, int* __restrict__ colour, unsigned short* __restrict__ colour16,
+                                  u64* __restrict__ y, int64_t hub_threshold, int2* __restrict__ chunks, int64_t hub_cap,
+                                  u64* __restrict__ hub_counter, u32* __restrict__ err) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const int64_t a = row_ptr[i], b = row_ptr[i + 1];
+  u32 e = 0;
+  if (i == 0 && a != expect_first) e |= kErrRowPtr;
+  if (i == n - 1 && b != expect_last) e |= kErrRowPtr;
+  if (a > b || a < expect_first || b > expect_last) e |= kErrRowPtr;
+  int64_t d = e ? 0 : b - a;
+  if ((u64)d >= (1ull << 32)) e |= kErrRowSum, d = 0;
+  colour[i] = 0;
+  colour16[i] = 0;
+  y[i] = (u64)d * w0;
+  if (d > hub_threshold) {
+    const int nc = (int)((d + kHubChunk - 1) / kHubChunk);
+    const u64 base = atomicAdd(hub_counter, (u64)nc);
+    if ((int64_t)(base + nc) <= hub_cap) {
+      for (int c = 0; c < nc; ++c) chunks[base + c] = make_int2((int)i, c);
+    } else {
+      e |= kErrRowPtr;  // only overlapping (malformed) rows can exceed the capacity derived from m
     }
   }
   if (e) atomicOr(err, e);
@@ -179,11 +212,22 @@ __device__ __forceinline__ u64 colour_id(const CT* __restrict__ colour, int j, i
 // sector holds 16 nodes; measured 267 vs 125 G gathers/s on the scale-27 access pattern).
 constexpr int kSmallRow = 8;
 
-template <bool WEIGHTED, typename CT, bool RANGED>
+// clamps a column id that is not a node of [0, n_targets) and remembers that it saw one (VALIDATE: S0's range check)
+template <bool VALIDATE>
+__device__ __forceinline__ int checked_col(int c, int64_t n_targets, bool& bad) {
+  if (VALIDATE && (unsigned)c >= (unsigned)n_targets) {
+    bad = true;
+    return 0;
+  }
+  return c;
+}
+
+template <bool WEIGHTED, typename CT, bool RANGED, bool VALIDATE>
 __global__ void __launch_bounds__(256)
 spmv_rows32_kernel(int64_t nrows, const int* __restrict__ rows, const int64_t* __restrict__ row_ptr,
                    const int* __restrict__ col, const u32* __restrict__ wt, const CT* __restrict__ colour, u64 key,
-                   u64* __restrict__ y, int64_t hub_threshold, int lo, int hi) {
+                   u64* __restrict__ y, int64_t hub_threshold, int lo, int hi, int64_t n_targets,
+                   u32* __restrict__ err) {
   const int lane = threadIdx.x & 31;
   const int64_t base = (((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5) << 5;
   if (base >= nrows) return;
@@ -198,11 +242,12 @@ spmv_rows32_kernel(int64_t nrows, const int* __restrict__ rows, const int64_t* _
   const int64_t d = b - a;
   const bool small = d <= kSmallRow;
   u64 acc = 0;
+  bool bad = false;
   {
     const int dd = small ? (int)d : 0;
     int cidx[kSmallRow];
 #pragma unroll
-    for (int t = 0; t < kSmallRow; ++t) cidx[t] = t < dd ? __ldg(col + a + t) : -1;
+    for (int t = 0; t < kSmallRow; ++t) cidx[t] = t < dd ? checked_col<VALIDATE>(__ldg(col + a + t), n_targets, bad) : -1;
 #pragma unroll
     for (int t = 0; t < kSmallRow; ++t) {
       if (cidx[t] >= 0) {
@@ -220,8 +265,10 @@ spmv_rows32_kernel(int64_t nrows, const int* __restrict__ rows, const int64_t* _
     u64 s = 0;
     int64_t p = ra + lane;
     for (; p + 96 < rb; p += 128) {  // four independent gathers in flight per lane
-      const int c0 = ld_stream_i32(col + p), c1 = ld_stream_i32(col + p + 32), c2 = ld_stream_i32(col + p + 64),
-                c3 = ld_stream_i32(col + p + 96);
+      const int c0 = checked_col<VALIDATE>(ld_stream_i32(col + p), n_targets, bad),
+                c1 = checked_col<VALIDATE>(ld_stream_i32(col + p + 32), n_targets, bad),
+                c2 = checked_col<VALIDATE>(ld_stream_i32(col + p + 64), n_targets, bad),
+                c3 = checked_col<VALIDATE>(ld_stream_i32(col + p + 96), n_targets, bad);
       u64 v0 = weight_of(key, colour_id<RANGED>(colour, c0, lo, hi)),
           v1 = weight_of(key, colour_id<RANGED>(colour, c1, lo, hi)),
           v2 = weight_of(key, colour_id<RANGED>(colour, c2, lo, hi)),
@@ -235,7 +282,7 @@ spmv_rows32_kernel(int64_t nrows, const int* __restrict__ rows, const int64_t* _
       s += (v0 + v1) + (v2 + v3);
     }
     for (; p < rb; p += 32) {
-      u64 v = weight_of(key, colour_id<RANGED>(colour, ld_stream_i32(col + p), lo, hi));
+      u64 v = weight_of(key, colour_id<RANGED>(colour, checked_col<VALIDATE>(ld_stream_i32(col + p), n_targets, bad), lo, hi));
       if (WEIGHTED) v *= (u64)ld_stream_u32(wt + p);
       s += v;
     }
@@ -244,12 +291,11 @@ spmv_rows32_kernel(int64_t nrows, const int* __restrict__ rows, const int64_t* _
     if (lane == src) acc = s;
   }
   if (valid) y[i] = acc;
+  if (VALIDATE && bad) atomicOr(err, kErrCol);
 }
 
 // Hub rows (degree > hub_threshold) are cut into chunks of kHubChunk entries, one CTA each; partial sums meet in y
 // through one no-return 64-bit add per CTA (exact under any order: sums in Z/2^64).
-constexpr int kHubChunk = 4096;
-constexpr int kHubThreads = 256;
 
 __global__ void hub_collect_kernel(int64_t n, const int64_t* __restrict__ row_ptr, int64_t hub_threshold,
                                    int2* __restrict__ chunks, u64* __restrict__ counter) {
@@ -263,22 +309,30 @@ __global__ void hub_collect_kernel(int64_t n, const int64_t* __restrict__ row_pt
 }
 
 // active == NULL: every hub row; else only rows whose block is still splittable (stamp[colour[row]] == live_stamp)
-template <bool WEIGHTED, typename CT, bool RANGED>
+template <bool WEIGHTED, typename CT, bool RANGED, bool VALIDATE>
 __global__ void __launch_bounds__(kHubThreads)
 spmv_hub_kernel(const int2* __restrict__ chunks, const int64_t* __restrict__ row_ptr, const int* __restrict__ col,
                 const u32* __restrict__ wt, const CT* __restrict__ colour, u64 key, u64* __restrict__ y,
-                const int* __restrict__ colour32, const int* __restrict__ stamp, int live_stamp, int lo, int hi) {
+                const int* __restrict__ colour32, const int* __restrict__ stamp, int live_stamp, int lo, int hi,
+                int64_t n_targets, u32* __restrict__ err) {
   const int2 ch = chunks[blockIdx.x];
   const int64_t row = ch.x;
-  if (stamp && stamp[colour32[row]] != live_stamp) return;
+  const bool inactive = stamp && stamp[colour32[row]] != live_stamp;
+  if (inactive && !VALIDATE) return;
   const int64_t a = row_ptr[row] + (int64_t)ch.y * kHubChunk;
   int64_t b = a + kHubChunk;
   const int64_t rend = row_ptr[row + 1];
   if (b > rend) b = rend;
   u64 acc = 0;
+  bool bad = false;
+  if (VALIDATE && inactive) {  // a pruned hub row: its columns are only range-checked
+    for (int64_t p = a + threadIdx.x; p < b; p += kHubThreads) checked_col<true>(ld_stream_i32(col + p), n_targets, bad);
+    if (bad) atomicOr(err, kErrCol);
+    return;
+  }
 #pragma unroll 4
   for (int64_t p = a + threadIdx.x; p < b; p += kHubThreads) {
-    u64 v = weight_of(key, colour_id<RANGED>(colour, ld_stream_i32(col + p), lo, hi));
+    u64 v = weight_of(key, colour_id<RANGED>(colour, checked_col<VALIDATE>(ld_stream_i32(col + p), n_targets, bad), lo, hi));
     if (WEIGHTED) v *= (u64)ld_stream_u32(wt + p);
     acc += v;
   }
@@ -295,6 +349,157 @@ spmv_hub_kernel(const int2* __restrict__ chunks, const int64_t* __restrict__ row
   }
 }
 
+// ---------------------------------------------------------------------------------------------------------------------
+// S1+S2, edge-balanced and register-only: the kernel of the rounds in which (nearly) every row is active.
+// The edge array is cut into super-chunks of kEbSuper consecutive entries, one warp each, whatever the degree
+// distribution (empty rows cost nothing, a hub row is simply many chunks).  Per sub-chunk of 256 entries lane l owns the
+// entries 32 t + l: coalesced streaming column loads, kEbU independent colour gathers in flight per lane (adjacent lanes
+// gather for adjacent sorted columns and share sectors), weights inline.  A sub-chunk without a row end just accumulates
+// per lane.  Otherwise warp scans give F(q) = sum of the first q products of the sub-chunk and the lanes take one ROW END
+// each (row_ptr read coalesced): the row's sum is F(end) - F(previous end), exact in Z/2^64.  A row that lies
+// inside the super-chunk is written with a plain store; the (at most two) rows cut by the super-chunk's borders add their
+// pieces with no-return 64-bit adds (exact under any order), eb_setup_kernel having zeroed them first.
+// VALIDATE folds the column range check of S0 into the first pass that reads the columns (bad ids are clamped).
+// ---------------------------------------------------------------------------------------------------------------------
+constexpr int kEbU = 8;
+constexpr int kEbSub = 32 * kEbU;
+constexpr int kEbSubs = 8;
+constexpr int kEbSuper = kEbSub * kEbSubs;
+
+// chunk_row[c] = the row that contains entry e_anchor + c * kEbSuper (row 0 for c == 0); a row cut by that border is
+// zeroed in y.  e_anchor <= row_ptr[0] is the origin of the chunk grid.
+__global__ void eb_setup_kernel(int64_t n, const int64_t* __restrict__ row_ptr, int64_t e_anchor, int64_t nchunks,
+                                int* __restrict__ chunk_row, u64* __restrict__ y) {
+  const int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= nchunks) return;
+  if (c == 0) {
+    chunk_row[0] = 0;
+    return;
+  }
+  const int64_t B = e_anchor + c * kEbSuper;  // row_ptr[0] < B < row_ptr[n]
+  int64_t lo = 0, hi = n - 1;                 // first row whose end lies beyond B
+  while (lo < hi) {
+    const int64_t mid = (lo + hi) >> 1;
+    if (row_ptr[mid + 1] > B) hi = mid;
+    else lo = mid + 1;
+  }
+  chunk_row[c] = (int)lo;
+  if (row_ptr[lo] < B) y[lo] = 0;
+}
+
+template <bool WEIGHTED, typename CT, bool RANGED, bool VALIDATE>
+__global__ void __launch_bounds__(256)
+spmv_eb_kernel(int64_t n, const int64_t* __restrict__ row_ptr, const int* __restrict__ col, const u32* __restrict__ wt,
+               const CT* __restrict__ colour, u64 key, u64* __restrict__ y, const int* __restrict__ chunk_row,
+               int64_t e_anchor, int64_t e_first, int64_t e_last, int lo, int hi, int64_t n_targets,
+               u32* __restrict__ err) {
+  constexpr unsigned kFull = 0xffffffffu;
+  const int lane = threadIdx.x & 31;
+  const int64_t c = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  const int64_t E0 = e_anchor + c * kEbSuper;
+  if (E0 >= e_last) return;
+  const int64_t E1 = E0 + kEbSuper < e_last ? E0 + kEbSuper : e_last;
+  int64_t r_open = chunk_row[c];  // the row that is open at the current position
+  const int64_t r_first = r_open;
+  const bool first_cut = row_ptr[r_open] < E0;  // it started in an earlier super-chunk
+  u64 carry = 0;     // products of the open row seen so far in this super-chunk: carry + sum over lanes of lane_acc
+  u64 lane_acc = 0;
+  bool bad = false;
+  for (int64_t Es = E0; Es < E1; Es += kEbSub) {
+    const int64_t sub_end = Es + kEbSub < E1 ? Es + kEbSub : E1;
+    // entry Es + 32 t + lane: adjacent lanes read adjacent (sorted) columns, so their gathers share sectors
+    int ci[kEbU];
+    if (Es >= e_first && Es + kEbSub <= sub_end) {
+#pragma unroll
+      for (int t = 0; t < kEbU; ++t) ci[t] = ld_stream_i32(col + Es + 32 * t + lane);
+    } else {
+#pragma unroll
+      for (int t = 0; t < kEbU; ++t) {
+        const int64_t e = Es + 32 * t + lane;
+        ci[t] = (e >= e_first && e < sub_end) ? ld_stream_i32(col + e) : -1;
+      }
+    }
+    if (VALIDATE) {
+#pragma unroll
+      for (int t = 0; t < kEbU; ++t)
+        if (ci[t] != -1 && (unsigned)ci[t] >= (unsigned)n_targets) bad = true, ci[t] = 0;
+    }
+    u64 v[kEbU];
+#pragma unroll
+    for (int t = 0; t < kEbU; ++t) v[t] = ci[t] >= 0 ? colour_id<RANGED>(colour, ci[t], lo, hi) : 0ull;
+#pragma unroll
+    for (int t = 0; t < kEbU; ++t) {
+      v[t] = ci[t] >= 0 ? weight_of(key, v[t]) : 0ull;
+      if (WEIGHTED) v[t] *= ci[t] >= 0 ? (u64)ld_stream_u32(wt + Es + 32 * t + lane) : 0ull;
+    }
+    // row ends inside the sub-chunk, one per lane (row_ptr is non-decreasing: the lanes that have one form a prefix)
+    int64_t r = r_open + lane;
+    int64_t endpos = r < n ? row_ptr[r + 1] : (int64_t)0x7fffffffffffffffll;
+    unsigned em = __ballot_sync(kFull, endpos <= sub_end);
+    if (em == 0) {  // the whole sub-chunk lies inside the open row
+#pragma unroll
+      for (int t = 0; t < kEbU; ++t) lane_acc += v[t];
+      continue;
+    }
+    // S[t] of lane l = sum of the products at positions 0 .. 32 t + l of the sub-chunk
+    u64 T = 0;
+#pragma unroll
+    for (int t = 0; t < kEbU; ++t) {
+      u64 inc = v[t];
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const u64 x = __shfl_up_sync(kFull, inc, o);
+        if (lane >= o) inc += x;
+      }
+      v[t] = T + inc;
+      T += __shfl_sync(kFull, inc, 31);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) lane_acc += __shfl_xor_sync(kFull, lane_acc, o);
+    carry += lane_acc;
+    lane_acc = 0;
+    u64 Fprev = 0;
+    bool first_trip = true;
+    while (true) {  // 32 row ends per trip
+      const bool is_end = endpos <= sub_end;
+      const int cnt = __popc(em);
+      const int qm = is_end ? (int)(endpos - Es) - 1 : -1;  // F(q) = S at position q - 1; F(0) = 0
+      const int src = qm & 31, tt = qm >> 5;
+      u64 Fq = 0;
+#pragma unroll
+      for (int t = 0; t < kEbU; ++t) {
+        const u64 g = __shfl_sync(kFull, v[t], src);
+        if (tt == t) Fq = g;
+      }
+      u64 Fp = __shfl_up_sync(kFull, Fq, 1);
+      if (lane == 0) Fp = Fprev;
+      u64 sum = Fq - Fp;
+      if (lane == 0 && first_trip) sum += carry;
+      if (is_end) {
+        if (first_cut && r == r_first) {
+          if (sum) red_add_u64(y + r, sum);
+        } else {
+          y[r] = sum;
+        }
+      }
+      Fprev = __shfl_sync(kFull, Fq, cnt - 1);
+      first_trip = false;
+      r_open += cnt;
+      if (cnt < 32) break;
+      r = r_open + lane;
+      endpos = r < n ? row_ptr[r + 1] : (int64_t)0x7fffffffffffffffll;
+      em = __ballot_sync(kFull, endpos <= sub_end);
+      if (em == 0) break;
+    }
+    carry = T - Fprev;
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) lane_acc += __shfl_xor_sync(kFull, lane_acc, o);
+  carry += lane_acc;
+  if (lane == 0 && carry != 0 && r_open < n) red_add_u64(y + r_open, carry);  // continues in the next super-chunk
+  if (VALIDATE && bad) atomicOr(err, kErrCol);
+}
+
 // narrow copy of caller-supplied colour ids (wl_spmv_round with WL_FLAG_NARROW_COLORS; wl_refine keeps its own mirror)
 __global__ void narrow_kernel(int64_t n, const int* __restrict__ colour, unsigned short* __restrict__ colour16) {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -305,15 +510,37 @@ __global__ void narrow_kernel(int64_t n, const int* __restrict__ colour, unsigne
 // id, so its row needs neither y nor a relabel.  next = nodes of `nodes` (NULL: all) whose block still has >= 2 members
 // after round `round`; counters[0] += |next|, counters[1] += sum of their out-degrees.  Rows without out-edges are
 // dropped as soon as their block's representative has none either (their y is 0 in every round).
+// check_col != NULL (the column range check of S0 is still pending): the rows dropped here are never read
+// by a row kernel, so their columns are range-checked now, one warp per row (hub rows are left to spmv_hub_kernel).
 __global__ void __launch_bounds__(256)
 compact_active_kernel(int64_t count, const int* __restrict__ nodes, const int* __restrict__ colour,
                       const int* __restrict__ stamp, const int* __restrict__ rep, int round,
                       const int64_t* __restrict__ row_ptr, int64_t hub_threshold, int* __restrict__ next,
-                      u64* __restrict__ counters, u64* __restrict__ hub_counter) {
+                      u64* __restrict__ counters, u64* __restrict__ hub_counter, const int* __restrict__ check_col,
+                      int64_t n_targets, u32* __restrict__ err) {
   int64_t t = (int64_t)blockIdx.x * 256 + threadIdx.x;
   bool keep = false;
   int i = 0;
   u64 deg = 0;
+  if (check_col) {
+    int64_t a = 0, b = 0;
+    bool dropped = false;
+    if (t < count) {
+      const int node = nodes ? nodes[t] : (int)t;
+      a = row_ptr[node];
+      b = row_ptr[node + 1];
+      dropped = stamp[colour[node]] != round && b > a && b - a <= hub_threshold;
+    }
+    unsigned todo = __ballot_sync(0xffffffffu, dropped);
+    bool bad = false;
+    while (todo) {
+      const int src = __ffs(todo) - 1;
+      todo &= todo - 1;
+      const int64_t ra = __shfl_sync(0xffffffffu, a, src), rb = __shfl_sync(0xffffffffu, b, src);
+      for (int64_t p = ra + (threadIdx.x & 31); p < rb; p += 32) checked_col<true>(ld_stream_i32(check_col + p), n_targets, bad);
+    }
+    if (bad) atomicOr(err, kErrCol);
+  }
   if (t < count) {
     i = nodes ? nodes[t] : (int)t;
     const int c = colour[i];

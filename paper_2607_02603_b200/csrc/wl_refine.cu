@@ -52,6 +52,7 @@ Layout make_layout(int64_t n, int64_t m) {
   L.o_act1 = take(sizeof(int) * (size_t)n);
   L.hub_cap = m / kHubChunk + m / (kHubThreshold + 1) + 1;
   L.o_hub = take(sizeof(int2) * (size_t)L.hub_cap);
+  L.o_chunk_row = take(sizeof(int) * (size_t)(m / kEbSuper + 4));
   L.bytes = off;
   return L;
 }
@@ -77,20 +78,49 @@ struct SpmvArgs {
   int live_stamp;
   bool ranged;           // batched local RSC: targets outside [lo, hi) are implicit singletons
   int lo, hi;
+  bool eb = false;       // edge-balanced kernel over ALL rows (rows / hub_chunks ignored)
+  bool validate = false; // fold the column range check of S0 into this pass (it must read every column: no row list)
+  int* chunk_row = nullptr;
+  int64_t e_first = 0;   // row_ptr[0]
+  int64_t n_targets = 0;
+  u32* err = nullptr;
 };
 
-template <bool W, typename CT, bool R>
+// edge-balanced S1+S2 over all rows of g (see spmv_eb_kernel)
+template <bool W, typename CT, bool R, bool V>
+static void launch_eb3(const wl_csr& g, const SpmvArgs& a, const CT* colour, u64 key, u64* y, cudaStream_t st) {
+  const int64_t e_first = a.e_first, e_last = e_first + g.m;
+  const int64_t e_anchor = e_first;
+  const int64_t nchunks = (e_last - e_anchor + kEbSuper - 1) / kEbSuper;
+  ++g_launches; eb_setup_kernel<<<blocks_for(nchunks, 256), 256, 0, st>>>(g.n, g.row_ptr, e_anchor, nchunks, a.chunk_row, y);
+  ++g_launches; spmv_eb_kernel<W, CT, R, V><<<blocks_for(nchunks * 32, 256), 256, 0, st>>>(g.n, g.row_ptr, g.col_idx, g.weights, colour, key, y, a.chunk_row, e_anchor, e_first, e_last, a.lo, a.hi, a.n_targets, a.err);
+}
+template <bool W, typename CT>
+static void launch_eb(const wl_csr& g, const SpmvArgs& a, const CT* colour, u64 key, u64* y, cudaStream_t st) {
+  if (a.ranged) {
+    if (a.validate) launch_eb3<W, CT, true, true>(g, a, colour, key, y, st);
+    else launch_eb3<W, CT, true, false>(g, a, colour, key, y, st);
+  } else {
+    if (a.validate) launch_eb3<W, CT, false, true>(g, a, colour, key, y, st);
+    else launch_eb3<W, CT, false, false>(g, a, colour, key, y, st);
+  }
+}
+
+constexpr int kRowsCta = 64;  // two warps per CTA: a warp stuck on long rows does not hold six finished ones' slots (measured)
+
+template <bool W, typename CT, bool R, bool V>
 static void launch_row_hub2(const wl_csr& g, const SpmvArgs& a, const CT* colour, u64 key, u64* y, cudaStream_t st) {
-  unsigned grid = blocks_for(a.nrows, 256);
-  ++g_launches; spmv_rows32_kernel<W, CT, R><<<grid, 256, 0, st>>>(a.nrows, a.rows, g.row_ptr, g.col_idx, g.weights, colour, key, y, kHubThreshold, a.lo, a.hi);
+  unsigned grid = blocks_for(a.nrows, kRowsCta);
+  ++g_launches; spmv_rows32_kernel<W, CT, R, V><<<grid, kRowsCta, 0, st>>>(a.nrows, a.rows, g.row_ptr, g.col_idx, g.weights, colour, key, y, kHubThreshold, a.lo, a.hi, a.n_targets, a.err);
   if (a.num_hub_chunks > 0) {
-    ++g_launches; spmv_hub_kernel<W, CT, R><<<(unsigned)a.num_hub_chunks, kHubThreads, 0, st>>>(a.hub_chunks, g.row_ptr, g.col_idx, g.weights, colour, key, y, a.colour, a.stamp, a.live_stamp, a.lo, a.hi);
+    ++g_launches; spmv_hub_kernel<W, CT, R, V><<<(unsigned)a.num_hub_chunks, kHubThreads, 0, st>>>(a.hub_chunks, g.row_ptr, g.col_idx, g.weights, colour, key, y, a.colour, a.stamp, a.live_stamp, a.lo, a.hi, a.n_targets, a.err);
   }
 }
 template <bool W, typename CT>
 static void launch_row_hub(const wl_csr& g, const SpmvArgs& a, const CT* colour, u64 key, u64* y, cudaStream_t st) {
-  if (a.ranged) launch_row_hub2<W, CT, true>(g, a, colour, key, y, st);
-  else launch_row_hub2<W, CT, false>(g, a, colour, key, y, st);
+  if (a.ranged) launch_row_hub2<W, CT, true, false>(g, a, colour, key, y, st);
+  else if (a.validate) launch_row_hub2<W, CT, false, true>(g, a, colour, key, y, st);
+  else launch_row_hub2<W, CT, false, false>(g, a, colour, key, y, st);
 }
 
 void launch_spmv(const Layout& L, const wl_csr& g, const SpmvArgs& a, u64 key, const int* tile_row, u64* y, bool merge,
@@ -101,6 +131,16 @@ void launch_spmv(const Layout& L, const wl_csr& g, const SpmvArgs& a, u64 key, c
       ++g_launches; spmv_merge_kernel<true><<<(unsigned)L.ntiles, kSpmvThreads, 0, st>>>(g.n, g.m, g.row_ptr, g.col_idx, g.weights, a.colour, key, tile_row, y);
     } else {
       ++g_launches; spmv_merge_kernel<false><<<(unsigned)L.ntiles, kSpmvThreads, 0, st>>>(g.n, g.m, g.row_ptr, g.col_idx, g.weights, a.colour, key, tile_row, y);
+    }
+    return;
+  }
+  if (a.eb) {
+    if (g.weights) {
+      if (a.narrow) launch_eb<true, unsigned short>(g, a, a.colour16, key, y, st);
+      else launch_eb<true, int>(g, a, a.colour, key, y, st);
+    } else {
+      if (a.narrow) launch_eb<false, unsigned short>(g, a, a.colour16, key, y, st);
+      else launch_eb<false, int>(g, a, a.colour, key, y, st);
     }
     return;
   }
@@ -207,21 +247,31 @@ uint64_t wl_weight(uint64_t key, uint64_t color) { return weight_of(key, color);
 
 namespace wl {
 
-// Side stream of refine_core: the column validation pass and the bulk of the table memset run next to round 1 when
-// that round reads neither (uniform start: y = outdeg * w(0), at most sqrt(2m) distinct keys).
+// Side stream of refine_core: the bulk of the table memset runs next to S0 and round 1 when that round needs only a small
+// prefix of the table (uniform start: y = outdeg * w(0), at most sqrt(2m) distinct keys).  It is cut in two pieces so that
+// a round whose table fits the lower half does not wait for the upper one.
 struct AuxStream {
   cudaStream_t s = nullptr;
-  cudaEvent_t fork = nullptr, join = nullptr;
-  bool pending = false;
+  cudaEvent_t fork = nullptr, done_a = nullptr, done_b = nullptr;
+  u64 slots_a = 0, slots_b = 0;  // slots [0, slots_a) are empty after done_a, [0, slots_b) after done_b
+  bool active = false;
   int init() {
     if (cudaStreamCreateWithFlags(&s, cudaStreamNonBlocking) != cudaSuccess) return WL_ECUDA;
     cudaEventCreateWithFlags(&fork, cudaEventDisableTiming);
-    cudaEventCreateWithFlags(&join, cudaEventDisableTiming);
+    cudaEventCreateWithFlags(&done_a, cudaEventDisableTiming);
+    cudaEventCreateWithFlags(&done_b, cudaEventDisableTiming);
     return WL_OK;
   }
+  // make `st` wait until slots [0, slots) are empty
+  void need(cudaStream_t st, u64 slots, u64 prefix) {
+    if (!active || slots <= prefix) return;
+    cudaStreamWaitEvent(st, slots <= slots_a ? done_a : done_b, 0);
+  }
   ~AuxStream() {
+    if (s) cudaStreamSynchronize(s);  // the workspace belongs to the caller again once refine_core returns
     if (fork) cudaEventDestroy(fork);
-    if (join) cudaEventDestroy(join);
+    if (done_a) cudaEventDestroy(done_a);
+    if (done_b) cudaEventDestroy(done_b);
     if (s) cudaStreamDestroy(s);
   }
 };
@@ -248,6 +298,7 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
   u32* slot_of = (u32*)(ws + L.o_tmp);
   u64* y = (u64*)(ws + L.o_y);
   int* tile_row = (int*)(ws + L.o_tile_row);
+  int* chunk_row = (int*)(ws + L.o_chunk_row);
   Slot* table = (Slot*)(ws + L.o_table);
   unsigned short* colour16 = (unsigned short*)(ws + L.o_colour16);
   int* act[2] = {(int*)(ws + L.o_act0), (int*)(ws + L.o_act1)};
@@ -261,7 +312,15 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
   // ---- S0: setup ---------------------------------------------------------------------------------------------------
   cudaMemsetAsync(scal, 0, sizeof(u64) * kNumScal, st);
   u32* d_err = (u32*)(scal + kScalErr);
-  if (validate) {
+  // Round 1 from a uniform start with unit weights is y = outdeg * w(0): no column is read and at most sqrt(2m) + 1
+  // distinct keys exist (distinct degrees d_1 < d_2 < ... sum to at most m), so it runs in a small prefix of the table
+  // while the side stream empties the rest; one kernel validates the offsets, sets the initial colour, computes that y
+  // and collects the hub chunks.  The column range check is folded into the first kernel that reads the columns.
+  const bool uniform_start = !init_colors && !g->weights && !ranged && !merge;
+  const bool force_eb = (flags & WL_FLAG_EDGE_BALANCED) != 0 && !merge && m > 0;
+  bool cols_checked = !validate || m == 0;
+  bool dropped_checked = false;  // the rows outside the active list have had their columns range-checked
+  if (validate && !uniform_start) {
     // the kernels below walk row_ptr: make sure it is well formed first
     ++g_launches; validate_rows_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, g->row_ptr, g->weights, edge_first, edge_first + m, d_err);
     cudaMemcpyAsync(hs + kScalErr, scal + kScalErr, sizeof(u64), cudaMemcpyDeviceToHost, st);
@@ -271,59 +330,65 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
     if (e & kErrRowPtr) return WL_EINVAL;
     if (e & kErrRowSum) return WL_ERANGE;
   }
-  // Round 1 from a uniform start with unit weights is y = outdeg * w(0): no column is read and at most sqrt(2m) + 1
-  // distinct keys exist (distinct degrees d_1 < d_2 < ... sum to at most m), so it runs in a small prefix of the table
-  // while the side stream validates the columns and empties the rest of the table.
-  const bool uniform_start = !init_colors && !g->weights && !ranged && !merge;
-  u64 prefix_slots = (u64)L.table_mask + 1;
+  const u64 table_slots = (u64)L.table_mask + 1;
+  u64 prefix_slots = table_slots;
   if (uniform_start) {
     u64 keys = 2;
     while (keys * keys < 2ull * (u64)m + 4) keys <<= 1;  // power of two >= sqrt(2m)
     u64 want = std::max<u64>(1024, 4 * keys);
     if (want < prefix_slots) prefix_slots = want;
   }
-  const bool overlap = uniform_start && prefix_slots < (u64)L.table_mask + 1 && n >= (1 << 16);
+  const bool overlap = uniform_start && prefix_slots < table_slots && n >= (1 << 16);
   AuxStream aux;
-  cudaMemsetAsync(table, 0xff, sizeof(Slot) * (overlap ? prefix_slots : (u64)L.table_mask + 1), st);
+  cudaMemsetAsync(table, 0xff, sizeof(Slot) * (overlap ? prefix_slots : table_slots), st);
   cudaMemsetAsync(stamp, 0xff, sizeof(int) * (size_t)n, st);
   if (overlap) {
     if ((rc = aux.init())) return check_cuda(cudaGetLastError());
     cudaEventRecord(aux.fork, st);
     cudaStreamWaitEvent(aux.s, aux.fork, 0);
-    cudaMemsetAsync(table + prefix_slots, 0xff, sizeof(Slot) * ((u64)L.table_mask + 1 - prefix_slots), aux.s);
-    if (validate && m > 0) { ++g_launches; validate_cols_kernel<<<148 * 8, 256, 0, aux.s>>>(n_targets, edge_first, edge_first + m, g->col_idx, (u32*)(scal + kScalErrAux)); }
-    cudaMemcpyAsync(hs + kNumScal, scal + kScalErrAux, sizeof(u64), cudaMemcpyDeviceToHost, aux.s);
-    cudaEventRecord(aux.join, aux.s);
-    aux.pending = true;
-  } else if (validate && m > 0) {
-    ++g_launches; validate_cols_kernel<<<148 * 8, 256, 0, st>>>(n_targets, edge_first, edge_first + m, g->col_idx, d_err);
+    aux.slots_a = std::max<u64>(prefix_slots, table_slots / 2);
+    aux.slots_b = table_slots;
+    if (aux.slots_a > prefix_slots) cudaMemsetAsync(table + prefix_slots, 0xff, sizeof(Slot) * (aux.slots_a - prefix_slots), aux.s);
+    cudaEventRecord(aux.done_a, aux.s);
+    cudaMemsetAsync(table + aux.slots_a, 0xff, sizeof(Slot) * (aux.slots_b - aux.slots_a), aux.s);
+    cudaEventRecord(aux.done_b, aux.s);
+    aux.active = true;
   }
-  if (merge) launch_tile_search(L, *g, tile_row, st);
-  else launch_hub_collect(L, *g, hub_chunks, scal + kScalHub, st);
-
-  // initial partition: colour 0 everywhere; a given init is densified by one relabel step keyed on the label (L94)
+  if (uniform_start) {
+    const u64 w0 = weight_of(round_key(seed, stream_id, 1), 0);
+    ++g_launches; s0_uniform_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, g->row_ptr, edge_first, edge_first + m, w0, colour, colour16, y, kHubThreshold, hub_chunks, L.hub_cap, scal + kScalHub, d_err);
+  } else {
+    if (!cols_checked) {
+      ++g_launches; validate_cols_kernel<<<148 * 8, 256, 0, st>>>(n_targets, edge_first, edge_first + m, g->col_idx, d_err);
+      cols_checked = true;
+    }
+    if (merge) launch_tile_search(L, *g, tile_row, st);
+    else launch_hub_collect(L, *g, hub_chunks, scal + kScalHub, st);
+    // initial partition: colour 0 everywhere; a given init is densified by one relabel step keyed on the label (L94)
+    ++g_launches; init_labels_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, init_colors, colour, colour16, y, d_err);
+  }
   int64_t k = 1;
-  ++g_launches; init_labels_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, init_colors, colour, colour16, y, d_err);
   // rep[0] = node 0; stamp[0] = 0 marks block 0 as non-singleton
   cudaMemsetAsync(rep, 0, sizeof(int), st);
   cudaMemsetAsync(stamp, 0, sizeof(int), st);
-  const u64 one = 1;
-  cudaMemcpyAsync(scal + kScalK, &one, sizeof(u64), cudaMemcpyHostToDevice, st);
-  if (init_colors)
-    launch_relabel(L.table_mask, n, nullptr, colour, colour16, y, rep, stamp, /*round=*/0, table, slot_of, scal, nullptr, 0, /*clean=*/false, st);
-  cudaMemcpyAsync(hs, scal, sizeof(u64) * kNumScal, cudaMemcpyDeviceToHost, st);
-  rc = check_cuda(cudaStreamSynchronize(st));
-  if (rc) return rc;
-  {
+  hs[kNumScal] = 1;
+  cudaMemcpyAsync(scal + kScalK, hs + kNumScal, sizeof(u64), cudaMemcpyHostToDevice, st);
+  int64_t num_hub_chunks = 0;
+  if (!uniform_start) {
+    if (init_colors)
+      launch_relabel(L.table_mask, n, nullptr, colour, colour16, y, rep, stamp, /*round=*/0, table, slot_of, scal, nullptr, 0, /*clean=*/false, st);
+    cudaMemcpyAsync(hs, scal, sizeof(u64) * kNumScal, cudaMemcpyDeviceToHost, st);
+    rc = check_cuda(cudaStreamSynchronize(st));
+    if (rc) return rc;
     const u32 e = (u32)hs[kScalErr];
     if (e & kErrCol) return WL_EINVAL;
     if (e & kErrInit) return WL_EINVAL;
+    k = (int64_t)hs[kScalK];
+    num_hub_chunks = merge ? 0 : (int64_t)hs[kScalHub];
   }
-  k = (int64_t)hs[kScalK];
   // slots still claimed by the previous relabel step (emptied before the next one, when the host knows their number)
   int64_t dirty_first = 1, dirty_count = init_colors ? k - 1 : 0;
   u32 dirty_mask = L.table_mask;
-  const int64_t num_hub_chunks = merge ? 0 : (int64_t)hs[kScalHub];
   int64_t active_hubs = num_hub_chunks;  // > 0: some hub row may still be in a splittable block
 
   // ---- S1-S5: rounds -------------------------------------------------------------------------------------------------
@@ -338,15 +403,6 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
   const int* cur_list = nullptr;  // NULL: every node is active
   int64_t n_active = n, active_edges = m, pending_new = 0;
   int cur = 0;
-  // the side stream's work must be complete (and its verdict known) before a kernel reads a column or the whole table
-  auto join_aux = [&]() -> int {
-    if (!aux.pending) return WL_OK;
-    aux.pending = false;
-    int rc2 = check_cuda(cudaStreamSynchronize(aux.s));
-    if (rc2) return rc2;
-    if ((u32)hs[kNumScal] & kErrCol) return WL_EINVAL;
-    return WL_OK;
-  };
   // One refinement round queued on the stream (S1-S4); no host decision inside.
   auto queue_round = [&](int64_t r, bool narrow, bool mirror, bool clean, u64* log, int log_slot, cudaEvent_t ek0,
                          cudaEvent_t ek1) -> bool {
@@ -354,19 +410,42 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
     bool streamed = false;
     u32 mask_r = round_table_mask(L, n_active);
     if (k == 1 && uniform_start && r == 1) {
-      ++g_launches; spmv_uniform_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, g->row_ptr, weight_of(key, 0), y);
-      if (aux.pending) mask_r = (u32)(prefix_slots - 1);
+      // y = outdeg * w(0) was written by s0_uniform_kernel (R2); its keys fit the table prefix emptied on `st`
+      if (aux.active) mask_r = (u32)(prefix_slots - 1);
     } else {
       if (merge) cudaMemsetAsync(y, 0, sizeof(u64) * (size_t)n, st);
+      // row kernels over the active list by default; WL_FLAG_EDGE_BALANCED: the edge-balanced kernel over all rows
+      const bool eb = force_eb;
       SpmvArgs a{cur_list, n_active, colour, colour16, narrow, hub_chunks, active_hubs > 0 ? num_hub_chunks : 0,
                  cur_list ? stamp : nullptr, (int)r - 1, ranged, lo, hi};
+      a.eb = eb;
+      a.chunk_row = chunk_row;
+      a.e_first = edge_first;
+      a.n_targets = n_targets;
+      a.err = d_err;
+      bool all_rows = eb;
+      if (!cols_checked) {  // S0's column range check rides on the first pass over the columns, which then takes every row
+        if (merge || ranged) {
+          ++g_launches; validate_cols_kernel<<<148 * 8, 256, 0, st>>>(n_targets, edge_first, edge_first + m, g->col_idx, d_err);
+        } else {
+          a.validate = true;
+          a.num_hub_chunks = num_hub_chunks;  // every hub chunk: pruned hub rows are only range-checked
+          if (!eb && cur_list && !dropped_checked) {  // cannot happen with the current round order; kept for safety
+            a.rows = nullptr, a.nrows = n, a.stamp = nullptr;
+            all_rows = true;
+          }
+        }
+        cols_checked = true;
+      }
       cudaEventRecord(ek0, st);
       launch_spmv(L, *g, a, key, tile_row, y, merge, st);
       cudaEventRecord(ek1, st);
-      edges_streamed += active_edges;
-      spmv_alg_bytes += (int64_t)(4 + (narrow ? 2 : 4) + (g->weights ? 4 : 0)) * active_edges + 16 * n_active;
+      const int64_t e_r = all_rows ? m : active_edges, n_r = all_rows ? n : n_active;
+      edges_streamed += e_r;
+      spmv_alg_bytes += (int64_t)(4 + (narrow ? 2 : 4) + (g->weights ? 4 : 0)) * e_r + 16 * n_r;
       streamed = true;
     }
+    aux.need(st, (u64)mask_r + 1, prefix_slots);
     clean_table(table, dirty_mask, slot_of, dirty_first, dirty_count, st);
     dirty_count = 0;
     dirty_mask = mask_r;
@@ -377,7 +456,10 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
   auto queue_compaction = [&](int64_t r) {
     cudaMemsetAsync(scal + kScalActive, 0, 2 * sizeof(u64), st);
     cudaMemsetAsync(scal + kScalActiveHub, 0, sizeof(u64), st);
-    ++g_launches; compact_active_kernel<<<blocks_for(n_active, 256), 256, 0, st>>>(n_active, cur_list, colour, stamp, rep, (int)r, g->row_ptr, kHubThreshold, act[cur], scal + kScalActive, scal + kScalActiveHub);
+    // while the column range check is pending the rows dropped here are checked here (a row kernel never reads them)
+    const bool check = !cols_checked && !merge && !ranged;
+    ++g_launches; compact_active_kernel<<<blocks_for(n_active, 256), 256, 0, st>>>(n_active, cur_list, colour, stamp, rep, (int)r, g->row_ptr, kHubThreshold, act[cur], scal + kScalActive, scal + kScalActiveHub, check ? g->col_idx : nullptr, n_targets, d_err);
+    if (check) dropped_checked = true;
   };
   // host side of a compaction whose counters have been read back; returns true when nothing is left to refine
   auto adopt_compaction = [&]() -> bool {
@@ -408,7 +490,6 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
     // it is harmless; `rounds` and the trajectory stop at the first repeated count exactly as in the per-round mode.
     const bool window = !no_runahead && r > kSyncRounds;
     const int R = window ? (int)std::min<int64_t>(kRunAhead, max_rounds - r + 1) : 1;
-    if (!(k == 1 && uniform_start && r == 1) && (rc = join_aux())) return rc;
     cudaEvent_t e0 = evp.get(2), e2 = evp.get(4);
     cudaEventRecord(e0, st);
     bool streamed[kRunAhead];
@@ -423,6 +504,15 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
     cudaMemcpyAsync(hs, scal, sizeof(u64) * kNumScal, cudaMemcpyDeviceToHost, st);
     rc = check_cuda(cudaStreamSynchronize(st));
     if (rc) return rc;
+    {
+      const u32 e = (u32)hs[kScalErr];  // verdicts of the checks folded into S0 / the first column pass
+      if (e & (kErrRowPtr | kErrCol)) return WL_EINVAL;
+      if (e & kErrRowSum) return WL_ERANGE;
+    }
+    if (uniform_start && r == 1) {
+      num_hub_chunks = (int64_t)hs[kScalHub];
+      active_hubs = num_hub_chunks;
+    }
     float t_all = 0, t_spmv = 0;
     cudaEventElapsedTime(&t_all, e0, e2);
     for (int j = 0; j < R; ++j)
@@ -465,7 +555,13 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
       break;
     }
   }
-  if ((rc = join_aux())) return rc;
+  if (!cols_checked) {  // no round read a column (everything was settled by the degrees): check them now
+    ++g_launches; validate_cols_kernel<<<148 * 8, 256, 0, st>>>(n_targets, edge_first, edge_first + m, g->col_idx, d_err);
+    cudaMemcpyAsync(hs + kScalErr, scal + kScalErr, sizeof(u64), cudaMemcpyDeviceToHost, st);
+    rc = check_cuda(cudaStreamSynchronize(st));
+    if (rc) return rc;
+    if ((u32)hs[kScalErr] & kErrCol) return WL_EINVAL;
+  }
   res->k = k;
   res->rounds = rounds;
   res->edges_streamed = edges_streamed;
@@ -632,6 +728,11 @@ int wl_spmv_round(const wl_csr* g, const int32_t* colors, uint64_t key, uint64_t
     if (rc) return rc;
     a.num_hub_chunks = (int64_t)hs[kScalHub];
     if (narrow) { ++g_launches; narrow_kernel<<<blocks_for(g->n, 256), 256, 0, st>>>(g->n, colors, (unsigned short*)(ws + L.o_colour16)); }
+    if ((flags & WL_FLAG_EDGE_BALANCED) && g->m > 0) {
+      a.eb = true;
+      a.chunk_row = (int*)(ws + L.o_chunk_row);
+      a.n_targets = g->n;
+    }
   }
   launch_spmv(L, *g, a, key, tile_row, (u64*)y, merge, st);
   rc = check_cuda(cudaStreamSynchronize(st));

@@ -134,6 +134,18 @@ def test_batched_device_cap_and_limits():
     assert oracle.is_stable(n, rp, ci, wt, res.colors.numpy())  # every outer iteration ends on a stable colouring
 
 
+@pytest.mark.parametrize("name", ["rmat11_dir", "weighted", "hub"])
+def test_batched_with_edge_balanced_local_rsc(name):
+    """Local RSC through the edge-balanced kernel: batch slices start at arbitrary entry positions (shifted column pointer,
+    unaligned origin) and targets outside V_k are implicit singletons."""
+    g = BATCH_GRAPHS[name]()
+    n, rp, ci, wt = g.numpy()
+    cap = max(1, g.m // 3 + 1)
+    want, k_want, _, _ = oracle.rbsc(n, rp, ci, wt, cap)
+    res = wl.wl_refine_batched(n, g.row_ptr, g.col, g.weights, max_batch_edges=cap, seed=5, flags=wl.WL_FLAG_EDGE_BALANCED)
+    assert res.colors.numpy().tolist() == want.tolist() and res.num_colors == k_want
+
+
 def test_batched_seed_independence():
     g = gg.rmat(10, seed=6, symmetrize=False)
     a = wl.wl_refine_batched(g.n, g.row_ptr, g.col, None, max_batch_edges=g.m // 5, seed=1).colors

@@ -57,7 +57,7 @@ GRAPHS = {
 
 # ------------------------------------------------------------------ S1+S2
 @pytest.mark.parametrize("name", list(GRAPHS))
-@pytest.mark.parametrize("flags", [0, 4, 32])
+@pytest.mark.parametrize("flags", [0, 4, 32, 128, 128 | 32])
 def test_spmv_bit_exact(name, flags):
     g = GRAPHS[name]()
     n, rp, ci, wt = g.numpy()
@@ -67,6 +67,29 @@ def test_spmv_bit_exact(name, flags):
     want = oracle.spmv_u64(n, rp, ci, wt, oracle_w(key, colors))
     dn, drp, dci, dwt = dgraph(g)
     y = wl.wl_spmv_round(dn, drp, dci, dwt, torch.from_numpy(colors).to(dev()), key, flags=flags)
+    assert (u64(y) == want).all()
+
+
+@pytest.mark.parametrize("shift", [1, 2, 3])
+@pytest.mark.parametrize("name", ["rmat12_sym", "hub_20000", "weighted", "empty_rows_mix"])
+def test_spmv_edge_balanced_unaligned_columns(name, shift):
+    """A column array that starts 4, 8 or 12 bytes past a 16-byte boundary (a slice of a larger buffer, as the batched
+    path passes them) must give the same sums; graphs with runs of empty rows and rows crossing chunk borders."""
+    if name == "empty_rows_mix":  # runs of empty rows at the start, in the middle and at the end; rows crossing 2048-entry chunks
+        edges = [(i, (7 * i + j) % 9000) for i in range(100, 4000) for j in range(i % 5)] + \
+                [(5000, j) for j in range(0, 9000, 2)] + [(8000 + i, i) for i in range(50)]
+        g = gg.from_edge_list(9000, edges)
+    else:
+        g = GRAPHS[name]()
+    n, rp, ci, wt = g.numpy()
+    colors = gg.random_partition(n, max(1, n // 4), 5).numpy()
+    key = wl.wl_round_key(77, 3, 9)
+    want = oracle.spmv_u64(n, rp, ci, wt, oracle_w(key, colors))
+    dn, drp, dci, dwt = dgraph(g)
+    pad = torch.zeros(shift, dtype=torch.int32, device=dev())
+    dci2 = torch.cat([pad, dci])[shift:]
+    assert dci2.data_ptr() % 16 == 4 * shift
+    y = wl.wl_spmv_round(dn, drp, dci2, dwt, torch.from_numpy(colors).to(dev()), key, flags=wl.WL_FLAG_EDGE_BALANCED)
     assert (u64(y) == want).all()
 
 
@@ -124,7 +147,7 @@ def test_canonicalize(n):
 
 # ------------------------------------------------------------------ whole Algorithm 1
 @pytest.mark.parametrize("name", list(GRAPHS))
-@pytest.mark.parametrize("flags", [0, 2, 4, 64])
+@pytest.mark.parametrize("flags", [0, 2, 4, 64, 128, 128 | 2])
 def test_refine_equals_oracle(name, flags):
     g = GRAPHS[name]()
     n, rp, ci, wt = g.numpy()
@@ -184,6 +207,12 @@ def test_error_codes():
     with pytest.raises(wl.WlError) as e:
         wl.wl_refine(n, rp, bad)
     assert e.value.code == wl.WL_EINVAL
+    for flags in (wl.WL_FLAG_EDGE_BALANCED, wl.WL_FLAG_NO_PRUNE):
+        bad2 = ci.clone()
+        bad2[-1] = -7
+        with pytest.raises(wl.WlError) as e:
+            wl.wl_refine(n, rp, bad2, flags=flags)
+        assert e.value.code == wl.WL_EINVAL
     bad_rp = rp.clone()
     bad_rp[3] = bad_rp[4] + 1
     with pytest.raises(wl.WlError) as e:
