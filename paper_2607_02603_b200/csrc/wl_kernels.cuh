@@ -203,14 +203,17 @@ __device__ __forceinline__ u64 colour_id(const CT* __restrict__ colour, int j, i
 // S1+S2, default kernel: one warp owns 32 consecutive rows (or 32 entries of the active row list).
 //   * rows with at most kSmallRow entries are summed by their own lane (thread per row, no shuffles, up to kSmallRow
 //     independent gathers in flight per lane);
+//   * rows of up to kMidRow entries are summed four at a time by groups of eight lanes (up to eight gathers in flight
+//     per lane, three-step butterfly per group);
 //   * longer rows are processed one after the other by the whole warp (coalesced column loads, four gathers in flight
-//     per lane, butterfly reduction);
+//     per lane, the last partial step predicated so that its gathers are in flight together, butterfly reduction);
 //   * rows longer than hub_threshold are left to spmv_hub_kernel (y = 0 here).
 // Everything accumulates in registers: the divergent gathers and shared-memory traffic share the LSU pipe, and staging
 // through shared memory (spmv_merge_kernel) more than doubled the time on B200 (profiles/).
 // CT = int or unsigned short (narrow colour ids while k <= 65536: the gathered array is half the size and a 32-byte
 // sector holds 16 nodes; measured 267 vs 125 G gathers/s on the scale-27 access pattern).
 constexpr int kSmallRow = 8;
+constexpr int kMidRow = 64;  // rows up to this length are summed by eight lanes
 
 // clamps a column id that is not a node of [0, n_targets) and remembers that it saw one (VALIDATE: S0's range check)
 template <bool VALIDATE>
@@ -258,6 +261,45 @@ spmv_rows32_kernel(int64_t nrows, const int* __restrict__ rows, const int64_t* _
     }
   }
   unsigned big = __ballot_sync(0xffffffffu, valid && !small && d <= hub_threshold);
+  {
+    // rows of kSmallRow+1 .. kMidRow entries: four at a time, eight lanes each, up to eight gathers in flight per lane
+    unsigned med = __ballot_sync(0xffffffffu, valid && !small && d <= kMidRow);
+    big &= ~med;
+    const int sub = lane & 7, grp = lane >> 3;
+    while (med) {
+      unsigned mm = med;
+      for (int q = 0; q < grp; ++q) mm &= mm - 1;
+      const int src = mm ? __ffs(mm) - 1 : -1;
+#pragma unroll
+      for (int q = 0; q < 4; ++q) med &= med - 1;
+      int64_t ra = __shfl_sync(0xffffffffu, a, src < 0 ? 0 : src), rb = __shfl_sync(0xffffffffu, b, src < 0 ? 0 : src);
+      if (src < 0) ra = rb = 0;
+      int c[kMidRow / 8];
+#pragma unroll
+      for (int t = 0; t < kMidRow / 8; ++t) {
+        const int64_t p = ra + sub + 8 * t;
+        c[t] = p < rb ? checked_col<VALIDATE>(ld_stream_i32(col + p), n_targets, bad) : -1;
+      }
+      u64 s = 0;
+#pragma unroll
+      for (int t = 0; t < kMidRow / 8; ++t) {
+        if (c[t] >= 0) {
+          u64 v = weight_of(key, colour_id<RANGED>(colour, c[t], lo, hi));
+          if (WEIGHTED) v *= (u64)ld_stream_u32(wt + ra + sub + 8 * t);
+          s += v;
+        }
+      }
+      s += __shfl_xor_sync(0xffffffffu, s, 1);
+      s += __shfl_xor_sync(0xffffffffu, s, 2);
+      s += __shfl_xor_sync(0xffffffffu, s, 4);
+#pragma unroll
+      for (int g = 0; g < 4; ++g) {
+        const int sg = __shfl_sync(0xffffffffu, src, g * 8);
+        const u64 vg = __shfl_sync(0xffffffffu, s, g * 8);
+        if (lane == sg) acc = vg;
+      }
+    }
+  }
   while (big) {
     const int src = __ffs(big) - 1;
     big &= big - 1;
@@ -281,10 +323,19 @@ spmv_rows32_kernel(int64_t nrows, const int* __restrict__ rows, const int64_t* _
       }
       s += (v0 + v1) + (v2 + v3);
     }
-    for (; p < rb; p += 32) {
-      u64 v = weight_of(key, colour_id<RANGED>(colour, checked_col<VALIDATE>(ld_stream_i32(col + p), n_targets, bad), lo, hi));
-      if (WEIGHTED) v *= (u64)ld_stream_u32(wt + p);
-      s += v;
+    if (p < rb) {  // fewer than 128 entries left: one predicated step, all gathers in flight together
+      int c[4];
+#pragma unroll
+      for (int t = 0; t < 4; ++t)
+        c[t] = p + 32 * t < rb ? checked_col<VALIDATE>(ld_stream_i32(col + p + 32 * t), n_targets, bad) : -1;
+#pragma unroll
+      for (int t = 0; t < 4; ++t) {
+        if (c[t] >= 0) {
+          u64 v = weight_of(key, colour_id<RANGED>(colour, c[t], lo, hi));
+          if (WEIGHTED) v *= (u64)ld_stream_u32(wt + p + 32 * t);
+          s += v;
+        }
+      }
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
