@@ -73,6 +73,11 @@ typedef struct wl_options {
   int64_t* round_colors;    /* host, optional: number of colours after every round (the trajectory the oracle prints) */
   int32_t round_colors_cap; /* capacity of round_colors                                                              */
   int32_t max_outer_iters;  /* batched only; <= 0: unlimited                                                          */
+  void* host_workspace;     /* batched only, optional: PINNED HOST scratch for the quotient graphs of Alg. 2 line 13 (they
+                               exceed device memory by assumption, L135).  NULL: the library pins its own (first touch of
+                               host pages costs far more than the transfers; callers that refine repeatedly should pass
+                               one).  Caller-owned, contents undefined before and after.                               */
+  size_t host_workspace_bytes; /* wl_refine_batched_host_bytes(n, m) always suffices; a smaller one is ignored          */
 } wl_options;
 
 typedef struct wl_stats {
@@ -170,6 +175,11 @@ typedef struct wl_edge_batch {
 int wl_refine_batched(int64_t n, int32_t num_batches, const wl_edge_batch* batches, const wl_csr* whole, uint64_t seed,
                       size_t device_cap_bytes, int64_t max_batch_edges, int32_t* out_colors, wl_stats* stats,
                       const wl_options* opt, void* cuda_stream);
+
+/* Bytes of pinned host scratch that always suffice for wl_options.host_workspace: two offset arrays of n + 1 entries and
+ * one weighted entry array of m entries (a quotient never has more nodes or entries than its graph, Def. 4; later
+ * quotients overwrite the first one in place). */
+size_t wl_refine_batched_host_bytes(int64_t n, int64_t m);
 
 /* B2: inner-node labels of Def. 5 (L139-L145) by the method of L463.  edge_batch: DEVICE int32[m] batch id of every CSR edge
  * slot; sink_batch: DEVICE int32[n] label given to nodes without out-edges (Q9); label: DEVICE int32[n], -1 = boundary. */

@@ -23,7 +23,7 @@ WL_FLAG_EDGE_BALANCED = 128
 
 EXPORTS = [
     "wl_refine_workspace_bytes", "wl_refine", "wl_refine_host", "wl_round_key", "wl_weight", "wl_spmv_round",
-    "wl_relabel", "wl_canonicalize", "wl_refine_batched", "wl_inner_labels", "wl_quotient",
+    "wl_relabel", "wl_canonicalize", "wl_refine_batched", "wl_refine_batched_host_bytes", "wl_inner_labels", "wl_quotient",
     "wl_quotient_workspace_bytes", "wl_strerror", "wl_last_cuda_error", "wl_version", "wl_kernel_launches",
 ]
 
@@ -44,7 +44,8 @@ class wl_csr(C.Structure):
 
 class wl_options(C.Structure):
     _fields_ = [("flags", C.c_uint32), ("max_rounds", C.c_int32), ("stream_id", C.c_uint64),
-                ("round_colors", C.c_void_p), ("round_colors_cap", C.c_int32), ("max_outer_iters", C.c_int32)]
+                ("round_colors", C.c_void_p), ("round_colors_cap", C.c_int32), ("max_outer_iters", C.c_int32),
+                ("host_workspace", C.c_void_p), ("host_workspace_bytes", C.c_size_t)]
 
 
 class wl_stats(C.Structure):
@@ -91,6 +92,8 @@ def lib():
         L.wl_refine_batched.restype = C.c_int
         L.wl_refine_batched.argtypes = [i64, i32, C.POINTER(wl_edge_batch), C.POINTER(wl_csr), u64, sz, i64, vp,
                                         C.POINTER(wl_stats), C.POINTER(wl_options), vp]
+        L.wl_refine_batched_host_bytes.restype = sz
+        L.wl_refine_batched_host_bytes.argtypes = [i64, i64]
         L.wl_inner_labels.restype = C.c_int
         L.wl_inner_labels.argtypes = [i64, vp, vp, vp, vp, vp]
         L.wl_quotient.restype = C.c_int
@@ -180,7 +183,7 @@ def wl_refine(n: int, row_ptr: torch.Tensor, col_idx: torch.Tensor, weights: Opt
     if workspace is None:
         workspace = torch.empty(max(need, 256), dtype=torch.uint8, device=dev)
     rc_buf = (C.c_int64 * round_cap)()
-    opt = wl_options(flags, max_rounds, stream_id, C.cast(rc_buf, C.c_void_p), round_cap, 0)
+    opt = wl_options(flags, max_rounds, stream_id, C.cast(rc_buf, C.c_void_p), round_cap, 0, None, 0)
     st = wl_stats()
     with torch.cuda.device(dev):
         rc = L.wl_refine(C.byref(g), _ptr(init_colors), seed, _ptr(out), C.byref(st), C.byref(opt), _ptr(workspace),
@@ -204,7 +207,7 @@ def wl_refine_host(n: int, row_ptr: torch.Tensor, col_idx: torch.Tensor, weights
         out = torch.empty(n, dtype=torch.int32, pin_memory=True)
     _check(out, torch.int32, "cpu", "out", n)
     rc_buf = (C.c_int64 * round_cap)()
-    opt = wl_options(flags, max_rounds, 0, C.cast(rc_buf, C.c_void_p), round_cap, 0)
+    opt = wl_options(flags, max_rounds, 0, C.cast(rc_buf, C.c_void_p), round_cap, 0, None, 0)
     st = wl_stats()
     with torch.cuda.device(dev):
         rc = L.wl_refine_host(C.byref(g), _ptr(init_colors), seed, _ptr(out), C.byref(st), C.byref(opt),
@@ -322,7 +325,7 @@ def wl_quotient(n, row_ptr, col_idx, weights, colors: torch.Tensor, k: int):
 def wl_refine_batched(n: int, row_ptr: torch.Tensor, col_idx: torch.Tensor, weights: Optional[torch.Tensor] = None, *,
                       max_batch_edges: int, cuts=None, seed: int = 0, device_cap_bytes: int = 0, flags: int = 0,
                       max_outer_iters: int = 0, out: Optional[torch.Tensor] = None, device=None,
-                      allow_limit: bool = False) -> RefineResult:
+                      allow_limit: bool = False, host_workspace: Optional[torch.Tensor] = None) -> RefineResult:
     """Algorithm 2 over a HOST-resident CSR (pinned recommended).  cuts (optional, increasing edge positions from 0 to m)
     gives the edge partition of the first outer iteration as consecutive CSR slices; otherwise the library cuts by
     max_batch_edges.  Returns canonical colours on the original nodes (host int32[n])."""
@@ -334,7 +337,11 @@ def wl_refine_batched(n: int, row_ptr: torch.Tensor, col_idx: torch.Tensor, weig
     if out is None:
         out = torch.empty(n, dtype=torch.int32)
     _check(out, torch.int32, "cpu", "out", n)
-    opt = wl_options(flags, 0, 0, None, 0, max_outer_iters)
+    if host_workspace is not None:
+        if host_workspace.device.type != "cpu" or not host_workspace.is_pinned() or host_workspace.dtype != torch.uint8:
+            raise ValueError("host_workspace must be a pinned host uint8 tensor")
+    opt = wl_options(flags, 0, 0, None, 0, max_outer_iters, _ptr(host_workspace),
+                     0 if host_workspace is None else host_workspace.numel())
     st = wl_stats()
     nb = 0
     batches = None
@@ -356,6 +363,10 @@ def wl_refine_batched(n: int, row_ptr: torch.Tensor, col_idx: torch.Tensor, weig
     if rc != WL_OK and not (allow_limit and rc == WL_EMAXROUNDS):
         raise WlError(rc, "wl_refine_batched")
     return RefineResult(out, st.num_colors, st.rounds, [], _stats_dict(st), rc)
+
+
+def wl_refine_batched_host_bytes(n: int, m: int) -> int:
+    return int(lib().wl_refine_batched_host_bytes(n, m))
 
 
 def wl_strerror(code: int) -> str:

@@ -15,6 +15,7 @@
 // COO-form (arbitrary) first partitions are not accepted by wl_refine_batched yet (WL_EINVAL); wl_inner_labels covers
 // their Def. 5 mask.
 #include <algorithm>
+#include <chrono>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
@@ -85,37 +86,77 @@ __global__ void rep_lower_bound_kernel(const int* __restrict__ rep_of_block, int
 
 // Quotient, step 1: every entry (i_B, j) of a representative row becomes key (B, H(j)); equal keys meet in one slot whose
 // value accumulates the weights (a'_{B,B'} = sum_{l in B'} a_{i_B,l}, Eq. 1).  Slot = {key + 1 : 64 | weight sum : 64},
-// empty = 0.  The claimer of a slot counts one distinct target for block B.  One warp per row.
+// empty = {0, 0}.  A new key claims its slot together with its first weight by one 128-bit CAS; only a repeated key
+// needs a second atomic (the add).  Returns true when the entry claimed a slot (= one more distinct target for block B).
+__device__ __forceinline__ bool quot_insert_one(Slot* __restrict__ table, u64 mask, int b, int target, u64 weight) {
+  const u64 key1 = (((u64)(u32)b << 32) | (u64)(u32)target) + 1;
+  u64 slot = slot_hash((u32)b, key1) & mask;
+  while (true) {
+    Slot v = load_slot(table + slot);
+    if (v.y == 0) {
+      const Slot empty = {0ull, 0ull}, mine = {key1, weight};
+      v = cas128(table + slot, empty, mine);
+      if (v.y == 0) return true;
+    }
+    if (v.y == key1) {
+      atomicAdd(&table[slot].cx, weight);
+      return false;
+    }
+    slot = (slot + 1) & mask;
+  }
+}
+
+constexpr int kQuotLongRow = 4096;  // longer pieces are left to quot_insert_long_kernel (whole grid per row)
+
+// One warp per row of [row_base, row_base + n_rows); only the representative row of a block contributes (Def. 4, Q17).
+// The piece of the row inside the uploaded edge range [clip_lo, clip_hi) is inserted; pieces longer than kQuotLongRow are
+// queued in long_rows (a single warp would walk a hub row of 10^5-10^6 entries alone).
 __global__ void __launch_bounds__(256)
-quot_insert_kernel(int64_t row_base, int64_t n_rows, const int64_t* __restrict__ row_ptr, const int* __restrict__ col,
-                   const u32* __restrict__ wt, const int* __restrict__ Hc, const int* __restrict__ rep_of_block,
-                   u64* __restrict__ table, u64 table_mask, int* __restrict__ cnt) {
+quot_insert_kernel(int64_t row_base, int64_t n_rows, const int64_t* __restrict__ row_ptr, int64_t clip_lo, int64_t clip_hi,
+                   const int* __restrict__ col, const u32* __restrict__ wt, const int* __restrict__ Hc,
+                   const int* __restrict__ rep_of_block, Slot* __restrict__ table, u64 table_mask, int* __restrict__ cnt,
+                   int* __restrict__ long_rows, u32* __restrict__ long_count) {
   const int lane = threadIdx.x & 31;
   const int64_t w = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   if (w >= n_rows) return;
   const int64_t i = row_base + w;
   const int b = Hc[i];
   if (rep_of_block[b] != (int)i) return;
-  const int64_t a = row_ptr[w], e = row_ptr[w + 1];
-  for (int64_t p = a + lane; p < e; p += 32) {
-    const u64 key = (((u64)(u32)b << 32) | (u64)(u32)Hc[col[p]]) + 1;
-    const u64 weight = wt ? (u64)wt[p] : 1ull;
-    u64 slot = slot_hash((u32)b, key) & table_mask;
-    while (true) {
-      u64 cur = table[2 * slot];
-      if (cur == 0) {
-        cur = atomicCAS(table + 2 * slot, 0ull, key);
-        if (cur == 0) {
-          atomicAdd(cnt + b, 1);
-          cur = key;
-        }
-      }
-      if (cur == key) {
-        atomicAdd(table + 2 * slot + 1, weight);
-        break;
-      }
-      slot = (slot + 1) & table_mask;
-    }
+  int64_t a = row_ptr[w], e = row_ptr[w + 1];
+  if (a < clip_lo) a = clip_lo;
+  if (e > clip_hi) e = clip_hi;
+  if (e - a > kQuotLongRow) {
+    if (lane == 0) long_rows[atomicAdd(long_count, 1u)] = (int)w;
+    return;
+  }
+  int fresh = 0;
+  for (int64_t p = a + lane; p < e; p += 32)
+    fresh += quot_insert_one(table, table_mask, b, Hc[col[p]], wt ? (u64)wt[p] : 1ull) ? 1 : 0;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) fresh += __shfl_xor_sync(0xffffffffu, fresh, o);
+  if (lane == 0 && fresh) atomicAdd(cnt + b, fresh);
+}
+
+// the queued long pieces, one after the other, each spread over the whole grid
+__global__ void __launch_bounds__(256)
+quot_insert_long_kernel(int64_t row_base, const int64_t* __restrict__ row_ptr, int64_t clip_lo, int64_t clip_hi,
+                        const int* __restrict__ col, const u32* __restrict__ wt, const int* __restrict__ Hc,
+                        Slot* __restrict__ table, u64 table_mask, int* __restrict__ cnt,
+                        const int* __restrict__ long_rows, const u32* __restrict__ long_count) {
+  const u32 n_long = *long_count;
+  const int64_t tid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x, stride = (int64_t)gridDim.x * blockDim.x;
+  for (u32 j = 0; j < n_long; ++j) {
+    const int64_t w = long_rows[j];
+    const int b = Hc[row_base + w];
+    int64_t a = row_ptr[w], e = row_ptr[w + 1];
+    if (a < clip_lo) a = clip_lo;
+    if (e > clip_hi) e = clip_hi;
+    int fresh = 0;
+    for (int64_t p = a + tid; p < e; p += stride)
+      fresh += quot_insert_one(table, table_mask, b, Hc[col[p]], wt ? (u64)wt[p] : 1ull) ? 1 : 0;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) fresh += __shfl_xor_sync(0xffffffffu, fresh, o);
+    if ((threadIdx.x & 31) == 0 && fresh) atomicAdd(cnt + b, fresh);
   }
 }
 
@@ -233,6 +274,51 @@ struct DevBuf {
   T* as() const { return (T*)p; }
 };
 
+// Pinned host storage of the quotient graphs (Alg. 2 line 13): two offset arrays (the graph being read and the quotient
+// being written) and ONE array pair for the weighted entries.  The first quotient is written while the caller's graph is
+// streamed; every later quotient overwrites its predecessor in place: its rows come out in the order of its graph's
+// rows and never hold more entries (Def. 4), so the write position never passes the position the streaming pass has
+// already uploaded.
+struct HostQuot {
+  char* base = nullptr;
+  bool owned = false;
+  int64_t* rp[2] = {nullptr, nullptr};
+  int* col = nullptr;
+  u32* wt = nullptr;
+  int64_t cap_nodes = 0, cap_edges = 0;
+  static size_t bytes_for(int64_t n, int64_t m) {
+    return 2 * align_up(sizeof(int64_t) * (size_t)(n + 1)) + 2 * align_up(sizeof(int) * (size_t)m);
+  }
+  int init(int64_t n, int64_t m, void* ws, size_t ws_bytes) {
+    if (base) return WL_OK;
+    const size_t need = bytes_for(n, m);
+    if (ws && ws_bytes >= need) {
+      base = (char*)ws;
+    } else {
+      if (cudaHostAlloc((void**)&base, need, cudaHostAllocDefault) != cudaSuccess) {
+        cudaGetLastError();
+        base = nullptr;
+        return WL_ENOMEM;
+      }
+      owned = true;
+    }
+    size_t off = 0;
+    rp[0] = (int64_t*)(base + off);
+    off += align_up(sizeof(int64_t) * (size_t)(n + 1));
+    rp[1] = (int64_t*)(base + off);
+    off += align_up(sizeof(int64_t) * (size_t)(n + 1));
+    col = (int*)(base + off);
+    off += align_up(sizeof(int) * (size_t)m);
+    wt = (u32*)(base + off);
+    cap_nodes = n;
+    cap_edges = m;
+    return WL_OK;
+  }
+  ~HostQuot() {
+    if (owned && base) cudaFreeHost(base);
+  }
+};
+
 // exclusive scan of cnt[0..n) into out[0..n] starting at base_off (device arrays); bsum: ceil(n / kScanC) + 1 u64
 static void launch_scan32(const int* cnt, int64_t n, int64_t base_off, int64_t* out, u64* bsum, u64* total,
                           cudaStream_t st) {
@@ -241,6 +327,17 @@ static void launch_scan32(const int* cnt, int64_t n, int64_t base_off, int64_t* 
   ++g_launches; scan32_sum_kernel<<<(unsigned)nb, kScanT, 0, st>>>(cnt, n, bsum);
   ++g_launches; scan64_serial_kernel<<<1, 32, 0, st>>>(bsum, nb, total);
   ++g_launches; scan32_apply_kernel<<<(unsigned)nb, kScanT, 0, st>>>(cnt, n, bsum, base_off, out);
+}
+
+// step 1 of the quotient for the rows [row_base, row_base + n_rows) whose offsets are row_ptr[0..n_rows]; long_rows needs
+// (clip_hi - clip_lo) / kQuotLongRow + 2 ints, *long_count is zeroed here
+static void launch_quot_insert(int64_t row_base, int64_t n_rows, const int64_t* row_ptr, int64_t clip_lo, int64_t clip_hi,
+                               const int* col, const u32* wt, const int* Hc, const int* rep_of_block, u64* table,
+                               u64 table_mask, int* cnt, int* long_rows, u32* long_count, cudaStream_t st) {
+  if (n_rows <= 0) return;
+  cudaMemsetAsync(long_count, 0, sizeof(u32), st);
+  ++g_launches; quot_insert_kernel<<<blocks_for(n_rows * 32, 256), 256, 0, st>>>(row_base, n_rows, row_ptr, clip_lo, clip_hi, col, wt, Hc, rep_of_block, (Slot*)table, table_mask, cnt, long_rows, long_count);
+  ++g_launches; quot_insert_long_kernel<<<148 * 8, 256, 0, st>>>(row_base, row_ptr, clip_lo, clip_hi, col, wt, Hc, (Slot*)table, table_mask, cnt, long_rows, long_count);
 }
 
 static u64 quot_table_slots(int64_t entries) {
@@ -297,6 +394,11 @@ int wl_inner_labels(int64_t n, const int64_t* row_ptr, const int32_t* edge_batch
   return check_cuda(cudaGetLastError());
 }
 
+size_t wl_refine_batched_host_bytes(int64_t n, int64_t m) {
+  if (n < 0 || m < 0 || n > kMaxNodes) return 0;
+  return HostQuot::bytes_for(n, m);
+}
+
 size_t wl_quotient_workspace_bytes(int64_t n, int64_t m) {
   if (n < 0 || m < 0 || n > kMaxNodes) return 0;
   size_t off = 0;
@@ -304,6 +406,7 @@ size_t wl_quotient_workspace_bytes(int64_t n, int64_t m) {
   off += align_up(sizeof(int) * (size_t)n) * 3;  // rep_of_block, cnt, cursor (k <= n)
   off += align_up(sizeof(u64) * (size_t)((n + kScanC - 1) / kScanC + 2));
   off += 256;
+  off += align_up(sizeof(int) * (size_t)(m / kQuotLongRow + 2));  // queue of long rows
   return off;
 }
 
@@ -332,12 +435,15 @@ int wl_quotient(const wl_csr* g, const int32_t* colors, int64_t k, int64_t* q_ro
   u64* bsum = (u64*)(ws + off);
   off += align_up(sizeof(u64) * (size_t)((n + kScanC - 1) / kScanC + 2));
   u64* total = (u64*)(ws + off);
+  off += 256;
+  int* long_rows = (int*)(ws + off);
   cudaMemsetAsync(table, 0, sizeof(u64) * 2 * slots, st);
   cudaMemsetAsync(rep_of_block, 0x7f, sizeof(int) * (size_t)k, st);
   cudaMemsetAsync(cnt, 0, sizeof(int) * (size_t)k, st);
   cudaMemsetAsync(cursor, 0, sizeof(int) * (size_t)k, st);
   ++g_launches; block_rep_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, colors, rep_of_block);
-  ++g_launches; quot_insert_kernel<<<blocks_for(n * 32, 256), 256, 0, st>>>(0, n, g->row_ptr, g->col_idx, g->weights, colors, rep_of_block, table, slots - 1, cnt);
+  launch_quot_insert(0, n, g->row_ptr, 0, m, g->col_idx, g->weights, colors, rep_of_block, table, slots - 1, cnt, long_rows,
+                     (u32*)(total + 1), st);
   launch_scan32(cnt, k, 0, q_row_ptr, bsum, total, st);
   u64 h_total = 0;
   cudaMemcpyAsync(&h_total, total, sizeof(u64), cudaMemcpyDeviceToHost, st);
@@ -407,31 +513,43 @@ int wl_refine_batched(int64_t n, int32_t num_batches, const wl_edge_batch* batch
 
   u64* hs = host_scal();
   if (!hs) return WL_ECUDA;
-  cudaStream_t copy_st;
+  cudaStream_t copy_st, down_st;  // host -> device uploads; device -> host return of quotient rows
   if (cudaStreamCreateWithFlags(&copy_st, cudaStreamNonBlocking) != cudaSuccess) return check_cuda(cudaGetLastError());
-  cudaEvent_t ev_begin, ev_end, ev_up[2];
+  if (cudaStreamCreateWithFlags(&down_st, cudaStreamNonBlocking) != cudaSuccess) {
+    cudaStreamDestroy(copy_st);
+    return check_cuda(cudaGetLastError());
+  }
+  cudaEvent_t ev_begin, ev_end, ev_up[2], ev_ins[2], ev_emit[2], ev_down[2];
   cudaEventCreate(&ev_begin);
   cudaEventCreate(&ev_end);
-  cudaEventCreateWithFlags(&ev_up[0], cudaEventDisableTiming);
-  cudaEventCreateWithFlags(&ev_up[1], cudaEventDisableTiming);
+  for (int b = 0; b < 2; ++b) {
+    cudaEventCreateWithFlags(&ev_up[b], cudaEventDisableTiming);
+    cudaEventCreateWithFlags(&ev_ins[b], cudaEventDisableTiming);
+    cudaEventCreateWithFlags(&ev_emit[b], cudaEventDisableTiming);
+    cudaEventCreateWithFlags(&ev_down[b], cudaEventDisableTiming);
+  }
   cudaEventRecord(ev_begin, st);
   auto cleanup = [&]() {
+    cudaStreamSynchronize(copy_st);
+    cudaStreamSynchronize(down_st);
     cudaEventDestroy(ev_begin);
     cudaEventDestroy(ev_end);
-    cudaEventDestroy(ev_up[0]);
-    cudaEventDestroy(ev_up[1]);
+    for (int b = 0; b < 2; ++b) {
+      cudaEventDestroy(ev_up[b]);
+      cudaEventDestroy(ev_ins[b]);
+      cudaEventDestroy(ev_emit[b]);
+      cudaEventDestroy(ev_down[b]);
+    }
     cudaStreamDestroy(copy_st);
+    cudaStreamDestroy(down_st);
   };
 
   const int64_t n0 = n;
   size_t used = 0;
   DevBuf d_map0;  // original node -> node of the current graph (identity in iteration 1: left unallocated until needed)
   bool map0_identity = true;
-  // quotient graphs of later iterations live in these host vectors
-  std::vector<int64_t> q_rp[2];
-  std::vector<int> q_col[2];
-  std::vector<u32> q_wt[2];
-  int qsel = 0;
+  HostQuot hq;  // quotient graphs of later iterations (pinned host memory)
+  const int64_t rp0_edges = rp[n];
 
   int64_t n_t = n;
   int outer = 0;
@@ -443,6 +561,16 @@ int wl_refine_batched(int64_t n, int32_t num_batches, const wl_edge_batch* batch
   int rc = WL_OK;
   bool hit_limit = false;
 
+  const bool debug = std::getenv("WL_DEBUG") != nullptr;
+  auto wall = [] { return std::chrono::duration<double>(std::chrono::steady_clock::now().time_since_epoch()).count(); };
+  double t_mark = wall();
+  auto phase = [&](const char* what) {  // WL_DEBUG: host wall-clock per phase (each phase ends on a synchronised stream)
+    if (!debug) return;
+    cudaStreamSynchronize(st);
+    const double t = wall();
+    std::fprintf(stderr, "[wl_refine_batched] outer %d %-22s %9.3f ms\n", outer, what, 1e3 * (t - t_mark));
+    t_mark = t;
+  };
   while (true) {
     ++outer;
     const int nb = (int)cuts.size() - 1;
@@ -462,7 +590,7 @@ int wl_refine_batched(int64_t n, int32_t num_batches, const wl_edge_batch* batch
     // ---- device memory of this outer iteration ---------------------------------------------------------------------
     size_t used_iter = used;
     DevBuf d_H, d_Hc, d_first, d_cof, d_bsum, d_ws, d_col[2], d_wt[2], d_rp[2], d_rep, d_cnt, d_cursor, d_qrp, d_qtab,
-        d_qcol, d_qwt, d_sbsum, d_misc;
+        d_qcol[2], d_qwt[2], d_sbsum, d_misc, d_query, d_long;
     const int64_t nscan = (n_t + kCanonChunk - 1) / kCanonChunk;
 #define WL_ALLOC(buf, bytes)                                   \
   if ((rc = buf.alloc((bytes), &used_iter, device_cap_bytes))) \
@@ -476,7 +604,7 @@ int wl_refine_batched(int64_t n, int32_t num_batches, const wl_edge_batch* batch
     for (int b = 0; b < 2; ++b) {
       WL_ALLOC(d_col[b], sizeof(int) * (size_t)max_edges);
       if (weighted) WL_ALLOC(d_wt[b], sizeof(u32) * (size_t)max_edges);
-      WL_ALLOC(d_rp[b], sizeof(int64_t) * (size_t)(max_rows + 2));
+      WL_ALLOC(d_rp[b], sizeof(int64_t) * (size_t)(max_rows + 4));  // the quotient pass adds the rows cut at either end
     }
     WL_ALLOC(d_misc, 4096);
     if (rc) break;
@@ -484,8 +612,8 @@ int wl_refine_batched(int64_t n, int32_t num_batches, const wl_edge_batch* batch
     auto upload_batch = [&](int k, int buf, bool rows_all) {
       // rows_all: the quotient pass needs every row that starts inside the batch's node range (incl. a crossing one)
       const int64_t c0 = cuts[k], c1 = cuts[k + 1];
-      const int* hc = (outer == 1) ? batch_col(k) : q_col[qsel].data() + c0;
-      const u32* hw = (outer == 1) ? batch_wt(k) : q_wt[qsel].data() + c0;
+      const int* hc = (outer == 1) ? batch_col(k) : hq.col + c0;
+      const u32* hw = (outer == 1) ? batch_wt(k) : hq.wt + c0;
       if (c1 > c0) {
         cudaMemcpyAsync(d_col[buf].p, hc, sizeof(int) * (size_t)(c1 - c0), cudaMemcpyHostToDevice, copy_st);
         bytes_h2d += sizeof(int) * (c1 - c0);
@@ -501,6 +629,7 @@ int wl_refine_batched(int64_t n, int32_t num_batches, const wl_edge_batch* batch
       cudaEventRecord(ev_up[buf], copy_st);
     };
 
+    phase("alloc");
     // ---- Alg. 2 lines 7-11: local refinement per batch, merge ---------------------------------------------------------
     int64_t base_id = 0;
     cudaStreamSynchronize(st);  // buffers of the previous iteration are free
@@ -520,6 +649,7 @@ int wl_refine_batched(int64_t n, int32_t num_batches, const wl_edge_batch* batch
       lg.weights = weighted ? d_wt[buf].as<u32>() - cuts[k] : nullptr;
       wl_options lo{};
       lo.flags = flags & (WL_FLAG_NO_VALIDATE | WL_FLAG_NO_PRUNE | WL_FLAG_EDGE_BALANCED);
+      if (outer > 1) lo.flags |= WL_FLAG_NO_VALIDATE;  // a quotient made by this library is well formed and keeps row sums (L447)
       lo.max_rounds = opt ? opt->max_rounds : 0;
       lo.stream_id = ((u64)outer << 32) | (u64)(u32)k;
       const Layout L = make_layout(nr, lg.m);
@@ -537,6 +667,7 @@ int wl_refine_batched(int64_t n, int32_t num_batches, const wl_edge_batch* batch
       rc = check_cuda(cudaStreamSynchronize(st));  // the workspace and this buffer are reused by the next batch
     }
     if (rc) break;
+    phase("local refinement");
     // ---- Alg. 2 lines 11-12: boundary nodes become singletons ---------------------------------------------------------
     std::vector<int> bnodes, bids;
     {
@@ -584,7 +715,13 @@ int wl_refine_batched(int64_t n, int32_t num_batches, const wl_edge_batch* batch
       break;
     }
 
+    phase("merge + canonical");
     // ---- Alg. 2 line 13: quotient (Def. 4), second streaming pass -------------------------------------------------------
+    // Three streams: copy_st uploads batch k + 1 while st inserts / emits batch k and down_st returns the rows emitted for
+    // batch k - 1 to the host (double buffers on both sides; one host synchronisation per batch, to learn the emitted size).
+    if ((rc = hq.init(n0, rp0_edges, opt ? opt->host_workspace : nullptr, opt ? opt->host_workspace_bytes : 0))) break;
+    const int osel = outer & 1;  // offsets of the quotient being written; the graph being read uses the other array
+    int64_t* nrp = hq.rp[osel];
     WL_ALLOC(d_rep, sizeof(int) * (size_t)K);
     WL_ALLOC(d_cnt, sizeof(int) * (size_t)K);
     WL_ALLOC(d_cursor, sizeof(int) * (size_t)K);
@@ -594,11 +731,16 @@ int wl_refine_batched(int64_t n, int32_t num_batches, const wl_edge_batch* batch
       const int64_t r = (std::upper_bound(rp, rp + n_t + 1, cuts[k]) - rp) - 1;
       if (r >= 0 && r < n_t && rp[r] < cuts[k]) longest_cut_row = std::max(longest_cut_row, rp[r + 1] - rp[r]);
     }
-    const u64 qslots = quot_table_slots(max_edges + longest_cut_row);
+    const int64_t out_cap = max_edges + longest_cut_row;  // entries one emission can hold
+    const u64 qslots = quot_table_slots(out_cap);
     WL_ALLOC(d_qtab, sizeof(u64) * 2 * qslots);
-    WL_ALLOC(d_qcol, sizeof(int) * (size_t)max_edges);
-    WL_ALLOC(d_qwt, sizeof(u32) * (size_t)max_edges);
+    for (int b = 0; b < 2; ++b) {
+      WL_ALLOC(d_qcol[b], sizeof(int) * (size_t)out_cap);
+      WL_ALLOC(d_qwt[b], sizeof(u32) * (size_t)out_cap);
+    }
     WL_ALLOC(d_sbsum, sizeof(u64) * (size_t)((K + kScanC - 1) / kScanC + 2));
+    WL_ALLOC(d_query, sizeof(int64_t) * 2 * (size_t)nb);
+    WL_ALLOC(d_long, sizeof(int) * (size_t)(max_edges / kQuotLongRow + 2));
     if (rc) break;
 #undef WL_ALLOC
     cudaMemsetAsync(d_rep.p, 0x7f, sizeof(int) * (size_t)K, st);
@@ -606,94 +748,94 @@ int wl_refine_batched(int64_t n, int32_t num_batches, const wl_edge_batch* batch
     cudaMemsetAsync(d_cursor.p, 0, sizeof(int) * (size_t)K, st);
     cudaMemsetAsync(d_qtab.p, 0, sizeof(u64) * 2 * qslots, st);
     ++g_launches; block_rep_kernel<<<blocks_for(n_t, 256), 256, 0, st>>>(n_t, d_Hc.as<int>(), d_rep.as<int>());
-    int64_t* d_queries = (int64_t*)((char*)d_misc.p + 256);
-    int64_t* d_answers = (int64_t*)((char*)d_misc.p + 2048);
-    std::vector<int64_t>& nrp = q_rp[qsel ^ 1];
-    std::vector<int>& ncol = q_col[qsel ^ 1];
-    std::vector<u32>& nwt = q_wt[qsel ^ 1];
-    nrp.assign((size_t)K + 1, 0);
-    ncol.clear();
-    nwt.clear();
-    int64_t q_off = 0, emitted_blocks = 0;
-    // rows that cross a cut are uploaded in pieces: the piece of batch k is attributed to the node that owns it
-    for (int k = 0; k < nb && !rc; ++k) {
-      // upload the edge range of the batch plus the (clipped) row offsets of ALL nodes whose row intersects it
+    // per batch: the nodes whose row intersects it, and the number of blocks whose representative row is complete after it
+    std::vector<int64_t> na(nb), nz(nb), done_nodes(nb), done_blocks(nb);
+    for (int k = 0; k < nb; ++k) {
       const int64_t c0 = cuts[k], c1 = cuts[k + 1];
-      size_t dummy = 0;
-      // nodes intersecting [c0, c1): from the node containing c0 to the node containing c1 - 1
-      int64_t na = (std::upper_bound(rp, rp + n_t + 1, c0) - rp) - 1;
-      int64_t nz = c1 > c0 ? (std::upper_bound(rp, rp + n_t + 1, c1 - 1) - rp) : na;
-      if (na < 0) na = 0;
-      if (nz > n_t) nz = n_t;
-      if (c1 == c0) continue;
-      const int* hc = (outer == 1) ? batch_col(k) : q_col[qsel].data() + c0;
-      const u32* hw = (outer == 1) ? batch_wt(k) : q_wt[qsel].data() + c0;
-      cudaMemcpyAsync(d_col[0].p, hc, sizeof(int) * (size_t)(c1 - c0), cudaMemcpyHostToDevice, st);
-      bytes_h2d += sizeof(int) * (c1 - c0);
-      if (weighted) {
-        cudaMemcpyAsync(d_wt[0].p, hw, sizeof(u32) * (size_t)(c1 - c0), cudaMemcpyHostToDevice, st);
-        bytes_h2d += sizeof(u32) * (c1 - c0);
+      na[k] = std::max<int64_t>(0, (std::upper_bound(rp, rp + n_t + 1, c0) - rp) - 1);
+      nz[k] = c1 > c0 ? std::min<int64_t>(n_t, std::upper_bound(rp, rp + n_t + 1, c1 - 1) - rp) : na[k];
+      done_nodes[k] = k == nb - 1 ? n_t : (std::upper_bound(rp + 1, rp + n_t + 1, c1) - (rp + 1));  // rp[i + 1] <= c1
+    }
+    cudaMemcpyAsync(d_query.p, done_nodes.data(), sizeof(int64_t) * (size_t)nb, cudaMemcpyHostToDevice, st);
+    ++g_launches; rep_lower_bound_kernel<<<blocks_for(nb, 128), 128, 0, st>>>(d_rep.as<int>(), K, d_query.as<int64_t>(), nb, d_query.as<int64_t>() + nb);
+    cudaMemcpyAsync(done_blocks.data(), d_query.as<int64_t>() + nb, sizeof(int64_t) * (size_t)nb, cudaMemcpyDeviceToHost, st);
+    rc = check_cuda(cudaStreamSynchronize(st));
+    if (rc) break;
+    auto upload_quot = [&](int k, int buf) {
+      const int64_t c0 = cuts[k], c1 = cuts[k + 1];
+      if (c1 > c0) {
+        const int* hc = (outer == 1) ? batch_col(k) : hq.col + c0;
+        const u32* hw = (outer == 1) ? batch_wt(k) : hq.wt + c0;
+        cudaMemcpyAsync(d_col[buf].p, hc, sizeof(int) * (size_t)(c1 - c0), cudaMemcpyHostToDevice, copy_st);
+        bytes_h2d += sizeof(int) * (c1 - c0);
+        if (weighted) {
+          cudaMemcpyAsync(d_wt[buf].p, hw, sizeof(u32) * (size_t)(c1 - c0), cudaMemcpyHostToDevice, copy_st);
+          bytes_h2d += sizeof(u32) * (c1 - c0);
+        }
+        cudaMemcpyAsync(d_rp[buf].p, rp + na[k], sizeof(int64_t) * (size_t)(nz[k] - na[k] + 1), cudaMemcpyHostToDevice, copy_st);
+        bytes_h2d += sizeof(int64_t) * (nz[k] - na[k] + 1);
       }
-      // clipped row offsets for nodes na..nz
-      std::vector<int64_t> clip((size_t)(nz - na + 1));
-      for (int64_t i = na; i <= nz; ++i) clip[(size_t)(i - na)] = std::min(std::max(rp[i], c0), c1);
-      DevBuf d_clip;
-      if ((rc = d_clip.alloc(sizeof(int64_t) * clip.size(), &dummy, 0))) break;
-      cudaMemcpyAsync(d_clip.p, clip.data(), sizeof(int64_t) * clip.size(), cudaMemcpyHostToDevice, st);
-      bytes_h2d += sizeof(int64_t) * clip.size();
-      ++g_launches; quot_insert_kernel<<<blocks_for((nz - na) * 32, 256), 256, 0, st>>>(na, nz - na, d_clip.as<int64_t>(), d_col[0].as<int>() - c0, weighted ? d_wt[0].as<u32>() - c0 : nullptr, d_Hc.as<int>(), d_rep.as<int>(), d_qtab.as<u64>(), qslots - 1, d_cnt.as<int>());
-      rc = check_cuda(cudaStreamSynchronize(st));  // clip (host vector) and d_clip are released at the end of the scope
-      if (rc) break;
+      cudaEventRecord(ev_up[buf], copy_st);
+    };
+    int64_t q_off = 0, emitted_blocks = 0;
+    int n_emit = 0;
+    upload_quot(0, 0);
+    for (int k = 0; k < nb && !rc; ++k) {
+      const int buf = k & 1;
+      const int64_t c0 = cuts[k], c1 = cuts[k + 1];
+      if (k + 1 < nb) {
+        if (k >= 1) cudaStreamWaitEvent(copy_st, ev_ins[buf ^ 1], 0);  // batch k - 1 has been read out of that buffer
+        upload_quot(k + 1, buf ^ 1);
+      }
+      cudaStreamWaitEvent(st, ev_up[buf], 0);
+      if (c1 > c0 && nz[k] > na[k]) {
+        // rows that cross a cut arrive in pieces: the kernel clips every row to [c0, c1)
+        launch_quot_insert(na[k], nz[k] - na[k], d_rp[buf].as<int64_t>(), c0, c1, d_col[buf].as<int>() - c0,
+                           weighted ? d_wt[buf].as<u32>() - c0 : nullptr, d_Hc.as<int>(), d_rep.as<int>(), d_qtab.as<u64>(),
+                           qslots - 1, d_cnt.as<int>(), d_long.as<int>(), (u32*)(d_misc.as<u64>() + 16), st);
+      }
+      cudaEventRecord(ev_ins[buf], st);
       // a representative row that continues into the next batch is completed there: emit the blocks whose representative
       // row ends at or before c1 and that were not emitted yet
-      int64_t done_nodes = (std::upper_bound(rp + 1, rp + n_t + 1, c1) - (rp + 1));  // nodes with rp[i+1] <= c1
-      if (k == nb - 1) done_nodes = n_t;
-      int64_t done_blocks = 0;
-      cudaMemcpyAsync(d_queries, &done_nodes, sizeof(int64_t), cudaMemcpyHostToDevice, st);
-      ++g_launches; rep_lower_bound_kernel<<<1, 32, 0, st>>>(d_rep.as<int>(), K, d_queries, 1, d_answers);
-      cudaMemcpyAsync(&done_blocks, d_answers, sizeof(int64_t), cudaMemcpyDeviceToHost, st);
-      rc = check_cuda(cudaStreamSynchronize(st));
-      if (rc) break;
-      const int64_t b_lo = emitted_blocks, b_hi = done_blocks;
+      const int64_t b_lo = emitted_blocks, b_hi = done_blocks[k];
       if (b_hi > b_lo) {
         launch_scan32(d_cnt.as<int>() + b_lo, b_hi - b_lo, q_off, d_qrp.as<int64_t>() + b_lo, d_sbsum.as<u64>(),
                       d_misc.as<u64>() + 8, st);
-        u64 tot = 0;
-        cudaMemcpyAsync(&tot, d_misc.as<u64>() + 8, sizeof(u64), cudaMemcpyDeviceToHost, st);
+        cudaMemcpyAsync(hs + kNumScal + 1, d_misc.as<u64>() + 8, sizeof(u64), cudaMemcpyDeviceToHost, st);
         rc = check_cuda(cudaStreamSynchronize(st));
         if (rc) break;
-        // emit needs room for `tot` entries: the output buffers hold max_edges; finished rows may include a carried one
-        DevBuf d_oc, d_ow;
-        int* oc = d_qcol.as<int>();
-        u32* ow = d_qwt.as<u32>();
-        if ((int64_t)tot > max_edges) {
-          if ((rc = d_oc.alloc(sizeof(int) * (size_t)tot, &dummy, 0))) break;
-          if ((rc = d_ow.alloc(sizeof(u32) * (size_t)tot, &dummy, 0))) break;
-          oc = d_oc.as<int>();
-          ow = d_ow.as<u32>();
+        const int64_t tot = (int64_t)hs[kNumScal + 1];
+        if (tot > out_cap || q_off + tot > hq.cap_edges || b_hi > hq.cap_nodes) {
+          rc = WL_ECUDA;  // unreachable: a quotient has at most the entries and nodes of its graph
+          break;
         }
-        ++g_launches; quot_emit_kernel<<<blocks_for((int64_t)qslots, 256), 256, 0, st>>>(d_qtab.as<u64>(), qslots, d_qrp.as<int64_t>(), q_off, d_cursor.as<int>(), oc, ow, (int)b_lo, (int)b_hi);
-        ncol.resize((size_t)(q_off + (int64_t)tot));
-        nwt.resize((size_t)(q_off + (int64_t)tot));
+        const int ob = n_emit & 1;
+        if (n_emit >= 2) cudaStreamWaitEvent(st, ev_down[ob], 0);  // the rows emitted two emissions ago are on the host
+        ++n_emit;
+        ++g_launches; quot_emit_kernel<<<blocks_for((int64_t)qslots, 256), 256, 0, st>>>(d_qtab.as<u64>(), qslots, d_qrp.as<int64_t>(), q_off, d_cursor.as<int>(), d_qcol[ob].as<int>(), d_qwt[ob].as<u32>(), (int)b_lo, (int)b_hi);
+        cudaEventRecord(ev_emit[ob], st);
+        cudaStreamWaitEvent(down_st, ev_emit[ob], 0);
+        // in place from the second quotient on: q_off + tot <= c1, and everything below c1 has been uploaded already
         if (tot) {
-          cudaMemcpyAsync(ncol.data() + q_off, oc, sizeof(int) * (size_t)tot, cudaMemcpyDeviceToHost, st);
-          cudaMemcpyAsync(nwt.data() + q_off, ow, sizeof(u32) * (size_t)tot, cudaMemcpyDeviceToHost, st);
-          bytes_d2h += (sizeof(int) + sizeof(u32)) * (int64_t)tot;
+          cudaMemcpyAsync(hq.col + q_off, d_qcol[ob].p, sizeof(int) * (size_t)tot, cudaMemcpyDeviceToHost, down_st);
+          cudaMemcpyAsync(hq.wt + q_off, d_qwt[ob].p, sizeof(u32) * (size_t)tot, cudaMemcpyDeviceToHost, down_st);
+          bytes_d2h += (sizeof(int) + sizeof(u32)) * tot;
         }
-        cudaMemcpyAsync(nrp.data() + b_lo, d_qrp.as<int64_t>() + b_lo, sizeof(int64_t) * (size_t)(b_hi - b_lo + 1),
-                        cudaMemcpyDeviceToHost, st);
+        cudaMemcpyAsync(nrp + b_lo, d_qrp.as<int64_t>() + b_lo, sizeof(int64_t) * (size_t)(b_hi - b_lo + 1),
+                        cudaMemcpyDeviceToHost, down_st);
         bytes_d2h += sizeof(int64_t) * (b_hi - b_lo + 1);
-        rc = check_cuda(cudaStreamSynchronize(st));
-        if (rc) break;
-        q_off += (int64_t)tot;
+        cudaEventRecord(ev_down[ob], down_st);
+        q_off += tot;
         emitted_blocks = b_hi;
       }
     }
+    if (!rc) rc = check_cuda(cudaStreamSynchronize(down_st));
+    if (!rc) rc = check_cuda(cudaStreamSynchronize(st));
     if (rc) break;
     nrp[(size_t)K] = q_off;
+    phase("quotient");
     // ---- next outer iteration on the quotient ---------------------------------------------------------------------------
-    qsel ^= 1;
-    rp = q_rp[qsel].data();
+    rp = nrp;
     n_t = K;
     weighted = true;
     const int64_t next_nb_cap = max_batch_edges;
