@@ -29,6 +29,8 @@ if ROOT not in sys.path:
 RMAT_SEEDS = {22: 1, 27: 2, 30: 3}  # BASELINE.json configs[2..4]
 ORACLE_SAMPLE_SCALE = 21           # bounded sample of the same recipe for the CPU oracle (about 10-30 s)
 HBM_FALLBACK_GBS = 6650.0          # /opt/skills/guides/B200_PROFILING.md fallback
+# DRAM bytes of the dominant launch (round-2 row kernel 40.70 + 0.74 GB, hub kernel 8.49 + 0.005 GB), ncu --set full
+NCU_TRAFFIC_BYTES = 49.94e9
 
 
 def measured_peaks():
@@ -135,6 +137,60 @@ def run_reference(args):
     return 0
 
 
+def run_batched(args):
+    """--workload batched: Algorithm 2 (RBSC) over a HOST-resident directed R-MAT graph under a device-memory cap, the shape
+    of BASELINE.json configs[4] (scale 30 itself needs more host memory than the box has: DESIGN.md).  One step = one
+    wl_refine_batched call to its fixed point; inputs start in pinned host memory, the colours end there."""
+    import torch
+    import graphgen as gg
+    import paper_2607_02603_b200 as wl
+    dev = torch.device("cuda", int(os.environ.get("LOCAL_RANK", "0")))
+    torch.cuda.set_device(dev)
+    g = gg.rmat(args.scale, seed=RMAT_SEEDS[30], symmetrize=False, device=dev, chunk=1 << 27)
+    n, m = g.n, g.m
+    rp = torch.empty(n + 1, dtype=torch.int64, pin_memory=True)
+    col = torch.empty(m, dtype=torch.int32, pin_memory=True)
+    rp.copy_(g.row_ptr)
+    col.copy_(g.col)
+    del g
+    torch.cuda.empty_cache()
+    hws = torch.empty(wl.wl_refine_batched_host_bytes(n, m), dtype=torch.uint8, pin_memory=True)
+    out = torch.empty(n, dtype=torch.int32, pin_memory=True)
+    cap = int(args.cap_gb * (1 << 30))
+    flags = args.flags
+    times, res = [], None
+    for i in range(args.warmup + args.steps):
+        torch.cuda.synchronize(dev)
+        t0 = time.perf_counter()
+        res = wl.wl_refine_batched(n, rp, col, None, max_batch_edges=args.batch_edges, seed=300 + i, device_cap_bytes=cap,
+                                   flags=flags, host_workspace=hws, out=out)
+        torch.cuda.synchronize(dev)
+        if i >= args.warmup:
+            times.append(time.perf_counter() - t0)
+    st = res.stats
+    sec = sum(times) / len(times)
+    link = (st["bytes_h2d"] + st["bytes_d2h"]) / sec / 1e9
+    line = {"metric": "batched_refine_input_gedges_per_s", "value": m / sec / 1e9, "unit": "GEdges/s", "n_gpus": 1,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * sec, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "u64", "data": "synthetic",
+            "config": {"workload": f"R-MAT scale {args.scale}, edge factor 16, seed 3, directed, deduplicated, CSR in pinned host "
+                                   f"memory; device cap {args.cap_gb} GB, M_b = {args.batch_edges} edges "
+                                   f"(shape of BASELINE.json configs[4])", "n": n, "m": m,
+                       "step": "wl_refine_batched to the batched fixed point (Algorithm 2, B1-B7)"},
+            "seconds_to_stable_coloring": sec, "outer_iters": st["outer_iters"], "num_colors": st["num_colors"],
+            "reduction_power": st["num_colors"] / n, "last_num_batches": st["last_num_batches"],
+            "boundary_nodes": st["boundary_nodes"], "h2d_bytes_per_step": st["bytes_h2d"],
+            "d2h_bytes_per_step": st["bytes_d2h"],
+            "link": {"achieved": link, "unit": "GB/s", "peak": 50.0,
+                     "peak_kind": "measured pinned cudaMemcpy on this box, one direction (43 GB/s each way when both run)",
+                     "frac": link / 50.0},
+            "ms_inbatch_spmv": st["ms_spmv"], "gpu_launches": st["kernel_launches"],
+            "e2e": {"value": m / sec / 1e9, "unit": "GEdges/s", "h2d_bytes_per_step": st["bytes_h2d"],
+                    "d2h_bytes_per_step": st["bytes_d2h"]}}
+    print(json.dumps(line))
+    return 0
+
+
 def aggregate_over_ranks(dist, local_ms: float, units_per_rank: float, device=None):
     """Max-over-ranks time and whole-job throughput for N independent replicas (weak scaling, no data-path collective).
     dist = torch.distributed (initialised) or None for a single process.  Returns (ms_max, total_units_per_second)."""
@@ -169,10 +225,16 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--flags", type=int, default=0, help="WL_FLAG_* bits passed to wl_refine")
+    ap.add_argument("--workload", default="single", choices=["single", "batched"],
+                    help="single: wl_refine on the HBM-resident graph (the headline); batched: wl_refine_batched")
+    ap.add_argument("--cap-gb", type=float, default=16.0, help="batched: device memory cap")
+    ap.add_argument("--batch-edges", type=int, default=120_000_000, help="batched: M_b")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
     if args.impl == "reference":
         return run_reference(args)
+    if args.workload == "batched":
+        return run_batched(args)
 
     import torch
     import graphgen as gg
@@ -235,21 +297,32 @@ def main():
     ms_per_step = ms_total / args.steps
     value = edges_per_s / 1e9
 
-    # ---- roofline of the dominant kernel (S1+S2 SpMV), from the library's own CUDA events on the launch stream --------
+    # ---- roofline of the dominant kernel: the S1+S2 launch of the one un-pruned round (round 2 from a uniform start: the
+    # row kernel + the hub-chunk kernel), timed by the library's own CUDA events on the launch stream -------------------
     peaks, peak_kind = measured_peaks()
     spmv_ms = sum(r.stats["ms_spmv_kernel"] for r in results)
     spmv_launches = sum(r.stats["spmv_launches"] for r in results)
     alg_bytes = sum(r.stats["spmv_alg_bytes"] for r in results)  # (4+G) per streamed entry + 16 per row, DESIGN.md
     spmv_edges = sum(r.stats["edges_streamed"] for r in results)
+    top_ms = sum(r.stats["ms_spmv_top"] for r in results) / len(results)
+    top_bytes = results[-1].stats["spmv_top_alg_bytes"]
+    top_edges = results[-1].stats["spmv_top_edges"]
     roofline = None
-    if spmv_launches:
-        achieved = alg_bytes / (spmv_ms / 1e3) / 1e9
-        roofline = {"bound": "hbm", "kernel": "spmv_merge_kernel" if args.flags & 4 else "spmv_rows32_kernel(+spmv_hub_kernel)",
+    if spmv_launches and top_ms > 0:
+        achieved = top_bytes / (top_ms / 1e3) / 1e9
+        roofline = {"bound": "hbm", "kernel": "spmv_merge_kernel" if args.flags & 4 else
+                    "spmv_rows32_kernel<u16>+spmv_hub_kernel<u16> (S1+S2 of round 2, the un-pruned round)",
                     "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": achieved / peaks["hbm_gbs"],
-                    "peak_kind": f"{peak_kind} copy bandwidth", "algorithmic_bytes_per_launch": alg_bytes / spmv_launches,
-                    "avg_launch_ms": spmv_ms / spmv_launches, "launches_timed": spmv_launches,
-                    "gedges_per_s_in_kernel": spmv_edges / (spmv_ms / 1e3) / 1e9, "traffic": None,
-                    "share_of_step": spmv_ms / ms_total}
+                    "peak_kind": f"{peak_kind} copy bandwidth", "algorithmic_bytes_per_launch": top_bytes,
+                    "avg_launch_ms": top_ms, "launches_timed": len(results),
+                    "gedges_per_s_in_kernel": top_edges / (top_ms / 1e3) / 1e9,
+                    "traffic": NCU_TRAFFIC_BYTES if args.scale == 27 and not args.flags else None,
+                    "traffic_source": "profiles/r1d_ncu_full.md (dram__bytes_read.sum + dram__bytes_write.sum, row + hub kernel)",
+                    "share_of_step": top_ms / ms_per_step,
+                    "all_spmv_launches": {"launches": spmv_launches, "algorithmic_gb_per_s": alg_bytes / (spmv_ms / 1e3) / 1e9,
+                                          "gedges_per_s": spmv_edges / (spmv_ms / 1e3) / 1e9,
+                                          "share_of_step": spmv_ms / ms_total},
+                    "binding_unit": "L1TEX 76 % / L2 73 % of peak (ncu): one sector lookup per gathered 2-byte id; DRAM 43 %"}
 
     # ---- end to end through the host-buffer entry point ---------------------------------------------------------------
     e2e = None

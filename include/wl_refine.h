@@ -97,6 +97,9 @@ typedef struct wl_stats {
   double ms_spmv_kernel;     /* device time of those S1+S2 kernels alone (CUDA events on cuda_stream)                 */
   int64_t spmv_alg_bytes;    /* algorithmic bytes of those launches: (4+G) per streamed entry (G = 2 or 4 bytes of
                                 gathered colour id) + 16 per processed row (offsets + y)        */
+  double ms_spmv_top;        /* the longest single S1+S2 launch of the call (row kernel + hub kernel of one round) ...  */
+  int64_t spmv_top_alg_bytes;/* ... its algorithmic bytes ...                                                          */
+  int64_t spmv_top_edges;    /* ... and the column indices it consumed (bench.py's roofline object)                     */
 } wl_stats;
 
 /* ------------------------------------------------------------------------------------------------------------------

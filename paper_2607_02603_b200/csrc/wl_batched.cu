@@ -165,7 +165,8 @@ quot_insert_long_kernel(int64_t row_base, const int64_t* __restrict__ row_ptr, i
 // Only blocks b_lo <= B < b_hi are emitted (a representative row that continues in the next batch stays in the table).
 __global__ void quot_emit_kernel(u64* __restrict__ table, u64 table_slots, const int64_t* __restrict__ q_row_ptr,
                                  int64_t out_base, int* __restrict__ cursor, int* __restrict__ q_col,
-                                 u32* __restrict__ q_wt, int b_lo, int b_hi) {
+                                 u32* __restrict__ q_wt, int b_lo, int b_hi, int64_t cap = (1ll << 62),
+                                 long long* __restrict__ dbg = nullptr) {
   int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (s >= (int64_t)table_slots) return;
   const u64 key1 = table[2 * s];
@@ -174,11 +175,32 @@ __global__ void quot_emit_kernel(u64* __restrict__ table, u64 table_slots, const
   const int b = (int)(key >> 32), t = (int)(key & 0xffffffffu);
   if (b < b_lo || b >= b_hi) return;
   const u64 sum = table[2 * s + 1];
-  const int64_t pos = q_row_ptr[b] - out_base + atomicAdd(cursor + b, 1);
+  const int c = atomicAdd(cursor + b, 1);
+  const int64_t pos = q_row_ptr[b] - out_base + c;
+  if (pos < 0 || pos >= cap) {
+    if (dbg && atomicAdd((unsigned long long*)dbg, 1ull) == 0) {
+      dbg[1] = b; dbg[2] = pos; dbg[3] = q_row_ptr[b]; dbg[4] = c; dbg[5] = q_row_ptr[b + 1]; dbg[6] = s;
+    }
+    return;
+  }
   q_col[pos] = t;
   q_wt[pos] = (u32)sum;
   table[2 * s] = 0;
   table[2 * s + 1] = 0;
+}
+
+// WL_DEBUG: occupied slots whose block lies in [b_lo, b_hi), and the largest per-slot anomalies
+__global__ void quot_count_kernel(const u64* __restrict__ table, u64 table_slots, int b_lo, int b_hi, u64* __restrict__ out) {
+  int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (s >= (int64_t)table_slots) return;
+  const u64 key1 = table[2 * s];
+  if (key1 == 0) {
+    if (table[2 * s + 1] != 0) atomicAdd(out + 2, 1ull);  // weight without key
+    return;
+  }
+  const int b = (int)((key1 - 1) >> 32);
+  if (b >= b_lo && b < b_hi) atomicAdd(out, 1ull);
+  else atomicAdd(out + 1, 1ull);
 }
 
 // exclusive scan int32 counts -> int64 offsets (3 kernels)
@@ -592,9 +614,9 @@ int wl_refine_batched(int64_t n, int32_t num_batches, const wl_edge_batch* batch
     DevBuf d_H, d_Hc, d_first, d_cof, d_bsum, d_ws, d_col[2], d_wt[2], d_rp[2], d_rep, d_cnt, d_cursor, d_qrp, d_qtab,
         d_qcol[2], d_qwt[2], d_sbsum, d_misc, d_query, d_long;
     const int64_t nscan = (n_t + kCanonChunk - 1) / kCanonChunk;
-#define WL_ALLOC(buf, bytes)                                   \
-  if ((rc = buf.alloc((bytes), &used_iter, device_cap_bytes))) \
-    break;
+    // every allocation of the iteration goes through here: the first failure (device cap or cudaMalloc) sticks
+#define WL_ALLOC(buf, bytes) \
+  if (!rc) rc = buf.alloc((bytes), &used_iter, device_cap_bytes);
     WL_ALLOC(d_H, sizeof(int) * (size_t)n_t);
     WL_ALLOC(d_Hc, sizeof(int) * (size_t)n_t);
     WL_ALLOC(d_first, sizeof(int) * (size_t)n_t);
@@ -741,8 +763,8 @@ int wl_refine_batched(int64_t n, int32_t num_batches, const wl_edge_batch* batch
     WL_ALLOC(d_sbsum, sizeof(u64) * (size_t)((K + kScanC - 1) / kScanC + 2));
     WL_ALLOC(d_query, sizeof(int64_t) * 2 * (size_t)nb);
     WL_ALLOC(d_long, sizeof(int) * (size_t)(max_edges / kQuotLongRow + 2));
+    if (debug) std::fprintf(stderr, "[wl_refine_batched] outer %d device memory %.2f GB (cap %.2f GB)%s\n", outer, used_iter / 1073741824.0, device_cap_bytes / 1073741824.0, rc ? " -> WL_ENOMEM" : "");
     if (rc) break;
-#undef WL_ALLOC
     cudaMemsetAsync(d_rep.p, 0x7f, sizeof(int) * (size_t)K, st);
     cudaMemsetAsync(d_cnt.p, 0, sizeof(int) * (size_t)K, st);
     cudaMemsetAsync(d_cursor.p, 0, sizeof(int) * (size_t)K, st);
@@ -779,6 +801,12 @@ int wl_refine_batched(int64_t n, int32_t num_batches, const wl_edge_batch* batch
     };
     int64_t q_off = 0, emitted_blocks = 0;
     int n_emit = 0;
+    auto checkpoint = [&](const char* what, int k) {  // WL_DEBUG: find the launch that faults
+      if (!debug) return;
+      cudaError_t e = cudaDeviceSynchronize();
+      if (e != cudaSuccess) std::fprintf(stderr, "[wl_refine_batched] outer %d batch %d: %s -> %s\n", outer, k, what, cudaGetErrorString(e));
+    };
+    checkpoint("block_rep / lower_bound", -1);
     upload_quot(0, 0);
     for (int k = 0; k < nb && !rc; ++k) {
       const int buf = k & 1;
@@ -795,6 +823,7 @@ int wl_refine_batched(int64_t n, int32_t num_batches, const wl_edge_batch* batch
                            qslots - 1, d_cnt.as<int>(), d_long.as<int>(), (u32*)(d_misc.as<u64>() + 16), st);
       }
       cudaEventRecord(ev_ins[buf], st);
+      checkpoint("insert", k);
       // a representative row that continues into the next batch is completed there: emit the blocks whose representative
       // row ends at or before c1 and that were not emitted yet
       const int64_t b_lo = emitted_blocks, b_hi = done_blocks[k];
@@ -805,6 +834,7 @@ int wl_refine_batched(int64_t n, int32_t num_batches, const wl_edge_batch* batch
         rc = check_cuda(cudaStreamSynchronize(st));
         if (rc) break;
         const int64_t tot = (int64_t)hs[kNumScal + 1];
+        if (debug) std::fprintf(stderr, "[wl_refine_batched] outer %d batch %d: rows %lld..%lld blocks %lld..%lld entries %lld at %lld (cap %lld)\n", outer, k, (long long)na[k], (long long)nz[k], (long long)b_lo, (long long)b_hi, (long long)tot, (long long)q_off, (long long)out_cap);
         if (tot > out_cap || q_off + tot > hq.cap_edges || b_hi > hq.cap_nodes) {
           rc = WL_ECUDA;  // unreachable: a quotient has at most the entries and nodes of its graph
           break;
@@ -814,6 +844,7 @@ int wl_refine_batched(int64_t n, int32_t num_batches, const wl_edge_batch* batch
         ++n_emit;
         ++g_launches; quot_emit_kernel<<<blocks_for((int64_t)qslots, 256), 256, 0, st>>>(d_qtab.as<u64>(), qslots, d_qrp.as<int64_t>(), q_off, d_cursor.as<int>(), d_qcol[ob].as<int>(), d_qwt[ob].as<u32>(), (int)b_lo, (int)b_hi);
         cudaEventRecord(ev_emit[ob], st);
+        checkpoint("emit", k);
         cudaStreamWaitEvent(down_st, ev_emit[ob], 0);
         // in place from the second quotient on: q_off + tot <= c1, and everything below c1 has been uploaded already
         if (tot) {

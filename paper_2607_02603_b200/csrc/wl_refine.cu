@@ -392,8 +392,9 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
   int64_t active_hubs = num_hub_chunks;  // > 0: some hub row may still be in a splittable block
 
   // ---- S1-S5: rounds -------------------------------------------------------------------------------------------------
-  int64_t edges_streamed = 0, spmv_alg_bytes = 0;
-  double ms_spmv = 0, ms_relabel = 0, ms_spmv_kernel = 0;
+  int64_t edges_streamed = 0, spmv_alg_bytes = 0, last_alg_bytes = 0, last_edges = 0;
+  int64_t top_alg_bytes = 0, top_edges = 0;
+  double ms_spmv = 0, ms_relabel = 0, ms_spmv_kernel = 0, ms_spmv_top = 0;
   int32_t rounds = 0, spmv_launches = 0;
   bool converged = false;
   const bool debug = std::getenv("WL_DEBUG") != nullptr;
@@ -442,7 +443,9 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
       cudaEventRecord(ek1, st);
       const int64_t e_r = all_rows ? m : active_edges, n_r = all_rows ? n : n_active;
       edges_streamed += e_r;
-      spmv_alg_bytes += (int64_t)(4 + (narrow ? 2 : 4) + (g->weights ? 4 : 0)) * e_r + 16 * n_r;
+      last_alg_bytes = (int64_t)(4 + (narrow ? 2 : 4) + (g->weights ? 4 : 0)) * e_r + 16 * n_r;
+      last_edges = e_r;
+      spmv_alg_bytes += last_alg_bytes;
       streamed = true;
     }
     aux.need(st, (u64)mask_r + 1, prefix_slots);
@@ -521,6 +524,11 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
         cudaEventElapsedTime(&tc, evp.get(8 + 2 * j), evp.get(9 + 2 * j));
         t_spmv += tc;
         ++spmv_launches;
+        if (R == 1 && tc > ms_spmv_top) {  // (per-round bytes are only kept in the one-round-per-sync regime)
+          ms_spmv_top = tc;
+          top_alg_bytes = last_alg_bytes;
+          top_edges = last_edges;
+        }
       }
     ms_spmv_kernel += t_spmv;
     ms_spmv += t_spmv;
@@ -570,6 +578,9 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
   res->ms_relabel = ms_relabel;
   res->ms_spmv_kernel = ms_spmv_kernel;
   res->spmv_launches = spmv_launches;
+  res->ms_spmv_top = ms_spmv_top;
+  res->spmv_top_alg_bytes = top_alg_bytes;
+  res->spmv_top_edges = top_edges;
   res->kernel_launches = (int32_t)(g_launches - launches_at_entry);
   res->colour = colour;
   return converged ? WL_OK : WL_EMAXROUNDS;
@@ -625,6 +636,9 @@ int wl_refine(const wl_csr* g, const int32_t* init_colors, uint64_t seed, int32_
     stats->ms_spmv_kernel = cr.ms_spmv_kernel;
     stats->spmv_launches = cr.spmv_launches;
     stats->spmv_alg_bytes = cr.spmv_alg_bytes;
+    stats->ms_spmv_top = cr.ms_spmv_top;
+    stats->spmv_top_alg_bytes = cr.spmv_top_alg_bytes;
+    stats->spmv_top_edges = cr.spmv_top_edges;
     stats->kernel_launches = (int32_t)(g_launches - launches_at_entry);
   }
   return core_rc;
