@@ -191,6 +191,44 @@ def run_batched(args):
     return 0
 
 
+def run_batch_study(args):
+    """--workload batch-study: the shape of the paper's simulated-memory experiment (Tables 1 and 3, L237-L297): the
+    same graph refined with N_b = 1, 2, 4, ... row-contiguous edge batches; reports the reduction power |H|/|V| next to the
+    coarsest colouring's and the slow-down against N_b = 1."""
+    import torch
+    import graphgen as gg
+    import paper_2607_02603_b200 as wl
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    graphs = [("C1 Erdos-Renyi 10k/50k", gg.erdos_renyi()), ("grid 512^2", gg.grid2d(512, device=dev)),
+              (f"R-MAT scale {args.scale} symmetrised", gg.rmat(args.scale, seed=RMAT_SEEDS.get(args.scale, 1), device=dev)),
+              (f"R-MAT scale {args.scale} directed", gg.rmat(args.scale, seed=3, symmetrize=False, device=dev))]
+    rows = []
+    for name, g in graphs:
+        n, m = g.n, g.m
+        gd = g.to(dev)
+        single = wl.wl_refine(n, gd.row_ptr, gd.col, None, seed=1)
+        rp, col = gd.row_ptr.cpu().pin_memory(), gd.col.cpu().pin_memory()
+        hws = torch.empty(wl.wl_refine_batched_host_bytes(n, m), dtype=torch.uint8, pin_memory=True)
+        base = None
+        for nb in (1, 2, 4, 8):
+            best = None
+            for rep in range(3):
+                torch.cuda.synchronize(dev)
+                t0 = time.perf_counter()
+                r = wl.wl_refine_batched(n, rp, col, None, max_batch_edges=(m + nb - 1) // nb, seed=10 + rep, host_workspace=hws)
+                dt = time.perf_counter() - t0
+                best = dt if best is None else min(best, dt)
+            base = best if nb == 1 else base
+            rows.append({"graph": name, "n": n, "m": m, "N_b": nb, "colors": r.num_colors,
+                         "reduction_power_pct": 100.0 * r.num_colors / n,
+                         "coarsest_pct": 100.0 * single.num_colors / n,
+                         "gap_pp": 100.0 * (r.num_colors - single.num_colors) / n,
+                         "outer_iters": r.stats["outer_iters"], "seconds": best, "slowdown_vs_Nb1": best / base})
+    print(json.dumps({"metric": "batch_study", "unit": "table", "data": "synthetic", "rows": rows}))
+    return 0
+
+
 def aggregate_over_ranks(dist, local_ms: float, units_per_rank: float, device=None):
     """Max-over-ranks time and whole-job throughput for N independent replicas (weak scaling, no data-path collective).
     dist = torch.distributed (initialised) or None for a single process.  Returns (ms_max, total_units_per_second)."""
@@ -225,7 +263,7 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--flags", type=int, default=0, help="WL_FLAG_* bits passed to wl_refine")
-    ap.add_argument("--workload", default="single", choices=["single", "batched"],
+    ap.add_argument("--workload", default="single", choices=["single", "batched", "batch-study"],
                     help="single: wl_refine on the HBM-resident graph (the headline); batched: wl_refine_batched")
     ap.add_argument("--cap-gb", type=float, default=16.0, help="batched: device memory cap")
     ap.add_argument("--batch-edges", type=int, default=120_000_000, help="batched: M_b")
@@ -235,6 +273,8 @@ def main():
         return run_reference(args)
     if args.workload == "batched":
         return run_batched(args)
+    if args.workload == "batch-study":
+        return run_batch_study(args)
 
     import torch
     import graphgen as gg
