@@ -64,6 +64,8 @@ typedef struct wl_csr {
 #define WL_FLAG_EDGE_BALANCED 128u /* use the edge-balanced SpMV kernel (one warp per 2048 consecutive entries, all rows) in
                                       every round instead of the row kernels; results are identical (measured slower on the
                                       headline graph, kept for extreme degree skew)                          */
+#define WL_FLAG_NO_DEEP 256u     /* never switch to the worklist regime (below): every round recomputes every active row */
+#define WL_FLAG_DEEP_EARLY 512u  /* switch to the worklist regime at round 2 instead of round 7 (testing)                 */
 #define WL_FLAG_NO_CANONICAL 16u /* leave internal dense ids in out_colors (skips S6)                                  */
 
 typedef struct wl_options {
@@ -108,6 +110,11 @@ typedef struct wl_stats {
 
 /* Bytes of device workspace wl_refine needs for a graph with n nodes and m entries (0 on invalid sizes). */
 size_t wl_refine_workspace_bytes(int64_t n, int64_t m);
+
+/* Bytes of device workspace that also hold the in-neighbour lists and work lists of the deep-round (worklist) regime:
+ * from round 7 on only the rows with a changed out-neighbour are recomputed, under one fixed weight key (same partitions
+ * per round, same fixed point; S5).  wl_refine uses that regime when the workspace it is given is at least this large. */
+size_t wl_refine_deep_workspace_bytes(int64_t n, int64_t m);
 
 /* Coarsest stable colouring refining init_colors, with error probability <= 1e-9 (Theorem 1).
  *   g            CSR, all arrays DEVICE.

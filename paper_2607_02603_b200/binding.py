@@ -20,9 +20,11 @@ WL_FLAG_NO_VALIDATE, WL_FLAG_NO_PRUNE, WL_FLAG_MERGE_KERNEL, WL_FLAG_AGGRESSIVE_
 WL_FLAG_NARROW_COLORS = 32
 WL_FLAG_SYNC_EVERY_ROUND = 64
 WL_FLAG_EDGE_BALANCED = 128
+WL_FLAG_NO_DEEP = 256
+WL_FLAG_DEEP_EARLY = 512
 
 EXPORTS = [
-    "wl_refine_workspace_bytes", "wl_refine", "wl_refine_host", "wl_round_key", "wl_weight", "wl_spmv_round",
+    "wl_refine_workspace_bytes", "wl_refine_deep_workspace_bytes", "wl_refine", "wl_refine_host", "wl_round_key", "wl_weight", "wl_spmv_round",
     "wl_relabel", "wl_canonicalize", "wl_refine_batched", "wl_refine_batched_host_bytes", "wl_inner_labels", "wl_quotient",
     "wl_quotient_workspace_bytes", "wl_strerror", "wl_last_cuda_error", "wl_version", "wl_kernel_launches",
 ]
@@ -76,6 +78,8 @@ def lib():
         vp, i64, i32, u64, u32, sz = C.c_void_p, C.c_int64, C.c_int32, C.c_uint64, C.c_uint32, C.c_size_t
         L.wl_refine_workspace_bytes.restype = sz
         L.wl_refine_workspace_bytes.argtypes = [i64, i64]
+        L.wl_refine_deep_workspace_bytes.restype = sz
+        L.wl_refine_deep_workspace_bytes.argtypes = [i64, i64]
         L.wl_refine.restype = C.c_int
         L.wl_refine.argtypes = [C.POINTER(wl_csr), vp, u64, vp, C.POINTER(wl_stats), C.POINTER(wl_options), vp, sz, vp]
         L.wl_refine_host.restype = C.c_int
@@ -166,11 +170,16 @@ def wl_refine_workspace_bytes(n: int, m: int) -> int:
     return int(lib().wl_refine_workspace_bytes(n, m))
 
 
+def wl_refine_deep_workspace_bytes(n: int, m: int) -> int:
+    return int(lib().wl_refine_deep_workspace_bytes(n, m))
+
+
 def wl_refine(n: int, row_ptr: torch.Tensor, col_idx: torch.Tensor, weights: Optional[torch.Tensor] = None,
               init_colors: Optional[torch.Tensor] = None, seed: int = 0, *, flags: int = 0, max_rounds: int = 0,
               stream_id: int = 0, workspace: Optional[torch.Tensor] = None, out: Optional[torch.Tensor] = None,
-              round_cap: int = 4096, allow_max_rounds: bool = False) -> RefineResult:
-    """Algorithm 1 on device-resident CSR tensors.  Returns canonical colours (device int32[n])."""
+              round_cap: int = 4096, allow_max_rounds: bool = False, deep: bool = True) -> RefineResult:
+    """Algorithm 1 on device-resident CSR tensors.  Returns canonical colours (device int32[n]).  When no workspace is
+    given, one large enough for the deep-round (worklist) regime is allocated unless deep=False."""
     L = lib()
     dev = row_ptr.device
     if dev.type != "cuda":
@@ -180,7 +189,7 @@ def wl_refine(n: int, row_ptr: torch.Tensor, col_idx: torch.Tensor, weights: Opt
     if out is None:
         out = torch.empty(n, dtype=torch.int32, device=dev)
     _check(out, torch.int32, "cuda", "out", n)
-    need = wl_refine_workspace_bytes(n, col_idx.numel())
+    need = wl_refine_deep_workspace_bytes(n, col_idx.numel()) if deep else wl_refine_workspace_bytes(n, col_idx.numel())
     if workspace is None:
         workspace = torch.empty(max(need, 256), dtype=torch.uint8, device=dev)
     rc_buf = (C.c_int64 * round_cap)()

@@ -205,6 +205,7 @@ __global__ void quot_count_kernel(const u64* __restrict__ table, u64 table_slots
 
 // exclusive scan int32 counts -> int64 offsets (3 kernels)
 constexpr int kScanT = 256, kScanI = 8, kScanC = kScanT * kScanI;
+static_assert(kScanC == kScan32Chunk, "wl_refine.cu sizes the scan scratch with kScan32Chunk");
 
 __global__ void __launch_bounds__(kScanT)
 scan32_sum_kernel(const int* __restrict__ in, int64_t n, u64* __restrict__ bsum) {
@@ -342,8 +343,7 @@ struct HostQuot {
 };
 
 // exclusive scan of cnt[0..n) into out[0..n] starting at base_off (device arrays); bsum: ceil(n / kScanC) + 1 u64
-static void launch_scan32(const int* cnt, int64_t n, int64_t base_off, int64_t* out, u64* bsum, u64* total,
-                          cudaStream_t st) {
+void launch_scan32(const int* cnt, int64_t n, int64_t base_off, int64_t* out, u64* bsum, u64* total, cudaStream_t st) {
   if (n == 0) return;
   const int64_t nb = (n + kScanC - 1) / kScanC;
   ++g_launches; scan32_sum_kernel<<<(unsigned)nb, kScanT, 0, st>>>(cnt, n, bsum);
@@ -676,7 +676,7 @@ int wl_refine_batched(int64_t n, int32_t num_batches, const wl_edge_batch* batch
       lo.stream_id = ((u64)outer << 32) | (u64)(u32)k;
       const Layout L = make_layout(nr, lg.m);
       CoreResult cr{};
-      rc = refine_core(&lg, nullptr, seed, &lo, /*ranged=*/true, (int)r0[k], (int)r1[k], n_t, e0, d_ws.p, L, st, &cr);
+      rc = refine_core(&lg, nullptr, seed, &lo, /*ranged=*/true, (int)r0[k], (int)r1[k], n_t, e0, d_ws.p, L.bytes, L, st, &cr);
       if (rc) break;
       ++g_launches; merge_kernel<<<blocks_for(nr, 256), 256, 0, st>>>(nr, cr.colour, (int)base_id, d_H.as<int>() + r0[k]);
       base_id += cr.k;

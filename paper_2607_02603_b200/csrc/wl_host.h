@@ -23,6 +23,15 @@ struct Layout {
 };
 Layout make_layout(int64_t n, int64_t m);
 
+// extra workspace of the deep-round regime (wl_deep.cuh), laid out after Layout::bytes
+struct DeepLayout {
+  size_t o_scal, o_tp_ptr, o_tp_src, o_size, o_lcount[2], o_inherit, o_mark, o_leavers[2], o_leaver_block[2], o_slots,
+      o_changed[2], o_bsum, bytes;  // bytes = end of the whole workspace (base included)
+};
+DeepLayout make_deep_layout(const Layout& L);
+void launch_scan32(const int* cnt, int64_t n, int64_t base_off, int64_t* out, u64* bsum, u64* total, cudaStream_t st);
+constexpr int kScan32Chunk = 2048;  // elements per CTA of launch_scan32
+
 struct CoreResult {
   int64_t k, edges_streamed, spmv_alg_bytes;
   int32_t rounds, spmv_launches, kernel_launches;
@@ -32,8 +41,8 @@ struct CoreResult {
   int* colour;  // dense ids, inside the workspace
 };
 int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, const wl_options* opt, bool ranged, int lo,
-                int hi, int64_t n_targets, int64_t edge_first, void* workspace, const Layout& L, cudaStream_t st,
-                CoreResult* res);
+                int hi, int64_t n_targets, int64_t edge_first, void* workspace, size_t workspace_bytes, const Layout& L,
+                cudaStream_t st, CoreResult* res);
 void launch_canonical(const Layout& L, int64_t n, const int* colour, int* out, int* first, int* cof, int* bsum, u64* total,
                       cudaStream_t st);
 u64* host_scal();

@@ -645,6 +645,7 @@ __global__ void spmv_uniform_kernel(int64_t n, const int64_t* __restrict__ row_p
 //            polls.  The winner publishes without waiting on anything but its own CTA's phase 1, so the poll ends.
 // stamp[c] == round  <=>  block c has at least two nodes after this round (no atomics: plain idempotent stores).
 // colour16 (optional) mirrors the ids as 16 bits while k <= 65536 (narrow gathers in the SpMV).  nodes == NULL: all nodes.
+// changed (optional): list of the nodes whose id changed.
 // ---------------------------------------------------------------------------------------------------------------------
 constexpr int kRelabelThreads = 256;
 constexpr u32 kPending = 0xffffffffu;
@@ -662,7 +663,8 @@ __global__ void __launch_bounds__(kRelabelThreads)
 relabel_kernel(int64_t count, const int* __restrict__ nodes, int* __restrict__ colour,
                unsigned short* __restrict__ colour16, const u64* __restrict__ y, int* __restrict__ rep,
                int* __restrict__ stamp, int round, Slot* __restrict__ table, u32 table_mask,
-               u32* __restrict__ slot_of, const u64* __restrict__ k_ptr, u64* __restrict__ new_counter) {
+               u32* __restrict__ slot_of, const u64* __restrict__ k_ptr, u64* __restrict__ new_counter,
+               int* __restrict__ changed, u64* __restrict__ n_changed) {
   const int k_old = (int)*k_ptr;  // device-resident colour count: rounds can be queued without a host round trip
   int64_t t = (int64_t)blockIdx.x * kRelabelThreads + threadIdx.x;
   bool win = false, lose = false;
@@ -715,6 +717,17 @@ relabel_kernel(int64_t count, const int* __restrict__ nodes, int* __restrict__ c
   if (win || lose) {
     colour[i] = (int)id;
     if (colour16) colour16[i] = (unsigned short)id;
+  }
+  if (changed) {  // the nodes that got a new id, for the worklist regime (wl_deep.cuh); one atomic per warp
+    const bool ch = win || lose;
+    const unsigned bal = __ballot_sync(0xffffffffu, ch);
+    if (bal) {
+      const int lane = threadIdx.x & 31, leader = __ffs(bal) - 1;
+      u64 base = 0;
+      if (lane == leader) base = atomicAdd(n_changed, (u64)__popc(bal));
+      base = __shfl_sync(0xffffffffu, base, leader);
+      if (ch) changed[base + __popc(bal & ((1u << lane) - 1))] = i;
+    }
   }
 }
 

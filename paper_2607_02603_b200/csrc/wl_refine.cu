@@ -8,6 +8,7 @@
 #include <cstring>
 #include <vector>
 
+#include "wl_deep.cuh"
 #include "wl_kernels.cuh"
 
 namespace wl {
@@ -58,6 +59,33 @@ Layout make_layout(int64_t n, int64_t m) {
 }
 
 
+
+DeepLayout make_deep_layout(const Layout& L) {
+  DeepLayout D{};
+  size_t off = L.bytes;
+  auto take = [&](size_t bytes) {
+    size_t o = off;
+    off = align_up(off + bytes);
+    return o;
+  };
+  const size_t n = (size_t)L.n, m = (size_t)L.m;
+  D.o_scal = take(sizeof(u64) * kNumDeep);
+  D.o_tp_ptr = take(sizeof(int64_t) * (n + 1));
+  D.o_tp_src = take(sizeof(int) * m);
+  D.o_size = take(sizeof(int) * n);
+  D.o_inherit = take(sizeof(int) * n);
+  D.o_mark = take(sizeof(int) * n);
+  D.o_slots = take(sizeof(u32) * n);
+  for (int b = 0; b < 2; ++b) {  // double-buffered by round parity
+    D.o_lcount[b] = take(sizeof(int) * n);
+    D.o_leavers[b] = take(sizeof(int) * n);
+    D.o_leaver_block[b] = take(sizeof(int) * n);
+    D.o_changed[b] = take(sizeof(int) * n);
+  }
+  D.o_bsum = take(sizeof(u64) * (n / kScan32Chunk + 3));
+  D.bytes = off;
+  return D;
+}
 
 // ---- step launchers -----------------------------------------------------------------------------------------------
 void launch_tile_search(const Layout& L, const wl_csr& g, int* tile_row, cudaStream_t st) {
@@ -165,10 +193,10 @@ void launch_hub_collect(const Layout& L, const wl_csr& g, int2* chunks, u64* cou
 // clean == false: the claimed slots stay (the caller empties them with clean_table once it knows the new colour count).
 void launch_relabel(u32 table_mask, int64_t count, const int* nodes, int* colour, unsigned short* colour16, const u64* y,
                     int* rep, int* stamp, int round, Slot* table, u32* slot_of, u64* scal, u64* log, int log_slot,
-                    bool clean, cudaStream_t st) {
+                    bool clean, cudaStream_t st, int* changed = nullptr, u64* n_changed = nullptr) {
   if (count > 0) {
     unsigned grid = blocks_for(count, kRelabelThreads);
-    ++g_launches; relabel_kernel<<<grid, kRelabelThreads, 0, st>>>(count, nodes, colour, colour16, y, rep, stamp, round, table, table_mask, slot_of, scal + kScalK, scal + kScalNew);
+    ++g_launches; relabel_kernel<<<grid, kRelabelThreads, 0, st>>>(count, nodes, colour, colour16, y, rep, stamp, round, table, table_mask, slot_of, scal + kScalK, scal + kScalNew, changed, n_changed);
   }
   const unsigned fgrid = clean ? (unsigned)std::max<int64_t>(1, std::min<int64_t>(blocks_for(count, 256), 148 * 8)) : 1u;
   ++g_launches; relabel_finish_kernel<<<fgrid, 256, 0, st>>>(table, slot_of, scal, log, log_slot, clean ? 1 : 0);
@@ -240,6 +268,11 @@ size_t wl_refine_workspace_bytes(int64_t n, int64_t m) {
   return make_layout(n, m).bytes;
 }
 
+size_t wl_refine_deep_workspace_bytes(int64_t n, int64_t m) {
+  if (n < 0 || m < 0 || n > kMaxNodes) return 0;
+  return make_deep_layout(make_layout(n, m)).bytes;
+}
+
 uint64_t wl_round_key(uint64_t seed, uint64_t stream_id, uint64_t round) { return round_key(seed, stream_id, round); }
 uint64_t wl_weight(uint64_t key, uint64_t color) { return weight_of(key, color); }
 
@@ -280,8 +313,8 @@ struct AuxStream {
 // are implicit singletons and targets inside map to local node j - lo (Eq. 3).  On success the dense (non canonical)
 // colours are in the workspace's colour array and *k_out is their number.  Synchronises `st` once per round.
 int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, const wl_options* opt, bool ranged, int lo,
-                int hi, int64_t n_targets, int64_t edge_first, void* workspace, const Layout& L, cudaStream_t st,
-                CoreResult* res) {
+                int hi, int64_t n_targets, int64_t edge_first, void* workspace, size_t workspace_bytes, const Layout& L,
+                cudaStream_t st, CoreResult* res) {
   const int64_t n = g->n, m = g->m;
   int rc = WL_OK;
   const uint32_t flags = opt ? opt->flags : 0u;
@@ -318,6 +351,13 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
   // and collects the hub chunks.  The column range check is folded into the first kernel that reads the columns.
   const bool uniform_start = !init_colors && !g->weights && !ranged && !merge;
   const bool force_eb = (flags & WL_FLAG_EDGE_BALANCED) != 0 && !merge && m > 0;
+  constexpr int64_t kSyncRounds = 6;
+  // deep-round (worklist) regime, wl_deep.cuh: needs the larger workspace
+  const DeepLayout DL = make_deep_layout(L);
+  const bool deep_ok = !(flags & WL_FLAG_NO_DEEP) && !ranged && !merge && !force_eb && m > 0 && workspace_bytes >= DL.bytes;
+  const int64_t deep_start = (flags & WL_FLAG_DEEP_EARLY) ? 2 : kSyncRounds + 1;
+  u64* deep = (u64*)(ws + DL.o_scal);
+  int* changed[2] = {(int*)(ws + DL.o_changed[0]), (int*)(ws + DL.o_changed[1])};
   bool cols_checked = !validate || m == 0;
   bool dropped_checked = false;  // the rows outside the active list have had their columns range-checked
   if (validate && !uniform_start) {
@@ -400,13 +440,12 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
   const bool debug = std::getenv("WL_DEBUG") != nullptr;
   const double list_frac = std::getenv("WL_LIST_FRAC") ? std::atof(std::getenv("WL_LIST_FRAC")) : 0.75;
   const bool no_runahead = (flags & WL_FLAG_SYNC_EVERY_ROUND) != 0;
-  constexpr int64_t kSyncRounds = 6;
   const int* cur_list = nullptr;  // NULL: every node is active
   int64_t n_active = n, active_edges = m, pending_new = 0;
   int cur = 0;
   // One refinement round queued on the stream (S1-S4); no host decision inside.
   auto queue_round = [&](int64_t r, bool narrow, bool mirror, bool clean, u64* log, int log_slot, cudaEvent_t ek0,
-                         cudaEvent_t ek1) -> bool {
+                         cudaEvent_t ek1, bool list_changed = false) -> bool {
     const u64 key = round_key(seed, stream_id, (u64)r);
     bool streamed = false;
     u32 mask_r = round_table_mask(L, n_active);
@@ -453,7 +492,8 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
     dirty_count = 0;
     dirty_mask = mask_r;
     launch_relabel(mask_r, n_active, cur_list, colour, mirror ? colour16 : nullptr, y, rep, stamp, (int)r, table, slot_of,
-                   scal, log, log_slot, clean, st);
+                   scal, log, log_slot, clean, st, list_changed ? changed[(r + 1) & 1] : nullptr,
+                   list_changed ? deep + kDeepChanged0 + ((r + 1) & 1) : nullptr);
     return streamed;
   };
   auto queue_compaction = [&](int64_t r) {
@@ -486,12 +526,17 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
   };
 
   int64_t r = 1;
-  while (r <= max_rounds && !converged) {
+  bool deep_entered = false;
+  while (r <= max_rounds && !converged && !deep_entered) {
     // Rounds 1..kSyncRounds: one host synchronisation per round (the host picks kernels from k and the active count).
     // Deep-round regime (S5): up to kRunAhead rounds are queued back to back; the device keeps k, logs it per round,
     // and the host looks at the log once per window.  A round after the fixed point changes nothing, so running past
     // it is harmless; `rounds` and the trajectory stop at the first repeated count exactly as in the per-round mode.
-    const bool window = !no_runahead && r > kSyncRounds;
+    // the round at which the worklist regime starts is an ordinary round that also lists the nodes it moved; its key
+    // stays the key of every later round
+    const bool switch_round = deep_ok && r == deep_start;
+    if (switch_round) cudaMemsetAsync(deep, 0, sizeof(u64) * kNumDeep, st);
+    const bool window = !no_runahead && r > kSyncRounds && !switch_round;
     const int R = window ? (int)std::min<int64_t>(kRunAhead, max_rounds - r + 1) : 1;
     cudaEvent_t e0 = evp.get(2), e2 = evp.get(4);
     cudaEventRecord(e0, st);
@@ -499,9 +544,9 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
     // 16-bit ids: gathered while k <= 65536; the mirror is kept up to date by the relabel kernel as long as that holds
     const bool narrow = !merge && (window ? n <= 65536 : k <= 65536);
     for (int j = 0; j < R; ++j)
-      streamed[j] = queue_round(r + j, narrow, narrow, /*clean=*/window, scal + kScalLog, j, evp.get(8 + 2 * j), evp.get(9 + 2 * j));
+      streamed[j] = queue_round(r + j, narrow, narrow, /*clean=*/window, scal + kScalLog, j, evp.get(8 + 2 * j), evp.get(9 + 2 * j), switch_round);
     const int64_t r_last = r + R - 1;
-    const bool compact_now = prune && (window || r <= 2 || pending_new * 16 >= n_active);
+    const bool compact_now = prune && !switch_round && (window || r <= 2 || pending_new * 16 >= n_active);
     if (compact_now) queue_compaction(r_last);
     cudaEventRecord(e2, st);
     cudaMemcpyAsync(hs, scal, sizeof(u64) * kNumScal, cudaMemcpyDeviceToHost, st);
@@ -552,6 +597,10 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
     if (debug) std::fprintf(stderr, "[wl_refine]   %d round(s): spmv %.3f ms, rest %.3f ms\n", R, t_spmv, t_all - t_spmv);
     r += R;
     if (converged) break;
+    if (switch_round) {
+      deep_entered = true;
+      break;
+    }
     if (compact_now && adopt_compaction()) {
       // every block is a singleton (or can never split again): the next round cannot change anything and only
       // confirms (same trajectory as the un-pruned algorithm)
@@ -561,6 +610,80 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
         converged = true;
       }
       break;
+    }
+  }
+  // ---- S5, deep-round regime (wl_deep.cuh): only the rows with a changed out-neighbour are recomputed ---------------------
+  if (deep_entered && !converged && r <= max_rounds) {
+    const u64 key = round_key(seed, stream_id, (u64)deep_start);  // the key of the switch round, kept from here on
+    int64_t* tp_ptr = (int64_t*)(ws + DL.o_tp_ptr);
+    int* tp_src = (int*)(ws + DL.o_tp_src);
+    int* size = (int*)(ws + DL.o_size);
+    int* inherit = (int*)(ws + DL.o_inherit);
+    int* mark = (int*)(ws + DL.o_mark);
+    int* lcount[2] = {(int*)(ws + DL.o_lcount[0]), (int*)(ws + DL.o_lcount[1])};
+    int* leavers[2] = {(int*)(ws + DL.o_leavers[0]), (int*)(ws + DL.o_leavers[1])};
+    int* leaver_block[2] = {(int*)(ws + DL.o_leaver_block[0]), (int*)(ws + DL.o_leaver_block[1])};
+    u32* slots = (u32*)(ws + DL.o_slots);
+    u64* bsum = (u64*)(ws + DL.o_bsum);
+    cudaEvent_t d0 = evp.get(2), d1 = evp.get(4);
+    cudaEventRecord(d0, st);
+    // the table is empty between deep rounds; every slot may be used
+    clean_table(table, dirty_mask, slot_of, dirty_first, dirty_count, st);
+    dirty_count = 0;
+    aux.need(st, table_slots, prefix_slots);
+    // in-neighbour lists: in-degrees -> offsets -> fill (the in-degree array counts down to zero and becomes `mark`)
+    cudaMemsetAsync(mark, 0, sizeof(int) * (size_t)n, st);
+    cudaMemsetAsync(size, 0, sizeof(int) * (size_t)n, st);
+    cudaMemsetAsync(lcount[0], 0, sizeof(int) * (size_t)n, st);
+    cudaMemsetAsync(lcount[1], 0, sizeof(int) * (size_t)n, st);
+    cudaMemsetAsync(inherit, 0, sizeof(int) * (size_t)n, st);
+    ++g_launches; deep_indegree_kernel<<<148 * 8, 256, 0, st>>>(m, g->col_idx + edge_first, mark);
+    launch_scan32(mark, n, 0, tp_ptr, bsum, bsum + (n / kScan32Chunk + 2), st);
+    ++g_launches; deep_fill_kernel<<<blocks_for(n * 32, 256), 256, 0, st>>>(n, g->row_ptr, g->col_idx, tp_ptr, mark, tp_src);
+    ++g_launches; deep_sizes_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, colour, size);
+    constexpr unsigned kDeepGrid = 148 * 4, kDeepFinGrid = 148;
+    auto front = [&](const DeepFinishArgs& fin, int do_front, int round) {
+      const int in = round & 1;
+      const unsigned grid = fin.fin_ctas + (do_front ? kDeepGrid : 0);
+      ++g_launches;
+      if (g->weights)
+        deep_front_kernel<true><<<grid, 256, 0, st>>>(fin, do_front, changed[in], deep + kDeepChanged0 + in, tp_ptr, tp_src, mark, round, g->row_ptr, g->col_idx, g->weights, colour, key, y, size, lcount[in], leavers[in], leaver_block[in], deep + kDeepLeavers0 + in, table, slots, deep, scal);
+      else
+        deep_front_kernel<false><<<grid, 256, 0, st>>>(fin, do_front, changed[in], deep + kDeepChanged0 + in, tp_ptr, tp_src, mark, round, g->row_ptr, g->col_idx, g->weights, colour, key, y, size, lcount[in], leavers[in], leaver_block[in], deep + kDeepLeavers0 + in, table, slots, deep, scal);
+    };
+    // the bookkeeping that closes `round` (rides in the launch that opens the next round, or alone at the end of a window)
+    auto closing = [&](int round, int log_slot) {
+      const int in = round & 1;
+      DeepFinishArgs f{kDeepFinGrid, leavers[in], leaver_block[in], lcount[in], kDeepLeavers0 + in, kDeepChanged0 + in, log_slot,
+                       scal + kScalLog};
+      return f;
+    };
+    while (r <= max_rounds && !converged) {
+      const int R = no_runahead ? 1 : (int)std::min<int64_t>(kRunAhead, max_rounds - r + 1);
+      for (int j = 0; j < R; ++j) {
+        const int round = (int)(r + j), in = round & 1, out = (round + 1) & 1;
+        front(j == 0 ? DeepFinishArgs{0, nullptr, nullptr, nullptr, 0, 0, 0, nullptr} : closing(round - 1, j - 1), 1, round);
+        ++g_launches; deep_relabel_kernel<<<kDeepGrid, 256, 0, st>>>(leavers[in], leaver_block[in], deep + kDeepLeavers0 + in, colour, y, size, lcount[in], inherit, round, table, L.table_mask, slots, deep + kDeepSlots, scal + kScalK, deep + kDeepNew, changed[out], deep + kDeepChanged0 + out);
+      }
+      front(closing((int)(r + R - 1), R - 1), 0, (int)(r + R));
+      cudaEventRecord(d1, st);
+      cudaMemcpyAsync(hs, scal, sizeof(u64) * kNumScal, cudaMemcpyDeviceToHost, st);
+      rc = check_cuda(cudaStreamSynchronize(st));
+      if (rc) return rc;
+      float t_win = 0;
+      cudaEventElapsedTime(&t_win, d0, d1);
+      ms_relabel += t_win;
+      cudaEventRecord(d0, st);
+      for (int j = 0; j < R && !converged; ++j) {
+        const int64_t k_new = (int64_t)hs[kScalLog + j];
+        rounds = (int32_t)(r + j);
+        log_round(r + j, k_new);
+        if (debug)
+          std::fprintf(stderr, "[wl_refine] round %lld: k %lld -> %lld (worklist)\n", (long long)(r + j), (long long)k, (long long)k_new);
+        if (k_new == k) converged = true;
+        k = k_new;
+      }
+      r += R;
     }
   }
   if (!cols_checked) {  // no round read a column (everything was settled by the degrees): check them now
@@ -608,7 +731,7 @@ int wl_refine(const wl_csr* g, const int32_t* init_colors, uint64_t seed, int32_
   cudaEvent_t ev_begin = evp.get(0), ev_end = evp.get(1);
   cudaEventRecord(ev_begin, st);
   CoreResult cr{};
-  const int core_rc = refine_core(g, init_colors, seed, opt, /*ranged=*/false, 0, 0, n, /*edge_first=*/0, workspace, L, st, &cr);
+  const int core_rc = refine_core(g, init_colors, seed, opt, /*ranged=*/false, 0, 0, n, /*edge_first=*/0, workspace, workspace_bytes, L, st, &cr);
   if (core_rc != WL_OK && core_rc != WL_EMAXROUNDS) return core_rc;
   char* ws = (char*)workspace;
   // ---- S6: canonical ids ---------------------------------------------------------------------------------------------
@@ -653,7 +776,7 @@ int wl_refine_host(const wl_csr* g, const int32_t* init_colors, uint64_t seed, i
   if (n == 0) return WL_OK;
   if (!out_colors) return WL_EINVAL;
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  const size_t wsb = wl_refine_workspace_bytes(n, m);
+  size_t wsb = wl_refine_deep_workspace_bytes(n, m);  // room for the deep-round regime if the device has it
   char* d_all = nullptr;
   size_t o_rp = 0, o_col, o_wt, o_init, o_out, o_ws, off = 0;
   auto take = [&](size_t b) {
@@ -666,10 +789,17 @@ int wl_refine_host(const wl_csr* g, const int32_t* init_colors, uint64_t seed, i
   o_wt = take(g->weights ? sizeof(u32) * (size_t)m : 0);
   o_init = take(init_colors ? sizeof(int) * (size_t)n : 0);
   o_out = take(sizeof(int) * (size_t)n);
+  const size_t off_before_ws = off;
   o_ws = take(wsb);
   if (cudaMalloc((void**)&d_all, off) != cudaSuccess) {
     cudaGetLastError();
-    return WL_ENOMEM;
+    wsb = wl_refine_workspace_bytes(n, m);
+    off = off_before_ws;
+    o_ws = take(wsb);
+    if (cudaMalloc((void**)&d_all, off) != cudaSuccess) {
+      cudaGetLastError();
+      return WL_ENOMEM;
+    }
   }
   cudaEvent_t e0, e1;
   cudaEventCreate(&e0);

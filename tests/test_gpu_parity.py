@@ -146,8 +146,9 @@ def test_canonicalize(n):
 
 
 # ------------------------------------------------------------------ whole Algorithm 1
+# 256 = WL_FLAG_NO_DEEP, 512 = WL_FLAG_DEEP_EARLY (worklist regime from round 2 on: every graph goes through it)
 @pytest.mark.parametrize("name", list(GRAPHS))
-@pytest.mark.parametrize("flags", [0, 2, 4, 64, 128, 128 | 2])
+@pytest.mark.parametrize("flags", [0, 2, 4, 64, 128, 128 | 2, 256, 512, 512 | 64, 512 | 2])
 def test_refine_equals_oracle(name, flags):
     g = GRAPHS[name]()
     n, rp, ci, wt = g.numpy()
@@ -160,16 +161,47 @@ def test_refine_equals_oracle(name, flags):
         assert res.colors.cpu().numpy().tolist() == want.tolist()
 
 
+@pytest.mark.parametrize("flags", [0, 512])
 @pytest.mark.parametrize("seed", range(20))
-def test_refine_many_seeds_rmat(seed):
+def test_refine_many_seeds_rmat(seed, flags):
     g = gg.rmat(10, edge_factor=8, seed=seed, symmetrize=bool(seed % 2))
     n, rp, ci, wt = g.numpy()
     init = None if seed % 3 == 0 else gg.random_partition(n, 1 + seed, seed)
     want, counts, rounds = oracle.refine(n, rp, ci, wt, None if init is None else init.numpy())
     dn, drp, dci, dwt = dgraph(g)
-    res = wl.wl_refine(dn, drp, dci, dwt, None if init is None else (init * 3 + 5).to(dev()), seed=seed * 977)
+    res = wl.wl_refine(dn, drp, dci, dwt, None if init is None else (init * 3 + 5).to(dev()), seed=seed * 977, flags=flags)
     assert res.round_colors == counts
     assert res.colors.cpu().numpy().tolist() == want.tolist()
+
+
+DEEP_GRAPHS = {
+    "path_3001": lambda: gg.path_graph(3001),
+    "dpath_700": lambda: gg.directed_path(700),
+    "grid_97": lambda: gg.grid2d(97),
+    "btree_11": lambda: gg.from_edge_list(2 ** 11 - 1, [(i, 2 * i + 1) for i in range(2 ** 10 - 1)] +
+                                          [(i, 2 * i + 2) for i in range(2 ** 10 - 1)]),
+    "btree_11_up": lambda: gg.from_edge_list(2 ** 11 - 1, [(2 * i + 1, i) for i in range(2 ** 10 - 1)] +
+                                             [(2 * i + 2, i) for i in range(2 ** 10 - 1)]),
+    "weighted_chain": lambda: gg.from_edge_list(400, [(i, i + 1) for i in range(399)] + [(i + 1, i) for i in range(399)],
+                                                weights=[1 + (i % 3) for i in range(399)] * 2),
+    "comb": lambda: gg.from_edge_list(600, [(i, i + 1) for i in range(299)] + [(i + 1, i) for i in range(299)] +
+                                      [(i, 300 + i) for i in range(300)] + [(300 + i, i) for i in range(300)]),
+}
+
+
+@pytest.mark.parametrize("name", list(DEEP_GRAPHS))
+@pytest.mark.parametrize("flags", [0, 64, 256, 512])
+def test_refine_deep_rounds_equal_oracle(name, flags):
+    """Graphs that need tens to thousands of rounds: the worklist regime (rounds > 6, wl_deep.cuh) must give the oracle's
+    colouring AND its per-round colour counts, with and without run-ahead windows, and the same as the plain loop (256)."""
+    g = DEEP_GRAPHS[name]()
+    n, rp, ci, wt = g.numpy()
+    want, counts, rounds = oracle.refine(n, rp, ci, wt)
+    dn, drp, dci, dwt = dgraph(g)
+    for seed in (0, 7):
+        res = wl.wl_refine(dn, drp, dci, dwt, seed=seed, flags=flags)
+        assert res.rounds == rounds and res.round_colors == counts
+        assert res.colors.cpu().numpy().tolist() == want.tolist()
 
 
 def test_refine_weighted_equals_multigraph():
