@@ -357,6 +357,7 @@ def main():
                     "avg_launch_ms": top_ms, "launches_timed": len(results),
                     "gedges_per_s_in_kernel": top_edges / (top_ms / 1e3) / 1e9,
                     "traffic": NCU_TRAFFIC_BYTES if args.scale == 27 and not args.flags else None,
+                    "dram_gb_per_s_ncu_traffic": (NCU_TRAFFIC_BYTES / (top_ms / 1e3) / 1e9) if args.scale == 27 and not args.flags else None,
                     "traffic_source": "profiles/r1d_ncu_full.md (dram__bytes_read.sum + dram__bytes_write.sum, row + hub kernel)",
                     "share_of_step": top_ms / ms_per_step,
                     "all_spmv_launches": {"launches": spmv_launches, "algorithmic_gb_per_s": alg_bytes / (spmv_ms / 1e3) / 1e9,
