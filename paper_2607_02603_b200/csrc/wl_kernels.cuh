@@ -41,37 +41,6 @@ __global__ void validate_rows_kernel(int64_t n, const int64_t* __restrict__ row_
   if (e) atomicOr(err, e);
 }
 
-// S0 for a uniform start with unit weights, one pass over row_ptr: the offsets are validated (as validate_rows_kernel),
-// every node gets colour 0, y_i = outdeg(i) * w0 is round 1's product (R2: with one colour no column needs to be read)
-// and the rows longer than hub_threshold are cut into chunks (as hub_collect_kernel).
-__global__ void s0_uniform_kernel(int64_t n, const int64_t* __restrict__ row_ptr, int64_t expect_first, int64_t expect_last,
-                                  u64 w0, int* __restrict__ colour, unsigned short* __restrict__ colour16,
-                                  u64* __restrict__ y, int64_t hub_threshold, int2* __restrict__ chunks, int64_t hub_cap,
-                                  u64* __restrict__ hub_counter, u32* __restrict__ err) {
-  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n) return;
-  const int64_t a = row_ptr[i], b = row_ptr[i + 1];
-  u32 e = 0;
-  if (i == 0 && a != expect_first) e |= kErrRowPtr;
-  if (i == n - 1 && b != expect_last) e |= kErrRowPtr;
-  if (a > b || a < expect_first || b > expect_last) e |= kErrRowPtr;
-  int64_t d = e ? 0 : b - a;
-  if ((u64)d >= (1ull << 32)) e |= kErrRowSum, d = 0;
-  colour[i] = 0;
-  colour16[i] = 0;
-  y[i] = (u64)d * w0;
-  if (d > hub_threshold) {
-    const int nc = (int)((d + kHubChunk - 1) / kHubChunk);
-    const u64 base = atomicAdd(hub_counter, (u64)nc);
-    if ((int64_t)(base + nc) <= hub_cap) {
-      for (int c = 0; c < nc; ++c) chunks[base + c] = make_int2((int)i, c);
-    } else {
-      e |= kErrRowPtr;  // only overlapping (malformed) rows can exceed the capacity derived from m
-    }
-  }
-  if (e) atomicOr(err, e);
-}
-
 // every stored target must be a node id in [0, n_targets); entries [begin, m) of col are checked
 __global__ void validate_cols_kernel(int64_t n_targets, int64_t begin, int64_t m, const int* __restrict__ col,
                                      u32* __restrict__ err) {
@@ -729,6 +698,106 @@ relabel_kernel(int64_t count, const int* __restrict__ nodes, int* __restrict__ c
       if (ch) changed[base + __popc(bal & ((1u << lane) - 1))] = i;
     }
   }
+}
+
+// S0 + round 1 in one pass for a uniform start with unit weights (R2): z_i = outdeg(i) * w(0), so the round only reads
+// row_ptr.  Per node: offsets validated (as validate_rows_kernel), hub rows cut into chunks (as hub_collect_kernel), the
+// key (0, z_i) relabelled exactly as relabel_kernel does (node 0 represents colour 0), and the node appended to the active
+// list unless it has no out-edge (the class of edgeless nodes is represented by an edgeless node: it never needs another
+// look, see compact_active_kernel).  z is not stored: round 2 recomputes it for every listed row before reading it.
+// The list is a superset of what compact_active_kernel would keep (it keeps the few nodes whose degree is unique);
+// counters[0] = listed rows, counters[1] = their out-degree sum (= m), *hub_rows = listed rows longer than hub_threshold.
+__global__ void __launch_bounds__(kRelabelThreads)
+round1_uniform_kernel(int64_t n, const int64_t* __restrict__ row_ptr, int64_t expect_first, int64_t expect_last, u64 w0,
+                      int* __restrict__ colour, unsigned short* __restrict__ colour16, int* __restrict__ rep,
+                      int* __restrict__ stamp, Slot* __restrict__ table, u32 table_mask, u32* __restrict__ slot_of,
+                      u64* __restrict__ new_counter, int64_t hub_threshold, int2* __restrict__ chunks, int64_t hub_cap,
+                      u64* __restrict__ hub_counter, int* __restrict__ active, u64* __restrict__ counters,
+                      u64* __restrict__ hub_rows, u32* __restrict__ err) {
+  constexpr int round = 1, k_old = 1;
+  const int64_t t = (int64_t)blockIdx.x * kRelabelThreads + threadIdx.x;
+  const bool valid = t < n;
+  const int i = (int)t;
+  int64_t d = 0;
+  if (valid) {
+    const int64_t a = row_ptr[t], b = row_ptr[t + 1];
+    u32 e = 0;
+    if (t == 0 && a != expect_first) e |= kErrRowPtr;
+    if (t == n - 1 && b != expect_last) e |= kErrRowPtr;
+    if (a > b || a < expect_first || b > expect_last) e |= kErrRowPtr;
+    d = e ? 0 : b - a;
+    if ((u64)d >= (1ull << 32)) e |= kErrRowSum, d = 0;
+    if (d > hub_threshold) {
+      const int nc = (int)((d + kHubChunk - 1) / kHubChunk);
+      const u64 base = atomicAdd(hub_counter, (u64)nc);
+      if ((int64_t)(base + nc) <= hub_cap) {
+        for (int c = 0; c < nc; ++c) chunks[base + c] = make_int2(i, c);
+      } else {
+        e |= kErrRowPtr;  // only overlapping (malformed) rows can exceed the capacity derived from m
+      }
+      atomicAdd(hub_rows, 1ull);
+    }
+    if (e) atomicOr(err, e);
+  }
+  // the representative of colour 0 is node 0
+  int64_t d0 = row_ptr[1] - row_ptr[0];
+  if (d0 < 0 || (u64)d0 >= (1ull << 32)) d0 = 0;
+  bool win = false, lose = false;
+  u32 slot = 0, id = 0;
+  if (valid) {
+    const u64 yi = (u64)d * w0;
+    if (d == d0) {
+      if (i != 0 && stamp[0] != round) stamp[0] = round;
+    } else {
+      id = kPending;
+      const Slot mine = {yi, (u64)kPending << 32};
+      const Slot empty = {kEmpty, kEmpty};
+      slot = (u32)slot_hash(0u, yi) & table_mask;
+      while (true) {
+        Slot v = load_slot(table + slot);
+        if (v.y == kEmpty || v.cx == kEmpty) {
+          v = cas128(table + slot, empty, mine);
+          if (v.y == kEmpty && v.cx == kEmpty) {
+            win = true;
+            break;
+          }
+        }
+        if (v.y == yi && (u32)v.cx == 0u) {
+          lose = true;
+          id = (u32)(v.cx >> 32);
+          break;
+        }
+        slot = (slot + 1) & table_mask;
+      }
+    }
+  }
+  int total;
+  const int rank = block_rank<kRelabelThreads>(win, &total);
+  __shared__ u64 s_base;
+  if (threadIdx.x == 0 && total > 0) s_base = atomicAdd(new_counter, (u64)total);
+  __syncthreads();
+  if (win) {
+    id = (u32)(k_old + (int)s_base + rank);
+    st_slot_id(table + slot, id);
+    rep[id] = i;
+    slot_of[id] = slot;
+  } else if (lose) {
+    while (id == kPending) id = ld_slot_id(table + slot);
+    if (stamp[id] != round) stamp[id] = round;
+  }
+  if (valid) {
+    colour[i] = (int)id;
+    colour16[i] = (unsigned short)id;
+  }
+  // active list: every node with an out-edge
+  const bool keep = valid && d > 0;
+  int kept;
+  const int krank = block_rank<kRelabelThreads>(keep, &kept);
+  __shared__ u64 s_list;
+  if (threadIdx.x == 0 && kept > 0) s_list = atomicAdd(counters, (u64)kept);
+  __syncthreads();
+  if (keep) active[s_list + krank] = i;
+  if (t == 0) counters[1] = (u64)(expect_last - expect_first);
 }
 
 // End of a round (S4): if `clean`, the slots claimed by this round's new ids are emptied again (the table is empty

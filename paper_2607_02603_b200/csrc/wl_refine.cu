@@ -394,9 +394,16 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
     cudaEventRecord(aux.done_b, aux.s);
     aux.active = true;
   }
+  // rep[0] = node 0; stamp[0] = 0 marks block 0 as non-singleton; one colour
+  cudaMemsetAsync(rep, 0, sizeof(int), st);
+  cudaMemsetAsync(stamp, 0, sizeof(int), st);
+  hs[kNumScal] = 1;
+  cudaMemcpyAsync(scal + kScalK, hs + kNumScal, sizeof(u64), cudaMemcpyHostToDevice, st);
   if (uniform_start) {
+    // S0 and round 1 in one pass over row_ptr (round1_uniform_kernel); the loop below only closes the round
     const u64 w0 = weight_of(round_key(seed, stream_id, 1), 0);
-    ++g_launches; s0_uniform_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, g->row_ptr, edge_first, edge_first + m, w0, colour, colour16, y, kHubThreshold, hub_chunks, L.hub_cap, scal + kScalHub, d_err);
+    const u32 mask1 = overlap ? (u32)(prefix_slots - 1) : L.table_mask;
+    ++g_launches; round1_uniform_kernel<<<blocks_for(n, kRelabelThreads), kRelabelThreads, 0, st>>>(n, g->row_ptr, edge_first, edge_first + m, w0, colour, colour16, rep, stamp, table, mask1, slot_of, scal + kScalNew, kHubThreshold, hub_chunks, L.hub_cap, scal + kScalHub, act[0], scal + kScalActive, scal + kScalActiveHub, d_err);
   } else {
     if (!cols_checked) {
       ++g_launches; validate_cols_kernel<<<148 * 8, 256, 0, st>>>(n_targets, edge_first, edge_first + m, g->col_idx, d_err);
@@ -408,11 +415,6 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
     ++g_launches; init_labels_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, init_colors, colour, colour16, y, d_err);
   }
   int64_t k = 1;
-  // rep[0] = node 0; stamp[0] = 0 marks block 0 as non-singleton
-  cudaMemsetAsync(rep, 0, sizeof(int), st);
-  cudaMemsetAsync(stamp, 0, sizeof(int), st);
-  hs[kNumScal] = 1;
-  cudaMemcpyAsync(scal + kScalK, hs + kNumScal, sizeof(u64), cudaMemcpyHostToDevice, st);
   int64_t num_hub_chunks = 0;
   if (!uniform_start) {
     if (init_colors)
@@ -449,9 +451,9 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
     const u64 key = round_key(seed, stream_id, (u64)r);
     bool streamed = false;
     u32 mask_r = round_table_mask(L, n_active);
-    if (k == 1 && uniform_start && r == 1) {
-      // y = outdeg * w(0) was written by s0_uniform_kernel (R2); its keys fit the table prefix emptied on `st`
-      if (aux.active) mask_r = (u32)(prefix_slots - 1);
+    const bool round1_done = uniform_start && r == 1;  // round1_uniform_kernel did S1-S3 (R2); only S4 is left
+    if (round1_done) {
+      mask_r = aux.active ? (u32)(prefix_slots - 1) : L.table_mask;  // the slots its keys may have claimed
     } else {
       if (merge) cudaMemsetAsync(y, 0, sizeof(u64) * (size_t)n, st);
       // row kernels over the active list by default; WL_FLAG_EDGE_BALANCED: the edge-balanced kernel over all rows
@@ -491,12 +493,16 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
     clean_table(table, dirty_mask, slot_of, dirty_first, dirty_count, st);
     dirty_count = 0;
     dirty_mask = mask_r;
-    launch_relabel(mask_r, n_active, cur_list, colour, mirror ? colour16 : nullptr, y, rep, stamp, (int)r, table, slot_of,
+    launch_relabel(mask_r, round1_done ? 0 : n_active, cur_list, colour, mirror ? colour16 : nullptr, y, rep, stamp, (int)r, table, slot_of,
                    scal, log, log_slot, clean, st, list_changed ? changed[(r + 1) & 1] : nullptr,
                    list_changed ? deep + kDeepChanged0 + ((r + 1) & 1) : nullptr);
     return streamed;
   };
   auto queue_compaction = [&](int64_t r) {
+    if (uniform_start && r == 1) {  // round1_uniform_kernel listed every row with an out-edge and counted them
+      dropped_checked = true;       // the rows it dropped have no columns
+      return;
+    }
     cudaMemsetAsync(scal + kScalActive, 0, 2 * sizeof(u64), st);
     cudaMemsetAsync(scal + kScalActiveHub, 0, sizeof(u64), st);
     // while the column range check is pending the rows dropped here are checked here (a row kernel never reads them)
