@@ -66,6 +66,7 @@ typedef struct wl_csr {
                                       headline graph, kept for extreme degree skew)                          */
 #define WL_FLAG_NO_DEEP 256u     /* never switch to the worklist regime (below): every round recomputes every active row */
 #define WL_FLAG_DEEP_EARLY 512u  /* switch to the worklist regime at round 2 instead of round 7 (testing)                 */
+#define WL_FLAG_NO_FINAL 1024u   /* do not drop blocks whose whole neighbourhood is final from the active set (R5)        */
 #define WL_FLAG_NO_CANONICAL 16u /* leave internal dense ids in out_colors (skips S6)                                  */
 
 typedef struct wl_options {

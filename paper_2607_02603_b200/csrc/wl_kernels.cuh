@@ -530,14 +530,17 @@ __global__ void narrow_kernel(int64_t n, const int* __restrict__ colour, unsigne
 // id, so its row needs neither y nor a relabel.  next = nodes of `nodes` (NULL: all) whose block still has >= 2 members
 // after round `round`; counters[0] += |next|, counters[1] += sum of their out-degrees.  Rows without out-edges are
 // dropped as soon as their block's representative has none either (their y is 0 in every round).
+// final_col != NULL: blocks whose neighbourhood is final are dropped as well (see below; k_prev = colour count before the
+// round that just ended).
 // check_col != NULL (the column range check of S0 is still pending): the rows dropped here are never read
 // by a row kernel, so their columns are range-checked now, one warp per row (hub rows are left to spmv_hub_kernel).
+constexpr int kFinalRow = 32;  // rows up to this length are tested for finality
 __global__ void __launch_bounds__(256)
 compact_active_kernel(int64_t count, const int* __restrict__ nodes, const int* __restrict__ colour,
                       const int* __restrict__ stamp, const int* __restrict__ rep, int round,
                       const int64_t* __restrict__ row_ptr, int64_t hub_threshold, int* __restrict__ next,
                       u64* __restrict__ counters, u64* __restrict__ hub_counter, const int* __restrict__ check_col,
-                      int64_t n_targets, u32* __restrict__ err) {
+                      int64_t n_targets, u32* __restrict__ err, const int* __restrict__ final_col, int k_prev) {
   int64_t t = (int64_t)blockIdx.x * 256 + threadIdx.x;
   bool keep = false;
   int i = 0;
@@ -573,6 +576,21 @@ compact_active_kernel(int64_t count, const int* __restrict__ nodes, const int* _
         // out-edge is compared against y[rep] = 0 and leaves on its own; the edgeless members never need another look.
         const int r = rep[c];
         keep = row_ptr[r + 1] != row_ptr[r];
+      } else if (final_col && deg <= kFinalRow) {
+        // Final block (R5): every out-neighbour's colour existed before this round (id < k_prev) and its block was
+        // already out of the loop then (singleton or dropped: not seen with two members in the previous round).  This
+        // round's y was computed from exactly those colours, so the nodes that share this block have the same
+        // neighbour colours, all of which never change again: the block can never split.
+        const int64_t a = row_ptr[i];
+        bool all_final = true;
+        for (int64_t p = a; p < a + (int64_t)deg; ++p) {
+          const int cj = colour[final_col[p]];
+          if (cj >= k_prev || stamp[cj] >= round - 1) {
+            all_final = false;
+            break;
+          }
+        }
+        keep = !all_final;
       }
     }
   }

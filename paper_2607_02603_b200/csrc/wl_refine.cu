@@ -295,9 +295,16 @@ struct AuxStream {
     cudaEventCreateWithFlags(&done_b, cudaEventDisableTiming);
     return WL_OK;
   }
+  Slot* table = nullptr;
+  bool b_issued = false;  // the upper piece is only emptied if a round ever needs it (R-MAT: never, half the memset saved)
   // make `st` wait until slots [0, slots) are empty
   void need(cudaStream_t st, u64 slots, u64 prefix) {
     if (!active || slots <= prefix) return;
+    if (slots > slots_a && !b_issued) {
+      cudaMemsetAsync(table + slots_a, 0xff, sizeof(Slot) * (slots_b - slots_a), s);
+      cudaEventRecord(done_b, s);
+      b_issued = true;
+    }
     cudaStreamWaitEvent(st, slots <= slots_a ? done_a : done_b, 0);
   }
   ~AuxStream() {
@@ -390,8 +397,7 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
     aux.slots_b = table_slots;
     if (aux.slots_a > prefix_slots) cudaMemsetAsync(table + prefix_slots, 0xff, sizeof(Slot) * (aux.slots_a - prefix_slots), aux.s);
     cudaEventRecord(aux.done_a, aux.s);
-    cudaMemsetAsync(table + aux.slots_a, 0xff, sizeof(Slot) * (aux.slots_b - aux.slots_a), aux.s);
-    cudaEventRecord(aux.done_b, aux.s);
+    aux.table = table;
     aux.active = true;
   }
   // rep[0] = node 0; stamp[0] = 0 marks block 0 as non-singleton; one colour
@@ -498,7 +504,8 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
                    list_changed ? deep + kDeepChanged0 + ((r + 1) & 1) : nullptr);
     return streamed;
   };
-  auto queue_compaction = [&](int64_t r) {
+  // final_test: also drop the blocks whose neighbourhood can no longer change (R5); k_prev = colours before round r
+  auto queue_compaction = [&](int64_t r, bool final_test = false, int64_t k_prev = 0) {
     if (uniform_start && r == 1) {  // round1_uniform_kernel listed every row with an out-edge and counted them
       dropped_checked = true;       // the rows it dropped have no columns
       return;
@@ -507,7 +514,7 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
     cudaMemsetAsync(scal + kScalActiveHub, 0, sizeof(u64), st);
     // while the column range check is pending the rows dropped here are checked here (a row kernel never reads them)
     const bool check = !cols_checked && !merge && !ranged;
-    ++g_launches; compact_active_kernel<<<blocks_for(n_active, 256), 256, 0, st>>>(n_active, cur_list, colour, stamp, rep, (int)r, g->row_ptr, kHubThreshold, act[cur], scal + kScalActive, scal + kScalActiveHub, check ? g->col_idx : nullptr, n_targets, d_err);
+    ++g_launches; compact_active_kernel<<<blocks_for(n_active, 256), 256, 0, st>>>(n_active, cur_list, colour, stamp, rep, (int)r, g->row_ptr, kHubThreshold, act[cur], scal + kScalActive, scal + kScalActiveHub, check ? g->col_idx : nullptr, n_targets, d_err, final_test ? g->col_idx : nullptr, (int)k_prev);
     if (check) dropped_checked = true;
   };
   // host side of a compaction whose counters have been read back; returns true when nothing is left to refine
@@ -552,8 +559,15 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
     for (int j = 0; j < R; ++j)
       streamed[j] = queue_round(r + j, narrow, narrow, /*clean=*/window, scal + kScalLog, j, evp.get(8 + 2 * j), evp.get(9 + 2 * j), switch_round);
     const int64_t r_last = r + R - 1;
-    const bool compact_now = prune && !switch_round && (window || r <= 2 || pending_new * 16 >= n_active);
-    if (compact_now) queue_compaction(r_last);
+    // compaction rides behind rounds 1-2 and behind every window; in between it is decided after the round, when the host
+    // knows how many colours the round made (below)
+    const bool compact_now = prune && !switch_round && (window || r <= 2);
+    const int64_t k_before = k;
+    // the finality test needs the colour count before the round (host-known in the one-round-per-sync regime only) and a
+    // column check that is over; it pays when the rows that are left are short
+    const bool final_test = !window && !ranged && !(flags & WL_FLAG_NO_FINAL) && r >= 2 && cols_checked &&
+                            active_edges <= 8 * n_active;
+    if (compact_now) queue_compaction(r_last, final_test, k);
     cudaEventRecord(e2, st);
     cudaMemcpyAsync(hs, scal, sizeof(u64) * kNumScal, cudaMemcpyDeviceToHost, st);
     rc = check_cuda(cudaStreamSynchronize(st));
@@ -607,7 +621,15 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
       deep_entered = true;
       break;
     }
-    if (compact_now && adopt_compaction()) {
+    bool late_compact = false;
+    if (!compact_now && prune && !window && pending_new * 16 >= n_active) {
+      queue_compaction(r_last, final_test, k_before);
+      cudaMemcpyAsync(hs, scal, sizeof(u64) * kNumScal, cudaMemcpyDeviceToHost, st);
+      rc = check_cuda(cudaStreamSynchronize(st));
+      if (rc) return rc;
+      late_compact = true;
+    }
+    if ((compact_now || late_compact) && adopt_compaction()) {
       // every block is a singleton (or can never split again): the next round cannot change anything and only
       // confirms (same trajectory as the un-pruned algorithm)
       if (r <= max_rounds) {

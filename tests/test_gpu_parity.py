@@ -146,9 +146,10 @@ def test_canonicalize(n):
 
 
 # ------------------------------------------------------------------ whole Algorithm 1
-# 256 = WL_FLAG_NO_DEEP, 512 = WL_FLAG_DEEP_EARLY (worklist regime from round 2 on: every graph goes through it)
+# 256 = WL_FLAG_NO_DEEP, 512 = WL_FLAG_DEEP_EARLY (worklist regime from round 2 on: every graph goes through it),
+# 1024 = WL_FLAG_NO_FINAL (no finality pruning)
 @pytest.mark.parametrize("name", list(GRAPHS))
-@pytest.mark.parametrize("flags", [0, 2, 4, 64, 128, 128 | 2, 256, 512, 512 | 64, 512 | 2])
+@pytest.mark.parametrize("flags", [0, 2, 4, 64, 128, 128 | 2, 256, 512, 512 | 64, 512 | 2, 1024, 1024 | 256])
 def test_refine_equals_oracle(name, flags):
     g = GRAPHS[name]()
     n, rp, ci, wt = g.numpy()
