@@ -56,3 +56,16 @@ def test_strerror():
     import paper_2607_02603_b200 as wl
     assert wl.wl_strerror(0) == "ok"
     assert "workspace" in wl.wl_strerror(wl.WL_ENOMEM)
+
+
+def test_deep_and_batched_workspace_sizes():
+    import paper_2607_02603_b200 as wl
+    base = wl.wl_refine_workspace_bytes(1000, 5000)
+    deep = wl.wl_refine_deep_workspace_bytes(1000, 5000)
+    # the deep-round regime adds the in-neighbour lists (8(n+1) + 4m) and its work lists
+    assert deep >= base + 8 * 1001 + 4 * 5000
+    assert wl.wl_refine_deep_workspace_bytes(-1, 0) == 0
+    assert wl.wl_refine_deep_workspace_bytes(2000, 5000) >= deep
+    # pinned scratch of the batched path: two offset arrays + one weighted entry array
+    hb = wl.wl_refine_batched_host_bytes(1000, 5000)
+    assert hb >= 2 * 8 * 1001 + 8 * 5000 and wl.wl_refine_batched_host_bytes(-1, 0) == 0

@@ -124,6 +124,47 @@ def test_batched_cut_inside_a_long_row():
     assert oracle.is_stable(n, rp, ci, wt, res.colors.numpy())
 
 
+def test_batched_with_caller_host_workspace_and_long_hub_rows():
+    """The pinned host scratch of the quotients supplied by the caller (later quotients are written in place), on a graph
+    whose hub rows exceed kQuotLongRow (quot_insert_long_kernel) and are cut by batch borders; a workspace that is too
+    small is ignored (the library pins its own)."""
+    edges = [(h, j) for h in (0, 1, 2) for j in range(3, 9003)] + [(j, j + 1) for j in range(3, 9002)] + \
+            [(j, 0) for j in range(100, 4700)]
+    g = gg.from_edge_list(9003, edges)
+    n, rp, ci, wt = g.numpy()
+    cap = 5000
+    want, k_want, outer_want, nbl_want = oracle.rbsc(n, rp, ci, wt, cap)
+    rp_p, col_p = g.row_ptr.pin_memory(), g.col.pin_memory()
+    hws = torch.empty(wl.wl_refine_batched_host_bytes(n, g.m), dtype=torch.uint8).pin_memory()
+    small = torch.empty(64, dtype=torch.uint8).pin_memory()
+    for ws in (hws, small, None):
+        res = wl.wl_refine_batched(n, rp_p, col_p, None, max_batch_edges=cap, seed=9, host_workspace=ws)
+        assert res.colors.numpy().tolist() == want.tolist()
+        assert res.stats["outer_iters"] == outer_want and res.stats["last_num_batches"] == nbl_want
+    assert oracle.is_stable(n, rp, ci, wt, res.colors.numpy())
+
+
+def test_batched_device_cap_is_checked_for_every_allocation():
+    """A cap that admits the buffers of the local-refinement pass but not those of the quotient pass must give WL_ENOMEM
+    (a failed allocation used to be overwritten by the next successful one)."""
+    g = gg.rmat(12, seed=5, symmetrize=False)
+    cap_edges = g.m // 4 + 1
+    ok = wl.wl_refine_batched(g.n, g.row_ptr, g.col, None, max_batch_edges=cap_edges, seed=1)
+    assert ok.stats["outer_iters"] >= 2
+    # bisect the smallest cap that works; every smaller cap must fail cleanly with WL_ENOMEM, never with a CUDA error
+    lo, hi = 4096, 1 << 30
+    while hi - lo > 4096:
+        mid = (lo + hi) // 2
+        try:
+            r = wl.wl_refine_batched(g.n, g.row_ptr, g.col, None, max_batch_edges=cap_edges, seed=1, device_cap_bytes=mid)
+            assert r.colors.tolist() == ok.colors.tolist()
+            hi = mid
+        except wl.WlError as e:
+            assert e.code == wl.WL_ENOMEM
+            lo = mid
+    assert hi < (1 << 30)
+
+
 def test_batched_device_cap_and_limits():
     g = gg.rmat(10, seed=1)
     with pytest.raises(wl.WlError) as e:
