@@ -29,8 +29,8 @@ if ROOT not in sys.path:
 RMAT_SEEDS = {22: 1, 27: 2, 30: 3}  # BASELINE.json configs[2..4]
 ORACLE_SAMPLE_SCALE = 21           # bounded sample of the same recipe for the CPU oracle (about 10-30 s)
 HBM_FALLBACK_GBS = 6650.0          # /opt/skills/guides/B200_PROFILING.md fallback
-# DRAM bytes of the dominant launch (round-2 row kernel 40.70 + 0.74 GB, hub kernel 8.49 + 0.005 GB), ncu --set full
-NCU_TRAFFIC_BYTES = 49.94e9
+# DRAM bytes of the dominant launch (round-2 row kernel 40.71 + 0.74 GB, hub kernel 8.49 + 0.005 GB), ncu --set full
+NCU_TRAFFIC_BYTES = 49.95e9
 
 
 def measured_peaks():
@@ -358,7 +358,7 @@ def main():
                     "gedges_per_s_in_kernel": top_edges / (top_ms / 1e3) / 1e9,
                     "traffic": NCU_TRAFFIC_BYTES if args.scale == 27 and not args.flags else None,
                     "dram_gb_per_s_ncu_traffic": (NCU_TRAFFIC_BYTES / (top_ms / 1e3) / 1e9) if args.scale == 27 and not args.flags else None,
-                    "traffic_source": "profiles/r1d_ncu_full.md (dram__bytes_read.sum + dram__bytes_write.sum, row + hub kernel)",
+                    "traffic_source": "profiles/r1g_final_build.md (dram__bytes_read.sum + dram__bytes_write.sum, row + hub kernel)",
                     "share_of_step": top_ms / ms_per_step,
                     "all_spmv_launches": {"launches": spmv_launches, "algorithmic_gb_per_s": alg_bytes / (spmv_ms / 1e3) / 1e9,
                                           "gedges_per_s": spmv_edges / (spmv_ms / 1e3) / 1e9,
