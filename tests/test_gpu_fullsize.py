@@ -115,3 +115,27 @@ def test_c4_rmat27_properties_and_sampled_stability():
     if lens[0] != lens[other]:
         bad[0] = colours[other]
         assert not oracle.is_stable(sub_n, rp_full.numpy(), col_full.numpy(), None, bad.numpy())
+
+
+def test_c5_shape_batched_rmat20_directed():
+    """The shape of configs[4] at a size the oracle finishes: directed R-MAT scale 20 (1.05 M nodes, ~16 M edges) in pinned
+    host memory, 16 batches, caller-supplied pinned scratch.  Theorem 2 (stable on the original graph), L165 (refines the
+    coarsest colouring), seed independence, and bit-exact agreement with the CPU Algorithm 2 on the same edge partition."""
+    from helpers import refines
+    g = gg.rmat(20, seed=3, symmetrize=False, device=dev())
+    n, m = g.n, g.m
+    rp, col = g.row_ptr.cpu().pin_memory(), g.col.cpu().pin_memory()
+    hws = torch.empty(wl.wl_refine_batched_host_bytes(n, m), dtype=torch.uint8).pin_memory()
+    cap = m // 16 + 1
+    res = wl.wl_refine_batched(n, rp, col, None, max_batch_edges=cap, seed=1, host_workspace=hws, device_cap_bytes=2 << 30)
+    res2 = wl.wl_refine_batched(n, rp, col, None, max_batch_edges=cap, seed=77, host_workspace=hws)
+    assert res.stats["outer_iters"] >= 2 and res.stats["bytes_h2d"] > 2 * 4 * m
+    assert torch.equal(res.colors, res2.colors)
+    got = res.colors.numpy()
+    rpn, cin = rp.numpy(), col.numpy()
+    assert oracle.is_stable(n, rpn, cin, None, got)
+    coarsest, _, _ = oracle.refine(n, rpn, cin)
+    assert refines(got, coarsest) and res.num_colors >= int(coarsest.max()) + 1
+    want, k_want, outer_want, nbl_want = oracle.rbsc(n, rpn, cin, None, cap)
+    assert res.num_colors == k_want and res.stats["outer_iters"] == outer_want
+    assert (got == want).all()
