@@ -565,7 +565,9 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
     const int64_t k_before = k;
     // the finality test needs the colour count before the round (host-known in the one-round-per-sync regime only) and a
     // column check that is over; it pays when the rows that are left are short
-    const bool final_test = !window && !ranged && !(flags & WL_FLAG_NO_FINAL) && r >= 2 && cols_checked &&
+    // (unit weights only: there the members of a block have the same number of entries, so the row-length limit of the
+    // test treats them alike and a block leaves as a whole; its representative's y is never read again)
+    const bool final_test = !window && !ranged && !g->weights && !(flags & WL_FLAG_NO_FINAL) && r >= 2 && cols_checked &&
                             active_edges <= 8 * n_active;
     if (compact_now) queue_compaction(r_last, final_test, k);
     cudaEventRecord(e2, st);

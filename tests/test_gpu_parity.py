@@ -50,6 +50,10 @@ GRAPHS = {
     "empty_edges": lambda: gg.from_edge_list(17, []),
     "one_node": lambda: gg.from_edge_list(1, []),
     "self_loops": lambda: gg.from_edge_list(4, [(0, 0), (1, 1), (2, 3)]),
+    # duplicate CSR entries add (Q10); many sinks, twins and repeated targets: the finality pruning (R5) sees blocks whose
+    # members reach the same final colours through different nodes
+    "multigraph": lambda: gg.from_edge_list(400, [((7 * t) % 130, 130 + (t * t) % 270) for t in range(1500)] +
+                                            [(t % 130, (3 * t) % 130) for t in range(260)]),
     "weighted": lambda: gg.random_weighted_digraph(500, 3000, 5, max_w=4),
     "weighted_big_w": lambda: gg.random_weighted_digraph(200, 2000, 6, max_w=1 << 20),
 }
