@@ -67,6 +67,10 @@ typedef struct wl_csr {
 #define WL_FLAG_NO_DEEP 256u     /* never switch to the worklist regime (below): every round recomputes every active row */
 #define WL_FLAG_DEEP_EARLY 512u  /* switch to the worklist regime at round 2 instead of round 7 (testing)                 */
 #define WL_FLAG_NO_FINAL 1024u   /* do not drop blocks whose whole neighbourhood is final from the active set (R5)        */
+#define WL_FLAG_INHERIT_BATCHES 4096u /* batched: from the second outer iteration on, a quotient keeps the batches of its
+                                        graph (the rows emitted together) instead of being re-cut by M_b, and its local
+                                        refinement runs while those rows are still on the device: one upload pass per
+                                        iteration instead of two (reading Q14b)                               */
 #define WL_FLAG_NO_CANONICAL 16u /* leave internal dense ids in out_colors (skips S6)                                  */
 
 typedef struct wl_options {

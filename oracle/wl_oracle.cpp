@@ -224,8 +224,12 @@ static void greedy_cuts(i64 n, const i64* rp, i64 cap, std::vector<i64>& cuts) {
   }
 }
 
+// inherit != 0 (reading Q14b): from the second outer iteration on the edge partition is not re-cut by M_b;
+// the quotient inherits the batches of its graph: batch k of the quotient = the blocks whose representative row is complete
+// once batch k of the graph has been read (in node order), with exactly their rows.  L163 allows any partition.
 i64 oracle_rbsc(i64 n0, const i64* row_ptr0, const i32* col0, const u32* wt0, i64 max_batch_edges,
-                i32 nb0, const i64* first_cuts, const i32* first_edge_batch, i32 max_outer, i32* out, i64* stats) {
+                i32 nb0, const i64* first_cuts, const i32* first_edge_batch, i32 max_outer, i32 inherit, i32* out,
+                i64* stats) {
   i64 n = n0;
   std::vector<i64> rp(row_ptr0, row_ptr0 + n0 + 1);
   std::vector<i32> col(col0, col0 + rp[n0]);
@@ -235,13 +239,20 @@ i64 oracle_rbsc(i64 n0, const i64* row_ptr0, const i32* col0, const u32* wt0, i6
   for (i64 i = 0; i < n0; ++i) map[i] = (i32)i;
   i32 outer = 0;
   i64 nb_last = 0;
+  std::vector<i64> inh_cuts, inh_nodes;  // inherit: edge cuts and node ranges of the coming iteration
   while (true) {
     ++outer;
     i64 m = rp[n];
     std::vector<i32> eb(m);
     i64 nb;
-    std::vector<i64> cuts;
-    if (outer == 1 && first_edge_batch) {
+    std::vector<i64> cuts, node_cuts;
+    if (inherit && outer > 1) {
+      cuts = inh_cuts;
+      node_cuts = inh_nodes;
+      nb = (i64)cuts.size() - 1;
+      for (i64 k = 0; k < nb; ++k)
+        for (i64 e = cuts[k]; e < cuts[k + 1]; ++e) eb[e] = (i32)k;
+    } else if (outer == 1 && first_edge_batch) {
       nb = nb0;
       for (i64 e = 0; e < m; ++e) eb[e] = first_edge_batch[e];
     } else {
@@ -256,7 +267,10 @@ i64 oracle_rbsc(i64 n0, const i64* row_ptr0, const i32* col0, const u32* wt0, i6
     }
     // sinks: batch whose edge range contains the row's (empty) position; batch 0 for arbitrary partitions (Q9)
     std::vector<i32> sink(n, 0);
-    if (!cuts.empty())
+    if (!node_cuts.empty()) {  // inherited batches come with their node ranges
+      for (i64 k = 0; k < nb; ++k)
+        for (i64 i = node_cuts[k]; i < node_cuts[k + 1]; ++i) sink[i] = (i32)k;
+    } else if (!cuts.empty())
       for (i64 i = 0; i < n; ++i)
         if (rp[i] == rp[i + 1]) {
           i64 k = 0;
@@ -306,6 +320,27 @@ i64 oracle_rbsc(i64 n0, const i64* row_ptr0, const i32* col0, const u32* wt0, i6
     std::vector<u32> qwt(m > 0 ? m : 1);
     i64 qm = oracle_quotient(n, rp.data(), col.data(), wt.data(), Hc.data(), k, qrp.data(), qcol.data(), qwt.data());
     for (i64 i = 0; i < n0; ++i) map[i] = Hc[map[i]];
+    if (inherit && !cuts.empty()) {
+      // batch j of the quotient: blocks whose first node lies before done_nodes(j) = the nodes whose row is complete after
+      // batch j (all nodes after the last batch), minus the blocks of earlier batches; batches without blocks disappear
+      inh_cuts.assign(1, 0);
+      inh_nodes.assign(1, 0);
+      for (i64 j = 0; j < nb; ++j) {
+        i64 done_nodes;
+        if (!node_cuts.empty()) done_nodes = node_cuts[j + 1];
+        else if (j == nb - 1) done_nodes = n;
+        else {
+          done_nodes = 0;
+          while (done_nodes < n && rp[done_nodes + 1] <= cuts[j + 1]) ++done_nodes;
+        }
+        i64 done_blocks = 0;  // canonical ids are ordered by first node: blocks with first node < done_nodes
+        for (i64 i = 0; i < done_nodes; ++i) done_blocks = std::max<i64>(done_blocks, (i64)Hc[i] + 1);
+        if (done_blocks > inh_nodes.back()) {
+          inh_nodes.push_back(done_blocks);
+          inh_cuts.push_back(qrp[done_blocks]);
+        }
+      }
+    }
     bool stop = (nb == 1) || (k == n);  // Alg. 2 l.15 (L200), reading Q15
     nb_last = nb;
     rp.assign(qrp.begin(), qrp.end());

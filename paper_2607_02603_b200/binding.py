@@ -23,6 +23,7 @@ WL_FLAG_EDGE_BALANCED = 128
 WL_FLAG_NO_DEEP = 256
 WL_FLAG_DEEP_EARLY = 512
 WL_FLAG_NO_FINAL = 1024
+WL_FLAG_INHERIT_BATCHES = 4096
 
 EXPORTS = [
     "wl_refine_workspace_bytes", "wl_refine_deep_workspace_bytes", "wl_refine", "wl_refine_host", "wl_round_key", "wl_weight", "wl_spmv_round",

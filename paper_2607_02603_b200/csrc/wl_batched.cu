@@ -51,6 +51,11 @@ __global__ void merge_kernel(int64_t n_local, const int* __restrict__ local_colo
   if (i < n_local) H[i] = base + local_colour[i];
 }
 
+__global__ void fill_kernel(int64_t n, int* __restrict__ a, int v) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) a[i] = v;
+}
+
 __global__ void iota_kernel(int64_t n, int* __restrict__ a) {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i < n) a[i] = (int)i;
@@ -165,8 +170,7 @@ quot_insert_long_kernel(int64_t row_base, const int64_t* __restrict__ row_ptr, i
 // Only blocks b_lo <= B < b_hi are emitted (a representative row that continues in the next batch stays in the table).
 __global__ void quot_emit_kernel(u64* __restrict__ table, u64 table_slots, const int64_t* __restrict__ q_row_ptr,
                                  int64_t out_base, int* __restrict__ cursor, int* __restrict__ q_col,
-                                 u32* __restrict__ q_wt, int b_lo, int b_hi, int64_t cap = (1ll << 62),
-                                 long long* __restrict__ dbg = nullptr) {
+                                 u32* __restrict__ q_wt, int b_lo, int b_hi) {
   int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (s >= (int64_t)table_slots) return;
   const u64 key1 = table[2 * s];
@@ -175,32 +179,11 @@ __global__ void quot_emit_kernel(u64* __restrict__ table, u64 table_slots, const
   const int b = (int)(key >> 32), t = (int)(key & 0xffffffffu);
   if (b < b_lo || b >= b_hi) return;
   const u64 sum = table[2 * s + 1];
-  const int c = atomicAdd(cursor + b, 1);
-  const int64_t pos = q_row_ptr[b] - out_base + c;
-  if (pos < 0 || pos >= cap) {
-    if (dbg && atomicAdd((unsigned long long*)dbg, 1ull) == 0) {
-      dbg[1] = b; dbg[2] = pos; dbg[3] = q_row_ptr[b]; dbg[4] = c; dbg[5] = q_row_ptr[b + 1]; dbg[6] = s;
-    }
-    return;
-  }
+  const int64_t pos = q_row_ptr[b] - out_base + atomicAdd(cursor + b, 1);
   q_col[pos] = t;
   q_wt[pos] = (u32)sum;
   table[2 * s] = 0;
   table[2 * s + 1] = 0;
-}
-
-// WL_DEBUG: occupied slots whose block lies in [b_lo, b_hi), and the largest per-slot anomalies
-__global__ void quot_count_kernel(const u64* __restrict__ table, u64 table_slots, int b_lo, int b_hi, u64* __restrict__ out) {
-  int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (s >= (int64_t)table_slots) return;
-  const u64 key1 = table[2 * s];
-  if (key1 == 0) {
-    if (table[2 * s + 1] != 0) atomicAdd(out + 2, 1ull);  // weight without key
-    return;
-  }
-  const int b = (int)((key1 - 1) >> 32);
-  if (b >= b_lo && b < b_hi) atomicAdd(out, 1ull);
-  else atomicAdd(out + 1, 1ull);
 }
 
 // exclusive scan int32 counts -> int64 offsets (3 kernels)
@@ -535,13 +518,18 @@ int wl_refine_batched(int64_t n, int32_t num_batches, const wl_edge_batch* batch
 
   u64* hs = host_scal();
   if (!hs) return WL_ECUDA;
-  cudaStream_t copy_st, down_st;  // host -> device uploads; device -> host return of quotient rows
+  cudaStream_t copy_st, down_st, side_st;  // uploads; return of quotient rows; refinement of emitted pieces (inherit)
   if (cudaStreamCreateWithFlags(&copy_st, cudaStreamNonBlocking) != cudaSuccess) return check_cuda(cudaGetLastError());
   if (cudaStreamCreateWithFlags(&down_st, cudaStreamNonBlocking) != cudaSuccess) {
     cudaStreamDestroy(copy_st);
     return check_cuda(cudaGetLastError());
   }
-  cudaEvent_t ev_begin, ev_end, ev_up[2], ev_ins[2], ev_emit[2], ev_down[2];
+  if (cudaStreamCreateWithFlags(&side_st, cudaStreamNonBlocking) != cudaSuccess) {
+    cudaStreamDestroy(copy_st);
+    cudaStreamDestroy(down_st);
+    return check_cuda(cudaGetLastError());
+  }
+  cudaEvent_t ev_begin, ev_end, ev_up[2], ev_ins[2], ev_emit[2], ev_down[2], ev_piece[2];
   cudaEventCreate(&ev_begin);
   cudaEventCreate(&ev_end);
   for (int b = 0; b < 2; ++b) {
@@ -549,11 +537,13 @@ int wl_refine_batched(int64_t n, int32_t num_batches, const wl_edge_batch* batch
     cudaEventCreateWithFlags(&ev_ins[b], cudaEventDisableTiming);
     cudaEventCreateWithFlags(&ev_emit[b], cudaEventDisableTiming);
     cudaEventCreateWithFlags(&ev_down[b], cudaEventDisableTiming);
+    cudaEventCreateWithFlags(&ev_piece[b], cudaEventDisableTiming);
   }
   cudaEventRecord(ev_begin, st);
   auto cleanup = [&]() {
     cudaStreamSynchronize(copy_st);
     cudaStreamSynchronize(down_st);
+    cudaStreamSynchronize(side_st);
     cudaEventDestroy(ev_begin);
     cudaEventDestroy(ev_end);
     for (int b = 0; b < 2; ++b) {
@@ -561,9 +551,11 @@ int wl_refine_batched(int64_t n, int32_t num_batches, const wl_edge_batch* batch
       cudaEventDestroy(ev_ins[b]);
       cudaEventDestroy(ev_emit[b]);
       cudaEventDestroy(ev_down[b]);
+      cudaEventDestroy(ev_piece[b]);
     }
     cudaStreamDestroy(copy_st);
     cudaStreamDestroy(down_st);
+    cudaStreamDestroy(side_st);
   };
 
   const int64_t n0 = n;
@@ -583,6 +575,13 @@ int wl_refine_batched(int64_t n, int32_t num_batches, const wl_edge_batch* batch
   int rc = WL_OK;
   bool hit_limit = false;
 
+  // WL_FLAG_INHERIT_BATCHES (reading Q14b): the local refinement of the NEXT outer iteration runs on the quotient rows while
+  // they are still on the device, batch = the rows emitted together; the next iteration then starts at the merge.
+  const bool inherit = (flags & WL_FLAG_INHERIT_BATCHES) != 0;
+  bool have_next = false;          // the coming iteration's local refinement is done already
+  DevBuf d_Hnext_keep;             // ... its merged block map (before the boundary / canonical step)
+  std::vector<int64_t> node_cuts;  // ... and the node ranges of its batches
+  int64_t next_base_id = 0;
   const bool debug = std::getenv("WL_DEBUG") != nullptr;
   auto wall = [] { return std::chrono::duration<double>(std::chrono::steady_clock::now().time_since_epoch()).count(); };
   double t_mark = wall();
@@ -601,23 +600,36 @@ int wl_refine_batched(int64_t n, int32_t num_batches, const wl_edge_batch* batch
     std::vector<int64_t> r0(nb), r1(nb);
     int64_t max_rows = 1, max_edges = 1;
     for (int k = 0; k < nb; ++k) {
-      inner_range(n_t, rp, cuts[k], cuts[k + 1], k == nb - 1, &r0[k], &r1[k]);
+      if (have_next) {  // inherited batches hold whole rows of a known node range
+        r0[k] = node_cuts[k];
+        r1[k] = node_cuts[k + 1];
+      } else {
+        inner_range(n_t, rp, cuts[k], cuts[k + 1], k == nb - 1, &r0[k], &r1[k]);
+      }
       max_rows = std::max(max_rows, r1[k] - r0[k]);
       max_edges = std::max(max_edges, cuts[k + 1] - cuts[k]);
     }
     size_t ws_bytes = 0;
-    for (int k = 0; k < nb; ++k)
+    for (int k = 0; k < nb && !have_next; ++k)
       ws_bytes = std::max(ws_bytes, make_layout(r1[k] - r0[k], rp[r1[k]] - rp[r0[k]]).bytes);
 
     // ---- device memory of this outer iteration ---------------------------------------------------------------------
     size_t used_iter = used;
     DevBuf d_H, d_Hc, d_first, d_cof, d_bsum, d_ws, d_col[2], d_wt[2], d_rp[2], d_rep, d_cnt, d_cursor, d_qrp, d_qtab,
-        d_qcol[2], d_qwt[2], d_sbsum, d_misc, d_query, d_long;
+        d_qcol[2], d_qwt[2], d_sbsum, d_misc, d_query, d_long, d_Hnext, d_ws2;
     const int64_t nscan = (n_t + kCanonChunk - 1) / kCanonChunk;
     // every allocation of the iteration goes through here: the first failure (device cap or cudaMalloc) sticks
 #define WL_ALLOC(buf, bytes) \
   if (!rc) rc = buf.alloc((bytes), &used_iter, device_cap_bytes);
-    WL_ALLOC(d_H, sizeof(int) * (size_t)n_t);
+    if (have_next) {  // made by the previous iteration's quotient pass
+      d_H.p = d_Hnext_keep.p;
+      d_H.bytes = d_Hnext_keep.bytes;
+      d_Hnext_keep.p = nullptr;
+      used_iter += d_H.bytes;
+      if (device_cap_bytes && used_iter > device_cap_bytes) rc = WL_ENOMEM;
+    } else {
+      WL_ALLOC(d_H, sizeof(int) * (size_t)n_t);
+    }
     WL_ALLOC(d_Hc, sizeof(int) * (size_t)n_t);
     WL_ALLOC(d_first, sizeof(int) * (size_t)n_t);
     WL_ALLOC(d_cof, sizeof(int) * (size_t)n_t);
@@ -653,10 +665,10 @@ int wl_refine_batched(int64_t n, int32_t num_batches, const wl_edge_batch* batch
 
     phase("alloc");
     // ---- Alg. 2 lines 7-11: local refinement per batch, merge ---------------------------------------------------------
-    int64_t base_id = 0;
+    int64_t base_id = have_next ? next_base_id : 0;
     cudaStreamSynchronize(st);  // buffers of the previous iteration are free
-    upload_batch(0, 0, false);
-    for (int k = 0; k < nb && !rc; ++k) {
+    if (!have_next) upload_batch(0, 0, false);
+    for (int k = 0; k < nb && !rc && !have_next; ++k) {
       const int buf = k & 1;
       if (k + 1 < nb) upload_batch(k + 1, buf ^ 1, false);
       cudaStreamWaitEvent(st, ev_up[buf], 0);
@@ -777,12 +789,26 @@ int wl_refine_batched(int64_t n, int32_t num_batches, const wl_edge_batch* batch
       na[k] = std::max<int64_t>(0, (std::upper_bound(rp, rp + n_t + 1, c0) - rp) - 1);
       nz[k] = c1 > c0 ? std::min<int64_t>(n_t, std::upper_bound(rp, rp + n_t + 1, c1 - 1) - rp) : na[k];
       done_nodes[k] = k == nb - 1 ? n_t : (std::upper_bound(rp + 1, rp + n_t + 1, c1) - (rp + 1));  // rp[i + 1] <= c1
+      if (have_next) done_nodes[k] = node_cuts[k + 1];  // inherited batches: exactly their node range
     }
     cudaMemcpyAsync(d_query.p, done_nodes.data(), sizeof(int64_t) * (size_t)nb, cudaMemcpyHostToDevice, st);
     ++g_launches; rep_lower_bound_kernel<<<blocks_for(nb, 128), 128, 0, st>>>(d_rep.as<int>(), K, d_query.as<int64_t>(), nb, d_query.as<int64_t>() + nb);
     cudaMemcpyAsync(done_blocks.data(), d_query.as<int64_t>() + nb, sizeof(int64_t) * (size_t)nb, cudaMemcpyDeviceToHost, st);
     rc = check_cuda(cudaStreamSynchronize(st));
     if (rc) break;
+    // inherit: block map and workspace of the next iteration's local refinement (one "piece" per emission)
+    std::vector<int64_t> next_edge_cuts(1, 0), next_node_cuts(1, 0);
+    int64_t base_next = 0;
+    if (inherit) {
+      int64_t max_piece_rows = 1, prev = 0;
+      for (int k = 0; k < nb; ++k) {
+        max_piece_rows = std::max(max_piece_rows, done_blocks[k] - prev);
+        prev = std::max(prev, done_blocks[k]);
+      }
+      WL_ALLOC(d_Hnext, sizeof(int) * (size_t)K);
+      WL_ALLOC(d_ws2, make_layout(max_piece_rows, out_cap).bytes);
+      if (rc) break;
+    }
     auto upload_quot = [&](int k, int buf) {
       const int64_t c0 = cuts[k], c1 = cuts[k + 1];
       if (c1 > c0) {
@@ -798,6 +824,53 @@ int wl_refine_batched(int64_t n, int32_t num_batches, const wl_edge_batch* batch
         bytes_h2d += sizeof(int64_t) * (nz[k] - na[k] + 1);
       }
       cudaEventRecord(ev_up[buf], copy_st);
+    };
+    // Alg. 2 lines 7-10 of the NEXT iteration on a piece of quotient rows that is still on the device: nodes b_lo .. b_hi of
+    // the quotient, whole rows.  Runs on its own stream next to the insertion of the following batch (and next to the copy
+    // of the piece to the host); the host waits inside refine_core, which is why it is called after that insertion has
+    // been queued.
+    struct Piece {
+      bool valid;
+      int64_t b_lo, b_hi, tot, q_off;
+      int ob, index;
+    };
+    Piece pending{false, 0, 0, 0, 0, 0, 0};
+    auto refine_piece = [&]() -> int {
+      if (!pending.valid) return WL_OK;
+      pending.valid = false;
+      const int64_t nr = pending.b_hi - pending.b_lo;
+      cudaStreamWaitEvent(side_st, ev_emit[pending.ob], 0);
+      if (pending.tot == 0) {  // edgeless nodes only: one block (Eq. 3)
+        ++g_launches; fill_kernel<<<blocks_for(nr, 256), 256, 0, side_st>>>(nr, d_Hnext.as<int>() + pending.b_lo, (int)base_next);
+        base_next += 1;
+        return WL_OK;
+      }
+      wl_csr lg;
+      lg.n = nr;
+      lg.m = pending.tot;
+      lg.row_ptr = d_qrp.as<int64_t>() + pending.b_lo;  // global positions q_off .. q_off + tot
+      lg.col_idx = d_qcol[pending.ob].as<int>() - pending.q_off;
+      lg.weights = d_qwt[pending.ob].as<u32>() - pending.q_off;
+      wl_options lo{};
+      lo.flags = (flags & (WL_FLAG_NO_PRUNE | WL_FLAG_EDGE_BALANCED)) | WL_FLAG_NO_VALIDATE;
+      lo.max_rounds = opt ? opt->max_rounds : 0;
+      lo.stream_id = ((u64)(outer + 1) << 32) | (u64)(u32)pending.index;
+      const Layout L2 = make_layout(nr, pending.tot);
+      CoreResult cr{};
+      int prc = refine_core(&lg, nullptr, seed, &lo, /*ranged=*/true, (int)pending.b_lo, (int)pending.b_hi, K, pending.q_off,
+                            d_ws2.p, L2.bytes, L2, side_st, &cr);
+      if (prc) return prc;
+      ++g_launches; merge_kernel<<<blocks_for(nr, 256), 256, 0, side_st>>>(nr, cr.colour, (int)base_next, d_Hnext.as<int>() + pending.b_lo);
+      base_next += cr.k;
+      edges_streamed += cr.edges_streamed;
+      ms_spmv += cr.ms_spmv;
+      ms_relabel += cr.ms_relabel;
+      ms_spmv_kernel += cr.ms_spmv_kernel;
+      spmv_alg_bytes += cr.spmv_alg_bytes;
+      spmv_launches += cr.spmv_launches;
+      // the emission buffer may be overwritten once this piece is refined (emission + 2 waits on the stream `st`)
+      cudaEventRecord(ev_piece[pending.ob], side_st);
+      return WL_OK;
     };
     int64_t q_off = 0, emitted_blocks = 0;
     int n_emit = 0;
@@ -824,6 +897,7 @@ int wl_refine_batched(int64_t n, int32_t num_batches, const wl_edge_batch* batch
       }
       cudaEventRecord(ev_ins[buf], st);
       checkpoint("insert", k);
+      if ((rc = refine_piece())) break;  // the previous emission, next to this insertion
       // a representative row that continues into the next batch is completed there: emit the blocks whose representative
       // row ends at or before c1 and that were not emitted yet
       const int64_t b_lo = emitted_blocks, b_hi = done_blocks[k];
@@ -840,7 +914,10 @@ int wl_refine_batched(int64_t n, int32_t num_batches, const wl_edge_batch* batch
           break;
         }
         const int ob = n_emit & 1;
-        if (n_emit >= 2) cudaStreamWaitEvent(st, ev_down[ob], 0);  // the rows emitted two emissions ago are on the host
+        if (n_emit >= 2) {
+          cudaStreamWaitEvent(st, ev_down[ob], 0);  // the rows emitted two emissions ago are on the host ...
+          if (inherit) cudaStreamWaitEvent(st, ev_piece[ob], 0);  // ... and refined
+        }
         ++n_emit;
         ++g_launches; quot_emit_kernel<<<blocks_for((int64_t)qslots, 256), 256, 0, st>>>(d_qtab.as<u64>(), qslots, d_qrp.as<int64_t>(), q_off, d_cursor.as<int>(), d_qcol[ob].as<int>(), d_qwt[ob].as<u32>(), (int)b_lo, (int)b_hi);
         cudaEventRecord(ev_emit[ob], st);
@@ -856,10 +933,17 @@ int wl_refine_batched(int64_t n, int32_t num_batches, const wl_edge_batch* batch
                         cudaMemcpyDeviceToHost, down_st);
         bytes_d2h += sizeof(int64_t) * (b_hi - b_lo + 1);
         cudaEventRecord(ev_down[ob], down_st);
+        if (inherit) {  // refined while the next batch is being inserted (refine_piece)
+          pending = Piece{true, b_lo, b_hi, tot, q_off, ob, (int)next_node_cuts.size() - 1};
+          next_edge_cuts.push_back(q_off + tot);
+          next_node_cuts.push_back(b_hi);
+        }
         q_off += tot;
         emitted_blocks = b_hi;
       }
     }
+    if (!rc) rc = refine_piece();
+    if (!rc) rc = check_cuda(cudaStreamSynchronize(side_st));
     if (!rc) rc = check_cuda(cudaStreamSynchronize(down_st));
     if (!rc) rc = check_cuda(cudaStreamSynchronize(st));
     if (rc) break;
@@ -871,11 +955,25 @@ int wl_refine_batched(int64_t n, int32_t num_batches, const wl_edge_batch* batch
     weighted = true;
     const int64_t next_nb_cap = max_batch_edges;
     std::vector<int64_t> next_cuts;
-    greedy_cuts(n_t, rp, next_nb_cap, next_cuts);
+    if (inherit) {
+      next_cuts = next_edge_cuts;
+      if (next_cuts.size() == 1) next_cuts.push_back(0);  // no block at all cannot happen (K >= 1); keep one batch
+    } else {
+      greedy_cuts(n_t, rp, next_nb_cap, next_cuts);
+    }
     if ((flags & WL_FLAG_AGGRESSIVE_STOP) && (int64_t)next_cuts.size() - 1 >= nb) {  // L328
       break;
     }
     cuts.swap(next_cuts);
+    if (inherit) {
+      node_cuts.swap(next_node_cuts);
+      next_base_id = base_next;
+      if (d_Hnext_keep.p) cudaFree(d_Hnext_keep.p);
+      d_Hnext_keep.p = d_Hnext.p;  // survives this iteration's buffers
+      d_Hnext_keep.bytes = d_Hnext.bytes;
+      d_Hnext.p = nullptr;
+      have_next = true;
+    }
     (void)m_t;
   }
 

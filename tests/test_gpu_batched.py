@@ -104,6 +104,27 @@ def test_batched_equals_cpu_algorithm2_and_invariants(name, nb):
         assert got.tolist() == coarsest.tolist()
 
 
+@pytest.mark.parametrize("name", list(BATCH_GRAPHS))
+@pytest.mark.parametrize("nb", [2, 4, 16])
+def test_batched_inherited_batches_equal_cpu_algorithm2(name, nb):
+    """WL_FLAG_INHERIT_BATCHES (reading Q14b): from the second outer iteration on the quotient keeps the batches of its graph
+    and is refined while its rows are still on the device.  Bit-exact against the CPU Algorithm 2 with the same rule, plus
+    Theorem 2 and L165."""
+    g = BATCH_GRAPHS[name]()
+    n, rp, ci, wt = g.numpy()
+    cap = max(1, -(-g.m // nb))
+    coarsest, _, _ = oracle.refine(n, rp, ci, wt)
+    want, k_want, outer_want, nbl_want = oracle.rbsc(n, rp, ci, wt, cap, inherit=True)
+    res = wl.wl_refine_batched(n, g.row_ptr, g.col, g.weights, max_batch_edges=cap, seed=nb,
+                               flags=wl.WL_FLAG_INHERIT_BATCHES)
+    got = res.colors.numpy()
+    assert got.tolist() == want.tolist()
+    assert res.num_colors == k_want
+    assert res.stats["outer_iters"] == outer_want and res.stats["last_num_batches"] == nbl_want
+    assert oracle.is_stable(n, rp, ci, wt, got)
+    assert refines(got, coarsest)
+
+
 def test_batched_caller_supplied_slices():
     g = gg.rmat(10, seed=4)
     n, rp, ci, wt = g.numpy()

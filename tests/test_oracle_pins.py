@@ -256,6 +256,30 @@ def test_rbsc_invariants(seed):
     assert c1.tolist() == c2.tolist()
 
 
+@pytest.mark.parametrize("seed", range(12))
+def test_rbsc_inherited_batches_invariants(seed):
+    """Reading Q14b (the quotient keeps the batches of its graph): still Algorithm 2 on SOME edge partition per iteration, so
+    Theorem 2 (stability), L165 (refines the coarsest colouring) and case (i) (one batch = the coarsest colouring) must
+    hold; the first outer iteration is the same as without the rule, so the result can only be coarser or equal when both
+    stop after it."""
+    g = gg.rmat(6 + seed % 2, edge_factor=3, seed=seed, symmetrize=bool(seed % 2)) if seed < 8 else \
+        gg.random_weighted_digraph(60, 240, seed, max_w=3)
+    n, rp, ci, wt = _np(g)
+    coarsest, _, _ = oracle.refine(n, rp, ci, wt)
+    A = dense_adj(n, rp, ci, wt)
+    for nb in (1, 2, 3, 5):
+        cap = -(-g.m // nb)
+        c, k, outer, nb_last = oracle.rbsc(n, rp, ci, wt, cap, inherit=True)
+        assert stable_dense(A, c)
+        assert refines(c, coarsest)
+        if nb == 1:
+            assert c.tolist() == coarsest.tolist() and outer == 1
+        c1, _, _, _ = oracle.rbsc(n, rp, ci, wt, cap, max_outer=1)
+        ci1, _, _, _ = oracle.rbsc(n, rp, ci, wt, cap, max_outer=1, inherit=True)
+        assert c1.tolist() == ci1.tolist()  # the rule only changes iterations >= 2
+        assert refines(c1, c)               # every outer iteration coarsens (L206)
+
+
 def test_rbsc_single_batch_is_refine():
     g = gg.erdos_renyi(300, 900, seed=3)
     n, rp, ci, wt = _np(g)
