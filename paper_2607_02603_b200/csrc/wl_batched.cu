@@ -142,7 +142,9 @@ quot_insert_kernel(int64_t row_base, int64_t n_rows, const int64_t* __restrict__
   if (lane == 0 && fresh) atomicAdd(cnt + b, fresh);
 }
 
-// the queued long pieces, one after the other, each spread over the whole grid
+// the queued long pieces: up to kQuotGiantRow entries one CTA per piece (CTAs take pieces in turn), longer ones (hub rows of
+// 10^5-10^6 entries) one after the other, each spread over the whole grid
+constexpr int64_t kQuotGiantRow = 65536;
 __global__ void __launch_bounds__(256)
 quot_insert_long_kernel(int64_t row_base, const int64_t* __restrict__ row_ptr, int64_t clip_lo, int64_t clip_hi,
                         const int* __restrict__ col, const u32* __restrict__ wt, const int* __restrict__ Hc,
@@ -152,12 +154,14 @@ quot_insert_long_kernel(int64_t row_base, const int64_t* __restrict__ row_ptr, i
   const int64_t tid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x, stride = (int64_t)gridDim.x * blockDim.x;
   for (u32 j = 0; j < n_long; ++j) {
     const int64_t w = long_rows[j];
-    const int b = Hc[row_base + w];
     int64_t a = row_ptr[w], e = row_ptr[w + 1];
     if (a < clip_lo) a = clip_lo;
     if (e > clip_hi) e = clip_hi;
+    const bool giant = e - a > kQuotGiantRow;
+    if (!giant && j % gridDim.x != blockIdx.x) continue;  // this piece belongs to another CTA
+    const int b = Hc[row_base + w];
     int fresh = 0;
-    for (int64_t p = a + tid; p < e; p += stride)
+    for (int64_t p = a + (giant ? tid : (int64_t)threadIdx.x); p < e; p += giant ? stride : (int64_t)blockDim.x)
       fresh += quot_insert_one(table, table_mask, b, Hc[col[p]], wt ? (u64)wt[p] : 1ull) ? 1 : 0;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) fresh += __shfl_xor_sync(0xffffffffu, fresh, o);
