@@ -9,6 +9,7 @@
 namespace wl {
 
 constexpr int64_t kMaxNodes = (1ll << 31) - 2;
+constexpr uint32_t kFlagLazyDeep = 1u << 30;  // internal (wl_refine_host): the engine may cudaMalloc the deep-round workspace
 
 constexpr int kRunAhead = kNumScal - kScalLog;  // rounds queued per host synchronisation in the deep-round regime
 constexpr int kCanonChunk = 2048;        // nodes per CTA of the canonicalisation scan (== kScanChunk)

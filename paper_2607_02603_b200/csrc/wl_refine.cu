@@ -361,10 +361,25 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
   constexpr int64_t kSyncRounds = 6;
   // deep-round (worklist) regime, wl_deep.cuh: needs the larger workspace
   const DeepLayout DL = make_deep_layout(L);
-  const bool deep_ok = !(flags & WL_FLAG_NO_DEEP) && !ranged && !merge && !force_eb && m > 0 && workspace_bytes >= DL.bytes;
+  // (wl_refine_host lets the engine allocate that part itself, and only once the loop gets there: kFlagLazyDeep)
+  const bool deep_wanted = !(flags & WL_FLAG_NO_DEEP) && !ranged && !merge && !force_eb && m > 0;
+  struct LazyDeep {
+    char* p = nullptr;
+    ~LazyDeep() {
+      if (p) cudaFree(p);
+    }
+  } lazy_deep;
+  char* dws = ws;  // base the deep offsets are relative to
+  bool deep_ok = deep_wanted && (workspace_bytes >= DL.bytes || (flags & kFlagLazyDeep));
   const int64_t deep_start = (flags & WL_FLAG_DEEP_EARLY) ? 2 : kSyncRounds + 1;
-  u64* deep = (u64*)(ws + DL.o_scal);
-  int* changed[2] = {(int*)(ws + DL.o_changed[0]), (int*)(ws + DL.o_changed[1])};
+  u64* deep = nullptr;
+  int* changed[2] = {nullptr, nullptr};
+  auto bind_deep = [&]() {
+    deep = (u64*)(dws + DL.o_scal);
+    changed[0] = (int*)(dws + DL.o_changed[0]);
+    changed[1] = (int*)(dws + DL.o_changed[1]);
+  };
+  if (workspace_bytes >= DL.bytes) bind_deep();
   bool cols_checked = !validate || m == 0;
   bool dropped_checked = false;  // the rows outside the active list have had their columns range-checked
   if (validate && !uniform_start) {
@@ -547,6 +562,15 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
     // it is harmless; `rounds` and the trajectory stop at the first repeated count exactly as in the per-round mode.
     // the round at which the worklist regime starts is an ordinary round that also lists the nodes it moved; its key
     // stays the key of every later round
+    if (deep_ok && r == deep_start && !deep) {  // the deep part of the workspace is allocated now (wl_refine_host)
+      if (cudaMalloc((void**)&lazy_deep.p, DL.bytes - L.bytes) == cudaSuccess) {
+        dws = lazy_deep.p - L.bytes;
+        bind_deep();
+      } else {
+        cudaGetLastError();
+        deep_ok = false;  // no room: every round keeps recomputing every active row
+      }
+    }
     const bool switch_round = deep_ok && r == deep_start;
     if (switch_round) cudaMemsetAsync(deep, 0, sizeof(u64) * kNumDeep, st);
     const bool window = !no_runahead && r > kSyncRounds && !switch_round;
@@ -645,16 +669,16 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
   // ---- S5, deep-round regime (wl_deep.cuh): only the rows with a changed out-neighbour are recomputed ---------------------
   if (deep_entered && !converged && r <= max_rounds) {
     const u64 key = round_key(seed, stream_id, (u64)deep_start);  // the key of the switch round, kept from here on
-    int64_t* tp_ptr = (int64_t*)(ws + DL.o_tp_ptr);
-    int* tp_src = (int*)(ws + DL.o_tp_src);
-    int* size = (int*)(ws + DL.o_size);
-    int* inherit = (int*)(ws + DL.o_inherit);
-    int* mark = (int*)(ws + DL.o_mark);
-    int* lcount[2] = {(int*)(ws + DL.o_lcount[0]), (int*)(ws + DL.o_lcount[1])};
-    int* leavers[2] = {(int*)(ws + DL.o_leavers[0]), (int*)(ws + DL.o_leavers[1])};
-    int* leaver_block[2] = {(int*)(ws + DL.o_leaver_block[0]), (int*)(ws + DL.o_leaver_block[1])};
-    u32* slots = (u32*)(ws + DL.o_slots);
-    u64* bsum = (u64*)(ws + DL.o_bsum);
+    int64_t* tp_ptr = (int64_t*)(dws + DL.o_tp_ptr);
+    int* tp_src = (int*)(dws + DL.o_tp_src);
+    int* size = (int*)(dws + DL.o_size);
+    int* inherit = (int*)(dws + DL.o_inherit);
+    int* mark = (int*)(dws + DL.o_mark);
+    int* lcount[2] = {(int*)(dws + DL.o_lcount[0]), (int*)(dws + DL.o_lcount[1])};
+    int* leavers[2] = {(int*)(dws + DL.o_leavers[0]), (int*)(dws + DL.o_leavers[1])};
+    int* leaver_block[2] = {(int*)(dws + DL.o_leaver_block[0]), (int*)(dws + DL.o_leaver_block[1])};
+    u32* slots = (u32*)(dws + DL.o_slots);
+    u64* bsum = (u64*)(dws + DL.o_bsum);
     cudaEvent_t d0 = evp.get(2), d1 = evp.get(4);
     cudaEventRecord(d0, st);
     // the table is empty between deep rounds; every slot may be used
@@ -806,7 +830,7 @@ int wl_refine_host(const wl_csr* g, const int32_t* init_colors, uint64_t seed, i
   if (n == 0) return WL_OK;
   if (!out_colors) return WL_EINVAL;
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  size_t wsb = wl_refine_deep_workspace_bytes(n, m);  // room for the deep-round regime if the device has it
+  const size_t wsb = wl_refine_workspace_bytes(n, m);  // the deep-round part is allocated by the engine if the loop gets there
   char* d_all = nullptr;
   size_t o_rp = 0, o_col, o_wt, o_init, o_out, o_ws, off = 0;
   auto take = [&](size_t b) {
@@ -819,17 +843,10 @@ int wl_refine_host(const wl_csr* g, const int32_t* init_colors, uint64_t seed, i
   o_wt = take(g->weights ? sizeof(u32) * (size_t)m : 0);
   o_init = take(init_colors ? sizeof(int) * (size_t)n : 0);
   o_out = take(sizeof(int) * (size_t)n);
-  const size_t off_before_ws = off;
   o_ws = take(wsb);
   if (cudaMalloc((void**)&d_all, off) != cudaSuccess) {
     cudaGetLastError();
-    wsb = wl_refine_workspace_bytes(n, m);
-    off = off_before_ws;
-    o_ws = take(wsb);
-    if (cudaMalloc((void**)&d_all, off) != cudaSuccess) {
-      cudaGetLastError();
-      return WL_ENOMEM;
-    }
+    return WL_ENOMEM;
   }
   cudaEvent_t e0, e1;
   cudaEventCreate(&e0);
@@ -851,7 +868,10 @@ int wl_refine_host(const wl_csr* g, const int32_t* init_colors, uint64_t seed, i
   wl_csr dg = {n, m, (const int64_t*)(d_all + o_rp), (const int*)(d_all + o_col),
                g->weights ? (const u32*)(d_all + o_wt) : nullptr};
   wl_stats inner;
-  rc = wl_refine(&dg, init_colors ? (const int*)(d_all + o_init) : nullptr, seed, (int*)(d_all + o_out), &inner, opt,
+  wl_options hopt{};
+  if (opt) hopt = *opt;
+  hopt.flags |= kFlagLazyDeep;
+  rc = wl_refine(&dg, init_colors ? (const int*)(d_all + o_init) : nullptr, seed, (int*)(d_all + o_out), &inner, &hopt,
                  d_all + o_ws, wsb, cuda_stream);
   if (rc == WL_OK || rc == WL_EMAXROUNDS) {
     cudaMemcpyAsync(out_colors, d_all + o_out, sizeof(int) * (size_t)n, cudaMemcpyDeviceToHost, st);

@@ -236,6 +236,18 @@ def test_refine_host_entry_point():
 
 
 # ------------------------------------------------------------------ error behaviour
+def test_refine_host_entry_point_deep_rounds():
+    """wl_refine_host on a graph that needs 128 rounds: the engine allocates the worklist regime's workspace itself once the
+    loop gets to round 7 (kFlagLazyDeep) and must give the closed-form colouring and round count."""
+    s = 256
+    g = gg.grid2d(s)
+    res = wl.wl_refine_host(g.n, g.row_ptr.pin_memory(), g.col.pin_memory(), seed=4)
+    h = s // 2
+    assert res.rounds == h and res.num_colors == h * (h + 1) // 2
+    assert torch.equal(res.colors, gg.grid2d_orbit_colors(s))
+    assert res.stats["kernel_launches"] < 600  # two launches per round after the switch, not four
+
+
 def test_error_codes():
     g = gg.erdos_renyi(100, 300, seed=1)
     n, rp, ci, wt = dgraph(g)
