@@ -31,6 +31,8 @@ ORACLE_SAMPLE_SCALE = 21           # bounded sample of the same recipe for the C
 HBM_FALLBACK_GBS = 6650.0          # /opt/skills/guides/B200_PROFILING.md fallback
 # DRAM bytes of the dominant launch (round-2 row kernel 40.71 + 0.74 GB, hub kernel 8.49 + 0.005 GB), ncu --set full
 NCU_TRAFFIC_BYTES = 49.95e9
+# DRAM bytes of the round-2 relabel_kernel (8.08 + 2.32 GB, profiles/r1d_ncu_full.md); the compaction is not counted
+NCU_RELABEL_BYTES = 10.40e9
 
 
 def measured_peaks():
@@ -380,6 +382,14 @@ def main():
                     "all_spmv_launches": {"launches": spmv_launches, "algorithmic_gb_per_s": alg_bytes / (spmv_ms / 1e3) / 1e9,
                                           "gedges_per_s": spmv_edges / (spmv_ms / 1e3) / 1e9,
                                           "share_of_step": spmv_ms / ms_total},
+                    "round_pair": {  # the SpMV + relabel pair of that round, model bytes (4+G) m + 64 n
+                        "spmv_ms": top_ms, "relabel_and_compaction_ms": sum(r.stats["ms_rest_top"] for r in results) / len(results),
+                        "rows": results[-1].stats["rows_top"],
+                        "algorithmic_gb_per_s": (top_bytes + 48 * results[-1].stats["rows_top"]) /
+                        ((top_ms + sum(r.stats["ms_rest_top"] for r in results) / len(results)) / 1e3) / 1e9,
+                        "dram_gb_per_s_ncu": ((NCU_TRAFFIC_BYTES + NCU_RELABEL_BYTES) /
+                                              ((top_ms + sum(r.stats["ms_rest_top"] for r in results) / len(results)) / 1e3) / 1e9)
+                        if args.scale == 27 and not args.flags else None},
                     "binding_unit": "L1TEX 76 % / L2 73 % of peak (ncu): one sector lookup per gathered 2-byte id; DRAM 43 %"}
 
     # ---- end to end through the host-buffer entry point ---------------------------------------------------------------

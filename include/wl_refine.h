@@ -107,6 +107,8 @@ typedef struct wl_stats {
   double ms_spmv_top;        /* the longest single S1+S2 launch of the call (row kernel + hub kernel of one round) ...  */
   int64_t spmv_top_alg_bytes;/* ... its algorithmic bytes ...                                                          */
   int64_t spmv_top_edges;    /* ... and the column indices it consumed (bench.py's roofline object)                     */
+  double ms_rest_top;        /* S3+S4 (+ compaction) of that same round                                                */
+  int64_t rows_top;          /* rows that round processed                                                              */
 } wl_stats;
 
 /* ------------------------------------------------------------------------------------------------------------------

@@ -58,7 +58,8 @@ class wl_stats(C.Structure):
                 ("bytes_h2d", C.c_int64), ("bytes_d2h", C.c_int64), ("ms_total", C.c_double), ("ms_spmv", C.c_double),
                 ("ms_relabel", C.c_double), ("spmv_launches", C.c_int32), ("kernel_launches", C.c_int32),
                 ("ms_spmv_kernel", C.c_double), ("spmv_alg_bytes", C.c_int64), ("ms_spmv_top", C.c_double),
-                ("spmv_top_alg_bytes", C.c_int64), ("spmv_top_edges", C.c_int64)]
+                ("spmv_top_alg_bytes", C.c_int64), ("spmv_top_edges", C.c_int64), ("ms_rest_top", C.c_double),
+                ("rows_top", C.c_int64)]
 
 
 class wl_edge_batch(C.Structure):

@@ -38,7 +38,8 @@ struct CoreResult {
   int32_t rounds, spmv_launches, kernel_launches;
   double ms_spmv, ms_relabel, ms_spmv_kernel;
   double ms_spmv_top;                          // longest single S1+S2 launch and what it moved
-  int64_t spmv_top_alg_bytes, spmv_top_edges;
+  int64_t spmv_top_alg_bytes, spmv_top_edges, rows_top;
+  double ms_rest_top;
   int* colour;  // dense ids, inside the workspace
 };
 int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, const wl_options* opt, bool ranged, int lo,

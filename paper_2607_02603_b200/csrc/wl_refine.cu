@@ -457,7 +457,8 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
   // ---- S1-S5: rounds -------------------------------------------------------------------------------------------------
   int64_t edges_streamed = 0, spmv_alg_bytes = 0, last_alg_bytes = 0, last_edges = 0;
   int64_t top_alg_bytes = 0, top_edges = 0;
-  double ms_spmv = 0, ms_relabel = 0, ms_spmv_kernel = 0, ms_spmv_top = 0;
+  double ms_spmv = 0, ms_relabel = 0, ms_spmv_kernel = 0, ms_spmv_top = 0, ms_rest_top = 0;
+  int64_t rows_top = 0, last_rows = 0;
   int32_t rounds = 0, spmv_launches = 0;
   bool converged = false;
   const bool debug = std::getenv("WL_DEBUG") != nullptr;
@@ -507,6 +508,7 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
       edges_streamed += e_r;
       last_alg_bytes = (int64_t)(4 + (narrow ? 2 : 4) + (g->weights ? 4 : 0)) * e_r + 16 * n_r;
       last_edges = e_r;
+      last_rows = n_r;
       spmv_alg_bytes += last_alg_bytes;
       streamed = true;
     }
@@ -619,6 +621,8 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
           ms_spmv_top = tc;
           top_alg_bytes = last_alg_bytes;
           top_edges = last_edges;
+          ms_rest_top = t_all - tc;
+          rows_top = last_rows;
         }
       }
     ms_spmv_kernel += t_spmv;
@@ -758,6 +762,8 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
   res->ms_spmv_top = ms_spmv_top;
   res->spmv_top_alg_bytes = top_alg_bytes;
   res->spmv_top_edges = top_edges;
+  res->ms_rest_top = ms_rest_top;
+  res->rows_top = rows_top;
   res->kernel_launches = (int32_t)(g_launches - launches_at_entry);
   res->colour = colour;
   return converged ? WL_OK : WL_EMAXROUNDS;
@@ -816,6 +822,8 @@ int wl_refine(const wl_csr* g, const int32_t* init_colors, uint64_t seed, int32_
     stats->ms_spmv_top = cr.ms_spmv_top;
     stats->spmv_top_alg_bytes = cr.spmv_top_alg_bytes;
     stats->spmv_top_edges = cr.spmv_top_edges;
+    stats->ms_rest_top = cr.ms_rest_top;
+    stats->rows_top = cr.rows_top;
     stats->kernel_launches = (int32_t)(g_launches - launches_at_entry);
   }
   return core_rc;
