@@ -248,6 +248,47 @@ def run_batch_study(args):
     return 0
 
 
+def run_cap_sweep(args):
+    """--workload cap-sweep: the shape of the paper's Table 4 (L311-L332): the same host-resident graph refined with aggressive
+    termination (L328) under two batch caps M_b; reports seconds and reduction power per cap."""
+    import torch
+    import graphgen as gg
+    import paper_2607_02603_b200 as wl
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    g = gg.rmat(args.scale, seed=RMAT_SEEDS[30], symmetrize=False, device=dev, chunk=1 << 27)
+    n, m = g.n, g.m
+    rp = torch.empty(n + 1, dtype=torch.int64, pin_memory=True)
+    col = torch.empty(m, dtype=torch.int32, pin_memory=True)
+    rp.copy_(g.row_ptr)
+    col.copy_(g.col)
+    single = wl.wl_refine(n, g.row_ptr, g.col, None, seed=1, deep=False).num_colors if args.scale <= 27 else None
+    del g
+    torch.cuda.empty_cache()
+    hws = torch.empty(wl.wl_refine_batched_host_bytes(n, m), dtype=torch.uint8, pin_memory=True)
+    out = torch.empty(n, dtype=torch.int32, pin_memory=True)
+    rows = []
+    for cap_edges in (args.batch_edges, 4 * args.batch_edges):
+        for name, flags in (("aggressive (L328)", wl.WL_FLAG_AGGRESSIVE_STOP), ("paper termination (L200)", 0),
+                            ("inherited batches (Q14b)", wl.WL_FLAG_INHERIT_BATCHES)):
+            best, r = None, None
+            for rep in range(2):
+                torch.cuda.synchronize(dev)
+                t0 = time.perf_counter()
+                r = wl.wl_refine_batched(n, rp, col, None, max_batch_edges=cap_edges, seed=20 + rep, flags=flags,
+                                         host_workspace=hws, out=out)
+                torch.cuda.synchronize(dev)
+                dt = time.perf_counter() - t0
+                best = dt if best is None else min(best, dt)
+            rows.append({"M_b": cap_edges, "termination": name, "seconds": best, "outer_iters": r.stats["outer_iters"],
+                         "colors": r.num_colors, "reduction_power_pct": 100.0 * r.num_colors / n,
+                         "coarsest_pct": None if single is None else 100.0 * single / n,
+                         "first_num_batches": -(-m // cap_edges)})
+    print(json.dumps({"metric": "cap_sweep", "unit": "table", "data": "synthetic",
+                      "config": {"workload": f"R-MAT scale {args.scale}, directed, seed 3", "n": n, "m": m}, "rows": rows}))
+    return 0
+
+
 def aggregate_over_ranks(dist, local_ms: float, units_per_rank: float, device=None):
     """Max-over-ranks time and whole-job throughput for N independent replicas (weak scaling, no data-path collective).
     dist = torch.distributed (initialised) or None for a single process.  Returns (ms_max, total_units_per_second)."""
@@ -282,7 +323,7 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--flags", type=int, default=0, help="WL_FLAG_* bits passed to wl_refine")
-    ap.add_argument("--workload", default="single", choices=["single", "batched", "batch-study"],
+    ap.add_argument("--workload", default="single", choices=["single", "batched", "batch-study", "cap-sweep"],
                     help="single: wl_refine on the HBM-resident graph (the headline); batched: wl_refine_batched")
     ap.add_argument("--cap-gb", type=float, default=16.0, help="batched: device memory cap")
     ap.add_argument("--batch-edges", type=int, default=120_000_000, help="batched: M_b")
@@ -294,6 +335,8 @@ def main():
         return run_batched(args)
     if args.workload == "batch-study":
         return run_batch_study(args)
+    if args.workload == "cap-sweep":
+        return run_cap_sweep(args)
 
     import torch
     import graphgen as gg
