@@ -193,7 +193,7 @@ def run_batched(args):
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * sec, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "u64", "data": "synthetic",
             "config": {"workload": f"R-MAT scale {args.scale}, edge factor 16, seed 3, directed, deduplicated, CSR in pinned host "
-                                   f"memory; device cap {args.cap_gb} GB, M_b = {args.batch_edges} edges "
+                                   f"memory; device cap {args.cap_gb} GB, M_b = {args.batch_edges if args.batch_edges > 0 else 'derived from the cap'} "
                                    f"(shape of BASELINE.json configs[4])", "n": n, "m": m,
                        "step": "wl_refine_batched to the batched fixed point (Algorithm 2, B1-B7)"},
             "seconds_to_stable_coloring": sec, "outer_iters": st["outer_iters"], "num_colors": st["num_colors"],
@@ -326,7 +326,7 @@ def main():
     ap.add_argument("--workload", default="single", choices=["single", "batched", "batch-study", "cap-sweep"],
                     help="single: wl_refine on the HBM-resident graph (the headline); batched: wl_refine_batched")
     ap.add_argument("--cap-gb", type=float, default=16.0, help="batched: device memory cap")
-    ap.add_argument("--batch-edges", type=int, default=120_000_000, help="batched: M_b")
+    ap.add_argument("--batch-edges", type=int, default=0, help="batched: M_b (0: derived by the library from the device cap)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
     if args.impl == "reference":

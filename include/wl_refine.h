@@ -187,6 +187,7 @@ typedef struct wl_edge_batch {
  *                    num_batches == 0: `whole` must be given and the library cuts it itself (Q13).
  *   whole            HOST CSR of the full graph, or NULL when batches are given in COO form.
  *   max_batch_edges  M_b (L171): cap on edges per batch for the library's own partitions (later outer iterations, Q14).
+ *                    <= 0 (with `whole` and a device cap): the library derives the largest M_b that fits the cap.
  *   device_cap_bytes upper bound on device memory the call may allocate (0 = no cap); WL_ENOMEM if it cannot be met.
  *   out_colors       HOST int32[n], canonical ids on the ORIGINAL nodes (Q16). */
 int wl_refine_batched(int64_t n, int32_t num_batches, const wl_edge_batch* batches, const wl_csr* whole, uint64_t seed,

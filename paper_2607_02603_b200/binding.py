@@ -336,12 +336,13 @@ def wl_quotient(n, row_ptr, col_idx, weights, colors: torch.Tensor, k: int):
 
 
 def wl_refine_batched(n: int, row_ptr: torch.Tensor, col_idx: torch.Tensor, weights: Optional[torch.Tensor] = None, *,
-                      max_batch_edges: int, cuts=None, seed: int = 0, device_cap_bytes: int = 0, flags: int = 0,
+                      max_batch_edges: int = 0, cuts=None, seed: int = 0, device_cap_bytes: int = 0, flags: int = 0,
                       max_outer_iters: int = 0, out: Optional[torch.Tensor] = None, device=None,
                       allow_limit: bool = False, host_workspace: Optional[torch.Tensor] = None) -> RefineResult:
     """Algorithm 2 over a HOST-resident CSR (pinned recommended).  cuts (optional, increasing edge positions from 0 to m)
     gives the edge partition of the first outer iteration as consecutive CSR slices; otherwise the library cuts by
-    max_batch_edges.  Returns canonical colours on the original nodes (host int32[n])."""
+    max_batch_edges; max_batch_edges <= 0 (with device_cap_bytes > 0): the library derives M_b from the cap.
+    Returns canonical colours on the original nodes (host int32[n])."""
     L = lib()
     if not torch.cuda.is_available():
         raise RuntimeError("wl_refine_batched needs a CUDA device (no CPU fallback)")

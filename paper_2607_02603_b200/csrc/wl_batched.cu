@@ -470,9 +470,12 @@ int wl_quotient(const wl_csr* g, const int32_t* colors, int64_t k, int64_t* q_ro
 // ---------------------------------------------------------------------------------------------------------------------
 // Algorithm 2
 // ---------------------------------------------------------------------------------------------------------------------
-int wl_refine_batched(int64_t n, int32_t num_batches, const wl_edge_batch* batches, const wl_csr* whole, uint64_t seed,
-                      size_t device_cap_bytes, int64_t max_batch_edges, int32_t* out_colors, wl_stats* stats,
-                      const wl_options* opt, void* cuda_stream) {
+}  // extern "C"
+
+// Algorithm 2 for a given M_b (the exported entry point below picks M_b from the device cap when the caller gives none)
+static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batches, const wl_csr* whole, uint64_t seed,
+                       size_t device_cap_bytes, int64_t max_batch_edges, int32_t* out_colors, wl_stats* stats,
+                       const wl_options* opt, void* cuda_stream) {
   if (stats) std::memset(stats, 0, sizeof(*stats));
   if (n < 0 || num_batches < 0 || max_batch_edges <= 0) return WL_EINVAL;
   if (n > kMaxNodes) return WL_ERANGE;
@@ -1012,6 +1015,38 @@ int wl_refine_batched(int64_t n, int32_t num_batches, const wl_edge_batch* batch
   cleanup();
   if (rc == WL_OK && hit_limit) return WL_EMAXROUNDS;
   return rc;
+}
+
+// Rough device budget of batched_run for a batch cap M_b (DESIGN.md §8 "Device budget"): node arrays, two input and two
+// output buffers of 8 bytes per edge, the quotient table, the local workspace of a batch with its share of the rows.
+static double batched_budget(int64_t n, int64_t m, int64_t mb) {
+  double slots = 1024;
+  while (slots < 2.0 * (double)mb) slots *= 2;
+  const double rows = m > 0 ? (double)n * (double)mb / (double)m + 1 : (double)n;
+  return 44.0 * (double)n + 32.0 * (double)mb + 16.0 * slots + 80.0 * rows + (double)(1 << 20);
+}
+
+extern "C" {
+
+int wl_refine_batched(int64_t n, int32_t num_batches, const wl_edge_batch* batches, const wl_csr* whole, uint64_t seed,
+                      size_t device_cap_bytes, int64_t max_batch_edges, int32_t* out_colors, wl_stats* stats,
+                      const wl_options* opt, void* cuda_stream) {
+  if (max_batch_edges > 0)
+    return batched_run(n, num_batches, batches, whole, seed, device_cap_bytes, max_batch_edges, out_colors, stats, opt,
+                       cuda_stream);
+  // M_b <= 0: derive it from the device cap (BASELINE.json configs[4]: "a device working-set cap forces the batching").
+  // The largest M_b whose estimated budget fits 90 % of the cap; an estimate that turns out too low is answered by WL_ENOMEM
+  // from the checked allocations, and M_b shrinks until the run fits.
+  if (device_cap_bytes == 0 || num_batches != 0 || !whole || n <= 0) return WL_EINVAL;
+  const int64_t m = whole->m;
+  int64_t mb = m > 0 ? m : 1;
+  while (mb > 1024 && batched_budget(n, m, mb) > 0.9 * (double)device_cap_bytes) mb = (int64_t)((double)mb * 0.8);
+  for (int attempt = 0; attempt < 12; ++attempt) {
+    const int rc = batched_run(n, 0, nullptr, whole, seed, device_cap_bytes, mb, out_colors, stats, opt, cuda_stream);
+    if (rc != WL_ENOMEM || mb <= 1024) return rc;
+    mb = (int64_t)((double)mb * 0.7);
+  }
+  return WL_ENOMEM;
 }
 
 }  // extern "C"

@@ -186,6 +186,26 @@ def test_batched_device_cap_is_checked_for_every_allocation():
     assert hi < (1 << 30)
 
 
+def test_batched_batch_cap_derived_from_device_cap():
+    """max_batch_edges <= 0: M_b comes from the device cap (the shape of configs[4]: a cap forces the batching).  The run must
+    stay under the cap (every allocation is checked), use several batches, and give a stable refinement of the coarsest
+    colouring; without a cap the request is invalid."""
+    g = gg.rmat(14, seed=6, symmetrize=False)
+    n, rp, ci, wt = g.numpy()
+    coarsest, _, _ = oracle.refine(n, rp, ci)
+    for cap in (6 << 20, 12 << 20):
+        res = wl.wl_refine_batched(n, g.row_ptr, g.col, None, device_cap_bytes=cap, seed=2)
+        got = res.colors.numpy()
+        assert oracle.is_stable(n, rp, ci, None, got) and refines(got, coarsest)
+        assert res.stats["outer_iters"] >= 2  # more than one batch: the graph did not fit the cap
+    with pytest.raises(wl.WlError) as e:
+        wl.wl_refine_batched(n, g.row_ptr, g.col, None, seed=2)
+    assert e.value.code == wl.WL_EINVAL
+    with pytest.raises(wl.WlError) as e:
+        wl.wl_refine_batched(n, g.row_ptr, g.col, None, device_cap_bytes=1 << 16, seed=2)
+    assert e.value.code == wl.WL_ENOMEM
+
+
 def test_batched_device_cap_and_limits():
     g = gg.rmat(10, seed=1)
     with pytest.raises(wl.WlError) as e:
