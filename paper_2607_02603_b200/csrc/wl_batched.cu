@@ -280,6 +280,13 @@ struct DevBuf {
     *used += bytes;
     return WL_OK;
   }
+  void release(size_t* used) {  // give the memory back before the end of the scope
+    if (!p) return;
+    cudaFree(p);
+    p = nullptr;
+    if (*used >= bytes) *used -= bytes;
+    bytes = 0;
+  }
   template <typename T>
   T* as() const { return (T*)p; }
 };
@@ -757,6 +764,12 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
     }
 
     phase("merge + canonical");
+    // the uncanonical block map and the canonicalisation scratch are dead: their 12 bytes per node go to the quotient pass
+    cudaStreamSynchronize(st);
+    d_H.release(&used_iter);
+    d_first.release(&used_iter);
+    d_cof.release(&used_iter);
+    d_ws.release(&used_iter);
     // ---- Alg. 2 line 13: quotient (Def. 4), second streaming pass -------------------------------------------------------
     // Three streams: copy_st uploads batch k + 1 while st inserts / emits batch k and down_st returns the rows emitted for
     // batch k - 1 to the host (double buffers on both sides; one host synchronisation per batch, to learn the emitted size).
@@ -1023,7 +1036,7 @@ static double batched_budget(int64_t n, int64_t m, int64_t mb) {
   double slots = 1024;
   while (slots < 2.0 * (double)mb) slots *= 2;
   const double rows = m > 0 ? (double)n * (double)mb / (double)m + 1 : (double)n;
-  return 44.0 * (double)n + 32.0 * (double)mb + 16.0 * slots + 80.0 * rows + (double)(1 << 20);
+  return 32.0 * (double)n + 32.0 * (double)mb + 16.0 * slots + 80.0 * rows + (double)(1 << 20);
 }
 
 extern "C" {
