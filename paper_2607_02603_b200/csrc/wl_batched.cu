@@ -609,7 +609,6 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
   while (true) {
     ++outer;
     const int nb = (int)cuts.size() - 1;
-    const int64_t m_t = rp[n_t];
     // inner ranges and sizes
     std::vector<int64_t> r0(nb), r1(nb);
     int64_t max_rows = 1, max_edges = 1;
@@ -657,8 +656,7 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
     WL_ALLOC(d_misc, 4096);
     if (rc) break;
 
-    auto upload_batch = [&](int k, int buf, bool rows_all) {
-      // rows_all: the quotient pass needs every row that starts inside the batch's node range (incl. a crossing one)
+    auto upload_batch = [&](int k, int buf) {
       const int64_t c0 = cuts[k], c1 = cuts[k + 1];
       const int* hc = (outer == 1) ? batch_col(k) : hq.col + c0;
       const u32* hw = (outer == 1) ? batch_wt(k) : hq.wt + c0;
@@ -670,7 +668,6 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
           bytes_h2d += sizeof(u32) * (c1 - c0);
         }
       }
-      (void)rows_all;
       const int64_t nr = r1[k] - r0[k];
       cudaMemcpyAsync(d_rp[buf].p, rp + r0[k], sizeof(int64_t) * (size_t)(nr + 1), cudaMemcpyHostToDevice, copy_st);
       bytes_h2d += sizeof(int64_t) * (nr + 1);
@@ -681,10 +678,10 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
     // ---- Alg. 2 lines 7-11: local refinement per batch, merge ---------------------------------------------------------
     int64_t base_id = have_next ? next_base_id : 0;
     cudaStreamSynchronize(st);  // buffers of the previous iteration are free
-    if (!have_next) upload_batch(0, 0, false);
+    if (!have_next) upload_batch(0, 0);
     for (int k = 0; k < nb && !rc && !have_next; ++k) {
       const int buf = k & 1;
-      if (k + 1 < nb) upload_batch(k + 1, buf ^ 1, false);
+      if (k + 1 < nb) upload_batch(k + 1, buf ^ 1);
       cudaStreamWaitEvent(st, ev_up[buf], 0);
       const int64_t nr = r1[k] - r0[k];
       if (nr == 0) continue;
@@ -973,13 +970,12 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
     rp = nrp;
     n_t = K;
     weighted = true;
-    const int64_t next_nb_cap = max_batch_edges;
     std::vector<int64_t> next_cuts;
     if (inherit) {
       next_cuts = next_edge_cuts;
       if (next_cuts.size() == 1) next_cuts.push_back(0);  // no block at all cannot happen (K >= 1); keep one batch
     } else {
-      greedy_cuts(n_t, rp, next_nb_cap, next_cuts);
+      greedy_cuts(n_t, rp, max_batch_edges, next_cuts);
     }
     if ((flags & WL_FLAG_AGGRESSIVE_STOP) && (int64_t)next_cuts.size() - 1 >= nb) {  // L328
       break;
@@ -994,7 +990,6 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
       d_Hnext.p = nullptr;
       have_next = true;
     }
-    (void)m_t;
   }
 
   if (rc == WL_OK) {
