@@ -29,10 +29,15 @@ if ROOT not in sys.path:
 RMAT_SEEDS = {22: 1, 27: 2, 30: 3}  # BASELINE.json configs[2..4]
 ORACLE_SAMPLE_SCALE = 21           # bounded sample of the same recipe for the CPU oracle (about 10-30 s)
 HBM_FALLBACK_GBS = 6650.0          # /opt/skills/guides/B200_PROFILING.md fallback
-# DRAM bytes of the dominant launch (round-2 row kernel 40.71 + 0.74 GB, hub kernel 8.49 + 0.005 GB), ncu --set full
-NCU_TRAFFIC_BYTES = 49.95e9
-# DRAM bytes of the round-2 relabel_kernel (8.08 + 2.32 GB, profiles/r1d_ncu_full.md); the compaction is not counted
-NCU_RELABEL_BYTES = 10.40e9
+
+
+def ncu_traffic():
+    """DRAM bytes per launch of the round-2 kernels from the last `ncu --set full` capture: a tracked data file that names the
+    commit it was measured on (profiles/ncu_traffic.json), never a constant in this script."""
+    try:
+        return json.load(open(os.path.join(ROOT, "profiles", "ncu_traffic.json")))
+    except Exception:
+        return None
 
 
 def measured_peaks():
@@ -410,6 +415,9 @@ def main():
     top_bytes = results[-1].stats["spmv_top_alg_bytes"]
     top_edges = results[-1].stats["spmv_top_edges"]
     roofline = None
+    tr = ncu_traffic() if args.scale == 27 and not args.flags else None
+    NCU_TRAFFIC_BYTES = tr["spmv_round2_bytes"] if tr else None
+    NCU_RELABEL_BYTES = tr["relabel_round2_bytes"] if tr else None
     if spmv_launches and top_ms > 0:
         achieved = top_bytes / (top_ms / 1e3) / 1e9
         roofline = {"bound": "hbm", "kernel": "spmv_merge_kernel" if args.flags & 4 else
@@ -418,9 +426,10 @@ def main():
                     "peak_kind": f"{peak_kind} copy bandwidth", "algorithmic_bytes_per_launch": top_bytes,
                     "avg_launch_ms": top_ms, "launches_timed": len(results),
                     "gedges_per_s_in_kernel": top_edges / (top_ms / 1e3) / 1e9,
-                    "traffic": NCU_TRAFFIC_BYTES if args.scale == 27 and not args.flags else None,
-                    "dram_gb_per_s_ncu_traffic": (NCU_TRAFFIC_BYTES / (top_ms / 1e3) / 1e9) if args.scale == 27 and not args.flags else None,
-                    "traffic_source": "profiles/r1g_final_build.md (dram__bytes_read.sum + dram__bytes_write.sum, row + hub kernel)",
+                    "traffic": NCU_TRAFFIC_BYTES,
+                    "dram_gb_per_s_ncu_traffic": (NCU_TRAFFIC_BYTES / (top_ms / 1e3) / 1e9) if tr else None,
+                    "traffic_source": (f"profiles/ncu_traffic.json <- {tr['source']}, measured on commit {tr['measured_on_commit']} "
+                                       "(dram__bytes_read.sum + dram__bytes_write.sum, row + hub kernel)") if tr else None,
                     "share_of_step": top_ms / ms_per_step,
                     "all_spmv_launches": {"launches": spmv_launches, "algorithmic_gb_per_s": alg_bytes / (spmv_ms / 1e3) / 1e9,
                                           "gedges_per_s": spmv_edges / (spmv_ms / 1e3) / 1e9,
@@ -432,7 +441,7 @@ def main():
                         ((top_ms + sum(r.stats["ms_rest_top"] for r in results) / len(results)) / 1e3) / 1e9,
                         "dram_gb_per_s_ncu": ((NCU_TRAFFIC_BYTES + NCU_RELABEL_BYTES) /
                                               ((top_ms + sum(r.stats["ms_rest_top"] for r in results) / len(results)) / 1e3) / 1e9)
-                        if args.scale == 27 and not args.flags else None},
+                        if tr else None},
                     "binding_unit": "L1TEX 76 % / L2 73 % of peak (ncu): one sector lookup per gathered 2-byte id; DRAM 43 %"}
 
     # ---- end to end through the host-buffer entry point ---------------------------------------------------------------

@@ -215,17 +215,42 @@ scan32_sum_kernel(const int* __restrict__ in, int64_t n, u64* __restrict__ bsum)
   }
 }
 
-__global__ void scan64_serial_kernel(u64* __restrict__ bsum, int64_t nb, u64* __restrict__ total) {
-  // nb is n / 2048: a single thread is enough up to billions of nodes (<= 1M block sums)
-  if (blockIdx.x == 0 && threadIdx.x == 0) {
-    u64 run = 0;
-    for (int64_t i = 0; i < nb; ++i) {
-      u64 t = bsum[i];
-      bsum[i] = run;
-      run += t;
+// exclusive scan of the nb block sums by one CTA (nb = n / 2048: at most 2^20 sums for 2^31 nodes); total -> *total
+__global__ void __launch_bounds__(1024) scan64_bsum_kernel(u64* __restrict__ bsum, int64_t nb, u64* __restrict__ total) {
+  __shared__ u64 s_w[32];
+  __shared__ u64 s_carry;
+  if (threadIdx.x == 0) s_carry = 0;
+  __syncthreads();
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  for (int64_t base = 0; base < nb; base += 1024) {
+    const int64_t i = base + threadIdx.x;
+    const u64 v = i < nb ? bsum[i] : 0;
+    u64 x = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const u64 t = __shfl_up_sync(0xffffffffu, x, o);
+      if (lane >= o) x += t;
     }
-    *total = run;
+    if (lane == 31) s_w[wid] = x;
+    __syncthreads();
+    if (wid == 0) {
+      const u64 t = s_w[lane];
+      u64 xs = t;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const u64 u = __shfl_up_sync(0xffffffffu, xs, o);
+        if (lane >= o) xs += u;
+      }
+      s_w[lane] = xs - t;  // exclusive warp offsets
+    }
+    __syncthreads();
+    const u64 carry = s_carry;
+    if (i < nb) bsum[i] = carry + s_w[wid] + x - v;
+    __syncthreads();
+    if (threadIdx.x == 1023) s_carry = carry + s_w[wid] + x;
+    __syncthreads();
   }
+  if (threadIdx.x == 0) *total = s_carry;
 }
 
 __global__ void __launch_bounds__(kScanT)
@@ -341,7 +366,7 @@ void launch_scan32(const int* cnt, int64_t n, int64_t base_off, int64_t* out, u6
   if (n == 0) return;
   const int64_t nb = (n + kScanC - 1) / kScanC;
   ++g_launches; scan32_sum_kernel<<<(unsigned)nb, kScanT, 0, st>>>(cnt, n, bsum);
-  ++g_launches; scan64_serial_kernel<<<1, 32, 0, st>>>(bsum, nb, total);
+  ++g_launches; scan64_bsum_kernel<<<1, 1024, 0, st>>>(bsum, nb, total);
   ++g_launches; scan32_apply_kernel<<<(unsigned)nb, kScanT, 0, st>>>(cnt, n, bsum, base_off, out);
 }
 
@@ -454,7 +479,7 @@ int wl_quotient(const wl_csr* g, const int32_t* colors, int64_t k, int64_t* q_ro
   off += 256;
   int* long_rows = (int*)(ws + off);
   cudaMemsetAsync(table, 0, sizeof(u64) * 2 * slots, st);
-  cudaMemsetAsync(rep_of_block, 0x7f, sizeof(int) * (size_t)k, st);
+  if (k > 0) { ++g_launches; fill_kernel<<<blocks_for(k, 256), 256, 0, st>>>(k, rep_of_block, kNoNode); }
   cudaMemsetAsync(cnt, 0, sizeof(int) * (size_t)k, st);
   cudaMemsetAsync(cursor, 0, sizeof(int) * (size_t)k, st);
   ++g_launches; block_rep_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, colors, rep_of_block);
@@ -596,7 +621,7 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
   DevBuf d_Hnext_keep;             // ... its merged block map (before the boundary / canonical step)
   std::vector<int64_t> node_cuts;  // ... and the node ranges of its batches
   int64_t next_base_id = 0;
-  const bool debug = std::getenv("WL_DEBUG") != nullptr;
+  const bool debug = debug_enabled();
   auto wall = [] { return std::chrono::duration<double>(std::chrono::steady_clock::now().time_since_epoch()).count(); };
   double t_mark = wall();
   auto phase = [&](const char* what) {  // WL_DEBUG: host wall-clock per phase (each phase ends on a synchronised stream)
@@ -794,7 +819,7 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
     WL_ALLOC(d_long, sizeof(int) * (size_t)(max_edges / kQuotLongRow + 2));
     if (debug) std::fprintf(stderr, "[wl_refine_batched] outer %d device memory %.2f GB (cap %.2f GB)%s\n", outer, used_iter / 1073741824.0, device_cap_bytes / 1073741824.0, rc ? " -> WL_ENOMEM" : "");
     if (rc) break;
-    cudaMemsetAsync(d_rep.p, 0x7f, sizeof(int) * (size_t)K, st);
+    ++g_launches; fill_kernel<<<blocks_for(K, 256), 256, 0, st>>>(K, d_rep.as<int>(), kNoNode);
     cudaMemsetAsync(d_cnt.p, 0, sizeof(int) * (size_t)K, st);
     cudaMemsetAsync(d_cursor.p, 0, sizeof(int) * (size_t)K, st);
     cudaMemsetAsync(d_qtab.p, 0, sizeof(u64) * 2 * qslots, st);

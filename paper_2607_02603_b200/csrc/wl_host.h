@@ -9,6 +9,8 @@
 namespace wl {
 
 constexpr int64_t kMaxNodes = (1ll << 31) - 2;
+constexpr int kNoNode = 0x7fffffff;  // "no node yet" in the atomicMin arrays (first node per colour / block)
+static_assert((int64_t)kNoNode > kMaxNodes - 1, "the sentinel must exceed every node index");
 constexpr uint32_t kFlagLazyDeep = 1u << 30;  // internal (wl_refine_host): the engine may cudaMalloc the deep-round workspace
 
 constexpr int kRunAhead = kNumScal - kScalLog;  // rounds queued per host synchronisation in the deep-round regime
@@ -66,6 +68,7 @@ struct EventPool {
 extern thread_local int g_last_cuda_error;
 extern thread_local int64_t g_launches;
 int check_cuda(cudaError_t e);
+bool debug_enabled();
 int basic_csr_check(const wl_csr* g);
 
 }  // namespace wl

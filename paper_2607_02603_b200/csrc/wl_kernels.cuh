@@ -613,12 +613,6 @@ compact_active_kernel(int64_t count, const int* __restrict__ nodes, const int* _
   if (keep) next[s_base + rank] = i;
 }
 
-// Round with a single colour and unit weights: y_i = outdeg(i) * w(0); no column read.
-__global__ void spmv_uniform_kernel(int64_t n, const int64_t* __restrict__ row_ptr, u64 w0, u64* __restrict__ y) {
-  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i < n) y[i] = (u64)(row_ptr[i + 1] - row_ptr[i]) * w0;
-}
-
 // ---------------------------------------------------------------------------------------------------------------------
 // S3+S4: relabel (colour_i, y_i) -> dense id (Alg. 1 line 6, L122; Q6: exact 96-bit pairs, never a hash of them).
 // A block keeps its id for the sub-block that agrees with its representative rep[c]; every other distinct pair
@@ -876,6 +870,11 @@ __global__ void init_labels_kernel(int64_t n, const int* __restrict__ init, int*
 constexpr int kScanThreads = 256;
 constexpr int kScanItems = 8;
 constexpr int kScanChunk = kScanThreads * kScanItems;
+
+__global__ void fill_i32_kernel(int64_t n, int* __restrict__ a, int v) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) a[i] = v;
+}
 
 __global__ void first_node_kernel(int64_t n, const int* __restrict__ colour, int* __restrict__ first) {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;

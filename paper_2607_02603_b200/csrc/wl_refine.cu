@@ -224,12 +224,18 @@ static u32 round_table_mask(const Layout& L, int64_t n_active) {
 void launch_canonical(const Layout& L, int64_t n, const int* colour, int* out, int* first, int* cid, int* bsum,
                       u64* total, cudaStream_t st) {
   if (n == 0) return;
-  cudaMemsetAsync(first, 0x7f, sizeof(int) * (size_t)n, st);
+  ++g_launches; fill_i32_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, first, kNoNode);
   ++g_launches; first_node_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, colour, first);
   ++g_launches; canon_count_kernel<<<(unsigned)L.nscan, kScanThreads, 0, st>>>(n, colour, first, bsum);
   ++g_launches; scan_bsum_kernel<<<1, 1024, 0, st>>>(L.nscan, bsum, total);
   ++g_launches; canon_rank_kernel<<<(unsigned)L.nscan, kScanThreads, 0, st>>>(n, colour, first, bsum, cid);
   ++g_launches; canon_apply_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, colour, cid, out);
+}
+
+// WL_DEBUG (per-round trace on stderr) is read once per process, not per call
+bool debug_enabled() {
+  static const bool on = std::getenv("WL_DEBUG") != nullptr;
+  return on;
 }
 
 int check_cuda(cudaError_t e) {
@@ -461,8 +467,8 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
   int64_t rows_top = 0, last_rows = 0;
   int32_t rounds = 0, spmv_launches = 0;
   bool converged = false;
-  const bool debug = std::getenv("WL_DEBUG") != nullptr;
-  const double list_frac = std::getenv("WL_LIST_FRAC") ? std::atof(std::getenv("WL_LIST_FRAC")) : 0.75;
+  const bool debug = debug_enabled();
+  constexpr double list_frac = 0.75;  // an active list pays once a quarter of the rows has left (measured, scale 27)
   const bool no_runahead = (flags & WL_FLAG_SYNC_EVERY_ROUND) != 0;
   const int* cur_list = nullptr;  // NULL: every node is active
   int64_t n_active = n, active_edges = m, pending_new = 0;
