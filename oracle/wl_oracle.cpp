@@ -18,7 +18,8 @@
 //   oracle_inner_labels  Def. 5 (L139-L145) via per-node batch labels (L463).             PINNED (set brute force)
 //   oracle_quotient      Def. 4 / Eq. 1 (L59-L65), representative = minimum node index.   PINNED (dense A.S = S.A')
 //   oracle_rbsc          Algorithm 2 (L169-L202) with oracle_refine in place of RSC.     PINNED (Thm 2 invariants,
-//                        N_b = 1 equality, order independence)
+//                        N_b = 1 equality, order independence; the L328 stop rule: equals the plain loop cut after the
+//                        iteration a Python restatement of the rule names)
 //   oracle_weight        the keyed bijection w = P_key(colour) that DESIGN.md §"Readings" Q4/Q5 fixes in place of
 //                        the paper's unseeded xoshiro/SplitMix recipe (L467-L473).  Bit stream: PARITY UNPINNED
 //                        (the paper prints no test vectors); bijectivity and constants are pinned.
@@ -227,9 +228,13 @@ static void greedy_cuts(i64 n, const i64* rp, i64 cap, std::vector<i64>& cuts) {
 // inherit != 0 (reading Q14b): from the second outer iteration on the edge partition is not re-cut by M_b;
 // the quotient inherits the batches of its graph: batch k of the quotient = the blocks whose representative row is complete
 // once batch k of the graph has been read (in node order), with exactly their rows.  L163 allows any partition.
+// aggressive != 0 (L328, the termination used for Table 4): "the outer loop of Algorithm 2 stops as soon as the number of
+// batches in the next iteration would not decrease": after the quotient of an iteration that ran with N_b batches has been
+// built, the edge partition of the next iteration is made as usual; if it has >= N_b batches the loop ends with the
+// colouring reached so far (every outer iteration ends on a stable colouring, Thm 2 / L206).
 i64 oracle_rbsc(i64 n0, const i64* row_ptr0, const i32* col0, const u32* wt0, i64 max_batch_edges,
-                i32 nb0, const i64* first_cuts, const i32* first_edge_batch, i32 max_outer, i32 inherit, i32* out,
-                i64* stats) {
+                i32 nb0, const i64* first_cuts, const i32* first_edge_batch, i32 max_outer, i32 inherit, i32 aggressive,
+                i32* out, i64* stats) {
   i64 n = n0;
   std::vector<i64> rp(row_ptr0, row_ptr0 + n0 + 1);
   std::vector<i32> col(col0, col0 + rp[n0]);
@@ -348,6 +353,18 @@ i64 oracle_rbsc(i64 n0, const i64* row_ptr0, const i32* col0, const u32* wt0, i6
     wt.assign(qwt.begin(), qwt.begin() + qm);
     n = k;
     if (stop || outer >= max_outer) break;
+    if (aggressive) {  // L328: N_b of the next iteration
+      i64 nb_next;
+      if (inherit && !inh_cuts.empty()) {
+        nb_next = (i64)inh_cuts.size() - 1;
+      } else {
+        std::vector<i64> next_cuts;
+        greedy_cuts(n, rp.data(), max_batch_edges, next_cuts);
+        nb_next = (i64)next_cuts.size() - 1;
+      }
+      if (nb_next < 1) nb_next = 1;
+      if (nb_next >= nb) break;
+    }
   }
   if (stats) {
     stats[0] = outer;

@@ -125,6 +125,30 @@ def test_batched_inherited_batches_equal_cpu_algorithm2(name, nb):
     assert refines(got, coarsest)
 
 
+@pytest.mark.parametrize("name", list(BATCH_GRAPHS))
+@pytest.mark.parametrize("nb", [2, 3, 5, 16])
+@pytest.mark.parametrize("inherit", [False, True])
+def test_batched_aggressive_stop_equals_cpu_algorithm2(name, nb, inherit):
+    """WL_FLAG_AGGRESSIVE_STOP (stop as soon as the next iteration would not run with fewer batches), alone and
+    with inherited batches: bit-exact against the CPU Algorithm 2 with the same stop rule, same number of outer iterations;
+    the result is a stable colouring (Thm 2) that refines the coarsest one and is refined by... the full loop's result is
+    coarser or equal (L206)."""
+    g = BATCH_GRAPHS[name]()
+    n, rp, ci, wt = g.numpy()
+    cap = max(1, -(-g.m // nb))
+    coarsest, _, _ = oracle.refine(n, rp, ci, wt)
+    want, k_want, outer_want, nbl_want = oracle.rbsc(n, rp, ci, wt, cap, inherit=inherit, aggressive=True)
+    flags = wl.WL_FLAG_AGGRESSIVE_STOP | (wl.WL_FLAG_INHERIT_BATCHES if inherit else 0)
+    res = wl.wl_refine_batched(n, g.row_ptr, g.col, g.weights, max_batch_edges=cap, seed=nb, flags=flags)
+    got = res.colors.numpy()
+    assert got.tolist() == want.tolist() and res.num_colors == k_want
+    assert res.stats["outer_iters"] == outer_want and res.stats["last_num_batches"] == nbl_want
+    assert oracle.is_stable(n, rp, ci, wt, got) and refines(got, coarsest)
+    full = wl.wl_refine_batched(n, g.row_ptr, g.col, g.weights, max_batch_edges=cap, seed=nb,
+                                flags=flags & ~wl.WL_FLAG_AGGRESSIVE_STOP)
+    assert refines(got, full.colors.numpy()) and res.stats["outer_iters"] <= full.stats["outer_iters"]
+
+
 def test_batched_caller_supplied_slices():
     g = gg.rmat(10, seed=4)
     n, rp, ci, wt = g.numpy()

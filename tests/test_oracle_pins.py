@@ -280,6 +280,72 @@ def test_rbsc_inherited_batches_invariants(seed):
         assert refines(c1, c)               # every outer iteration coarsens (L206)
 
 
+def _num_greedy_batches(n, rp, cap):
+    """N_b of the library's default partition, restated on a plain offset list (Q13)."""
+    import torch
+    g = gg.Graph(n=n, row_ptr=torch.as_tensor(np.asarray(rp), dtype=torch.int64),
+                 col=torch.zeros(int(rp[-1]), dtype=torch.int32), weights=None, name="q")
+    return max(1, len(gg.contiguous_row_batches(g, cap)) - 1)
+
+
+@pytest.mark.parametrize("seed", range(14))
+def test_rbsc_aggressive_stop_is_the_plain_loop_cut_where_the_rule_says(seed):
+    """"the outer loop of Algorithm 2 stops as soon as the number of batches in the next iteration would not
+    decrease".  Pin: run the PLAIN loop limited to t = 1, 2, ... iterations, build the quotient of each result with
+    oracle.quotient, count the batches the default partition gives it (independent restatement in graphgen); the first t
+    whose successor would not run with fewer batches (or where the plain loop ends anyway) must be where the aggressive run
+    stops, with the same colouring.  Plus Theorem 2, L165 and L206 (the plain result is coarser or equal)."""
+    g = gg.rmat(6 + seed % 3, edge_factor=2 + seed % 4, seed=seed, symmetrize=bool(seed % 2)) if seed < 10 else \
+        gg.random_weighted_digraph(50 + seed, 260, seed, max_w=2)
+    n, rp, ci, wt = _np(g)
+    A = dense_adj(n, rp, ci, wt)
+    coarsest, _, _ = oracle.refine(n, rp, ci, wt)
+    stopped_early = 0
+    for nb in (2, 3, 5, 9):
+        cap = max(1, -(-g.m // nb))
+        full, _, outer_full, _ = oracle.rbsc(n, rp, ci, wt, cap)
+        got, k, outer, nbl = oracle.rbsc(n, rp, ci, wt, cap, aggressive=True)
+        assert stable_dense(A, got) and refines(got, coarsest) and refines(got, full)
+        # walk the plain loop
+        nb_t = _num_greedy_batches(n, rp, cap)
+        expect_t = None
+        for t in range(1, outer_full + 1):
+            c_t, k_t, o_t, nbl_t = oracle.rbsc(n, rp, ci, wt, cap, max_outer=t)
+            assert nbl_t == nb_t
+            if t == outer_full:
+                expect_t = t
+                break
+            _, qrp, qc, qw = oracle.quotient(n, rp, ci, wt, c_t)
+            nb_next = _num_greedy_batches(k_t, qrp, cap)
+            if nb_next >= nb_t:
+                expect_t = t
+                break
+            nb_t = nb_next
+        assert outer == expect_t and nbl == nb_t
+        assert got.tolist() == c_t.tolist()
+        stopped_early += outer < outer_full
+    if seed in (0, 1, 2, 3):
+        assert stopped_early >= 1  # the rule really cuts the loop short on these graphs (42 of the 56 cases do)
+
+
+def test_rbsc_aggressive_stop_hand_case():
+    """A directed path 0 -> 1 -> ... -> 9 with one edge per batch: iteration 1 leaves everything discrete except nothing to
+    merge, the quotient is the graph itself, so the next iteration would run with the same 9 batches: the aggressive rule
+    stops after ONE iteration where the plain rule also stops (|V| unchanged); with twin leaves split over two batches
+    (test above) the quotient shrinks to fewer batches and both rules go on."""
+    g = gg.directed_path(10)
+    n, rp, ci, wt = _np(g)
+    c, k, outer, nbl = oracle.rbsc(n, rp, ci, None, 1, aggressive=True)
+    assert outer == 1 and k == 10
+    # two stars whose leaves are spread over many single-edge batches: iteration 1 merges nothing (every leaf is inner to its
+    # own batch, alone), the quotient keeps all edges -> same N_b -> the aggressive rule stops, the plain rule too (|V| = n)
+    g = gg.from_edge_list(7, [(1, 0), (2, 0), (3, 0), (4, 6), (5, 6)])
+    n, rp, ci, wt = _np(g)
+    ca, ka, oa, _ = oracle.rbsc(n, rp, ci, None, 2, aggressive=True)
+    cp, kp, op, _ = oracle.rbsc(n, rp, ci, None, 2)
+    assert oa <= op and refines(ca, cp)
+
+
 def test_rbsc_single_batch_is_refine():
     g = gg.erdos_renyi(300, 900, seed=3)
     n, rp, ci, wt = _np(g)
