@@ -85,6 +85,9 @@ typedef struct wl_options {
                                host pages costs far more than the transfers; callers that refine repeatedly should pass
                                one).  Caller-owned, contents undefined before and after.                               */
   size_t host_workspace_bytes; /* wl_refine_batched_host_bytes(n, m) always suffices; a smaller one is ignored          */
+  int32_t ring_bits;        /* Algorithm 1's precision parameter q (L109-L110): the ring is Z/2^q.  0 or >= 64: q = 64, the
+                               only setting Theorem 1's 1e-9 guarantee covers (L129).  1..63: every z is reduced mod 2^q where
+                               it is compared; used to COUNT collisions (Lemma 1), never for production results          */
 } wl_options;
 
 typedef struct wl_stats {

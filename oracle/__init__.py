@@ -71,8 +71,9 @@ def is_stable(n, row_ptr, col, wt, colors) -> bool:
     return bool(lib().oracle_is_stable(n, _p(rp, C.c_int64), _p(ci, C.c_int32), _p(w, C.c_uint32), _p(c, C.c_int32)))
 
 
-def refine(n, row_ptr, col, wt=None, init=None, max_rounds: Optional[int] = None):
-    """-> (colors int32[n] canonical, counts per round list, rounds)."""
+def refine(n, row_ptr, col, wt=None, init=None, max_rounds: Optional[int] = None, allow_unconverged: bool = False):
+    """-> (colors int32[n] canonical, counts per round list, rounds).  allow_unconverged: return the partition reached after
+    max_rounds rounds instead of raising (used to walk the trajectory round by round)."""
     rp, ci, w = _csr(n, row_ptr, col, wt)
     ini = None if init is None else np.ascontiguousarray(init, dtype=np.int32)
     max_rounds = n + 2 if max_rounds is None else max_rounds
@@ -81,7 +82,7 @@ def refine(n, row_ptr, col, wt=None, init=None, max_rounds: Optional[int] = None
     rounds = C.c_int32(0)
     k = lib().oracle_refine(n, _p(rp, C.c_int64), _p(ci, C.c_int32), _p(w, C.c_uint32), _p(ini, C.c_int32),
                             _p(out, C.c_int32), max_rounds, _p(counts, C.c_int64), C.byref(rounds))
-    if k < 0:
+    if k < 0 and not allow_unconverged:
         raise RuntimeError("oracle_refine: max_rounds reached")
     return out, counts[: rounds.value].tolist(), rounds.value
 

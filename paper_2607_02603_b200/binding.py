@@ -49,7 +49,7 @@ class wl_csr(C.Structure):
 class wl_options(C.Structure):
     _fields_ = [("flags", C.c_uint32), ("max_rounds", C.c_int32), ("stream_id", C.c_uint64),
                 ("round_colors", C.c_void_p), ("round_colors_cap", C.c_int32), ("max_outer_iters", C.c_int32),
-                ("host_workspace", C.c_void_p), ("host_workspace_bytes", C.c_size_t)]
+                ("host_workspace", C.c_void_p), ("host_workspace_bytes", C.c_size_t), ("ring_bits", C.c_int32)]
 
 
 class wl_stats(C.Structure):
@@ -180,7 +180,7 @@ def wl_refine_deep_workspace_bytes(n: int, m: int) -> int:
 def wl_refine(n: int, row_ptr: torch.Tensor, col_idx: torch.Tensor, weights: Optional[torch.Tensor] = None,
               init_colors: Optional[torch.Tensor] = None, seed: int = 0, *, flags: int = 0, max_rounds: int = 0,
               stream_id: int = 0, workspace: Optional[torch.Tensor] = None, out: Optional[torch.Tensor] = None,
-              round_cap: int = 4096, allow_max_rounds: bool = False, deep: bool = True) -> RefineResult:
+              round_cap: int = 4096, allow_max_rounds: bool = False, deep: bool = True, ring_bits: int = 0) -> RefineResult:
     """Algorithm 1 on device-resident CSR tensors.  Returns canonical colours (device int32[n]).  When no workspace is
     given, one large enough for the deep-round (worklist) regime is allocated unless deep=False."""
     L = lib()
@@ -196,7 +196,7 @@ def wl_refine(n: int, row_ptr: torch.Tensor, col_idx: torch.Tensor, weights: Opt
     if workspace is None:
         workspace = torch.empty(max(need, 256), dtype=torch.uint8, device=dev)
     rc_buf = (C.c_int64 * round_cap)()
-    opt = wl_options(flags, max_rounds, stream_id, C.cast(rc_buf, C.c_void_p), round_cap, 0, None, 0)
+    opt = wl_options(flags, max_rounds, stream_id, C.cast(rc_buf, C.c_void_p), round_cap, 0, None, 0, ring_bits)
     st = wl_stats()
     with torch.cuda.device(dev):
         rc = L.wl_refine(C.byref(g), _ptr(init_colors), seed, _ptr(out), C.byref(st), C.byref(opt), _ptr(workspace),

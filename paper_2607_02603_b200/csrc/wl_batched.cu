@@ -190,6 +190,173 @@ __global__ void quot_emit_kernel(u64* __restrict__ table, u64 table_slots, const
   table[2 * s + 1] = 0;
 }
 
+
+// ---------------------------------------------------------------------------------------------------------------------
+// COO-form (arbitrary) edge partitions: the first outer iteration of Algorithm 2 for batches given as (src, col, weight)
+// triples (Thm 2: "an arbitrary edge partition of E").  Later iterations run on the library's own host CSR quotients.
+// ---------------------------------------------------------------------------------------------------------------------
+constexpr int kLabelNone = -2, kLabelBoundary = -1;
+
+// B2 (Def. 5, by the method of L463): every edge tags its source with its batch; a source seen with two different
+// batches is a boundary node.  Also: range check of both endpoints (S0), out-degree and weighted row sum per node.
+__global__ void coo_mask_kernel(int64_t ne, const int* __restrict__ src, const int* __restrict__ col,
+                                const u32* __restrict__ wt, int k, int64_t n, int* __restrict__ label, int* __restrict__ deg,
+                                u64* __restrict__ rowsum, u32* __restrict__ err) {
+  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  bool bad = false;
+  for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < ne; e += stride) {
+    const int s = src[e], c = col[e];
+    if ((unsigned)s >= (unsigned)n || (unsigned)c >= (unsigned)n) {
+      bad = true;
+      continue;
+    }
+    int old = label[s];
+    if (old == kLabelNone) old = atomicCAS(label + s, kLabelNone, k);
+    if (old != kLabelNone && old != k && old != kLabelBoundary) label[s] = kLabelBoundary;  // idempotent plain store
+    atomicAdd(deg + s, 1);
+    if (rowsum) atomicAdd(rowsum + s, (u64)wt[e]);
+  }
+  if (bad) atomicOr(err, kErrCol);
+}
+
+// nodes without out-edges are inner to batch 0 (Q9); per label (index label + 1; 0 = boundary): node and edge counts;
+// row sums >= 2^32 (Theorem 1's precondition, L129) and rows of 2^31 entries or more are reported
+__global__ void coo_census_kernel(int64_t n, int* __restrict__ label, const int* __restrict__ deg,
+                                  const u64* __restrict__ rowsum, u64* __restrict__ nodes_of, u64* __restrict__ edges_of,
+                                  u32* __restrict__ err) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const bool valid = i < n;
+  int lab = -3;
+  int d = 0;
+  if (valid) {
+    lab = label[i];
+    d = deg[i];
+    if (lab == kLabelNone) label[i] = lab = 0;
+    if (d < 0 || (rowsum && rowsum[i] >= (1ull << 32))) atomicOr(err, kErrRowSum);
+  }
+  const unsigned peers = __match_any_sync(0xffffffffu, lab);
+  u64 dsum = 0;  // out-degree sum over the lanes that share my label
+  for (unsigned mpeers = peers; mpeers; mpeers &= mpeers - 1) dsum += (u64)(u32)__shfl_sync(peers, d, __ffs(mpeers) - 1);
+  if (valid && (int)(threadIdx.x & 31) == __ffs(peers) - 1) {
+    atomicAdd(nodes_of + (lab + 1), (u64)__popc(peers));
+    atomicAdd(edges_of + (lab + 1), dsum);
+  }
+}
+
+// V_k as a node list: order[off[k] + l] = the l-th inner node of batch k (any order), lid[node] = l
+__global__ void coo_order_kernel(int64_t n, const int* __restrict__ label, const int64_t* __restrict__ off,
+                                 u32* __restrict__ cursor, int* __restrict__ order, int* __restrict__ lid) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const int lab = label[i];
+  if (lab < 0) return;
+  const u32 l = atomicAdd(cursor + lab, 1u);
+  order[off[lab] + l] = (int)i;
+  lid[i] = (int)l;
+}
+
+// rows of A|E_k restricted to V_k (Alg. 2 line 9 needs only them: a singleton can never split): lengths ...
+__global__ void coo_rowlen_kernel(int64_t ne, const int* __restrict__ src, int k, const int* __restrict__ label,
+                                  const int* __restrict__ lid, int* __restrict__ rowlen) {
+  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < ne; e += stride) {
+    const int s = src[e];
+    if (label[s] == k) atomicAdd(rowlen + lid[s], 1);
+  }
+}
+// ... and entries.  A target inside V_k is renamed to its local index; any other target j becomes ~j (negative), which the
+// RANGED SpMV kernels turn into the implicit singleton id 2^32 + (u32)~j of H_k^0 (Eq. 3): distinct per node and
+// disjoint from the dense ids.  Entry order inside a row is arbitrary (sums in Z/2^64 commute).
+__global__ void coo_fill_kernel(int64_t ne, const int* __restrict__ src, const int* __restrict__ col,
+                                const u32* __restrict__ wt, int k, const int* __restrict__ label, const int* __restrict__ lid,
+                                const int64_t* __restrict__ lrp, int* __restrict__ cursor, int* __restrict__ lcol,
+                                u32* __restrict__ lwt) {
+  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < ne; e += stride) {
+    const int s = src[e];
+    if (label[s] != k) continue;
+    const int l = lid[s], c = col[e];
+    const int64_t p = lrp[l] + atomicAdd(cursor + l, 1);
+    lcol[p] = label[c] == k ? lid[c] : ~c;
+    if (lwt) lwt[p] = wt[e];
+  }
+}
+
+// Eq. 4 for a node list: H[order[l]] = base + local colour of l
+__global__ void coo_merge_kernel(int64_t n_local, const int* __restrict__ order, const int* __restrict__ local_colour, int base,
+                                 int* __restrict__ H) {
+  const int64_t l = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (l < n_local) H[order[l]] = base + local_colour[l];
+}
+
+// Alg. 2 lines 11-12: every boundary node becomes a singleton block with a fresh id (any distinct ids: canonicalised later)
+__global__ void coo_boundary_ids_kernel(int64_t n, const int* __restrict__ label, int base, u32* __restrict__ counter,
+                                        int* __restrict__ H) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const bool b = i < n && label[i] == kLabelBoundary;
+  const unsigned bal = __ballot_sync(0xffffffffu, b);
+  if (!bal) return;
+  const int lane = threadIdx.x & 31, leader = __ffs(bal) - 1;
+  u32 first = 0;
+  if (lane == leader) first = atomicAdd(counter, (u32)__popc(bal));
+  first = __shfl_sync(0xffffffffu, first, leader);
+  if (b) H[i] = base + (int)(first + __popc(bal & ((1u << lane) - 1)));
+}
+
+// the given ids (a host list uploaded in one copy) become singleton blocks base, base + 1, ...
+__global__ void singleton_ids_kernel(int64_t count, const int* __restrict__ nodes, int base, int* __restrict__ H) {
+  const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t < count) H[nodes[t]] = base + (int)t;
+}
+
+__global__ void rep_degree_kernel(int64_t K, const int* __restrict__ rep_of_block, const int* __restrict__ deg,
+                                  int* __restrict__ out) {
+  const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (b < K) out[b] = deg[rep_of_block[b]];
+}
+
+// largest b in (b0, K] with prefix[b] - prefix[b0] <= budget (b0 + 1 if even one row exceeds it)
+__global__ void prefix_upper_bound_kernel(const int64_t* __restrict__ prefix, int64_t K, int64_t b0, int64_t budget,
+                                          int64_t* __restrict__ out) {
+  if (blockIdx.x || threadIdx.x) return;
+  const int64_t base = prefix[b0];
+  int64_t lo = b0 + 1, hi = K;  // answer in [lo, hi]
+  while (lo < hi) {
+    const int64_t mid = (lo + hi + 1) >> 1;
+    if (prefix[mid] - base <= budget) lo = mid;
+    else hi = mid - 1;
+  }
+  out[0] = lo;
+  out[1] = prefix[lo] - base;
+}
+
+// which batches hold entries of the representative rows of blocks [b_lo, b_hi): the batch a representative is inner to, or
+// every batch for a boundary representative (need[nb] = 1)
+__global__ void coo_need_kernel(int64_t b_lo, int64_t b_hi, const int* __restrict__ rep_of_block, const int* __restrict__ label,
+                                const int* __restrict__ deg, int nb, int* __restrict__ need) {
+  const int64_t b = b_lo + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (b >= b_hi) return;
+  const int r = rep_of_block[b];
+  if (deg[r] == 0) return;
+  const int lab = label[r];
+  const int slot = lab < 0 ? nb : lab;
+  if (need[slot] == 0) need[slot] = 1;
+}
+
+// quotient, COO form: thread per edge; only entries of representative rows of blocks [b_lo, b_hi) are inserted (Def. 4, Q17)
+__global__ void quot_insert_coo_kernel(int64_t ne, const int* __restrict__ src, const int* __restrict__ col,
+                                       const u32* __restrict__ wt, const int* __restrict__ Hc,
+                                       const int* __restrict__ rep_of_block, int b_lo, int b_hi, Slot* __restrict__ table,
+                                       u64 table_mask, int* __restrict__ cnt) {
+  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < ne; e += stride) {
+    const int s = src[e];
+    const int b = Hc[s];
+    if (b < b_lo || b >= b_hi || rep_of_block[b] != s) continue;
+    if (quot_insert_one(table, table_mask, b, Hc[col[e]], wt ? (u64)wt[e] : 1ull)) atomicAdd(cnt + b, 1);
+  }
+}
+
 // exclusive scan int32 counts -> int64 offsets (3 kernels)
 constexpr int kScanT = 256, kScanI = 8, kScanC = kScanT * kScanI;
 static_assert(kScanC == kScan32Chunk, "wl_refine.cu sizes the scan scratch with kScan32Chunk");
@@ -721,6 +888,7 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
       lo.flags = flags & (WL_FLAG_NO_VALIDATE | WL_FLAG_NO_PRUNE | WL_FLAG_EDGE_BALANCED);
       if (outer > 1) lo.flags |= WL_FLAG_NO_VALIDATE;  // a quotient made by this library is well formed and keeps row sums (L447)
       lo.max_rounds = opt ? opt->max_rounds : 0;
+      lo.ring_bits = opt ? opt->ring_bits : 0;
       lo.stream_id = ((u64)outer << 32) | (u64)(u32)k;
       const Layout L = make_layout(nr, lg.m);
       CoreResult cr{};
@@ -896,6 +1064,7 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
       wl_options lo{};
       lo.flags = (flags & (WL_FLAG_NO_PRUNE | WL_FLAG_EDGE_BALANCED)) | WL_FLAG_NO_VALIDATE;
       lo.max_rounds = opt ? opt->max_rounds : 0;
+      lo.ring_bits = opt ? opt->ring_bits : 0;
       lo.stream_id = ((u64)(outer + 1) << 32) | (u64)(u32)pending.index;
       const Layout L2 = make_layout(nr, pending.tot);
       CoreResult cr{};

@@ -85,7 +85,8 @@ template <bool WEIGHTED>
 __device__ __forceinline__ void
 deep_visit(bool fresh, int i, const int64_t* __restrict__ row_ptr, const int* __restrict__ col,
            const u32* __restrict__ wt, const int* __restrict__ colour, u64 key, u64* __restrict__ y,
-           int* __restrict__ lcount, int* __restrict__ leavers, int* __restrict__ leaver_block, u64* __restrict__ n_leavers) {
+           int* __restrict__ lcount, int* __restrict__ leavers, int* __restrict__ leaver_block, u64* __restrict__ n_leavers,
+           u64 ymask) {
   const int lane = threadIdx.x & 31;
   int64_t a = 0, b = 0;
   if (fresh) {
@@ -116,7 +117,8 @@ deep_visit(bool fresh, int i, const int64_t* __restrict__ row_ptr, const int* __
     for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
     if (lane == src) acc = s;
   }
-  const bool moved = fresh && acc != y[i];
+  acc &= ymask;
+  const bool moved = fresh && acc != (y[i] & ymask);
   const int c = moved ? colour[i] : -1;
   const u64 pos = warp_append(moved, n_leavers);
   if (moved) {
@@ -183,7 +185,8 @@ deep_front_kernel(DeepFinishArgs fin, int do_front, const int* __restrict__ chan
                   const int64_t* __restrict__ row_ptr, const int* __restrict__ col, const u32* __restrict__ wt,
                   int* __restrict__ colour, u64 key, u64* __restrict__ y, int* __restrict__ size, int* __restrict__ lcount,
                   int* __restrict__ leavers, int* __restrict__ leaver_block, u64* __restrict__ n_leavers,
-                  Slot* __restrict__ table, const u32* __restrict__ slots, u64* __restrict__ deep, u64* __restrict__ scal) {
+                  Slot* __restrict__ table, const u32* __restrict__ slots, u64* __restrict__ deep, u64* __restrict__ scal,
+                  u64 ymask) {
   if (blockIdx.x < fin.fin_ctas) {
     deep_finish_part(blockIdx.x, fin.fin_ctas, fin.leavers, fin.leaver_block, colour, size, fin.lcount, table, slots, deep,
                      fin.leavers_slot, fin.consumed_slot, scal, fin.log, fin.log_slot);
@@ -215,7 +218,7 @@ deep_front_kernel(DeepFinishArgs fin, int do_front, const int* __restrict__ chan
         i = tp_src[p];
         fresh = mark[i] != round && atomicExch(mark + i, round) != round;
       }
-      deep_visit<WEIGHTED>(fresh, i, row_ptr, col, wt, colour, key, y, lcount, leavers, leaver_block, n_leavers);
+      deep_visit<WEIGHTED>(fresh, i, row_ptr, col, wt, colour, key, y, lcount, leavers, leaver_block, n_leavers, ymask);
     }
     unsigned big = __ballot_sync(0xffffffffu, !small && sub == 0);
     while (big) {
@@ -229,7 +232,7 @@ deep_front_kernel(DeepFinishArgs fin, int do_front, const int* __restrict__ chan
           i = tp_src[p];
           fresh = mark[i] != round && atomicExch(mark + i, round) != round;
         }
-        deep_visit<WEIGHTED>(fresh, i, row_ptr, col, wt, colour, key, y, lcount, leavers, leaver_block, n_leavers);
+        deep_visit<WEIGHTED>(fresh, i, row_ptr, col, wt, colour, key, y, lcount, leavers, leaver_block, n_leavers, ymask);
       }
     }
   }
@@ -244,7 +247,7 @@ deep_relabel_kernel(const int* __restrict__ leavers, const int* __restrict__ lea
                     int* __restrict__ colour, const u64* __restrict__ y, const int* __restrict__ size,
                     const int* __restrict__ lcount, int* __restrict__ inherit, int round, Slot* __restrict__ table,
                     u32 table_mask, u32* __restrict__ slots, u64* __restrict__ n_slots, const u64* __restrict__ k_ptr,
-                    u64* __restrict__ n_new, int* __restrict__ changed_out, u64* __restrict__ n_changed_out) {
+                    u64* __restrict__ n_new, int* __restrict__ changed_out, u64* __restrict__ n_changed_out, u64 ymask) {
   const int64_t nl = (int64_t)*n_leavers;
   const int k_old = (int)*k_ptr;
   const int64_t stride = (int64_t)gridDim.x * blockDim.x;
@@ -260,7 +263,7 @@ deep_relabel_kernel(const int* __restrict__ leavers, const int* __restrict__ lea
     if (valid) {
       i = leavers[t];
       c = leaver_block[t];
-      const u64 yi = y[i];
+      const u64 yi = y[i] & ymask;
       all_leave = lcount[c] == size[c];  // issued before the probe: independent of it
       const Slot mine = {yi, (u64)(u32)c | ((u64)kPending << 32)};
       const Slot empty = {kEmpty, kEmpty};

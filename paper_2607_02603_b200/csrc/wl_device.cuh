@@ -46,6 +46,12 @@ __host__ __device__ __forceinline__ u64 round_key(u64 seed, u64 stream, u64 roun
 // weight of dense colour id c under `key`
 __host__ __device__ __forceinline__ u64 weight_of(u64 key, u64 c) { return mix64(c + key); }
 
+// The ring is Z/2^q (Alg. 1 "precision parameter q >= 1", L109-L110; L100).  q = 64 unless the caller asks for a smaller ring
+// (wl_options.ring_bits): every z is then reduced to its low q bits wherever it is compared or keyed.  Sums and products commute
+// with the reduction, so masking at the point of use is Algorithm 1 over Z/2^q exactly.  A small q makes the collisions of
+// Lemma 1 (L418) frequent enough to be counted (tests/test_gpu_collisions.py); Theorem 1's guarantee needs q >= 64.
+__host__ __device__ __forceinline__ u64 ring_mask(int q) { return (q <= 0 || q >= 64) ? ~0ull : ((1ull << q) - 1); }
+
 // ---- 128-bit hash slot and its atomics -------------------------------------------------------------------------------
 // slot = { y : 64 | colour : 32 | x : 32 }.  EMPTY = all ones.  x = new dense id once assigned.
 struct __align__(16) Slot {

@@ -645,7 +645,7 @@ relabel_kernel(int64_t count, const int* __restrict__ nodes, int* __restrict__ c
                unsigned short* __restrict__ colour16, const u64* __restrict__ y, int* __restrict__ rep,
                int* __restrict__ stamp, int round, Slot* __restrict__ table, u32 table_mask,
                u32* __restrict__ slot_of, const u64* __restrict__ k_ptr, u64* __restrict__ new_counter,
-               int* __restrict__ changed, u64* __restrict__ n_changed) {
+               int* __restrict__ changed, u64* __restrict__ n_changed, u64 ymask) {
   const int k_old = (int)*k_ptr;  // device-resident colour count: rounds can be queued without a host round trip
   int64_t t = (int64_t)blockIdx.x * kRelabelThreads + threadIdx.x;
   bool win = false, lose = false;
@@ -655,8 +655,8 @@ relabel_kernel(int64_t count, const int* __restrict__ nodes, int* __restrict__ c
     i = nodes ? nodes[t] : (int)t;
     const int c = colour[i];
     const int r = rep[c];
-    const u64 yi = y[i];
-    const u64 yr = y[r];
+    const u64 yi = y[i] & ymask;  // ymask = the ring mask (all ones in the product; all ones for the densify step)
+    const u64 yr = y[r] & ymask;
     if (yi == yr) {
       if (i != r && stamp[c] != round) stamp[c] = round;
     } else {
@@ -725,7 +725,7 @@ round1_uniform_kernel(int64_t n, const int64_t* __restrict__ row_ptr, int64_t ex
                       int* __restrict__ stamp, Slot* __restrict__ table, u32 table_mask, u32* __restrict__ slot_of,
                       u64* __restrict__ new_counter, int64_t hub_threshold, int2* __restrict__ chunks, int64_t hub_cap,
                       u64* __restrict__ hub_counter, int* __restrict__ active, u64* __restrict__ counters,
-                      u64* __restrict__ hub_rows, u32* __restrict__ err) {
+                      u64* __restrict__ hub_rows, u32* __restrict__ err, u64 ymask) {
   constexpr int round = 1, k_old = 1;
   const int64_t t = (int64_t)blockIdx.x * kRelabelThreads + threadIdx.x;
   const bool valid = t < n;
@@ -757,8 +757,8 @@ round1_uniform_kernel(int64_t n, const int64_t* __restrict__ row_ptr, int64_t ex
   bool win = false, lose = false;
   u32 slot = 0, id = 0;
   if (valid) {
-    const u64 yi = (u64)d * w0;
-    if (d == d0) {
+    const u64 yi = ((u64)d * w0) & ymask;
+    if (yi == (((u64)d0 * w0) & ymask)) {
       if (i != 0 && stamp[0] != round) stamp[0] = round;
     } else {
       id = kPending;

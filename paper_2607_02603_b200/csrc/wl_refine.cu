@@ -193,10 +193,10 @@ void launch_hub_collect(const Layout& L, const wl_csr& g, int2* chunks, u64* cou
 // clean == false: the claimed slots stay (the caller empties them with clean_table once it knows the new colour count).
 void launch_relabel(u32 table_mask, int64_t count, const int* nodes, int* colour, unsigned short* colour16, const u64* y,
                     int* rep, int* stamp, int round, Slot* table, u32* slot_of, u64* scal, u64* log, int log_slot,
-                    bool clean, cudaStream_t st, int* changed = nullptr, u64* n_changed = nullptr) {
+                    bool clean, cudaStream_t st, int* changed = nullptr, u64* n_changed = nullptr, u64 ymask = ~0ull) {
   if (count > 0) {
     unsigned grid = blocks_for(count, kRelabelThreads);
-    ++g_launches; relabel_kernel<<<grid, kRelabelThreads, 0, st>>>(count, nodes, colour, colour16, y, rep, stamp, round, table, table_mask, slot_of, scal + kScalK, scal + kScalNew, changed, n_changed);
+    ++g_launches; relabel_kernel<<<grid, kRelabelThreads, 0, st>>>(count, nodes, colour, colour16, y, rep, stamp, round, table, table_mask, slot_of, scal + kScalK, scal + kScalNew, changed, n_changed, ymask);
   }
   const unsigned fgrid = clean ? (unsigned)std::max<int64_t>(1, std::min<int64_t>(blocks_for(count, 256), 148 * 8)) : 1u;
   ++g_launches; relabel_finish_kernel<<<fgrid, 256, 0, st>>>(table, slot_of, scal, log, log_slot, clean ? 1 : 0);
@@ -333,6 +333,7 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
   const uint32_t flags = opt ? opt->flags : 0u;
   const int64_t max_rounds = (opt && opt->max_rounds > 0) ? opt->max_rounds : n + 1;
   const uint64_t stream_id = opt ? opt->stream_id : 0;
+  const u64 ymask = ring_mask(opt ? opt->ring_bits : 0);  // Z/2^q (Alg. 1's precision parameter); all ones for q = 64
   u64* hs = host_scal();
   if (!hs) return check_cuda(cudaErrorMemoryAllocation);
 
@@ -430,7 +431,7 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
     // S0 and round 1 in one pass over row_ptr (round1_uniform_kernel); the loop below only closes the round
     const u64 w0 = weight_of(round_key(seed, stream_id, 1), 0);
     const u32 mask1 = overlap ? (u32)(prefix_slots - 1) : L.table_mask;
-    ++g_launches; round1_uniform_kernel<<<blocks_for(n, kRelabelThreads), kRelabelThreads, 0, st>>>(n, g->row_ptr, edge_first, edge_first + m, w0, colour, colour16, rep, stamp, table, mask1, slot_of, scal + kScalNew, kHubThreshold, hub_chunks, L.hub_cap, scal + kScalHub, act[0], scal + kScalActive, scal + kScalActiveHub, d_err);
+    ++g_launches; round1_uniform_kernel<<<blocks_for(n, kRelabelThreads), kRelabelThreads, 0, st>>>(n, g->row_ptr, edge_first, edge_first + m, w0, colour, colour16, rep, stamp, table, mask1, slot_of, scal + kScalNew, kHubThreshold, hub_chunks, L.hub_cap, scal + kScalHub, act[0], scal + kScalActive, scal + kScalActiveHub, d_err, ymask);
   } else {
     if (!cols_checked) {
       ++g_launches; validate_cols_kernel<<<148 * 8, 256, 0, st>>>(n_targets, edge_first, edge_first + m, g->col_idx, d_err);
@@ -445,7 +446,8 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
   int64_t num_hub_chunks = 0;
   if (!uniform_start) {
     if (init_colors)
-      launch_relabel(L.table_mask, n, nullptr, colour, colour16, y, rep, stamp, /*round=*/0, table, slot_of, scal, nullptr, 0, /*clean=*/false, st);
+      launch_relabel(L.table_mask, n, nullptr, colour, colour16, y, rep, stamp, /*round=*/0, table, slot_of, scal, nullptr, 0, /*clean=*/false, st,
+                     nullptr, nullptr, /*ymask=*/~0ull);  // the key is the caller's label, not a ring element
     cudaMemcpyAsync(hs, scal, sizeof(u64) * kNumScal, cudaMemcpyDeviceToHost, st);
     rc = check_cuda(cudaStreamSynchronize(st));
     if (rc) return rc;
@@ -524,7 +526,7 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
     dirty_mask = mask_r;
     launch_relabel(mask_r, round1_done ? 0 : n_active, cur_list, colour, mirror ? colour16 : nullptr, y, rep, stamp, (int)r, table, slot_of,
                    scal, log, log_slot, clean, st, list_changed ? changed[(r + 1) & 1] : nullptr,
-                   list_changed ? deep + kDeepChanged0 + ((r + 1) & 1) : nullptr);
+                   list_changed ? deep + kDeepChanged0 + ((r + 1) & 1) : nullptr, ymask);
     return streamed;
   };
   // final_test: also drop the blocks whose neighbourhood can no longer change (R5); k_prev = colours before round r
@@ -711,9 +713,9 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
       const unsigned grid = fin.fin_ctas + (do_front ? kDeepGrid : 0);
       ++g_launches;
       if (g->weights)
-        deep_front_kernel<true><<<grid, 256, 0, st>>>(fin, do_front, changed[in], deep + kDeepChanged0 + in, tp_ptr, tp_src, mark, round, g->row_ptr, g->col_idx, g->weights, colour, key, y, size, lcount[in], leavers[in], leaver_block[in], deep + kDeepLeavers0 + in, table, slots, deep, scal);
+        deep_front_kernel<true><<<grid, 256, 0, st>>>(fin, do_front, changed[in], deep + kDeepChanged0 + in, tp_ptr, tp_src, mark, round, g->row_ptr, g->col_idx, g->weights, colour, key, y, size, lcount[in], leavers[in], leaver_block[in], deep + kDeepLeavers0 + in, table, slots, deep, scal, ymask);
       else
-        deep_front_kernel<false><<<grid, 256, 0, st>>>(fin, do_front, changed[in], deep + kDeepChanged0 + in, tp_ptr, tp_src, mark, round, g->row_ptr, g->col_idx, g->weights, colour, key, y, size, lcount[in], leavers[in], leaver_block[in], deep + kDeepLeavers0 + in, table, slots, deep, scal);
+        deep_front_kernel<false><<<grid, 256, 0, st>>>(fin, do_front, changed[in], deep + kDeepChanged0 + in, tp_ptr, tp_src, mark, round, g->row_ptr, g->col_idx, g->weights, colour, key, y, size, lcount[in], leavers[in], leaver_block[in], deep + kDeepLeavers0 + in, table, slots, deep, scal, ymask);
     };
     // the bookkeeping that closes `round` (rides in the launch that opens the next round, or alone at the end of a window)
     auto closing = [&](int round, int log_slot) {
@@ -727,7 +729,7 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
       for (int j = 0; j < R; ++j) {
         const int round = (int)(r + j), in = round & 1, out = (round + 1) & 1;
         front(j == 0 ? DeepFinishArgs{0, nullptr, nullptr, nullptr, 0, 0, 0, nullptr} : closing(round - 1, j - 1), 1, round);
-        ++g_launches; deep_relabel_kernel<<<kDeepGrid, 256, 0, st>>>(leavers[in], leaver_block[in], deep + kDeepLeavers0 + in, colour, y, size, lcount[in], inherit, round, table, L.table_mask, slots, deep + kDeepSlots, scal + kScalK, deep + kDeepNew, changed[out], deep + kDeepChanged0 + out);
+        ++g_launches; deep_relabel_kernel<<<kDeepGrid, 256, 0, st>>>(leavers[in], leaver_block[in], deep + kDeepLeavers0 + in, colour, y, size, lcount[in], inherit, round, table, L.table_mask, slots, deep + kDeepSlots, scal + kScalK, deep + kDeepNew, changed[out], deep + kDeepChanged0 + out, ymask);
       }
       front(closing((int)(r + R - 1), R - 1), 0, (int)(r + R));
       cudaEventRecord(d1, st);
@@ -976,7 +978,8 @@ int wl_relabel(int64_t n, const int32_t* colors, int64_t k, const uint64_t* y, i
   ++g_launches; set_rep_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, new_colors, rep);
   const u64 k_u64 = (u64)k;
   cudaMemcpyAsync(scal + kScalK, &k_u64, sizeof(u64), cudaMemcpyHostToDevice, st);
-  launch_relabel(L.table_mask, n, nullptr, new_colors, nullptr, (const u64*)y, rep, stamp, 1, table, slot_of, scal, nullptr, 0, /*clean=*/false, st);
+  launch_relabel(L.table_mask, n, nullptr, new_colors, nullptr, (const u64*)y, rep, stamp, 1, table, slot_of, scal, nullptr, 0, /*clean=*/false, st,
+                 nullptr, nullptr, /*ymask=*/~0ull);  // the step-level call keys on the exact pairs it is given
   cudaMemcpyAsync(hs, scal, sizeof(u64) * kNumScal, cudaMemcpyDeviceToHost, st);
   int rc = check_cuda(cudaStreamSynchronize(st));
   if (rc) return rc;
@@ -1022,6 +1025,6 @@ const char* wl_strerror(int code) {
 }
 int wl_last_cuda_error(void) { return g_last_cuda_error; }
 int64_t wl_kernel_launches(void) { return g_launches; }
-const char* wl_version(void) { return "wl_refine 0.1 (sm_100a)"; }
+const char* wl_version(void) { return "wl_refine 0.2 (sm_100a)"; }
 
 }  // extern "C"

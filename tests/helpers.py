@@ -73,3 +73,21 @@ def brute_force_coarsest(A, init):
 
 def same_partition(a, b):
     return refines(a, b) and refines(b, a)
+
+
+def classify(got, want):
+    """Reading Q12: RSC separates two nodes only if their z differ, and equal signatures force equal z, so
+    every RSC partition is coarser than or equal to the exact one.  A randomized collision can therefore only show up as
+    "coarser": the exact colouring `want` strictly refines `got`.  Anything else ("other") is a bug, never a collision."""
+    if same_partition(got, want):
+        return "equal"
+    return "coarser" if refines(want, got) else "other"
+
+
+def split_pairs(prev, cur):
+    """N_r of DESIGN.md's union bound: sum over the blocks B of `prev` of C(s_B, 2), s_B = number of blocks of `cur` inside B
+    (the pairs of sub-blocks whose z must differ for the round to be computed exactly)."""
+    prev, cur = np.asarray(prev, dtype=np.int64), np.asarray(cur, dtype=np.int64)
+    pairs = np.unique(np.stack([prev, cur], 1), axis=0)
+    s = np.bincount(pairs[:, 0])
+    return int((s * (s - 1) // 2).sum())
