@@ -376,3 +376,34 @@ def random_edge_batches(g: Graph, num_batches: int, seed: int) -> torch.Tensor:
     """Arbitrary partition (PAPER.md L163 'arbitrary edge partition'): batch id per CSR edge slot."""
     t = torch.arange(g.m, dtype=torch.int64)
     return (hash_u32(seed ^ 0xBA7C4, t) % num_batches).to(torch.int32)
+
+
+def edge_sources(g: Graph) -> torch.Tensor:
+    """Source node of every CSR edge slot (int32[m])."""
+    deg = g.row_ptr[1:] - g.row_ptr[:-1]
+    return torch.repeat_interleave(torch.arange(g.n, dtype=torch.int32, device=g.row_ptr.device), deg)
+
+
+def node_hash_edge_batches(g: Graph, num_batches: int, seed: int, flip_percent: int = 0) -> torch.Tensor:
+    """An arbitrary partition with few boundary nodes: every edge goes to the batch its SOURCE hashes to (all nodes inner,
+    V_k scattered over the id space), then `flip_percent` % of the edges are moved to a hashed batch of their own (their
+    sources become boundary nodes, Def. 5)."""
+    t = torch.arange(g.m, dtype=torch.int64)
+    src = edge_sources(g).to(torch.int64).cpu()
+    eb = hash_u32(seed ^ 0x50DE, src) % num_batches
+    if flip_percent > 0:
+        flip = (hash_u32(seed ^ 0xF11B, t) % 100) < flip_percent
+        eb = torch.where(flip, hash_u32(seed ^ 0xBA7C4, t) % num_batches, eb)
+    return eb.to(torch.int32)
+
+
+def coo_batches(g: Graph, edge_batch: torch.Tensor, num_batches: int):
+    """The edge partition `edge_batch` (batch id per CSR slot) as COO triples (src, col, weights or None) per batch."""
+    src = edge_sources(g).cpu()
+    col = g.col.cpu()
+    out = []
+    for k in range(num_batches):
+        sel = torch.nonzero(edge_batch == k).flatten()
+        out.append((src[sel].contiguous(), col[sel].contiguous(),
+                    None if g.weights is None else g.weights.cpu()[sel].contiguous()))
+    return out

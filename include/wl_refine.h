@@ -156,6 +156,12 @@ uint64_t wl_weight(uint64_t key, uint64_t color);
 int wl_spmv_round(const wl_csr* g, const int32_t* colors, uint64_t key, uint64_t* y, uint32_t flags, void* workspace,
                   size_t workspace_bytes, void* cuda_stream);
 
+/* S1+S2 restricted to an active row list (the pruned rounds, SURVEY.md §8(d) option 6): y[rows[t]] for t < num_rows as in
+ * wl_spmv_round; every other entry of y is left untouched.  rows: DEVICE int32[num_rows], distinct node ids.
+ * flags: WL_FLAG_NARROW_COLORS. */
+int wl_spmv_rows(const wl_csr* g, const int32_t* colors, uint64_t key, const int32_t* rows, int64_t num_rows, uint64_t* y,
+                 uint32_t flags, void* workspace, size_t workspace_bytes, void* cuda_stream);
+
 /* S3+S4: new_colors = dense ids (0..k'-1, unspecified order) of the exact pairs (colors[i], y[i]) (Alg. 1 line 6,
  * L122; Q6).  colors must be dense ids 0..k-1 (k given).  num_colors: HOST, receives k'.  new_colors may alias colors.
  * Blocks that do not split keep their id. */
@@ -175,7 +181,11 @@ int wl_canonicalize(int64_t n, const int32_t* colors, int32_t* out, int64_t* num
  *   CSR-slice form (src == NULL): the batch owns the consecutive CSR edge positions [edge_begin, edge_begin + num_edges) of a
  *     global CSR whose row_ptr (HOST, n + 1 offsets, shared by all batches) is given in every batch; col_idx / weights point at
  *     THIS batch's first entry; or
- *   COO form (src != NULL): arbitrary edges (src[e], col_idx[e]) with optional weights; row_ptr is ignored. */
+ *   COO form (src != NULL): arbitrary edges (src[e], col_idx[e]) with optional weights, num_edges of them, any order;
+ *     row_ptr and edge_begin are ignored.  All batches of a call have the same form.  The first outer iteration then runs
+ *     three streaming passes (inner mask of Def. 5 by the method of L463; local refinement of the gathered rows of V_k;
+ *     quotient by block ranges); later iterations run on the library's own quotient CSR.  Nodes without out-edges are inner
+ *     to batch 0 (Q9).  WL_FLAG_INHERIT_BATCHES is not defined for this form (WL_EINVAL). */
 typedef struct wl_edge_batch {
   int64_t edge_begin;
   int64_t num_edges;
@@ -188,7 +198,7 @@ typedef struct wl_edge_batch {
 /* Stable colouring of (V, A) by Algorithm 2; equals the coarsest one whenever the loop ends with N_b = 1 (L208).
  *   batches          HOST array of num_batches descriptors = the edge partition of outer iteration 1 (Alg. 2 line 5).
  *                    num_batches == 0: `whole` must be given and the library cuts it itself (Q13).
- *   whole            HOST CSR of the full graph, or NULL when batches are given in COO form.
+ *   whole            HOST CSR of the full graph (num_batches == 0), else NULL.
  *   max_batch_edges  M_b (L171): cap on edges per batch for the library's own partitions (later outer iterations, Q14).
  *                    <= 0 (with `whole` and a device cap): the library derives the largest M_b that fits the cap.
  *   device_cap_bytes upper bound on device memory the call may allocate (0 = no cap); WL_ENOMEM if it cannot be met.

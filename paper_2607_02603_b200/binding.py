@@ -27,7 +27,7 @@ WL_FLAG_INHERIT_BATCHES = 4096
 
 EXPORTS = [
     "wl_refine_workspace_bytes", "wl_refine_deep_workspace_bytes", "wl_refine", "wl_refine_host", "wl_round_key", "wl_weight", "wl_spmv_round",
-    "wl_relabel", "wl_canonicalize", "wl_refine_batched", "wl_refine_batched_host_bytes", "wl_inner_labels", "wl_quotient",
+    "wl_spmv_rows", "wl_relabel", "wl_canonicalize", "wl_refine_batched", "wl_refine_batched_host_bytes", "wl_inner_labels", "wl_quotient",
     "wl_quotient_workspace_bytes", "wl_strerror", "wl_last_cuda_error", "wl_version", "wl_kernel_launches",
 ]
 
@@ -93,6 +93,8 @@ def lib():
         L.wl_weight.argtypes = [u64, u64]
         L.wl_spmv_round.restype = C.c_int
         L.wl_spmv_round.argtypes = [C.POINTER(wl_csr), vp, u64, vp, u32, vp, sz, vp]
+        L.wl_spmv_rows.restype = C.c_int
+        L.wl_spmv_rows.argtypes = [C.POINTER(wl_csr), vp, u64, vp, i64, vp, u32, vp, sz, vp]
         L.wl_relabel.restype = C.c_int
         L.wl_relabel.argtypes = [i64, vp, i64, vp, vp, C.POINTER(i64), vp, sz, vp]
         L.wl_canonicalize.restype = C.c_int
@@ -256,6 +258,26 @@ def wl_spmv_round(n, row_ptr, col_idx, weights, colors, key: int, *, flags: int 
     return y
 
 
+def wl_spmv_rows(n, row_ptr, col_idx, weights, colors, key: int, rows: torch.Tensor, y: torch.Tensor, *, flags: int = 0,
+                 workspace=None) -> torch.Tensor:
+    """S1+S2 over an active row list: y[rows] is written, every other entry of y keeps its value.  Returns y."""
+    L = lib()
+    dev = row_ptr.device
+    g, w = _make_csr(n, row_ptr, col_idx, weights, "cuda")
+    _check(colors, torch.int32, "cuda", "colors", n)
+    _check(rows, torch.int32, "cuda", "rows")
+    _check(y, torch.int64, "cuda", "y", n)
+    need = wl_refine_workspace_bytes(n, col_idx.numel())
+    if workspace is None:
+        workspace = torch.empty(max(need, 256), dtype=torch.uint8, device=dev)
+    with torch.cuda.device(dev):
+        rc = L.wl_spmv_rows(C.byref(g), _ptr(colors), key, _ptr(rows), rows.numel(), _ptr(y), flags, _ptr(workspace),
+                            workspace.numel(), _stream_ptr(dev))
+    if rc != WL_OK:
+        raise WlError(rc, "wl_spmv_rows")
+    return y
+
+
 def wl_relabel(colors: torch.Tensor, k: int, y: torch.Tensor, *, workspace=None):
     """S3+S4: dense ids of the exact pairs (colors[i], y[i]).  -> (new_colors, k')."""
     L = lib()
@@ -338,16 +360,23 @@ def wl_quotient(n, row_ptr, col_idx, weights, colors: torch.Tensor, k: int):
 def wl_refine_batched(n: int, row_ptr: torch.Tensor, col_idx: torch.Tensor, weights: Optional[torch.Tensor] = None, *,
                       max_batch_edges: int = 0, cuts=None, seed: int = 0, device_cap_bytes: int = 0, flags: int = 0,
                       max_outer_iters: int = 0, out: Optional[torch.Tensor] = None, device=None,
-                      allow_limit: bool = False, host_workspace: Optional[torch.Tensor] = None) -> RefineResult:
+                      allow_limit: bool = False, host_workspace: Optional[torch.Tensor] = None,
+                      coo_batches=None) -> RefineResult:
     """Algorithm 2 over a HOST-resident CSR (pinned recommended).  cuts (optional, increasing edge positions from 0 to m)
     gives the edge partition of the first outer iteration as consecutive CSR slices; otherwise the library cuts by
     max_batch_edges; max_batch_edges <= 0 (with device_cap_bytes > 0): the library derives M_b from the cap.
+    coo_batches (optional): an ARBITRARY edge partition as a list of (src int32[e], col int32[e],
+    weights or None) host tensors, one triple per batch; row_ptr / col_idx / weights are then ignored (pass None).
     Returns canonical colours on the original nodes (host int32[n])."""
     L = lib()
     if not torch.cuda.is_available():
         raise RuntimeError("wl_refine_batched needs a CUDA device (no CPU fallback)")
     dev = torch.device("cuda", torch.cuda.current_device()) if device is None else torch.device(device)
-    g, w = _make_csr(n, row_ptr, col_idx, weights, "cpu")
+    keep = []
+    if coo_batches is not None:
+        g, w = None, None
+    else:
+        g, w = _make_csr(n, row_ptr, col_idx, weights, "cpu")
     if out is None:
         out = torch.empty(n, dtype=torch.int32)
     _check(out, torch.int32, "cpu", "out", n)
@@ -359,7 +388,24 @@ def wl_refine_batched(n: int, row_ptr: torch.Tensor, col_idx: torch.Tensor, weig
     st = wl_stats()
     nb = 0
     batches = None
-    if cuts is not None:
+    if coo_batches is not None:
+        nb = len(coo_batches)
+        arr = (wl_edge_batch * max(nb, 1))()
+        for k, (bs, bc, bw) in enumerate(coo_batches):
+            _check(bs, torch.int32, "cpu", "coo src")
+            _check(bc, torch.int32, "cpu", "coo col", bs.numel())
+            bw = _as_u32_weights(bw)
+            if bw is not None and (bw.device.type != "cpu" or bw.numel() != bs.numel() or bw.element_size() != 4):
+                raise TypeError("coo weights: expected contiguous 4-byte integers, one per edge")
+            keep.append((bs, bc, bw))
+            arr[k].edge_begin = 0
+            arr[k].num_edges = bs.numel()
+            arr[k].row_ptr = None
+            arr[k].col_idx = bc.data_ptr()
+            arr[k].weights = None if bw is None else bw.data_ptr()
+            arr[k].src = bs.data_ptr()
+        batches = arr
+    elif cuts is not None:
         cuts = [int(c) for c in cuts]
         nb = len(cuts) - 1
         arr = (wl_edge_batch * nb)()
@@ -372,7 +418,7 @@ def wl_refine_batched(n: int, row_ptr: torch.Tensor, col_idx: torch.Tensor, weig
             arr[k].src = None
         batches = arr
     with torch.cuda.device(dev):
-        rc = L.wl_refine_batched(n, nb, batches, C.byref(g) if cuts is None else None, seed, device_cap_bytes,
+        rc = L.wl_refine_batched(n, nb, batches, C.byref(g) if batches is None else None, seed, device_cap_bytes,
                                  max_batch_edges, _ptr(out), C.byref(st), C.byref(opt), _stream_ptr(dev))
     if rc != WL_OK and not (allow_limit and rc == WL_EMAXROUNDS):
         raise WlError(rc, "wl_refine_batched")

@@ -51,6 +51,15 @@ __global__ void merge_kernel(int64_t n_local, const int* __restrict__ local_colo
   if (i < n_local) H[i] = base + local_colour[i];
 }
 
+// every stored target of an uploaded slice must be a node id in [0, n)
+__global__ void slice_cols_check_kernel(int64_t n, int64_t count, const int* __restrict__ col, u32* __restrict__ err) {
+  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  bool bad = false;
+  for (int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; p < count; p += stride)
+    bad |= (unsigned)col[p] >= (unsigned)n;
+  if (bad) atomicOr(err, kErrCol);
+}
+
 __global__ void fill_kernel(int64_t n, int* __restrict__ a, int v) {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i < n) a[i] = v;
@@ -264,9 +273,10 @@ __global__ void coo_rowlen_kernel(int64_t ne, const int* __restrict__ src, int k
     if (label[s] == k) atomicAdd(rowlen + lid[s], 1);
   }
 }
-// ... and entries.  A target inside V_k is renamed to its local index; any other target j becomes ~j (negative), which the
-// RANGED SpMV kernels turn into the implicit singleton id 2^32 + (u32)~j of H_k^0 (Eq. 3): distinct per node and
-// disjoint from the dense ids.  Entry order inside a row is arbitrary (sums in Z/2^64 commute).
+// ... and entries.  A target inside V_k is renamed to its local index; any other target j becomes -2 - j (negative, never the
+// kernels' "no entry" mark -1), which the RANGED SpMV kernels turn into the implicit singleton id 2^32 + (u32)(-2 - j) of
+// H_k^0 (Eq. 3): distinct per node and disjoint from the dense ids.  Entry order inside a row is arbitrary (sums in
+// Z/2^64 commute).
 __global__ void coo_fill_kernel(int64_t ne, const int* __restrict__ src, const int* __restrict__ col,
                                 const u32* __restrict__ wt, int k, const int* __restrict__ label, const int* __restrict__ lid,
                                 const int64_t* __restrict__ lrp, int* __restrict__ cursor, int* __restrict__ lcol,
@@ -277,7 +287,7 @@ __global__ void coo_fill_kernel(int64_t ne, const int* __restrict__ src, const i
     if (label[s] != k) continue;
     const int l = lid[s], c = col[e];
     const int64_t p = lrp[l] + atomicAdd(cursor + l, 1);
-    lcol[p] = label[c] == k ? lid[c] : ~c;
+    lcol[p] = label[c] == k ? lid[c] : -2 - c;
     if (lwt) lwt[p] = wt[e];
   }
 }
@@ -307,6 +317,15 @@ __global__ void coo_boundary_ids_kernel(int64_t n, const int* __restrict__ label
 __global__ void singleton_ids_kernel(int64_t count, const int* __restrict__ nodes, int base, int* __restrict__ H) {
   const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (t < count) H[nodes[t]] = base + (int)t;
+}
+
+__global__ void max_i32_kernel(int64_t n, const int* __restrict__ a, unsigned long long* __restrict__ out) {
+  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  int m = 0;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) m = max(m, a[i]);
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) m = max(m, __shfl_xor_sync(0xffffffffu, m, o));
+  if ((threadIdx.x & 31) == 0 && m > 0) atomicMax(out, (unsigned long long)m);
 }
 
 __global__ void rep_degree_kernel(int64_t K, const int* __restrict__ rep_of_block, const int* __restrict__ deg,
@@ -671,6 +690,341 @@ int wl_quotient(const wl_csr* g, const int32_t* colors, int64_t k, int64_t* q_ro
 // ---------------------------------------------------------------------------------------------------------------------
 }  // extern "C"
 
+
+// ---------------------------------------------------------------------------------------------------------------------
+// First outer iteration of Algorithm 2 for COO-form batches (arbitrary edge partition, Thm 2).  Three streaming passes
+// over the host-resident batches (double-buffered on copy_st):
+//   1. mask    B2: inner labels of Def. 5 by the method of L463 (coo_mask_kernel), out-degrees, validation;
+//   2. local   B3-B5: per batch, the rows of V_k are gathered into a local CSR with targets renamed (coo_fill_kernel), refined
+//              by refine_core(ranged) and merged (Eq. 4); boundary nodes become singletons;
+//   3. quotient B6: block-range major.  The representative rows of an arbitrary partition are scattered over the batches, so
+//              the blocks are cut into ranges whose representative rows fit the device table (by out-degree), and for each
+//              range the batches that hold entries of those rows are streamed again; rows leave in block order, so the host
+//              quotient is the same CSR the CSR-slice path writes.
+// On return *K = number of blocks, d_map0 = canonical block map of the original nodes; unless *stopped (N_b = 1 or K = n:
+// Alg. 2 line 15), the quotient is in hq.rp[1] / hq.col / hq.wt with *q_m entries.
+// ---------------------------------------------------------------------------------------------------------------------
+struct CooStats {
+  int64_t K = 0, q_m = 0, boundary = 0, bytes_h2d = 0, bytes_d2h = 0, edges_streamed = 0, spmv_alg_bytes = 0;
+  double ms_spmv = 0, ms_relabel = 0, ms_spmv_kernel = 0;
+  int32_t spmv_launches = 0;
+  bool stopped = false;
+};
+
+static int coo_first_iteration(int64_t n, int nb, const wl_edge_batch* batches, int64_t m_total, uint64_t seed, uint32_t flags,
+                               const wl_options* opt, size_t cap, size_t* used_persistent, DevBuf& d_map0, HostQuot& hq,
+                               bool build_quotient, cudaStream_t st, cudaStream_t copy_st, cudaStream_t down_st, CooStats* out) {
+  bool weighted = false;
+  for (int k = 0; k < nb; ++k) weighted |= batches[k].num_edges > 0 && batches[k].weights != nullptr;
+  int64_t max_e = 1;
+  for (int k = 0; k < nb; ++k) {
+    const wl_edge_batch& b = batches[k];
+    if (b.num_edges < 0) return WL_EINVAL;
+    if (b.num_edges > 0 && (!b.src || !b.col_idx || (b.weights != nullptr) != weighted)) return WL_EINVAL;
+    max_e = std::max(max_e, b.num_edges);
+  }
+  u64* hs = host_scal();
+  if (!hs) return WL_ECUDA;
+  int rc = WL_OK;
+  size_t used = *used_persistent;
+  cudaEvent_t ev_up[2], ev_done[2], ev_emit[2], ev_down[2], ev_fence;
+  for (int b = 0; b < 2; ++b) {
+    cudaEventCreateWithFlags(&ev_up[b], cudaEventDisableTiming);
+    cudaEventCreateWithFlags(&ev_done[b], cudaEventDisableTiming);
+    cudaEventCreateWithFlags(&ev_emit[b], cudaEventDisableTiming);
+    cudaEventCreateWithFlags(&ev_down[b], cudaEventDisableTiming);
+  }
+  cudaEventCreateWithFlags(&ev_fence, cudaEventDisableTiming);
+  struct EvGuard {
+    cudaEvent_t* e[9];
+    cudaStream_t s[3];
+    ~EvGuard() {
+      for (cudaStream_t q : s) cudaStreamSynchronize(q);
+      for (cudaEvent_t* p : e) cudaEventDestroy(*p);
+    }
+  } guard{{&ev_up[0], &ev_up[1], &ev_done[0], &ev_done[1], &ev_emit[0], &ev_emit[1], &ev_down[0], &ev_down[1], &ev_fence},
+          {st, copy_st, down_st}};
+
+  DevBuf d_label, d_deg, d_rowsum, d_order, d_lid, d_src[2], d_col[2], d_wt[2], d_misc, d_cnts, d_off, d_lcur;
+#define COO_ALLOC(buf, bytes) \
+  if (!rc) rc = buf.alloc((bytes), &used, cap);
+  COO_ALLOC(d_label, sizeof(int) * (size_t)n);
+  COO_ALLOC(d_deg, sizeof(int) * (size_t)n);
+  if (weighted) COO_ALLOC(d_rowsum, sizeof(u64) * (size_t)n);
+  COO_ALLOC(d_order, sizeof(int) * (size_t)n);
+  COO_ALLOC(d_lid, sizeof(int) * (size_t)n);
+  for (int b = 0; b < 2; ++b) {
+    COO_ALLOC(d_src[b], sizeof(int) * (size_t)max_e);
+    COO_ALLOC(d_col[b], sizeof(int) * (size_t)max_e);
+    if (weighted) COO_ALLOC(d_wt[b], sizeof(u32) * (size_t)max_e);
+  }
+  COO_ALLOC(d_misc, 4096);
+  COO_ALLOC(d_cnts, sizeof(u64) * 2 * (size_t)(nb + 1));
+  COO_ALLOC(d_off, sizeof(int64_t) * (size_t)(nb + 1));
+  COO_ALLOC(d_lcur, sizeof(u32) * (size_t)(nb + 1));
+  if (rc) return rc;
+  u32* d_err = (u32*)d_misc.p;                 // validation bits
+  u32* d_bcount = (u32*)d_misc.p + 2;          // boundary-id counter
+  u64* d_total = (u64*)d_misc.p + 8;           // scan totals
+  int64_t* d_ub = (int64_t*)d_misc.p + 16;     // prefix_upper_bound_kernel's two results
+  u64* d_nodes_of = d_cnts.as<u64>();
+  u64* d_edges_of = d_nodes_of + (nb + 1);
+
+  // one batch into buffer `buf` on the copy stream
+  auto upload = [&](int k, int buf, bool with_col_wt) {
+    const wl_edge_batch& b = batches[k];
+    if (b.num_edges > 0) {
+      cudaMemcpyAsync(d_src[buf].p, b.src, sizeof(int) * (size_t)b.num_edges, cudaMemcpyHostToDevice, copy_st);
+      out->bytes_h2d += sizeof(int) * b.num_edges;
+      if (with_col_wt) {
+        cudaMemcpyAsync(d_col[buf].p, b.col_idx, sizeof(int) * (size_t)b.num_edges, cudaMemcpyHostToDevice, copy_st);
+        out->bytes_h2d += sizeof(int) * b.num_edges;
+        if (weighted) {
+          cudaMemcpyAsync(d_wt[buf].p, b.weights, sizeof(u32) * (size_t)b.num_edges, cudaMemcpyHostToDevice, copy_st);
+          out->bytes_h2d += sizeof(u32) * b.num_edges;
+        }
+      }
+    }
+    cudaEventRecord(ev_up[buf], copy_st);
+  };
+  // stream the batches `ks` through the two buffers; body(k, buf) queues the work of batch k on `st`.  sync_each: the body
+  // leaves `st` idle (it synchronises), so no event is needed before a buffer is overwritten.
+  auto stream_batches = [&](const std::vector<int>& ks, auto&& body) -> int {
+    if (ks.empty()) return WL_OK;
+    cudaEventRecord(ev_fence, st);  // everything queued so far may still read the buffers
+    cudaStreamWaitEvent(copy_st, ev_fence, 0);
+    upload(ks[0], 0, true);
+    for (size_t t = 0; t < ks.size(); ++t) {
+      const int buf = (int)(t & 1);
+      if (t + 1 < ks.size()) {
+        if (t >= 1) cudaStreamWaitEvent(copy_st, ev_done[buf ^ 1], 0);
+        upload(ks[t + 1], buf ^ 1, true);
+      }
+      cudaStreamWaitEvent(st, ev_up[buf], 0);
+      const int brc = body(ks[t], buf);
+      cudaEventRecord(ev_done[buf], st);
+      if (brc) return brc;
+    }
+    return WL_OK;
+  };
+  std::vector<int> all(nb);
+  for (int k = 0; k < nb; ++k) all[k] = k;
+
+  // ---- pass 1: B2 -------------------------------------------------------------------------------------------------------
+  ++g_launches; fill_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, d_label.as<int>(), kLabelNone);
+  cudaMemsetAsync(d_deg.p, 0, sizeof(int) * (size_t)n, st);
+  if (weighted) cudaMemsetAsync(d_rowsum.p, 0, sizeof(u64) * (size_t)n, st);
+  cudaMemsetAsync(d_misc.p, 0, 4096, st);
+  cudaMemsetAsync(d_cnts.p, 0, sizeof(u64) * 2 * (size_t)(nb + 1), st);
+  rc = stream_batches(all, [&](int k, int buf) -> int {
+    const int64_t ne = batches[k].num_edges;
+    if (ne > 0) {
+      ++g_launches; coo_mask_kernel<<<(unsigned)std::min<int64_t>(blocks_for(ne, 256), 148 * 16), 256, 0, st>>>(ne, d_src[buf].as<int>(), d_col[buf].as<int>(), weighted ? d_wt[buf].as<u32>() : nullptr, k, n, d_label.as<int>(), d_deg.as<int>(), weighted ? d_rowsum.as<u64>() : nullptr, d_err);
+    }
+    return WL_OK;
+  });
+  if (rc) return rc;
+  ++g_launches; coo_census_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, d_label.as<int>(), d_deg.as<int>(), weighted ? d_rowsum.as<u64>() : nullptr, d_nodes_of, d_edges_of, d_err);
+  std::vector<u64> h_cnts(2 * (size_t)(nb + 1));
+  cudaMemcpyAsync(h_cnts.data(), d_cnts.p, sizeof(u64) * h_cnts.size(), cudaMemcpyDeviceToHost, st);
+  cudaMemcpyAsync(hs, d_misc.p, sizeof(u64), cudaMemcpyDeviceToHost, st);
+  rc = check_cuda(cudaStreamSynchronize(st));
+  if (rc) return rc;
+  {
+    const u32 e = (u32)hs[0];
+    if (e & kErrCol) return WL_EINVAL;
+    if (e & kErrRowSum) return WL_ERANGE;
+  }
+  const u64* h_nodes_of = h_cnts.data();
+  const u64* h_edges_of = h_cnts.data() + (nb + 1);
+  out->boundary = (int64_t)h_nodes_of[0];
+  std::vector<int64_t> off(nb + 1, 0);
+  int64_t max_nl = 1, max_el = 1;
+  for (int k = 0; k < nb; ++k) {
+    off[k + 1] = off[k] + (int64_t)h_nodes_of[k + 1];
+    max_nl = std::max<int64_t>(max_nl, (int64_t)h_nodes_of[k + 1]);
+    max_el = std::max<int64_t>(max_el, (int64_t)h_edges_of[k + 1]);
+  }
+  cudaMemcpyAsync(d_off.p, off.data(), sizeof(int64_t) * (size_t)(nb + 1), cudaMemcpyHostToDevice, st);
+  cudaMemsetAsync(d_lcur.p, 0, sizeof(u32) * (size_t)(nb + 1), st);
+  ++g_launches; coo_order_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, d_label.as<int>(), d_off.as<int64_t>(), d_lcur.as<u32>(), d_order.as<int>(), d_lid.as<int>());
+
+  // ---- pass 2: B3-B5 ----------------------------------------------------------------------------------------------------
+  const int64_t nscan = (n + kCanonChunk - 1) / kCanonChunk;
+  DevBuf d_H, d_Hc, d_first, d_cof, d_bsum, d_ws, d_rowlen, d_lrp, d_lcol, d_lwt, d_sbsum;
+  size_t ws_bytes = 0;
+  for (int k = 0; k < nb; ++k)
+    ws_bytes = std::max(ws_bytes, make_layout((int64_t)h_nodes_of[k + 1], (int64_t)h_edges_of[k + 1]).bytes);
+  COO_ALLOC(d_H, sizeof(int) * (size_t)n);
+  COO_ALLOC(d_Hc, sizeof(int) * (size_t)n);
+  COO_ALLOC(d_first, sizeof(int) * (size_t)n);
+  COO_ALLOC(d_cof, sizeof(int) * (size_t)n);
+  COO_ALLOC(d_bsum, sizeof(int) * (size_t)(nscan + 1));
+  COO_ALLOC(d_ws, ws_bytes);
+  COO_ALLOC(d_rowlen, sizeof(int) * (size_t)max_nl);
+  COO_ALLOC(d_lrp, sizeof(int64_t) * (size_t)(max_nl + 1));
+  COO_ALLOC(d_lcol, sizeof(int) * (size_t)max_el);
+  if (weighted) COO_ALLOC(d_lwt, sizeof(u32) * (size_t)max_el);
+  COO_ALLOC(d_sbsum, sizeof(u64) * (size_t)(max_nl / kScanC + 3));
+  if (rc) return rc;
+  int64_t base_id = 0;
+  rc = stream_batches(all, [&](int k, int buf) -> int {
+    const int64_t ne = batches[k].num_edges, nl = (int64_t)h_nodes_of[k + 1], el = (int64_t)h_edges_of[k + 1];
+    if (nl == 0) return WL_OK;
+    const unsigned egrid = (unsigned)std::max<int64_t>(1, std::min<int64_t>(blocks_for(ne, 256), 148 * 16));
+    cudaMemsetAsync(d_rowlen.p, 0, sizeof(int) * (size_t)nl, st);
+    if (ne > 0) { ++g_launches; coo_rowlen_kernel<<<egrid, 256, 0, st>>>(ne, d_src[buf].as<int>(), k, d_label.as<int>(), d_lid.as<int>(), d_rowlen.as<int>()); }
+    launch_scan32(d_rowlen.as<int>(), nl, 0, d_lrp.as<int64_t>(), d_sbsum.as<u64>(), d_total, st);
+    cudaMemsetAsync(d_rowlen.p, 0, sizeof(int) * (size_t)nl, st);  // now the fill cursor
+    if (ne > 0) { ++g_launches; coo_fill_kernel<<<egrid, 256, 0, st>>>(ne, d_src[buf].as<int>(), d_col[buf].as<int>(), weighted ? d_wt[buf].as<u32>() : nullptr, k, d_label.as<int>(), d_lid.as<int>(), d_lrp.as<int64_t>(), d_rowlen.as<int>(), d_lcol.as<int>(), weighted ? d_lwt.as<u32>() : nullptr); }
+    wl_csr lg;
+    lg.n = nl;
+    lg.m = el;
+    lg.row_ptr = d_lrp.as<int64_t>();
+    lg.col_idx = d_lcol.as<int>();
+    lg.weights = weighted ? d_lwt.as<u32>() : nullptr;
+    wl_options lo{};
+    lo.flags = (flags & (WL_FLAG_NO_PRUNE | WL_FLAG_EDGE_BALANCED)) | WL_FLAG_NO_VALIDATE;  // validated in pass 1
+    lo.max_rounds = opt ? opt->max_rounds : 0;
+    lo.ring_bits = opt ? opt->ring_bits : 0;
+    lo.stream_id = (1ull << 32) | (u64)(u32)k;
+    const Layout L = make_layout(nl, el);
+    CoreResult cr{};
+    const int prc = refine_core(&lg, nullptr, seed, &lo, /*ranged=*/true, 0, (int)nl, n, 0, d_ws.p, L.bytes, L, st, &cr);
+    if (prc) return prc;
+    ++g_launches; coo_merge_kernel<<<blocks_for(nl, 256), 256, 0, st>>>(nl, d_order.as<int>() + off[k], cr.colour, (int)base_id, d_H.as<int>());
+    base_id += cr.k;
+    out->edges_streamed += cr.edges_streamed;
+    out->ms_spmv += cr.ms_spmv;
+    out->ms_relabel += cr.ms_relabel;
+    out->ms_spmv_kernel += cr.ms_spmv_kernel;
+    out->spmv_alg_bytes += cr.spmv_alg_bytes;
+    out->spmv_launches += cr.spmv_launches;
+    return check_cuda(cudaStreamSynchronize(st));  // the workspace and the local CSR are reused by the next batch
+  });
+  if (rc) return rc;
+  if (out->boundary > 0) {
+    ++g_launches; coo_boundary_ids_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, d_label.as<int>(), (int)base_id, d_bcount, d_H.as<int>());
+    base_id += out->boundary;
+  }
+  Layout Lc{};
+  Lc.nscan = nscan;
+  launch_canonical(Lc, n, d_H.as<int>(), d_Hc.as<int>(), d_first.as<int>(), d_cof.as<int>(), d_bsum.as<int>(), d_total, st);
+  cudaMemcpyAsync(hs, d_total, sizeof(u64), cudaMemcpyDeviceToHost, st);
+  rc = check_cuda(cudaStreamSynchronize(st));
+  if (rc) return rc;
+  const int64_t K = (int64_t)hs[0];
+  out->K = K;
+  if ((rc = d_map0.alloc(sizeof(int) * (size_t)n, used_persistent, cap))) return rc;
+  used += d_map0.bytes;
+  cudaMemcpyAsync(d_map0.p, d_Hc.p, sizeof(int) * (size_t)n, cudaMemcpyDeviceToDevice, st);
+  out->stopped = (nb == 1) || (K == n) || !build_quotient;
+  if (out->stopped) return check_cuda(cudaStreamSynchronize(st));
+
+  // ---- pass 3: B6, block-range major --------------------------------------------------------------------------------------
+  cudaStreamSynchronize(st);
+  d_H.release(&used);
+  d_first.release(&used);
+  d_cof.release(&used);
+  d_ws.release(&used);
+  d_rowlen.release(&used);
+  d_lrp.release(&used);
+  d_lcol.release(&used);
+  d_lwt.release(&used);
+  d_order.release(&used);
+  d_lid.release(&used);
+  if ((rc = hq.init(n, m_total, opt ? opt->host_workspace : nullptr, opt ? opt->host_workspace_bytes : 0))) return rc;
+  int64_t* nrp = hq.rp[1];
+  DevBuf d_rep, d_cnt, d_cursor, d_qrp, d_prefix, d_qtab, d_qcol[2], d_qwt[2], d_sb2, d_need;
+  COO_ALLOC(d_rep, sizeof(int) * (size_t)K);
+  COO_ALLOC(d_cnt, sizeof(int) * (size_t)K);
+  COO_ALLOC(d_cursor, sizeof(int) * (size_t)K);
+  COO_ALLOC(d_qrp, sizeof(int64_t) * (size_t)(K + 1));
+  COO_ALLOC(d_prefix, sizeof(int64_t) * (size_t)(K + 1));
+  COO_ALLOC(d_sb2, sizeof(u64) * (size_t)((K + kScanC - 1) / kScanC + 2));
+  COO_ALLOC(d_need, sizeof(int) * (size_t)(nb + 1));
+  if (rc) return rc;
+  ++g_launches; fill_kernel<<<blocks_for(K, 256), 256, 0, st>>>(K, d_rep.as<int>(), kNoNode);
+  ++g_launches; block_rep_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, d_Hc.as<int>(), d_rep.as<int>());
+  ++g_launches; rep_degree_kernel<<<blocks_for(K, 256), 256, 0, st>>>(K, d_rep.as<int>(), d_deg.as<int>(), d_cnt.as<int>());
+  launch_scan32(d_cnt.as<int>(), K, 0, d_prefix.as<int64_t>(), d_sb2.as<u64>(), d_total, st);
+  cudaMemsetAsync(d_cnt.p, 0, sizeof(int) * (size_t)K, st);
+  cudaMemsetAsync(d_cursor.p, 0, sizeof(int) * (size_t)K, st);
+  int64_t max_deg = 0;
+  // out_cap: entries one range may hold = max(largest batch, longest row): a range always holds at least one whole row
+  {
+    int64_t* d_max = d_ub + 4;
+    cudaMemsetAsync(d_max, 0, sizeof(int64_t), st);
+    ++g_launches; max_i32_kernel<<<(unsigned)std::max<int64_t>(1, std::min<int64_t>(blocks_for(n, 256), 148 * 8)), 256, 0, st>>>(n, d_deg.as<int>(), (unsigned long long*)d_max);
+    cudaMemcpyAsync(hs, d_max, sizeof(int64_t), cudaMemcpyDeviceToHost, st);
+    rc = check_cuda(cudaStreamSynchronize(st));
+    if (rc) return rc;
+    max_deg = (int64_t)hs[0];
+  }
+  const int64_t out_cap = std::max<int64_t>(max_e, max_deg);
+  const u64 qslots = quot_table_slots(out_cap);
+  COO_ALLOC(d_qtab, sizeof(u64) * 2 * qslots);
+  for (int b = 0; b < 2; ++b) {
+    COO_ALLOC(d_qcol[b], sizeof(int) * (size_t)out_cap);
+    COO_ALLOC(d_qwt[b], sizeof(u32) * (size_t)out_cap);
+  }
+  if (rc) return rc;
+  cudaMemsetAsync(d_qtab.p, 0, sizeof(u64) * 2 * qslots, st);
+  int64_t q_off = 0, b0 = 0;
+  int n_emit = 0;
+  std::vector<int> h_need(nb + 1);
+  while (b0 < K) {
+    ++g_launches; prefix_upper_bound_kernel<<<1, 1, 0, st>>>(d_prefix.as<int64_t>(), K, b0, out_cap, d_ub);
+    cudaMemcpyAsync(hs, d_ub, 2 * sizeof(int64_t), cudaMemcpyDeviceToHost, st);
+    rc = check_cuda(cudaStreamSynchronize(st));
+    if (rc) return rc;
+    const int64_t b1 = (int64_t)hs[0];
+    cudaMemsetAsync(d_need.p, 0, sizeof(int) * (size_t)(nb + 1), st);
+    ++g_launches; coo_need_kernel<<<blocks_for(b1 - b0, 256), 256, 0, st>>>(b0, b1, d_rep.as<int>(), d_label.as<int>(), d_deg.as<int>(), nb, d_need.as<int>());
+    cudaMemcpyAsync(h_need.data(), d_need.p, sizeof(int) * (size_t)(nb + 1), cudaMemcpyDeviceToHost, st);
+    rc = check_cuda(cudaStreamSynchronize(st));
+    if (rc) return rc;
+    std::vector<int> ks;
+    for (int k = 0; k < nb; ++k)
+      if ((h_need[k] || h_need[nb]) && batches[k].num_edges > 0) ks.push_back(k);
+    rc = stream_batches(ks, [&](int k, int buf) -> int {
+      const int64_t ne = batches[k].num_edges;
+      ++g_launches; quot_insert_coo_kernel<<<(unsigned)std::min<int64_t>(blocks_for(ne, 256), 148 * 16), 256, 0, st>>>(ne, d_src[buf].as<int>(), d_col[buf].as<int>(), weighted ? d_wt[buf].as<u32>() : nullptr, d_Hc.as<int>(), d_rep.as<int>(), (int)b0, (int)b1, (Slot*)d_qtab.p, qslots - 1, d_cnt.as<int>());
+      return WL_OK;
+    });
+    if (rc) return rc;
+    launch_scan32(d_cnt.as<int>() + b0, b1 - b0, q_off, d_qrp.as<int64_t>() + b0, d_sb2.as<u64>(), d_total, st);
+    cudaMemcpyAsync(hs, d_total, sizeof(u64), cudaMemcpyDeviceToHost, st);
+    rc = check_cuda(cudaStreamSynchronize(st));
+    if (rc) return rc;
+    const int64_t tot = (int64_t)hs[0];
+    if (tot > out_cap || q_off + tot > hq.cap_edges || b1 > hq.cap_nodes) return WL_ECUDA;  // unreachable (Def. 4)
+    const int ob = n_emit & 1;
+    if (n_emit >= 2) cudaStreamWaitEvent(st, ev_down[ob], 0);
+    ++n_emit;
+    ++g_launches; quot_emit_kernel<<<blocks_for((int64_t)qslots, 256), 256, 0, st>>>(d_qtab.as<u64>(), qslots, d_qrp.as<int64_t>(), q_off, d_cursor.as<int>(), d_qcol[ob].as<int>(), d_qwt[ob].as<u32>(), (int)b0, (int)b1);
+    cudaEventRecord(ev_emit[ob], st);
+    cudaStreamWaitEvent(down_st, ev_emit[ob], 0);
+    if (tot) {
+      cudaMemcpyAsync(hq.col + q_off, d_qcol[ob].p, sizeof(int) * (size_t)tot, cudaMemcpyDeviceToHost, down_st);
+      cudaMemcpyAsync(hq.wt + q_off, d_qwt[ob].p, sizeof(u32) * (size_t)tot, cudaMemcpyDeviceToHost, down_st);
+      out->bytes_d2h += (sizeof(int) + sizeof(u32)) * tot;
+    }
+    cudaMemcpyAsync(nrp + b0, d_qrp.as<int64_t>() + b0, sizeof(int64_t) * (size_t)(b1 - b0 + 1), cudaMemcpyDeviceToHost, down_st);
+    out->bytes_d2h += sizeof(int64_t) * (b1 - b0 + 1);
+    cudaEventRecord(ev_down[ob], down_st);
+    q_off += tot;
+    b0 = b1;
+  }
+  rc = check_cuda(cudaStreamSynchronize(down_st));
+  if (!rc) rc = check_cuda(cudaStreamSynchronize(st));
+  if (rc) return rc;
+  nrp[(size_t)K] = q_off;
+  out->q_m = q_off;
+  return WL_OK;
+#undef COO_ALLOC
+}
+
 // Algorithm 2 for a given M_b (the exported entry point below picks M_b from the device cap when the caller gives none)
 static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batches, const wl_csr* whole, uint64_t seed,
                        size_t device_cap_bytes, int64_t max_batch_edges, int32_t* out_colors, wl_stats* stats,
@@ -689,16 +1043,32 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
   const int* col = nullptr;
   const u32* wt = nullptr;
   std::vector<int64_t> cuts;
-  if (num_batches > 0) {
+  // COO form = arbitrary edge partition (Thm 2): some batch names its sources and none gives CSR offsets (an empty batch
+  // may leave all its pointers NULL)
+  bool coo = false;
+  for (int k = 0; k < num_batches && batches; ++k) coo |= batches[k].src != nullptr;
+  if (!coo && num_batches > 0 && batches) {
+    bool all_empty = true;
+    for (int k = 0; k < num_batches; ++k) all_empty &= batches[k].num_edges == 0 && !batches[k].row_ptr;
+    coo = all_empty;  // no edges at all and no offsets: every node is a sink
+  }
+  int64_t coo_edges = 0;
+  if (coo) {
+    if (flags & WL_FLAG_INHERIT_BATCHES) return WL_EINVAL;  // Q14b is defined for row-contiguous partitions only
+    for (int k = 0; k < num_batches; ++k) {
+      if (batches[k].num_edges < 0 || (batches[k].num_edges > 0 && !batches[k].src)) return WL_EINVAL;  // the forms do not mix
+      coo_edges += batches[k].num_edges;
+    }
+  } else if (num_batches > 0) {
     if (!batches) return WL_EINVAL;
-    // CSR-slice form only: all batches share one row_ptr and tile the edge array consecutively
+    // CSR-slice form: all batches share one row_ptr and tile the edge array consecutively
     rp = batches[0].row_ptr;
     if (!rp) return WL_EINVAL;
     int64_t pos = 0;
     cuts.push_back(0);
     for (int k = 0; k < num_batches; ++k) {
       const wl_edge_batch& b = batches[k];
-      if (b.src) return WL_EINVAL;  // COO-form partitions: not supported yet
+      if (b.src) return WL_EINVAL;  // the two forms do not mix
       if (b.row_ptr != rp || b.edge_begin != pos || b.num_edges < 0) return WL_EINVAL;
       if (b.num_edges > 0 && !b.col_idx) return WL_EINVAL;
       pos += b.num_edges;
@@ -721,6 +1091,15 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
     return num_batches > 0 ? batches[k].weights : (wt ? wt + cuts[k] : nullptr);
   };
   bool weighted = num_batches > 0 ? (batches[0].weights != nullptr) : (wt != nullptr);
+  // S0 on the host side of the CSR forms: the offsets steer the cuts, the inner ranges and every upload size
+  if (!coo && !(flags & WL_FLAG_NO_VALIDATE)) {
+    if (rp[0] != 0) return WL_EINVAL;
+    for (int64_t i = 0; i < n; ++i) {
+      const int64_t d = rp[i + 1] - rp[i];
+      if (d < 0) return WL_EINVAL;
+      if ((u64)d >= (1ull << 32)) return WL_ERANGE;
+    }
+  }
 
   u64* hs = host_scal();
   if (!hs) return WL_ECUDA;
@@ -769,7 +1148,7 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
   DevBuf d_map0;  // original node -> node of the current graph (identity in iteration 1: left unallocated until needed)
   bool map0_identity = true;
   HostQuot hq;  // quotient graphs of later iterations (pinned host memory)
-  const int64_t rp0_edges = rp[n];
+  const int64_t rp0_edges = coo ? coo_edges : rp[n];
 
   int64_t n_t = n;
   int outer = 0;
@@ -798,7 +1177,45 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
     std::fprintf(stderr, "[wl_refine_batched] outer %d %-22s %9.3f ms\n", outer, what, 1e3 * (t - t_mark));
     t_mark = t;
   };
-  while (true) {
+  // COO-form batches: the first outer iteration has its own three-pass driver; its quotient is an ordinary host CSR, so
+  // the loop below takes over from iteration 2
+  bool loop_done = false;
+  if (coo) {
+    outer = 1;
+    CooStats cs;
+    rc = coo_first_iteration(n, num_batches, batches, coo_edges, seed, flags, opt, device_cap_bytes, &used, d_map0, hq,
+                             /*build_quotient=*/max_outer > 1, st, copy_st, down_st, &cs);
+    edges_streamed += cs.edges_streamed;
+    bytes_h2d += cs.bytes_h2d;
+    bytes_d2h += cs.bytes_d2h;
+    ms_spmv += cs.ms_spmv;
+    ms_relabel += cs.ms_relabel;
+    ms_spmv_kernel += cs.ms_spmv_kernel;
+    spmv_alg_bytes += cs.spmv_alg_bytes;
+    spmv_launches += cs.spmv_launches;
+    if (rc) {
+      loop_done = true;
+    } else {
+      map0_identity = false;
+      nb_last = num_batches;
+      K_final = cs.K;
+      boundary_first = cs.boundary;
+      if (cs.stopped) {
+        loop_done = true;
+        hit_limit = !(num_batches == 1 || cs.K == n);  // stopped by max_outer_iters only
+      } else {
+        rp = hq.rp[1];
+        n_t = cs.K;
+        weighted = true;
+        std::vector<int64_t> next_cuts;
+        greedy_cuts(n_t, rp, max_batch_edges, next_cuts);
+        if ((flags & WL_FLAG_AGGRESSIVE_STOP) && (int64_t)next_cuts.size() - 1 >= num_batches) loop_done = true;  // L328
+        else cuts.swap(next_cuts);
+      }
+    }
+    phase("COO first iteration");
+  }
+  while (!loop_done) {
     ++outer;
     const int nb = (int)cuts.size() - 1;
     // inner ranges and sizes
@@ -847,6 +1264,7 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
     }
     WL_ALLOC(d_misc, 4096);
     if (rc) break;
+    cudaMemsetAsync(d_misc.p, 0, 4096, st);
 
     auto upload_batch = [&](int k, int buf) {
       const int64_t c0 = cuts[k], c1 = cuts[k + 1];
@@ -876,6 +1294,11 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
       if (k + 1 < nb) upload_batch(k + 1, buf ^ 1);
       cudaStreamWaitEvent(st, ev_up[buf], 0);
       const int64_t nr = r1[k] - r0[k];
+      if (outer == 1 && !(flags & WL_FLAG_NO_VALIDATE) && cuts[k + 1] > cuts[k]) {
+        // S0 for the entries outside the inner rows (rows cut by a batch border are never seen by refine_core, yet the
+        // quotient pass maps every stored target through the block map): range check of the WHOLE uploaded slice
+        ++g_launches; slice_cols_check_kernel<<<148 * 8, 256, 0, st>>>(n_t, cuts[k + 1] - cuts[k], d_col[buf].as<int>(), (u32*)d_misc.p + 64);
+      }
       if (nr == 0) continue;
       const int64_t e0 = rp[r0[k]], e1 = rp[r1[k]];
       wl_csr lg;
@@ -905,6 +1328,31 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
       rc = check_cuda(cudaStreamSynchronize(st));  // the workspace and this buffer are reused by the next batch
     }
     if (rc) break;
+    if (outer == 1 && !(flags & WL_FLAG_NO_VALIDATE)) {
+      cudaMemcpyAsync(hs + kNumScal + 2, (u32*)d_misc.p + 64, sizeof(u32), cudaMemcpyDeviceToHost, st);
+      rc = check_cuda(cudaStreamSynchronize(st));
+      if (rc) break;
+      if ((u32)hs[kNumScal + 2] & kErrCol) {
+        rc = WL_EINVAL;
+        break;
+      }
+      // row sums of the rows cut by a batch border (Theorem 1's precondition, L129): at most nb - 1 rows, summed on the host
+      // from the caller's weight arrays (refine_core checks the inner rows on the device)
+      if (weighted) {
+        for (int k = 1; k < nb && !rc; ++k) {
+          const int64_t r = (std::upper_bound(rp, rp + n_t + 1, cuts[k]) - rp) - 1;
+          if (r < 0 || r >= n_t || rp[r] >= cuts[k]) continue;  // the cut falls on a row boundary
+          u64 sum = 0;
+          for (int j = 0; j < nb; ++j) {
+            const int64_t a = std::max(rp[r], cuts[j]), b = std::min(rp[r + 1], cuts[j + 1]);
+            const u32* w = batch_wt(j);
+            for (int64_t p = a; p < b; ++p) sum += w[p - cuts[j]];
+          }
+          if (sum >= (1ull << 32)) rc = WL_ERANGE;
+        }
+        if (rc) break;
+      }
+    }
     phase("local refinement");
     // ---- Alg. 2 lines 11-12: boundary nodes become singletons ---------------------------------------------------------
     std::vector<int> bnodes, bids;
@@ -918,8 +1366,15 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
         }
         if (k < nb) next = r1[k];
       }
-      for (size_t j = 0; j < bnodes.size(); ++j)
-        cudaMemcpyAsync(d_H.as<int>() + bnodes[j], &bids[j], sizeof(int), cudaMemcpyHostToDevice, st);
+      if (!bnodes.empty()) {  // one upload of the node list, one kernel (ids are consecutive from bids[0])
+        DevBuf d_bn;
+        if ((rc = d_bn.alloc(sizeof(int) * bnodes.size(), &used_iter, device_cap_bytes))) break;
+        cudaMemcpyAsync(d_bn.p, bnodes.data(), sizeof(int) * bnodes.size(), cudaMemcpyHostToDevice, st);
+        bytes_h2d += sizeof(int) * bnodes.size();
+        ++g_launches; singleton_ids_kernel<<<blocks_for((int64_t)bnodes.size(), 256), 256, 0, st>>>((int64_t)bnodes.size(), d_bn.as<int>(), bids[0], d_H.as<int>());
+        cudaStreamSynchronize(st);  // bnodes is pageable and d_bn dies with this scope
+        d_bn.release(&used_iter);
+      }
       if (outer == 1) boundary_first = (int64_t)bnodes.size();
     }
     // canonical block map of this iteration (first-occurrence ids keep the composed map canonical)

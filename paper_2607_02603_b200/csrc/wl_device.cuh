@@ -25,6 +25,9 @@ enum {
   kNumScal = 64
 };
 
+// error bits written by device-side validation
+constexpr u32 kErrRowPtr = 1u, kErrCol = 2u, kErrRowSum = 4u, kErrInit = 8u;
+
 // ---- weight bijection (readings Q4/Q5; Alg. 1 lines 3-4) -------------------------------
 // mix is a bijection of Z/2^64: xor-shifts and odd multipliers are invertible.  M1/M2/G are
 // floor(frac(sqrt 2) 2^64)|1, floor(frac(sqrt 3) 2^64)|1, floor(frac(golden ratio) 2^64)|1.

@@ -12,8 +12,6 @@ constexpr int kHubChunk = 4096;  // entries per CTA of spmv_hub_kernel
 constexpr int kHubThreads = 256;
 constexpr u32 kWinBit = 0x80000000u;
 
-// error bits written by device-side validation
-constexpr u32 kErrRowPtr = 1u, kErrCol = 2u, kErrRowSum = 4u, kErrInit = 8u;
 
 // ---------------------------------------------------------------------------------------------------------------------
 // S0: validation of the CSR (WL_EINVAL / WL_ERANGE conditions of include/wl_refine.h)
@@ -222,7 +220,7 @@ spmv_rows32_kernel(int64_t nrows, const int* __restrict__ rows, const int64_t* _
     for (int t = 0; t < kSmallRow; ++t) cidx[t] = t < dd ? checked_col<VALIDATE>(__ldg(col + a + t), n_targets, bad) : -1;
 #pragma unroll
     for (int t = 0; t < kSmallRow; ++t) {
-      if (cidx[t] >= 0) {
+      if (cidx[t] != -1) {  // -1 = no entry; other negative values are renamed outside targets (RANGED, wl_batched.cu)
         u64 v = weight_of(key, colour_id<RANGED>(colour, cidx[t], lo, hi));
         if (WEIGHTED) v *= (u64)__ldg(wt + a + t);
         acc += v;
@@ -252,7 +250,7 @@ spmv_rows32_kernel(int64_t nrows, const int* __restrict__ rows, const int64_t* _
       u64 s = 0;
 #pragma unroll
       for (int t = 0; t < kMidRow / 8; ++t) {
-        if (c[t] >= 0) {
+        if (c[t] != -1) {
           u64 v = weight_of(key, colour_id<RANGED>(colour, c[t], lo, hi));
           if (WEIGHTED) v *= (u64)ld_stream_u32(wt + ra + sub + 8 * t);
           s += v;
@@ -299,7 +297,7 @@ spmv_rows32_kernel(int64_t nrows, const int* __restrict__ rows, const int64_t* _
         c[t] = p + 32 * t < rb ? checked_col<VALIDATE>(ld_stream_i32(col + p + 32 * t), n_targets, bad) : -1;
 #pragma unroll
       for (int t = 0; t < 4; ++t) {
-        if (c[t] >= 0) {
+        if (c[t] != -1) {
           u64 v = weight_of(key, colour_id<RANGED>(colour, c[t], lo, hi));
           if (WEIGHTED) v *= (u64)ld_stream_u32(wt + p + 32 * t);
           s += v;
@@ -326,6 +324,19 @@ __global__ void hub_collect_kernel(int64_t n, const int64_t* __restrict__ row_pt
   const int nc = (int)((d + kHubChunk - 1) / kHubChunk);
   const u64 base = atomicAdd(counter, (u64)nc);
   for (int c = 0; c < nc; ++c) chunks[base + c] = make_int2((int)i, c);
+}
+
+// the same for the rows of a list (wl_spmv_rows)
+__global__ void hub_collect_rows_kernel(int64_t nrows, const int* __restrict__ rows, const int64_t* __restrict__ row_ptr,
+                                        int64_t hub_threshold, int2* __restrict__ chunks, u64* __restrict__ counter) {
+  int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= nrows) return;
+  const int i = rows[t];
+  const int64_t d = row_ptr[i + 1] - row_ptr[i];
+  if (d <= hub_threshold) return;
+  const int nc = (int)((d + kHubChunk - 1) / kHubChunk);
+  const u64 base = atomicAdd(counter, (u64)nc);
+  for (int c = 0; c < nc; ++c) chunks[base + c] = make_int2(i, c);
 }
 
 // active == NULL: every hub row; else only rows whose block is still splittable (stamp[colour[row]] == live_stamp)
@@ -446,11 +457,11 @@ spmv_eb_kernel(int64_t n, const int64_t* __restrict__ row_ptr, const int* __rest
     }
     u64 v[kEbU];
 #pragma unroll
-    for (int t = 0; t < kEbU; ++t) v[t] = ci[t] >= 0 ? colour_id<RANGED>(colour, ci[t], lo, hi) : 0ull;
+    for (int t = 0; t < kEbU; ++t) v[t] = ci[t] != -1 ? colour_id<RANGED>(colour, ci[t], lo, hi) : 0ull;
 #pragma unroll
     for (int t = 0; t < kEbU; ++t) {
-      v[t] = ci[t] >= 0 ? weight_of(key, v[t]) : 0ull;
-      if (WEIGHTED) v[t] *= ci[t] >= 0 ? (u64)ld_stream_u32(wt + Es + 32 * t + lane) : 0ull;
+      v[t] = ci[t] != -1 ? weight_of(key, v[t]) : 0ull;
+      if (WEIGHTED) v[t] *= ci[t] != -1 ? (u64)ld_stream_u32(wt + Es + 32 * t + lane) : 0ull;
     }
     // row ends inside the sub-chunk, one per lane (row_ptr is non-decreasing: the lanes that have one form a prefix)
     int64_t r = r_open + lane;

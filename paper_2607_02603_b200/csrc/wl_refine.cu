@@ -950,6 +950,36 @@ int wl_spmv_round(const wl_csr* g, const int32_t* colors, uint64_t key, uint64_t
   return check_cuda(cudaGetLastError());
 }
 
+int wl_spmv_rows(const wl_csr* g, const int32_t* colors, uint64_t key, const int32_t* rows, int64_t num_rows, uint64_t* y,
+                 uint32_t flags, void* workspace, size_t workspace_bytes, void* cuda_stream) {
+  int rc = basic_csr_check(g);
+  if (rc) return rc;
+  if (num_rows < 0 || num_rows > g->n) return WL_EINVAL;
+  if (g->n == 0 || num_rows == 0) return WL_OK;
+  if (!colors || !y || !workspace || !rows) return WL_EINVAL;
+  const Layout L = make_layout(g->n, g->m);
+  if (workspace_bytes < L.bytes) return WL_ENOMEM;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  char* ws = (char*)workspace;
+  u64* scal = (u64*)(ws + L.o_scal);
+  u64* hs = host_scal();
+  if (!hs) return WL_ECUDA;
+  const bool narrow = (flags & WL_FLAG_NARROW_COLORS) != 0;
+  int2* chunks = (int2*)(ws + L.o_hub);
+  cudaMemsetAsync(scal, 0, sizeof(u64) * kNumScal, st);
+  ++g_launches; hub_collect_rows_kernel<<<blocks_for(num_rows, 256), 256, 0, st>>>(num_rows, rows, g->row_ptr, kHubThreshold, chunks, scal + kScalHub);
+  cudaMemcpyAsync(hs, scal, sizeof(u64) * kNumScal, cudaMemcpyDeviceToHost, st);
+  rc = check_cuda(cudaStreamSynchronize(st));
+  if (rc) return rc;
+  if (narrow) { ++g_launches; narrow_kernel<<<blocks_for(g->n, 256), 256, 0, st>>>(g->n, colors, (unsigned short*)(ws + L.o_colour16)); }
+  SpmvArgs a{rows, num_rows, colors, (unsigned short*)(ws + L.o_colour16), narrow, chunks, (int64_t)hs[kScalHub], nullptr, 0,
+             false, 0, 0};
+  launch_spmv(L, *g, a, key, nullptr, (u64*)y, /*merge=*/false, st);
+  rc = check_cuda(cudaStreamSynchronize(st));
+  if (rc) return rc;
+  return check_cuda(cudaGetLastError());
+}
+
 int wl_relabel(int64_t n, const int32_t* colors, int64_t k, const uint64_t* y, int32_t* new_colors, int64_t* num_colors,
                void* workspace, size_t workspace_bytes, void* cuda_stream) {
   if (n < 0 || k < 0 || k > n) return WL_EINVAL;

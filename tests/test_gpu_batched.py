@@ -149,6 +149,86 @@ def test_batched_aggressive_stop_equals_cpu_algorithm2(name, nb, inherit):
     assert refines(got, full.colors.numpy()) and res.stats["outer_iters"] <= full.stats["outer_iters"]
 
 
+# ------------------------------------------------------------------ arbitrary (COO) edge partitions, Thm 2
+COO_PARTITIONS = {
+    "random_edges": lambda g, nb, seed: gg.random_edge_batches(g, nb, seed),          # nearly every node is a boundary node
+    "by_source": lambda g, nb, seed: gg.node_hash_edge_batches(g, nb, seed),          # all inner, V_k scattered
+    "by_source_flip5": lambda g, nb, seed: gg.node_hash_edge_batches(g, nb, seed, 5),  # some boundary nodes, several iterations
+}
+
+
+@pytest.mark.parametrize("name", list(BATCH_GRAPHS))
+@pytest.mark.parametrize("nb", [2, 3, 4])
+@pytest.mark.parametrize("part", list(COO_PARTITIONS))
+def test_batched_coo_partitions_equal_cpu_algorithm2(name, nb, part):
+    """wl_refine_batched over an ARBITRARY edge partition given as COO batches: bit-exact against the CPU Algorithm 2 run on
+    the same per-edge batch labels (oracle.rbsc(first_edge_batch=...)), Theorem 2 stability, refinement of the coarsest
+    colouring, and invariance under renumbering the batches (L213)."""
+    g = BATCH_GRAPHS[name]()
+    n, rp, ci, wt = g.numpy()
+    eb = COO_PARTITIONS[part](g, nb, 7)
+    cap = max(1, -(-g.m // nb))
+    coarsest, _, _ = oracle.refine(n, rp, ci, wt)
+    want, k_want, outer_want, nbl_want = oracle.rbsc(n, rp, ci, wt, cap, first_edge_batch=eb.numpy(), num_first_batches=nb)
+    res = wl.wl_refine_batched(n, None, None, None, max_batch_edges=cap, seed=nb, coo_batches=gg.coo_batches(g, eb, nb))
+    got = res.colors.numpy()
+    assert got.tolist() == want.tolist() and res.num_colors == k_want
+    assert res.stats["outer_iters"] == outer_want and res.stats["last_num_batches"] == nbl_want
+    assert oracle.is_stable(n, rp, ci, wt, got) and refines(got, coarsest)
+    # Def. 5 census of the first iteration
+    src = gg.edge_sources(g).numpy()
+    nbatches_of = np.zeros(n, dtype=np.int64)
+    for k in range(nb):
+        nbatches_of[np.unique(src[eb.numpy() == k])] += 1
+    assert res.stats["boundary_nodes"] == int((nbatches_of >= 2).sum())
+    # renumbering the batches (and shuffling the edges inside them) changes nothing
+    perm = torch.tensor([(k + 1) % nb for k in range(nb)], dtype=torch.int32)
+    batches2 = gg.coo_batches(g, perm[eb.long()], nb)
+    batches2 = [(s.flip(0).contiguous(), c.flip(0).contiguous(), None if w is None else w.flip(0).contiguous())
+                for s, c, w in batches2]
+    # (sinks are inner to batch 0 by reading Q9, so a renumbering may group them with other nodes in iteration 1: the
+    # renumbered run is compared with the CPU Algorithm 2 on the renumbered labels, and must be stable all the same)
+    res2 = wl.wl_refine_batched(n, None, None, None, max_batch_edges=cap, seed=99, coo_batches=batches2)
+    assert oracle.is_stable(n, rp, ci, wt, res2.colors.numpy()) and refines(res2.colors.numpy(), coarsest)
+    want2, _, _, _ = oracle.rbsc(n, rp, ci, wt, cap, first_edge_batch=perm[eb.long()].numpy(), num_first_batches=nb)
+    assert res2.colors.numpy().tolist() == want2.tolist()
+
+
+def test_batched_coo_errors_and_edge_cases():
+    g = gg.rmat(9, seed=2, symmetrize=False)
+    n = g.n
+    eb = gg.random_edge_batches(g, 3, 1)
+    batches = gg.coo_batches(g, eb, 3)
+    bad = [(s.clone(), c.clone(), w) for s, c, w in batches]
+    bad[1][1][0] = n  # target out of range
+    with pytest.raises(wl.WlError) as e:
+        wl.wl_refine_batched(n, None, None, None, max_batch_edges=g.m, coo_batches=bad)
+    assert e.value.code == wl.WL_EINVAL
+    bad = [(s.clone(), c.clone(), w) for s, c, w in batches]
+    bad[2][0][-1] = -1  # source out of range
+    with pytest.raises(wl.WlError) as e:
+        wl.wl_refine_batched(n, None, None, None, max_batch_edges=g.m, coo_batches=bad)
+    assert e.value.code == wl.WL_EINVAL
+    with pytest.raises(wl.WlError) as e:  # inherited batches are defined for row-contiguous partitions only
+        wl.wl_refine_batched(n, None, None, None, max_batch_edges=g.m, coo_batches=batches, flags=wl.WL_FLAG_INHERIT_BATCHES)
+    assert e.value.code == wl.WL_EINVAL
+    # an empty batch, and a graph without edges
+    empty = (torch.empty(0, dtype=torch.int32), torch.empty(0, dtype=torch.int32), None)
+    res = wl.wl_refine_batched(n, None, None, None, max_batch_edges=g.m, coo_batches=batches + [empty])
+    nn, rp, ci, wt = g.numpy()
+    want, _, _, _ = oracle.rbsc(nn, rp, ci, wt, g.m, first_edge_batch=eb.numpy(), num_first_batches=4)
+    assert res.colors.numpy().tolist() == want.tolist()
+    res = wl.wl_refine_batched(5, None, None, None, max_batch_edges=1, coo_batches=[empty, empty])
+    assert res.colors.tolist() == [0] * 5
+    # a weighted row whose pieces sum to 2^32 across two batches (Theorem 1's precondition is per ROW, L129)
+    s0 = torch.tensor([0, 1], dtype=torch.int32)
+    c0 = torch.tensor([1, 0], dtype=torch.int32)
+    w0 = torch.tensor([(1 << 31), 1], dtype=torch.int64)
+    with pytest.raises(wl.WlError) as e:
+        wl.wl_refine_batched(2, None, None, None, max_batch_edges=4, coo_batches=[(s0, c0, w0), (s0[:1], c0[:1], w0[:1])])
+    assert e.value.code == wl.WL_ERANGE
+
+
 def test_batched_caller_supplied_slices():
     g = gg.rmat(10, seed=4)
     n, rp, ci, wt = g.numpy()
@@ -187,6 +267,36 @@ def test_batched_with_caller_host_workspace_and_long_hub_rows():
         assert res.colors.numpy().tolist() == want.tolist()
         assert res.stats["outer_iters"] == outer_want and res.stats["last_num_batches"] == nbl_want
     assert oracle.is_stable(n, rp, ci, wt, res.colors.numpy())
+
+
+def test_batched_validation_reaches_cut_rows_and_host_offsets():
+    """S0 in the batched path: a bad target inside a row that is CUT by a batch border (a boundary node: refine_core never
+    sees that row, the quotient pass maps it through the block map), malformed host offsets, and a weighted cut row whose
+    sum reaches 2^32 (Theorem 1's precondition, L129) must come back as WL_EINVAL / WL_ERANGE, never as a CUDA fault."""
+    g = BATCH_GRAPHS["hub"]()  # row 0 has 3000 entries; cap 1000 cuts it twice
+    n, m = g.n, g.m
+    for pos, val in ((1500, n + 5), (2999, -4), (10, n)):
+        bad = g.col.clone()
+        bad[pos] = val
+        with pytest.raises(wl.WlError) as e:
+            wl.wl_refine_batched(n, g.row_ptr, bad, None, max_batch_edges=1000, seed=1)
+        assert e.value.code == wl.WL_EINVAL
+    for mutate in (lambda rp: rp.__setitem__(5, int(rp[6]) + 1), lambda rp: rp.__setitem__(0, 1)):
+        rp2 = g.row_ptr.clone()
+        mutate(rp2)
+        with pytest.raises(wl.WlError) as e:
+            wl.wl_refine_batched(n, rp2, g.col, None, max_batch_edges=1000, seed=1)
+        assert e.value.code == wl.WL_EINVAL
+    w = torch.ones(m, dtype=torch.int64)
+    w[:3000] = 1 << 21  # 3000 * 2^21 > 2^32 on the cut row
+    with pytest.raises(wl.WlError) as e:
+        wl.wl_refine_batched(n, g.row_ptr, g.col, w, max_batch_edges=1000, seed=1)
+    assert e.value.code == wl.WL_ERANGE
+    w[:3000] = 1 << 20  # 3000 * 2^20 < 2^32: fine, and equal to the CPU Algorithm 2
+    nn, rp, ci, _ = g.numpy()
+    want, _, _, _ = oracle.rbsc(nn, rp, ci, w.numpy().astype(np.uint32), 1000)
+    res = wl.wl_refine_batched(n, g.row_ptr, g.col, w, max_batch_edges=1000, seed=1)
+    assert res.colors.numpy().tolist() == want.tolist()
 
 
 def test_batched_device_cap_is_checked_for_every_allocation():

@@ -97,6 +97,52 @@ def test_spmv_edge_balanced_unaligned_columns(name, shift):
     assert (u64(y) == want).all()
 
 
+@pytest.mark.parametrize("name", ["weighted", "weighted_big_w", "rmat12_sym", "hub_20000", "twin_hubs", "multigraph"])
+@pytest.mark.parametrize("narrow", [False, True])
+def test_spmv_active_row_list_bit_exact(name, narrow):
+    """Step-level S1+S2 with an ACTIVE ROW LIST (the kernels of the pruned rounds: rows != NULL), weighted and unweighted,
+    32-bit and 16-bit colour ids, hub rows inside and outside the list: the listed entries of y equal the oracle's u64 SpMV,
+    every other entry keeps the value it had."""
+    g = GRAPHS[name]()
+    n, rp, ci, wt = g.numpy()
+    colors = gg.random_partition(n, max(1, min(n // 3, 60000)), 17).numpy()
+    key = wl.wl_round_key(5, 2, 3)
+    want = oracle.spmv_u64(n, rp, ci, wt, oracle_w(key, colors))
+    dn, drp, dci, dwt = dgraph(g)
+    for frac, sd in ((2, 1), (7, 2)):
+        pick = torch.nonzero(gg.hash_u32(sd, torch.arange(n, dtype=torch.int64)) % frac == 0).flatten().to(torch.int32)
+        if name in ("hub_20000", "twin_hubs") and sd == 2:
+            pick = pick[pick != 0]  # the hub row (node 0) stays outside the list: its y must not be touched
+        marker = 0x0123456789ABCDEF
+        y = torch.full((n,), marker, dtype=torch.int64, device=dev())
+        wl.wl_spmv_rows(dn, drp, dci, dwt, torch.from_numpy(colors).to(dev()), key, pick.to(dev()), y,
+                        flags=wl.WL_FLAG_NARROW_COLORS if narrow else 0)
+        got = u64(y)
+        listed = np.zeros(n, dtype=bool)
+        listed[pick.numpy()] = True
+        assert (got[listed] == want[listed]).all()
+        assert (got[~listed] == np.uint64(marker)).all()
+
+
+@pytest.mark.parametrize("name", ["rmat12_sym", "rmat13_dir", "weighted", "grid_33", "twin_hubs", "multigraph", "er_c1"])
+@pytest.mark.parametrize("flags", [0, 2, 1024, 512, 64, 256])
+def test_refine_with_init_equals_oracle(name, flags):
+    """Arbitrary initial partition (L94): sparse, non-dense labels, the output aliasing the init array.  Colours and the
+    per-round colour counts equal the oracle's over the flag matrix (pruning, finality, worklist regime, per-round sync)."""
+    g = GRAPHS[name]()
+    n, rp, ci, wt = g.numpy()
+    dn, drp, dci, dwt = dgraph(g)
+    for k0, seed in ((2, 1), (7, 2), (max(2, n // 5), 3)):
+        init = gg.random_partition(n, k0, seed)
+        want, counts, rounds = oracle.refine(n, rp, ci, wt, init.numpy())
+        labels = (init.to(torch.int64) * 1000003 % 2147483000).to(torch.int32).to(dev())  # sparse non-dense labels
+        assert torch.unique(labels).numel() == torch.unique(init).numel()
+        res = wl.wl_refine(dn, drp, dci, dwt, labels, seed=seed * 31, flags=flags, out=labels)  # out aliases init
+        assert res.round_colors == counts and res.rounds == rounds
+        assert res.colors.cpu().numpy().tolist() == want.tolist()
+        assert res.colors.data_ptr() == labels.data_ptr()
+
+
 def test_spmv_uniform_gives_degrees_times_w0():
     g = gg.rmat(12, seed=4)
     n, rp, ci, wt = g.numpy()
