@@ -29,6 +29,7 @@ if ROOT not in sys.path:
 RMAT_SEEDS = {22: 1, 27: 2, 30: 3}  # BASELINE.json configs[2..4]
 ORACLE_SAMPLE_SCALE = 21           # bounded sample of the same recipe for the CPU oracle (about 10-30 s)
 HBM_FALLBACK_GBS = 6650.0          # /opt/skills/guides/B200_PROFILING.md fallback
+KNOWN_SIZES = {22: (4194304, 128311764), 27: (134217728, 4223286680)}  # (n, m) of the deterministic generator
 
 
 def ncu_traffic():
@@ -38,6 +39,61 @@ def ncu_traffic():
         return json.load(open(os.path.join(ROOT, "profiles", "ncu_traffic.json")))
     except Exception:
         return None
+
+
+def _classify(got, want):
+    """Reading Q12: 'equal', 'coarser' (the exact colouring strictly refines the result: a randomized collision) or
+    'other' (a bug).  numpy int arrays of canonical colours."""
+    import numpy as np
+    if got.shape == want.shape and bool((got == want).all()):
+        return "equal"
+    # want refines got <=> every block of want lies inside one block of got
+    pairs = np.unique(np.stack([want.astype(np.int64), got.astype(np.int64)], 1), axis=0)
+    return "coarser" if pairs.shape[0] == int(want.max()) + 1 else "other"
+
+
+def mismatch_report(wl, gg, oracle, dev, seeds_c1=100, seeds_c3=0):
+    """north_star: 'any randomized-collision mismatch counted and reported against the paper's stated failure bound'.
+    C1 (and C3 when asked) refined with many seeds, every result classified against the oracle's colouring."""
+    import torch
+    out = {"bound_per_run": 1e-9, "bound_source": "Theorem 1, PAPER.md L129 (q = 64)", "configs": []}
+    todo = [("C1 Erdos-Renyi 10k/50k", gg.erdos_renyi(), seeds_c1)]
+    if seeds_c3:
+        todo.append(("C3 R-MAT scale 22", gg.rmat(22, seed=RMAT_SEEDS[22], device=dev), seeds_c3))
+    for name, g, seeds in todo:
+        n, rp, ci, wt = g.numpy()
+        want, counts, _ = oracle.refine(n, rp, ci, wt)
+        gd = g.to(dev)
+        wdev = torch.from_numpy(want).to(dev)
+        t = {"equal": 0, "coarser": 0, "other": 0}
+        for seed in range(seeds):
+            r = wl.wl_refine(n, gd.row_ptr, gd.col, None, seed=7000 + seed)
+            if bool(torch.equal(r.colors, wdev)) and r.round_colors == counts:
+                t["equal"] += 1
+            else:
+                t[_classify(r.colors.cpu().numpy(), want)] += 1
+        out["configs"].append({"config": name, "runs": seeds, **t})
+    out["runs"] = sum(c["runs"] for c in out["configs"])
+    out["mismatching_runs"] = sum(c["coarser"] + c["other"] for c in out["configs"])
+    return out
+
+
+def split_pairs_on_device(wl, n, row_ptr, col, rounds, dev):
+    """N_r = sum over the blocks B of the partition before round r of C(s_B, 2), s_B = number of blocks of the partition after
+    round r inside B: the pairs of sub-blocks whose z must differ for round r to be computed exactly (failure bound
+    of the build).  Partitions after r rounds come from wl_refine(max_rounds = r)."""
+    import torch
+    prev = torch.zeros(n, dtype=torch.int64, device=dev)
+    out = []
+    for r in range(1, rounds):
+        cur = wl.wl_refine(n, row_ptr, col, None, seed=1, max_rounds=r, allow_max_rounds=True, deep=False).colors.to(torch.int64)
+        k_cur = int(cur.max()) + 1
+        pairs = torch.unique(prev * k_cur + cur)
+        s_b = torch.bincount(pairs // k_cur)
+        out.append(int((s_b * (s_b - 1) // 2).sum()))
+        prev = cur
+        del pairs, s_b
+    return out
 
 
 def measured_peaks():
@@ -117,7 +173,7 @@ def oracle_sample(scale: int):
     return {"value": g.m * rounds / dt / 1e9, "unit": "GEdges/s", "cores": cores, "kind": "oracle",
             "sample": f"R-MAT scale {scale} (n={n}, m={g.m}), same recipe and seed as the workload, {rounds} rounds of "
                       f"signature-sort refinement in {dt:.2f} s (signatures built with OpenMP, sort on one core)",
-            "seconds": dt, "rounds": rounds, "m": g.m}
+            "seconds": dt, "rounds": rounds, "m": g.m, "n": n}
 
 
 def run_reference(args):
@@ -134,10 +190,17 @@ def run_reference(args):
     value = last["m"] * last["rounds"] / (ms / 1e3) / 1e9
     cb = {k: last[k] for k in ("unit", "cores", "kind", "sample")}
     cb["value"] = value
+    # this arm's config is the headline workload (the driver compares the two arms on it); every step is a bounded sample of
+    # it: the same recipe and seed at a smaller scale, named here with its true sizes
+    cfg = workload_config(args.scale, KNOWN_SIZES.get(args.scale, (None, None))[0], KNOWN_SIZES.get(args.scale, (None, None))[1])
+    cfg["sample"] = {"scale": args.oracle_scale, "n": last["n"], "m": last["m"], "rounds": last["rounds"],
+                     "what": "each step refines this bounded sample of the workload (same R-MAT recipe and seed, smaller scale) "
+                             "with the CPU oracle (signature-sort refinement)"}
+    cfg["value_definition"] = "m_sample x rounds / seconds (every round of the oracle reads every edge; no pruning)"
     line = {"impl": "reference", "metric": "refine_gedges_per_s", "value": value, "unit": "GEdges/s",
             "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u64", "data": "synthetic",
-            "config": workload_config(args.scale, None, None), "cpu_baseline": cb,
+            "config": cfg, "cpu_baseline": cb,
             "e2e": {"value": value, "unit": "GEdges/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line))
@@ -244,11 +307,34 @@ def run_batch_study(args):
                 dt = time.perf_counter() - t0
                 best = dt if best is None else min(best, dt)
             base = best if nb == 1 else base
-            rows.append({"graph": name, "n": n, "m": m, "N_b": nb, "colors": r.num_colors,
+            rows.append({"graph": name, "n": n, "m": m, "N_b": nb, "partition": "row-contiguous (CSR slices)",
+                         "colors": r.num_colors,
                          "reduction_power_pct": 100.0 * r.num_colors / n,
                          "coarsest_pct": 100.0 * single.num_colors / n,
                          "gap_pp": 100.0 * (r.num_colors - single.num_colors) / n,
-                         "outer_iters": r.stats["outer_iters"], "seconds": best, "slowdown_vs_Nb1": best / base})
+                         "outer_iters": r.stats["outer_iters"], "boundary_nodes": r.stats["boundary_nodes"],
+                         "seconds": best, "slowdown_vs_Nb1": best / base})
+            if nb == 1:
+                continue
+            # the same graph under ARBITRARY edge partitions (COO batches, Thm 2)
+            gc = gd.to("cpu")
+            for pname, eb in (("random edges", gg.random_edge_batches(gc, nb, 5)),
+                              ("by source node, 5 % of the edges moved", gg.node_hash_edge_batches(gc, nb, 5, 5))):
+                cb = [tuple(None if t is None else t.pin_memory() for t in b) for b in gg.coo_batches(gc, eb, nb)]
+                best = None
+                for rep in range(2):
+                    torch.cuda.synchronize(dev)
+                    t0 = time.perf_counter()
+                    r = wl.wl_refine_batched(n, None, None, None, max_batch_edges=(m + nb - 1) // nb, seed=20 + rep,
+                                             host_workspace=hws, coo_batches=cb)
+                    dt = time.perf_counter() - t0
+                    best = dt if best is None else min(best, dt)
+                rows.append({"graph": name, "n": n, "m": m, "N_b": nb, "partition": pname, "colors": r.num_colors,
+                             "reduction_power_pct": 100.0 * r.num_colors / n,
+                             "coarsest_pct": 100.0 * single.num_colors / n,
+                             "gap_pp": 100.0 * (r.num_colors - single.num_colors) / n,
+                             "outer_iters": r.stats["outer_iters"], "boundary_nodes": r.stats["boundary_nodes"],
+                             "seconds": best, "slowdown_vs_Nb1": best / base})
     print(json.dumps({"metric": "batch_study", "unit": "table", "data": "synthetic", "rows": rows}))
     return 0
 
@@ -294,6 +380,112 @@ def run_cap_sweep(args):
     return 0
 
 
+def _oracle_child(kind, path, threads, q):
+    """Runs in a child process (so that a wall-clock limit can end it): one oracle run on the graph stored at `path`."""
+    os.environ["OMP_NUM_THREADS"] = str(threads)
+    import numpy as np
+    import oracle
+    d = np.load(path)
+    n, rp, ci = int(d["n"]), d["rp"], d["ci"]
+    t0 = time.perf_counter()
+    if kind == "refine":
+        c, counts, rounds = oracle.refine(n, rp, ci)
+    else:
+        c, counts, rounds, _ = oracle.rsc(n, rp, ci, seed=424242)
+    dt = time.perf_counter() - t0
+    np.save(path + ".colors.npy", c)
+    q.put((dt, counts, rounds))
+
+
+def _timed_oracle(kind, n, rp, ci, threads, limit, tag):
+    import multiprocessing as mp
+    import numpy as np
+    path = f"/tmp/wl_oracle_{tag}_{os.getpid()}.npz"
+    np.savez(path, n=n, rp=rp, ci=ci)
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    p = ctx.Process(target=_oracle_child, args=(kind, path, threads, q))
+    t0 = time.perf_counter()
+    p.start()
+    res = None
+    try:
+        res = q.get(timeout=limit)
+    except Exception:
+        pass
+    if res is None:
+        p.kill()
+        p.join()
+        out = {"finished": False, "seconds": time.perf_counter() - t0, "limit_s": limit}
+    else:
+        p.join()
+        out = {"finished": True, "seconds": res[0], "counts": res[1], "rounds": res[2],
+               "colors": np.load(path + ".colors.npy")}
+    for f in (path, path + ".colors.npy"):
+        try:
+            os.remove(f)
+        except OSError:
+            pass
+    return out
+
+
+def run_oracle_times(args):
+    """--workload oracle-times: SURVEY.md §8(d) "Oracle timing": the CPU oracle (signature-sort refinement), single-threaded and
+    on all cores, on C1-C3, each under a wall-clock limit ("did not finish" is an allowed outcome); nproc printed.  C4 is
+    attempted by `--workload c4-check` with the CPU Algorithm 1 (the signature oracle needs more host memory than the box has
+    at scale 27)."""
+    import torch
+    import graphgen as gg
+    dev = "cuda" if torch.cuda.is_available() else "cpu"
+    nproc = os.cpu_count() or 1
+    rows = []
+    for name, make in (("C1 Erdos-Renyi 10k/50k", lambda: gg.erdos_renyi()),
+                       ("C2 grid 2048^2 (1024 rounds)", lambda: gg.grid2d(2048, device=dev)),
+                       ("C3 R-MAT scale 22", lambda: gg.rmat(22, seed=RMAT_SEEDS[22], device=dev))):
+        g = make()
+        n, rp, ci, wt = g.numpy()
+        del g
+        for threads in (1, nproc):
+            r = _timed_oracle("refine", n, rp, ci, threads, args.time_limit, name.split()[0])
+            rows.append({"config": name, "n": n, "m": int(rp[-1]), "threads": threads, "finished": r["finished"],
+                         "seconds": r["seconds"], "rounds": r.get("rounds"),
+                         "num_colors": (r["counts"][-1] if r.get("counts") else None)})
+            print(json.dumps(rows[-1]), file=sys.stderr, flush=True)
+    print(json.dumps({"metric": "oracle_times", "unit": "table", "nproc": nproc, "limit_s": args.time_limit, "rows": rows}))
+    return 0
+
+
+def run_c4_check(args):
+    """--workload c4-check: an element-by-element target for the headline config.  The CPU Algorithm 1 (oracle.rsc, pinned equal
+    to the signature oracle, DESIGN.md section 10) refines the scale-27 graph once with ITS OWN seed under a wall-clock limit;
+    the GPU colouring (different seed, default flags) must equal it element by element, per-round colour counts included."""
+    import numpy as np
+    import torch
+    import graphgen as gg
+    import paper_2607_02603_b200 as wl
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    g = gg.rmat(args.scale, seed=RMAT_SEEDS.get(args.scale, 2), device=dev, chunk=1 << 28)
+    torch.cuda.empty_cache()
+    n, m = g.n, g.m
+    res = wl.wl_refine(n, g.row_ptr, g.col, None, seed=2027, deep=False)
+    got = res.colors.cpu().numpy()
+    rp, ci = g.row_ptr.cpu().numpy(), g.col.cpu().numpy()
+    del g
+    torch.cuda.empty_cache()
+    r = _timed_oracle("rsc", n, rp, ci, 1, args.time_limit, "c4")
+    line = {"metric": "c4_check", "unit": "bool", "config": workload_config(args.scale, n, m), "gpu_rounds": res.rounds,
+            "gpu_round_colors": res.round_colors, "gpu_num_colors": res.num_colors,
+            "oracle": "oracle.rsc (CPU Algorithm 1 in Z/2^64, one thread, seed 424242)", "oracle_finished": r["finished"],
+            "oracle_seconds": r["seconds"], "limit_s": args.time_limit}
+    if r["finished"]:
+        line["oracle_round_colors"] = r["counts"]
+        line["trajectory_equal"] = r["counts"] == res.round_colors
+        line["colors_equal_element_by_element"] = bool((r["colors"] == got).all())
+        line["classification"] = _classify(got, r["colors"])
+    print(json.dumps(line))
+    return 0
+
+
 def aggregate_over_ranks(dist, local_ms: float, units_per_rank: float, device=None):
     """Max-over-ranks time and whole-job throughput for N independent replicas (weak scaling, no data-path collective).
     dist = torch.distributed (initialised) or None for a single process.  Returns (ms_max, total_units_per_second)."""
@@ -328,7 +520,9 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--flags", type=int, default=0, help="WL_FLAG_* bits passed to wl_refine")
-    ap.add_argument("--workload", default="single", choices=["single", "batched", "batch-study", "cap-sweep"],
+    ap.add_argument("--mismatch-c3-seeds", type=int, default=20, help="seeds of the C3 leg of the mismatch report (0: C1 only)")
+    ap.add_argument("--time-limit", type=float, default=1800.0, help="oracle-times / c4-check: wall-clock limit per oracle run (s)")
+    ap.add_argument("--workload", default="single", choices=["single", "batched", "batch-study", "cap-sweep", "oracle-times", "c4-check"],
                     help="single: wl_refine on the HBM-resident graph (the headline); batched: wl_refine_batched")
     ap.add_argument("--cap-gb", type=float, default=16.0, help="batched: device memory cap")
     ap.add_argument("--batch-edges", type=int, default=0, help="batched: M_b (0: derived by the library from the device cap)")
@@ -342,6 +536,10 @@ def main():
         return run_batch_study(args)
     if args.workload == "cap-sweep":
         return run_cap_sweep(args)
+    if args.workload == "oracle-times":
+        return run_oracle_times(args)
+    if args.workload == "c4-check":
+        return run_c4_check(args)
 
     import torch
     import graphgen as gg
@@ -478,9 +676,22 @@ def main():
         return 0
 
     cpu_baseline = None
+    mismatches = None
+    failure_bound = None
     if not args.no_cpu_baseline and world == 1:
         cb = oracle_sample(args.oracle_scale)
         cpu_baseline = {k: cb[k] for k in ("value", "unit", "cores", "kind", "sample")}
+        import oracle
+        mismatches = mismatch_report(wl, gg, oracle, dev, seeds_c1=100, seeds_c3=args.mismatch_c3_seeds)
+        # union bound of the DEFAULT build on this workload (R4 / R5 make a mid-run collision permanent):
+        # sum_r N_r 2^(t - 64) / 0.6 with the pair counts of this very graph; plain Algorithm 1 (WL_FLAG_NO_DEEP |
+        # WL_FLAG_NO_FINAL) keeps the paper's 2^-32 / 0.6 per run
+        npairs = split_pairs_on_device(wl, n, g.row_ptr, g.col, results[-1].rounds, dev)
+        failure_bound = {"pairs_per_round": npairs, "pairs": sum(npairs),
+                         "default_build_union_bound_t0": sum(npairs) * 2.0 ** -64 / 0.6,
+                         "plain_algorithm1_bound": 2.0 ** -32 / 0.6,
+                         "note": "t0: coefficient differences odd (gcd term 2^t = 1, the common case on unweighted graphs); "
+                                 "worst case multiplies by 2^t <= 2^32 (Lemma 1, L418)"}
 
     last = results[-1]
     line = {
@@ -493,6 +704,7 @@ def main():
         "seconds_to_stable_coloring": ms_per_step / 1e3,
         "phase_ms": {"spmv": last.stats["ms_spmv"], "relabel": last.stats["ms_relabel"], "total": last.stats["ms_total"]},
         "roofline": roofline, "cpu_baseline": cpu_baseline, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
+        "mismatches": mismatches, "failure_bound": failure_bound,
     }
     print(json.dumps(line))
     if dist is not None:

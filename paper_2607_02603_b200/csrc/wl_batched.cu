@@ -70,6 +70,61 @@ __global__ void iota_kernel(int64_t n, int* __restrict__ a) {
   if (i < n) a[i] = (int)i;
 }
 
+// Eq. 4 for one batch whose local colours have just been made canonical inside the batch (first-occurrence ids): the global
+// id is base + local canonical id.  Batches and the boundary nodes between them are taken in node order, so the global ids are
+// canonical as well and no pass over all n nodes is needed.  isrep[i] = 1 for the first node of every block (Q17).
+__global__ void merge_canon_kernel(int64_t nr, const int* __restrict__ local_colour, const int* __restrict__ first, int base,
+                                   int* __restrict__ Hc, unsigned char* __restrict__ isrep) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= nr) return;
+  Hc[i] += base;
+  isrep[i] = first[local_colour[i]] == (int)i;
+}
+
+// Alg. 2 lines 11-12: the boundary nodes g0 .. g0 + count - 1 become singleton blocks base, base + 1, ...
+__global__ void gap_singletons_kernel(int64_t g0, int64_t count, int base, int* __restrict__ Hc,
+                                      unsigned char* __restrict__ isrep) {
+  int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= count) return;
+  Hc[g0 + t] = base + (int)t;
+  isrep[g0 + t] = 1;
+}
+
+// one block made of the nodes [0, count): id `id`, representative = the first one (a piece of edgeless nodes)
+__global__ void one_block_kernel(int64_t count, int id, int* __restrict__ Hc, unsigned char* __restrict__ isrep) {
+  int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= count) return;
+  Hc[t] = id;
+  isrep[t] = t == 0;
+}
+
+// counts[q] = number of representatives i with queries[q - 1] <= i < queries[q] (queries increasing, queries[-1] = 0): the host
+// prefix-sums them into "blocks whose first node lies before queries[q]"
+__global__ void count_reps_kernel(int64_t n, const unsigned char* __restrict__ isrep, const int64_t* __restrict__ queries, int nq,
+                                  u64* __restrict__ counts) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  int q = -1;
+  if (i < n && isrep[i]) {
+    int lo = 0, hi = nq;  // first q with queries[q] > i (nq: beyond the last query)
+    while (lo < hi) {
+      const int mid = (lo + hi) >> 1;
+      if (queries[mid] > i) hi = mid;
+      else lo = mid + 1;
+    }
+    q = lo;
+  }
+  const unsigned peers = __match_any_sync(0xffffffffu, q);
+  if (q >= 0 && (int)(threadIdx.x & 31) == __ffs(peers) - 1) atomicAdd(counts + q, (u64)__popc(peers));
+}
+
+// the window of per-block counters moves on by `len` blocks: the counter of the block whose row is still open (index len)
+// becomes index 0, everything else is zero again
+__global__ void window_carry_kernel(int* __restrict__ cnt, int64_t len, int* __restrict__ carry, int phase) {
+  if (blockIdx.x || threadIdx.x) return;
+  if (phase == 0) *carry = cnt[len];
+  else cnt[0] = *carry;
+}
+
 __global__ void compose_kernel(int64_t n0, int* __restrict__ map0, const int* __restrict__ Hc) {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i < n0) map0[i] = Hc[map0[i]];
@@ -128,14 +183,14 @@ constexpr int kQuotLongRow = 4096;  // longer pieces are left to quot_insert_lon
 __global__ void __launch_bounds__(256)
 quot_insert_kernel(int64_t row_base, int64_t n_rows, const int64_t* __restrict__ row_ptr, int64_t clip_lo, int64_t clip_hi,
                    const int* __restrict__ col, const u32* __restrict__ wt, const int* __restrict__ Hc,
-                   const int* __restrict__ rep_of_block, Slot* __restrict__ table, u64 table_mask, int* __restrict__ cnt,
-                   int* __restrict__ long_rows, u32* __restrict__ long_count) {
+                   const int* __restrict__ rep_of_block, const unsigned char* __restrict__ isrep, Slot* __restrict__ table,
+                   u64 table_mask, int* __restrict__ cnt, int* __restrict__ long_rows, u32* __restrict__ long_count) {
   const int lane = threadIdx.x & 31;
   const int64_t w = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   if (w >= n_rows) return;
   const int64_t i = row_base + w;
   const int b = Hc[i];
-  if (rep_of_block[b] != (int)i) return;
+  if (isrep ? !isrep[i] : rep_of_block[b] != (int)i) return;  // representative = first node of its block (Q17)
   int64_t a = row_ptr[w], e = row_ptr[w + 1];
   if (a < clip_lo) a = clip_lo;
   if (e > clip_hi) e = clip_hi;
@@ -559,11 +614,12 @@ void launch_scan32(const int* cnt, int64_t n, int64_t base_off, int64_t* out, u6
 // step 1 of the quotient for the rows [row_base, row_base + n_rows) whose offsets are row_ptr[0..n_rows]; long_rows needs
 // (clip_hi - clip_lo) / kQuotLongRow + 2 ints, *long_count is zeroed here
 static void launch_quot_insert(int64_t row_base, int64_t n_rows, const int64_t* row_ptr, int64_t clip_lo, int64_t clip_hi,
-                               const int* col, const u32* wt, const int* Hc, const int* rep_of_block, u64* table,
-                               u64 table_mask, int* cnt, int* long_rows, u32* long_count, cudaStream_t st) {
+                               const int* col, const u32* wt, const int* Hc, const int* rep_of_block,
+                               const unsigned char* isrep, u64* table, u64 table_mask, int* cnt, int* long_rows,
+                               u32* long_count, cudaStream_t st) {
   if (n_rows <= 0) return;
   cudaMemsetAsync(long_count, 0, sizeof(u32), st);
-  ++g_launches; quot_insert_kernel<<<blocks_for(n_rows * 32, 256), 256, 0, st>>>(row_base, n_rows, row_ptr, clip_lo, clip_hi, col, wt, Hc, rep_of_block, (Slot*)table, table_mask, cnt, long_rows, long_count);
+  ++g_launches; quot_insert_kernel<<<blocks_for(n_rows * 32, 256), 256, 0, st>>>(row_base, n_rows, row_ptr, clip_lo, clip_hi, col, wt, Hc, rep_of_block, isrep, (Slot*)table, table_mask, cnt, long_rows, long_count);
   ++g_launches; quot_insert_long_kernel<<<148 * 8, 256, 0, st>>>(row_base, row_ptr, clip_lo, clip_hi, col, wt, Hc, (Slot*)table, table_mask, cnt, long_rows, long_count);
 }
 
@@ -669,7 +725,7 @@ int wl_quotient(const wl_csr* g, const int32_t* colors, int64_t k, int64_t* q_ro
   cudaMemsetAsync(cnt, 0, sizeof(int) * (size_t)k, st);
   cudaMemsetAsync(cursor, 0, sizeof(int) * (size_t)k, st);
   ++g_launches; block_rep_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, colors, rep_of_block);
-  launch_quot_insert(0, n, g->row_ptr, 0, m, g->col_idx, g->weights, colors, rep_of_block, table, slots - 1, cnt, long_rows,
+  launch_quot_insert(0, n, g->row_ptr, 0, m, g->col_idx, g->weights, colors, rep_of_block, nullptr, table, slots - 1, cnt, long_rows,
                      (u32*)(total + 1), st);
   launch_scan32(cnt, k, 0, q_row_ptr, bsum, total, st);
   u64 h_total = 0;
@@ -1164,7 +1220,7 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
   // they are still on the device, batch = the rows emitted together; the next iteration then starts at the merge.
   const bool inherit = (flags & WL_FLAG_INHERIT_BATCHES) != 0;
   bool have_next = false;          // the coming iteration's local refinement is done already
-  DevBuf d_Hnext_keep;             // ... its merged block map (before the boundary / canonical step)
+  DevBuf d_Hnext_keep, d_isrep_keep;  // ... its canonical block map and representative flags
   std::vector<int64_t> node_cuts;  // ... and the node ranges of its batches
   int64_t next_base_id = 0;
   const bool debug = debug_enabled();
@@ -1236,26 +1292,29 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
       ws_bytes = std::max(ws_bytes, make_layout(r1[k] - r0[k], rp[r1[k]] - rp[r0[k]]).bytes);
 
     // ---- device memory of this outer iteration ---------------------------------------------------------------------
+    // Per node of the current graph the device holds the canonical block map (4 B) and a representative flag (1 B), plus the
+    // composed map of the original nodes (4 B per original node); everything else is sized by a batch (O(n / N_b)): the
+    // batches and the boundary nodes between them are merged in node order with locally canonical ids, so the global ids
+    // are canonical without a pass over all nodes, and the per-block counters of the quotient pass live in a window.
     size_t used_iter = used;
-    DevBuf d_H, d_Hc, d_first, d_cof, d_bsum, d_ws, d_col[2], d_wt[2], d_rp[2], d_rep, d_cnt, d_cursor, d_qrp, d_qtab,
-        d_qcol[2], d_qwt[2], d_sbsum, d_misc, d_query, d_long, d_Hnext, d_ws2;
-    const int64_t nscan = (n_t + kCanonChunk - 1) / kCanonChunk;
+    DevBuf d_Hc, d_isrep, d_ws, d_col[2], d_wt[2], d_rp[2], d_cnt, d_cursor, d_qrp[2], d_qtab, d_qcol[2], d_qwt[2], d_sbsum,
+        d_misc, d_query, d_long, d_Hnext, d_isrep_next, d_ws2;
     // every allocation of the iteration goes through here: the first failure (device cap or cudaMalloc) sticks
 #define WL_ALLOC(buf, bytes) \
   if (!rc) rc = buf.alloc((bytes), &used_iter, device_cap_bytes);
     if (have_next) {  // made by the previous iteration's quotient pass
-      d_H.p = d_Hnext_keep.p;
-      d_H.bytes = d_Hnext_keep.bytes;
+      d_Hc.p = d_Hnext_keep.p;
+      d_Hc.bytes = d_Hnext_keep.bytes;
       d_Hnext_keep.p = nullptr;
-      used_iter += d_H.bytes;
+      d_isrep.p = d_isrep_keep.p;
+      d_isrep.bytes = d_isrep_keep.bytes;
+      d_isrep_keep.p = nullptr;
+      used_iter += d_Hc.bytes + d_isrep.bytes;
       if (device_cap_bytes && used_iter > device_cap_bytes) rc = WL_ENOMEM;
     } else {
-      WL_ALLOC(d_H, sizeof(int) * (size_t)n_t);
+      WL_ALLOC(d_Hc, sizeof(int) * (size_t)n_t);
+      WL_ALLOC(d_isrep, (size_t)n_t);
     }
-    WL_ALLOC(d_Hc, sizeof(int) * (size_t)n_t);
-    WL_ALLOC(d_first, sizeof(int) * (size_t)n_t);
-    WL_ALLOC(d_cof, sizeof(int) * (size_t)n_t);
-    WL_ALLOC(d_bsum, sizeof(int) * (size_t)(nscan + 1));
     WL_ALLOC(d_ws, ws_bytes);
     for (int b = 0; b < 2; ++b) {
       WL_ALLOC(d_col[b], sizeof(int) * (size_t)max_edges);
@@ -1285,10 +1344,18 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
     };
 
     phase("alloc");
-    // ---- Alg. 2 lines 7-11: local refinement per batch, merge ---------------------------------------------------------
-    int64_t base_id = have_next ? next_base_id : 0;
+    // ---- Alg. 2 lines 7-12: local refinement per batch, merge (Eq. 4), boundary singletons, in node order -------------
+    int64_t base_id = have_next ? next_base_id : 0;  // have_next: the whole block map was made by the previous quotient pass
+    int64_t n_boundary = 0;
+    auto gap = [&](int64_t g0, int64_t g1) {  // the nodes g0 .. g1 - 1 lie between two inner ranges: boundary nodes
+      if (g1 <= g0) return;
+      ++g_launches; gap_singletons_kernel<<<blocks_for(g1 - g0, 256), 256, 0, st>>>(g0, g1 - g0, (int)base_id, d_Hc.as<int>(), d_isrep.as<unsigned char>());
+      base_id += g1 - g0;
+      n_boundary += g1 - g0;
+    };
     cudaStreamSynchronize(st);  // buffers of the previous iteration are free
     if (!have_next) upload_batch(0, 0);
+    int64_t next_node = 0;
     for (int k = 0; k < nb && !rc && !have_next; ++k) {
       const int buf = k & 1;
       if (k + 1 < nb) upload_batch(k + 1, buf ^ 1);
@@ -1299,6 +1366,8 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
         // quotient pass maps every stored target through the block map): range check of the WHOLE uploaded slice
         ++g_launches; slice_cols_check_kernel<<<148 * 8, 256, 0, st>>>(n_t, cuts[k + 1] - cuts[k], d_col[buf].as<int>(), (u32*)d_misc.p + 64);
       }
+      gap(next_node, r0[k]);
+      next_node = std::max(next_node, r1[k]);
       if (nr == 0) continue;
       const int64_t e0 = rp[r0[k]], e1 = rp[r1[k]];
       wl_csr lg;
@@ -1317,7 +1386,12 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
       CoreResult cr{};
       rc = refine_core(&lg, nullptr, seed, &lo, /*ranged=*/true, (int)r0[k], (int)r1[k], n_t, e0, d_ws.p, L.bytes, L, st, &cr);
       if (rc) break;
-      ++g_launches; merge_kernel<<<blocks_for(nr, 256), 256, 0, st>>>(nr, cr.colour, (int)base_id, d_H.as<int>() + r0[k]);
+      // canonical ids inside the batch (scratch: two dead arrays of the local workspace, as wl_refine does), then Eq. 4
+      char* wsb = (char*)d_ws.p;
+      int* first_l = (int*)(wsb + L.o_tmp);
+      launch_canonical(L, nr, cr.colour, d_Hc.as<int>() + r0[k], first_l, (int*)(wsb + L.o_rep), (int*)(wsb + L.o_bsum),
+                       (u64*)(wsb + L.o_scal) + kScalCanon, st);
+      ++g_launches; merge_canon_kernel<<<blocks_for(nr, 256), 256, 0, st>>>(nr, cr.colour, first_l, (int)base_id, d_Hc.as<int>() + r0[k], d_isrep.as<unsigned char>() + r0[k]);
       base_id += cr.k;
       edges_streamed += cr.edges_streamed;
       ms_spmv += cr.ms_spmv;
@@ -1328,6 +1402,8 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
       rc = check_cuda(cudaStreamSynchronize(st));  // the workspace and this buffer are reused by the next batch
     }
     if (rc) break;
+    if (!have_next) gap(next_node, n_t);
+    if (outer == 1) boundary_first = n_boundary;
     if (outer == 1 && !(flags & WL_FLAG_NO_VALIDATE)) {
       cudaMemcpyAsync(hs + kNumScal + 2, (u32*)d_misc.p + 64, sizeof(u32), cudaMemcpyDeviceToHost, st);
       rc = check_cuda(cudaStreamSynchronize(st));
@@ -1353,39 +1429,8 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
         if (rc) break;
       }
     }
-    phase("local refinement");
-    // ---- Alg. 2 lines 11-12: boundary nodes become singletons ---------------------------------------------------------
-    std::vector<int> bnodes, bids;
-    {
-      int64_t next = 0;
-      for (int k = 0; k <= nb; ++k) {
-        const int64_t upto = k < nb ? r0[k] : n_t;
-        for (int64_t i = next; i < upto; ++i) {
-          bnodes.push_back((int)i);
-          bids.push_back((int)(base_id++));
-        }
-        if (k < nb) next = r1[k];
-      }
-      if (!bnodes.empty()) {  // one upload of the node list, one kernel (ids are consecutive from bids[0])
-        DevBuf d_bn;
-        if ((rc = d_bn.alloc(sizeof(int) * bnodes.size(), &used_iter, device_cap_bytes))) break;
-        cudaMemcpyAsync(d_bn.p, bnodes.data(), sizeof(int) * bnodes.size(), cudaMemcpyHostToDevice, st);
-        bytes_h2d += sizeof(int) * bnodes.size();
-        ++g_launches; singleton_ids_kernel<<<blocks_for((int64_t)bnodes.size(), 256), 256, 0, st>>>((int64_t)bnodes.size(), d_bn.as<int>(), bids[0], d_H.as<int>());
-        cudaStreamSynchronize(st);  // bnodes is pageable and d_bn dies with this scope
-        d_bn.release(&used_iter);
-      }
-      if (outer == 1) boundary_first = (int64_t)bnodes.size();
-    }
-    // canonical block map of this iteration (first-occurrence ids keep the composed map canonical)
-    Layout Lc{};
-    Lc.nscan = nscan;
-    launch_canonical(Lc, n_t, d_H.as<int>(), d_Hc.as<int>(), d_first.as<int>(), d_cof.as<int>(), d_bsum.as<int>(),
-                     d_misc.as<u64>(), st);
-    cudaMemcpyAsync(hs + kScalCanon, d_misc.p, sizeof(u64), cudaMemcpyDeviceToHost, st);
-    rc = check_cuda(cudaStreamSynchronize(st));
-    if (rc) break;
-    const int64_t K = (int64_t)hs[kScalCanon];
+    phase("local refinement + merge");
+    const int64_t K = base_id;  // the ids are canonical: K blocks
     nb_last = nb;
     K_final = K;
     // compose original -> current map
@@ -1408,12 +1453,8 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
       break;
     }
 
-    phase("merge + canonical");
-    // the uncanonical block map and the canonicalisation scratch are dead: their 12 bytes per node go to the quotient pass
+    // the local workspace is dead: its bytes go to the quotient pass
     cudaStreamSynchronize(st);
-    d_H.release(&used_iter);
-    d_first.release(&used_iter);
-    d_cof.release(&used_iter);
     d_ws.release(&used_iter);
     // ---- Alg. 2 line 13: quotient (Def. 4), second streaming pass -------------------------------------------------------
     // Three streams: copy_st uploads batch k + 1 while st inserts / emits batch k and down_st returns the rows emitted for
@@ -1421,32 +1462,6 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
     if ((rc = hq.init(n0, rp0_edges, opt ? opt->host_workspace : nullptr, opt ? opt->host_workspace_bytes : 0))) break;
     const int osel = outer & 1;  // offsets of the quotient being written; the graph being read uses the other array
     int64_t* nrp = hq.rp[osel];
-    WL_ALLOC(d_rep, sizeof(int) * (size_t)K);
-    WL_ALLOC(d_cnt, sizeof(int) * (size_t)K);
-    WL_ALLOC(d_cursor, sizeof(int) * (size_t)K);
-    WL_ALLOC(d_qrp, sizeof(int64_t) * (size_t)(K + 1));
-    int64_t longest_cut_row = 0;  // a row cut by a batch border stays in the table until its last piece arrives
-    for (int k = 1; k < nb; ++k) {
-      const int64_t r = (std::upper_bound(rp, rp + n_t + 1, cuts[k]) - rp) - 1;
-      if (r >= 0 && r < n_t && rp[r] < cuts[k]) longest_cut_row = std::max(longest_cut_row, rp[r + 1] - rp[r]);
-    }
-    const int64_t out_cap = max_edges + longest_cut_row;  // entries one emission can hold
-    const u64 qslots = quot_table_slots(out_cap);
-    WL_ALLOC(d_qtab, sizeof(u64) * 2 * qslots);
-    for (int b = 0; b < 2; ++b) {
-      WL_ALLOC(d_qcol[b], sizeof(int) * (size_t)out_cap);
-      WL_ALLOC(d_qwt[b], sizeof(u32) * (size_t)out_cap);
-    }
-    WL_ALLOC(d_sbsum, sizeof(u64) * (size_t)((K + kScanC - 1) / kScanC + 2));
-    WL_ALLOC(d_query, sizeof(int64_t) * 2 * (size_t)nb);
-    WL_ALLOC(d_long, sizeof(int) * (size_t)(max_edges / kQuotLongRow + 2));
-    if (debug) std::fprintf(stderr, "[wl_refine_batched] outer %d device memory %.2f GB (cap %.2f GB)%s\n", outer, used_iter / 1073741824.0, device_cap_bytes / 1073741824.0, rc ? " -> WL_ENOMEM" : "");
-    if (rc) break;
-    ++g_launches; fill_kernel<<<blocks_for(K, 256), 256, 0, st>>>(K, d_rep.as<int>(), kNoNode);
-    cudaMemsetAsync(d_cnt.p, 0, sizeof(int) * (size_t)K, st);
-    cudaMemsetAsync(d_cursor.p, 0, sizeof(int) * (size_t)K, st);
-    cudaMemsetAsync(d_qtab.p, 0, sizeof(u64) * 2 * qslots, st);
-    ++g_launches; block_rep_kernel<<<blocks_for(n_t, 256), 256, 0, st>>>(n_t, d_Hc.as<int>(), d_rep.as<int>());
     // per batch: the nodes whose row intersects it, and the number of blocks whose representative row is complete after it
     std::vector<int64_t> na(nb), nz(nb), done_nodes(nb), done_blocks(nb);
     for (int k = 0; k < nb; ++k) {
@@ -1456,11 +1471,55 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
       done_nodes[k] = k == nb - 1 ? n_t : (std::upper_bound(rp + 1, rp + n_t + 1, c1) - (rp + 1));  // rp[i + 1] <= c1
       if (have_next) done_nodes[k] = node_cuts[k + 1];  // inherited batches: exactly their node range
     }
-    cudaMemcpyAsync(d_query.p, done_nodes.data(), sizeof(int64_t) * (size_t)nb, cudaMemcpyHostToDevice, st);
-    ++g_launches; rep_lower_bound_kernel<<<blocks_for(nb, 128), 128, 0, st>>>(d_rep.as<int>(), K, d_query.as<int64_t>(), nb, d_query.as<int64_t>() + nb);
-    cudaMemcpyAsync(done_blocks.data(), d_query.as<int64_t>() + nb, sizeof(int64_t) * (size_t)nb, cudaMemcpyDeviceToHost, st);
-    rc = check_cuda(cudaStreamSynchronize(st));
+    WL_ALLOC(d_query, sizeof(int64_t) * (size_t)nb + sizeof(u64) * (size_t)(nb + 1));
     if (rc) break;
+    {
+      // blocks whose first node lies before done_nodes[k]: one pass over the representative flags
+      u64* d_counts = (u64*)(d_query.as<int64_t>() + nb);
+      std::vector<u64> h_counts(nb + 1);
+      cudaMemcpyAsync(d_query.p, done_nodes.data(), sizeof(int64_t) * (size_t)nb, cudaMemcpyHostToDevice, st);
+      cudaMemsetAsync(d_counts, 0, sizeof(u64) * (size_t)(nb + 1), st);
+      ++g_launches; count_reps_kernel<<<blocks_for(n_t, 256), 256, 0, st>>>(n_t, d_isrep.as<unsigned char>(), d_query.as<int64_t>(), nb, d_counts);
+      cudaMemcpyAsync(h_counts.data(), d_counts, sizeof(u64) * (size_t)(nb + 1), cudaMemcpyDeviceToHost, st);
+      rc = check_cuda(cudaStreamSynchronize(st));
+      if (rc) break;
+      int64_t run = 0;
+      for (int k = 0; k < nb; ++k) {
+        run += (int64_t)h_counts[k];
+        done_blocks[k] = run;
+      }
+    }
+    int64_t longest_cut_row = 0;  // a row cut by a batch border stays in the table until its last piece arrives
+    for (int k = 1; k < nb; ++k) {
+      const int64_t r = (std::upper_bound(rp, rp + n_t + 1, cuts[k]) - rp) - 1;
+      if (r >= 0 && r < n_t && rp[r] < cuts[k]) longest_cut_row = std::max(longest_cut_row, rp[r + 1] - rp[r]);
+    }
+    const int64_t out_cap = max_edges + longest_cut_row;  // entries one emission can hold
+    const u64 qslots = quot_table_slots(out_cap);
+    // window of per-block counters: the blocks emitted together, plus the one whose row is still open
+    int64_t win = 2;
+    {
+      int64_t prev = 0;
+      for (int k = 0; k < nb; ++k) {
+        win = std::max(win, done_blocks[k] - prev + 2);
+        prev = std::max(prev, done_blocks[k]);
+      }
+    }
+    WL_ALLOC(d_cnt, sizeof(int) * (size_t)win);
+    WL_ALLOC(d_cursor, sizeof(int) * (size_t)win);
+    for (int b = 0; b < 2; ++b) WL_ALLOC(d_qrp[b], sizeof(int64_t) * (size_t)(win + 1));
+    WL_ALLOC(d_qtab, sizeof(u64) * 2 * qslots);
+    for (int b = 0; b < 2; ++b) {
+      WL_ALLOC(d_qcol[b], sizeof(int) * (size_t)out_cap);
+      WL_ALLOC(d_qwt[b], sizeof(u32) * (size_t)out_cap);
+    }
+    WL_ALLOC(d_sbsum, sizeof(u64) * (size_t)((win + kScanC - 1) / kScanC + 2));
+    WL_ALLOC(d_long, sizeof(int) * (size_t)(max_edges / kQuotLongRow + 2));
+    if (debug) std::fprintf(stderr, "[wl_refine_batched] outer %d device memory %.2f GB (cap %.2f GB)%s\n", outer, used_iter / 1073741824.0, device_cap_bytes / 1073741824.0, rc ? " -> WL_ENOMEM" : "");
+    if (rc) break;
+    cudaMemsetAsync(d_cnt.p, 0, sizeof(int) * (size_t)win, st);
+    cudaMemsetAsync(d_cursor.p, 0, sizeof(int) * (size_t)win, st);
+    cudaMemsetAsync(d_qtab.p, 0, sizeof(u64) * 2 * qslots, st);
     // inherit: block map and workspace of the next iteration's local refinement (one "piece" per emission)
     std::vector<int64_t> next_edge_cuts(1, 0), next_node_cuts(1, 0);
     int64_t base_next = 0;
@@ -1471,6 +1530,7 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
         prev = std::max(prev, done_blocks[k]);
       }
       WL_ALLOC(d_Hnext, sizeof(int) * (size_t)K);
+      WL_ALLOC(d_isrep_next, (size_t)K);
       WL_ALLOC(d_ws2, make_layout(max_piece_rows, out_cap).bytes);
       if (rc) break;
     }
@@ -1493,7 +1553,7 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
     // Alg. 2 lines 7-10 of the NEXT iteration on a piece of quotient rows that is still on the device: nodes b_lo .. b_hi of
     // the quotient, whole rows.  Runs on its own stream next to the insertion of the following batch (and next to the copy
     // of the piece to the host); the host waits inside refine_core, which is why it is called after that insertion has
-    // been queued.
+    // been queued.  The piece's blocks get canonical ids inside the piece, so the next block map is canonical as it is.
     struct Piece {
       bool valid;
       int64_t b_lo, b_hi, tot, q_off;
@@ -1506,14 +1566,15 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
       const int64_t nr = pending.b_hi - pending.b_lo;
       cudaStreamWaitEvent(side_st, ev_emit[pending.ob], 0);
       if (pending.tot == 0) {  // edgeless nodes only: one block (Eq. 3)
-        ++g_launches; fill_kernel<<<blocks_for(nr, 256), 256, 0, side_st>>>(nr, d_Hnext.as<int>() + pending.b_lo, (int)base_next);
+        ++g_launches; one_block_kernel<<<blocks_for(nr, 256), 256, 0, side_st>>>(nr, (int)base_next, d_Hnext.as<int>() + pending.b_lo, d_isrep_next.as<unsigned char>() + pending.b_lo);
         base_next += 1;
+        cudaEventRecord(ev_piece[pending.ob], side_st);
         return WL_OK;
       }
       wl_csr lg;
       lg.n = nr;
       lg.m = pending.tot;
-      lg.row_ptr = d_qrp.as<int64_t>() + pending.b_lo;  // global positions q_off .. q_off + tot
+      lg.row_ptr = d_qrp[pending.ob].as<int64_t>();  // global positions q_off .. q_off + tot
       lg.col_idx = d_qcol[pending.ob].as<int>() - pending.q_off;
       lg.weights = d_qwt[pending.ob].as<u32>() - pending.q_off;
       wl_options lo{};
@@ -1526,7 +1587,11 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
       int prc = refine_core(&lg, nullptr, seed, &lo, /*ranged=*/true, (int)pending.b_lo, (int)pending.b_hi, K, pending.q_off,
                             d_ws2.p, L2.bytes, L2, side_st, &cr);
       if (prc) return prc;
-      ++g_launches; merge_kernel<<<blocks_for(nr, 256), 256, 0, side_st>>>(nr, cr.colour, (int)base_next, d_Hnext.as<int>() + pending.b_lo);
+      char* wsb = (char*)d_ws2.p;
+      int* first_l = (int*)(wsb + L2.o_tmp);
+      launch_canonical(L2, nr, cr.colour, d_Hnext.as<int>() + pending.b_lo, first_l, (int*)(wsb + L2.o_rep), (int*)(wsb + L2.o_bsum),
+                       (u64*)(wsb + L2.o_scal) + kScalCanon, side_st);
+      ++g_launches; merge_canon_kernel<<<blocks_for(nr, 256), 256, 0, side_st>>>(nr, cr.colour, first_l, (int)base_next, d_Hnext.as<int>() + pending.b_lo, d_isrep_next.as<unsigned char>() + pending.b_lo);
       base_next += cr.k;
       edges_streamed += cr.edges_streamed;
       ms_spmv += cr.ms_spmv;
@@ -1534,9 +1599,9 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
       ms_spmv_kernel += cr.ms_spmv_kernel;
       spmv_alg_bytes += cr.spmv_alg_bytes;
       spmv_launches += cr.spmv_launches;
-      // the emission buffer may be overwritten once this piece is refined (emission + 2 waits on the stream `st`)
+      // the emission buffers may be overwritten once this piece is refined (emission + 2 waits on the stream `st`)
       cudaEventRecord(ev_piece[pending.ob], side_st);
-      return WL_OK;
+      return check_cuda(cudaStreamSynchronize(side_st));  // d_ws2 is reused by the next piece
     };
     int64_t q_off = 0, emitted_blocks = 0;
     int n_emit = 0;
@@ -1545,7 +1610,6 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
       cudaError_t e = cudaDeviceSynchronize();
       if (e != cudaSuccess) std::fprintf(stderr, "[wl_refine_batched] outer %d batch %d: %s -> %s\n", outer, k, what, cudaGetErrorString(e));
     };
-    checkpoint("block_rep / lower_bound", -1);
     upload_quot(0, 0);
     for (int k = 0; k < nb && !rc; ++k) {
       const int buf = k & 1;
@@ -1555,11 +1619,12 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
         upload_quot(k + 1, buf ^ 1);
       }
       cudaStreamWaitEvent(st, ev_up[buf], 0);
+      const int64_t wb = emitted_blocks;  // window base: block wb is index 0 of the counters
       if (c1 > c0 && nz[k] > na[k]) {
         // rows that cross a cut arrive in pieces: the kernel clips every row to [c0, c1)
         launch_quot_insert(na[k], nz[k] - na[k], d_rp[buf].as<int64_t>(), c0, c1, d_col[buf].as<int>() - c0,
-                           weighted ? d_wt[buf].as<u32>() - c0 : nullptr, d_Hc.as<int>(), d_rep.as<int>(), d_qtab.as<u64>(),
-                           qslots - 1, d_cnt.as<int>(), d_long.as<int>(), (u32*)(d_misc.as<u64>() + 16), st);
+                           weighted ? d_wt[buf].as<u32>() - c0 : nullptr, d_Hc.as<int>(), nullptr, d_isrep.as<unsigned char>(),
+                           d_qtab.as<u64>(), qslots - 1, d_cnt.as<int>() - wb, d_long.as<int>(), (u32*)(d_misc.as<u64>() + 16), st);
       }
       cudaEventRecord(ev_ins[buf], st);
       checkpoint("insert", k);
@@ -1568,8 +1633,12 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
       // row ends at or before c1 and that were not emitted yet
       const int64_t b_lo = emitted_blocks, b_hi = done_blocks[k];
       if (b_hi > b_lo) {
-        launch_scan32(d_cnt.as<int>() + b_lo, b_hi - b_lo, q_off, d_qrp.as<int64_t>() + b_lo, d_sbsum.as<u64>(),
-                      d_misc.as<u64>() + 8, st);
+        const int ob = n_emit & 1;
+        if (n_emit >= 2) {
+          cudaStreamWaitEvent(st, ev_down[ob], 0);  // the rows emitted two emissions ago are on the host ...
+          if (inherit) cudaStreamWaitEvent(st, ev_piece[ob], 0);  // ... and refined
+        }
+        launch_scan32(d_cnt.as<int>(), b_hi - b_lo, q_off, d_qrp[ob].as<int64_t>(), d_sbsum.as<u64>(), d_misc.as<u64>() + 8, st);
         cudaMemcpyAsync(hs + kNumScal + 1, d_misc.as<u64>() + 8, sizeof(u64), cudaMemcpyDeviceToHost, st);
         rc = check_cuda(cudaStreamSynchronize(st));
         if (rc) break;
@@ -1579,15 +1648,15 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
           rc = WL_ECUDA;  // unreachable: a quotient has at most the entries and nodes of its graph
           break;
         }
-        const int ob = n_emit & 1;
-        if (n_emit >= 2) {
-          cudaStreamWaitEvent(st, ev_down[ob], 0);  // the rows emitted two emissions ago are on the host ...
-          if (inherit) cudaStreamWaitEvent(st, ev_piece[ob], 0);  // ... and refined
-        }
         ++n_emit;
-        ++g_launches; quot_emit_kernel<<<blocks_for((int64_t)qslots, 256), 256, 0, st>>>(d_qtab.as<u64>(), qslots, d_qrp.as<int64_t>(), q_off, d_cursor.as<int>(), d_qcol[ob].as<int>(), d_qwt[ob].as<u32>(), (int)b_lo, (int)b_hi);
+        ++g_launches; quot_emit_kernel<<<blocks_for((int64_t)qslots, 256), 256, 0, st>>>(d_qtab.as<u64>(), qslots, d_qrp[ob].as<int64_t>() - b_lo, q_off, d_cursor.as<int>() - b_lo, d_qcol[ob].as<int>(), d_qwt[ob].as<u32>(), (int)b_lo, (int)b_hi);
         cudaEventRecord(ev_emit[ob], st);
         checkpoint("emit", k);
+        // the window moves on: the counter of the block whose row is still open becomes index 0
+        ++g_launches; window_carry_kernel<<<1, 1, 0, st>>>(d_cnt.as<int>(), b_hi - b_lo, (int*)(d_misc.as<u64>() + 24), 0);
+        cudaMemsetAsync(d_cnt.p, 0, sizeof(int) * (size_t)(b_hi - b_lo + 1), st);
+        cudaMemsetAsync(d_cursor.p, 0, sizeof(int) * (size_t)(b_hi - b_lo + 1), st);
+        ++g_launches; window_carry_kernel<<<1, 1, 0, st>>>(d_cnt.as<int>(), b_hi - b_lo, (int*)(d_misc.as<u64>() + 24), 1);
         cudaStreamWaitEvent(down_st, ev_emit[ob], 0);
         // in place from the second quotient on: q_off + tot <= c1, and everything below c1 has been uploaded already
         if (tot) {
@@ -1595,8 +1664,7 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
           cudaMemcpyAsync(hq.wt + q_off, d_qwt[ob].p, sizeof(u32) * (size_t)tot, cudaMemcpyDeviceToHost, down_st);
           bytes_d2h += (sizeof(int) + sizeof(u32)) * tot;
         }
-        cudaMemcpyAsync(nrp + b_lo, d_qrp.as<int64_t>() + b_lo, sizeof(int64_t) * (size_t)(b_hi - b_lo + 1),
-                        cudaMemcpyDeviceToHost, down_st);
+        cudaMemcpyAsync(nrp + b_lo, d_qrp[ob].p, sizeof(int64_t) * (size_t)(b_hi - b_lo + 1), cudaMemcpyDeviceToHost, down_st);
         bytes_d2h += sizeof(int64_t) * (b_hi - b_lo + 1);
         cudaEventRecord(ev_down[ob], down_st);
         if (inherit) {  // refined while the next batch is being inserted (refine_piece)
@@ -1634,9 +1702,13 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
       node_cuts.swap(next_node_cuts);
       next_base_id = base_next;
       if (d_Hnext_keep.p) cudaFree(d_Hnext_keep.p);
-      d_Hnext_keep.p = d_Hnext.p;  // survives this iteration's buffers
+      if (d_isrep_keep.p) cudaFree(d_isrep_keep.p);
+      d_Hnext_keep.p = d_Hnext.p;  // survive this iteration's buffers
       d_Hnext_keep.bytes = d_Hnext.bytes;
       d_Hnext.p = nullptr;
+      d_isrep_keep.p = d_isrep_next.p;
+      d_isrep_keep.bytes = d_isrep_next.bytes;
+      d_isrep_next.p = nullptr;
       have_next = true;
     }
   }
@@ -1680,7 +1752,7 @@ static double batched_budget(int64_t n, int64_t m, int64_t mb) {
   double slots = 1024;
   while (slots < 2.0 * (double)mb) slots *= 2;
   const double rows = m > 0 ? (double)n * (double)mb / (double)m + 1 : (double)n;
-  return 32.0 * (double)n + 32.0 * (double)mb + 16.0 * slots + 80.0 * rows + (double)(1 << 20);
+  return 14.0 * (double)n + 32.0 * (double)mb + 16.0 * slots + 100.0 * rows + (double)(1 << 20);
 }
 
 extern "C" {
