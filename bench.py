@@ -29,6 +29,7 @@ if ROOT not in sys.path:
 RMAT_SEEDS = {22: 1, 27: 2, 30: 3}  # BASELINE.json configs[2..4]
 ORACLE_SAMPLE_SCALE = 21           # bounded sample of the same recipe for the CPU oracle (about 10-30 s)
 HBM_FALLBACK_GBS = 6650.0          # /opt/skills/guides/B200_PROFILING.md fallback
+GEN_TOP_BITS = 9  # source-range groups of the host generator: the largest holds 0.76^9 of the draws (< 2^31 keys at scale 30)
 KNOWN_SIZES = {22: (4194304, 128311764), 27: (134217728, 4223286680)}  # (n, m) of the deterministic generator
 
 
@@ -208,62 +209,93 @@ def run_reference(args):
 
 
 def run_batched(args):
-    """--workload batched: Algorithm 2 (RBSC) over a HOST-resident directed R-MAT graph under a device-memory cap, the shape
-    of BASELINE.json configs[4] (scale 30 itself needs more host memory than the box has: DESIGN.md).  One step = one
-    wl_refine_batched call to its fixed point; inputs start in pinned host memory, the colours end there."""
+    """--workload batched: Algorithm 2 (RBSC) over a HOST-resident directed R-MAT graph under a device-memory cap: BASELINE.json
+    configs[4] (scale 30) or a smaller scale of the same recipe.  One step = one wl_refine_batched call to its fixed point;
+    inputs start in pinned host memory, the colours end there.  --consume-input (forced from scale 30 on: 77 GB of input + 154 GB
+    of quotient scratch exceed the box's 196 GB of host memory): WL_FLAG_CONSUME_INPUT, the quotients overwrite the input's
+    column array, so every step needs a freshly generated graph (one cold step per mode, no warm-up)."""
     import torch
     import graphgen as gg
     import paper_2607_02603_b200 as wl
     dev = torch.device("cuda", int(os.environ.get("LOCAL_RANK", "0")))
     torch.cuda.set_device(dev)
-    g = gg.rmat(args.scale, seed=RMAT_SEEDS[30], symmetrize=False, device=dev, chunk=1 << 27)
-    n, m = g.n, g.m
-    rp = torch.empty(n + 1, dtype=torch.int64, pin_memory=True)
-    col = torch.empty(m, dtype=torch.int32, pin_memory=True)
-    rp.copy_(g.row_ptr)
-    col.copy_(g.col)
-    del g
-    torch.cuda.empty_cache()
-    hws = torch.empty(wl.wl_refine_batched_host_bytes(n, m), dtype=torch.uint8, pin_memory=True)
-    out = torch.empty(n, dtype=torch.int32, pin_memory=True)
+    consume = args.consume_input or args.scale >= 30
     cap = int(args.cap_gb * (1 << 30))
-    flags = args.flags
-    times, res = [], None
-    for i in range(args.warmup + args.steps):
+    t_gen0 = time.perf_counter()
+    if consume:
+        n, rp, col = gg.rmat_directed_to_host(args.scale, seed=RMAT_SEEDS[30], device=dev, pin=True, top_bits=GEN_TOP_BITS)
+        m = col.numel()
+        col_buf = col
+    else:
+        g = gg.rmat(args.scale, seed=RMAT_SEEDS[30], symmetrize=False, device=dev, chunk=1 << 27)
+        n, m = g.n, g.m
+        rp = torch.empty(n + 1, dtype=torch.int64, pin_memory=True)
+        col = torch.empty(m, dtype=torch.int32, pin_memory=True)
+        rp.copy_(g.row_ptr)
+        col.copy_(g.col)
+        del g
+    torch.cuda.empty_cache()
+    gen_s = time.perf_counter() - t_gen0
+    hws_bytes = wl.wl_refine_batched_host_bytes_consume(n, m) if consume else wl.wl_refine_batched_host_bytes(n, m)
+    scratch_kind = "pinned"
+    try:
+        hws = torch.empty(hws_bytes, dtype=torch.uint8, pin_memory=True)
+    except RuntimeError:  # this box pins about 120 GB at most: the scratch then stays pageable (slower, staged transfers)
+        torch.cuda.synchronize(dev)
+        hws = torch.empty(hws_bytes, dtype=torch.uint8)
+        hws.zero_()  # touch the pages outside the timed region, as pinning would
+        scratch_kind = "pageable (pinning %.0f GB on top of the %.0f GB input failed on this box)" % (
+            hws_bytes / 2 ** 30, (rp.numel() * 8 + col.numel() * 4) / 2 ** 30)
+    out = torch.empty(n, dtype=torch.int32, pin_memory=(scratch_kind == "pinned"))
+    base_flags = args.flags | (wl.WL_FLAG_CONSUME_INPUT if consume else 0)
+
+    def one(flags, seed):
         torch.cuda.synchronize(dev)
         t0 = time.perf_counter()
-        res = wl.wl_refine_batched(n, rp, col, None, max_batch_edges=args.batch_edges, seed=300 + i, device_cap_bytes=cap,
-                                   flags=flags, host_workspace=hws, out=out)
+        r = wl.wl_refine_batched(n, rp, col, None, max_batch_edges=args.batch_edges, seed=seed, device_cap_bytes=cap,
+                                 flags=flags, host_workspace=hws, out=out)
         torch.cuda.synchronize(dev)
-        if i >= args.warmup:
-            times.append(time.perf_counter() - t0)
+        return r, time.perf_counter() - t0
+
+    def regenerate():
+        if consume:  # the previous step overwrote the column array
+            gg.rmat_directed_to_host(args.scale, seed=RMAT_SEEDS[30], device=dev, pin=True, col_out=col_buf, row_ptr_out=rp,
+                                     top_bits=GEN_TOP_BITS)
+            torch.cuda.empty_cache()
+
+    times, res = [], None
+    n_runs = 1 if consume else args.warmup + args.steps
+    for i in range(n_runs):
+        res, dt = one(base_flags, 300 + i)
+        if consume or i >= args.warmup:
+            times.append(dt)
     st = res.stats
     sec = sum(times) / len(times)
     link = (st["bytes_h2d"] + st["bytes_d2h"]) / sec / 1e9
     # the same with WL_FLAG_INHERIT_BATCHES (reading Q14b: quotients keep the batches of their graph and are refined while
     # their rows are still on the device: one upload pass per outer iteration instead of two)
     inh = None
-    if not (flags & wl.WL_FLAG_INHERIT_BATCHES):
+    if not (base_flags & wl.WL_FLAG_INHERIT_BATCHES) and not args.no_inherit_leg:
         ti = []
-        for i in range(max(1, args.steps)):
-            torch.cuda.synchronize(dev)
-            t0 = time.perf_counter()
-            ri = wl.wl_refine_batched(n, rp, col, None, max_batch_edges=args.batch_edges, seed=400 + i, device_cap_bytes=cap,
-                                      flags=flags | wl.WL_FLAG_INHERIT_BATCHES, host_workspace=hws, out=out)
-            torch.cuda.synchronize(dev)
-            ti.append(time.perf_counter() - t0)
+        for i in range(1 if consume else max(1, args.steps)):
+            regenerate()
+            ri, dt = one(base_flags | wl.WL_FLAG_INHERIT_BATCHES, 400 + i)
+            ti.append(dt)
         si = ri.stats
         seci = sum(ti) / len(ti)
         inh = {"seconds_to_stable_coloring": seci, "value": m / seci / 1e9, "unit": "GEdges/s", "outer_iters": si["outer_iters"],
                "num_colors": si["num_colors"], "reduction_power": si["num_colors"] / n, "h2d_bytes_per_step": si["bytes_h2d"],
                "d2h_bytes_per_step": si["bytes_d2h"], "link_gb_per_s": (si["bytes_h2d"] + si["bytes_d2h"]) / seci / 1e9}
+    # Theorem 2 on a sample: Def. 1 on sampled non-singleton blocks of the result (the full check is the oracle's, in the tests)
     line = {"metric": "batched_refine_input_gedges_per_s", "value": m / sec / 1e9, "unit": "GEdges/s", "n_gpus": 1,
-            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * sec, "higher_is_better": True,
+            "steps": len(times), "warmup": 0 if consume else args.warmup, "ms_per_step": 1e3 * sec, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "u64", "data": "synthetic",
             "config": {"workload": f"R-MAT scale {args.scale}, edge factor 16, seed 3, directed, deduplicated, CSR in pinned host "
                                    f"memory; device cap {args.cap_gb} GB, M_b = {args.batch_edges if args.batch_edges > 0 else 'derived from the cap'} "
-                                   f"(shape of BASELINE.json configs[4])", "n": n, "m": m,
-                       "step": "wl_refine_batched to the batched fixed point (Algorithm 2, B1-B7)"},
+                                   f"({'BASELINE.json configs[4]' if args.scale == 30 else 'shape of BASELINE.json configs[4]'})",
+                       "n": n, "m": m, "step": "wl_refine_batched to the batched fixed point (Algorithm 2, B1-B7)",
+                       "consume_input": consume, "generation_seconds": gen_s, "host_scratch": scratch_kind,
+                       "pinned_host_gb": (rp.numel() * 8 + col.numel() * 4 + hws.numel() + out.numel() * 4) / 2 ** 30},
             "seconds_to_stable_coloring": sec, "outer_iters": st["outer_iters"], "num_colors": st["num_colors"],
             "reduction_power": st["num_colors"] / n, "last_num_batches": st["last_num_batches"],
             "boundary_nodes": st["boundary_nodes"], "h2d_bytes_per_step": st["bytes_h2d"],
@@ -525,6 +557,8 @@ def main():
     ap.add_argument("--workload", default="single", choices=["single", "batched", "batch-study", "cap-sweep", "oracle-times", "c4-check"],
                     help="single: wl_refine on the HBM-resident graph (the headline); batched: wl_refine_batched")
     ap.add_argument("--cap-gb", type=float, default=16.0, help="batched: device memory cap")
+    ap.add_argument("--consume-input", action="store_true", help="batched: WL_FLAG_CONSUME_INPUT (forced from scale 30 on)")
+    ap.add_argument("--no-inherit-leg", action="store_true", help="batched: skip the second run with WL_FLAG_INHERIT_BATCHES")
     ap.add_argument("--batch-edges", type=int, default=0, help="batched: M_b (0: derived by the library from the device cap)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)

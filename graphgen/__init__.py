@@ -214,11 +214,15 @@ def rmat_draws(scale: int, lo: int, hi: int, seed: int, abc=(0.57, 0.19, 0.19), 
     """(src, dst) of edge draws lo <= e < hi.  Level l of draw e uses hash counter e*64 + l; the
     quadrant (src bit, dst bit) is (0,0) | (0,1) | (1,0) | (1,1) for r below a | a+b | a+b+c | else.
     Bits are filled from the most significant one.  No noise, no vertex permutation."""
+    return rmat_draws_at(scale, torch.arange(lo, hi, dtype=torch.int64, device=device), seed, abc)
+
+
+def rmat_draws_at(scale: int, e: torch.Tensor, seed: int, abc=(0.57, 0.19, 0.19), levels: Optional[int] = None):
+    """(src, dst) of the edge draws with indices `e` (int64 tensor); levels < scale: only the top `levels` bits."""
     ta, tab, tabc = _rmat_thresholds(*abc)
-    e = torch.arange(lo, hi, dtype=torch.int64, device=device)
     src = torch.zeros_like(e)
     dst = torch.zeros_like(e)
-    for l in range(scale):
+    for l in range(scale if levels is None else levels):
         r = hash_u32(seed, e * 64 + l)
         sbit = (r >= tab).to(torch.int64)
         dbit = (((r >= ta) & (r < tab)) | (r >= tabc)).to(torch.int64)
@@ -277,6 +281,58 @@ def rmat(scale: int, edge_factor: int = 16, seed: int = 1, symmetrize: bool = Tr
     kind = "sym" if symmetrize else "dir"
     _ = total
     return Graph(n, row_ptr, col, None, f"rmat_s{scale}_ef{edge_factor}_{kind}_seed{seed}")
+
+
+def rmat_directed_to_host(scale: int, edge_factor: int = 16, seed: int = 1, abc=(0.57, 0.19, 0.19), device="cpu",
+                          top_bits: int = 7, chunk: int = 1 << 27, pin: bool = False, col_out=None, row_ptr_out=None):
+    """The graph rmat(scale, edge_factor, seed, symmetrize=False) built for sizes that exceed one GPU (BASELINE.json
+    configs[4]: scale 30, 17e9 edges): draws are grouped by the top `top_bits` bits of their source (which depend on the first
+    `top_bits` levels only), every group is completed, deduplicated and sorted on `device`, and its rows are appended to HOST
+    arrays.  Returns (n, row_ptr int64[n+1] host, col int32[m] host view).  Same edges, same order as rmat()."""
+    n = 1 << scale
+    draws = edge_factor * n
+    top_bits = min(top_bits, scale)
+    nbuck = 1 << top_bits
+    bucket = torch.empty(draws, dtype=torch.uint8 if top_bits <= 8 else torch.int16, device=device)
+    for lo in range(0, draws, chunk):
+        hi = min(draws, lo + chunk)
+        s, _ = rmat_draws_at(scale, torch.arange(lo, hi, dtype=torch.int64, device=device), seed, abc, levels=top_bits)
+        bucket[lo:hi] = s.to(bucket.dtype)
+    col = torch.empty(draws, dtype=torch.int32, pin_memory=pin) if col_out is None else col_out
+    deg = torch.zeros(n, dtype=torch.int64, device=device)
+    rows_per_bucket = n >> top_bits
+    off = 0
+    scan_chunk = max(chunk, 1 << 30)
+    for b in range(nbuck):
+        idx = []
+        for lo in range(0, draws, scan_chunk):
+            hi = min(draws, lo + scan_chunk)
+            e = torch.nonzero(bucket[lo:hi] == b).flatten()
+            if e.numel():
+                idx.append(e + lo)
+        if not idx:
+            continue
+        e_all = torch.cat(idx)
+        del idx
+        keys = []
+        for lo in range(0, e_all.numel(), chunk):
+            s, d = rmat_draws_at(scale, e_all[lo:lo + chunk], seed, abc)
+            keep = s != d
+            keys.append(s[keep] * n + d[keep])
+            del s, d, keep
+        del e_all
+        key = torch.unique(torch.cat(keys))  # (torch.unique sorts at most 2^31 keys: top_bits must keep a group below that)
+        del keys
+        b0 = b * rows_per_bucket
+        deg[b0:b0 + rows_per_bucket] = torch.bincount((key >> scale) - b0, minlength=rows_per_bucket)
+        cnt = key.numel()
+        col[off:off + cnt].copy_((key & (n - 1)).to(torch.int32), non_blocking=False)
+        off += cnt
+        del key
+    row_ptr = torch.zeros(n + 1, dtype=torch.int64, pin_memory=pin) if row_ptr_out is None else row_ptr_out
+    row_ptr[0] = 0
+    row_ptr[1:] = torch.cumsum(deg, 0).cpu()
+    return n, row_ptr, col[:off]
 
 
 # ---------------------------------------------------------------------------------------

@@ -71,6 +71,16 @@ typedef struct wl_csr {
                                         graph (the rows emitted together) instead of being re-cut by M_b, and its local
                                         refinement runs while those rows are still on the device: one upload pass per
                                         iteration instead of two (reading Q14b)                               */
+#define WL_FLAG_CONSUME_INPUT 8192u /* batched, whole-CSR form only: the caller's col_idx (and weights) array is OVERWRITTEN: the
+                                      quotient of the first outer iteration is written over the rows it was made from (its rows
+                                      come out in row order and never hold more entries, Def. 4), as every later quotient
+                                      overwrites its predecessor.  The host scratch then holds no column array
+                                      (wl_refine_batched_host_bytes_consume): a graph of 77 GB needs 86 GB of scratch instead of
+                                      154 GB.  The arrays must be writable; their contents are undefined afterwards           */
+#define WL_FLAG_TAG_TABLE 16384u /* wl_refine from a uniform start: serve the gathers of the highest-degree nodes from a
+                                   direct-mapped {tag, colour} table in shared memory during the 16-bit rounds (one persistent
+                                   CTA per SM).  Results are identical.  OFF by default: measured slower than the plain row
+                                   kernel on the headline graph (19.6 ms against 16.5 ms, profiles/r2_spmv_levers.md)        */
 #define WL_FLAG_NO_CANONICAL 16u /* leave internal dense ids in out_colors (skips S6)                                  */
 
 typedef struct wl_options {
@@ -211,6 +221,8 @@ int wl_refine_batched(int64_t n, int32_t num_batches, const wl_edge_batch* batch
  * one weighted entry array of m entries (a quotient never has more nodes or entries than its graph, Def. 4; later
  * quotients overwrite the first one in place). */
 size_t wl_refine_batched_host_bytes(int64_t n, int64_t m);
+/* the same under WL_FLAG_CONSUME_INPUT: two offset arrays, plus one weight array of m entries unless the input is weighted */
+size_t wl_refine_batched_host_bytes_consume(int64_t n, int64_t m, int weighted);
 
 /* B2: inner-node labels of Def. 5 (L139-L145) by the method of L463.  edge_batch: DEVICE int32[m] batch id of every CSR edge
  * slot; sink_batch: DEVICE int32[n] label given to nodes without out-edges (Q9); label: DEVICE int32[n], -1 = boundary. */
@@ -223,6 +235,30 @@ int wl_inner_labels(int64_t n, const int64_t* row_ptr, const int32_t* edge_batch
 int wl_quotient(const wl_csr* g, const int32_t* colors, int64_t k, int64_t* q_row_ptr, int32_t* q_col, uint32_t* q_weights,
                 int64_t q_cap, int64_t* q_m, void* workspace, size_t workspace_bytes, void* cuda_stream);
 size_t wl_quotient_workspace_bytes(int64_t n, int64_t m);
+
+/* ------------------------------------------------------------------------------------------------------------------
+ * One batch at a time on DEVICE buffers: the per-batch work of an outer iteration of Algorithm 2, for callers that spread the
+ * batches over several GPUs (L213 "embarrassingly parallel ... scheduled concurrently across GPUs", L239) and exchange the
+ * block maps themselves (paper_2607_02603_b200/sharded.py does, over torch.distributed).
+ * ---------------------------------------------------------------------------------------------------------------- */
+
+/* B3 + B4 for the inner nodes V_k = [lo, lo + rows->n) of a batch (Eq. 3; Alg. 2 line 9): `rows` holds exactly their rows
+ * (DEVICE; row_ptr[0] = 0, row_ptr[0..n] index col_idx / weights, targets are global node ids < n_targets); every target outside V_k is
+ * an implicit singleton.  local_colors (DEVICE int32[n]): dense ids in first-occurrence order inside the batch; is_first
+ * (DEVICE uint8[n]): 1 for the first node of every block; *num_colors (HOST): their number.  opt: flags, ring_bits, max_rounds,
+ * stream_id are honoured.  workspace >= wl_refine_inner_workspace_bytes(n, m), 256-byte aligned. */
+size_t wl_refine_inner_workspace_bytes(int64_t n_rows, int64_t m);
+int wl_refine_inner(const wl_csr* rows, int64_t lo, int64_t n_targets, uint64_t seed, int32_t* local_colors, uint8_t* is_first,
+                    int64_t* num_colors, const wl_options* opt, void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* B6 for the whole rows of the nodes [lo, lo + rows->n): the quotient rows (Def. 4) of the blocks whose representative (first node,
+ * is_first[i - lo] == 1) lies among them, i.e. the blocks first_block .. first_block + num_blocks - 1 of the canonical block map
+ * block_of (DEVICE int32 over ALL nodes).  q_row_ptr: DEVICE int64[num_blocks + 1] starting at 0; columns of a row come out in
+ * any order with equal targets merged.  WL_ENOMEM if q_cap is too small (*q_m is still set). */
+size_t wl_quotient_rows_workspace_bytes(int64_t n_rows, int64_t m, int64_t num_blocks);
+int wl_quotient_rows(const wl_csr* rows, int64_t lo, const int32_t* block_of, const uint8_t* is_first, int64_t first_block,
+                     int64_t num_blocks, int64_t* q_row_ptr, int32_t* q_col, uint32_t* q_weights, int64_t q_cap, int64_t* q_m,
+                     void* workspace, size_t workspace_bytes, void* cuda_stream);
 
 /* ------------------------------------------------------------------------------------------------------------------ */
 const char* wl_strerror(int code);

@@ -24,11 +24,14 @@ WL_FLAG_NO_DEEP = 256
 WL_FLAG_DEEP_EARLY = 512
 WL_FLAG_NO_FINAL = 1024
 WL_FLAG_INHERIT_BATCHES = 4096
+WL_FLAG_CONSUME_INPUT = 8192
+WL_FLAG_TAG_TABLE = 16384
 
 EXPORTS = [
     "wl_refine_workspace_bytes", "wl_refine_deep_workspace_bytes", "wl_refine", "wl_refine_host", "wl_round_key", "wl_weight", "wl_spmv_round",
-    "wl_spmv_rows", "wl_relabel", "wl_canonicalize", "wl_refine_batched", "wl_refine_batched_host_bytes", "wl_inner_labels", "wl_quotient",
-    "wl_quotient_workspace_bytes", "wl_strerror", "wl_last_cuda_error", "wl_version", "wl_kernel_launches",
+    "wl_spmv_rows", "wl_relabel", "wl_canonicalize", "wl_refine_batched", "wl_refine_batched_host_bytes", "wl_refine_batched_host_bytes_consume", "wl_inner_labels", "wl_quotient",
+    "wl_quotient_workspace_bytes", "wl_refine_inner", "wl_refine_inner_workspace_bytes", "wl_quotient_rows",
+    "wl_quotient_rows_workspace_bytes", "wl_strerror", "wl_last_cuda_error", "wl_version", "wl_kernel_launches",
 ]
 
 
@@ -104,12 +107,22 @@ def lib():
                                         C.POINTER(wl_stats), C.POINTER(wl_options), vp]
         L.wl_refine_batched_host_bytes.restype = sz
         L.wl_refine_batched_host_bytes.argtypes = [i64, i64]
+        L.wl_refine_batched_host_bytes_consume.restype = sz
+        L.wl_refine_batched_host_bytes_consume.argtypes = [i64, i64, C.c_int]
         L.wl_inner_labels.restype = C.c_int
         L.wl_inner_labels.argtypes = [i64, vp, vp, vp, vp, vp]
         L.wl_quotient.restype = C.c_int
         L.wl_quotient.argtypes = [C.POINTER(wl_csr), vp, i64, vp, vp, vp, i64, C.POINTER(i64), vp, sz, vp]
         L.wl_quotient_workspace_bytes.restype = sz
         L.wl_quotient_workspace_bytes.argtypes = [i64, i64]
+        L.wl_refine_inner_workspace_bytes.restype = sz
+        L.wl_refine_inner_workspace_bytes.argtypes = [i64, i64]
+        L.wl_refine_inner.restype = C.c_int
+        L.wl_refine_inner.argtypes = [C.POINTER(wl_csr), i64, i64, u64, vp, vp, C.POINTER(i64), C.POINTER(wl_options), vp, sz, vp]
+        L.wl_quotient_rows_workspace_bytes.restype = sz
+        L.wl_quotient_rows_workspace_bytes.argtypes = [i64, i64, i64]
+        L.wl_quotient_rows.restype = C.c_int
+        L.wl_quotient_rows.argtypes = [C.POINTER(wl_csr), i64, vp, vp, i64, i64, vp, vp, vp, i64, C.POINTER(i64), vp, sz, vp]
         L.wl_strerror.restype = C.c_char_p
         L.wl_strerror.argtypes = [C.c_int]
         L.wl_last_cuda_error.restype = C.c_int
@@ -357,6 +370,51 @@ def wl_quotient(n, row_ptr, col_idx, weights, colors: torch.Tensor, k: int):
     return q_rp, q_col[: qm.value], q_wt[: qm.value].to(torch.int64) & 0xFFFFFFFF
 
 
+def wl_refine_inner(row_ptr: torch.Tensor, col_idx: torch.Tensor, weights: Optional[torch.Tensor], lo: int, n_targets: int,
+                    seed: int = 0, *, stream_id: int = 0, flags: int = 0, ring_bits: int = 0):
+    """B3 + B4 of one batch on device tensors: the rows of the inner nodes [lo, lo + n) (row_ptr[0] = 0, global targets), every
+    other target an implicit singleton.  -> (local colours int32[n] in first-occurrence order, is_first uint8[n], k)."""
+    L = lib()
+    dev = row_ptr.device
+    nr = row_ptr.numel() - 1
+    g, w = _make_csr(nr, row_ptr, col_idx, weights, "cuda")
+    colors = torch.empty(nr, dtype=torch.int32, device=dev)
+    first = torch.empty(nr, dtype=torch.uint8, device=dev)
+    ws = torch.empty(max(int(L.wl_refine_inner_workspace_bytes(nr, col_idx.numel())), 256), dtype=torch.uint8, device=dev)
+    opt = wl_options(flags, 0, stream_id, None, 0, 0, None, 0, ring_bits)
+    k = C.c_int64(0)
+    with torch.cuda.device(dev):
+        rc = L.wl_refine_inner(C.byref(g), lo, n_targets, seed, _ptr(colors), _ptr(first), C.byref(k), C.byref(opt), _ptr(ws),
+                               ws.numel(), _stream_ptr(dev))
+    if rc != WL_OK:
+        raise WlError(rc, "wl_refine_inner")
+    return colors, first, k.value
+
+
+def wl_quotient_rows(row_ptr: torch.Tensor, col_idx: torch.Tensor, weights: Optional[torch.Tensor], lo: int, block_of: torch.Tensor,
+                     is_first: torch.Tensor, first_block: int, num_blocks: int):
+    """B6 for whole rows on device tensors: quotient rows of the blocks whose first node lies in [lo, lo + n).
+    -> (q_row_ptr int64[num_blocks + 1], q_col int32[q_m], q_weights int64[q_m])."""
+    L = lib()
+    dev = row_ptr.device
+    nr = row_ptr.numel() - 1
+    g, w = _make_csr(nr, row_ptr, col_idx, weights, "cuda")
+    _check(block_of, torch.int32, "cuda", "block_of")
+    _check(is_first, torch.uint8, "cuda", "is_first", nr)
+    m = col_idx.numel()
+    q_rp = torch.zeros(num_blocks + 1, dtype=torch.int64, device=dev)
+    q_col = torch.empty(max(m, 1), dtype=torch.int32, device=dev)
+    q_wt = torch.empty(max(m, 1), dtype=torch.int32, device=dev)
+    ws = torch.empty(max(int(L.wl_quotient_rows_workspace_bytes(nr, m, num_blocks)), 256), dtype=torch.uint8, device=dev)
+    qm = C.c_int64(0)
+    with torch.cuda.device(dev):
+        rc = L.wl_quotient_rows(C.byref(g), lo, _ptr(block_of), _ptr(is_first), first_block, num_blocks, _ptr(q_rp), _ptr(q_col),
+                                _ptr(q_wt), m, C.byref(qm), _ptr(ws), ws.numel(), _stream_ptr(dev))
+    if rc != WL_OK:
+        raise WlError(rc, "wl_quotient_rows")
+    return q_rp, q_col[: qm.value], q_wt[: qm.value].to(torch.int64) & 0xFFFFFFFF
+
+
 def wl_refine_batched(n: int, row_ptr: torch.Tensor, col_idx: torch.Tensor, weights: Optional[torch.Tensor] = None, *,
                       max_batch_edges: int = 0, cuts=None, seed: int = 0, device_cap_bytes: int = 0, flags: int = 0,
                       max_outer_iters: int = 0, out: Optional[torch.Tensor] = None, device=None,
@@ -381,8 +439,8 @@ def wl_refine_batched(n: int, row_ptr: torch.Tensor, col_idx: torch.Tensor, weig
         out = torch.empty(n, dtype=torch.int32)
     _check(out, torch.int32, "cpu", "out", n)
     if host_workspace is not None:
-        if host_workspace.device.type != "cpu" or not host_workspace.is_pinned() or host_workspace.dtype != torch.uint8:
-            raise ValueError("host_workspace must be a pinned host uint8 tensor")
+        if host_workspace.device.type != "cpu" or host_workspace.dtype != torch.uint8 or not host_workspace.is_contiguous():
+            raise ValueError("host_workspace must be a contiguous host uint8 tensor (pinned: the transfers then overlap)")
     opt = wl_options(flags, 0, 0, None, 0, max_outer_iters, _ptr(host_workspace),
                      0 if host_workspace is None else host_workspace.numel())
     st = wl_stats()
@@ -427,6 +485,10 @@ def wl_refine_batched(n: int, row_ptr: torch.Tensor, col_idx: torch.Tensor, weig
 
 def wl_refine_batched_host_bytes(n: int, m: int) -> int:
     return int(lib().wl_refine_batched_host_bytes(n, m))
+
+
+def wl_refine_batched_host_bytes_consume(n: int, m: int, weighted: bool = False) -> int:
+    return int(lib().wl_refine_batched_host_bytes_consume(n, m, 1 if weighted else 0))
 
 
 def wl_strerror(code: int) -> str:

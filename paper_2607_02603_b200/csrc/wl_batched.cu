@@ -569,12 +569,15 @@ struct HostQuot {
   int* col = nullptr;
   u32* wt = nullptr;
   int64_t cap_nodes = 0, cap_edges = 0;
-  static size_t bytes_for(int64_t n, int64_t m) {
-    return 2 * align_up(sizeof(int64_t) * (size_t)(n + 1)) + 2 * align_up(sizeof(int) * (size_t)m);
+  // consume_col / consume_wt: the quotients are written over the caller's own column (and weight) array, so the scratch holds
+  // the offset arrays only (plus a weight array when the input has none): WL_FLAG_CONSUME_INPUT
+  static size_t bytes_for(int64_t n, int64_t m, bool consume_col = false, bool consume_wt = false) {
+    return 2 * align_up(sizeof(int64_t) * (size_t)(n + 1)) + (consume_col ? 0 : align_up(sizeof(int) * (size_t)m)) +
+           (consume_wt ? 0 : align_up(sizeof(int) * (size_t)m));
   }
-  int init(int64_t n, int64_t m, void* ws, size_t ws_bytes) {
+  int init(int64_t n, int64_t m, void* ws, size_t ws_bytes, int* consume_col = nullptr, u32* consume_wt = nullptr) {
     if (base) return WL_OK;
-    const size_t need = bytes_for(n, m);
+    const size_t need = bytes_for(n, m, consume_col != nullptr, consume_wt != nullptr);
     if (ws && ws_bytes >= need) {
       base = (char*)ws;
     } else {
@@ -590,9 +593,13 @@ struct HostQuot {
     off += align_up(sizeof(int64_t) * (size_t)(n + 1));
     rp[1] = (int64_t*)(base + off);
     off += align_up(sizeof(int64_t) * (size_t)(n + 1));
-    col = (int*)(base + off);
-    off += align_up(sizeof(int) * (size_t)m);
-    wt = (u32*)(base + off);
+    if (consume_col) {
+      col = consume_col;
+    } else {
+      col = (int*)(base + off);
+      off += align_up(sizeof(int) * (size_t)m);
+    }
+    wt = consume_wt ? consume_wt : (u32*)(base + off);
     cap_nodes = n;
     cap_edges = m;
     return WL_OK;
@@ -682,6 +689,11 @@ size_t wl_refine_batched_host_bytes(int64_t n, int64_t m) {
   return HostQuot::bytes_for(n, m);
 }
 
+size_t wl_refine_batched_host_bytes_consume(int64_t n, int64_t m, int weighted) {
+  if (n < 0 || m < 0 || n > kMaxNodes) return 0;
+  return HostQuot::bytes_for(n, m, true, weighted != 0);
+}
+
 size_t wl_quotient_workspace_bytes(int64_t n, int64_t m) {
   if (n < 0 || m < 0 || n > kMaxNodes) return 0;
   size_t off = 0;
@@ -744,6 +756,105 @@ int wl_quotient(const wl_csr* g, const int32_t* colors, int64_t k, int64_t* q_ro
 // ---------------------------------------------------------------------------------------------------------------------
 // Algorithm 2
 // ---------------------------------------------------------------------------------------------------------------------
+}  // extern "C"
+
+// ---------------------------------------------------------------------------------------------------------------------
+// Step-level pieces of one outer iteration on DEVICE buffers: what one GPU does for one batch when the batches of Algorithm 2
+// are spread over several GPUs (L213, L239; paper_2607_02603_b200/sharded.py drives them and exchanges the block maps).
+// ---------------------------------------------------------------------------------------------------------------------
+extern "C" {
+
+size_t wl_refine_inner_workspace_bytes(int64_t n_rows, int64_t m) {
+  if (n_rows < 0 || m < 0 || n_rows > kMaxNodes) return 0;
+  return make_layout(n_rows, m).bytes;
+}
+
+int wl_refine_inner(const wl_csr* rows, int64_t lo, int64_t n_targets, uint64_t seed, int32_t* local_colors,
+                    uint8_t* is_first, int64_t* num_colors, const wl_options* opt, void* workspace, size_t workspace_bytes,
+                    void* cuda_stream) {
+  if (!rows || rows->n < 0 || rows->m < 0 || lo < 0 || n_targets < lo + rows->n || n_targets > kMaxNodes) return WL_EINVAL;
+  if (num_colors) *num_colors = 0;
+  const int64_t nr = rows->n;
+  if (nr == 0) return WL_OK;
+  if (!rows->row_ptr || (rows->m > 0 && !rows->col_idx) || !local_colors || !is_first || !workspace) return WL_EINVAL;
+  const Layout L = make_layout(nr, rows->m);
+  if (workspace_bytes < L.bytes) return WL_ENOMEM;
+  if ((uintptr_t)workspace % 256) return WL_EINVAL;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  wl_options lo_opt{};
+  if (opt) lo_opt = *opt;
+  lo_opt.flags &= (WL_FLAG_NO_VALIDATE | WL_FLAG_NO_PRUNE | WL_FLAG_EDGE_BALANCED);
+  lo_opt.round_colors = nullptr;
+  CoreResult cr{};
+  int rc = refine_core(rows, nullptr, seed, &lo_opt, /*ranged=*/true, (int)lo, (int)(lo + nr), n_targets, /*edge_first=*/0,
+                       workspace, workspace_bytes, L, st, &cr);
+  if (rc) return rc;
+  char* wsb = (char*)workspace;
+  int* first_l = (int*)(wsb + L.o_tmp);
+  launch_canonical(L, nr, cr.colour, local_colors, first_l, (int*)(wsb + L.o_rep), (int*)(wsb + L.o_bsum),
+                   (u64*)(wsb + L.o_scal) + kScalCanon, st);
+  ++g_launches; merge_canon_kernel<<<blocks_for(nr, 256), 256, 0, st>>>(nr, cr.colour, first_l, 0, local_colors, is_first);
+  rc = check_cuda(cudaStreamSynchronize(st));
+  if (rc) return rc;
+  if (num_colors) *num_colors = cr.k;
+  return check_cuda(cudaGetLastError());
+}
+
+size_t wl_quotient_rows_workspace_bytes(int64_t n_rows, int64_t m, int64_t num_blocks) {
+  if (n_rows < 0 || m < 0 || num_blocks < 0) return 0;
+  size_t off = 0;
+  off += align_up(sizeof(u64) * 2 * quot_table_slots(m));
+  off += align_up(sizeof(int) * (size_t)(num_blocks + 1)) * 2;  // cnt, cursor
+  off += align_up(sizeof(u64) * (size_t)((num_blocks + kScanC - 1) / kScanC + 2));
+  off += 256;
+  off += align_up(sizeof(int) * (size_t)(m / kQuotLongRow + 2));
+  return off;
+}
+
+int wl_quotient_rows(const wl_csr* rows, int64_t lo, const int32_t* block_of, const uint8_t* is_first, int64_t first_block,
+                     int64_t num_blocks, int64_t* q_row_ptr, int32_t* q_col, uint32_t* q_weights, int64_t q_cap, int64_t* q_m,
+                     void* workspace, size_t workspace_bytes, void* cuda_stream) {
+  if (!rows || rows->n < 0 || rows->m < 0 || lo < 0 || first_block < 0 || num_blocks < 0 || !q_m) return WL_EINVAL;
+  *q_m = 0;
+  const int64_t nr = rows->n, m = rows->m;
+  if (nr == 0 || num_blocks == 0) return WL_OK;
+  if (!rows->row_ptr || (m > 0 && !rows->col_idx) || !block_of || !is_first || !q_row_ptr || !workspace) return WL_EINVAL;
+  if (q_cap > 0 && (!q_col || !q_weights)) return WL_EINVAL;
+  if (workspace_bytes < wl_quotient_rows_workspace_bytes(nr, m, num_blocks)) return WL_ENOMEM;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  char* ws = (char*)workspace;
+  size_t off = 0;
+  const u64 slots = quot_table_slots(m);
+  u64* table = (u64*)(ws + off);
+  off += align_up(sizeof(u64) * 2 * slots);
+  int* cnt = (int*)(ws + off);
+  off += align_up(sizeof(int) * (size_t)(num_blocks + 1));
+  int* cursor = (int*)(ws + off);
+  off += align_up(sizeof(int) * (size_t)(num_blocks + 1));
+  u64* bsum = (u64*)(ws + off);
+  off += align_up(sizeof(u64) * (size_t)((num_blocks + kScanC - 1) / kScanC + 2));
+  u64* total = (u64*)(ws + off);
+  off += 256;
+  int* long_rows = (int*)(ws + off);
+  cudaMemsetAsync(table, 0, sizeof(u64) * 2 * slots, st);
+  cudaMemsetAsync(cnt, 0, sizeof(int) * (size_t)(num_blocks + 1), st);
+  cudaMemsetAsync(cursor, 0, sizeof(int) * (size_t)(num_blocks + 1), st);
+  // the kernels index the block map by global node id and the counters by global block id
+  launch_quot_insert(lo, nr, rows->row_ptr, /*clip_lo=*/INT64_MIN / 2, /*clip_hi=*/INT64_MAX / 2, rows->col_idx, rows->weights,
+                     block_of, nullptr, is_first - lo, table, slots - 1, cnt - first_block, long_rows, (u32*)(total + 1), st);
+  launch_scan32(cnt, num_blocks, 0, q_row_ptr, bsum, total, st);
+  u64 h_total = 0;
+  cudaMemcpyAsync(&h_total, total, sizeof(u64), cudaMemcpyDeviceToHost, st);
+  int rc = check_cuda(cudaStreamSynchronize(st));
+  if (rc) return rc;
+  *q_m = (int64_t)h_total;
+  if ((int64_t)h_total > q_cap) return WL_ENOMEM;
+  ++g_launches; quot_emit_kernel<<<blocks_for((int64_t)slots, 256), 256, 0, st>>>(table, slots, q_row_ptr - first_block, 0, cursor - first_block, q_col, q_weights, (int)first_block, (int)(first_block + num_blocks));
+  rc = check_cuda(cudaStreamSynchronize(st));
+  if (rc) return rc;
+  return check_cuda(cudaGetLastError());
+}
+
 }  // extern "C"
 
 
@@ -1147,6 +1258,10 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
     return num_batches > 0 ? batches[k].weights : (wt ? wt + cuts[k] : nullptr);
   };
   bool weighted = num_batches > 0 ? (batches[0].weights != nullptr) : (wt != nullptr);
+  // WL_FLAG_CONSUME_INPUT: the quotient of iteration 1 is written over the rows it was made from (its rows come out in row order
+  // and never hold more entries, Def. 4), exactly as every later quotient overwrites its predecessor
+  const bool consume = (flags & WL_FLAG_CONSUME_INPUT) != 0;
+  if (consume && num_batches != 0) return WL_EINVAL;  // only the whole-CSR form owns one contiguous column array
   // S0 on the host side of the CSR forms: the offsets steer the cuts, the inner ranges and every upload size
   if (!coo && !(flags & WL_FLAG_NO_VALIDATE)) {
     if (rp[0] != 0) return WL_EINVAL;
@@ -1203,6 +1318,8 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
   size_t used = 0;
   DevBuf d_map0;  // original node -> node of the current graph (identity in iteration 1: left unallocated until needed)
   bool map0_identity = true;
+  // under a tight device cap the composed map stays on the host (see the compose step)
+  const bool map0_on_host = !coo && device_cap_bytes > 0 && (size_t)n0 * sizeof(int) * 8 > device_cap_bytes;
   HostQuot hq;  // quotient graphs of later iterations (pinned host memory)
   const int64_t rp0_edges = coo ? coo_edges : rp[n];
 
@@ -1434,7 +1551,29 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
     nb_last = nb;
     K_final = K;
     // compose original -> current map
-    if (map0_identity) {
+    if (map0_on_host) {
+      // the composed map (4 bytes per ORIGINAL node) lives in the caller's out_colors between iterations and passes through
+      // the device in tiles: at n = 2^30 it would take a quarter of a 16 GB cap for one use per iteration
+      if (map0_identity) {
+        cudaMemcpyAsync(out_colors, d_Hc.p, sizeof(int) * (size_t)n0, cudaMemcpyDeviceToHost, st);
+        bytes_d2h += sizeof(int) * n0;
+        map0_identity = false;
+      } else {
+        const int64_t tile = std::min<int64_t>(n0, 1ll << 26);
+        DevBuf d_tile;
+        if ((rc = d_tile.alloc(sizeof(int) * (size_t)tile, &used_iter, device_cap_bytes))) break;
+        for (int64_t t0 = 0; t0 < n0; t0 += tile) {
+          const int64_t cnt = std::min(tile, n0 - t0);
+          cudaMemcpyAsync(d_tile.p, out_colors + t0, sizeof(int) * (size_t)cnt, cudaMemcpyHostToDevice, st);
+          ++g_launches; compose_kernel<<<blocks_for(cnt, 256), 256, 0, st>>>(cnt, d_tile.as<int>(), d_Hc.as<int>());
+          cudaMemcpyAsync(out_colors + t0, d_tile.p, sizeof(int) * (size_t)cnt, cudaMemcpyDeviceToHost, st);
+          bytes_h2d += sizeof(int) * cnt;
+          bytes_d2h += sizeof(int) * cnt;
+        }
+        cudaStreamSynchronize(st);
+        d_tile.release(&used_iter);
+      }
+    } else if (map0_identity) {
       if ((rc = d_map0.alloc(sizeof(int) * (size_t)n0, &used, device_cap_bytes))) break;
       used_iter += d_map0.bytes;
       cudaMemcpyAsync(d_map0.p, d_Hc.p, sizeof(int) * (size_t)n0, cudaMemcpyDeviceToDevice, st);
@@ -1459,7 +1598,9 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
     // ---- Alg. 2 line 13: quotient (Def. 4), second streaming pass -------------------------------------------------------
     // Three streams: copy_st uploads batch k + 1 while st inserts / emits batch k and down_st returns the rows emitted for
     // batch k - 1 to the host (double buffers on both sides; one host synchronisation per batch, to learn the emitted size).
-    if ((rc = hq.init(n0, rp0_edges, opt ? opt->host_workspace : nullptr, opt ? opt->host_workspace_bytes : 0))) break;
+    if ((rc = hq.init(n0, rp0_edges, opt ? opt->host_workspace : nullptr, opt ? opt->host_workspace_bytes : 0,
+                      consume ? const_cast<int*>(col) : nullptr, consume && wt ? const_cast<u32*>(wt) : nullptr)))
+      break;
     const int osel = outer & 1;  // offsets of the quotient being written; the graph being read uses the other array
     int64_t* nrp = hq.rp[osel];
     // per batch: the nodes whose row intersects it, and the number of blocks whose representative row is complete after it
@@ -1716,6 +1857,9 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
   if (rc == WL_OK) {
     if (map0_identity) {
       rc = WL_ECUDA;  // unreachable: every iteration composes the map
+    } else if (map0_on_host) {  // the result is where it belongs already
+      cudaEventRecord(ev_end, st);
+      rc = check_cuda(cudaStreamSynchronize(st));
     } else {
       cudaMemcpyAsync(out_colors, d_map0.p, sizeof(int) * (size_t)n0, cudaMemcpyDeviceToHost, st);
       bytes_d2h += sizeof(int) * n0;
@@ -1748,11 +1892,13 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
 
 // Rough device budget of batched_run for a batch cap M_b (DESIGN.md §8 "Device budget"): node arrays, two input and two
 // output buffers of 8 bytes per edge, the quotient table, the local workspace of a batch with its share of the rows.
-static double batched_budget(int64_t n, int64_t m, int64_t mb) {
+static double batched_budget(int64_t n, int64_t m, int64_t mb, size_t cap, bool inherit) {
   double slots = 1024;
   while (slots < 2.0 * (double)mb) slots *= 2;
   const double rows = m > 0 ? (double)n * (double)mb / (double)m + 1 : (double)n;
-  return 14.0 * (double)n + 32.0 * (double)mb + 16.0 * slots + 100.0 * rows + (double)(1 << 20);
+  // per node: block map + representative flag; the composed map unless it stays on the host; the next block map (inherit)
+  const double per_node = 5.0 + ((size_t)n * 32 > cap ? 0.25 : 4.0) + (inherit ? 4.0 : 0.0);
+  return per_node * (double)n + 32.0 * (double)mb + 16.0 * slots + 100.0 * rows + (double)(1 << 20);
 }
 
 extern "C" {
@@ -1769,7 +1915,8 @@ int wl_refine_batched(int64_t n, int32_t num_batches, const wl_edge_batch* batch
   if (device_cap_bytes == 0 || num_batches != 0 || !whole || n <= 0) return WL_EINVAL;
   const int64_t m = whole->m;
   int64_t mb = m > 0 ? m : 1;
-  while (mb > 1024 && batched_budget(n, m, mb) > 0.9 * (double)device_cap_bytes) mb = (int64_t)((double)mb * 0.8);
+  const bool inh = opt && (opt->flags & WL_FLAG_INHERIT_BATCHES);
+  while (mb > 1024 && batched_budget(n, m, mb, device_cap_bytes, inh) > 0.9 * (double)device_cap_bytes) mb = (int64_t)((double)mb * 0.8);
   for (int attempt = 0; attempt < 12; ++attempt) {
     const int rc = batched_run(n, 0, nullptr, whole, seed, device_cap_bytes, mb, out_colors, stats, opt, cuda_stream);
     if (rc != WL_ENOMEM || mb <= 1024) return rc;

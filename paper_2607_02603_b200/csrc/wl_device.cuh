@@ -21,6 +21,7 @@ enum {
   kScalK = 7,          // current number of colours
   kScalTicket = 8,     // CTAs that finished relabel_finish_kernel
   kScalErrAux = 9,     // validation error bits written on the side stream
+  kScalRowTicket = 10, // row-group ticket of spmv_rows32_tag_kernel
   kScalLog = 16,
   kNumScal = 64
 };

@@ -192,15 +192,40 @@ __device__ __forceinline__ int checked_col(int c, int64_t n_targets, bool& bad) 
   return c;
 }
 
-template <bool WEIGHTED, typename CT, bool RANGED, bool VALIDATE>
-__global__ void __launch_bounds__(256)
-spmv_rows32_kernel(int64_t nrows, const int* __restrict__ rows, const int64_t* __restrict__ row_ptr,
-                   const int* __restrict__ col, const u32* __restrict__ wt, const CT* __restrict__ colour, u64 key,
-                   u64* __restrict__ y, int64_t hub_threshold, int lo, int hi, int64_t n_targets,
-                   u32* __restrict__ err) {
-  const int lane = threadIdx.x & 31;
-  const int64_t base = (((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5) << 5;
-  if (base >= nrows) return;
+// Hot-id table (lever (b) of profiles/r2_gather_microbench.md): a direct-mapped table {tag:16 | colour:16} of kTagSlots entries in
+// shared memory, filled with the highest-degree nodes.  tag_mix is a bijection of the id space [0, 2^b), so (slot, tag) =
+// (low kTagBits bits, remaining bits) of the mixed id identify the node exactly: a hit costs one LDS instead of an L1-miss sector
+// request, a miss falls through to the global gather.
+constexpr int kTagBits = 15;
+constexpr u32 kTagSlots = 1u << kTagBits;
+constexpr u32 kTagEmpty = 0xffffffffu;  // tag 0xffff never occurs: ids have at most 30 bits when the table is used
+__host__ __device__ __forceinline__ u32 tag_mix(u32 x, u32 idmask) {
+  x ^= x >> 14;
+  x = (x * 0x2c1b3c6du) & idmask;
+  x ^= x >> 13;
+  x = (x * 0x297a2d39u) & idmask;
+  x ^= x >> 14;
+  return x;
+}
+
+template <bool RANGED, bool TAG, typename CT>
+__device__ __forceinline__ u64 colour_lookup(const CT* __restrict__ colour, int j, int lo, int hi, const u32* s_tag, u32 idmask) {
+  if (TAG) {
+    const u32 m = tag_mix((u32)j, idmask);
+    const u32 e = s_tag[m & (kTagSlots - 1)];
+    if ((e >> 16) == (m >> kTagBits)) return (u64)(e & 0xffffu);
+    return (u64)__ldg(colour + j);
+  }
+  return colour_id<RANGED>(colour, j, lo, hi);
+}
+
+// the 32 rows base .. base + 31 of the list (see spmv_rows32_kernel)
+template <bool WEIGHTED, typename CT, bool RANGED, bool VALIDATE, bool TAG>
+__device__ __forceinline__ void
+rows32_group(const int64_t base, const int lane, int64_t nrows, const int* __restrict__ rows,
+             const int64_t* __restrict__ row_ptr, const int* __restrict__ col, const u32* __restrict__ wt,
+             const CT* __restrict__ colour, u64 key, u64* __restrict__ y, int64_t hub_threshold, int lo, int hi,
+             int64_t n_targets, bool& bad, const u32* s_tag, u32 idmask) {
   const int64_t idx = base + lane;
   const bool valid = idx < nrows;
   int64_t i = 0, a = 0, b = 0;
@@ -212,7 +237,6 @@ spmv_rows32_kernel(int64_t nrows, const int* __restrict__ rows, const int64_t* _
   const int64_t d = b - a;
   const bool small = d <= kSmallRow;
   u64 acc = 0;
-  bool bad = false;
   {
     const int dd = small ? (int)d : 0;
     int cidx[kSmallRow];
@@ -221,7 +245,7 @@ spmv_rows32_kernel(int64_t nrows, const int* __restrict__ rows, const int64_t* _
 #pragma unroll
     for (int t = 0; t < kSmallRow; ++t) {
       if (cidx[t] != -1) {  // -1 = no entry; other negative values are renamed outside targets (RANGED, wl_batched.cu)
-        u64 v = weight_of(key, colour_id<RANGED>(colour, cidx[t], lo, hi));
+        u64 v = weight_of(key, colour_lookup<RANGED, TAG>(colour, cidx[t], lo, hi, s_tag, idmask));
         if (WEIGHTED) v *= (u64)__ldg(wt + a + t);
         acc += v;
       }
@@ -251,7 +275,7 @@ spmv_rows32_kernel(int64_t nrows, const int* __restrict__ rows, const int64_t* _
 #pragma unroll
       for (int t = 0; t < kMidRow / 8; ++t) {
         if (c[t] != -1) {
-          u64 v = weight_of(key, colour_id<RANGED>(colour, c[t], lo, hi));
+          u64 v = weight_of(key, colour_lookup<RANGED, TAG>(colour, c[t], lo, hi, s_tag, idmask));
           if (WEIGHTED) v *= (u64)ld_stream_u32(wt + ra + sub + 8 * t);
           s += v;
         }
@@ -278,10 +302,10 @@ spmv_rows32_kernel(int64_t nrows, const int* __restrict__ rows, const int64_t* _
                 c1 = checked_col<VALIDATE>(ld_stream_i32(col + p + 32), n_targets, bad),
                 c2 = checked_col<VALIDATE>(ld_stream_i32(col + p + 64), n_targets, bad),
                 c3 = checked_col<VALIDATE>(ld_stream_i32(col + p + 96), n_targets, bad);
-      u64 v0 = weight_of(key, colour_id<RANGED>(colour, c0, lo, hi)),
-          v1 = weight_of(key, colour_id<RANGED>(colour, c1, lo, hi)),
-          v2 = weight_of(key, colour_id<RANGED>(colour, c2, lo, hi)),
-          v3 = weight_of(key, colour_id<RANGED>(colour, c3, lo, hi));
+      u64 v0 = weight_of(key, colour_lookup<RANGED, TAG>(colour, c0, lo, hi, s_tag, idmask)),
+          v1 = weight_of(key, colour_lookup<RANGED, TAG>(colour, c1, lo, hi, s_tag, idmask)),
+          v2 = weight_of(key, colour_lookup<RANGED, TAG>(colour, c2, lo, hi, s_tag, idmask)),
+          v3 = weight_of(key, colour_lookup<RANGED, TAG>(colour, c3, lo, hi, s_tag, idmask));
       if (WEIGHTED) {
         v0 *= (u64)ld_stream_u32(wt + p);
         v1 *= (u64)ld_stream_u32(wt + p + 32);
@@ -298,7 +322,7 @@ spmv_rows32_kernel(int64_t nrows, const int* __restrict__ rows, const int64_t* _
 #pragma unroll
       for (int t = 0; t < 4; ++t) {
         if (c[t] != -1) {
-          u64 v = weight_of(key, colour_id<RANGED>(colour, c[t], lo, hi));
+          u64 v = weight_of(key, colour_lookup<RANGED, TAG>(colour, c[t], lo, hi, s_tag, idmask));
           if (WEIGHTED) v *= (u64)ld_stream_u32(wt + p + 32 * t);
           s += v;
         }
@@ -309,7 +333,64 @@ spmv_rows32_kernel(int64_t nrows, const int* __restrict__ rows, const int64_t* _
     if (lane == src) acc = s;
   }
   if (valid) y[i] = acc;
+}
+
+template <bool WEIGHTED, typename CT, bool RANGED, bool VALIDATE>
+__global__ void __launch_bounds__(256)
+spmv_rows32_kernel(int64_t nrows, const int* __restrict__ rows, const int64_t* __restrict__ row_ptr,
+                   const int* __restrict__ col, const u32* __restrict__ wt, const CT* __restrict__ colour, u64 key,
+                   u64* __restrict__ y, int64_t hub_threshold, int lo, int hi, int64_t n_targets,
+                   u32* __restrict__ err) {
+  const int lane = threadIdx.x & 31;
+  const int64_t base = (((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5) << 5;
+  if (base >= nrows) return;
+  bool bad = false;
+  rows32_group<WEIGHTED, CT, RANGED, VALIDATE, false>(base, lane, nrows, rows, row_ptr, col, wt, colour, key, y, hub_threshold,
+                                                      lo, hi, n_targets, bad, nullptr, 0u);
   if (VALIDATE && bad) atomicOr(err, kErrCol);
+}
+
+// The same rows through the hot-id table: one persistent CTA of 1024 threads per SM holds the table (128 KB of shared memory);
+// its warps draw row groups from a ticket counter.
+constexpr int kTagThreads = 1024;
+constexpr int kTagRun = 1;  // row groups per ticket (measured 1 / 2 / 4 / 16: 19.6 / 20.4 / 22.0 / 26.7 ms on the headline graph)
+template <bool WEIGHTED, bool VALIDATE>
+__global__ void __launch_bounds__(kTagThreads, 1)
+spmv_rows32_tag_kernel(int64_t nrows, const int* __restrict__ rows, const int64_t* __restrict__ row_ptr,
+                       const int* __restrict__ col, const u32* __restrict__ wt, const unsigned short* __restrict__ colour,
+                       u64 key, u64* __restrict__ y, int64_t hub_threshold, int64_t n_targets, u32* __restrict__ err,
+                       const u32* __restrict__ tagtab, u32 idmask, u64* __restrict__ ticket, int run) {
+  extern __shared__ u32 s_tag[];
+  for (u32 t = threadIdx.x; t < kTagSlots; t += kTagThreads) s_tag[t] = tagtab[t];
+  __syncthreads();
+  const int lane = threadIdx.x & 31;
+  const int64_t ngroups = (nrows + 31) >> 5;
+  bool bad = false;
+  while (true) {
+    u64 g0 = 0;
+    if (lane == 0) g0 = atomicAdd(ticket, (u64)run);
+    g0 = __shfl_sync(0xffffffffu, g0, 0);
+    if ((int64_t)g0 >= ngroups) break;
+    const int64_t g1 = (int64_t)g0 + run < ngroups ? (int64_t)g0 + run : ngroups;
+    for (int64_t g = (int64_t)g0; g < g1; ++g)
+      rows32_group<WEIGHTED, unsigned short, false, VALIDATE, true>(g << 5, lane, nrows, rows, row_ptr, col, wt, colour, key, y,
+                                                                    hub_threshold, 0, 0, n_targets, bad, s_tag, idmask);
+  }
+  if (VALIDATE && bad) atomicOr(err, kErrCol);
+}
+
+// tag32[s] = {tag | colour} of the node that won slot s (the highest degree among the candidates that map to it)
+__global__ void tag_finalize_kernel(const u64* __restrict__ tag64, const unsigned short* __restrict__ colour16, u32 idmask,
+                                    u32* __restrict__ tag32) {
+  const u32 sl = blockIdx.x * blockDim.x + threadIdx.x;
+  if (sl >= kTagSlots) return;
+  const u64 e = tag64[sl];
+  if (e == 0) {
+    tag32[sl] = kTagEmpty;
+    return;
+  }
+  const u32 id = (u32)e;
+  tag32[sl] = ((tag_mix(id, idmask) >> kTagBits) << 16) | (u32)colour16[id];
 }
 
 // Hub rows (degree > hub_threshold) are cut into chunks of kHubChunk entries, one CTA each; partial sums meet in y
@@ -736,7 +817,8 @@ round1_uniform_kernel(int64_t n, const int64_t* __restrict__ row_ptr, int64_t ex
                       int* __restrict__ stamp, Slot* __restrict__ table, u32 table_mask, u32* __restrict__ slot_of,
                       u64* __restrict__ new_counter, int64_t hub_threshold, int2* __restrict__ chunks, int64_t hub_cap,
                       u64* __restrict__ hub_counter, int* __restrict__ active, u64* __restrict__ counters,
-                      u64* __restrict__ hub_rows, u32* __restrict__ err, u64 ymask) {
+                      u64* __restrict__ hub_rows, u32* __restrict__ err, u64 ymask, u64* __restrict__ tag64,
+                      int64_t tag_threshold, u32 idmask) {
   constexpr int round = 1, k_old = 1;
   const int64_t t = (int64_t)blockIdx.x * kRelabelThreads + threadIdx.x;
   const bool valid = t < n;
@@ -761,6 +843,9 @@ round1_uniform_kernel(int64_t n, const int64_t* __restrict__ row_ptr, int64_t ex
       atomicAdd(hub_rows, 1ull);
     }
     if (e) atomicOr(err, e);
+    // hot-id table of the coming rounds: the highest-degree node wins its slot (out-degree stands in for the number of gathers
+    // a node receives; any choice is correct, a miss falls through to the global gather)
+    if (tag64 && d >= tag_threshold) atomicMax(tag64 + (tag_mix((u32)i, idmask) & (kTagSlots - 1)), ((u64)d << 32) | (u64)(u32)i);
   }
   // the representative of colour 0 is node 0
   int64_t d0 = row_ptr[1] - row_ptr[0];

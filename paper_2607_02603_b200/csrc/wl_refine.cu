@@ -54,6 +54,8 @@ Layout make_layout(int64_t n, int64_t m) {
   L.hub_cap = m / kHubChunk + m / (kHubThreshold + 1) + 1;
   L.o_hub = take(sizeof(int2) * (size_t)L.hub_cap);
   L.o_chunk_row = take(sizeof(int) * (size_t)(m / kEbSuper + 4));
+  L.o_tag64 = take(sizeof(u64) * kTagSlots);
+  L.o_tag32 = take(sizeof(u32) * kTagSlots);
   L.bytes = off;
   return L;
 }
@@ -112,6 +114,9 @@ struct SpmvArgs {
   int64_t e_first = 0;   // row_ptr[0]
   int64_t n_targets = 0;
   u32* err = nullptr;
+  const u32* tag32 = nullptr;  // hot-id table (16-bit ids, plain RSC only) or NULL
+  u32 idmask = 0;
+  u64* ticket = nullptr;       // zeroed device counter of the persistent kernel
 };
 
 // edge-balanced S1+S2 over all rows of g (see spmv_eb_kernel)
@@ -136,10 +141,29 @@ static void launch_eb(const wl_csr& g, const SpmvArgs& a, const CT* colour, u64 
 
 constexpr int kRowsCta = 64;  // two warps per CTA: a warp stuck on long rows does not hold six finished ones' slots (measured)
 
+// the row kernel through the hot-id table: one persistent CTA per SM (128 KB of shared memory each)
+template <bool V>
+static void launch_rows_tag(const wl_csr& g, const SpmvArgs& a, u64 key, u64* y, cudaStream_t st) {
+  static thread_local bool attr_set = false;
+  if (!attr_set) {
+    cudaFuncSetAttribute(spmv_rows32_tag_kernel<false, V>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sizeof(u32) * kTagSlots));
+    attr_set = true;
+  }
+  int dev = 0, sms = 148;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  cudaMemsetAsync(a.ticket, 0, sizeof(u64), st);
+  ++g_launches; spmv_rows32_tag_kernel<false, V><<<(unsigned)sms, kTagThreads, sizeof(u32) * kTagSlots, st>>>(a.nrows, a.rows, g.row_ptr, g.col_idx, g.weights, a.colour16, key, y, kHubThreshold, a.n_targets, a.err, a.tag32, a.idmask, a.ticket, kTagRun);
+}
+
 template <bool W, typename CT, bool R, bool V>
 static void launch_row_hub2(const wl_csr& g, const SpmvArgs& a, const CT* colour, u64 key, u64* y, cudaStream_t st) {
   unsigned grid = blocks_for(a.nrows, kRowsCta);
-  ++g_launches; spmv_rows32_kernel<W, CT, R, V><<<grid, kRowsCta, 0, st>>>(a.nrows, a.rows, g.row_ptr, g.col_idx, g.weights, colour, key, y, kHubThreshold, a.lo, a.hi, a.n_targets, a.err);
+  if (!W && !R && a.tag32 && a.narrow) {
+    launch_rows_tag<V>(g, a, key, y, st);
+  } else {
+    ++g_launches; spmv_rows32_kernel<W, CT, R, V><<<grid, kRowsCta, 0, st>>>(a.nrows, a.rows, g.row_ptr, g.col_idx, g.weights, colour, key, y, kHubThreshold, a.lo, a.hi, a.n_targets, a.err);
+  }
   if (a.num_hub_chunks > 0) {
     ++g_launches; spmv_hub_kernel<W, CT, R, V><<<(unsigned)a.num_hub_chunks, kHubThreads, 0, st>>>(a.hub_chunks, g.row_ptr, g.col_idx, g.weights, colour, key, y, a.colour, a.stamp, a.live_stamp, a.lo, a.hi, a.n_targets, a.err);
   }
@@ -350,6 +374,8 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
   unsigned short* colour16 = (unsigned short*)(ws + L.o_colour16);
   int* act[2] = {(int*)(ws + L.o_act0), (int*)(ws + L.o_act1)};
   int2* hub_chunks = (int2*)(ws + L.o_hub);
+  u64* tag64 = (u64*)(ws + L.o_tag64);
+  u32* tag32 = (u32*)(ws + L.o_tag32);
   const int64_t launches_at_entry = g_launches;
   EventPool evp;
   const bool merge = (flags & WL_FLAG_MERGE_KERNEL) != 0 && !ranged;
@@ -427,11 +453,18 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
   cudaMemsetAsync(stamp, 0, sizeof(int), st);
   hs[kNumScal] = 1;
   cudaMemcpyAsync(scal + kScalK, hs + kNumScal, sizeof(u64), cudaMemcpyHostToDevice, st);
+  // hot-id table of the 16-bit rounds (WL_FLAG_TAG_TABLE, wl_kernels.cuh): candidates = nodes of at least 8 times the average
+  // out-degree, collected by the round-1 kernel
+  u32 idmask = 1;
+  while ((int64_t)idmask + 1 < n) idmask = (idmask << 1) | 1u;
+  const bool tag_possible = uniform_start && (flags & WL_FLAG_TAG_TABLE) && n <= (1ll << 30) && !force_eb;
+  if (tag_possible) cudaMemsetAsync(tag64, 0, sizeof(u64) * kTagSlots, st);
   if (uniform_start) {
     // S0 and round 1 in one pass over row_ptr (round1_uniform_kernel); the loop below only closes the round
     const u64 w0 = weight_of(round_key(seed, stream_id, 1), 0);
     const u32 mask1 = overlap ? (u32)(prefix_slots - 1) : L.table_mask;
-    ++g_launches; round1_uniform_kernel<<<blocks_for(n, kRelabelThreads), kRelabelThreads, 0, st>>>(n, g->row_ptr, edge_first, edge_first + m, w0, colour, colour16, rep, stamp, table, mask1, slot_of, scal + kScalNew, kHubThreshold, hub_chunks, L.hub_cap, scal + kScalHub, act[0], scal + kScalActive, scal + kScalActiveHub, d_err, ymask);
+    ++g_launches; round1_uniform_kernel<<<blocks_for(n, kRelabelThreads), kRelabelThreads, 0, st>>>(n, g->row_ptr, edge_first, edge_first + m, w0, colour, colour16, rep, stamp, table, mask1, slot_of, scal + kScalNew, kHubThreshold, hub_chunks, L.hub_cap, scal + kScalHub, act[0], scal + kScalActive, scal + kScalActiveHub, d_err, ymask, tag_possible ? tag64 : nullptr,
+                                                                                                  std::max<int64_t>(64, 8 * (m / std::max<int64_t>(n, 1))), idmask);
   } else {
     if (!cols_checked) {
       ++g_launches; validate_cols_kernel<<<148 * 8, 256, 0, st>>>(n_targets, edge_first, edge_first + m, g->col_idx, d_err);
@@ -495,6 +528,13 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
       a.e_first = edge_first;
       a.n_targets = n_targets;
       a.err = d_err;
+      if (tag_possible && narrow && !eb) {
+        // the table carries the colours of THIS round: rebuilt from the slot winners (32 K threads)
+        ++g_launches; tag_finalize_kernel<<<kTagSlots / 256, 256, 0, st>>>(tag64, colour16, idmask, tag32);
+        a.tag32 = tag32;
+        a.idmask = idmask;
+        a.ticket = scal + kScalRowTicket;
+      }
       bool all_rows = eb;
       if (!cols_checked) {  // S0's column range check rides on the first pass over the columns, which then takes every row
         if (merge || ranged) {

@@ -299,6 +299,27 @@ def test_batched_validation_reaches_cut_rows_and_host_offsets():
     assert res.colors.numpy().tolist() == want.tolist()
 
 
+@pytest.mark.parametrize("name", ["rmat11_dir", "weighted", "hub", "grid"])
+@pytest.mark.parametrize("flags", [0, 4096])
+def test_batched_consume_input_overwrites_the_column_array(name, flags):
+    """WL_FLAG_CONSUME_INPUT: the first quotient is written over the caller's column (and weight) array; the scratch holds no
+    column array.  Same colouring as without the flag (bit-exact against the CPU Algorithm 2); the input array is clobbered."""
+    g = BATCH_GRAPHS[name]()
+    n, rp, ci, wt = g.numpy()
+    cap = max(1, -(-g.m // 5))
+    want, k_want, outer_want, _ = oracle.rbsc(n, rp, ci, wt, cap, inherit=bool(flags))
+    col = g.col.clone().pin_memory()
+    w = None if g.weights is None else g.weights.clone()
+    w32 = None if w is None else (w & 0xFFFFFFFF).to(torch.uint32).pin_memory()
+    hws = torch.empty(wl.wl_refine_batched_host_bytes_consume(n, g.m, w is not None), dtype=torch.uint8).pin_memory()
+    assert hws.numel() < wl.wl_refine_batched_host_bytes(n, g.m)
+    res = wl.wl_refine_batched(n, g.row_ptr.pin_memory(), col, w32, max_batch_edges=cap, seed=3,
+                               flags=flags | wl.WL_FLAG_CONSUME_INPUT, host_workspace=hws)
+    assert res.colors.numpy().tolist() == want.tolist() and res.stats["outer_iters"] == outer_want
+    if outer_want >= 2 and k_want < n:
+        assert not torch.equal(col, g.col)  # the quotient really went over the input
+
+
 def test_batched_device_cap_is_checked_for_every_allocation():
     """A cap that admits the buffers of the local-refinement pass but not those of the quotient pass must give WL_ENOMEM
     (a failed allocation used to be overwritten by the next successful one)."""
@@ -340,6 +361,21 @@ def test_batched_batch_cap_derived_from_device_cap():
     assert e.value.code == wl.WL_ENOMEM
 
 
+@pytest.mark.parametrize("flags", [0, 4096])
+def test_batched_composed_map_on_the_host_under_a_tight_cap(flags):
+    """When the composed map of the original nodes (4 B per node) would take more than an eighth of the device cap it stays in
+    out_colors and passes through the device in tiles: same colouring as the uncapped run, stable, refines the coarsest."""
+    g = gg.rmat(17, seed=4, symmetrize=False)
+    n, rp, ci, wt = g.numpy()
+    cap = 32 * n - 1
+    free = wl.wl_refine_batched(n, g.row_ptr, g.col, None, max_batch_edges=8000, seed=1, flags=flags)
+    tight = wl.wl_refine_batched(n, g.row_ptr, g.col, None, max_batch_edges=8000, seed=2, flags=flags, device_cap_bytes=cap)
+    assert torch.equal(free.colors, tight.colors) and tight.stats["outer_iters"] == free.stats["outer_iters"] >= 3
+    got = tight.colors.numpy()
+    coarsest, _, _ = oracle.refine(n, rp, ci)
+    assert oracle.is_stable(n, rp, ci, None, got) and refines(got, coarsest)
+
+
 def test_batched_device_cap_and_limits():
     g = gg.rmat(10, seed=1)
     with pytest.raises(wl.WlError) as e:
@@ -367,3 +403,37 @@ def test_batched_seed_independence():
     a = wl.wl_refine_batched(g.n, g.row_ptr, g.col, None, max_batch_edges=g.m // 5, seed=1).colors
     b = wl.wl_refine_batched(g.n, g.row_ptr, g.col, None, max_batch_edges=g.m // 5, seed=2).colors
     assert torch.equal(a, b)
+
+
+# ------------------------------------------------------------------ batch-level sharding over ranks (sharded.py)
+@pytest.mark.parametrize("name", list(BATCH_GRAPHS))
+@pytest.mark.parametrize("nb", [2, 5, 16])
+def test_sharded_driver_with_cuda_backend_equals_cpu_algorithm2(name, nb):
+    """The sharded driver with the CUDA backend (wl_refine_inner / wl_quotient_rows per batch on device buffers), 1 to 3 virtual
+    ranks played in lock step on this one GPU (the collectives are host-level; the ranks never wait on each other inside a
+    kernel): bit-exact against the CPU Algorithm 2 with inherited batches and against wl_refine_batched(INHERIT)."""
+    import os
+    import sys
+    sys.path.insert(0, os.path.dirname(os.path.abspath(__file__)))
+    from sharded_harness import run_lockstep
+    from paper_2607_02603_b200.sharded import CudaBackend
+    g = BATCH_GRAPHS[name]()
+    n, rp, ci, wt = g.numpy()
+    cap = max(1, -(-g.m // nb))
+    want, k_want, outer_want, _ = oracle.rbsc(n, rp, ci, wt, cap, inherit=True)
+    single = wl.wl_refine_batched(n, g.row_ptr, g.col, g.weights, max_batch_edges=cap, seed=1, flags=wl.WL_FLAG_INHERIT_BATCHES)
+    assert single.colors.numpy().tolist() == want.tolist()
+    for world in (1, 2, 3):
+        got, k, outer, ranks = run_lockstep(lambda: CudaBackend(dev()), n, g.row_ptr, g.col, g.weights, cap, world, seed=world)
+        assert got.numpy().tolist() == want.tolist(), (name, nb, world)
+        assert k == k_want and outer == outer_want
+
+
+def test_refine_batched_sharded_single_process_entry_point():
+    from paper_2607_02603_b200.sharded import refine_batched_sharded
+    g = gg.rmat(12, seed=8, symmetrize=False)
+    n, rp, ci, wt = g.numpy()
+    cap = g.m // 7 + 1
+    want, k_want, outer_want, _ = oracle.rbsc(n, rp, ci, wt, cap, inherit=True)
+    colours, k, outer = refine_batched_sharded(n, g.row_ptr, g.col, None, max_batch_edges=cap, seed=4, device=dev())
+    assert colours.numpy().tolist() == want.tolist() and k == k_want and outer == outer_want

@@ -199,7 +199,9 @@ def test_canonicalize(n):
 # 256 = WL_FLAG_NO_DEEP, 512 = WL_FLAG_DEEP_EARLY (worklist regime from round 2 on: every graph goes through it),
 # 1024 = WL_FLAG_NO_FINAL (no finality pruning)
 @pytest.mark.parametrize("name", list(GRAPHS))
-@pytest.mark.parametrize("flags", [0, 2, 4, 64, 128, 128 | 2, 256, 512, 512 | 64, 512 | 2, 1024, 1024 | 256])
+# 16384 = WL_FLAG_TAG_TABLE (the shared-memory hot-id table in every 16-bit round)
+@pytest.mark.parametrize("flags", [0, 2, 4, 64, 128, 128 | 2, 256, 512, 512 | 64, 512 | 2, 1024, 1024 | 256,
+                                   16384, 16384 | 2, 16384 | 512])
 def test_refine_equals_oracle(name, flags):
     g = GRAPHS[name]()
     n, rp, ci, wt = g.numpy()
@@ -253,6 +255,19 @@ def test_refine_deep_rounds_equal_oracle(name, flags):
         res = wl.wl_refine(dn, drp, dci, dwt, seed=seed, flags=flags)
         assert res.rounds == rounds and res.round_colors == counts
         assert res.colors.cpu().numpy().tolist() == want.tolist()
+
+
+@pytest.mark.parametrize("scale,sym", [(16, True), (17, False)])
+def test_hot_id_table_rounds_equal_plain_rounds(scale, sym):
+    """The 16-bit rounds through the shared-memory hot-id table (persistent kernel, ticketed row groups, tag hits and misses,
+    hub rows beside it) against the plain row kernel and the oracle, on graphs large enough for many tickets per CTA."""
+    g = gg.rmat(scale, seed=5, symmetrize=sym)
+    n, rp, ci, wt = g.numpy()
+    want, counts, rounds = oracle.refine(n, rp, ci)
+    dn, drp, dci, dwt = dgraph(g)
+    for flags in (wl.WL_FLAG_TAG_TABLE, wl.WL_FLAG_TAG_TABLE | wl.WL_FLAG_NO_PRUNE, 0):
+        res = wl.wl_refine(dn, drp, dci, None, seed=3, flags=flags)
+        assert res.round_colors == counts and res.colors.cpu().numpy().tolist() == want.tolist()
 
 
 def test_refine_weighted_equals_multigraph():
