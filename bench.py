@@ -717,20 +717,25 @@ def main():
         cpu_baseline = {k: cb[k] for k in ("value", "unit", "cores", "kind", "sample")}
         import oracle
         mismatches = mismatch_report(wl, gg, oracle, dev, seeds_c1=100, seeds_c3=args.mismatch_c3_seeds)
-        # union bound of the DEFAULT build on this workload (R4 / R5 make a mid-run collision permanent):
-        # sum_r N_r 2^(t - 64) / 0.6 with the pair counts of this very graph; plain Algorithm 1 (WL_FLAG_NO_DEEP |
-        # WL_FLAG_NO_FINAL) keeps the paper's 2^-32 / 0.6 per run
+        # the failure bound of the default build on this workload: plain Algorithm 1 fails only if the
+        # confirming round misses one witness pair (the paper's eps); R5 (final blocks) can make a mid-run merge permanent
+        # only if the same pair of sub-blocks collides under TWO independent keys, over all N pairs of the trajectory
         npairs = split_pairs_on_device(wl, n, g.row_ptr, g.col, results[-1].rounds, dev)
-        failure_bound = {"pairs_per_round": npairs, "pairs": sum(npairs),
-                         "default_build_union_bound_t0": sum(npairs) * 2.0 ** -64 / 0.6,
-                         "plain_algorithm1_bound": 2.0 ** -32 / 0.6,
-                         "note": "t0: coefficient differences odd (gcd term 2^t = 1, the common case on unweighted graphs); "
-                                 "worst case multiplies by 2^t <= 2^32 (Lemma 1, L418)"}
+        eps_paper = 2.0 ** -32 / 0.6
+        eps_row32 = 2.0 ** (5 - 64) / 0.6  # rows of <= 32 unit entries: coefficient differences below 2^5
+        failure_bound = {"pairs_per_round": npairs, "pairs": sum(npairs), "paper_eps_per_run": eps_paper,
+                         "default_build_bound": eps_paper + sum(npairs) * eps_row32 ** 2,
+                         "single_key_finality_would_be": sum(npairs) * 2.0 ** -64 / 0.6,
+                         "note": "default_build_bound = paper's terminal-round eps + N x (2^(5-64)/0.6)^2 for the doubly "
+                                 "confirmed final blocks; single_key_finality_would_be = the union bound of the round-1 design "
+                                 "(one sum per round, odd coefficient differences)"}
 
     last = results[-1]
     line = {
         "metric": "refine_gedges_per_s", "value": value, "unit": "GEdges/s", "n_gpus": world, "steps": args.steps,
         "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+        "scaling_kind": "replicas only: every rank refines its own copy, no data-path collective (DESIGN.md section 9); not a "
+                        "scaling curve of the method",
         "vs_baseline": None, "dtype": "u64", "data": "synthetic", "config": workload_config(args.scale, n, m),
         "rounds": last.rounds, "num_colors": last.num_colors, "round_colors": last.round_colors,
         "edges_streamed_per_step": edges_per_step,

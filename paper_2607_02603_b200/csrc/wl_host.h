@@ -22,7 +22,7 @@ struct Layout {
   u32 table_mask;
   int64_t hub_cap;
   size_t o_scal, o_colour, o_rep, o_stamp, o_tmp, o_y, o_tile_row, o_bsum, o_table, o_colour16, o_act0, o_act1, o_hub,
-      o_chunk_row, o_tag64, o_tag32, bytes;
+      o_chunk_row, o_tag64, o_tag32, o_y2, bytes;
 };
 Layout make_layout(int64_t n, int64_t m);
 

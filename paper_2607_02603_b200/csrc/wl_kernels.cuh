@@ -220,12 +220,14 @@ __device__ __forceinline__ u64 colour_lookup(const CT* __restrict__ colour, int 
 }
 
 // the 32 rows base .. base + 31 of the list (see spmv_rows32_kernel)
-template <bool WEIGHTED, typename CT, bool RANGED, bool VALIDATE, bool TAG>
+// DUAL: rows of at most kMidRow entries are also summed under a second key into y2 (the gathers are shared): the finality test
+// of compact_active_kernel wants two independent sums before it lets a block leave for good.
+template <bool WEIGHTED, typename CT, bool RANGED, bool VALIDATE, bool TAG, bool DUAL = false>
 __device__ __forceinline__ void
 rows32_group(const int64_t base, const int lane, int64_t nrows, const int* __restrict__ rows,
              const int64_t* __restrict__ row_ptr, const int* __restrict__ col, const u32* __restrict__ wt,
              const CT* __restrict__ colour, u64 key, u64* __restrict__ y, int64_t hub_threshold, int lo, int hi,
-             int64_t n_targets, bool& bad, const u32* s_tag, u32 idmask) {
+             int64_t n_targets, bool& bad, const u32* s_tag, u32 idmask, u64 key2 = 0, u64* __restrict__ y2 = nullptr) {
   const int64_t idx = base + lane;
   const bool valid = idx < nrows;
   int64_t i = 0, a = 0, b = 0;
@@ -236,7 +238,7 @@ rows32_group(const int64_t base, const int lane, int64_t nrows, const int* __res
   }
   const int64_t d = b - a;
   const bool small = d <= kSmallRow;
-  u64 acc = 0;
+  u64 acc = 0, acc2 = 0;
   {
     const int dd = small ? (int)d : 0;
     int cidx[kSmallRow];
@@ -245,9 +247,11 @@ rows32_group(const int64_t base, const int lane, int64_t nrows, const int* __res
 #pragma unroll
     for (int t = 0; t < kSmallRow; ++t) {
       if (cidx[t] != -1) {  // -1 = no entry; other negative values are renamed outside targets (RANGED, wl_batched.cu)
-        u64 v = weight_of(key, colour_lookup<RANGED, TAG>(colour, cidx[t], lo, hi, s_tag, idmask));
+        const u64 cid = colour_lookup<RANGED, TAG>(colour, cidx[t], lo, hi, s_tag, idmask);
+        u64 v = weight_of(key, cid);
         if (WEIGHTED) v *= (u64)__ldg(wt + a + t);
         acc += v;
+        if (DUAL) acc2 += weight_of(key2, cid);
       }
     }
   }
@@ -271,23 +275,34 @@ rows32_group(const int64_t base, const int lane, int64_t nrows, const int* __res
         const int64_t p = ra + sub + 8 * t;
         c[t] = p < rb ? checked_col<VALIDATE>(ld_stream_i32(col + p), n_targets, bad) : -1;
       }
-      u64 s = 0;
+      u64 s = 0, s2 = 0;
 #pragma unroll
       for (int t = 0; t < kMidRow / 8; ++t) {
         if (c[t] != -1) {
-          u64 v = weight_of(key, colour_lookup<RANGED, TAG>(colour, c[t], lo, hi, s_tag, idmask));
+          const u64 cid = colour_lookup<RANGED, TAG>(colour, c[t], lo, hi, s_tag, idmask);
+          u64 v = weight_of(key, cid);
           if (WEIGHTED) v *= (u64)ld_stream_u32(wt + ra + sub + 8 * t);
           s += v;
+          if (DUAL) s2 += weight_of(key2, cid);
         }
       }
       s += __shfl_xor_sync(0xffffffffu, s, 1);
       s += __shfl_xor_sync(0xffffffffu, s, 2);
       s += __shfl_xor_sync(0xffffffffu, s, 4);
+      if (DUAL) {
+        s2 += __shfl_xor_sync(0xffffffffu, s2, 1);
+        s2 += __shfl_xor_sync(0xffffffffu, s2, 2);
+        s2 += __shfl_xor_sync(0xffffffffu, s2, 4);
+      }
 #pragma unroll
       for (int g = 0; g < 4; ++g) {
         const int sg = __shfl_sync(0xffffffffu, src, g * 8);
         const u64 vg = __shfl_sync(0xffffffffu, s, g * 8);
         if (lane == sg) acc = vg;
+        if (DUAL) {
+          const u64 vg2 = __shfl_sync(0xffffffffu, s2, g * 8);
+          if (lane == sg) acc2 = vg2;
+        }
       }
     }
   }
@@ -333,20 +348,21 @@ rows32_group(const int64_t base, const int lane, int64_t nrows, const int* __res
     if (lane == src) acc = s;
   }
   if (valid) y[i] = acc;
+  if (DUAL && valid && d <= kMidRow) y2[i] = acc2;
 }
 
-template <bool WEIGHTED, typename CT, bool RANGED, bool VALIDATE>
+template <bool WEIGHTED, typename CT, bool RANGED, bool VALIDATE, bool DUAL = false>
 __global__ void __launch_bounds__(256)
 spmv_rows32_kernel(int64_t nrows, const int* __restrict__ rows, const int64_t* __restrict__ row_ptr,
                    const int* __restrict__ col, const u32* __restrict__ wt, const CT* __restrict__ colour, u64 key,
                    u64* __restrict__ y, int64_t hub_threshold, int lo, int hi, int64_t n_targets,
-                   u32* __restrict__ err) {
+                   u32* __restrict__ err, u64 key2 = 0, u64* __restrict__ y2 = nullptr) {
   const int lane = threadIdx.x & 31;
   const int64_t base = (((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5) << 5;
   if (base >= nrows) return;
   bool bad = false;
-  rows32_group<WEIGHTED, CT, RANGED, VALIDATE, false>(base, lane, nrows, rows, row_ptr, col, wt, colour, key, y, hub_threshold,
-                                                      lo, hi, n_targets, bad, nullptr, 0u);
+  rows32_group<WEIGHTED, CT, RANGED, VALIDATE, false, DUAL>(base, lane, nrows, rows, row_ptr, col, wt, colour, key, y,
+                                                            hub_threshold, lo, hi, n_targets, bad, nullptr, 0u, key2, y2);
   if (VALIDATE && bad) atomicOr(err, kErrCol);
 }
 
@@ -632,7 +648,8 @@ compact_active_kernel(int64_t count, const int* __restrict__ nodes, const int* _
                       const int* __restrict__ stamp, const int* __restrict__ rep, int round,
                       const int64_t* __restrict__ row_ptr, int64_t hub_threshold, int* __restrict__ next,
                       u64* __restrict__ counters, u64* __restrict__ hub_counter, const int* __restrict__ check_col,
-                      int64_t n_targets, u32* __restrict__ err, const int* __restrict__ final_col, int k_prev) {
+                      int64_t n_targets, u32* __restrict__ err, const int* __restrict__ final_col, int k_prev,
+                      const u64* __restrict__ y2) {
   int64_t t = (int64_t)blockIdx.x * 256 + threadIdx.x;
   bool keep = false;
   int i = 0;
@@ -672,7 +689,10 @@ compact_active_kernel(int64_t count, const int* __restrict__ nodes, const int* _
         // Final block (R5): every out-neighbour's colour existed before this round (id < k_prev) and its block was
         // already out of the loop then (singleton or dropped: not seen with two members in the previous round).  This
         // round's y was computed from exactly those colours, so the nodes that share this block have the same
-        // neighbour colours, all of which never change again: the block can never split.
+        // neighbour colours, all of which never change again: the block can never split.  "Share this block" is decided
+        // by TWO independent sums: the round's y (the relabel key) and y2, the same sum under a second key (DUAL rows of
+        // the row kernel); a node whose y2 differs from its representative's stays active, so a wrong merge can only
+        // become permanent if the same pair collides under both keys.
         const int64_t a = row_ptr[i];
         bool all_final = true;
         for (int64_t p = a; p < a + (int64_t)deg; ++p) {
@@ -682,7 +702,7 @@ compact_active_kernel(int64_t count, const int* __restrict__ nodes, const int* _
             break;
           }
         }
-        keep = !all_final;
+        keep = !all_final || y2[i] != y2[rep[c]];
       }
     }
   }

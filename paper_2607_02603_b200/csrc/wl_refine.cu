@@ -56,6 +56,7 @@ Layout make_layout(int64_t n, int64_t m) {
   L.o_chunk_row = take(sizeof(int) * (size_t)(m / kEbSuper + 4));
   L.o_tag64 = take(sizeof(u64) * kTagSlots);
   L.o_tag32 = take(sizeof(u32) * kTagSlots);
+  L.o_y2 = take(sizeof(u64) * (size_t)n);
   L.bytes = off;
   return L;
 }
@@ -117,6 +118,8 @@ struct SpmvArgs {
   const u32* tag32 = nullptr;  // hot-id table (16-bit ids, plain RSC only) or NULL
   u32 idmask = 0;
   u64* ticket = nullptr;       // zeroed device counter of the persistent kernel
+  u64 key2 = 0;                // DUAL rows: second key and second sum (finality test of the coming compaction)
+  u64* y2 = nullptr;
 };
 
 // edge-balanced S1+S2 over all rows of g (see spmv_eb_kernel)
@@ -161,6 +164,8 @@ static void launch_row_hub2(const wl_csr& g, const SpmvArgs& a, const CT* colour
   unsigned grid = blocks_for(a.nrows, kRowsCta);
   if (!W && !R && a.tag32 && a.narrow) {
     launch_rows_tag<V>(g, a, key, y, st);
+  } else if (!W && !R && !V && a.y2 && sizeof(CT) == 4) {
+    ++g_launches; spmv_rows32_kernel<false, int, false, false, true><<<grid, kRowsCta, 0, st>>>(a.nrows, a.rows, g.row_ptr, g.col_idx, g.weights, a.colour, key, y, kHubThreshold, a.lo, a.hi, a.n_targets, a.err, a.key2, a.y2);
   } else {
     ++g_launches; spmv_rows32_kernel<W, CT, R, V><<<grid, kRowsCta, 0, st>>>(a.nrows, a.rows, g.row_ptr, g.col_idx, g.weights, colour, key, y, kHubThreshold, a.lo, a.hi, a.n_targets, a.err);
   }
@@ -376,6 +381,7 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
   int2* hub_chunks = (int2*)(ws + L.o_hub);
   u64* tag64 = (u64*)(ws + L.o_tag64);
   u32* tag32 = (u32*)(ws + L.o_tag32);
+  u64* y2 = (u64*)(ws + L.o_y2);
   const int64_t launches_at_entry = g_launches;
   EventPool evp;
   const bool merge = (flags & WL_FLAG_MERGE_KERNEL) != 0 && !ranged;
@@ -510,7 +516,7 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
   int cur = 0;
   // One refinement round queued on the stream (S1-S4); no host decision inside.
   auto queue_round = [&](int64_t r, bool narrow, bool mirror, bool clean, u64* log, int log_slot, cudaEvent_t ek0,
-                         cudaEvent_t ek1, bool list_changed = false) -> bool {
+                         cudaEvent_t ek1, bool list_changed = false, bool dual = false) -> bool {
     const u64 key = round_key(seed, stream_id, (u64)r);
     bool streamed = false;
     u32 mask_r = round_table_mask(L, n_active);
@@ -528,6 +534,10 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
       a.e_first = edge_first;
       a.n_targets = n_targets;
       a.err = d_err;
+      if (dual && !narrow && !eb && !a.validate) {  // second, independent sum for the finality test that follows this round
+        a.key2 = round_key(seed, stream_id ^ 0x5ec0dd5ec0dd5ec0ull, (u64)r);
+        a.y2 = y2;
+      }
       if (tag_possible && narrow && !eb) {
         // the table carries the colours of THIS round: rebuilt from the slot winners (32 K threads)
         ++g_launches; tag_finalize_kernel<<<kTagSlots / 256, 256, 0, st>>>(tag64, colour16, idmask, tag32);
@@ -579,7 +589,7 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
     cudaMemsetAsync(scal + kScalActiveHub, 0, sizeof(u64), st);
     // while the column range check is pending the rows dropped here are checked here (a row kernel never reads them)
     const bool check = !cols_checked && !merge && !ranged;
-    ++g_launches; compact_active_kernel<<<blocks_for(n_active, 256), 256, 0, st>>>(n_active, cur_list, colour, stamp, rep, (int)r, g->row_ptr, kHubThreshold, act[cur], scal + kScalActive, scal + kScalActiveHub, check ? g->col_idx : nullptr, n_targets, d_err, final_test ? g->col_idx : nullptr, (int)k_prev);
+    ++g_launches; compact_active_kernel<<<blocks_for(n_active, 256), 256, 0, st>>>(n_active, cur_list, colour, stamp, rep, (int)r, g->row_ptr, kHubThreshold, act[cur], scal + kScalActive, scal + kScalActiveHub, check ? g->col_idx : nullptr, n_targets, d_err, final_test ? g->col_idx : nullptr, (int)k_prev, y2);
     if (check) dropped_checked = true;
   };
   // host side of a compaction whose counters have been read back; returns true when nothing is left to refine
@@ -605,6 +615,10 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
 
   int64_t r = 1;
   bool deep_entered = false;
+  int64_t deep_start_cur = deep_start;  // the round at which the worklist regime is (re-)entered
+  bool tp_built = false;            // the in-neighbour lists exist (first entry into the worklist regime)
+  while (true) {  // plain rounds -> worklist rounds under one key -> one plain confirming round under a fresh key -> ...
+  deep_entered = false;
   while (r <= max_rounds && !converged && !deep_entered) {
     // Rounds 1..kSyncRounds: one host synchronisation per round (the host picks kernels from k and the active count).
     // Deep-round regime (S5): up to kRunAhead rounds are queued back to back; the device keeps k, logs it per round,
@@ -612,7 +626,7 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
     // it is harmless; `rounds` and the trajectory stop at the first repeated count exactly as in the per-round mode.
     // the round at which the worklist regime starts is an ordinary round that also lists the nodes it moved; its key
     // stays the key of every later round
-    if (deep_ok && r == deep_start && !deep) {  // the deep part of the workspace is allocated now (wl_refine_host)
+    if (deep_ok && r == deep_start_cur && !deep) {  // the deep part of the workspace is allocated now (wl_refine_host)
       if (cudaMalloc((void**)&lazy_deep.p, DL.bytes - L.bytes) == cudaSuccess) {
         dws = lazy_deep.p - L.bytes;
         bind_deep();
@@ -621,28 +635,33 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
         deep_ok = false;  // no room: every round keeps recomputing every active row
       }
     }
-    const bool switch_round = deep_ok && r == deep_start;
+    const bool switch_round = deep_ok && r == deep_start_cur;
     if (switch_round) cudaMemsetAsync(deep, 0, sizeof(u64) * kNumDeep, st);
+    if (switch_round && tp_built) {
+      // the worklist rounds do not maintain the representatives the plain relabel compares with: any member will do
+      ++g_launches; set_rep_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, colour, rep);
+    }
+    const int64_t k_before = k;
     const bool window = !no_runahead && r > kSyncRounds && !switch_round;
     const int R = window ? (int)std::min<int64_t>(kRunAhead, max_rounds - r + 1) : 1;
     cudaEvent_t e0 = evp.get(2), e2 = evp.get(4);
     cudaEventRecord(e0, st);
     bool streamed[kRunAhead];
     // 16-bit ids: gathered while k <= 65536; the mirror is kept up to date by the relabel kernel as long as that holds
-    const bool narrow = !merge && (window ? n <= 65536 : k <= 65536);
+    // (the worklist rounds do not maintain the mirror: after them the 32-bit ids are gathered)
+    const bool narrow = !merge && !tp_built && (window ? n <= 65536 : k <= 65536);
+    // the finality test (R5) needs the colour count before the round (host-known in the one-round-per-sync regime only), a
+    // column check that is over and 32-bit ids (the DUAL rows of the row kernel); it pays when the rows that are left are short
+    // (unit weights only: there the members of a block have the same number of entries, so the row-length limit of the
+    // test treats them alike and a block leaves as a whole; its representative's y is never read again)
+    const bool final_test = !window && !switch_round && !ranged && !g->weights && !(flags & WL_FLAG_NO_FINAL) && r >= 2 &&
+                            cols_checked && !narrow && !force_eb && !merge && cur_list != nullptr && active_edges <= 8 * n_active;
     for (int j = 0; j < R; ++j)
-      streamed[j] = queue_round(r + j, narrow, narrow, /*clean=*/window, scal + kScalLog, j, evp.get(8 + 2 * j), evp.get(9 + 2 * j), switch_round);
+      streamed[j] = queue_round(r + j, narrow, narrow, /*clean=*/window, scal + kScalLog, j, evp.get(8 + 2 * j), evp.get(9 + 2 * j), switch_round, final_test);
     const int64_t r_last = r + R - 1;
     // compaction rides behind rounds 1-2 and behind every window; in between it is decided after the round, when the host
     // knows how many colours the round made (below)
     const bool compact_now = prune && !switch_round && (window || r <= 2);
-    const int64_t k_before = k;
-    // the finality test needs the colour count before the round (host-known in the one-round-per-sync regime only) and a
-    // column check that is over; it pays when the rows that are left are short
-    // (unit weights only: there the members of a block have the same number of entries, so the row-length limit of the
-    // test treats them alike and a block leaves as a whole; its representative's y is never read again)
-    const bool final_test = !window && !ranged && !g->weights && !(flags & WL_FLAG_NO_FINAL) && r >= 2 && cols_checked &&
-                            active_edges <= 8 * n_active;
     if (compact_now) queue_compaction(r_last, final_test, k);
     cudaEventRecord(e2, st);
     cudaMemcpyAsync(hs, scal, sizeof(u64) * kNumScal, cudaMemcpyDeviceToHost, st);
@@ -719,8 +738,9 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
     }
   }
   // ---- S5, deep-round regime (wl_deep.cuh): only the rows with a changed out-neighbour are recomputed ---------------------
-  if (deep_entered && !converged && r <= max_rounds) {
-    const u64 key = round_key(seed, stream_id, (u64)deep_start);  // the key of the switch round, kept from here on
+  if (!(deep_entered && !converged && r <= max_rounds)) break;
+  {
+    const u64 key = round_key(seed, stream_id, (u64)deep_start_cur);  // the key of the switch round, kept until the fixed point
     int64_t* tp_ptr = (int64_t*)(dws + DL.o_tp_ptr);
     int* tp_src = (int*)(dws + DL.o_tp_src);
     int* size = (int*)(dws + DL.o_size);
@@ -737,15 +757,18 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
     clean_table(table, dirty_mask, slot_of, dirty_first, dirty_count, st);
     dirty_count = 0;
     aux.need(st, table_slots, prefix_slots);
-    // in-neighbour lists: in-degrees -> offsets -> fill (the in-degree array counts down to zero and becomes `mark`)
-    cudaMemsetAsync(mark, 0, sizeof(int) * (size_t)n, st);
     cudaMemsetAsync(size, 0, sizeof(int) * (size_t)n, st);
-    cudaMemsetAsync(lcount[0], 0, sizeof(int) * (size_t)n, st);
-    cudaMemsetAsync(lcount[1], 0, sizeof(int) * (size_t)n, st);
-    cudaMemsetAsync(inherit, 0, sizeof(int) * (size_t)n, st);
-    ++g_launches; deep_indegree_kernel<<<148 * 8, 256, 0, st>>>(m, g->col_idx + edge_first, mark);
-    launch_scan32(mark, n, 0, tp_ptr, bsum, bsum + (n / kScan32Chunk + 2), st);
-    ++g_launches; deep_fill_kernel<<<blocks_for(n * 32, 256), 256, 0, st>>>(n, g->row_ptr, g->col_idx, tp_ptr, mark, tp_src);
+    if (!tp_built) {
+      // in-neighbour lists: in-degrees -> offsets -> fill (the in-degree array counts down to zero and becomes `mark`)
+      cudaMemsetAsync(mark, 0, sizeof(int) * (size_t)n, st);
+      cudaMemsetAsync(lcount[0], 0, sizeof(int) * (size_t)n, st);
+      cudaMemsetAsync(lcount[1], 0, sizeof(int) * (size_t)n, st);
+      cudaMemsetAsync(inherit, 0, sizeof(int) * (size_t)n, st);
+      ++g_launches; deep_indegree_kernel<<<148 * 8, 256, 0, st>>>(m, g->col_idx + edge_first, mark);
+      launch_scan32(mark, n, 0, tp_ptr, bsum, bsum + (n / kScan32Chunk + 2), st);
+      ++g_launches; deep_fill_kernel<<<blocks_for(n * 32, 256), 256, 0, st>>>(n, g->row_ptr, g->col_idx, tp_ptr, mark, tp_src);
+      tp_built = true;  // (on a re-entry mark / inherit hold stamps of earlier rounds and the leaver counts are zero again)
+    }
     ++g_launches; deep_sizes_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, colour, size);
     constexpr unsigned kDeepGrid = 148 * 4, kDeepFinGrid = 148;
     auto front = [&](const DeepFinishArgs& fin, int do_front, int round) {
@@ -764,7 +787,12 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
                        scal + kScalLog};
       return f;
     };
-    while (r <= max_rounds && !converged) {
+    // The worklist rounds stop at the fixed point UNDER THIS KEY; a pair that collides under it would stay merged for good.
+    // The confirming round of Algorithm 1 is therefore run as a plain round with a fresh key over every active row (the loop
+    // above, as a new switch round): if it changes nothing the paper's terminal argument applies as it stands (L408-L414), else
+    // the worklist rounds go on under the new key.
+    bool fixed_point = false;
+    while (r <= max_rounds && !fixed_point) {
       const int R = no_runahead ? 1 : (int)std::min<int64_t>(kRunAhead, max_rounds - r + 1);
       for (int j = 0; j < R; ++j) {
         const int round = (int)(r + j), in = round & 1, out = (round + 1) & 1;
@@ -780,18 +808,25 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
       cudaEventElapsedTime(&t_win, d0, d1);
       ms_relabel += t_win;
       cudaEventRecord(d0, st);
-      for (int j = 0; j < R && !converged; ++j) {
+      int done = R;
+      for (int j = 0; j < R; ++j) {
         const int64_t k_new = (int64_t)hs[kScalLog + j];
+        if (k_new == k) {  // nothing moved in round r + j: that round is re-run as the plain confirming round
+          fixed_point = true;
+          done = j;
+          break;
+        }
         rounds = (int32_t)(r + j);
         log_round(r + j, k_new);
         if (debug)
           std::fprintf(stderr, "[wl_refine] round %lld: k %lld -> %lld (worklist)\n", (long long)(r + j), (long long)k, (long long)k_new);
-        if (k_new == k) converged = true;
-        k = k_new;
+          k = k_new;
       }
-      r += R;
+      r += done;
     }
+    deep_start_cur = r;
   }
+  }  // while (true)
   if (!cols_checked) {  // no round read a column (everything was settled by the degrees): check them now
     ++g_launches; validate_cols_kernel<<<148 * 8, 256, 0, st>>>(n_targets, edge_first, edge_first + m, g->col_idx, d_err);
     cudaMemcpyAsync(hs + kScalErr, scal + kScalErr, sizeof(u64), cudaMemcpyDeviceToHost, st);
