@@ -81,6 +81,8 @@ typedef struct wl_csr {
                                    direct-mapped {tag, colour} table in shared memory during the 16-bit rounds (one persistent
                                    CTA per SM).  Results are identical.  OFF by default: measured slower than the plain row
                                    kernel on the headline graph (19.6 ms against 16.5 ms, profiles/r2_spmv_levers.md)        */
+#define WL_FLAG_TEST_SMALL_OVERFLOW 536870912u /* testing: the device-side overflow list of the compressed quotient weights holds 2
+                                                  entries, so that the fallback to plain uint32 weights is exercised            */
 #define WL_FLAG_NO_CANONICAL 16u /* leave internal dense ids in out_colors (skips S6)                                  */
 
 typedef struct wl_options {
@@ -217,7 +219,10 @@ int wl_refine_batched(int64_t n, int32_t num_batches, const wl_edge_batch* batch
                       size_t device_cap_bytes, int64_t max_batch_edges, int32_t* out_colors, wl_stats* stats,
                       const wl_options* opt, void* cuda_stream);
 
-/* Bytes of pinned host scratch that always suffice for wl_options.host_workspace: two offset arrays of n + 1 entries and
+/* Quotient weights of an UNWEIGHTED input are stored and moved as one byte each plus per-emission overflow lists for the weights
+ * >= 255 (at most m / 255 of them: a quotient row sums to the out-degree of its representative, L447); a batch with more heavy
+ * weights than the device-side list takes makes the call start over with uint32 weights (with WL_FLAG_CONSUME_INPUT: WL_ENOMEM).
+ * Bytes of pinned host scratch that always suffice for wl_options.host_workspace: two offset arrays of n + 1 entries and
  * one weighted entry array of m entries (a quotient never has more nodes or entries than its graph, Def. 4; later
  * quotients overwrite the first one in place). */
 size_t wl_refine_batched_host_bytes(int64_t n, int64_t m);

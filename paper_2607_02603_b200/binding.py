@@ -26,6 +26,7 @@ WL_FLAG_NO_FINAL = 1024
 WL_FLAG_INHERIT_BATCHES = 4096
 WL_FLAG_CONSUME_INPUT = 8192
 WL_FLAG_TAG_TABLE = 16384
+WL_FLAG_TEST_SMALL_OVERFLOW = 1 << 29
 
 EXPORTS = [
     "wl_refine_workspace_bytes", "wl_refine_deep_workspace_bytes", "wl_refine", "wl_refine_host", "wl_round_key", "wl_weight", "wl_spmv_round",

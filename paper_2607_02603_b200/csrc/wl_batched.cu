@@ -431,6 +431,37 @@ __global__ void quot_insert_coo_kernel(int64_t ne, const int* __restrict__ src, 
   }
 }
 
+
+// ---------------------------------------------------------------------------------------------------------------------
+// Compressed quotient weights.  A quotient entry of an UNWEIGHTED input is a multiplicity whose row sums to the out-degree of the
+// block's representative (L447), so almost every weight is tiny: on the host (and on the link, which bounds the batched path) a
+// weight travels as ONE byte, 255 meaning "look it up in the overflow list of this emission" ({position inside the emission,
+// weight} pairs; a row of out-degree d has at most d / 255 of them).  The kernels themselves keep working on uint32 weights.
+// ---------------------------------------------------------------------------------------------------------------------
+__global__ void wt_pack_kernel(int64_t tot, const u32* __restrict__ w32, unsigned char* __restrict__ w8, u64* __restrict__ ovf,
+                               u32* __restrict__ ovf_count, u32 ovf_cap) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= tot) return;
+  const u32 w = w32[i];
+  w8[i] = (unsigned char)(w < 255u ? w : 255u);
+  if (w >= 255u) {
+    const u32 idx = atomicAdd(ovf_count, 1u);
+    if (idx < ovf_cap) ovf[idx] = (u64)(u32)i | ((u64)w << 32);
+  }
+}
+__global__ void wt_expand_kernel(int64_t cnt, const unsigned char* __restrict__ w8, u32* __restrict__ w32) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < cnt) w32[i] = (u32)w8[i];
+}
+// overflow entries of one emission that starts `base_rel` entries after the first entry of the uploaded slice
+__global__ void wt_patch_kernel(u32 count, const u64* __restrict__ ovf, int64_t base_rel, int64_t cnt, u32* __restrict__ w32) {
+  const u32 t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= count) return;
+  const u64 e = ovf[t];
+  const int64_t pos = (int64_t)(u32)e + base_rel;
+  if (pos >= 0 && pos < cnt) w32[pos] = (u32)(e >> 32);
+}
+
 // exclusive scan int32 counts -> int64 offsets (3 kernels)
 constexpr int kScanT = 256, kScanI = 8, kScanC = kScanT * kScanI;
 static_assert(kScanC == kScan32Chunk, "wl_refine.cu sizes the scan scratch with kScan32Chunk");
@@ -571,13 +602,46 @@ struct HostQuot {
   int64_t cap_nodes = 0, cap_edges = 0;
   // consume_col / consume_wt: the quotients are written over the caller's own column (and weight) array, so the scratch holds
   // the offset arrays only (plus a weight array when the input has none): WL_FLAG_CONSUME_INPUT
-  static size_t bytes_for(int64_t n, int64_t m, bool consume_col = false, bool consume_wt = false) {
+  // wt8 != NULL: weights stored as one byte each + per-emission overflow lists (see wt_pack_kernel); the overflow lists of the
+  // two quotient generations alive at a time live in library-owned pinned memory (a few bytes per 255 entries)
+  unsigned char* wt8 = nullptr;
+  struct Emission {
+    int64_t q_begin, q_end;  // entries of the quotient this emission wrote
+    size_t ovf_off;          // its overflow list inside Generation::ovf
+    u32 count;
+  };
+  struct Generation {
+    std::vector<Emission> em;
+    u64* ovf = nullptr;  // {position inside the emission : 32 | weight : 32}
+    size_t cap = 0, used = 0;
+  } gen[2];
+  static size_t bytes_for(int64_t n, int64_t m, bool consume_col = false, bool consume_wt = false, bool compressed = false) {
     return 2 * align_up(sizeof(int64_t) * (size_t)(n + 1)) + (consume_col ? 0 : align_up(sizeof(int) * (size_t)m)) +
-           (consume_wt ? 0 : align_up(sizeof(int) * (size_t)m));
+           (consume_wt ? 0 : align_up((compressed ? 1 : sizeof(int)) * (size_t)m));
   }
-  int init(int64_t n, int64_t m, void* ws, size_t ws_bytes, int* consume_col = nullptr, u32* consume_wt = nullptr) {
+  // start generation g with room for `entries` overflow entries (the weights of a quotient of an unweighted graph sum to at
+  // most its edge count, so at most m / 255 of them reach 255)
+  int reserve_generation(int g, size_t entries) {
+    Generation& G = gen[g];
+    G.em.clear();
+    G.used = 0;
+    if (G.ovf && G.cap < entries) {
+      cudaFreeHost(G.ovf);
+      G.ovf = nullptr;
+    }
+    if (!G.ovf) {
+      if (cudaHostAlloc((void**)&G.ovf, sizeof(u64) * std::max<size_t>(1, entries), cudaHostAllocDefault) != cudaSuccess) {
+        cudaGetLastError();
+        return WL_ENOMEM;
+      }
+      G.cap = entries;
+    }
+    return WL_OK;
+  }
+  int init(int64_t n, int64_t m, void* ws, size_t ws_bytes, int* consume_col = nullptr, u32* consume_wt = nullptr,
+           bool compressed = false) {
     if (base) return WL_OK;
-    const size_t need = bytes_for(n, m, consume_col != nullptr, consume_wt != nullptr);
+    const size_t need = bytes_for(n, m, consume_col != nullptr, consume_wt != nullptr, compressed);
     if (ws && ws_bytes >= need) {
       base = (char*)ws;
     } else {
@@ -600,12 +664,18 @@ struct HostQuot {
       off += align_up(sizeof(int) * (size_t)m);
     }
     wt = consume_wt ? consume_wt : (u32*)(base + off);
+    if (compressed) {
+      wt8 = (unsigned char*)wt;
+      wt = nullptr;
+    }
     cap_nodes = n;
     cap_edges = m;
     return WL_OK;
   }
   ~HostQuot() {
     if (owned && base) cudaFreeHost(base);
+    for (Generation& G : gen)
+      if (G.ovf) cudaFreeHost(G.ovf);
   }
 };
 
@@ -691,7 +761,7 @@ size_t wl_refine_batched_host_bytes(int64_t n, int64_t m) {
 
 size_t wl_refine_batched_host_bytes_consume(int64_t n, int64_t m, int weighted) {
   if (n < 0 || m < 0 || n > kMaxNodes) return 0;
-  return HostQuot::bytes_for(n, m, true, weighted != 0);
+  return HostQuot::bytes_for(n, m, true, weighted != 0, /*compressed=*/weighted == 0);
 }
 
 size_t wl_quotient_workspace_bytes(int64_t n, int64_t m) {
@@ -1193,9 +1263,11 @@ static int coo_first_iteration(int64_t n, int nb, const wl_edge_batch* batches, 
 }
 
 // Algorithm 2 for a given M_b (the exported entry point below picks M_b from the device cap when the caller gives none)
+constexpr int kCompressOverflow = -100;  // internal: an emission held more heavy weights than the device list takes
+
 static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batches, const wl_csr* whole, uint64_t seed,
                        size_t device_cap_bytes, int64_t max_batch_edges, int32_t* out_colors, wl_stats* stats,
-                       const wl_options* opt, void* cuda_stream) {
+                       const wl_options* opt, void* cuda_stream, bool allow_compress = true) {
   if (stats) std::memset(stats, 0, sizeof(*stats));
   if (n < 0 || num_batches < 0 || max_batch_edges <= 0) return WL_EINVAL;
   if (n > kMaxNodes) return WL_ERANGE;
@@ -1262,6 +1334,8 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
   // and never hold more entries, Def. 4), exactly as every later quotient overwrites its predecessor
   const bool consume = (flags & WL_FLAG_CONSUME_INPUT) != 0;
   if (consume && num_batches != 0) return WL_EINVAL;  // only the whole-CSR form owns one contiguous column array
+  // quotient weights of an unweighted input travel as one byte + overflow lists (wt_pack_kernel)
+  const bool compress = allow_compress && !coo && !weighted;
   // S0 on the host side of the CSR forms: the offsets steer the cuts, the inner ranges and every upload size
   if (!coo && !(flags & WL_FLAG_NO_VALIDATE)) {
     if (rp[0] != 0) return WL_EINVAL;
@@ -1415,7 +1489,19 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
     // are canonical without a pass over all nodes, and the per-block counters of the quotient pass live in a window.
     size_t used_iter = used;
     DevBuf d_Hc, d_isrep, d_ws, d_col[2], d_wt[2], d_rp[2], d_cnt, d_cursor, d_qrp[2], d_qtab, d_qcol[2], d_qwt[2], d_sbsum,
-        d_misc, d_query, d_long, d_Hnext, d_isrep_next, d_ws2;
+        d_misc, d_query, d_long, d_Hnext, d_isrep_next, d_ws2, d_wt8[2], d_ovf_up[2], d_qwt8[2], d_qovf[2];
+    // the graph of this iteration has compressed weights (it is a quotient this call wrote)
+    const bool read_compressed = compress && outer > 1;
+    HostQuot::Generation& Gr = hq.gen[(outer & 1) ^ 1];  // overflow lists of the graph being read
+    size_t max_up_ovf = 1;
+    if (read_compressed) {
+      for (int k = 0; k < nb; ++k) {  // overflow entries a batch may need: those of the emissions it overlaps
+        size_t need = 0;
+        for (const HostQuot::Emission& e : Gr.em)
+          if (e.q_begin < cuts[k + 1] && e.q_end > cuts[k]) need += e.count;
+        max_up_ovf = std::max(max_up_ovf, need);
+      }
+    }
     // every allocation of the iteration goes through here: the first failure (device cap or cudaMalloc) sticks
 #define WL_ALLOC(buf, bytes) \
   if (!rc) rc = buf.alloc((bytes), &used_iter, device_cap_bytes);
@@ -1436,23 +1522,46 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
     for (int b = 0; b < 2; ++b) {
       WL_ALLOC(d_col[b], sizeof(int) * (size_t)max_edges);
       if (weighted) WL_ALLOC(d_wt[b], sizeof(u32) * (size_t)max_edges);
+      if (read_compressed) {
+        WL_ALLOC(d_wt8[b], (size_t)max_edges);
+        WL_ALLOC(d_ovf_up[b], sizeof(u64) * max_up_ovf);
+      }
       WL_ALLOC(d_rp[b], sizeof(int64_t) * (size_t)(max_rows + 4));  // the quotient pass adds the rows cut at either end
     }
     WL_ALLOC(d_misc, 4096);
     if (rc) break;
     cudaMemsetAsync(d_misc.p, 0, 4096, st);
+    // weights of the edge positions [c0, c1) of the current graph into d_wt[buf], on the copy stream
+    auto upload_weights = [&](int k, int buf, int64_t c0, int64_t c1) {
+      if (!weighted || c1 <= c0) return;
+      const int64_t cnt = c1 - c0;
+      if (!read_compressed) {
+        const u32* hw = (outer == 1) ? batch_wt(k) : hq.wt + c0;
+        cudaMemcpyAsync(d_wt[buf].p, hw, sizeof(u32) * (size_t)cnt, cudaMemcpyHostToDevice, copy_st);
+        bytes_h2d += sizeof(u32) * cnt;
+        return;
+      }
+      cudaMemcpyAsync(d_wt8[buf].p, hq.wt8 + c0, (size_t)cnt, cudaMemcpyHostToDevice, copy_st);
+      bytes_h2d += cnt;
+      ++g_launches; wt_expand_kernel<<<blocks_for(cnt, 256), 256, 0, copy_st>>>(cnt, d_wt8[buf].as<unsigned char>(), d_wt[buf].as<u32>());
+      size_t at = 0;
+      for (const HostQuot::Emission& e : Gr.em) {
+        if (e.count == 0 || e.q_begin >= c1 || e.q_end <= c0) continue;
+        u64* d_list = d_ovf_up[buf].as<u64>() + at;
+        cudaMemcpyAsync(d_list, Gr.ovf + e.ovf_off, sizeof(u64) * e.count, cudaMemcpyHostToDevice, copy_st);
+        bytes_h2d += sizeof(u64) * e.count;
+        ++g_launches; wt_patch_kernel<<<blocks_for(e.count, 256), 256, 0, copy_st>>>(e.count, d_list, e.q_begin - c0, cnt, d_wt[buf].as<u32>());
+        at += e.count;
+      }
+    };
 
     auto upload_batch = [&](int k, int buf) {
       const int64_t c0 = cuts[k], c1 = cuts[k + 1];
       const int* hc = (outer == 1) ? batch_col(k) : hq.col + c0;
-      const u32* hw = (outer == 1) ? batch_wt(k) : hq.wt + c0;
       if (c1 > c0) {
         cudaMemcpyAsync(d_col[buf].p, hc, sizeof(int) * (size_t)(c1 - c0), cudaMemcpyHostToDevice, copy_st);
         bytes_h2d += sizeof(int) * (c1 - c0);
-        if (weighted) {
-          cudaMemcpyAsync(d_wt[buf].p, hw, sizeof(u32) * (size_t)(c1 - c0), cudaMemcpyHostToDevice, copy_st);
-          bytes_h2d += sizeof(u32) * (c1 - c0);
-        }
+        upload_weights(k, buf, c0, c1);
       }
       const int64_t nr = r1[k] - r0[k];
       cudaMemcpyAsync(d_rp[buf].p, rp + r0[k], sizeof(int64_t) * (size_t)(nr + 1), cudaMemcpyHostToDevice, copy_st);
@@ -1599,7 +1708,7 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
     // Three streams: copy_st uploads batch k + 1 while st inserts / emits batch k and down_st returns the rows emitted for
     // batch k - 1 to the host (double buffers on both sides; one host synchronisation per batch, to learn the emitted size).
     if ((rc = hq.init(n0, rp0_edges, opt ? opt->host_workspace : nullptr, opt ? opt->host_workspace_bytes : 0,
-                      consume ? const_cast<int*>(col) : nullptr, consume && wt ? const_cast<u32*>(wt) : nullptr)))
+                      consume ? const_cast<int*>(col) : nullptr, consume && wt ? const_cast<u32*>(wt) : nullptr, compress)))
       break;
     const int osel = outer & 1;  // offsets of the quotient being written; the graph being read uses the other array
     int64_t* nrp = hq.rp[osel];
@@ -1650,10 +1759,18 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
     WL_ALLOC(d_cursor, sizeof(int) * (size_t)win);
     for (int b = 0; b < 2; ++b) WL_ALLOC(d_qrp[b], sizeof(int64_t) * (size_t)(win + 1));
     WL_ALLOC(d_qtab, sizeof(u64) * 2 * qslots);
+    // heavy weights (>= 255) one emission may hold on the device before the call falls back to plain uint32 weights
+    const u32 ovf_dev_cap = (flags & WL_FLAG_TEST_SMALL_OVERFLOW) ? 2u : (u32)std::min<int64_t>(out_cap, out_cap / 16 + 4096);
+    HostQuot::Generation& Gw = hq.gen[outer & 1];                                   // overflow lists of the quotient being written
     for (int b = 0; b < 2; ++b) {
       WL_ALLOC(d_qcol[b], sizeof(int) * (size_t)out_cap);
       WL_ALLOC(d_qwt[b], sizeof(u32) * (size_t)out_cap);
+      if (compress) {
+        WL_ALLOC(d_qwt8[b], (size_t)out_cap);
+        WL_ALLOC(d_qovf[b], sizeof(u64) * (size_t)ovf_dev_cap);
+      }
     }
+    if (compress && !rc) rc = hq.reserve_generation(outer & 1, (size_t)(rp0_edges / 255 + nb + 1024));
     WL_ALLOC(d_sbsum, sizeof(u64) * (size_t)((win + kScanC - 1) / kScanC + 2));
     WL_ALLOC(d_long, sizeof(int) * (size_t)(max_edges / kQuotLongRow + 2));
     if (debug) std::fprintf(stderr, "[wl_refine_batched] outer %d device memory %.2f GB (cap %.2f GB)%s\n", outer, used_iter / 1073741824.0, device_cap_bytes / 1073741824.0, rc ? " -> WL_ENOMEM" : "");
@@ -1679,13 +1796,9 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
       const int64_t c0 = cuts[k], c1 = cuts[k + 1];
       if (c1 > c0) {
         const int* hc = (outer == 1) ? batch_col(k) : hq.col + c0;
-        const u32* hw = (outer == 1) ? batch_wt(k) : hq.wt + c0;
         cudaMemcpyAsync(d_col[buf].p, hc, sizeof(int) * (size_t)(c1 - c0), cudaMemcpyHostToDevice, copy_st);
         bytes_h2d += sizeof(int) * (c1 - c0);
-        if (weighted) {
-          cudaMemcpyAsync(d_wt[buf].p, hw, sizeof(u32) * (size_t)(c1 - c0), cudaMemcpyHostToDevice, copy_st);
-          bytes_h2d += sizeof(u32) * (c1 - c0);
-        }
+        upload_weights(k, buf, c0, c1);
         cudaMemcpyAsync(d_rp[buf].p, rp + na[k], sizeof(int64_t) * (size_t)(nz[k] - na[k] + 1), cudaMemcpyHostToDevice, copy_st);
         bytes_h2d += sizeof(int64_t) * (nz[k] - na[k] + 1);
       }
@@ -1746,6 +1859,31 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
     };
     int64_t q_off = 0, emitted_blocks = 0;
     int n_emit = 0;
+    // compressed weights: the overflow list of an emission goes to the host one synchronisation later, when its length is known
+    u32* d_ovf_cnt = (u32*)(d_misc.as<u64>() + 32);  // two counters (by emission parity)
+    volatile u64* h_ovf_cnt = hs + kNumScal + 4;      // their host copies
+    struct PendingOvf {
+      bool valid;
+      int ob;
+      size_t em_index;
+    } pend_ovf{false, 0, 0};
+    auto flush_overflow = [&]() -> int {  // call right after a synchronisation of `st`
+      if (!pend_ovf.valid) return WL_OK;
+      pend_ovf.valid = false;
+      const u32 cnt = (u32)h_ovf_cnt[pend_ovf.ob];
+      if (cnt > ovf_dev_cap) return kCompressOverflow;
+      HostQuot::Emission& e = Gw.em[pend_ovf.em_index];
+      if (Gw.used + cnt > Gw.cap) return WL_ECUDA;  // unreachable: at most m / 255 weights reach 255 (L447)
+      e.ovf_off = Gw.used;
+      e.count = cnt;
+      if (cnt) {
+        cudaMemcpyAsync(Gw.ovf + Gw.used, d_qovf[pend_ovf.ob].p, sizeof(u64) * cnt, cudaMemcpyDeviceToHost, down_st);
+        bytes_d2h += sizeof(u64) * cnt;
+        cudaEventRecord(ev_down[pend_ovf.ob], down_st);  // the buffer is free again only after this copy
+        Gw.used += cnt;
+      }
+      return WL_OK;
+    };
     auto checkpoint = [&](const char* what, int k) {  // WL_DEBUG: find the launch that faults
       if (!debug) return;
       cudaError_t e = cudaDeviceSynchronize();
@@ -1784,6 +1922,7 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
         rc = check_cuda(cudaStreamSynchronize(st));
         if (rc) break;
         const int64_t tot = (int64_t)hs[kNumScal + 1];
+        if ((rc = flush_overflow())) break;
         if (debug) std::fprintf(stderr, "[wl_refine_batched] outer %d batch %d: rows %lld..%lld blocks %lld..%lld entries %lld at %lld (cap %lld)\n", outer, k, (long long)na[k], (long long)nz[k], (long long)b_lo, (long long)b_hi, (long long)tot, (long long)q_off, (long long)out_cap);
         if (tot > out_cap || q_off + tot > hq.cap_edges || b_hi > hq.cap_nodes) {
           rc = WL_ECUDA;  // unreachable: a quotient has at most the entries and nodes of its graph
@@ -1791,6 +1930,11 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
         }
         ++n_emit;
         ++g_launches; quot_emit_kernel<<<blocks_for((int64_t)qslots, 256), 256, 0, st>>>(d_qtab.as<u64>(), qslots, d_qrp[ob].as<int64_t>() - b_lo, q_off, d_cursor.as<int>() - b_lo, d_qcol[ob].as<int>(), d_qwt[ob].as<u32>(), (int)b_lo, (int)b_hi);
+        if (compress && tot) {
+          cudaMemsetAsync(d_ovf_cnt + ob, 0, sizeof(u32), st);
+          ++g_launches; wt_pack_kernel<<<blocks_for(tot, 256), 256, 0, st>>>(tot, d_qwt[ob].as<u32>(), d_qwt8[ob].as<unsigned char>(), d_qovf[ob].as<u64>(), d_ovf_cnt + ob, ovf_dev_cap);
+          cudaMemcpyAsync((void*)(h_ovf_cnt + ob), d_ovf_cnt + ob, sizeof(u32), cudaMemcpyDeviceToHost, st);
+        }
         cudaEventRecord(ev_emit[ob], st);
         checkpoint("emit", k);
         // the window moves on: the counter of the block whose row is still open becomes index 0
@@ -1802,8 +1946,15 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
         // in place from the second quotient on: q_off + tot <= c1, and everything below c1 has been uploaded already
         if (tot) {
           cudaMemcpyAsync(hq.col + q_off, d_qcol[ob].p, sizeof(int) * (size_t)tot, cudaMemcpyDeviceToHost, down_st);
-          cudaMemcpyAsync(hq.wt + q_off, d_qwt[ob].p, sizeof(u32) * (size_t)tot, cudaMemcpyDeviceToHost, down_st);
-          bytes_d2h += (sizeof(int) + sizeof(u32)) * tot;
+          if (compress) {
+            cudaMemcpyAsync(hq.wt8 + q_off, d_qwt8[ob].p, (size_t)tot, cudaMemcpyDeviceToHost, down_st);
+            bytes_d2h += (sizeof(int) + 1) * tot;
+            Gw.em.push_back(HostQuot::Emission{q_off, q_off + tot, 0, 0});
+            pend_ovf = PendingOvf{true, ob, Gw.em.size() - 1};
+          } else {
+            cudaMemcpyAsync(hq.wt + q_off, d_qwt[ob].p, sizeof(u32) * (size_t)tot, cudaMemcpyDeviceToHost, down_st);
+            bytes_d2h += (sizeof(int) + sizeof(u32)) * tot;
+          }
         }
         cudaMemcpyAsync(nrp + b_lo, d_qrp[ob].p, sizeof(int64_t) * (size_t)(b_hi - b_lo + 1), cudaMemcpyDeviceToHost, down_st);
         bytes_d2h += sizeof(int64_t) * (b_hi - b_lo + 1);
@@ -1819,8 +1970,9 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
     }
     if (!rc) rc = refine_piece();
     if (!rc) rc = check_cuda(cudaStreamSynchronize(side_st));
-    if (!rc) rc = check_cuda(cudaStreamSynchronize(down_st));
     if (!rc) rc = check_cuda(cudaStreamSynchronize(st));
+    if (!rc) rc = flush_overflow();
+    if (!rc) rc = check_cuda(cudaStreamSynchronize(down_st));
     if (rc) break;
     nrp[(size_t)K] = q_off;
     phase("quotient");
@@ -1906,9 +2058,17 @@ extern "C" {
 int wl_refine_batched(int64_t n, int32_t num_batches, const wl_edge_batch* batches, const wl_csr* whole, uint64_t seed,
                       size_t device_cap_bytes, int64_t max_batch_edges, int32_t* out_colors, wl_stats* stats,
                       const wl_options* opt, void* cuda_stream) {
-  if (max_batch_edges > 0)
-    return batched_run(n, num_batches, batches, whole, seed, device_cap_bytes, max_batch_edges, out_colors, stats, opt,
-                       cuda_stream);
+  // compressed quotient weights are tried first; a batch with too many heavy weights for the device-side overflow list makes the
+  // call start over with plain uint32 weights (impossible once the input has been consumed: WL_ENOMEM then)
+  auto run = [&](int64_t mb) -> int {
+    int rc = batched_run(n, num_batches, batches, whole, seed, device_cap_bytes, mb, out_colors, stats, opt, cuda_stream, true);
+    if (rc == kCompressOverflow) {
+      if (opt && (opt->flags & WL_FLAG_CONSUME_INPUT)) return WL_ENOMEM;
+      rc = batched_run(n, num_batches, batches, whole, seed, device_cap_bytes, mb, out_colors, stats, opt, cuda_stream, false);
+    }
+    return rc;
+  };
+  if (max_batch_edges > 0) return run(max_batch_edges);
   // M_b <= 0: derive it from the device cap (BASELINE.json configs[4]: "a device working-set cap forces the batching").
   // The largest M_b whose estimated budget fits 90 % of the cap; an estimate that turns out too low is answered by WL_ENOMEM
   // from the checked allocations, and M_b shrinks until the run fits.
@@ -1918,7 +2078,7 @@ int wl_refine_batched(int64_t n, int32_t num_batches, const wl_edge_batch* batch
   const bool inh = opt && (opt->flags & WL_FLAG_INHERIT_BATCHES);
   while (mb > 1024 && batched_budget(n, m, mb, device_cap_bytes, inh) > 0.9 * (double)device_cap_bytes) mb = (int64_t)((double)mb * 0.8);
   for (int attempt = 0; attempt < 12; ++attempt) {
-    const int rc = batched_run(n, 0, nullptr, whole, seed, device_cap_bytes, mb, out_colors, stats, opt, cuda_stream);
+    const int rc = run(mb);
     if (rc != WL_ENOMEM || mb <= 1024) return rc;
     mb = (int64_t)((double)mb * 0.7);
   }

@@ -320,6 +320,34 @@ def test_batched_consume_input_overwrites_the_column_array(name, flags):
         assert not torch.equal(col, g.col)  # the quotient really went over the input
 
 
+def _heavy_multigraph():
+    # duplicate CSR entries add (Q10): six classes of ten twin nodes, each twin points 254 + c times to each of the five sinks of
+    # its class -> quotient weights 254, 255, 256, ... and their multiples: the escape value of the compressed weights and its
+    # neighbours, nearly every entry in the overflow lists; several outer iterations are needed to merge the twins across batches
+    edges = []
+    for c in range(6):
+        for l in range(10):
+            for r in range(5):
+                edges += [(c * 10 + l, 60 + c * 5 + r)] * (254 + c)
+    edges += [(60, 61)] * 3
+    return gg.from_edge_list(90, edges)
+
+
+@pytest.mark.parametrize("flags", [0, 4096, 1 << 29, (1 << 29) | 4096])
+@pytest.mark.parametrize("nb", [3, 7, 20])
+def test_batched_compressed_weights_with_heavy_entries(flags, nb):
+    """Quotient weights travel as one byte + overflow lists (unweighted inputs).  A multigraph whose quotient weights are all
+    >= 255 (and some exactly 254 / 255 / 256 / 300k), with inherited and re-cut batches, and with the device-side overflow list
+    shrunk to 2 entries so that the fallback to uint32 weights runs: bit-exact against the CPU Algorithm 2 every time."""
+    for g in (_heavy_multigraph(), BATCH_GRAPHS["hub"](), BATCH_GRAPHS["rmat10_sym"]()):
+        n, rp, ci, wt = g.numpy()
+        cap = max(1, -(-g.m // nb))
+        want, k_want, outer_want, _ = oracle.rbsc(n, rp, ci, wt, cap, inherit=bool(flags & 4096))
+        res = wl.wl_refine_batched(n, g.row_ptr, g.col, None, max_batch_edges=cap, seed=5, flags=flags)
+        assert res.colors.numpy().tolist() == want.tolist() and res.stats["outer_iters"] == outer_want
+        assert oracle.is_stable(n, rp, ci, wt, res.colors.numpy())
+
+
 def test_batched_device_cap_is_checked_for_every_allocation():
     """A cap that admits the buffers of the local-refinement pass but not those of the quotient pass must give WL_ENOMEM
     (a failed allocation used to be overwritten by the next successful one)."""
