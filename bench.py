@@ -518,6 +518,56 @@ def run_c4_check(args):
     return 0
 
 
+def run_sharded(args):
+    """--workload sharded: Algorithm 2 with the batches of every outer iteration spread over the ranks (sharded.py): STRONG scaling
+    of one fixed host-resident graph over N GPUs (torchrun), the exchange being one all-gather of block counts and one
+    all-gather-v of the block-map slices per outer iteration.  N = 1 runs the same driver on one GPU."""
+    import torch
+    import graphgen as gg
+    from paper_2607_02603_b200.sharded import refine_batched_sharded
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    dev = torch.device("cuda", local_rank)
+    torch.cuda.set_device(dev)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+    g = gg.rmat(args.scale, seed=RMAT_SEEDS[30], symmetrize=False, device=dev, chunk=1 << 27)
+    n, m = g.n, g.m
+    rp, col = g.row_ptr.cpu().pin_memory(), g.col.cpu().pin_memory()
+    del g
+    torch.cuda.empty_cache()
+    cap = args.batch_edges if args.batch_edges > 0 else max(1, m // 32 + 1)
+    times, res = [], None
+    for i in range(args.warmup + args.steps):
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+        t0 = time.perf_counter()
+        res = refine_batched_sharded(n, rp, col, None, max_batch_edges=cap, seed=500 + i, dist=dist, device=dev)
+        torch.cuda.synchronize(dev)
+        if i >= args.warmup:
+            times.append(time.perf_counter() - t0)
+    local = sum(times) / len(times)
+    t = torch.tensor([local], dtype=torch.float64, device=dev)
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    sec = float(t.item())
+    if rank == 0:
+        colours, k, outer = res
+        print(json.dumps({"metric": "sharded_batched_refine_input_gedges_per_s", "value": m / sec / 1e9, "unit": "GEdges/s",
+                          "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * sec,
+                          "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "u64", "data": "synthetic",
+                          "config": {"workload": f"R-MAT scale {args.scale}, directed, seed 3, host-resident; batches of {cap} edges "
+                                                 "spread over the ranks (sharded.py, inherited batches)", "n": n, "m": m},
+                          "num_colors": k, "outer_iters": outer, "reduction_power": k / n}))
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
 def aggregate_over_ranks(dist, local_ms: float, units_per_rank: float, device=None):
     """Max-over-ranks time and whole-job throughput for N independent replicas (weak scaling, no data-path collective).
     dist = torch.distributed (initialised) or None for a single process.  Returns (ms_max, total_units_per_second)."""
@@ -554,7 +604,7 @@ def main():
     ap.add_argument("--flags", type=int, default=0, help="WL_FLAG_* bits passed to wl_refine")
     ap.add_argument("--mismatch-c3-seeds", type=int, default=20, help="seeds of the C3 leg of the mismatch report (0: C1 only)")
     ap.add_argument("--time-limit", type=float, default=1800.0, help="oracle-times / c4-check: wall-clock limit per oracle run (s)")
-    ap.add_argument("--workload", default="single", choices=["single", "batched", "batch-study", "cap-sweep", "oracle-times", "c4-check"],
+    ap.add_argument("--workload", default="single", choices=["single", "batched", "batch-study", "cap-sweep", "oracle-times", "c4-check", "sharded"],
                     help="single: wl_refine on the HBM-resident graph (the headline); batched: wl_refine_batched")
     ap.add_argument("--cap-gb", type=float, default=16.0, help="batched: device memory cap")
     ap.add_argument("--consume-input", action="store_true", help="batched: WL_FLAG_CONSUME_INPUT (forced from scale 30 on)")
@@ -574,6 +624,8 @@ def main():
         return run_oracle_times(args)
     if args.workload == "c4-check":
         return run_c4_check(args)
+    if args.workload == "sharded":
+        return run_sharded(args)
 
     import torch
     import graphgen as gg
