@@ -1264,6 +1264,7 @@ static int coo_first_iteration(int64_t n, int nb, const wl_edge_batch* batches, 
 
 // Algorithm 2 for a given M_b (the exported entry point below picks M_b from the device cap when the caller gives none)
 constexpr int kCompressOverflow = -100;  // internal: an emission held more heavy weights than the device list takes
+static thread_local bool g_input_consumed = false;  // WL_FLAG_CONSUME_INPUT: the caller's arrays have been written to (no retry)
 
 static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batches, const wl_csr* whole, uint64_t seed,
                        size_t device_cap_bytes, int64_t max_batch_edges, int32_t* out_colors, wl_stats* stats,
@@ -1945,6 +1946,7 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
         cudaStreamWaitEvent(down_st, ev_emit[ob], 0);
         // in place from the second quotient on: q_off + tot <= c1, and everything below c1 has been uploaded already
         if (tot) {
+          if (consume) g_input_consumed = true;
           cudaMemcpyAsync(hq.col + q_off, d_qcol[ob].p, sizeof(int) * (size_t)tot, cudaMemcpyDeviceToHost, down_st);
           if (compress) {
             cudaMemcpyAsync(hq.wt8 + q_off, d_qwt8[ob].p, (size_t)tot, cudaMemcpyDeviceToHost, down_st);
@@ -2060,10 +2062,11 @@ int wl_refine_batched(int64_t n, int32_t num_batches, const wl_edge_batch* batch
                       const wl_options* opt, void* cuda_stream) {
   // compressed quotient weights are tried first; a batch with too many heavy weights for the device-side overflow list makes the
   // call start over with plain uint32 weights (impossible once the input has been consumed: WL_ENOMEM then)
+  g_input_consumed = false;
   auto run = [&](int64_t mb) -> int {
     int rc = batched_run(n, num_batches, batches, whole, seed, device_cap_bytes, mb, out_colors, stats, opt, cuda_stream, true);
     if (rc == kCompressOverflow) {
-      if (opt && (opt->flags & WL_FLAG_CONSUME_INPUT)) return WL_ENOMEM;
+      if (g_input_consumed) return WL_ENOMEM;
       rc = batched_run(n, num_batches, batches, whole, seed, device_cap_bytes, mb, out_colors, stats, opt, cuda_stream, false);
     }
     return rc;
@@ -2079,7 +2082,7 @@ int wl_refine_batched(int64_t n, int32_t num_batches, const wl_edge_batch* batch
   while (mb > 1024 && batched_budget(n, m, mb, device_cap_bytes, inh) > 0.9 * (double)device_cap_bytes) mb = (int64_t)((double)mb * 0.8);
   for (int attempt = 0; attempt < 12; ++attempt) {
     const int rc = run(mb);
-    if (rc != WL_ENOMEM || mb <= 1024) return rc;
+    if (rc != WL_ENOMEM || mb <= 1024 || g_input_consumed) return rc;  // a consumed input cannot be read a second time
     mb = (int64_t)((double)mb * 0.7);
   }
   return WL_ENOMEM;

@@ -465,3 +465,39 @@ def test_refine_batched_sharded_single_process_entry_point():
     want, k_want, outer_want, _ = oracle.rbsc(n, rp, ci, wt, cap, inherit=True)
     colours, k, outer = refine_batched_sharded(n, g.row_ptr, g.col, None, max_batch_edges=cap, seed=4, device=dev())
     assert colours.numpy().tolist() == want.tolist() and k == k_want and outer == outer_want
+
+
+@pytest.mark.parametrize("seed", range(5))
+def test_per_batch_device_calls_match_the_definitions(seed):
+    """wl_refine_inner (B3 + B4 of one batch: inner nodes one block, every outside target an implicit singleton, ids in
+    first-occurrence order) and wl_quotient_rows (Def. 4 for the representatives among a node range) against the oracle-made
+    backend of the sharded tests, on a node range in the middle of a graph."""
+    import os
+    import sys
+    sys.path.insert(0, os.path.dirname(os.path.abspath(__file__)))
+    from sharded_harness import OracleBackend
+    g = gg.rmat(10, edge_factor=6, seed=seed, symmetrize=bool(seed % 2)) if seed < 4 else gg.random_weighted_digraph(600, 5000, seed, max_w=4)
+    n = g.n
+    lo, hi = n // 5, n // 5 + n // 2
+    a, b = int(g.row_ptr[lo]), int(g.row_ptr[hi])
+    rp = (g.row_ptr[lo:hi + 1] - a).contiguous()
+    col = g.col[a:b].contiguous()
+    wt = None if g.weights is None else g.weights[a:b].contiguous()
+    ob = OracleBackend()
+    want_c, want_f, want_k = ob.refine_inner(rp, col, wt, lo, n, 0, 0)
+    c, f, k = wl.wl_refine_inner(rp.to(dev()), col.to(dev()), None if wt is None else wt.to(dev()), lo, n, seed=seed)
+    assert k == want_k and c.cpu().tolist() == want_c.tolist() and f.cpu().tolist() == want_f.tolist()
+    # a block map of the whole graph: the inner range keeps its local blocks, everybody else is a singleton
+    block_of = torch.empty(n, dtype=torch.int32)
+    block_of[:lo] = torch.arange(lo, dtype=torch.int32)
+    block_of[lo:hi] = want_c + lo
+    block_of[hi:] = torch.arange(n - hi, dtype=torch.int32) + lo + k
+    ob.set_block_map(block_of)
+    wr, wc, ww = ob.quotient_rows(rp, col, wt, lo, want_f, lo, k)
+    qr, qc, qw = wl.wl_quotient_rows(rp.to(dev()), col.to(dev()), None if wt is None else wt.to(dev()), lo, block_of.to(dev()),
+                                     f, lo, k)
+    assert qr.cpu().tolist() == wr.tolist()
+    assert _rows_as_dicts(k, qr.cpu().numpy(), qc.cpu().numpy(), qw.cpu().numpy()) == _rows_as_dicts(k, wr.numpy(), wc.numpy(), ww.numpy())
+    with pytest.raises(wl.WlError) as e:  # the range does not fit the node count
+        wl.wl_refine_inner(rp.to(dev()), col.to(dev()), None, n, n, seed=1)
+    assert e.value.code == wl.WL_EINVAL
