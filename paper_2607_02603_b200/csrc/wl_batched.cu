@@ -862,7 +862,7 @@ int wl_refine_inner(const wl_csr* rows, int64_t lo, int64_t n_targets, uint64_t 
   char* wsb = (char*)workspace;
   int* first_l = (int*)(wsb + L.o_tmp);
   launch_canonical(L, nr, cr.colour, local_colors, first_l, (int*)(wsb + L.o_rep), (int*)(wsb + L.o_bsum),
-                   (u64*)(wsb + L.o_scal) + kScalCanon, st);
+                   (u64*)(wsb + L.o_scal) + kScalCanon, st, cr.k);
   ++g_launches; merge_canon_kernel<<<blocks_for(nr, 256), 256, 0, st>>>(nr, cr.colour, first_l, 0, local_colors, is_first);
   rc = check_cuda(cudaStreamSynchronize(st));
   if (rc) return rc;
@@ -1096,7 +1096,7 @@ static int coo_first_iteration(int64_t n, int nb, const wl_edge_batch* batches, 
   COO_ALLOC(d_Hc, sizeof(int) * (size_t)n);
   COO_ALLOC(d_first, sizeof(int) * (size_t)n);
   COO_ALLOC(d_cof, sizeof(int) * (size_t)n);
-  COO_ALLOC(d_bsum, sizeof(int) * (size_t)(nscan + 1));
+  COO_ALLOC(d_bsum, sizeof(int) * canon_scratch_ints(n));
   COO_ALLOC(d_ws, ws_bytes);
   COO_ALLOC(d_rowlen, sizeof(int) * (size_t)max_nl);
   COO_ALLOC(d_lrp, sizeof(int64_t) * (size_t)(max_nl + 1));
@@ -1595,7 +1595,11 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
       }
       gap(next_node, r0[k]);
       next_node = std::max(next_node, r1[k]);
-      if (nr == 0) continue;
+      if (nr == 0) {  // a batch inside one cut row: nothing to refine, but its range check must have read the buffer before
+                      // the upload after next reuses it (the synchronisation that ends every other batch)
+        rc = check_cuda(cudaStreamSynchronize(st));
+        continue;
+      }
       const int64_t e0 = rp[r0[k]], e1 = rp[r1[k]];
       wl_csr lg;
       lg.n = nr;
@@ -1617,7 +1621,7 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
       char* wsb = (char*)d_ws.p;
       int* first_l = (int*)(wsb + L.o_tmp);
       launch_canonical(L, nr, cr.colour, d_Hc.as<int>() + r0[k], first_l, (int*)(wsb + L.o_rep), (int*)(wsb + L.o_bsum),
-                       (u64*)(wsb + L.o_scal) + kScalCanon, st);
+                       (u64*)(wsb + L.o_scal) + kScalCanon, st, cr.k);
       ++g_launches; merge_canon_kernel<<<blocks_for(nr, 256), 256, 0, st>>>(nr, cr.colour, first_l, (int)base_id, d_Hc.as<int>() + r0[k], d_isrep.as<unsigned char>() + r0[k]);
       base_id += cr.k;
       edges_streamed += cr.edges_streamed;
@@ -1845,7 +1849,7 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
       char* wsb = (char*)d_ws2.p;
       int* first_l = (int*)(wsb + L2.o_tmp);
       launch_canonical(L2, nr, cr.colour, d_Hnext.as<int>() + pending.b_lo, first_l, (int*)(wsb + L2.o_rep), (int*)(wsb + L2.o_bsum),
-                       (u64*)(wsb + L2.o_scal) + kScalCanon, side_st);
+                       (u64*)(wsb + L2.o_scal) + kScalCanon, side_st, cr.k);
       ++g_launches; merge_canon_kernel<<<blocks_for(nr, 256), 256, 0, side_st>>>(nr, cr.colour, first_l, (int)base_next, d_Hnext.as<int>() + pending.b_lo, d_isrep_next.as<unsigned char>() + pending.b_lo);
       base_next += cr.k;
       edges_streamed += cr.edges_streamed;

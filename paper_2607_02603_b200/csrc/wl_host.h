@@ -47,8 +47,13 @@ struct CoreResult {
 int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, const wl_options* opt, bool ranged, int lo,
                 int hi, int64_t n_targets, int64_t edge_first, void* workspace, size_t workspace_bytes, const Layout& L,
                 cudaStream_t st, CoreResult* res);
+// ints of scan scratch the canonicalisation needs: chunk sums + one flag bit per node (kCanonChunk / 32 words per chunk)
+static inline size_t canon_scratch_ints(int64_t n) {
+  const size_t nscan = (size_t)((n + kCanonChunk - 1) / kCanonChunk);
+  return nscan + 1 + nscan * (kCanonChunk / 32);
+}
 void launch_canonical(const Layout& L, int64_t n, const int* colour, int* out, int* first, int* cof, int* bsum, u64* total,
-                      cudaStream_t st);
+                      cudaStream_t st, int64_t k = -1);
 u64* host_scal();
 static inline unsigned blocks_for(int64_t count, int threads) { return (unsigned)((count + threads - 1) / threads); }
 static inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }

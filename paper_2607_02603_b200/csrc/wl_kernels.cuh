@@ -831,6 +831,12 @@ relabel_kernel(int64_t count, const int* __restrict__ nodes, int* __restrict__ c
 // look, see compact_active_kernel).  z is not stored: round 2 recomputes it for every listed row before reading it.
 // The list is a superset of what compact_active_kernel would keep (it keeps the few nodes whose degree is unique);
 // counters[0] = listed rows, counters[1] = their out-degree sum (= m), *hub_rows = listed rows longer than hub_threshold.
+// Degree classes repeat: 63 M listed rows of the headline graph share 3 855 keys, so every CTA keeps the ids it has already
+// seen in shared memory (s_id[d] = id of the class of out-degree d, bit 30 = "stamp[id] is known to be set") and walks its
+// tiles grid-stride; only the first sight of a degree in a CTA goes to the global table (1.29 ms -> see profiles/).
+constexpr int kR1Cache = 4096;       // out-degrees below this are cached per CTA (16 KB)
+constexpr int kR1Sub = 8;            // sub-tiles of kRelabelThreads nodes per list reservation
+constexpr int kR1Stamped = 1 << 30;  // round-1 ids stay far below 2^30 (at most sqrt(2m) + 1 distinct degrees)
 __global__ void __launch_bounds__(kRelabelThreads)
 round1_uniform_kernel(int64_t n, const int64_t* __restrict__ row_ptr, int64_t expect_first, int64_t expect_last, u64 w0,
                       int* __restrict__ colour, unsigned short* __restrict__ colour16, int* __restrict__ rep,
@@ -840,92 +846,144 @@ round1_uniform_kernel(int64_t n, const int64_t* __restrict__ row_ptr, int64_t ex
                       u64* __restrict__ hub_rows, u32* __restrict__ err, u64 ymask, u64* __restrict__ tag64,
                       int64_t tag_threshold, u32 idmask) {
   constexpr int round = 1, k_old = 1;
-  const int64_t t = (int64_t)blockIdx.x * kRelabelThreads + threadIdx.x;
-  const bool valid = t < n;
-  const int i = (int)t;
-  int64_t d = 0;
-  if (valid) {
-    const int64_t a = row_ptr[t], b = row_ptr[t + 1];
-    u32 e = 0;
-    if (t == 0 && a != expect_first) e |= kErrRowPtr;
-    if (t == n - 1 && b != expect_last) e |= kErrRowPtr;
-    if (a > b || a < expect_first || b > expect_last) e |= kErrRowPtr;
-    d = e ? 0 : b - a;
-    if ((u64)d >= (1ull << 32)) e |= kErrRowSum, d = 0;
-    if (d > hub_threshold) {
-      const int nc = (int)((d + kHubChunk - 1) / kHubChunk);
-      const u64 base = atomicAdd(hub_counter, (u64)nc);
-      if ((int64_t)(base + nc) <= hub_cap) {
-        for (int c = 0; c < nc; ++c) chunks[base + c] = make_int2(i, c);
-      } else {
-        e |= kErrRowPtr;  // only overlapping (malformed) rows can exceed the capacity derived from m
-      }
-      atomicAdd(hub_rows, 1ull);
-    }
-    if (e) atomicOr(err, e);
-    // hot-id table of the coming rounds: the highest-degree node wins its slot (out-degree stands in for the number of gathers
-    // a node receives; any choice is correct, a miss falls through to the global gather)
-    if (tag64 && d >= tag_threshold) atomicMax(tag64 + (tag_mix((u32)i, idmask) & (kTagSlots - 1)), ((u64)d << 32) | (u64)(u32)i);
-  }
+  constexpr int kWarps = kRelabelThreads / 32;
+  __shared__ int s_id[kR1Cache];
+  __shared__ u64 s_base, s_list;
+  __shared__ int s_stamp0;
+  __shared__ int s_cnt[kR1Sub * kWarps];
+  for (int j = threadIdx.x; j < kR1Cache; j += kRelabelThreads) s_id[j] = -1;
+  if (threadIdx.x == 0) s_stamp0 = 0;
+  __syncthreads();
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   // the representative of colour 0 is node 0
   int64_t d0 = row_ptr[1] - row_ptr[0];
   if (d0 < 0 || (u64)d0 >= (1ull << 32)) d0 = 0;
-  bool win = false, lose = false;
-  u32 slot = 0, id = 0;
-  if (valid) {
-    const u64 yi = ((u64)d * w0) & ymask;
-    if (yi == (((u64)d0 * w0) & ymask)) {
-      if (i != 0 && stamp[0] != round) stamp[0] = round;
-    } else {
-      id = kPending;
-      const Slot mine = {yi, (u64)kPending << 32};
-      const Slot empty = {kEmpty, kEmpty};
-      slot = (u32)slot_hash(0u, yi) & table_mask;
-      while (true) {
-        Slot v = load_slot(table + slot);
-        if (v.y == kEmpty || v.cx == kEmpty) {
-          v = cas128(table + slot, empty, mine);
-          if (v.y == kEmpty && v.cx == kEmpty) {
-            win = true;
-            break;
+  const u64 y0 = ((u64)d0 * w0) & ymask;
+  constexpr int64_t kSuper = (int64_t)kR1Sub * kRelabelThreads;
+  const int64_t supers = (n + kSuper - 1) / kSuper;
+  for (int64_t sup = blockIdx.x; sup < supers; sup += gridDim.x) {
+    unsigned kb[kR1Sub];  // per sub-tile: which lanes of this warp list their node
+#pragma unroll
+    for (int q = 0; q < kR1Sub; ++q) {
+      const int64_t t = sup * kSuper + (int64_t)q * kRelabelThreads + threadIdx.x;
+      const bool valid = t < n;
+      const int i = (int)t;
+      int64_t d = 0;
+      if (valid) {
+        const int64_t a = row_ptr[t], b = row_ptr[t + 1];
+        u32 e = 0;
+        if (t == 0 && a != expect_first) e |= kErrRowPtr;
+        if (t == n - 1 && b != expect_last) e |= kErrRowPtr;
+        if (a > b || a < expect_first || b > expect_last) e |= kErrRowPtr;
+        d = e ? 0 : b - a;
+        if ((u64)d >= (1ull << 32)) e |= kErrRowSum, d = 0;
+        if (d > hub_threshold) {
+          const int nc = (int)((d + kHubChunk - 1) / kHubChunk);
+          const u64 base = atomicAdd(hub_counter, (u64)nc);
+          if ((int64_t)(base + nc) <= hub_cap) {
+            for (int c = 0; c < nc; ++c) chunks[base + c] = make_int2(i, c);
+          } else {
+            e |= kErrRowPtr;  // only overlapping (malformed) rows can exceed the capacity derived from m
+          }
+          atomicAdd(hub_rows, 1ull);
+        }
+        if (e) atomicOr(err, e);
+        // hot-id table of the coming rounds: the highest-degree node wins its slot (out-degree stands in for the number of
+        // gathers a node receives; any choice is correct, a miss falls through to the global gather)
+        if (tag64 && d >= tag_threshold) atomicMax(tag64 + (tag_mix((u32)i, idmask) & (kTagSlots - 1)), ((u64)d << 32) | (u64)(u32)i);
+      }
+      bool win = false, lose = false;
+      u32 slot = 0, id = 0;
+      if (valid) {
+        const u64 yi = ((u64)d * w0) & ymask;
+        if (yi == y0) {
+          if (i != 0 && !s_stamp0) {
+            if (stamp[0] != round) stamp[0] = round;
+            s_stamp0 = 1;
+          }
+        } else {
+          const int e = d < kR1Cache ? s_id[d] : -1;
+          if (e >= 0) {  // this CTA has met the class before: same out-degree, same key, same id
+            id = (u32)(e & (kR1Stamped - 1));
+            if (!(e & kR1Stamped)) {
+              if (stamp[id] != round) stamp[id] = round;
+              s_id[d] = e | kR1Stamped;
+            }
+          } else {
+            id = kPending;
+            const Slot mine = {yi, (u64)kPending << 32};
+            const Slot empty = {kEmpty, kEmpty};
+            slot = (u32)slot_hash(0u, yi) & table_mask;
+            while (true) {
+              Slot v = load_slot(table + slot);
+              if (v.y == kEmpty || v.cx == kEmpty) {
+                v = cas128(table + slot, empty, mine);
+                if (v.y == kEmpty && v.cx == kEmpty) {
+                  win = true;
+                  break;
+                }
+              }
+              if (v.y == yi && (u32)v.cx == 0u) {
+                lose = true;
+                id = (u32)(v.cx >> 32);
+                break;
+              }
+              slot = (slot + 1) & table_mask;
+            }
           }
         }
-        if (v.y == yi && (u32)v.cx == 0u) {
-          lose = true;
-          id = (u32)(v.cx >> 32);
-          break;
-        }
-        slot = (slot + 1) & table_mask;
       }
+      if (__syncthreads_or(win)) {  // rare after the first tiles of a CTA: some thread claimed a new class
+        int total;
+        const int rank = block_rank<kRelabelThreads>(win, &total);
+        if (threadIdx.x == 0) s_base = atomicAdd(new_counter, (u64)total);
+        __syncthreads();
+        if (win) {
+          id = (u32)(k_old + (int)s_base + rank);
+          st_slot_id(table + slot, id);
+          rep[id] = i;
+          slot_of[id] = slot;
+          if (d < kR1Cache && id < (u32)kR1Stamped) s_id[d] = (int)id;
+        }
+      }
+      if (lose) {
+        while (id == kPending) id = ld_slot_id(table + slot);
+        if (stamp[id] != round) stamp[id] = round;
+        if (d < kR1Cache && id < (u32)kR1Stamped) s_id[d] = (int)id | kR1Stamped;
+      }
+      if (valid) {
+        colour[i] = (int)id;
+        colour16[i] = (unsigned short)id;
+      }
+      // active list: every node with an out-edge
+      kb[q] = __ballot_sync(0xffffffffu, valid && d > 0);
+      if (lane == 0) s_cnt[q * kWarps + wid] = __popc(kb[q]);
     }
+    // one list reservation per super-tile (the same-address atomic is what bounds a tile-per-atomic version); node order kept
+    __syncthreads();
+    if (wid == 0) {
+      static_assert(kR1Sub * kWarps == 64, "one warp scans two counts per lane");
+      const int c0 = s_cnt[2 * lane], c1 = s_cnt[2 * lane + 1];
+      int x = c0 + c1;
+      const int mine = x;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        int u = __shfl_up_sync(0xffffffffu, x, o);
+        if (lane >= o) x += u;
+      }
+      s_cnt[2 * lane] = x - mine;
+      s_cnt[2 * lane + 1] = x - mine + c0;
+      if (lane == 31 && x > 0) s_list = atomicAdd(counters, (u64)x);
+    }
+    __syncthreads();
+#pragma unroll
+    for (int q = 0; q < kR1Sub; ++q)
+      if ((kb[q] >> lane) & 1u)
+        active[s_list + s_cnt[q * kWarps + wid] + __popc(kb[q] & ((1u << lane) - 1))] =
+            (int)(sup * kSuper + (int64_t)q * kRelabelThreads + threadIdx.x);
+    __syncthreads();  // s_cnt / s_list are rewritten by the next super-tile
   }
-  int total;
-  const int rank = block_rank<kRelabelThreads>(win, &total);
-  __shared__ u64 s_base;
-  if (threadIdx.x == 0 && total > 0) s_base = atomicAdd(new_counter, (u64)total);
-  __syncthreads();
-  if (win) {
-    id = (u32)(k_old + (int)s_base + rank);
-    st_slot_id(table + slot, id);
-    rep[id] = i;
-    slot_of[id] = slot;
-  } else if (lose) {
-    while (id == kPending) id = ld_slot_id(table + slot);
-    if (stamp[id] != round) stamp[id] = round;
-  }
-  if (valid) {
-    colour[i] = (int)id;
-    colour16[i] = (unsigned short)id;
-  }
-  // active list: every node with an out-edge
-  const bool keep = valid && d > 0;
-  int kept;
-  const int krank = block_rank<kRelabelThreads>(keep, &kept);
-  __shared__ u64 s_list;
-  if (threadIdx.x == 0 && kept > 0) s_list = atomicAdd(counters, (u64)kept);
-  __syncthreads();
-  if (keep) active[s_list + krank] = i;
-  if (t == 0) counters[1] = (u64)(expect_last - expect_first);
+  if (blockIdx.x == 0 && threadIdx.x == 0) counters[1] = (u64)(expect_last - expect_first);
 }
 
 // End of a round (S4): if `clean`, the slots claimed by this round's new ids are emptied again (the table is empty
@@ -992,26 +1050,43 @@ __global__ void fill_i32_kernel(int64_t n, int* __restrict__ a, int v) {
   if (i < n) a[i] = v;
 }
 
-__global__ void first_node_kernel(int64_t n, const int* __restrict__ colour, int* __restrict__ first) {
-  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n) return;
-  const int c = colour[i];
-  if (first[c] > (int)i) atomicMin(first + c, (int)i);
+// four nodes per thread (strided by the CTA width): the colour loads, then the four dependent first[] loads, are in flight together
+constexpr int kFirstItems = 4;
+__global__ void __launch_bounds__(256)
+first_node_kernel(int64_t n, const int* __restrict__ colour, int* __restrict__ first) {
+  const int64_t base = (int64_t)blockIdx.x * (256 * kFirstItems) + threadIdx.x;
+  int c[kFirstItems], f[kFirstItems];
+#pragma unroll
+  for (int k = 0; k < kFirstItems; ++k) c[k] = base + k * 256 < n ? colour[base + k * 256] : -1;
+#pragma unroll
+  for (int k = 0; k < kFirstItems; ++k) f[k] = c[k] >= 0 ? first[c[k]] : 0;
+#pragma unroll
+  for (int k = 0; k < kFirstItems; ++k)
+    if (c[k] >= 0 && f[k] > (int)(base + k * 256)) atomicMin(first + c[k], (int)(base + k * 256));
 }
 
+// flags: one bit per node, "node i is the first node of its block", kCanonWords words per chunk of kScanChunk nodes (word
+// 8 k + w of a chunk = nodes 32 (8 k + w) .. + 31 of it).  Written once here; the rank and apply passes read the bits
+// instead of gathering first[colour[i]] again.
+constexpr int kCanonWords = kScanChunk / 32;
 __global__ void __launch_bounds__(kScanThreads)
-canon_count_kernel(int64_t n, const int* __restrict__ colour, const int* __restrict__ first, int* __restrict__ bsum) {
+canon_count_kernel(int64_t n, const int* __restrict__ colour, const int* __restrict__ first, int* __restrict__ bsum,
+                   u32* __restrict__ flags) {
   const int64_t base = (int64_t)blockIdx.x * kScanChunk;
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   int cnt = 0;
 #pragma unroll
   for (int k = 0; k < kScanItems; ++k) {
     int64_t i = base + threadIdx.x + k * kScanThreads;
-    if (i < n) cnt += (first[colour[i]] == (int)i);
+    const bool f = i < n && first[colour[i]] == (int)i;
+    const unsigned b = __ballot_sync(0xffffffffu, f);
+    if (lane == 0) flags[(int64_t)blockIdx.x * kCanonWords + k * (kScanThreads / 32) + wid] = b;
+    cnt += f;
   }
   __shared__ int s[kScanThreads / 32];
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) cnt += __shfl_xor_sync(0xffffffffu, cnt, o);
-  if ((threadIdx.x & 31) == 0) s[threadIdx.x >> 5] = cnt;
+  if (lane == 0) s[wid] = cnt;
   __syncthreads();
   if (threadIdx.x == 0) {
     int t = 0;
@@ -1058,46 +1133,77 @@ __global__ void __launch_bounds__(1024) scan_bsum_kernel(int64_t nb, int* __rest
   if (threadIdx.x == 0) *out_total = (u64)s_carry;
 }
 
-// cid[c] = rank of block c among the blocks ordered by their first node
-__global__ void __launch_bounds__(kScanThreads)
-canon_rank_kernel(int64_t n, const int* __restrict__ colour, const int* __restrict__ first,
-                  const int* __restrict__ bsum, int* __restrict__ cid) {
-  // blocked arrangement so that ranks follow node order
-  const int64_t base = (int64_t)blockIdx.x * kScanChunk + (int64_t)threadIdx.x * kScanItems;
-  int f[kScanItems];  // colour of node base + k if it is the first node of its block, else -1
-  int cnt = 0;
-#pragma unroll
-  for (int k = 0; k < kScanItems; ++k) {
-    int64_t i = base + k;
-    f[k] = -1;
-    if (i < n) {
-      const int c = colour[i];
-      if (first[c] == (int)i) f[k] = c;
-    }
-    cnt += f[k] >= 0;
-  }
+// the flag words of this CTA's chunk and their exclusive prefix counts (both in shared memory)
+__device__ __forceinline__ void canon_chunk_prefix(const u32* __restrict__ flags, u32* s_word, int* s_pref) {
+  static_assert(kCanonWords == 64, "two warps scan the flag words of a chunk");
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-  int x = cnt;
+  __shared__ int s_half;
+  if (wid < 2) {
+    const u32 w = flags[(int64_t)blockIdx.x * kCanonWords + threadIdx.x];
+    const int c = __popc(w);
+    int x = c;
 #pragma unroll
-  for (int o = 1; o < 32; o <<= 1) {
-    int t = __shfl_up_sync(0xffffffffu, x, o);
-    if (lane >= o) x += t;
+    for (int o = 1; o < 32; o <<= 1) {
+      int t = __shfl_up_sync(0xffffffffu, x, o);
+      if (lane >= o) x += t;
+    }
+    s_word[threadIdx.x] = w;
+    s_pref[threadIdx.x] = x - c;
+    if (threadIdx.x == 31) s_half = x;
   }
-  __shared__ int s_w[kScanThreads / 32];
-  if (lane == 31) s_w[wid] = x;
   __syncthreads();
-  int woff = 0;
-  for (int w = 0; w < wid; ++w) woff += s_w[w];
-  int r = bsum[blockIdx.x] + woff + x - cnt;
-#pragma unroll
-  for (int k = 0; k < kScanItems; ++k)
-    if (f[k] >= 0) cid[f[k]] = r++;
+  if (wid == 1) s_pref[threadIdx.x] += s_half;
+  __syncthreads();
 }
 
-__global__ void canon_apply_kernel(int64_t n, const int* __restrict__ colour, const int* __restrict__ cid,
-                                   int* __restrict__ out) {
-  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i < n) out[i] = cid[colour[i]];
+// cid[c] = rank of block c among the blocks ordered by their first node (the flagged nodes, in node order)
+__global__ void __launch_bounds__(kScanThreads)
+canon_rank_kernel(int64_t n, const int* __restrict__ colour, const u32* __restrict__ flags,
+                  const int* __restrict__ bsum, int* __restrict__ cid) {
+  __shared__ u32 s_word[kCanonWords];
+  __shared__ int s_pref[kCanonWords];
+  canon_chunk_prefix(flags, s_word, s_pref);
+  const int64_t base = (int64_t)blockIdx.x * kScanChunk;
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  const int r0 = bsum[blockIdx.x];
+#pragma unroll
+  for (int k = 0; k < kScanItems; ++k) {
+    const int wi = k * (kScanThreads / 32) + wid;
+    const u32 w = s_word[wi];
+    if ((w >> lane) & 1u) {
+      const int64_t i = base + threadIdx.x + k * kScanThreads;
+      cid[colour[i]] = r0 + s_pref[wi] + __popc(w & ((1u << lane) - 1));
+    }
+  }
+}
+
+// out[i] = canonical id of node i's block: its own rank for a first node (from the flag bits), cid[colour[i]] otherwise
+__global__ void __launch_bounds__(kScanThreads)
+canon_apply_kernel(int64_t n, const int* __restrict__ colour, const int* __restrict__ cid, const u32* __restrict__ flags,
+                   const int* __restrict__ bsum, int* __restrict__ out) {
+  __shared__ u32 s_word[kCanonWords];
+  __shared__ int s_pref[kCanonWords];
+  canon_chunk_prefix(flags, s_word, s_pref);
+  const int64_t base = (int64_t)blockIdx.x * kScanChunk;
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  const int r0 = bsum[blockIdx.x];
+  int c[kScanItems], v[kScanItems];
+#pragma unroll
+  for (int k = 0; k < kScanItems; ++k) {  // colours of the nodes that are not the first of their block (the others need none)
+    const int64_t i = base + threadIdx.x + k * kScanThreads;
+    const u32 w = s_word[k * (kScanThreads / 32) + wid];
+    c[k] = (i < n && !((w >> lane) & 1u)) ? colour[i] : -1;
+  }
+#pragma unroll
+  for (int k = 0; k < kScanItems; ++k) v[k] = c[k] >= 0 ? cid[c[k]] : 0;
+#pragma unroll
+  for (int k = 0; k < kScanItems; ++k) {
+    const int64_t i = base + threadIdx.x + k * kScanThreads;
+    if (i >= n) continue;
+    const int wi = k * (kScanThreads / 32) + wid;
+    const u32 w = s_word[wi];
+    out[i] = ((w >> lane) & 1u) ? r0 + s_pref[wi] + __popc(w & ((1u << lane) - 1)) : v[k];
+  }
 }
 
 }  // namespace wl

@@ -3,6 +3,7 @@
 #include "wl_host.h"
 
 #include <algorithm>
+#include <chrono>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
@@ -46,7 +47,7 @@ Layout make_layout(int64_t n, int64_t m) {
   L.o_tmp = take(sizeof(u32) * (size_t)n);
   L.o_y = take(sizeof(u64) * (size_t)n);
   L.o_tile_row = take(sizeof(int) * (size_t)(L.ntiles + 1));
-  L.o_bsum = take(sizeof(int) * (size_t)(L.nscan + 1));
+  L.o_bsum = take(sizeof(int) * canon_scratch_ints(n));
   L.o_table = take(sizeof(Slot) * ((size_t)L.table_mask + 1));
   L.o_colour16 = take(sizeof(unsigned short) * (size_t)n);
   L.o_act0 = take(sizeof(int) * (size_t)n);
@@ -249,16 +250,20 @@ static u32 round_table_mask(const Layout& L, int64_t n_active) {
   return (u32)(s - 1);
 }
 
-// canonical ids: uses `first` (int[n], first node per colour) and `cid` (int[n], canonical id per colour) as scratch, bsum int[nscan+1], total -> scal slot
+// canonical ids: uses `first` (int[n], first node per colour) and `cid` (int[n], canonical id per colour) as scratch, bsum =
+// canon_scratch_ints(n) ints (chunk sums + one flag bit per node), total -> scal slot.  k > 0: the colour ids are < k (only that
+// much of `first` is initialised and meaningful afterwards).
 void launch_canonical(const Layout& L, int64_t n, const int* colour, int* out, int* first, int* cid, int* bsum,
-                      u64* total, cudaStream_t st) {
+                      u64* total, cudaStream_t st, int64_t k) {
   if (n == 0) return;
-  ++g_launches; fill_i32_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, first, kNoNode);
-  ++g_launches; first_node_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, colour, first);
-  ++g_launches; canon_count_kernel<<<(unsigned)L.nscan, kScanThreads, 0, st>>>(n, colour, first, bsum);
+  const int64_t kk = k > 0 && k < n ? k : n;
+  u32* flags = (u32*)(bsum + L.nscan + 1);
+  ++g_launches; fill_i32_kernel<<<blocks_for(kk, 256), 256, 0, st>>>(kk, first, kNoNode);
+  ++g_launches; first_node_kernel<<<blocks_for(n, 256 * kFirstItems), 256, 0, st>>>(n, colour, first);
+  ++g_launches; canon_count_kernel<<<(unsigned)L.nscan, kScanThreads, 0, st>>>(n, colour, first, bsum, flags);
   ++g_launches; scan_bsum_kernel<<<1, 1024, 0, st>>>(L.nscan, bsum, total);
-  ++g_launches; canon_rank_kernel<<<(unsigned)L.nscan, kScanThreads, 0, st>>>(n, colour, first, bsum, cid);
-  ++g_launches; canon_apply_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, colour, cid, out);
+  ++g_launches; canon_rank_kernel<<<(unsigned)L.nscan, kScanThreads, 0, st>>>(n, colour, flags, bsum, cid);
+  ++g_launches; canon_apply_kernel<<<(unsigned)L.nscan, kScanThreads, 0, st>>>(n, colour, cid, flags, bsum, out);
 }
 
 // WL_DEBUG (per-round trace on stderr) is read once per process, not per call
@@ -359,6 +364,7 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
                 cudaStream_t st, CoreResult* res) {
   const int64_t n = g->n, m = g->m;
   int rc = WL_OK;
+  const auto t_entry = std::chrono::steady_clock::now();  // (WL_DEBUG trace only)
   const uint32_t flags = opt ? opt->flags : 0u;
   const int64_t max_rounds = (opt && opt->max_rounds > 0) ? opt->max_rounds : n + 1;
   const uint64_t stream_id = opt ? opt->stream_id : 0;
@@ -469,7 +475,7 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
     // S0 and round 1 in one pass over row_ptr (round1_uniform_kernel); the loop below only closes the round
     const u64 w0 = weight_of(round_key(seed, stream_id, 1), 0);
     const u32 mask1 = overlap ? (u32)(prefix_slots - 1) : L.table_mask;
-    ++g_launches; round1_uniform_kernel<<<blocks_for(n, kRelabelThreads), kRelabelThreads, 0, st>>>(n, g->row_ptr, edge_first, edge_first + m, w0, colour, colour16, rep, stamp, table, mask1, slot_of, scal + kScalNew, kHubThreshold, hub_chunks, L.hub_cap, scal + kScalHub, act[0], scal + kScalActive, scal + kScalActiveHub, d_err, ymask, tag_possible ? tag64 : nullptr,
+    ++g_launches; round1_uniform_kernel<<<(unsigned)std::min<int64_t>(blocks_for(n, kRelabelThreads * kR1Sub), 148 * 8), kRelabelThreads, 0, st>>>(n, g->row_ptr, edge_first, edge_first + m, w0, colour, colour16, rep, stamp, table, mask1, slot_of, scal + kScalNew, kHubThreshold, hub_chunks, L.hub_cap, scal + kScalHub, act[0], scal + kScalActive, scal + kScalActiveHub, d_err, ymask, tag_possible ? tag64 : nullptr,
                                                                                                   std::max<int64_t>(64, 8 * (m / std::max<int64_t>(n, 1))), idmask);
   } else {
     if (!cols_checked) {
@@ -509,6 +515,7 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
   int32_t rounds = 0, spmv_launches = 0;
   bool converged = false;
   const bool debug = debug_enabled();
+  auto wall_ms = [&]() { return std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t_entry).count(); };
   constexpr double list_frac = 0.75;  // an active list pays once a quarter of the rows has left (measured, scale 27)
   const bool no_runahead = (flags & WL_FLAG_SYNC_EVERY_ROUND) != 0;
   const int* cur_list = nullptr;  // NULL: every node is active
@@ -711,7 +718,7 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
       pending_new += k_new - k;
       k = k_new;
     }
-    if (debug) std::fprintf(stderr, "[wl_refine]   %d round(s): spmv %.3f ms, rest %.3f ms\n", R, t_spmv, t_all - t_spmv);
+    if (debug) std::fprintf(stderr, "[wl_refine]   %d round(s): spmv %.3f ms, rest %.3f ms; host clock %.3f ms since the rounds began\n", R, t_spmv, t_all - t_spmv, wall_ms());
     r += R;
     if (converged) break;
     if (switch_round) {
@@ -877,13 +884,15 @@ int wl_refine(const wl_csr* g, const int32_t* init_colors, uint64_t seed, int32_
   const int core_rc = refine_core(g, init_colors, seed, opt, /*ranged=*/false, 0, 0, n, /*edge_first=*/0, workspace, workspace_bytes, L, st, &cr);
   if (core_rc != WL_OK && core_rc != WL_EMAXROUNDS) return core_rc;
   char* ws = (char*)workspace;
+  cudaEvent_t ev_s6 = evp.get(2);
+  cudaEventRecord(ev_s6, st);
   // ---- S6: canonical ids ---------------------------------------------------------------------------------------------
   if (flags & WL_FLAG_NO_CANONICAL) {
     cudaMemcpyAsync(out_colors, cr.colour, sizeof(int) * (size_t)n, cudaMemcpyDeviceToDevice, st);
   } else {
     // scratch: tmp -> first node per colour, rep -> canonical id per colour (both dead now)
     launch_canonical(L, n, cr.colour, out_colors, (int*)(ws + L.o_tmp), (int*)(ws + L.o_rep), (int*)(ws + L.o_bsum),
-                     (u64*)(ws + L.o_scal) + kScalCanon, st);
+                     (u64*)(ws + L.o_scal) + kScalCanon, st, cr.k);
   }
   cudaEventRecord(ev_end, st);
   rc = check_cuda(cudaStreamSynchronize(st));
@@ -893,6 +902,11 @@ int wl_refine(const wl_csr* g, const int32_t* init_colors, uint64_t seed, int32_
   if (stats) {
     float t = 0;
     cudaEventElapsedTime(&t, ev_begin, ev_end);
+    if (debug_enabled()) {
+      float t6 = 0;
+      cudaEventElapsedTime(&t6, ev_s6, ev_end);
+      std::fprintf(stderr, "[wl_refine] total %.3f ms on the stream, of which S6 %.3f ms\n", t, t6);
+    }
     stats->rounds = cr.rounds;
     stats->num_colors = cr.k;
     stats->edges_streamed = cr.edges_streamed;
