@@ -100,6 +100,13 @@ typedef struct wl_options {
   int32_t ring_bits;        /* Algorithm 1's precision parameter q (L109-L110): the ring is Z/2^q.  0 or >= 64: q = 64, the
                                only setting Theorem 1's 1e-9 guarantee covers (L129).  1..63: every z is reduced mod 2^q where
                                it is compared; used to COUNT collisions (Lemma 1), never for production results          */
+  int32_t host_pieces;      /* wl_refine_host only: number of pieces (whole rows each) the column upload is cut into so that the
+                               first pass over the columns runs behind the link; <= 0: about 256 MB per piece, at most 32     */
+  void* device_workspace;   /* wl_refine_host only, optional: DEVICE scratch (256-byte aligned) that holds the uploaded graph and
+                               the refinement workspace; NULL: the library allocates its own inside the call and frees it before
+                               returning (cudaFree of the 28.6 GB a scale-27 call needs costs 9-17 ms: callers that refine
+                               repeatedly pass one).  Caller-owned, contents undefined before and after.                       */
+  size_t device_workspace_bytes; /* >= wl_refine_host_device_bytes(n, m, weighted, with_init); a smaller one is WL_ENOMEM      */
 } wl_options;
 
 typedef struct wl_stats {
@@ -137,6 +144,8 @@ size_t wl_refine_workspace_bytes(int64_t n, int64_t m);
  * from round 7 on only the rows with a changed out-neighbour are recomputed, under one fixed weight key (same partitions
  * per round, same fixed point; S5).  wl_refine uses that regime when the workspace it is given is at least this large. */
 size_t wl_refine_deep_workspace_bytes(int64_t n, int64_t m);
+/* device bytes one wl_refine_host call needs (CSR + optional weights / initial partition + colours + wl_refine_workspace_bytes) */
+size_t wl_refine_host_device_bytes(int64_t n, int64_t m, int weighted, int with_init);
 
 /* Coarsest stable colouring refining init_colors, with error probability <= 1e-9 (Theorem 1).
  *   g            CSR, all arrays DEVICE.
@@ -150,7 +159,10 @@ int wl_refine(const wl_csr* g, const int32_t* init_colors, uint64_t seed, int32_
               const wl_options* opt, void* workspace, size_t workspace_bytes, void* cuda_stream);
 
 /* Same computation from HOST buffers (the end-to-end call): allocates its own device memory, copies the CSR and
- * init_colors host -> device, runs wl_refine, copies the colours device -> host.  g arrays, init_colors, out_colors: HOST. */
+ * init_colors host -> device, runs wl_refine, copies the colours device -> host.  g arrays, init_colors, out_colors: HOST
+ * (pinned memory if the copies are to overlap the rounds).  The uploads run on a stream of the library's own in the order
+ * the rounds need them (row offsets, then the columns in opt->host_pieces pieces of whole rows); S0, round 1 and the first
+ * pass over the columns (S1+S2 piece by piece) run behind the link.  Same results as wl_refine. */
 int wl_refine_host(const wl_csr* g, const int32_t* init_colors, uint64_t seed, int32_t* out_colors, wl_stats* stats,
                    const wl_options* opt, void* cuda_stream);
 

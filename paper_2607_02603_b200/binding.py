@@ -29,7 +29,7 @@ WL_FLAG_TAG_TABLE = 16384
 WL_FLAG_TEST_SMALL_OVERFLOW = 1 << 29
 
 EXPORTS = [
-    "wl_refine_workspace_bytes", "wl_refine_deep_workspace_bytes", "wl_refine", "wl_refine_host", "wl_round_key", "wl_weight", "wl_spmv_round",
+    "wl_refine_workspace_bytes", "wl_refine_deep_workspace_bytes", "wl_refine_host_device_bytes", "wl_refine", "wl_refine_host", "wl_round_key", "wl_weight", "wl_spmv_round",
     "wl_spmv_rows", "wl_relabel", "wl_canonicalize", "wl_refine_batched", "wl_refine_batched_host_bytes", "wl_refine_batched_host_bytes_consume", "wl_inner_labels", "wl_quotient",
     "wl_quotient_workspace_bytes", "wl_refine_inner", "wl_refine_inner_workspace_bytes", "wl_quotient_rows",
     "wl_quotient_rows_workspace_bytes", "wl_strerror", "wl_last_cuda_error", "wl_version", "wl_kernel_launches",
@@ -53,7 +53,8 @@ class wl_csr(C.Structure):
 class wl_options(C.Structure):
     _fields_ = [("flags", C.c_uint32), ("max_rounds", C.c_int32), ("stream_id", C.c_uint64),
                 ("round_colors", C.c_void_p), ("round_colors_cap", C.c_int32), ("max_outer_iters", C.c_int32),
-                ("host_workspace", C.c_void_p), ("host_workspace_bytes", C.c_size_t), ("ring_bits", C.c_int32)]
+                ("host_workspace", C.c_void_p), ("host_workspace_bytes", C.c_size_t), ("ring_bits", C.c_int32),
+                ("host_pieces", C.c_int32), ("device_workspace", C.c_void_p), ("device_workspace_bytes", C.c_size_t)]
 
 
 class wl_stats(C.Structure):
@@ -87,6 +88,8 @@ def lib():
         L.wl_refine_workspace_bytes.argtypes = [i64, i64]
         L.wl_refine_deep_workspace_bytes.restype = sz
         L.wl_refine_deep_workspace_bytes.argtypes = [i64, i64]
+        L.wl_refine_host_device_bytes.restype = sz
+        L.wl_refine_host_device_bytes.argtypes = [i64, i64, C.c_int, C.c_int]
         L.wl_refine.restype = C.c_int
         L.wl_refine.argtypes = [C.POINTER(wl_csr), vp, u64, vp, C.POINTER(wl_stats), C.POINTER(wl_options), vp, sz, vp]
         L.wl_refine_host.restype = C.c_int
@@ -193,6 +196,10 @@ def wl_refine_deep_workspace_bytes(n: int, m: int) -> int:
     return int(lib().wl_refine_deep_workspace_bytes(n, m))
 
 
+def wl_refine_host_device_bytes(n: int, m: int, weighted: bool = False, with_init: bool = False) -> int:
+    return int(lib().wl_refine_host_device_bytes(n, m, int(weighted), int(with_init)))
+
+
 def wl_refine(n: int, row_ptr: torch.Tensor, col_idx: torch.Tensor, weights: Optional[torch.Tensor] = None,
               init_colors: Optional[torch.Tensor] = None, seed: int = 0, *, flags: int = 0, max_rounds: int = 0,
               stream_id: int = 0, workspace: Optional[torch.Tensor] = None, out: Optional[torch.Tensor] = None,
@@ -224,8 +231,10 @@ def wl_refine(n: int, row_ptr: torch.Tensor, col_idx: torch.Tensor, weights: Opt
 
 def wl_refine_host(n: int, row_ptr: torch.Tensor, col_idx: torch.Tensor, weights: Optional[torch.Tensor] = None,
                    init_colors: Optional[torch.Tensor] = None, seed: int = 0, *, flags: int = 0, max_rounds: int = 0,
-                   out: Optional[torch.Tensor] = None, round_cap: int = 4096, device=None) -> RefineResult:
-    """Same computation from HOST tensors (pinned recommended): H2D, refine, D2H all inside the call."""
+                   out: Optional[torch.Tensor] = None, round_cap: int = 4096, device=None, pieces: int = 0,
+                   device_workspace: Optional[torch.Tensor] = None) -> RefineResult:
+    """Same computation from HOST tensors (pinned recommended): H2D, refine, D2H all inside the call; the columns are uploaded
+    in `pieces` pieces (0: chosen by the library) behind which the first rounds already run."""
     L = lib()
     if not torch.cuda.is_available():
         raise RuntimeError("wl_refine_host needs a CUDA device (no CPU fallback)")
@@ -236,7 +245,9 @@ def wl_refine_host(n: int, row_ptr: torch.Tensor, col_idx: torch.Tensor, weights
         out = torch.empty(n, dtype=torch.int32, pin_memory=True)
     _check(out, torch.int32, "cpu", "out", n)
     rc_buf = (C.c_int64 * round_cap)()
-    opt = wl_options(flags, max_rounds, 0, C.cast(rc_buf, C.c_void_p), round_cap, 0, None, 0)
+    _check(device_workspace, torch.uint8, "cuda", "device_workspace")
+    opt = wl_options(flags, max_rounds, 0, C.cast(rc_buf, C.c_void_p), round_cap, 0, None, 0, 0, pieces,
+                     _ptr(device_workspace), 0 if device_workspace is None else device_workspace.numel())
     st = wl_stats()
     with torch.cuda.device(dev):
         rc = L.wl_refine_host(C.byref(g), _ptr(init_colors), seed, _ptr(out), C.byref(st), C.byref(opt),

@@ -44,9 +44,18 @@ struct CoreResult {
   double ms_rest_top;
   int* colour;  // dense ids, inside the workspace
 };
+// wl_refine_host: the column array arrives in pieces while the rounds already run.  row_ptr is complete once `rows_ready` has
+// fired; piece j = the rows [node_end[j-1], node_end[j]) with all their entries, on the device once ready[j] has fired
+// (node_end[pieces-1] = n).  refine_core makes its stream wait for exactly what the next launch reads.
+struct ColumnFeed {
+  int pieces;
+  const int64_t* node_end;
+  const cudaEvent_t* ready;
+  cudaEvent_t rows_ready;
+};
 int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, const wl_options* opt, bool ranged, int lo,
                 int hi, int64_t n_targets, int64_t edge_first, void* workspace, size_t workspace_bytes, const Layout& L,
-                cudaStream_t st, CoreResult* res);
+                cudaStream_t st, CoreResult* res, const ColumnFeed* feed = nullptr);
 // ints of scan scratch the canonicalisation needs: chunk sums + one flag bit per node (kCanonChunk / 32 words per chunk)
 static inline size_t canon_scratch_ints(int64_t n) {
   const size_t nscan = (size_t)((n + kCanonChunk - 1) / kCanonChunk);

@@ -121,6 +121,7 @@ struct SpmvArgs {
   u64* ticket = nullptr;       // zeroed device counter of the persistent kernel
   u64 key2 = 0;                // DUAL rows: second key and second sum (finality test of the coming compaction)
   u64* y2 = nullptr;
+  bool hubs_only = false;      // the row kernel has been launched piece by piece (ColumnFeed): only the hub chunks are left
 };
 
 // edge-balanced S1+S2 over all rows of g (see spmv_eb_kernel)
@@ -163,7 +164,8 @@ static void launch_rows_tag(const wl_csr& g, const SpmvArgs& a, u64 key, u64* y,
 template <bool W, typename CT, bool R, bool V>
 static void launch_row_hub2(const wl_csr& g, const SpmvArgs& a, const CT* colour, u64 key, u64* y, cudaStream_t st) {
   unsigned grid = blocks_for(a.nrows, kRowsCta);
-  if (!W && !R && a.tag32 && a.narrow) {
+  if (a.hubs_only) {
+  } else if (!W && !R && a.tag32 && a.narrow) {
     launch_rows_tag<V>(g, a, key, y, st);
   } else if (!W && !R && !V && a.y2 && sizeof(CT) == 4) {
     ++g_launches; spmv_rows32_kernel<false, int, false, false, true><<<grid, kRowsCta, 0, st>>>(a.nrows, a.rows, g.row_ptr, g.col_idx, g.weights, a.colour, key, y, kHubThreshold, a.lo, a.hi, a.n_targets, a.err, a.key2, a.y2);
@@ -361,7 +363,7 @@ struct AuxStream {
 // colours are in the workspace's colour array and *k_out is their number.  Synchronises `st` once per round.
 int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, const wl_options* opt, bool ranged, int lo,
                 int hi, int64_t n_targets, int64_t edge_first, void* workspace, size_t workspace_bytes, const Layout& L,
-                cudaStream_t st, CoreResult* res) {
+                cudaStream_t st, CoreResult* res, const ColumnFeed* feed) {
   const int64_t n = g->n, m = g->m;
   int rc = WL_OK;
   const auto t_entry = std::chrono::steady_clock::now();  // (WL_DEBUG trace only)
@@ -427,6 +429,14 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
   if (workspace_bytes >= DL.bytes) bind_deep();
   bool cols_checked = !validate || m == 0;
   bool dropped_checked = false;  // the rows outside the active list have had their columns range-checked
+  // wl_refine_host (ColumnFeed): row_ptr is needed from here on; the columns arrive piece by piece behind it
+  bool feed_pending = feed != nullptr && feed->pieces > 0;
+  if (feed) cudaStreamWaitEvent(st, feed->rows_ready, 0);
+  auto cols_wait_all = [&]() {  // before any launch that may read any column
+    if (!feed_pending) return;
+    cudaStreamWaitEvent(st, feed->ready[feed->pieces - 1], 0);  // the pieces are copied in order on one stream
+    feed_pending = false;
+  };
   if (validate && !uniform_start) {
     // the kernels below walk row_ptr: make sure it is well formed first
     ++g_launches; validate_rows_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, g->row_ptr, g->weights, edge_first, edge_first + m, d_err);
@@ -475,10 +485,11 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
     // S0 and round 1 in one pass over row_ptr (round1_uniform_kernel); the loop below only closes the round
     const u64 w0 = weight_of(round_key(seed, stream_id, 1), 0);
     const u32 mask1 = overlap ? (u32)(prefix_slots - 1) : L.table_mask;
-    ++g_launches; round1_uniform_kernel<<<(unsigned)std::min<int64_t>(blocks_for(n, kRelabelThreads * kR1Sub), 148 * 8), kRelabelThreads, 0, st>>>(n, g->row_ptr, edge_first, edge_first + m, w0, colour, colour16, rep, stamp, table, mask1, slot_of, scal + kScalNew, kHubThreshold, hub_chunks, L.hub_cap, scal + kScalHub, act[0], scal + kScalActive, scal + kScalActiveHub, d_err, ymask, tag_possible ? tag64 : nullptr,
+    ++g_launches; round1_uniform_kernel<<<(unsigned)std::min<int64_t>(blocks_for(n, kRelabelThreads * kR1Sub), 148 * 32), kRelabelThreads, 0, st>>>(n, g->row_ptr, edge_first, edge_first + m, w0, colour, colour16, rep, stamp, table, mask1, slot_of, scal + kScalNew, kHubThreshold, hub_chunks, L.hub_cap, scal + kScalHub, act[0], scal + kScalActive, scal + kScalActiveHub, d_err, ymask, tag_possible ? tag64 : nullptr,
                                                                                                   std::max<int64_t>(64, 8 * (m / std::max<int64_t>(n, 1))), idmask);
   } else {
     if (!cols_checked) {
+      cols_wait_all();
       ++g_launches; validate_cols_kernel<<<148 * 8, 256, 0, st>>>(n_targets, edge_first, edge_first + m, g->col_idx, d_err);
       cols_checked = true;
     }
@@ -567,7 +578,34 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
         cols_checked = true;
       }
       cudaEventRecord(ek0, st);
-      launch_spmv(L, *g, a, key, tile_row, y, merge, st);
+      if (feed_pending && !merge && !eb && !ranged && !a.tag32) {
+        // the first pass over the columns of a wl_refine_host call: the row kernel takes the rows piece by piece as their
+        // columns land (every row of a piece, empty rows cost one lane-step: no list), the hub chunks follow the last piece
+        int64_t node0 = 0;
+        for (int j = 0; j < feed->pieces; ++j) {
+          cudaStreamWaitEvent(st, feed->ready[j], 0);
+          const int64_t node1 = feed->node_end[j];
+          if (node1 > node0) {
+            SpmvArgs aj = a;
+            aj.rows = nullptr;
+            aj.nrows = node1 - node0;
+            aj.num_hub_chunks = 0;
+            if (aj.y2) aj.y2 += node0;
+            wl_csr gj = *g;
+            gj.row_ptr += node0;
+            launch_spmv(L, gj, aj, key, tile_row, y + node0, merge, st);
+          }
+          node0 = node1;
+        }
+        feed_pending = false;
+        if (a.num_hub_chunks > 0) {
+          a.hubs_only = true;
+          launch_spmv(L, *g, a, key, tile_row, y, merge, st);
+        }
+      } else {
+        cols_wait_all();
+        launch_spmv(L, *g, a, key, tile_row, y, merge, st);
+      }
       cudaEventRecord(ek1, st);
       const int64_t e_r = all_rows ? m : active_edges, n_r = all_rows ? n : n_active;
       edges_streamed += e_r;
@@ -596,6 +634,7 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
     cudaMemsetAsync(scal + kScalActiveHub, 0, sizeof(u64), st);
     // while the column range check is pending the rows dropped here are checked here (a row kernel never reads them)
     const bool check = !cols_checked && !merge && !ranged;
+    if (check || final_test) cols_wait_all();
     ++g_launches; compact_active_kernel<<<blocks_for(n_active, 256), 256, 0, st>>>(n_active, cur_list, colour, stamp, rep, (int)r, g->row_ptr, kHubThreshold, act[cur], scal + kScalActive, scal + kScalActiveHub, check ? g->col_idx : nullptr, n_targets, d_err, final_test ? g->col_idx : nullptr, (int)k_prev, y2);
     if (check) dropped_checked = true;
   };
@@ -765,6 +804,7 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
     dirty_count = 0;
     aux.need(st, table_slots, prefix_slots);
     cudaMemsetAsync(size, 0, sizeof(int) * (size_t)n, st);
+    cols_wait_all();
     if (!tp_built) {
       // in-neighbour lists: in-degrees -> offsets -> fill (the in-degree array counts down to zero and becomes `mark`)
       cudaMemsetAsync(mark, 0, sizeof(int) * (size_t)n, st);
@@ -834,6 +874,7 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
     deep_start_cur = r;
   }
   }  // while (true)
+  cols_wait_all();  // (a call that never read a column still has to see the uploads finished before its buffers go)
   if (!cols_checked) {  // no round read a column (everything was settled by the degrees): check them now
     ++g_launches; validate_cols_kernel<<<148 * 8, 256, 0, st>>>(n_targets, edge_first, edge_first + m, g->col_idx, d_err);
     cudaMemcpyAsync(hs + kScalErr, scal + kScalErr, sizeof(u64), cudaMemcpyDeviceToHost, st);
@@ -863,8 +904,10 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
 
 extern "C" {
 
-int wl_refine(const wl_csr* g, const int32_t* init_colors, uint64_t seed, int32_t* out_colors, wl_stats* stats,
-              const wl_options* opt, void* workspace, size_t workspace_bytes, void* cuda_stream) {
+// wl_refine with an optional column feed (wl_refine_host uploads the columns while the first rounds run)
+static int refine_device(const wl_csr* g, const int32_t* init_colors, uint64_t seed, int32_t* out_colors, wl_stats* stats,
+                         const wl_options* opt, void* workspace, size_t workspace_bytes, void* cuda_stream,
+                         const wl::ColumnFeed* feed) {
   int rc = basic_csr_check(g);
   if (rc) return rc;
   const int64_t n = g->n, m = g->m;
@@ -881,7 +924,7 @@ int wl_refine(const wl_csr* g, const int32_t* init_colors, uint64_t seed, int32_
   cudaEvent_t ev_begin = evp.get(0), ev_end = evp.get(1);
   cudaEventRecord(ev_begin, st);
   CoreResult cr{};
-  const int core_rc = refine_core(g, init_colors, seed, opt, /*ranged=*/false, 0, 0, n, /*edge_first=*/0, workspace, workspace_bytes, L, st, &cr);
+  const int core_rc = refine_core(g, init_colors, seed, opt, /*ranged=*/false, 0, 0, n, /*edge_first=*/0, workspace, workspace_bytes, L, st, &cr, feed);
   if (core_rc != WL_OK && core_rc != WL_EMAXROUNDS) return core_rc;
   char* ws = (char*)workspace;
   cudaEvent_t ev_s6 = evp.get(2);
@@ -926,6 +969,37 @@ int wl_refine(const wl_csr* g, const int32_t* init_colors, uint64_t seed, int32_
   return core_rc;
 }
 
+int wl_refine(const wl_csr* g, const int32_t* init_colors, uint64_t seed, int32_t* out_colors, wl_stats* stats,
+              const wl_options* opt, void* workspace, size_t workspace_bytes, void* cuda_stream) {
+  return refine_device(g, init_colors, seed, out_colors, stats, opt, workspace, workspace_bytes, cuda_stream, nullptr);
+}
+
+// device arena of one wl_refine_host call
+struct HostArena {
+  size_t o_rp, o_col, o_wt, o_init, o_out, o_ws, bytes;
+};
+static HostArena host_arena(int64_t n, int64_t m, bool weighted, bool with_init) {
+  HostArena A{};
+  size_t off = 0;
+  auto take = [&](size_t b) {
+    size_t o = off;
+    off = align_up(off + b);
+    return o;
+  };
+  A.o_rp = take(sizeof(int64_t) * (size_t)(n + 1));
+  A.o_col = take(sizeof(int) * (size_t)m);
+  A.o_wt = take(weighted ? sizeof(u32) * (size_t)m : 0);
+  A.o_init = take(with_init ? sizeof(int) * (size_t)n : 0);
+  A.o_out = take(sizeof(int) * (size_t)n);
+  A.o_ws = take(wl_refine_workspace_bytes(n, m));
+  A.bytes = off;
+  return A;
+}
+size_t wl_refine_host_device_bytes(int64_t n, int64_t m, int weighted, int with_init) {
+  if (n < 0 || m < 0) return 0;
+  return host_arena(n, m, weighted != 0, with_init != 0).bytes;
+}
+
 int wl_refine_host(const wl_csr* g, const int32_t* init_colors, uint64_t seed, int32_t* out_colors, wl_stats* stats,
                    const wl_options* opt, void* cuda_stream) {
   int rc = basic_csr_check(g);
@@ -937,47 +1011,84 @@ int wl_refine_host(const wl_csr* g, const int32_t* init_colors, uint64_t seed, i
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const size_t wsb = wl_refine_workspace_bytes(n, m);  // the deep-round part is allocated by the engine if the loop gets there
   char* d_all = nullptr;
-  size_t o_rp = 0, o_col, o_wt, o_init, o_out, o_ws, off = 0;
-  auto take = [&](size_t b) {
-    size_t o = off;
-    off = align_up(off + b);
-    return o;
-  };
-  o_rp = take(sizeof(int64_t) * (size_t)(n + 1));
-  o_col = take(sizeof(int) * (size_t)m);
-  o_wt = take(g->weights ? sizeof(u32) * (size_t)m : 0);
-  o_init = take(init_colors ? sizeof(int) * (size_t)n : 0);
-  o_out = take(sizeof(int) * (size_t)n);
-  o_ws = take(wsb);
-  if (cudaMalloc((void**)&d_all, off) != cudaSuccess) {
+  const HostArena A = host_arena(n, m, g->weights != nullptr, init_colors != nullptr);
+  const size_t o_rp = A.o_rp, o_col = A.o_col, o_wt = A.o_wt, o_init = A.o_init, o_out = A.o_out, o_ws = A.o_ws, off = A.bytes;
+  const auto t_host0 = std::chrono::steady_clock::now();  // (WL_DEBUG trace only)
+  auto host_ms = [&]() { return std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t_host0).count(); };
+  const bool own_arena = !(opt && opt->device_workspace);
+  if (!own_arena) {
+    if (opt->device_workspace_bytes < off) return WL_ENOMEM;
+    if ((uintptr_t)opt->device_workspace % 256) return WL_EINVAL;
+    d_all = (char*)opt->device_workspace;
+  } else if (cudaMalloc((void**)&d_all, off) != cudaSuccess) {
     cudaGetLastError();
     return WL_ENOMEM;
   }
-  cudaEvent_t e0, e1;
+  const double t_malloc = host_ms();
+  // Uploads run on a stream of their own, in the order the rounds need them: row offsets (+ the initial partition), then the
+  // columns (+ weights) in pieces of whole rows.  The compute stream waits piece by piece (ColumnFeed), so S0, round 1 and the
+  // first pass over the columns overlap the link; what is left after the last piece lands is the tail of that pass.
+  constexpr int kMaxPieces = 32;
+  cudaStream_t copy_st = nullptr;
+  if (cudaStreamCreateWithFlags(&copy_st, cudaStreamNonBlocking) != cudaSuccess) {
+    if (own_arena) cudaFree(d_all);
+    return check_cuda(cudaGetLastError());
+  }
+  cudaEvent_t e0, e1, rows_ready, ready[kMaxPieces];
   cudaEventCreate(&e0);
   cudaEventCreate(&e1);
+  cudaEventCreateWithFlags(&rows_ready, cudaEventDisableTiming);
+  const int pieces = (opt && opt->host_pieces > 0) ? std::min<int>(opt->host_pieces, kMaxPieces)
+                                                   : (int)std::max<int64_t>(1, std::min<int64_t>(kMaxPieces, m / (64ll << 20)));
+  for (int j = 0; j < pieces; ++j) cudaEventCreateWithFlags(&ready[j], cudaEventDisableTiming);
   cudaEventRecord(e0, st);
+  cudaStreamWaitEvent(copy_st, e0, 0);  // whatever the caller queued before this call may still own nothing here, but keep order
   int64_t h2d = 0;
-  cudaMemcpyAsync(d_all + o_rp, g->row_ptr, sizeof(int64_t) * (size_t)(n + 1), cudaMemcpyHostToDevice, st);
+  cudaMemcpyAsync(d_all + o_rp, g->row_ptr, sizeof(int64_t) * (size_t)(n + 1), cudaMemcpyHostToDevice, copy_st);
   h2d += sizeof(int64_t) * (n + 1);
-  if (m) cudaMemcpyAsync(d_all + o_col, g->col_idx, sizeof(int) * (size_t)m, cudaMemcpyHostToDevice, st);
-  h2d += sizeof(int) * m;
-  if (g->weights && m) {
-    cudaMemcpyAsync(d_all + o_wt, g->weights, sizeof(u32) * (size_t)m, cudaMemcpyHostToDevice, st);
-    h2d += sizeof(u32) * m;
-  }
   if (init_colors) {
-    cudaMemcpyAsync(d_all + o_init, init_colors, sizeof(int) * (size_t)n, cudaMemcpyHostToDevice, st);
+    cudaMemcpyAsync(d_all + o_init, init_colors, sizeof(int) * (size_t)n, cudaMemcpyHostToDevice, copy_st);
     h2d += sizeof(int) * n;
   }
+  cudaEventRecord(rows_ready, copy_st);
+  int64_t node_end[kMaxPieces];
+  {
+    // piece borders on row boundaries, read from the caller's offsets (still unvalidated: clamped and kept monotone, so the
+    // copies stay inside the arrays whatever the offsets say; S0 on the device rejects a malformed row_ptr before any column
+    // is used)
+    int64_t node0 = 0, e_prev = 0;
+    for (int j = 0; j < pieces; ++j) {
+      int64_t node1 = n;
+      if (j + 1 < pieces) {
+        const int64_t target = (int64_t)((__int128)m * (j + 1) / pieces);
+        node1 = (std::upper_bound(g->row_ptr, g->row_ptr + n + 1, target) - g->row_ptr) - 1;
+        node1 = std::max(node0, std::min(node1, n));
+      }
+      int64_t e_next = j + 1 < pieces ? g->row_ptr[node1] : m;
+      e_next = std::max(e_prev, std::min(e_next, m));
+      if (e_next > e_prev) {
+        cudaMemcpyAsync(d_all + o_col + sizeof(int) * (size_t)e_prev, g->col_idx + e_prev, sizeof(int) * (size_t)(e_next - e_prev),
+                        cudaMemcpyHostToDevice, copy_st);
+        if (g->weights)
+          cudaMemcpyAsync(d_all + o_wt + sizeof(u32) * (size_t)e_prev, g->weights + e_prev, sizeof(u32) * (size_t)(e_next - e_prev),
+                          cudaMemcpyHostToDevice, copy_st);
+      }
+      cudaEventRecord(ready[j], copy_st);
+      node_end[j] = node1;
+      node0 = node1;
+      e_prev = e_next;
+    }
+    h2d += sizeof(int) * m + (g->weights ? sizeof(u32) * m : 0);
+  }
+  const ColumnFeed feed{pieces, node_end, ready, rows_ready};
   wl_csr dg = {n, m, (const int64_t*)(d_all + o_rp), (const int*)(d_all + o_col),
                g->weights ? (const u32*)(d_all + o_wt) : nullptr};
   wl_stats inner;
   wl_options hopt{};
   if (opt) hopt = *opt;
   hopt.flags |= kFlagLazyDeep;
-  rc = wl_refine(&dg, init_colors ? (const int*)(d_all + o_init) : nullptr, seed, (int*)(d_all + o_out), &inner, &hopt,
-                 d_all + o_ws, wsb, cuda_stream);
+  rc = refine_device(&dg, init_colors ? (const int*)(d_all + o_init) : nullptr, seed, (int*)(d_all + o_out), &inner, &hopt,
+                     d_all + o_ws, wsb, cuda_stream, &feed);
   if (rc == WL_OK || rc == WL_EMAXROUNDS) {
     cudaMemcpyAsync(out_colors, d_all + o_out, sizeof(int) * (size_t)n, cudaMemcpyDeviceToHost, st);
     cudaEventRecord(e1, st);
@@ -992,9 +1103,18 @@ int wl_refine_host(const wl_csr* g, const int32_t* init_colors, uint64_t seed, i
       stats->bytes_d2h = sizeof(int) * n;
     }
   }
+  cudaStreamSynchronize(copy_st);  // (an early error return leaves uploads in flight: they must be over before the buffers go)
+  cudaStreamSynchronize(st);
+  const double t_done = host_ms();
   cudaEventDestroy(e0);
   cudaEventDestroy(e1);
-  cudaFree(d_all);
+  cudaEventDestroy(rows_ready);
+  for (int j = 0; j < pieces; ++j) cudaEventDestroy(ready[j]);
+  cudaStreamDestroy(copy_st);
+  if (own_arena) cudaFree(d_all);
+  if (debug_enabled())
+    std::fprintf(stderr, "[wl_refine_host] host clock: cudaMalloc %.3f ms, uploads + rounds + download %.3f ms, cudaFree %.3f ms (%d pieces)\n",
+                 t_malloc, t_done - t_malloc, host_ms() - t_done, pieces);
   return rc;
 }
 

@@ -296,6 +296,65 @@ def test_refine_host_entry_point():
     assert res.stats["bytes_h2d"] == 8 * (n + 1) + 4 * g.m and res.stats["bytes_d2h"] == 4 * n
 
 
+@pytest.mark.parametrize("name", list(GRAPHS))
+@pytest.mark.parametrize("pieces", [0, 2, 5, 32])
+def test_refine_host_column_pieces_equal_oracle(name, pieces):
+    """wl_refine_host uploads the columns in pieces of whole rows and runs the first pass over them piece by piece behind the
+    copies (ColumnFeed): same colouring and trajectory as the oracle for any number of pieces, for weighted graphs, empty graphs,
+    hub rows, with and without an initial partition, from pinned and from pageable host memory."""
+    g = GRAPHS[name]()
+    n, rp, ci, wt = g.numpy()
+    want, counts, _ = oracle.refine(n, rp, ci, wt)
+    w = None if g.weights is None else g.weights
+    pin = (lambda t: t.pin_memory()) if pieces != 5 else (lambda t: t)  # pieces == 5: pageable memory
+    res = wl.wl_refine_host(n, pin(g.row_ptr), pin(g.col), None if w is None else pin(w), seed=13, pieces=pieces)
+    assert res.colors.numpy().tolist() == want.tolist() and res.round_colors == counts
+    if n >= 4:
+        init = gg.random_partition(n, 3, 2)
+        want2, counts2, _ = oracle.refine(n, rp, ci, wt, init.numpy())
+        res = wl.wl_refine_host(n, pin(g.row_ptr), pin(g.col), None if w is None else pin(w), pin(init), seed=14, pieces=pieces)
+        assert res.colors.numpy().tolist() == want2.tolist() and res.round_colors == counts2
+
+
+def test_refine_host_with_caller_device_workspace():
+    """wl_options.device_workspace: the call uploads into and works in the caller's device arena (no cudaMalloc / cudaFree inside
+    the call); too small an arena is WL_ENOMEM; same colouring, also when the arena is reused by the next call."""
+    g = GRAPHS["rmat12_sym"]()
+    n, rp, ci, wt = g.numpy()
+    want, counts, _ = oracle.refine(n, rp, ci, wt)
+    need = wl.wl_refine_host_device_bytes(n, g.m)
+    assert need >= wl.wl_refine_workspace_bytes(n, g.m) + 8 * (n + 1) + 4 * g.m + 4 * n
+    arena = torch.full((need,), 0xAB, dtype=torch.uint8, device=dev())
+    for seed in (1, 2):
+        res = wl.wl_refine_host(n, g.row_ptr.pin_memory(), g.col.pin_memory(), seed=seed, device_workspace=arena, pieces=3)
+        assert res.colors.numpy().tolist() == want.tolist() and res.round_colors == counts
+    with pytest.raises(wl.WlError) as e:
+        wl.wl_refine_host(n, g.row_ptr.pin_memory(), g.col.pin_memory(), seed=1, device_workspace=arena[: need - 256])
+    assert e.value.code == wl.WL_ENOMEM
+    gw = GRAPHS["weighted"]()
+    assert wl.wl_refine_host_device_bytes(gw.n, gw.m, True, True) > wl.wl_refine_host_device_bytes(gw.n, gw.m)
+
+
+@pytest.mark.parametrize("pieces", [1, 4])
+def test_refine_host_rejects_malformed_input_in_any_piece(pieces):
+    """S0 through the host entry point: a bad target in the first / last piece, decreasing offsets and a wrong last offset come
+    back as WL_EINVAL (the piece borders are read from the unvalidated offsets: the copies must stay inside the arrays)."""
+    g = gg.rmat(10, seed=4)
+    n, m = g.n, g.m
+    for pos, val in ((3, n), (m - 2, -1), (m // 2, n + 7)):
+        bad = g.col.clone()
+        bad[pos] = val
+        with pytest.raises(wl.WlError) as e:
+            wl.wl_refine_host(n, g.row_ptr.pin_memory(), bad.pin_memory(), seed=1, pieces=pieces)
+        assert e.value.code == wl.WL_EINVAL
+    for i, v in ((n // 2, 10 * m), (n // 3, -5), (n, m - 1)):
+        rp2 = g.row_ptr.clone()
+        rp2[i] = v
+        with pytest.raises(wl.WlError) as e:
+            wl.wl_refine_host(n, rp2.pin_memory(), g.col.pin_memory(), seed=1, pieces=pieces)
+        assert e.value.code == wl.WL_EINVAL
+
+
 # ------------------------------------------------------------------ error behaviour
 def test_refine_host_entry_point_deep_rounds():
     """wl_refine_host on a graph that needs 128 rounds: the engine allocates the worklist regime's workspace itself once the
