@@ -91,3 +91,71 @@ def split_pairs(prev, cur):
     pairs = np.unique(np.stack([prev, cur], 1), axis=0)
     s = np.bincount(pairs[:, 0])
     return int((s * (s - 1) // 2).sum())
+
+
+def sampled_block_stability(row_ptr, col, colors, k, dev, n_blocks=300, max_block=64, max_row=20000, seed=0, min_row=0):
+    """Def. 1 on sampled non-singleton blocks of a colouring too large for a full check: the rows of every
+    member of the sampled blocks are cut out (row_ptr / col may live on the host or on `dev`), their targets are replaced by
+    the targets' colours, and oracle.is_stable runs on that auxiliary graph (sampled nodes keep their block, the target
+    colours are discrete).  Also checks, on ALL nodes, that the members of a block have equal out-degree (necessary for
+    stability).  min_row: only blocks whose members have at least that many entries (most non-singleton blocks of an R-MAT
+    graph are twins with a single out-edge; a second sample with min_row > 1 looks at the others).  Returns (blocks checked, nodes checked, entries checked, verdict, verdict of a planted violation or None)."""
+    import torch
+    import graphgen as gg
+    import oracle
+    n = colors.numel()
+    c = colors.to(dev)
+    c64 = c.to(torch.int64)
+    sizes = torch.bincount(c64, minlength=k)
+    rpd = row_ptr.to(dev)
+    deg = rpd[1:] - rpd[:-1]
+    del rpd
+    dmax = torch.zeros(k, dtype=torch.int64, device=dev).scatter_reduce_(0, c64, deg, "amax", include_self=False)
+    dmin = torch.zeros(k, dtype=torch.int64, device=dev).scatter_reduce_(0, c64, deg, "amin", include_self=False)
+    degrees_equal = bool((dmax == dmin).all())
+    multi = torch.nonzero((sizes >= 2) & (sizes <= max_block) & (dmax <= max_row) & (dmax >= min_row)).flatten()
+    del dmin, sizes
+    gen = torch.Generator(device=dev).manual_seed(seed)
+    pick = multi[torch.randperm(multi.numel(), device=dev, generator=gen)[:n_blocks]]
+    lut = torch.zeros(k, dtype=torch.bool, device=dev)
+    lut[pick] = True
+    nodes = torch.nonzero(lut[c64]).flatten()
+    del lut, c64, dmax
+    nn = nodes.numel()
+    if nn == 0:  # no block of the asked shape exists
+        return {"blocks": 0, "nodes": 0, "entries": 0, "stable": True, "degrees_equal_on_all_nodes": degrees_equal,
+                "planted_violation_passes": None, "candidate_blocks": 0}
+    n_candidates = int(multi.numel())
+    nodes_rp = nodes.to(row_ptr.device)
+    a, b = row_ptr[nodes_rp], row_ptr[nodes_rp + 1]
+    lens = (b - a)
+    total = int(lens.sum())
+    starts = torch.repeat_interleave(a, lens)
+    offs = torch.arange(total, device=a.device) - torch.repeat_interleave(torch.cumsum(lens, 0) - lens, lens)
+    targets = col[(starts + offs).to(col.device)].to(dev).to(torch.int64)
+    tgt_col = c[targets].to(torch.int64)
+    sub_rp = torch.zeros(nn + 1, dtype=torch.int64)
+    sub_rp[1:] = torch.cumsum(lens.cpu(), 0)
+    # nodes of the auxiliary graph: the sampled nodes, then one node per distinct target colour (compressed: the colour ids of
+    # a billion-node graph plus the sample would not fit int32 node ids)
+    uniq, inv = torch.unique(tgt_col.cpu(), return_inverse=True)
+    kk2 = uniq.numel()
+    sub_n = nn + kk2
+    rp_full = torch.cat([sub_rp, torch.full((kk2,), int(sub_rp[-1]), dtype=torch.int64)])
+    col_small = (inv + nn).to(torch.int32)
+    colours = torch.cat([c[nodes].cpu().to(torch.int64) + (nn + kk2), torch.arange(kk2) + nn]).to(torch.int64)
+    colours = gg.canonical_first_occurrence(colours)
+    ok = bool(oracle.is_stable(sub_n, rp_full.numpy(), col_small.numpy(), None, colours.numpy()))
+    # the checker must notice a node moved into a block whose members see other colours: take the first sampled node of
+    # another block whose row (as a sorted list of target colours) differs from node 0's
+    planted = None
+    rows_np, col_np = sub_rp.numpy(), col_small.numpy()
+    sig0 = sorted(col_np[rows_np[0]:rows_np[1]].tolist())
+    for t in torch.nonzero(colours[:nn] != colours[0]).flatten()[:2000].tolist():
+        if sorted(col_np[rows_np[t]:rows_np[t + 1]].tolist()) != sig0:
+            bad = colours.clone()
+            bad[0] = colours[t]
+            planted = bool(oracle.is_stable(sub_n, rp_full.numpy(), col_small.numpy(), None, bad.numpy()))
+            break
+    return {"blocks": int(pick.numel()), "nodes": nn, "entries": total, "stable": ok, "degrees_equal_on_all_nodes": degrees_equal,
+            "planted_violation_passes": planted, "candidate_blocks": n_candidates}
