@@ -805,7 +805,7 @@ relabel_kernel(int64_t count, const int* __restrict__ nodes, int* __restrict__ c
     slot_of[id] = slot;
   } else if (lose) {
     while (id == kPending) id = ld_slot_id(table + slot);
-    if (stamp[id] != round) stamp[id] = round;
+    if (stamp[id] != round) stamp[id] = round;  // (a blind store measured no faster: 4.03 against 3.99 ms on the headline round)
   }
   if (win || lose) {
     colour[i] = (int)id;
@@ -832,8 +832,9 @@ relabel_kernel(int64_t count, const int* __restrict__ nodes, int* __restrict__ c
 // The list is a superset of what compact_active_kernel would keep (it keeps the few nodes whose degree is unique);
 // counters[0] = listed rows, counters[1] = their out-degree sum (= m), *hub_rows = listed rows longer than hub_threshold.
 // Degree classes repeat: 63 M listed rows of the headline graph share 3 855 keys, so every CTA keeps the ids it has already
-// seen in shared memory (s_id[d] = id of the class of out-degree d, bit 30 = "stamp[id] is known to be set") and walks its
-// tiles grid-stride; only the first sight of a degree in a CTA goes to the global table (1.29 ms -> see profiles/).
+// seen in shared memory (s_id[d] = id of the class of out-degree d, bit 30 = "stamp[id] is known to be set"); only the first
+// sight of a degree in a CTA goes to the global table.  One CTA per super-tile of kR1Sub * 256 nodes (the loop is grid-stride, but
+// a grid of all super-tiles keeps the active list closest to node order, which the row kernel of round 2 likes best).
 constexpr int kR1Cache = 4096;       // out-degrees below this are cached per CTA (16 KB)
 constexpr int kR1Sub = 8;            // sub-tiles of kRelabelThreads nodes per list reservation
 constexpr int kR1Stamped = 1 << 30;  // round-1 ids stay far below 2^30 (at most sqrt(2m) + 1 distinct degrees)

@@ -47,7 +47,6 @@ Layout make_layout(int64_t n, int64_t m) {
   L.o_tmp = take(sizeof(u32) * (size_t)n);
   L.o_y = take(sizeof(u64) * (size_t)n);
   L.o_tile_row = take(sizeof(int) * (size_t)(L.ntiles + 1));
-  L.o_bsum = take(sizeof(int) * canon_scratch_ints(n));
   L.o_table = take(sizeof(Slot) * ((size_t)L.table_mask + 1));
   L.o_colour16 = take(sizeof(unsigned short) * (size_t)n);
   L.o_act0 = take(sizeof(int) * (size_t)n);
@@ -58,6 +57,7 @@ Layout make_layout(int64_t n, int64_t m) {
   L.o_tag64 = take(sizeof(u64) * kTagSlots);
   L.o_tag32 = take(sizeof(u32) * kTagSlots);
   L.o_y2 = take(sizeof(u64) * (size_t)n);
+  L.o_bsum = take(sizeof(int) * canon_scratch_ints(n));  // (last: the arrays the gathers read keep their place)
   L.bytes = off;
   return L;
 }
@@ -485,7 +485,7 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
     // S0 and round 1 in one pass over row_ptr (round1_uniform_kernel); the loop below only closes the round
     const u64 w0 = weight_of(round_key(seed, stream_id, 1), 0);
     const u32 mask1 = overlap ? (u32)(prefix_slots - 1) : L.table_mask;
-    ++g_launches; round1_uniform_kernel<<<(unsigned)std::min<int64_t>(blocks_for(n, kRelabelThreads * kR1Sub), 148 * 32), kRelabelThreads, 0, st>>>(n, g->row_ptr, edge_first, edge_first + m, w0, colour, colour16, rep, stamp, table, mask1, slot_of, scal + kScalNew, kHubThreshold, hub_chunks, L.hub_cap, scal + kScalHub, act[0], scal + kScalActive, scal + kScalActiveHub, d_err, ymask, tag_possible ? tag64 : nullptr,
+    ++g_launches; round1_uniform_kernel<<<blocks_for(n, kRelabelThreads * kR1Sub), kRelabelThreads, 0, st>>>(n, g->row_ptr, edge_first, edge_first + m, w0, colour, colour16, rep, stamp, table, mask1, slot_of, scal + kScalNew, kHubThreshold, hub_chunks, L.hub_cap, scal + kScalHub, act[0], scal + kScalActive, scal + kScalActiveHub, d_err, ymask, tag_possible ? tag64 : nullptr,
                                                                                                   std::max<int64_t>(64, 8 * (m / std::max<int64_t>(n, 1))), idmask);
   } else {
     if (!cols_checked) {
