@@ -69,3 +69,33 @@ def test_deep_and_batched_workspace_sizes():
     # pinned scratch of the batched path: two offset arrays + one weighted entry array
     hb = wl.wl_refine_batched_host_bytes(1000, 5000)
     assert hb >= 2 * 8 * 1001 + 8 * 5000 and wl.wl_refine_batched_host_bytes(-1, 0) == 0
+
+
+def test_ctypes_structs_mirror_the_header_layout(repo_root, tmp_path):
+    """The binding's ctypes structures must have the size and the field offsets gcc gives the structs of include/wl_refine.h
+    (a field added on one side only would shift every later field silently)."""
+    import ctypes
+    import shutil
+    import subprocess
+    from paper_2607_02603_b200 import binding as B
+    if shutil.which("gcc") is None:
+        pytest.skip("no gcc")
+    structs = {"wl_csr": B.wl_csr, "wl_options": B.wl_options, "wl_stats": B.wl_stats, "wl_edge_batch": B.wl_edge_batch}
+    lines = ["#include <stdio.h>", "#include <stddef.h>", '#include "wl_refine.h"', "int main(void) {"]
+    for name, cls in structs.items():
+        lines.append(f'  printf("{name} %zu\\n", sizeof({name}));')
+        for field, _ in cls._fields_:
+            lines.append(f'  printf("{name}.{field} %zu\\n", offsetof({name}, {field}));')
+    lines += ["  return 0;", "}"]
+    src = tmp_path / "layout.c"
+    src.write_text("\n".join(lines))
+    exe = tmp_path / "layout"
+    subprocess.run(["gcc", "-I", os.path.join(repo_root, "include"), "-o", str(exe), str(src)], check=True)
+    got = dict(line.split() for line in subprocess.run([str(exe)], check=True, capture_output=True, text=True).stdout.splitlines())
+    header = re.sub(r"/\*.*?\*/", "", open(os.path.join(repo_root, "include", "wl_refine.h")).read(), flags=re.S)
+    for name, cls in structs.items():
+        assert int(got[name]) == ctypes.sizeof(cls), name
+        for field, _ in cls._fields_:
+            assert int(got[f"{name}.{field}"]) == getattr(cls, field).offset, f"{name}.{field}"
+        body = re.search(r"typedef struct %s \{(.*?)\} %s;" % (name, name), header, flags=re.S).group(1)
+        assert len([d for d in body.split(";") if d.strip()]) == len(cls._fields_), f"{name}: field count differs from the header"
