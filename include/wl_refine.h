@@ -66,6 +66,9 @@ typedef struct wl_csr {
                                       headline graph, kept for extreme degree skew)                          */
 #define WL_FLAG_NO_DEEP 256u     /* never switch to the worklist regime (below): every round recomputes every active row */
 #define WL_FLAG_DEEP_EARLY 512u  /* switch to the worklist regime at round 2 instead of round 7 (testing)                 */
+#define WL_FLAG_DEEP_CLUSTER 32768u /* worklist regime: every window of queued rounds as ONE launch by one thread-block cluster
+                                       (cluster barriers between the phases instead of kernel boundaries).  Same results; measured
+                                       slower than the default two kernels per round on B200, kept for testing                */
 #define WL_FLAG_NO_FINAL 1024u   /* do not drop blocks whose whole neighbourhood is final from the active set (R5)        */
 #define WL_FLAG_INHERIT_BATCHES 4096u /* batched: from the second outer iteration on, a quotient keeps the batches of its
                                         graph (the rows emitted together) instead of being re-cut by M_b, and its local

@@ -156,6 +156,7 @@ deep_finish_part(unsigned cta, unsigned part, const int* __restrict__ leavers, c
       scal[kScalK] = k_old + n_new;
       scal[kScalTicket] = 0;
       if (log) log[log_slot] = k_old + n_new;
+      if (nl > scal[kScalFrontier]) scal[kScalFrontier] = nl;  // largest |L| since the host last looked (it picks the launch shape)
       deep[leavers_slot] = 0;
       deep[kDeepSlots] = 0;
       deep[kDeepNew] = 0;
@@ -178,26 +179,19 @@ struct DeepFinishArgs {  // the round being closed (fin_ctas == 0: nothing to cl
 // kDeepSmall entries are walked by eight lanes each (step by step, so that the appends of a step share one atomic), longer
 // ones by the whole warp.  do_front == 0: only the closing part runs (end of a window).
 constexpr int kDeepSmall = 64;
+// the front of one round by the CTAs cta = 0 .. nctas - 1 of whatever launch runs it (a grid of its own, or a cluster)
 template <bool WEIGHTED>
-__global__ void __launch_bounds__(256)
-deep_front_kernel(DeepFinishArgs fin, int do_front, const int* __restrict__ changed, const u64* __restrict__ n_changed,
-                  const int64_t* __restrict__ tp_ptr, const int* __restrict__ tp_src, int* __restrict__ mark, int round,
-                  const int64_t* __restrict__ row_ptr, const int* __restrict__ col, const u32* __restrict__ wt,
-                  int* __restrict__ colour, u64 key, u64* __restrict__ y, int* __restrict__ size, int* __restrict__ lcount,
-                  int* __restrict__ leavers, int* __restrict__ leaver_block, u64* __restrict__ n_leavers,
-                  Slot* __restrict__ table, const u32* __restrict__ slots, u64* __restrict__ deep, u64* __restrict__ scal,
-                  u64 ymask) {
-  if (blockIdx.x < fin.fin_ctas) {
-    deep_finish_part(blockIdx.x, fin.fin_ctas, fin.leavers, fin.leaver_block, colour, size, fin.lcount, table, slots, deep,
-                     fin.leavers_slot, fin.consumed_slot, scal, fin.log, fin.log_slot);
-    return;
-  }
-  if (!do_front) return;
+__device__ __forceinline__ void
+deep_front_part(unsigned cta, unsigned nctas, const int* __restrict__ changed, const u64* __restrict__ n_changed,
+                const int64_t* __restrict__ tp_ptr, const int* __restrict__ tp_src, int* __restrict__ mark, int round,
+                const int64_t* __restrict__ row_ptr, const int* __restrict__ col, const u32* __restrict__ wt,
+                int* __restrict__ colour, u64 key, u64* __restrict__ y, int* __restrict__ lcount,
+                int* __restrict__ leavers, int* __restrict__ leaver_block, u64* __restrict__ n_leavers, u64 ymask) {
   const int lane = threadIdx.x & 31, sub = lane & 7, grp = lane >> 3;
   const int64_t nc = (int64_t)*n_changed;
   // a warp takes four changed nodes per trip, eight lanes each
-  const int64_t nwarps = ((int64_t)(gridDim.x - fin.fin_ctas) * blockDim.x) >> 5;
-  const int64_t warp = ((int64_t)(blockIdx.x - fin.fin_ctas) * blockDim.x + threadIdx.x) >> 5;
+  const int64_t nwarps = ((int64_t)nctas * blockDim.x) >> 5;
+  const int64_t warp = ((int64_t)cta * blockDim.x + threadIdx.x) >> 5;
   for (int64_t base = warp * 4; base < nc; base += nwarps * 4) {
     const int64_t t = base + grp;
     int64_t a = 0, b = 0;
@@ -238,20 +232,40 @@ deep_front_kernel(DeepFinishArgs fin, int do_front, const int* __restrict__ chan
   }
 }
 
+template <bool WEIGHTED>
+__global__ void __launch_bounds__(256)
+deep_front_kernel(DeepFinishArgs fin, int do_front, const int* __restrict__ changed, const u64* __restrict__ n_changed,
+                  const int64_t* __restrict__ tp_ptr, const int* __restrict__ tp_src, int* __restrict__ mark, int round,
+                  const int64_t* __restrict__ row_ptr, const int* __restrict__ col, const u32* __restrict__ wt,
+                  int* __restrict__ colour, u64 key, u64* __restrict__ y, int* __restrict__ size, int* __restrict__ lcount,
+                  int* __restrict__ leavers, int* __restrict__ leaver_block, u64* __restrict__ n_leavers,
+                  Slot* __restrict__ table, const u32* __restrict__ slots, u64* __restrict__ deep, u64* __restrict__ scal,
+                  u64 ymask) {
+  if (blockIdx.x < fin.fin_ctas) {
+    deep_finish_part(blockIdx.x, fin.fin_ctas, fin.leavers, fin.leaver_block, colour, size, fin.lcount, table, slots, deep,
+                     fin.leavers_slot, fin.consumed_slot, scal, fin.log, fin.log_slot);
+    return;
+  }
+  if (!do_front) return;
+  deep_front_part<WEIGHTED>(blockIdx.x - fin.fin_ctas, gridDim.x - fin.fin_ctas, changed, n_changed, tp_ptr, tp_src, mark, round,
+                            row_ptr, col, wt, colour, key, y, lcount, leavers, leaver_block, n_leavers, ymask);
+}
+
 // L -> new blocks.  Thread per leaver: the exact key (old colour, new y) claims or finds a slot of the relabel table; the
 // claimer takes the old id if the whole block is leaving and nobody took it yet this round, otherwise a fresh id.
 // Program order inside a warp is claim -> publish -> poll, so a polling lane never waits on a lane of its own warp, and a
 // claimer publishes without waiting on anybody: the polls terminate.
-__global__ void __launch_bounds__(256)
-deep_relabel_kernel(const int* __restrict__ leavers, const int* __restrict__ leaver_block, const u64* __restrict__ n_leavers,
-                    int* __restrict__ colour, const u64* __restrict__ y, const int* __restrict__ size,
-                    const int* __restrict__ lcount, int* __restrict__ inherit, int round, Slot* __restrict__ table,
-                    u32 table_mask, u32* __restrict__ slots, u64* __restrict__ n_slots, const u64* __restrict__ k_ptr,
-                    u64* __restrict__ n_new, int* __restrict__ changed_out, u64* __restrict__ n_changed_out, u64 ymask) {
+__device__ __forceinline__ void
+deep_relabel_part(unsigned cta, unsigned nctas, const int* __restrict__ leavers, const int* __restrict__ leaver_block,
+                  const u64* __restrict__ n_leavers, int* __restrict__ colour, const u64* __restrict__ y,
+                  const int* __restrict__ size, const int* __restrict__ lcount, int* __restrict__ inherit, int round,
+                  Slot* __restrict__ table, u32 table_mask, u32* __restrict__ slots, u64* __restrict__ n_slots,
+                  const u64* __restrict__ k_ptr, u64* __restrict__ n_new, int* __restrict__ changed_out,
+                  u64* __restrict__ n_changed_out, u64 ymask) {
   const int64_t nl = (int64_t)*n_leavers;
   const int k_old = (int)*k_ptr;
-  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
-  const int64_t first = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int64_t stride = (int64_t)nctas * blockDim.x;
+  const int64_t first = (int64_t)cta * blockDim.x + threadIdx.x;
   // whole warps iterate together (the last trip is padded) so that __syncwarp() sees every lane
   for (int64_t base = first - (threadIdx.x & 31); base < nl; base += stride) {
     const int64_t t = base + (threadIdx.x & 31);
@@ -307,6 +321,75 @@ deep_relabel_kernel(const int* __restrict__ leavers, const int* __restrict__ lea
       changed_out[cpos] = i;
     }
   }
+}
+
+__global__ void __launch_bounds__(256)
+deep_relabel_kernel(const int* __restrict__ leavers, const int* __restrict__ leaver_block, const u64* __restrict__ n_leavers,
+                    int* __restrict__ colour, const u64* __restrict__ y, const int* __restrict__ size,
+                    const int* __restrict__ lcount, int* __restrict__ inherit, int round, Slot* __restrict__ table,
+                    u32 table_mask, u32* __restrict__ slots, u64* __restrict__ n_slots, const u64* __restrict__ k_ptr,
+                    u64* __restrict__ n_new, int* __restrict__ changed_out, u64* __restrict__ n_changed_out, u64 ymask) {
+  deep_relabel_part(blockIdx.x, gridDim.x, leavers, leaver_block, n_leavers, colour, y, size, lcount, inherit, round, table,
+                    table_mask, slots, n_slots, k_ptr, n_new, changed_out, n_changed_out, ymask);
+}
+
+// ---- a window of rounds in ONE launch by one thread-block cluster ------------------------------------------------------------
+// A round of this regime is two launches of a few microseconds each.  A cluster of kDeepClusterCtas CTAs runs the same three parts
+// (front, relabel, closing) for `rounds` rounds back to back; the phases are separated by the hardware cluster barrier
+// (arrive.release / wait.acquire: a few hundred cycles, and it makes the other CTAs' global writes visible) instead of kernel
+// boundaries.  Same device functions, same data, same results as the two-kernel form.  Measured on B200 and NOT the default
+// (WL_FLAG_DEEP_CLUSTER): what bounds a round is its two dependent chains of about ten L2 accesses, not the launches, and eight
+// SMs are too few for the 26 k leavers per round of the 2048^2 grid (profiles/r2b_deep_cluster.md).
+constexpr int kDeepClusterCtas = 8;      // portable cluster size
+constexpr int kDeepClusterThreads = 1024;
+struct DeepClusterArgs {
+  int* changed[2];
+  int* lcount[2];
+  int* leavers[2];
+  int* leaver_block[2];
+  const int64_t* tp_ptr;
+  const int* tp_src;
+  int* mark;
+  const int64_t* row_ptr;
+  const int* col;
+  const u32* wt;
+  int* colour;
+  u64 key;
+  u64* y;
+  int* size;
+  int* inherit;
+  Slot* table;
+  u32 table_mask;
+  u32* slots;
+  u64* deep;
+  u64* scal;
+  u64 ymask;
+  int round0, rounds;
+};
+__device__ __forceinline__ void cluster_barrier() {
+  asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+template <bool WEIGHTED>
+__global__ void __launch_bounds__(kDeepClusterThreads, 1)
+deep_cluster_kernel(const DeepClusterArgs a) {
+  const unsigned cta = blockIdx.x, nctas = gridDim.x;  // the grid is one cluster
+  for (int j = 0; j < a.rounds; ++j) {
+    const int round = a.round0 + j, in = round & 1, out = in ^ 1;
+    if (j > 0)  // close round - 1 (touches nothing the front of this round reads or writes, see deep_front_kernel)
+      deep_finish_part(cta, nctas, a.leavers[out], a.leaver_block[out], a.colour, a.size, a.lcount[out], a.table, a.slots, a.deep,
+                       kDeepLeavers0 + out, kDeepChanged0 + out, a.scal, a.scal + kScalLog, j - 1);
+    deep_front_part<WEIGHTED>(cta, nctas, a.changed[in], a.deep + kDeepChanged0 + in, a.tp_ptr, a.tp_src, a.mark, round, a.row_ptr,
+                              a.col, a.wt, a.colour, a.key, a.y, a.lcount[in], a.leavers[in], a.leaver_block[in],
+                              a.deep + kDeepLeavers0 + in, a.ymask);
+    cluster_barrier();
+    deep_relabel_part(cta, nctas, a.leavers[in], a.leaver_block[in], a.deep + kDeepLeavers0 + in, a.colour, a.y, a.size,
+                      a.lcount[in], a.inherit, round, a.table, a.table_mask, a.slots, a.deep + kDeepSlots, a.scal + kScalK,
+                      a.deep + kDeepNew, a.changed[out], a.deep + kDeepChanged0 + out, a.ymask);
+    cluster_barrier();
+  }
+  const int last = (a.round0 + a.rounds - 1) & 1;
+  deep_finish_part(cta, nctas, a.leavers[last], a.leaver_block[last], a.colour, a.size, a.lcount[last], a.table, a.slots, a.deep,
+                   kDeepLeavers0 + last, kDeepChanged0 + last, a.scal, a.scal + kScalLog, a.rounds - 1);
 }
 
 }  // namespace wl

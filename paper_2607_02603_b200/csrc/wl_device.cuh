@@ -22,6 +22,7 @@ enum {
   kScalTicket = 8,     // CTAs that finished relabel_finish_kernel
   kScalErrAux = 9,     // validation error bits written on the side stream
   kScalRowTicket = 10, // row-group ticket of spmv_rows32_tag_kernel
+  kScalFrontier = 11,  // worklist regime: largest |L| of a round since the host last reset it
   kScalLog = 16,
   kNumScal = 64
 };

@@ -839,14 +839,54 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
     // above, as a new switch round): if it changes nothing the paper's terminal argument applies as it stands (L408-L414), else
     // the worklist rounds go on under the new key.
     bool fixed_point = false;
+    // Launch shape of a window: two kernels per round over the whole GPU (default), or ONE launch by one thread-block cluster that
+    // runs all rounds of the window with cluster barriers between the phases (deep_cluster_kernel, WL_FLAG_DEEP_CLUSTER: measured
+    // and not the default: a round is two dependent chains of about ten L2 accesses whatever separates them, and eight SMs are too
+    // few for the 26 k leavers per round of the 2048^2 grid: 75 us per round against 21, 17 against 10.5 on its last, small rounds;
+    // profiles/r2b_deep_cluster.md).
+    bool cluster_ok = (flags & WL_FLAG_DEEP_CLUSTER) != 0 && !no_runahead;
+    double us_round[2] = {-1.0, -1.0};  // [0] two kernels per round, [1] cluster (WL_DEBUG trace)
+    int64_t frontier = -1;
     while (r <= max_rounds && !fixed_point) {
       const int R = no_runahead ? 1 : (int)std::min<int64_t>(kRunAhead, max_rounds - r + 1);
-      for (int j = 0; j < R; ++j) {
-        const int round = (int)(r + j), in = round & 1, out = (round + 1) & 1;
-        front(j == 0 ? DeepFinishArgs{0, nullptr, nullptr, nullptr, 0, 0, 0, nullptr} : closing(round - 1, j - 1), 1, round);
-        ++g_launches; deep_relabel_kernel<<<kDeepGrid, 256, 0, st>>>(leavers[in], leaver_block[in], deep + kDeepLeavers0 + in, colour, y, size, lcount[in], inherit, round, table, L.table_mask, slots, deep + kDeepSlots, scal + kScalK, deep + kDeepNew, changed[out], deep + kDeepChanged0 + out, ymask);
+      int shape = cluster_ok ? 1 : 0;
+      cudaMemsetAsync(scal + kScalFrontier, 0, sizeof(u64), st);
+      if (shape == 1) {
+        DeepClusterArgs ca{};
+        for (int b = 0; b < 2; ++b) {
+          ca.changed[b] = changed[b];
+          ca.lcount[b] = lcount[b];
+          ca.leavers[b] = leavers[b];
+          ca.leaver_block[b] = leaver_block[b];
+        }
+        ca.tp_ptr = tp_ptr, ca.tp_src = tp_src, ca.mark = mark, ca.row_ptr = g->row_ptr, ca.col = g->col_idx, ca.wt = g->weights;
+        ca.colour = colour, ca.key = key, ca.y = y, ca.size = size, ca.inherit = inherit, ca.table = table;
+        ca.table_mask = L.table_mask, ca.slots = slots, ca.deep = deep, ca.scal = scal, ca.ymask = ymask;
+        ca.round0 = (int)r, ca.rounds = R;
+        cudaLaunchConfig_t cfg{};
+        cfg.gridDim = dim3(kDeepClusterCtas), cfg.blockDim = dim3(kDeepClusterThreads), cfg.dynamicSmemBytes = 0, cfg.stream = st;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = kDeepClusterCtas, attr[0].val.clusterDim.y = 1, attr[0].val.clusterDim.z = 1;
+        cfg.attrs = attr, cfg.numAttrs = 1;
+        const cudaError_t le = g->weights ? cudaLaunchKernelEx(&cfg, deep_cluster_kernel<true>, ca)
+                                          : cudaLaunchKernelEx(&cfg, deep_cluster_kernel<false>, ca);
+        if (le != cudaSuccess) {  // no room for the cluster on this device: the two-kernel shape always works
+          cudaGetLastError();
+          cluster_ok = false;
+          shape = 0;
+        } else {
+          ++g_launches;
+        }
       }
-      front(closing((int)(r + R - 1), R - 1), 0, (int)(r + R));
+      if (shape == 0) {
+        for (int j = 0; j < R; ++j) {
+          const int round = (int)(r + j), in = round & 1, out = (round + 1) & 1;
+          front(j == 0 ? DeepFinishArgs{0, nullptr, nullptr, nullptr, 0, 0, 0, nullptr} : closing(round - 1, j - 1), 1, round);
+          ++g_launches; deep_relabel_kernel<<<kDeepGrid, 256, 0, st>>>(leavers[in], leaver_block[in], deep + kDeepLeavers0 + in, colour, y, size, lcount[in], inherit, round, table, L.table_mask, slots, deep + kDeepSlots, scal + kScalK, deep + kDeepNew, changed[out], deep + kDeepChanged0 + out, ymask);
+        }
+        front(closing((int)(r + R - 1), R - 1), 0, (int)(r + R));
+      }
       cudaEventRecord(d1, st);
       cudaMemcpyAsync(hs, scal, sizeof(u64) * kNumScal, cudaMemcpyDeviceToHost, st);
       rc = check_cuda(cudaStreamSynchronize(st));
@@ -855,6 +895,11 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
       cudaEventElapsedTime(&t_win, d0, d1);
       ms_relabel += t_win;
       cudaEventRecord(d0, st);
+      frontier = (int64_t)hs[kScalFrontier];
+      us_round[shape] = 1e3 * (double)t_win / R;
+      if (debug)
+        std::fprintf(stderr, "[wl_refine]   worklist window of %d rounds, %s: %.1f us per round, largest |L| %lld\n", R,
+                     shape ? "one cluster launch" : "two kernels per round", us_round[shape], (long long)frontier);
       int done = R;
       for (int j = 0; j < R; ++j) {
         const int64_t k_new = (int64_t)hs[kScalLog + j];

@@ -197,11 +197,11 @@ def test_canonicalize(n):
 
 # ------------------------------------------------------------------ whole Algorithm 1
 # 256 = WL_FLAG_NO_DEEP, 512 = WL_FLAG_DEEP_EARLY (worklist regime from round 2 on: every graph goes through it),
-# 1024 = WL_FLAG_NO_FINAL (no finality pruning)
+# 1024 = WL_FLAG_NO_FINAL (no finality pruning), 32768 = WL_FLAG_DEEP_CLUSTER (every worklist window as one cluster launch)
 @pytest.mark.parametrize("name", list(GRAPHS))
 # 16384 = WL_FLAG_TAG_TABLE (the shared-memory hot-id table in every 16-bit round)
 @pytest.mark.parametrize("flags", [0, 2, 4, 64, 128, 128 | 2, 256, 512, 512 | 64, 512 | 2, 1024, 1024 | 256,
-                                   16384, 16384 | 2, 16384 | 512])
+                                   16384, 16384 | 2, 16384 | 512, 512 | 32768, 32768 | 2])
 def test_refine_equals_oracle(name, flags):
     g = GRAPHS[name]()
     n, rp, ci, wt = g.numpy()
@@ -243,7 +243,7 @@ DEEP_GRAPHS = {
 
 
 @pytest.mark.parametrize("name", list(DEEP_GRAPHS))
-@pytest.mark.parametrize("flags", [0, 64, 256, 512])
+@pytest.mark.parametrize("flags", [0, 64, 256, 512, 32768, 512 | 32768])
 def test_refine_deep_rounds_equal_oracle(name, flags):
     """Graphs that need tens to thousands of rounds: the worklist regime (rounds > 6, wl_deep.cuh) must give the oracle's
     colouring AND its per-round colour counts, with and without run-ahead windows, and the same as the plain loop (256)."""
