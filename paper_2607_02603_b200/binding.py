@@ -405,9 +405,10 @@ def wl_refine_inner(row_ptr: torch.Tensor, col_idx: torch.Tensor, weights: Optio
 
 
 def wl_quotient_rows(row_ptr: torch.Tensor, col_idx: torch.Tensor, weights: Optional[torch.Tensor], lo: int, block_of: torch.Tensor,
-                     is_first: torch.Tensor, first_block: int, num_blocks: int):
+                     is_first: torch.Tensor, first_block: int, num_blocks: int, raw: bool = False):
     """B6 for whole rows on device tensors: quotient rows of the blocks whose first node lies in [lo, lo + n).
-    -> (q_row_ptr int64[num_blocks + 1], q_col int32[q_m], q_weights int64[q_m])."""
+    -> (q_row_ptr int64[num_blocks + 1], q_col int32[q_m], q_weights int64[q_m]); raw: the buffers as the library wrote them
+    (q_row_ptr, q_col int32[capacity], q_weights int32[capacity] = uint32 bit patterns, q_m)."""
     L = lib()
     dev = row_ptr.device
     nr = row_ptr.numel() - 1
@@ -425,6 +426,8 @@ def wl_quotient_rows(row_ptr: torch.Tensor, col_idx: torch.Tensor, weights: Opti
                                 _ptr(q_wt), m, C.byref(qm), _ptr(ws), ws.numel(), _stream_ptr(dev))
     if rc != WL_OK:
         raise WlError(rc, "wl_quotient_rows")
+    if raw:
+        return q_rp, q_col, q_wt, qm.value
     return q_rp, q_col[: qm.value], q_wt[: qm.value].to(torch.int64) & 0xFFFFFFFF
 
 

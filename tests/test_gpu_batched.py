@@ -484,7 +484,7 @@ def test_per_batch_device_calls_match_the_definitions(seed):
     col = g.col[a:b].contiguous()
     wt = None if g.weights is None else g.weights[a:b].contiguous()
     ob = OracleBackend()
-    want_c, want_f, want_k = ob.refine_inner(rp, col, wt, lo, n, 0, 0)
+    want_c, want_f, want_k = ob.refine_inner(rp, 0, col, wt, lo, n, 0, 0)
     c, f, k = wl.wl_refine_inner(rp.to(dev()), col.to(dev()), None if wt is None else wt.to(dev()), lo, n, seed=seed)
     assert k == want_k and c.cpu().tolist() == want_c.tolist() and f.cpu().tolist() == want_f.tolist()
     # a block map of the whole graph: the inner range keeps its local blocks, everybody else is a singleton
@@ -493,7 +493,10 @@ def test_per_batch_device_calls_match_the_definitions(seed):
     block_of[lo:hi] = want_c + lo
     block_of[hi:] = torch.arange(n - hi, dtype=torch.int32) + lo + k
     ob.set_block_map(block_of)
-    wr, wc, ww = ob.quotient_rows(rp, col, wt, lo, want_f, lo, k)
+    h_rp, _, h_col, h_wt = ob.host_buffers(k, col.numel())
+    qm = ob.quotient_rows(rp, 0, col, wt, lo, want_f, lo, k, h_rp[1:], h_col, h_wt, 0)
+    h_rp[0] = 0
+    wr, wc, ww = h_rp[:k + 1], h_col[:qm], torch.from_numpy(h_wt[:qm].numpy().view(np.uint32).astype(np.int64))
     qr, qc, qw = wl.wl_quotient_rows(rp.to(dev()), col.to(dev()), None if wt is None else wt.to(dev()), lo, block_of.to(dev()),
                                      f, lo, k)
     assert qr.cpu().tolist() == wr.tolist()
