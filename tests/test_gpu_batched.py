@@ -1,4 +1,5 @@
 """GPU parity tests of the batched path (Algorithm 2) and its step-level pieces."""
+import os
 import numpy as np
 import pytest
 import torch
@@ -504,3 +505,50 @@ def test_per_batch_device_calls_match_the_definitions(seed):
     with pytest.raises(wl.WlError) as e:  # the range does not fit the node count
         wl.wl_refine_inner(rp.to(dev()), col.to(dev()), None, n, n, seed=1)
     assert e.value.code == wl.WL_EINVAL
+
+
+def _sharded_cuda_worker(rank, world, port, q):
+    import os
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    sys.path.insert(0, root)
+    import torch.distributed as dist
+    from paper_2607_02603_b200.sharded import refine_batched_sharded
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    out = {}
+    for name in ("rmat11_dir", "weighted", "hub"):
+        g = BATCH_GRAPHS[name]()
+        cap = max(1, g.m // 6 + 1)
+        colours, k, outer = refine_batched_sharded(g.n, g.row_ptr.pin_memory(), g.col.pin_memory(),
+                                                   None if g.weights is None else g.weights.pin_memory(), max_batch_edges=cap,
+                                                   seed=3 + rank, dist=dist, device=torch.device("cuda", 0))
+        out[name] = (colours.tolist(), k, outer)
+    dist.barrier()
+    q.put((rank, out))
+    dist.destroy_process_group()
+
+
+def test_sharded_two_processes_with_cuda_backend_over_gloo():
+    """The real loop of the sharded driver (run(): all-gather of the block counts, all-gather-v of the block-map slices that
+    live on the GPU) with the CUDA backend in TWO processes; both use this one GPU and talk over gloo (host-level collectives
+    only: no kernel of one rank ever waits for the other).  Both ranks must end with the colouring of the CPU Algorithm 2."""
+    import torch.multiprocessing as mp
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = 32500 + os.getpid() % 2000
+    procs = [ctx.Process(target=_sharded_cuda_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    res = dict(q.get(timeout=600) for _ in procs)
+    for p in procs:
+        p.join(timeout=120)
+        assert p.exitcode == 0
+    for name in ("rmat11_dir", "weighted", "hub"):
+        g = BATCH_GRAPHS[name]()
+        n, rp, ci, wt = g.numpy()
+        want, k_want, outer_want, _ = oracle.rbsc(n, rp, ci, wt, max(1, g.m // 6 + 1), inherit=True)
+        for rank in (0, 1):
+            colours, k, outer = res[rank][name]
+            assert colours == want.tolist() and k == k_want and outer == outer_want, (name, rank)
