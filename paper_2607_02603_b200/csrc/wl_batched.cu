@@ -206,27 +206,35 @@ quot_insert_kernel(int64_t row_base, int64_t n_rows, const int64_t* __restrict__
   if (lane == 0 && fresh) atomicAdd(cnt + b, fresh);
 }
 
-// the queued long pieces: up to kQuotGiantRow entries one CTA per piece (CTAs take pieces in turn), longer ones (hub rows of
-// 10^5-10^6 entries) one after the other, each spread over the whole grid
-constexpr int64_t kQuotGiantRow = 65536;
+// the queued long pieces, cut into chunks of kQuotChunk entries that the CTAs take in turn (chunk g of the whole list goes to CTA
+// g mod gridDim: every CTA walks the short list of pieces and keeps the running chunk count, so no prefix array is needed).  The
+// work is spread by entries, whatever the mix of 5 k-entry rows and 10^6-entry hub rows (one CTA per piece left most SMs idle:
+// 1.19 ms per 33 M-entry batch for the 10-20 % of the entries that sit in such rows).
+constexpr int64_t kQuotChunk = 2048;
 __global__ void __launch_bounds__(256)
 quot_insert_long_kernel(int64_t row_base, const int64_t* __restrict__ row_ptr, int64_t clip_lo, int64_t clip_hi,
                         const int* __restrict__ col, const u32* __restrict__ wt, const int* __restrict__ Hc,
                         Slot* __restrict__ table, u64 table_mask, int* __restrict__ cnt,
                         const int* __restrict__ long_rows, const u32* __restrict__ long_count) {
   const u32 n_long = *long_count;
-  const int64_t tid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x, stride = (int64_t)gridDim.x * blockDim.x;
+  int64_t chunk0 = 0;  // chunks of the pieces before piece j
   for (u32 j = 0; j < n_long; ++j) {
     const int64_t w = long_rows[j];
     int64_t a = row_ptr[w], e = row_ptr[w + 1];
     if (a < clip_lo) a = clip_lo;
     if (e > clip_hi) e = clip_hi;
-    const bool giant = e - a > kQuotGiantRow;
-    if (!giant && j % gridDim.x != blockIdx.x) continue;  // this piece belongs to another CTA
+    const int64_t nch = (e - a + kQuotChunk - 1) / kQuotChunk;
+    // first chunk of this piece that is mine: the smallest q >= 0 with (chunk0 + q) mod gridDim == blockIdx
+    int64_t q = ((int64_t)blockIdx.x - chunk0 % (int64_t)gridDim.x + (int64_t)gridDim.x) % (int64_t)gridDim.x;
+    chunk0 += nch;
+    if (q >= nch) continue;
     const int b = Hc[row_base + w];
     int fresh = 0;
-    for (int64_t p = a + (giant ? tid : (int64_t)threadIdx.x); p < e; p += giant ? stride : (int64_t)blockDim.x)
-      fresh += quot_insert_one(table, table_mask, b, Hc[col[p]], wt ? (u64)wt[p] : 1ull) ? 1 : 0;
+    for (; q < nch; q += gridDim.x) {
+      const int64_t ca = a + q * kQuotChunk, ce = ca + kQuotChunk < e ? ca + kQuotChunk : e;
+      for (int64_t p = ca + threadIdx.x; p < ce; p += blockDim.x)
+        fresh += quot_insert_one(table, table_mask, b, Hc[col[p]], wt ? (u64)wt[p] : 1ull) ? 1 : 0;
+    }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) fresh += __shfl_xor_sync(0xffffffffu, fresh, o);
     if ((threadIdx.x & 31) == 0 && fresh) atomicAdd(cnt + b, fresh);
