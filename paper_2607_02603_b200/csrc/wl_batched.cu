@@ -175,6 +175,37 @@ __device__ __forceinline__ bool quot_insert_one(Slot* __restrict__ table, u64 ma
   }
 }
 
+// The same insertion, but the probe sequence of an entry of row [A, A + len) of the edge array STARTS inside the row's own region
+// of the table, slots [2 A, 2 (A + len)) mod the table size (equal keys can only meet inside one row, so nothing is lost; keys
+// still carry the block, so regions that wrap or overlap - a row longer than the table, a cut row next to later batches - are
+// merely less local, never wrong).  The slots of a short row then share a few 128-byte lines instead of one random sector per
+// entry, and the emission, which sweeps the table in slot order, finds the entries of a block next to each other: its output
+// positions are consecutive and its writes coalesce.
+__device__ __forceinline__ bool quot_insert_at(Slot* __restrict__ table, u64 mask, u64 region_base, u64 region_size, int b,
+                                               int target, u64 weight) {
+  const u64 key1 = (((u64)(u32)b << 32) | (u64)(u32)target) + 1;
+  u64 slot = (region_base + __umul64hi(slot_hash((u32)target, key1), region_size)) & mask;
+  while (true) {
+    Slot v = load_slot(table + slot);
+    if (v.y == 0) {
+      const Slot empty = {0ull, 0ull}, mine = {key1, weight};
+      v = cas128(table + slot, empty, mine);
+      if (v.y == 0) return true;
+    }
+    if (v.y == key1) {
+      atomicAdd(&table[slot].cx, weight);
+      return false;
+    }
+    slot = (slot + 1) & mask;
+  }
+}
+// region of the row whose entries are the positions [A, E) of the edge array (unclipped)
+__device__ __forceinline__ void quot_region(int64_t A, int64_t E, u64 mask, u64* base, u64* size) {
+  const u64 len = (u64)(E - A);
+  *base = 2ull * (u64)A;
+  *size = len == 0 ? 1 : (2 * len > mask + 1 ? mask + 1 : 2 * len);
+}
+
 constexpr int kQuotLongRow = 4096;  // longer pieces are left to quot_insert_long_kernel (whole grid per row)
 
 // One warp per row of [row_base, row_base + n_rows); only the representative row of a block contributes (Def. 4, Q17).
@@ -192,6 +223,8 @@ quot_insert_kernel(int64_t row_base, int64_t n_rows, const int64_t* __restrict__
   const int b = Hc[i];
   if (isrep ? !isrep[i] : rep_of_block[b] != (int)i) return;  // representative = first node of its block (Q17)
   int64_t a = row_ptr[w], e = row_ptr[w + 1];
+  u64 rbase, rsize;
+  quot_region(a, e, table_mask, &rbase, &rsize);
   if (a < clip_lo) a = clip_lo;
   if (e > clip_hi) e = clip_hi;
   if (e - a > kQuotLongRow) {
@@ -200,7 +233,7 @@ quot_insert_kernel(int64_t row_base, int64_t n_rows, const int64_t* __restrict__
   }
   int fresh = 0;
   for (int64_t p = a + lane; p < e; p += 32)
-    fresh += quot_insert_one(table, table_mask, b, Hc[col[p]], wt ? (u64)wt[p] : 1ull) ? 1 : 0;
+    fresh += quot_insert_at(table, table_mask, rbase, rsize, b, Hc[col[p]], wt ? (u64)wt[p] : 1ull) ? 1 : 0;
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) fresh += __shfl_xor_sync(0xffffffffu, fresh, o);
   if (lane == 0 && fresh) atomicAdd(cnt + b, fresh);
@@ -221,6 +254,8 @@ quot_insert_long_kernel(int64_t row_base, const int64_t* __restrict__ row_ptr, i
   for (u32 j = 0; j < n_long; ++j) {
     const int64_t w = long_rows[j];
     int64_t a = row_ptr[w], e = row_ptr[w + 1];
+    u64 rbase, rsize;
+    quot_region(a, e, table_mask, &rbase, &rsize);
     if (a < clip_lo) a = clip_lo;
     if (e > clip_hi) e = clip_hi;
     const int64_t nch = (e - a + kQuotChunk - 1) / kQuotChunk;
@@ -233,7 +268,7 @@ quot_insert_long_kernel(int64_t row_base, const int64_t* __restrict__ row_ptr, i
     for (; q < nch; q += gridDim.x) {
       const int64_t ca = a + q * kQuotChunk, ce = ca + kQuotChunk < e ? ca + kQuotChunk : e;
       for (int64_t p = ca + threadIdx.x; p < ce; p += blockDim.x)
-        fresh += quot_insert_one(table, table_mask, b, Hc[col[p]], wt ? (u64)wt[p] : 1ull) ? 1 : 0;
+        fresh += quot_insert_at(table, table_mask, rbase, rsize, b, Hc[col[p]], wt ? (u64)wt[p] : 1ull) ? 1 : 0;
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) fresh += __shfl_xor_sync(0xffffffffu, fresh, o);
@@ -247,15 +282,22 @@ quot_insert_long_kernel(int64_t row_base, const int64_t* __restrict__ row_ptr, i
 __global__ void quot_emit_kernel(u64* __restrict__ table, u64 table_slots, const int64_t* __restrict__ q_row_ptr,
                                  int64_t out_base, int* __restrict__ cursor, int* __restrict__ q_col,
                                  u32* __restrict__ q_wt, int b_lo, int b_hi) {
-  int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (s >= (int64_t)table_slots) return;
-  const u64 key1 = table[2 * s];
-  if (key1 == 0) return;
+  const int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int lane = threadIdx.x & 31;
+  u64 key1 = 0;
+  if (s < (int64_t)table_slots) key1 = table[2 * s];
   const u64 key = key1 - 1;
   const int b = (int)(key >> 32), t = (int)(key & 0xffffffffu);
-  if (b < b_lo || b >= b_hi) return;
+  const bool live = key1 != 0 && b >= b_lo && b < b_hi;
+  // neighbouring slots mostly hold entries of one block (quot_insert_at): the lanes of a block reserve their positions together
+  const unsigned peers = __match_any_sync(0xffffffffu, live ? b : -1 - lane);
+  const int leader = __ffs(peers) - 1;
+  int base = 0;
+  if (live && lane == leader) base = atomicAdd(cursor + b, __popc(peers));
+  base = __shfl_sync(0xffffffffu, base, leader);
+  if (!live) return;
   const u64 sum = table[2 * s + 1];
-  const int64_t pos = q_row_ptr[b] - out_base + atomicAdd(cursor + b, 1);
+  const int64_t pos = q_row_ptr[b] - out_base + base + __popc(peers & ((1u << lane) - 1));
   q_col[pos] = t;
   q_wt[pos] = (u32)sum;
   table[2 * s] = 0;
