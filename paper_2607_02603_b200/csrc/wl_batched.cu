@@ -19,6 +19,10 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <condition_variable>
+#include <functional>
+#include <mutex>
+#include <thread>
 #include <vector>
 
 #include "wl_host.h"
@@ -50,6 +54,65 @@ __global__ void merge_kernel(int64_t n_local, const int* __restrict__ local_colo
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i < n_local) H[i] = base + local_colour[i];
 }
+
+// One helper thread per wl_refine_batched call (WL_FLAG_INHERIT_BATCHES): the local refinement of the rows the quotient pass has
+// just emitted synchronises its stream once per round, and while the calling thread sat in it the next emission could not be
+// queued.  The helper runs those refinements one after the other (their block ids build on each other); the caller submits a
+// piece and waits for it only when the piece's buffers are needed again.
+class PieceWorker {
+ public:
+  explicit PieceWorker(int device) : device_(device) {}
+  ~PieceWorker() {
+    if (!th_.joinable()) return;
+    {
+      std::lock_guard<std::mutex> g(mu_);
+      stop_ = true;
+    }
+    cv_.notify_all();
+    th_.join();
+  }
+  void submit(std::function<int()> f) {  // at most one task is outstanding: wait() first
+    if (!th_.joinable()) th_ = std::thread([this] { loop(); });
+    {
+      std::lock_guard<std::mutex> g(mu_);
+      task_ = std::move(f);
+      busy_ = true;
+    }
+    cv_.notify_all();
+  }
+  int wait() {  // result of the last task (WL_OK when none was submitted)
+    std::unique_lock<std::mutex> g(mu_);
+    cv_.wait(g, [this] { return !busy_; });
+    const int r = result_;
+    result_ = WL_OK;
+    return r;
+  }
+
+ private:
+  void loop() {
+    cudaSetDevice(device_);
+    std::unique_lock<std::mutex> g(mu_);
+    while (true) {
+      cv_.wait(g, [this] { return stop_ || (busy_ && task_); });
+      if (stop_) return;
+      std::function<int()> f = std::move(task_);
+      task_ = nullptr;
+      g.unlock();
+      const int r = f();
+      g.lock();
+      result_ = r;
+      busy_ = false;
+      cv_.notify_all();
+    }
+  }
+  int device_;
+  std::thread th_;
+  std::mutex mu_;
+  std::condition_variable cv_;
+  std::function<int()> task_;
+  bool busy_ = false, stop_ = false;
+  int result_ = WL_OK;
+};
 
 // every stored target of an uploaded slice must be a node id in [0, n)
 __global__ void slice_cols_check_kernel(int64_t n, int64_t count, const int* __restrict__ col, u32* __restrict__ err) {
@@ -1399,6 +1462,9 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
 
   u64* hs = host_scal();
   if (!hs) return WL_ECUDA;
+  int dev_id = 0;
+  cudaGetDevice(&dev_id);
+  PieceWorker piece_worker(dev_id);  // (declared before everything its tasks touch: it is joined last)
   cudaStream_t copy_st, down_st, side_st;  // uploads; return of quotient rows; refinement of emitted pieces (inherit)
   if (cudaStreamCreateWithFlags(&copy_st, cudaStreamNonBlocking) != cudaSuccess) return check_cuda(cudaGetLastError());
   if (cudaStreamCreateWithFlags(&down_st, cudaStreamNonBlocking) != cudaSuccess) {
@@ -1869,9 +1935,14 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
       int ob, index;
     };
     Piece pending{false, 0, 0, 0, 0, 0, 0};
-    auto refine_piece = [&]() -> int {
-      if (!pending.valid) return WL_OK;
-      pending.valid = false;
+    int64_t piece_launches = 0;  // kernels launched by the helper thread (g_launches is per thread)
+    auto refine_piece_body = [&](const Piece pending) -> int {
+      const int64_t launches0 = g_launches;
+      struct Count {
+        int64_t& sum;
+        int64_t from;
+        ~Count() { sum += g_launches - from; }
+      } count{piece_launches, launches0};
       const int64_t nr = pending.b_hi - pending.b_lo;
       cudaStreamWaitEvent(side_st, ev_emit[pending.ob], 0);
       if (pending.tot == 0) {  // edgeless nodes only: one block (Eq. 3)
@@ -1911,6 +1982,16 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
       // the emission buffers may be overwritten once this piece is refined (emission + 2 waits on the stream `st`)
       cudaEventRecord(ev_piece[pending.ob], side_st);
       return check_cuda(cudaStreamSynchronize(side_st));  // d_ws2 is reused by the next piece
+    };
+    // joins the piece before (its ids come first, its workspace is reused) and hands the pending one to the helper thread
+    auto refine_piece = [&]() -> int {
+      const int prc = piece_worker.wait();
+      if (prc) return prc;
+      if (!pending.valid) return WL_OK;
+      const Piece p = pending;
+      pending.valid = false;
+      piece_worker.submit([&refine_piece_body, p]() { return refine_piece_body(p); });
+      return WL_OK;
     };
     int64_t q_off = 0, emitted_blocks = 0;
     int n_emit = 0;
@@ -2025,6 +2106,11 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
       }
     }
     if (!rc) rc = refine_piece();
+    {
+      const int prc = piece_worker.wait();  // (also on an error path: nothing of this iteration may outlive it)
+      if (!rc) rc = prc;
+    }
+    g_launches += piece_launches;
     if (!rc) rc = check_cuda(cudaStreamSynchronize(side_st));
     if (!rc) rc = check_cuda(cudaStreamSynchronize(st));
     if (!rc) rc = flush_overflow();

@@ -290,13 +290,20 @@ int basic_csr_check(const wl_csr* g) {
   return WL_OK;
 }
 
-// pinned host mirror of the device scalars (one per host thread)
+// pinned host mirror of the device scalars (one per host thread; released when the thread ends: the batched path runs
+// refinements on a helper thread of its own per call)
 u64* host_scal() {
-  static thread_local u64* p = nullptr;
-  if (!p) {
-    if (cudaHostAlloc((void**)&p, sizeof(u64) * (kNumScal + 8), cudaHostAllocDefault) != cudaSuccess) p = nullptr;
+  struct Holder {
+    u64* p = nullptr;
+    ~Holder() {
+      if (p) cudaFreeHost(p);
+    }
+  };
+  static thread_local Holder h;
+  if (!h.p) {
+    if (cudaHostAlloc((void**)&h.p, sizeof(u64) * (kNumScal + 8), cudaHostAllocDefault) != cudaSuccess) h.p = nullptr;
   }
-  return p;
+  return h.p;
 }
 
 }  // namespace wl
