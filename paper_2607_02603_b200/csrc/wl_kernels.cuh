@@ -227,7 +227,8 @@ __device__ __forceinline__ void
 rows32_group(const int64_t base, const int lane, int64_t nrows, const int* __restrict__ rows,
              const int64_t* __restrict__ row_ptr, const int* __restrict__ col, const u32* __restrict__ wt,
              const CT* __restrict__ colour, u64 key, u64* __restrict__ y, int64_t hub_threshold, int lo, int hi,
-             int64_t n_targets, bool& bad, const u32* s_tag, u32 idmask, u64 key2 = 0, u64* __restrict__ y2 = nullptr) {
+             int64_t n_targets, bool& bad, const u32* s_tag, u32 idmask, u64 key2 = 0, u64* __restrict__ y2 = nullptr,
+             bool hub_store = true) {
   const int64_t idx = base + lane;
   const bool valid = idx < nrows;
   int64_t i = 0, a = 0, b = 0;
@@ -347,7 +348,8 @@ rows32_group(const int64_t base, const int lane, int64_t nrows, const int* __res
     for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
     if (lane == src) acc = s;
   }
-  if (valid) y[i] = acc;
+  // (hub_store == false: the hub kernel runs NEXT TO this one on a second stream and adds into y[i], zeroed beforehand)
+  if (valid && (hub_store || d <= hub_threshold)) y[i] = acc;
   if (DUAL && valid && d <= kMidRow) y2[i] = acc2;
 }
 
@@ -356,13 +358,14 @@ __global__ void __launch_bounds__(256)
 spmv_rows32_kernel(int64_t nrows, const int* __restrict__ rows, const int64_t* __restrict__ row_ptr,
                    const int* __restrict__ col, const u32* __restrict__ wt, const CT* __restrict__ colour, u64 key,
                    u64* __restrict__ y, int64_t hub_threshold, int lo, int hi, int64_t n_targets,
-                   u32* __restrict__ err, u64 key2 = 0, u64* __restrict__ y2 = nullptr) {
+                   u32* __restrict__ err, u64 key2 = 0, u64* __restrict__ y2 = nullptr, int hub_store = 1) {
   const int lane = threadIdx.x & 31;
   const int64_t base = (((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5) << 5;
   if (base >= nrows) return;
   bool bad = false;
   rows32_group<WEIGHTED, CT, RANGED, VALIDATE, false, DUAL>(base, lane, nrows, rows, row_ptr, col, wt, colour, key, y,
-                                                            hub_threshold, lo, hi, n_targets, bad, nullptr, 0u, key2, y2);
+                                                            hub_threshold, lo, hi, n_targets, bad, nullptr, 0u, key2, y2,
+                                                            hub_store != 0);
   if (VALIDATE && bad) atomicOr(err, kErrCol);
 }
 
@@ -434,6 +437,12 @@ __global__ void hub_collect_rows_kernel(int64_t nrows, const int* __restrict__ r
   const int nc = (int)((d + kHubChunk - 1) / kHubChunk);
   const u64 base = atomicAdd(counter, (u64)nc);
   for (int c = 0; c < nc; ++c) chunks[base + c] = make_int2(i, c);
+}
+
+// y of every hub row = 0 (its first chunk does it): the hub kernel may then run next to the row kernel
+__global__ void hub_zero_kernel(int64_t nchunks, const int2* __restrict__ chunks, u64* __restrict__ y) {
+  const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t < nchunks && chunks[t].y == 0) y[chunks[t].x] = 0;
 }
 
 // active == NULL: every hub row; else only rows whose block is still splittable (stamp[colour[row]] == live_stamp)

@@ -122,6 +122,8 @@ struct SpmvArgs {
   u64 key2 = 0;                // DUAL rows: second key and second sum (finality test of the coming compaction)
   u64* y2 = nullptr;
   bool hubs_only = false;      // the row kernel has been launched piece by piece (ColumnFeed): only the hub chunks are left
+  cudaStream_t hub_stream = nullptr;  // not NULL: the hub kernel runs on this stream NEXT TO the row kernel (it fills the row
+  cudaEvent_t hub_fork = nullptr, hub_join = nullptr;  // kernel's tail: 4 % of its time on the headline round)
 };
 
 // edge-balanced S1+S2 over all rows of g (see spmv_eb_kernel)
@@ -164,16 +166,30 @@ static void launch_rows_tag(const wl_csr& g, const SpmvArgs& a, u64 key, u64* y,
 template <bool W, typename CT, bool R, bool V>
 static void launch_row_hub2(const wl_csr& g, const SpmvArgs& a, const CT* colour, u64 key, u64* y, cudaStream_t st) {
   unsigned grid = blocks_for(a.nrows, kRowsCta);
+  // side by side: y of the hub rows is zeroed first, the row kernel leaves those rows alone, the hub kernel is queued on the
+  // second stream right behind the row kernel's launch: its CTAs get the SMs the row kernel no longer fills
+  const bool beside = a.hub_stream && a.num_hub_chunks > 0 && !a.hubs_only && !(!W && !R && a.tag32 && a.narrow);
+  if (beside) {
+    ++g_launches; hub_zero_kernel<<<blocks_for(a.num_hub_chunks, 256), 256, 0, st>>>(a.num_hub_chunks, a.hub_chunks, y);
+    cudaEventRecord(a.hub_fork, st);
+    cudaStreamWaitEvent(a.hub_stream, a.hub_fork, 0);
+  }
+  const int hub_store = beside ? 0 : 1;
   if (a.hubs_only) {
   } else if (!W && !R && a.tag32 && a.narrow) {
     launch_rows_tag<V>(g, a, key, y, st);
   } else if (!W && !R && !V && a.y2 && sizeof(CT) == 4) {
-    ++g_launches; spmv_rows32_kernel<false, int, false, false, true><<<grid, kRowsCta, 0, st>>>(a.nrows, a.rows, g.row_ptr, g.col_idx, g.weights, a.colour, key, y, kHubThreshold, a.lo, a.hi, a.n_targets, a.err, a.key2, a.y2);
+    ++g_launches; spmv_rows32_kernel<false, int, false, false, true><<<grid, kRowsCta, 0, st>>>(a.nrows, a.rows, g.row_ptr, g.col_idx, g.weights, a.colour, key, y, kHubThreshold, a.lo, a.hi, a.n_targets, a.err, a.key2, a.y2, hub_store);
   } else {
-    ++g_launches; spmv_rows32_kernel<W, CT, R, V><<<grid, kRowsCta, 0, st>>>(a.nrows, a.rows, g.row_ptr, g.col_idx, g.weights, colour, key, y, kHubThreshold, a.lo, a.hi, a.n_targets, a.err);
+    ++g_launches; spmv_rows32_kernel<W, CT, R, V><<<grid, kRowsCta, 0, st>>>(a.nrows, a.rows, g.row_ptr, g.col_idx, g.weights, colour, key, y, kHubThreshold, a.lo, a.hi, a.n_targets, a.err, 0, nullptr, hub_store);
   }
   if (a.num_hub_chunks > 0) {
-    ++g_launches; spmv_hub_kernel<W, CT, R, V><<<(unsigned)a.num_hub_chunks, kHubThreads, 0, st>>>(a.hub_chunks, g.row_ptr, g.col_idx, g.weights, colour, key, y, a.colour, a.stamp, a.live_stamp, a.lo, a.hi, a.n_targets, a.err);
+    cudaStream_t hs = beside ? a.hub_stream : st;
+    ++g_launches; spmv_hub_kernel<W, CT, R, V><<<(unsigned)a.num_hub_chunks, kHubThreads, 0, hs>>>(a.hub_chunks, g.row_ptr, g.col_idx, g.weights, colour, key, y, a.colour, a.stamp, a.live_stamp, a.lo, a.hi, a.n_targets, a.err);
+    if (beside) {
+      cudaEventRecord(a.hub_join, a.hub_stream);
+      cudaStreamWaitEvent(st, a.hub_join, 0);
+    }
   }
 }
 template <bool W, typename CT>
@@ -334,7 +350,7 @@ namespace wl {
 // a round whose table fits the lower half does not wait for the upper one.
 struct AuxStream {
   cudaStream_t s = nullptr;
-  cudaEvent_t fork = nullptr, done_a = nullptr, done_b = nullptr;
+  cudaEvent_t fork = nullptr, done_a = nullptr, done_b = nullptr, hub_fork = nullptr, hub_join = nullptr;
   u64 slots_a = 0, slots_b = 0;  // slots [0, slots_a) are empty after done_a, [0, slots_b) after done_b
   bool active = false;
   int init() {
@@ -342,6 +358,8 @@ struct AuxStream {
     cudaEventCreateWithFlags(&fork, cudaEventDisableTiming);
     cudaEventCreateWithFlags(&done_a, cudaEventDisableTiming);
     cudaEventCreateWithFlags(&done_b, cudaEventDisableTiming);
+    cudaEventCreateWithFlags(&hub_fork, cudaEventDisableTiming);
+    cudaEventCreateWithFlags(&hub_join, cudaEventDisableTiming);
     return WL_OK;
   }
   Slot* table = nullptr;
@@ -361,6 +379,8 @@ struct AuxStream {
     if (fork) cudaEventDestroy(fork);
     if (done_a) cudaEventDestroy(done_a);
     if (done_b) cudaEventDestroy(done_b);
+    if (hub_fork) cudaEventDestroy(hub_fork);
+    if (hub_join) cudaEventDestroy(hub_join);
     if (s) cudaStreamDestroy(s);
   }
 };
@@ -555,6 +575,11 @@ int refine_core(const wl_csr* g, const int32_t* init_colors, uint64_t seed, cons
       SpmvArgs a{cur_list, n_active, colour, colour16, narrow, hub_chunks, active_hubs > 0 ? num_hub_chunks : 0,
                  cur_list ? stamp : nullptr, (int)r - 1, ranged, lo, hi};
       a.eb = eb;
+      if (aux.active && !(flags & WL_FLAG_SYNC_EVERY_ROUND)) {  // (the side stream exists for large uniform starts)
+        a.hub_stream = aux.s;
+        a.hub_fork = aux.hub_fork;
+        a.hub_join = aux.hub_join;
+      }
       a.chunk_row = chunk_row;
       a.e_first = edge_first;
       a.n_targets = n_targets;
