@@ -69,6 +69,9 @@ typedef struct wl_csr {
 #define WL_FLAG_DEEP_CLUSTER 32768u /* worklist regime: every window of queued rounds as ONE launch by one thread-block cluster
                                        (cluster barriers between the phases instead of kernel boundaries).  Same results; measured
                                        slower than the default two kernels per round on B200, kept for testing                */
+#define WL_FLAG_NO_FUSED_RECUT 2048u /* batched, default (re-cut) mode: always upload every batch again for its local refinement
+                                        (default: the quotient pass refines the next iteration's greedy batches on the rows it
+                                        has just emitted, whenever every row fits a batch).  Same results                       */
 #define WL_FLAG_NO_FINAL 1024u   /* do not drop blocks whose whole neighbourhood is final from the active set (R5)        */
 #define WL_FLAG_INHERIT_BATCHES 4096u /* batched: from the second outer iteration on, a quotient keeps the batches of its
                                         graph (the rows emitted together) instead of being re-cut by M_b, and its local

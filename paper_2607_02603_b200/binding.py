@@ -23,6 +23,7 @@ WL_FLAG_EDGE_BALANCED = 128
 WL_FLAG_NO_DEEP = 256
 WL_FLAG_DEEP_EARLY = 512
 WL_FLAG_NO_FINAL = 1024
+WL_FLAG_NO_FUSED_RECUT = 2048
 WL_FLAG_DEEP_CLUSTER = 32768
 WL_FLAG_INHERIT_BATCHES = 4096
 WL_FLAG_CONSUME_INPUT = 8192

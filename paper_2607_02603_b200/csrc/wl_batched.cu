@@ -180,6 +180,37 @@ __global__ void count_reps_kernel(int64_t n, const unsigned char* __restrict__ i
   if (q >= 0 && (int)(threadIdx.x & 31) == __ffs(peers) - 1) atomicAdd(counts + q, (u64)__popc(peers));
 }
 
+// *out = max(*out, max of a[0 .. n)) (the longest row of the quotient being emitted: its row lengths are the block counters)
+__global__ void max_i32_kernel(int64_t n, const int* __restrict__ a, int* __restrict__ out) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  int v = i < n ? a[i] : 0;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v = max(v, __shfl_xor_sync(0xffffffffu, v, o));
+  if ((threadIdx.x & 31) == 0 && v > 0) atomicMax(out, v);
+}
+
+// res[1] = the largest row offset <= limit (rp increasing, rp[0] <= limit): the greedy cut (Q13); res[0] = the first index that has it
+__global__ void cut_search_kernel(const int64_t* __restrict__ rp, int64_t n, int64_t limit, int64_t* __restrict__ res) {
+  if (blockIdx.x || threadIdx.x) return;
+  int64_t lo = 0, hi = n;  // invariant: rp[lo] <= limit
+  while (lo < hi) {
+    const int64_t mid = (lo + hi + 1) >> 1;
+    if (rp[mid] <= limit) lo = mid;
+    else hi = mid - 1;
+  }
+  // rows without entries that sit exactly on the cut belong to the NEXT batch (inner_range: its first node is the first one
+  // whose row starts at or after the cut): back to the first index with this offset
+  const int64_t edge = rp[lo];
+  int64_t a = 0, b = lo;  // first index in [0, lo] with rp[index] >= edge
+  while (a < b) {
+    const int64_t mid = (a + b) >> 1;
+    if (rp[mid] >= edge) b = mid;
+    else a = mid + 1;
+  }
+  res[0] = a;
+  res[1] = edge;
+}
+
 // the window of per-block counters moves on by `len` blocks: the counter of the block whose row is still open (index len)
 // becomes index 0, everything else is zero again
 __global__ void window_carry_kernel(int* __restrict__ cnt, int64_t len, int* __restrict__ carry, int phase) {
@@ -1451,13 +1482,17 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
   // quotient weights of an unweighted input travel as one byte + overflow lists (wt_pack_kernel)
   const bool compress = allow_compress && !coo && !weighted;
   // S0 on the host side of the CSR forms: the offsets steer the cuts, the inner ranges and every upload size
+  int64_t max_row_cur = INT64_MAX;  // longest row of the current graph, when known (it bounds the rows of its quotient, Def. 4)
   if (!coo && !(flags & WL_FLAG_NO_VALIDATE)) {
     if (rp[0] != 0) return WL_EINVAL;
+    int64_t longest = 0;
     for (int64_t i = 0; i < n; ++i) {
       const int64_t d = rp[i + 1] - rp[i];
       if (d < 0) return WL_EINVAL;
       if ((u64)d >= (1ull << 32)) return WL_ERANGE;
+      longest = std::max(longest, d);
     }
+    max_row_cur = longest;
   }
 
   u64* hs = host_scal();
@@ -1476,7 +1511,7 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
     cudaStreamDestroy(down_st);
     return check_cuda(cudaGetLastError());
   }
-  cudaEvent_t ev_begin, ev_end, ev_up[2], ev_ins[2], ev_emit[2], ev_down[2], ev_piece[2];
+  cudaEvent_t ev_begin, ev_end, ev_up[2], ev_ins[2], ev_emit[2], ev_down[2], ev_piece[2], ev_stage[2], ev_staged[2];
   cudaEventCreate(&ev_begin);
   cudaEventCreate(&ev_end);
   for (int b = 0; b < 2; ++b) {
@@ -1485,6 +1520,8 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
     cudaEventCreateWithFlags(&ev_emit[b], cudaEventDisableTiming);
     cudaEventCreateWithFlags(&ev_down[b], cudaEventDisableTiming);
     cudaEventCreateWithFlags(&ev_piece[b], cudaEventDisableTiming);
+    cudaEventCreateWithFlags(&ev_stage[b], cudaEventDisableTiming);
+    cudaEventCreateWithFlags(&ev_staged[b], cudaEventDisableTiming);
   }
   cudaEventRecord(ev_begin, st);
   auto cleanup = [&]() {
@@ -1499,6 +1536,8 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
       cudaEventDestroy(ev_emit[b]);
       cudaEventDestroy(ev_down[b]);
       cudaEventDestroy(ev_piece[b]);
+      cudaEventDestroy(ev_stage[b]);
+      cudaEventDestroy(ev_staged[b]);
     }
     cudaStreamDestroy(copy_st);
     cudaStreamDestroy(down_st);
@@ -1606,7 +1645,8 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
     // are canonical without a pass over all nodes, and the per-block counters of the quotient pass live in a window.
     size_t used_iter = used;
     DevBuf d_Hc, d_isrep, d_ws, d_col[2], d_wt[2], d_rp[2], d_cnt, d_cursor, d_qrp[2], d_qtab, d_qcol[2], d_qwt[2], d_sbsum,
-        d_misc, d_query, d_long, d_Hnext, d_isrep_next, d_ws2, d_wt8[2], d_ovf_up[2], d_qwt8[2], d_qovf[2];
+        d_misc, d_query, d_long, d_Hnext, d_isrep_next, d_ws2, d_wt8[2], d_ovf_up[2], d_qwt8[2], d_qovf[2], d_stg_rp[2],
+        d_stg_col[2], d_stg_wt[2];
     // the graph of this iteration has compressed weights (it is a quotient this call wrote)
     const bool read_compressed = compress && outer > 1;
     HostQuot::Generation& Gr = hq.gen[(outer & 1) ^ 1];  // overflow lists of the graph being read
@@ -1913,6 +1953,39 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
       WL_ALLOC(d_ws2, make_layout(max_piece_rows, out_cap).bytes);
       if (rc) break;
     }
+    // Re-cut mode (the default, Alg. 2 as printed), fused: the emitted rows arrive in the row order of the next graph, so they are
+    // staged on the device and cut by the same greedy rule (Q13) as they come; every cut is refined at once (as the inherited
+    // mode does with its pieces), and the next outer iteration starts at the merge: ONE upload pass per iteration.  Needs every
+    // row of the quotient to fit a batch (then every cut falls on a row boundary and no row is ever cut): rows of a quotient
+    // are no longer than the longest row of their graph (Def. 4).  Anything unexpected (staging too small, a piece with more
+    // rows than prepared for, cuts that differ from the host's greedy cuts at the end) just drops the fusion for this
+    // iteration: the next one then uploads its batches for the local refinement as before.
+    const int64_t stage_cap_e = max_batch_edges + out_cap;     // entries a staging buffer holds
+    const int64_t piece_rows_cap = 2 * max_rows + win + 1024;  // rows of one greedy batch we are prepared for
+    const int64_t stage_cap_r = piece_rows_cap + win + 2;
+    bool fuse = !inherit && max_row_cur <= max_batch_edges && !(flags & WL_FLAG_NO_FUSED_RECUT);
+    size_t fuse_ws_bytes = 0;
+    if (fuse) {
+      fuse_ws_bytes = make_layout(piece_rows_cap, max_batch_edges).bytes;
+      const size_t extra = 5 * (size_t)K + fuse_ws_bytes + 2 * (8 * (size_t)stage_cap_r + 8 * (size_t)stage_cap_e) + 4096;
+      if (device_cap_bytes && used_iter + extra > device_cap_bytes) fuse = false;  // optional: never a reason to fail
+    }
+    if (fuse) {
+      WL_ALLOC(d_Hnext, sizeof(int) * (size_t)K);
+      WL_ALLOC(d_isrep_next, (size_t)K);
+      WL_ALLOC(d_ws2, fuse_ws_bytes);
+      for (int b = 0; b < 2; ++b) {
+        WL_ALLOC(d_stg_rp[b], sizeof(int64_t) * (size_t)stage_cap_r);
+        WL_ALLOC(d_stg_col[b], sizeof(int) * (size_t)stage_cap_e);
+        WL_ALLOC(d_stg_wt[b], sizeof(u32) * (size_t)stage_cap_e);
+      }
+      if (rc) break;
+    }
+    int64_t* d_cutres = (int64_t*)(d_misc.as<u64>() + 40);  // cut_search_kernel's two results
+    int* d_maxrow = (int*)(d_misc.as<u64>() + 44);          // longest row of the quotient being emitted
+    cudaMemsetAsync(d_maxrow, 0, sizeof(int), st);
+    int stg_cur = 0;
+    int64_t stg_row0 = 0, stg_rows = 0, stg_e0 = 0, stg_e1 = 0;  // staged: rows [row0, row0 + rows), entries [e0, e1) of the quotient
     auto upload_quot = [&](int k, int buf) {
       const int64_t c0 = cuts[k], c1 = cuts[k + 1];
       if (c1 > c0) {
@@ -1933,8 +2006,12 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
       bool valid;
       int64_t b_lo, b_hi, tot, q_off;
       int ob, index;
+      const int64_t* rp_ptr;  // row offsets of the piece (global edge positions q_off .. q_off + tot)
+      const int* col_base;    // columns, indexed by global edge position
+      const u32* wt_base;     // weights, likewise
+      cudaEvent_t ready, done;  // the rows are in place / the piece has been refined
     };
-    Piece pending{false, 0, 0, 0, 0, 0, 0};
+    Piece pending{false, 0, 0, 0, 0, 0, 0, nullptr, nullptr, nullptr, nullptr, nullptr};
     int64_t piece_launches = 0;  // kernels launched by the helper thread (g_launches is per thread)
     auto refine_piece_body = [&](const Piece pending) -> int {
       const int64_t launches0 = g_launches;
@@ -1944,19 +2021,19 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
         ~Count() { sum += g_launches - from; }
       } count{piece_launches, launches0};
       const int64_t nr = pending.b_hi - pending.b_lo;
-      cudaStreamWaitEvent(side_st, ev_emit[pending.ob], 0);
+      cudaStreamWaitEvent(side_st, pending.ready, 0);
       if (pending.tot == 0) {  // edgeless nodes only: one block (Eq. 3)
         ++g_launches; one_block_kernel<<<blocks_for(nr, 256), 256, 0, side_st>>>(nr, (int)base_next, d_Hnext.as<int>() + pending.b_lo, d_isrep_next.as<unsigned char>() + pending.b_lo);
         base_next += 1;
-        cudaEventRecord(ev_piece[pending.ob], side_st);
-        return WL_OK;
+        cudaEventRecord(pending.done, side_st);
+        return check_cuda(cudaStreamSynchronize(side_st));
       }
       wl_csr lg;
       lg.n = nr;
       lg.m = pending.tot;
-      lg.row_ptr = d_qrp[pending.ob].as<int64_t>();  // global positions q_off .. q_off + tot
-      lg.col_idx = d_qcol[pending.ob].as<int>() - pending.q_off;
-      lg.weights = d_qwt[pending.ob].as<u32>() - pending.q_off;
+      lg.row_ptr = pending.rp_ptr;  // global positions q_off .. q_off + tot
+      lg.col_idx = pending.col_base;
+      lg.weights = pending.wt_base;
       wl_options lo{};
       lo.flags = (flags & (WL_FLAG_NO_PRUNE | WL_FLAG_EDGE_BALANCED)) | WL_FLAG_NO_VALIDATE;
       lo.max_rounds = opt ? opt->max_rounds : 0;
@@ -1980,7 +2057,7 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
       spmv_alg_bytes += cr.spmv_alg_bytes;
       spmv_launches += cr.spmv_launches;
       // the emission buffers may be overwritten once this piece is refined (emission + 2 waits on the stream `st`)
-      cudaEventRecord(ev_piece[pending.ob], side_st);
+      cudaEventRecord(pending.done, side_st);
       return check_cuda(cudaStreamSynchronize(side_st));  // d_ws2 is reused by the next piece
     };
     // joins the piece before (its ids come first, its workspace is reused) and hands the pending one to the helper thread
@@ -2025,6 +2102,44 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
       cudaError_t e = cudaDeviceSynchronize();
       if (e != cudaSuccess) std::fprintf(stderr, "[wl_refine_batched] outer %d batch %d: %s -> %s\n", outer, k, what, cudaGetErrorString(e));
     };
+    // fused re-cut: one greedy batch of the quotient, rows [stg_row0, stg_row0 + idx) of what is staged, handed to the helper
+    // thread; the rest of the staged rows moves to the other staging buffer (the piece keeps reading this one)
+    auto form_piece = [&](int64_t limit, bool take_all) -> int {
+      int64_t idx = stg_rows, cut_edge = stg_e1;
+      if (!take_all) {
+        ++g_launches; cut_search_kernel<<<1, 1, 0, st>>>(d_stg_rp[stg_cur].as<int64_t>(), stg_rows, limit, d_cutres);
+        cudaMemcpyAsync(hs + kNumScal + 6, d_cutres, 2 * sizeof(int64_t), cudaMemcpyDeviceToHost, st);
+        const int src = check_cuda(cudaStreamSynchronize(st));
+        if (src) return src;
+        idx = (int64_t)hs[kNumScal + 6];
+        cut_edge = (int64_t)hs[kNumScal + 7];
+      }
+      if (idx <= 0 || idx > piece_rows_cap) {  // (a batch without rows cannot happen when every row fits a batch)
+        fuse = false;                            // more rows than prepared for: no fusion this time
+        return WL_OK;
+      }
+      const int prc = piece_worker.wait();  // the piece before read the other staging buffer
+      if (prc) return prc;
+      cudaEventRecord(ev_stage[stg_cur], st);
+      pending = Piece{true, stg_row0, stg_row0 + idx, cut_edge - stg_e0, stg_e0, stg_cur, (int)next_node_cuts.size() - 1,
+                      d_stg_rp[stg_cur].as<int64_t>(), d_stg_col[stg_cur].as<int>() - stg_e0, d_stg_wt[stg_cur].as<u32>() - stg_e0,
+                      ev_stage[stg_cur], ev_staged[stg_cur]};
+      next_edge_cuts.push_back(cut_edge);
+      next_node_cuts.push_back(stg_row0 + idx);
+      const int64_t rem_rows = stg_rows - idx, rem_e = stg_e1 - cut_edge;
+      const int other = stg_cur ^ 1;
+      cudaMemcpyAsync(d_stg_rp[other].p, d_stg_rp[stg_cur].as<int64_t>() + idx, sizeof(int64_t) * (size_t)(rem_rows + 1), cudaMemcpyDeviceToDevice, st);
+      if (rem_e > 0) {
+        cudaMemcpyAsync(d_stg_col[other].p, d_stg_col[stg_cur].as<int>() + (cut_edge - stg_e0), sizeof(int) * (size_t)rem_e, cudaMemcpyDeviceToDevice, st);
+        cudaMemcpyAsync(d_stg_wt[other].p, d_stg_wt[stg_cur].as<u32>() + (cut_edge - stg_e0), sizeof(u32) * (size_t)rem_e, cudaMemcpyDeviceToDevice, st);
+      }
+      const int qrc = refine_piece();  // (nothing to join any more: submits)
+      stg_row0 += idx;
+      stg_rows = rem_rows;
+      stg_e0 = cut_edge;
+      stg_cur = other;
+      return qrc;
+    };
     upload_quot(0, 0);
     for (int k = 0; k < nb && !rc; ++k) {
       const int buf = k & 1;
@@ -2043,7 +2158,7 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
       }
       cudaEventRecord(ev_ins[buf], st);
       checkpoint("insert", k);
-      if ((rc = refine_piece())) break;  // the previous emission, next to this insertion
+      if (!fuse && (rc = refine_piece())) break;  // the previous emission, next to this insertion
       // a representative row that continues into the next batch is completed there: emit the blocks whose representative
       // row ends at or before c1 and that were not emitted yet
       const int64_t b_lo = emitted_blocks, b_hi = done_blocks[k];
@@ -2054,6 +2169,9 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
           if (inherit) cudaStreamWaitEvent(st, ev_piece[ob], 0);  // ... and refined
         }
         launch_scan32(d_cnt.as<int>(), b_hi - b_lo, q_off, d_qrp[ob].as<int64_t>(), d_sbsum.as<u64>(), d_misc.as<u64>() + 8, st);
+        if (!inherit) {  // row lengths of the quotient = the block counters: the longest one decides whether the NEXT pass may fuse
+          ++g_launches; max_i32_kernel<<<blocks_for(b_hi - b_lo, 256), 256, 0, st>>>(b_hi - b_lo, d_cnt.as<int>(), d_maxrow);
+        }
         cudaMemcpyAsync(hs + kNumScal + 1, d_misc.as<u64>() + 8, sizeof(u64), cudaMemcpyDeviceToHost, st);
         rc = check_cuda(cudaStreamSynchronize(st));
         if (rc) break;
@@ -2097,13 +2215,38 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
         bytes_d2h += sizeof(int64_t) * (b_hi - b_lo + 1);
         cudaEventRecord(ev_down[ob], down_st);
         if (inherit) {  // refined while the next batch is being inserted (refine_piece)
-          pending = Piece{true, b_lo, b_hi, tot, q_off, ob, (int)next_node_cuts.size() - 1};
+          pending = Piece{true, b_lo, b_hi, tot, q_off, ob, (int)next_node_cuts.size() - 1, d_qrp[ob].as<int64_t>(),
+                          d_qcol[ob].as<int>() - q_off, d_qwt[ob].as<u32>() - q_off, ev_emit[ob], ev_piece[ob]};
           next_edge_cuts.push_back(q_off + tot);
           next_node_cuts.push_back(b_hi);
+        }
+        if (fuse) {  // the emitted rows join the staged ones; every greedy batch that is complete by now is cut off and refined
+          const int64_t nrows_e = b_hi - b_lo;
+          if (stg_rows + nrows_e + 1 > stage_cap_r || (stg_e1 - stg_e0) + tot > stage_cap_e) {
+            fuse = false;
+          } else {
+            cudaMemcpyAsync(d_stg_rp[stg_cur].as<int64_t>() + stg_rows, d_qrp[ob].p, sizeof(int64_t) * (size_t)(nrows_e + 1), cudaMemcpyDeviceToDevice, st);
+            if (tot) {
+              cudaMemcpyAsync(d_stg_col[stg_cur].as<int>() + (q_off - stg_e0), d_qcol[ob].p, sizeof(int) * (size_t)tot, cudaMemcpyDeviceToDevice, st);
+              cudaMemcpyAsync(d_stg_wt[stg_cur].as<u32>() + (q_off - stg_e0), d_qwt[ob].p, sizeof(u32) * (size_t)tot, cudaMemcpyDeviceToDevice, st);
+            }
+            stg_rows += nrows_e;
+            stg_e1 = q_off + tot;
+            while (fuse && !rc && stg_e1 - stg_e0 >= max_batch_edges && b_hi < K) rc = form_piece(stg_e0 + max_batch_edges, false);
+            if (rc) break;
+          }
         }
         q_off += tot;
         emitted_blocks = b_hi;
       }
+    }
+    if (fuse && !rc && emitted_blocks == K) {  // everything is staged: the last greedy batches
+      while (fuse && !rc && stg_rows > 0) {
+        const bool last = stg_e1 - stg_e0 <= max_batch_edges;
+        rc = form_piece(stg_e0 + max_batch_edges, last);
+      }
+    } else if (fuse) {
+      fuse = false;
     }
     if (!rc) rc = refine_piece();
     {
@@ -2128,12 +2271,21 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
       if (next_cuts.size() == 1) next_cuts.push_back(0);  // no block at all cannot happen (K >= 1); keep one batch
     } else {
       greedy_cuts(n_t, rp, max_batch_edges, next_cuts);
+      // the fused cuts are used only if they are exactly the cuts the greedy rule gives on the finished quotient
+      if (fuse && (next_cuts != next_edge_cuts || next_node_cuts.back() != K)) fuse = false;
+      {
+        int h_maxrow = 0;
+        cudaMemcpy(&h_maxrow, d_maxrow, sizeof(int), cudaMemcpyDeviceToHost);  // (every stream of the pass is idle here)
+        max_row_cur = h_maxrow;
+      }
+      if (debug) std::fprintf(stderr, "[wl_refine_batched] outer %d: %s, longest row of the quotient %lld\n", outer,
+                              fuse ? "local refinement of the next iteration done on the staged rows" : "next iteration uploads its batches for the local refinement", (long long)max_row_cur);
     }
     if ((flags & WL_FLAG_AGGRESSIVE_STOP) && (int64_t)next_cuts.size() - 1 >= nb) {  // L328
       break;
     }
     cuts.swap(next_cuts);
-    if (inherit) {
+    if (inherit || fuse) {
       node_cuts.swap(next_node_cuts);
       next_base_id = base_next;
       if (d_Hnext_keep.p) cudaFree(d_Hnext_keep.p);
@@ -2191,8 +2343,9 @@ static double batched_budget(int64_t n, int64_t m, int64_t mb, size_t cap, bool 
   while (slots < 2.0 * (double)mb) slots *= 2;
   const double rows = m > 0 ? (double)n * (double)mb / (double)m + 1 : (double)n;
   // per node: block map + representative flag; the composed map unless it stays on the host; the next block map (inherit)
-  const double per_node = 5.0 + ((size_t)n * 32 > cap ? 0.25 : 4.0) + (inherit ? 4.0 : 0.0);
-  return per_node * (double)n + 32.0 * (double)mb + 16.0 * slots + 100.0 * rows + (double)(1 << 20);
+  // (the default mode refines the next iteration's batches on staged quotient rows: next block map + two staging buffers)
+  const double per_node = 5.0 + ((size_t)n * 32 > cap ? 0.25 : 4.0) + 5.0;
+  return per_node * (double)n + (inherit ? 32.0 : 64.0) * (double)mb + 16.0 * slots + (inherit ? 100.0 : 300.0) * rows + (double)(1 << 20);
 }
 
 extern "C" {

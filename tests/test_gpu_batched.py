@@ -96,6 +96,11 @@ def test_batched_equals_cpu_algorithm2_and_invariants(name, nb):
     got = res.colors.numpy()
     # bit-exact against the CPU Algorithm 2 that uses the deterministic oracle as RSC on the same edge partition
     assert got.tolist() == want.tolist()
+    # the same with every batch uploaded again for its local refinement (no refinement on the staged quotient rows)
+    res_nf = wl.wl_refine_batched(n, g.row_ptr, g.col, g.weights, max_batch_edges=cap, seed=nb, flags=wl.WL_FLAG_NO_FUSED_RECUT)
+    assert res_nf.colors.numpy().tolist() == want.tolist() and res_nf.stats["outer_iters"] == res.stats["outer_iters"]
+    if res.stats["outer_iters"] >= 3 and name != "hub":  # (hub: a row longer than a batch, no fusion)
+        assert res.stats["bytes_h2d"] < res_nf.stats["bytes_h2d"]  # one upload pass per later iteration instead of two
     assert res.num_colors == k_want
     assert res.stats["outer_iters"] == outer_want and res.stats["last_num_batches"] == nbl_want
     # Theorem 2 (L163), refinement of the coarsest colouring (L165), case (i) (L208)
