@@ -2343,9 +2343,14 @@ static double batched_budget(int64_t n, int64_t m, int64_t mb, size_t cap, bool 
   while (slots < 2.0 * (double)mb) slots *= 2;
   const double rows = m > 0 ? (double)n * (double)mb / (double)m + 1 : (double)n;
   // per node: block map + representative flag; the composed map unless it stays on the host; the next block map (inherit)
-  // (the default mode refines the next iteration's batches on staged quotient rows: next block map + two staging buffers)
-  const double per_node = 5.0 + ((size_t)n * 32 > cap ? 0.25 : 4.0) + 5.0;
-  return per_node * (double)n + (inherit ? 32.0 : 64.0) * (double)mb + 16.0 * slots + (inherit ? 100.0 : 300.0) * rows + (double)(1 << 20);
+  // The default mode can refine the next iteration's batches on staged quotient rows (next block map + two staging buffers:
+  // one upload pass per iteration).  That is budgeted for only while the extra per-node array is small against the cap: at
+  // configs[4] (n = 2^30 under 16 GB) it would take a third of the cap from the batches, M_b would drop fourfold, and the finer
+  // batching costs more colours and iterations than the saved uploads buy (measured: 516 batches, 7 iterations, 28.1 s
+  // against 136 batches, 6 iterations, 27-28 s).  Without the budget the staging simply does not fit and the pass uploads twice.
+  const bool fused = !inherit && 5.0 * (double)n < 0.1 * (double)cap;
+  const double per_node = 5.0 + ((size_t)n * 32 > cap ? 0.25 : 4.0) + (inherit ? 4.0 : 0.0) + (fused ? 5.0 : 0.0);
+  return per_node * (double)n + (fused ? 64.0 : 32.0) * (double)mb + 16.0 * slots + (fused ? 300.0 : 100.0) * rows + (double)(1 << 20);
 }
 
 extern "C" {
