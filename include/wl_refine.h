@@ -203,6 +203,27 @@ int wl_relabel(int64_t n, const int32_t* colors, int64_t k, const uint64_t* y, i
 int wl_canonicalize(int64_t n, const int32_t* colors, int32_t* out, int64_t* num_colors, void* workspace,
                     size_t workspace_bytes, void* cuda_stream);
 
+/* S6 for callers that cannot allocate (code under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc):
+ * the same renumbering as wl_canonicalize, by the same kernels, with their scratch in a fixed file-scope device array of the
+ * library instead of a caller workspace.  The call allocates nothing (no cudaMalloc / cudaFree / cudaHostAlloc, no allocating
+ * library routine), copies nothing to the host and never synchronises: it only enqueues its kernels on cuda_stream and returns.
+ *   n          at most WL_STATIC_MAX_NODES; a larger n returns WL_ERANGE with nothing enqueued (use wl_canonicalize).
+ *   colors     DEVICE int32[n], ids in [0, n); out: DEVICE int32[n], may alias colors.
+ *   num_colors DEVICE int64* (8-byte aligned; NOT host memory, unlike wl_canonicalize's) receiving the number of distinct
+ *              colours when the stream reaches the end of the call, or NULL.  n == 0 writes nothing.
+ * The array (about 8.2 MiB: two int32 per node of the maximum, plus the scan words) is held by every GPU that loads the library
+ * until the process exits.  EVERY call on a device shares it and it keeps the last call's contents; each call rewrites all it
+ * reads, so calls one after another (same stream, or ordered by events) are independent, but two calls that OVERLAP on one
+ * GPU (different streams, or different host threads on unordered streams) race on it and both results are undefined.  The
+ * device of cuda_stream must be the current device: the array's address is looked up for the current device on the first call
+ * there (cudaGetSymbolAddress; make that first call outside any stream capture).
+ * Returns WL_OK once everything is enqueued; WL_EINVAL (negative n, null colors / out), WL_ERANGE (n above the maximum),
+ * WL_ECUDA (symbol lookup or launch failure, see wl_last_cuda_error).  Errors of the kernels themselves surface at the caller's
+ * next synchronisation of the stream. */
+#define WL_STATIC_MAX_NODES 1048576
+int wl_canonicalize_static(int64_t n, const int32_t* colors, int32_t* out, int64_t* num_colors, void* cuda_stream);
+int64_t wl_canonicalize_static_max_nodes(void); /* = WL_STATIC_MAX_NODES of the library that is loaded */
+
 /* ------------------------------------------------------------------------------------------------------------------
  * Batched: Algorithm 2 (RBSC), L169-L202, over HOST-resident edge batches.
  * ---------------------------------------------------------------------------------------------------------------- */

@@ -32,7 +32,7 @@ WL_FLAG_TEST_SMALL_OVERFLOW = 1 << 29
 
 EXPORTS = [
     "wl_refine_workspace_bytes", "wl_refine_deep_workspace_bytes", "wl_refine_host_device_bytes", "wl_refine", "wl_refine_host", "wl_round_key", "wl_weight", "wl_spmv_round",
-    "wl_spmv_rows", "wl_relabel", "wl_canonicalize", "wl_refine_batched", "wl_refine_batched_host_bytes", "wl_refine_batched_host_bytes_consume", "wl_inner_labels", "wl_quotient",
+    "wl_spmv_rows", "wl_relabel", "wl_canonicalize", "wl_canonicalize_static", "wl_canonicalize_static_max_nodes", "wl_refine_batched", "wl_refine_batched_host_bytes", "wl_refine_batched_host_bytes_consume", "wl_inner_labels", "wl_quotient",
     "wl_quotient_workspace_bytes", "wl_refine_inner", "wl_refine_inner_workspace_bytes", "wl_quotient_rows",
     "wl_quotient_rows_workspace_bytes", "wl_strerror", "wl_last_cuda_error", "wl_version", "wl_kernel_launches",
 ]
@@ -108,6 +108,10 @@ def lib():
         L.wl_relabel.argtypes = [i64, vp, i64, vp, vp, C.POINTER(i64), vp, sz, vp]
         L.wl_canonicalize.restype = C.c_int
         L.wl_canonicalize.argtypes = [i64, vp, vp, C.POINTER(i64), vp, sz, vp]
+        L.wl_canonicalize_static.restype = C.c_int
+        L.wl_canonicalize_static.argtypes = [i64, vp, vp, vp, vp]
+        L.wl_canonicalize_static_max_nodes.restype = i64
+        L.wl_canonicalize_static_max_nodes.argtypes = []
         L.wl_refine_batched.restype = C.c_int
         L.wl_refine_batched.argtypes = [i64, i32, C.POINTER(wl_edge_batch), C.POINTER(wl_csr), u64, sz, i64, vp,
                                         C.POINTER(wl_stats), C.POINTER(wl_options), vp]
@@ -342,6 +346,34 @@ def wl_canonicalize(colors: torch.Tensor, *, workspace=None):
     if rc != WL_OK:
         raise WlError(rc, "wl_canonicalize")
     return out, kk.value
+
+
+def wl_canonicalize_static_max_nodes() -> int:
+    """Largest n wl_canonicalize_static takes (the size its fixed device scratch was built for)."""
+    return int(lib().wl_canonicalize_static_max_nodes())
+
+
+def wl_canonicalize_static(colors: torch.Tensor, out: torch.Tensor, num_colors: torch.Tensor = None) -> None:
+    """S6 with no allocation anywhere (library or binding): the caller owns `out` (int32[n], may be `colors`) and
+    `num_colors` (int64[1] on the same device, or None).  Only enqueues on the current stream of the tensors' device and
+    returns; results are valid once that stream gets there.  n above wl_canonicalize_static_max_nodes() raises
+    WlError(WL_ERANGE).  Calls that overlap on one GPU race on the shared scratch (include/wl_refine.h)."""
+    L = lib()
+    n = colors.numel()
+    dev = colors.device
+    _check(colors, torch.int32, "cuda", "colors")
+    _check(out, torch.int32, "cuda", "out")
+    if out.numel() != n or out.device != dev:
+        raise ValueError("out must have the shape and device of colors")
+    if num_colors is not None:
+        _check(num_colors, torch.int64, "cuda", "num_colors")
+        if num_colors.numel() < 1 or num_colors.device != dev:
+            raise ValueError("num_colors must be an int64 tensor on the device of colors")
+    with torch.cuda.device(dev):
+        rc = L.wl_canonicalize_static(n, _ptr(colors), _ptr(out), _ptr(num_colors) if num_colors is not None else None,
+                                      _stream_ptr(dev))
+    if rc != WL_OK:
+        raise WlError(rc, "wl_canonicalize_static")
 
 
 def wl_inner_labels(n: int, row_ptr: torch.Tensor, edge_batch: torch.Tensor, sink_batch: torch.Tensor) -> torch.Tensor:

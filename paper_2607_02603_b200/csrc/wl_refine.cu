@@ -1344,3 +1344,76 @@ int64_t wl_kernel_launches(void) { return g_launches; }
 const char* wl_version(void) { return "wl_refine 0.2 (sm_100a)"; }
 
 }  // extern "C"
+
+// ---------------------------------------------------------------------------------------------------------------------
+// S6 without any allocation: wl_canonicalize_static (include/wl_refine.h).  The scratch of the S6 kernels (first node per
+// colour, canonical id per colour, chunk sums + first-node bits, the colour count) lives in ONE file-scope device array of
+// fixed size; every GPU that loads the library holds it until the process exits.  In host code `g_static_scratch` is only the
+// host-side stand-in of the symbol: the address the kernels get is the one cudaGetSymbolAddress returns for the CURRENT
+// device, looked up once per device below.
+// ---------------------------------------------------------------------------------------------------------------------
+#include <atomic>
+
+namespace wl {
+
+constexpr int64_t kStaticMaxNodes = WL_STATIC_MAX_NODES;
+constexpr size_t kStaticFirstOff = 0;                                                        // int[kStaticMaxNodes]
+constexpr size_t kStaticCidOff = kStaticFirstOff + sizeof(int) * (size_t)kStaticMaxNodes;    // int[kStaticMaxNodes]
+constexpr size_t kStaticScanInts =
+    (size_t)((kStaticMaxNodes + kCanonChunk - 1) / kCanonChunk) * (1 + kCanonChunk / 32) + 1;  // = canon_scratch_ints(max)
+constexpr size_t kStaticBsumOff = kStaticCidOff + sizeof(int) * (size_t)kStaticMaxNodes;     // int[kStaticScanInts]
+constexpr size_t kStaticTotalOff = (kStaticBsumOff + sizeof(int) * kStaticScanInts + 255) / 256 * 256;  // u64
+constexpr size_t kStaticBytes = kStaticTotalOff + 256;
+static_assert(kStaticCidOff % 256 == 0 && kStaticBsumOff % 256 == 0, "every part of the scratch stays 256-byte aligned");
+
+static __device__ __align__(256) unsigned char g_static_scratch[kStaticBytes];
+
+constexpr int kStaticMaxDevices = 64;
+static std::atomic<unsigned char*> g_static_ptr[kStaticMaxDevices];  // device address of g_static_scratch, per device
+
+// device address of the scratch on the current device (nullptr + WL_ECUDA on failure); no allocation, no synchronisation
+static int static_scratch(unsigned char** out) {
+  int dev = -1;
+  int rc = check_cuda(cudaGetDevice(&dev));
+  if (rc) return rc;
+  if (dev < 0 || dev >= kStaticMaxDevices) return WL_ERANGE;
+  unsigned char* p = g_static_ptr[dev].load(std::memory_order_acquire);
+  if (!p) {
+    void* sym = nullptr;
+    rc = check_cuda(cudaGetSymbolAddress(&sym, g_static_scratch));
+    if (rc) return rc;
+    if (!sym) return WL_ECUDA;
+    p = (unsigned char*)sym;
+    g_static_ptr[dev].store(p, std::memory_order_release);  // two threads racing here store the same address
+  }
+  *out = p;
+  return WL_OK;
+}
+
+}  // namespace wl
+
+extern "C" {
+
+int64_t wl_canonicalize_static_max_nodes(void) { return kStaticMaxNodes; }
+
+int wl_canonicalize_static(int64_t n, const int32_t* colors, int32_t* out, int64_t* num_colors, void* cuda_stream) {
+  if (n < 0) return WL_EINVAL;
+  if (n > kStaticMaxNodes) return WL_ERANGE;  // beyond the fixed scratch: use wl_canonicalize with a workspace
+  if (n == 0) return WL_OK;                   // nothing is written, num_colors included (it is device memory)
+  if (!colors || !out) return WL_EINVAL;
+  unsigned char* s = nullptr;
+  int rc = static_scratch(&s);
+  if (rc) return rc;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  Layout L{};
+  L.nscan = (n + kCanonChunk - 1) / kCanonChunk;  // the only field launch_canonical reads
+  u64* total = num_colors ? (u64*)num_colors : (u64*)(s + kStaticTotalOff);
+  // every word of the scratch the kernels read is written earlier in this same call (first[] is filled with kNoNode, the
+  // chunk sums and bits are stored for every chunk, cid[] is read only at colours whose first node wrote it): nothing
+  // of the previous call's contents survives into the result
+  launch_canonical(L, n, colors, out, (int*)(s + kStaticFirstOff), (int*)(s + kStaticCidOff), (int*)(s + kStaticBsumOff),
+                   total, st);
+  return check_cuda(cudaGetLastError());
+}
+
+}  // extern "C"
