@@ -38,6 +38,8 @@ def lib():
         L.oracle_quotient.argtypes = [i64, pi64, pi32, pu32, pi32, i64, pi64, pi32, pu32]
         L.oracle_rbsc.restype = i64
         L.oracle_rbsc.argtypes = [i64, pi64, pi32, pu32, i64, i32, pi64, pi32, i32, i32, i32, pi32, pi64]
+        L.oracle_rbsc_init.restype = i64
+        L.oracle_rbsc_init.argtypes = [i64, pi64, pi32, pu32, pi32, i64, i32, pi64, pi32, i32, i32, i32, pi32, pi64]
         L.oracle_round_key.restype = u64
         L.oracle_round_key.argtypes = [u64, u64, u64]
         L.oracle_weight.restype = u64
@@ -110,19 +112,21 @@ def quotient(n, row_ptr, col, wt, colors):
 
 
 def rbsc(n, row_ptr, col, wt, max_batch_edges, first_cuts=None, first_edge_batch=None, num_first_batches=0,
-         max_outer=1 << 30, inherit=False, aggressive=False):
+         max_outer=1 << 30, inherit=False, aggressive=False, init=None):
     """Algorithm 2 with the deterministic oracle as RSC.  -> (colors, k, outer_iters, last_num_batches).
     inherit: the quotient keeps the batches of its graph instead of being re-cut by max_batch_edges (reading Q14b).
-    aggressive: stop as soon as the next iteration would not run with fewer batches."""
+    aggressive: stop as soon as the next iteration would not run with fewer batches.
+    init: initial classes (reading Q18): Eq. 3's local start intersected with them."""
     rp, ci, w = _csr(n, row_ptr, col, wt)
     fc = None if first_cuts is None else np.ascontiguousarray(first_cuts, dtype=np.int64)
     fb = None if first_edge_batch is None else np.ascontiguousarray(first_edge_batch, dtype=np.int32)
     nb0 = num_first_batches if fb is not None else (0 if fc is None else fc.size - 1)
     out = np.empty(n, dtype=np.int32)
     stats = np.zeros(2, dtype=np.int64)
-    k = lib().oracle_rbsc(n, _p(rp, C.c_int64), _p(ci, C.c_int32), _p(w, C.c_uint32), max_batch_edges, nb0,
-                          _p(fc, C.c_int64), _p(fb, C.c_int32), max_outer, 1 if inherit else 0, 1 if aggressive else 0,
-                          _p(out, C.c_int32), _p(stats, C.c_int64))
+    ini = None if init is None else np.ascontiguousarray(init, dtype=np.int32)
+    k = lib().oracle_rbsc_init(n, _p(rp, C.c_int64), _p(ci, C.c_int32), _p(w, C.c_uint32), _p(ini, C.c_int32), max_batch_edges,
+                               nb0, _p(fc, C.c_int64), _p(fb, C.c_int32), max_outer, 1 if inherit else 0,
+                               1 if aggressive else 0, _p(out, C.c_int32), _p(stats, C.c_int64))
     return out, int(k), int(stats[0]), int(stats[1])
 
 

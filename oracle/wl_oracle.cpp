@@ -20,6 +20,8 @@
 //   oracle_rbsc          Algorithm 2 (L169-L202) with oracle_refine in place of RSC.     PINNED (Thm 2 invariants,
 //                        N_b = 1 equality, order independence; the L328 stop rule: equals the plain loop cut after the
 //                        iteration a Python restatement of the rule names)
+//   oracle_rbsc_init     the same from initial classes (reading Q18: Eq. 3 intersected with them). PINNED (stable, refines
+//                        the classes and oracle_refine(init), equals it on one batch, naming independence, hand cases)
 //   oracle_weight        the keyed bijection w = P_key(colour) that DESIGN.md §"Readings" Q4/Q5 fixes in place of
 //                        the paper's unseeded xoshiro/SplitMix recipe (L467-L473).  Bit stream: PARITY UNPINNED
 //                        (the paper prints no test vectors); bijectivity and constants are pinned.
@@ -232,10 +234,16 @@ static void greedy_cuts(i64 n, const i64* rp, i64 cap, std::vector<i64>& cuts) {
 // batches in the next iteration would not decrease": after the quotient of an iteration that ran with N_b batches has been
 // built, the edge partition of the next iteration is made as usual; if it has >= N_b batches the loop ends with the
 // colouring reached so far (every outer iteration ends on a stable colouring, Thm 2 / L206).
-i64 oracle_rbsc(i64 n0, const i64* row_ptr0, const i32* col0, const u32* wt0, i64 max_batch_edges,
-                i32 nb0, const i64* first_cuts, const i32* first_edge_batch, i32 max_outer, i32 inherit, i32 aggressive,
-                i32* out, i64* stats) {
+// init0 != NULL (reading Q18; optional extension): Algorithm 2 has no initial partition (L171), Algorithm 1
+// has (L94).  With init classes the local start of batch k is Eq. 3's partition intersected with them: the inner nodes of batch k
+// are grouped by their class, every other node stays a singleton (L151).  A node of a quotient graph (a block, Def. 4) carries the
+// class of its nodes: every H_k refines its start, so a block never spans two classes.  Everything else is Algorithm 2 as written.
+i64 oracle_rbsc_init(i64 n0, const i64* row_ptr0, const i32* col0, const u32* wt0, const i32* init0, i64 max_batch_edges,
+                     i32 nb0, const i64* first_cuts, const i32* first_edge_batch, i32 max_outer, i32 inherit, i32 aggressive,
+                     i32* out, i64* stats) {
   i64 n = n0;
+  std::vector<i32> cls(n0, 0);  // class of every node of the current graph, dense ids (first occurrence)
+  if (init0) canonical(n0, init0, cls.data());
   std::vector<i64> rp(row_ptr0, row_ptr0 + n0 + 1);
   std::vector<i32> col(col0, col0 + rp[n0]);
   std::vector<u32> wt(rp[n0]);
@@ -301,8 +309,9 @@ i64 oracle_rbsc(i64 n0, const i64* row_ptr0, const i32* col0, const u32* wt0, i6
         brp[i + 1] = (i64)bcol.size();
       }
       // H_k^0: inner nodes of k share one block, everyone else is a singleton (Eq. 3)
+      // (with init classes, Q18: inner nodes keep their class id c < n, node i outside V_k is the singleton n + i)
       std::vector<i32> init(n), loc(n);
-      for (i64 i = 0; i < n; ++i) init[i] = (label[i] == k) ? 0 : (i32)(i + 1);
+      for (i64 i = 0; i < n; ++i) init[i] = (label[i] == k) ? cls[i] : (i32)(n + i);
       i32 rounds;
       i64 kk = oracle_refine(n, brp.data(), bcol.data(), bwt.data(), init.data(), loc.data(), (i32)(n + 2), nullptr, &rounds);
       (void)kk;
@@ -325,6 +334,12 @@ i64 oracle_rbsc(i64 n0, const i64* row_ptr0, const i32* col0, const u32* wt0, i6
     std::vector<u32> qwt(m > 0 ? m : 1);
     i64 qm = oracle_quotient(n, rp.data(), col.data(), wt.data(), Hc.data(), k, qrp.data(), qcol.data(), qwt.data());
     for (i64 i = 0; i < n0; ++i) map[i] = Hc[map[i]];
+    {  // class of a block = class of its first node (canonical ids are numbered by first node)
+      std::vector<i32> next_cls;
+      for (i64 i = 0; i < n; ++i)
+        if ((i64)Hc[i] == (i64)next_cls.size()) next_cls.push_back(cls[i]);
+      cls.swap(next_cls);
+    }
     if (inherit && !cuts.empty()) {
       // batch j of the quotient: blocks whose first node lies before done_nodes(j) = the nodes whose row is complete after
       // batch j (all nodes after the last batch), minus the blocks of earlier batches; batches without blocks disappear
@@ -371,6 +386,13 @@ i64 oracle_rbsc(i64 n0, const i64* row_ptr0, const i32* col0, const u32* wt0, i6
     stats[1] = nb_last;
   }
   return canonical(n0, map.data(), out);
+}
+
+i64 oracle_rbsc(i64 n0, const i64* row_ptr0, const i32* col0, const u32* wt0, i64 max_batch_edges,
+                i32 nb0, const i64* first_cuts, const i32* first_edge_batch, i32 max_outer, i32 inherit, i32 aggressive,
+                i32* out, i64* stats) {
+  return oracle_rbsc_init(n0, row_ptr0, col0, wt0, nullptr, max_batch_edges, nb0, first_cuts, first_edge_batch, max_outer, inherit,
+                          aggressive, out, stats);
 }
 
 // ---------------------------------------------------------------------------------

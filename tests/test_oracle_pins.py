@@ -368,6 +368,66 @@ def test_rbsc_twin_leaves_merge_only_if_same_batch():
     assert k == 3 and outer == 1  # |V| unchanged after the first contraction: fixed point (L209), finer than coarsest
 
 
+@pytest.mark.parametrize("seed", range(12))
+def test_rbsc_with_init_classes_invariants(seed):
+    """Reading Q18 (Algorithm 2 from initial classes, L94 + Eq. 3): the result is a stable colouring (Thm 2) that refines the
+    classes, is refined by nothing coarser than the coarsest stable colouring refining them (computed by oracle.refine with the
+    same init, itself pinned by brute force), equals it when the loop ends on one batch (case (i), L208), does not depend on how
+    the classes are named, and with one class is Algorithm 2 as written."""
+    g = gg.rmat(6 + seed % 2, edge_factor=3, seed=seed, symmetrize=bool(seed % 2)) if seed < 8 else \
+        gg.random_weighted_digraph(60, 240, seed, max_w=3)
+    n, rp, ci, wt = _np(g)
+    A = dense_adj(n, rp, ci, wt)
+    init = gg.random_partition(n, 2 + seed % 4, seed).numpy()
+    coarsest, _, _ = oracle.refine(n, rp, ci, wt, init)
+    plain, _, _ = oracle.refine(n, rp, ci, wt)
+    renamed = (init.max() - init) * 7 + 3  # another naming of the same classes, not dense, other order
+    eb = gg.random_edge_batches(g, 3, seed).numpy()
+    for inherit in (False, True):
+        for nb in (1, 2, 3, 5):
+            cap = -(-g.m // nb)
+            c, k, outer, nb_last = oracle.rbsc(n, rp, ci, wt, cap, inherit=inherit, init=init)
+            assert stable_dense(A, c)
+            assert refines(c, init)
+            assert refines(c, coarsest)
+            if nb_last == 1:
+                assert c.tolist() == coarsest.tolist()
+            assert oracle.rbsc(n, rp, ci, wt, cap, inherit=inherit, init=renamed)[0].tolist() == c.tolist()
+            one = oracle.rbsc(n, rp, ci, wt, cap, inherit=inherit, init=np.full(n, 5, dtype=np.int32))
+            none = oracle.rbsc(n, rp, ci, wt, cap, inherit=inherit)
+            assert (one[0].tolist(), one[1:]) == (none[0].tolist(), none[1:])
+    c, k, _, _ = oracle.rbsc(n, rp, ci, wt, -(-g.m // 3), first_edge_batch=eb, num_first_batches=3, init=init)
+    assert stable_dense(A, c) and refines(c, init) and refines(c, coarsest)
+    # the classes matter on these inputs: the coarsest colouring without them does not refine them
+    if not refines(plain, init):
+        assert not same_partition(coarsest, plain)
+    # discrete classes stay discrete
+    c, k, outer, _ = oracle.rbsc(n, rp, ci, wt, -(-g.m // 2), init=np.arange(n, dtype=np.int32))
+    assert k == n and c.tolist() == list(range(n))
+
+
+def test_rbsc_with_init_classes_hand_case():
+    """Twin leaves 0, 1 -> 2 (one batch: they merge).  Put them in different classes and they must stay apart; put node 2 alone
+    in a class and nothing changes."""
+    g = gg.from_edge_list(3, [(0, 2), (1, 2)])
+    n, rp, ci, wt = _np(g)
+    assert oracle.rbsc(n, rp, ci, None, 2)[0].tolist() == [0, 0, 1]
+    assert oracle.rbsc(n, rp, ci, None, 2, init=[0, 1, 0])[0].tolist() == [0, 1, 2]
+    assert oracle.rbsc(n, rp, ci, None, 2, init=[4, 4, 9])[0].tolist() == [0, 0, 1]
+    # two batches: apart after the first iteration either way, merged by the quotient iteration only if the classes allow it
+    g = gg.from_edge_list(4, [(0, 2), (1, 2), (3, 2)])
+    n, rp, ci, wt = _np(g)
+    assert oracle.rbsc(n, rp, ci, None, 2, init=[0, 0, 0, 0])[0].tolist() == oracle.refine(n, rp, ci)[0].tolist()
+    assert oracle.refine(n, rp, ci)[0].tolist() == [0, 0, 1, 0]
+    got = oracle.rbsc(n, rp, ci, None, 2, init=[0, 0, 0, 1])[0].tolist()  # batches {0->2, 1->2}, {3->2}; sink 2 inner to the second
+    assert got == oracle.refine(n, rp, ci, None, [0, 0, 0, 1])[0].tolist() == [0, 0, 1, 2]
+    # classes that split the only mergeable pair of the first batch: |V| unchanged after the first contraction, the loop ends
+    # (L209) on a colouring finer than the coarsest one [0, 1, 2, 0]
+    c, k, outer, _ = oracle.rbsc(n, rp, ci, None, 2, init=[0, 1, 0, 0])
+    assert c.tolist() == [0, 1, 2, 3] and outer == 1
+    assert oracle.refine(n, rp, ci, None, [0, 1, 0, 0])[0].tolist() == [0, 1, 2, 0]
+
+
 # ------------------------------------------------------------------ weights / SpMV / Algorithm 1
 def test_mix_constants_are_the_documented_ones():
     def frac_sqrt(p):
