@@ -113,6 +113,12 @@ typedef struct wl_options {
                                returning (cudaFree of the 28.6 GB a scale-27 call needs costs 9-17 ms: callers that refine
                                repeatedly pass one).  Caller-owned, contents undefined before and after.                       */
   size_t device_workspace_bytes; /* >= wl_refine_host_device_bytes(n, m, weighted, with_init); a smaller one is WL_ENOMEM      */
+  const int32_t* batched_init_colors; /* wl_refine_batched only, optional: HOST int32[n], arbitrary non-negative labels (equal label
+                               = same class), the initial partition L94 gives Algorithm 1, carried into Algorithm 2 (L171 has none;
+                               reading Q18): the local start of every batch (Eq. 3) is intersected with the classes, a block of
+                               a quotient carries the class of its nodes.  The result is a stable colouring that refines the classes,
+                               the coarsest such one whenever the loop ends with N_b = 1.  NULL: one class.  8 more bytes per node on
+                               the device.  A negative label is WL_EINVAL.                                                       */
 } wl_options;
 
 typedef struct wl_stats {

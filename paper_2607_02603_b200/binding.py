@@ -56,7 +56,8 @@ class wl_options(C.Structure):
     _fields_ = [("flags", C.c_uint32), ("max_rounds", C.c_int32), ("stream_id", C.c_uint64),
                 ("round_colors", C.c_void_p), ("round_colors_cap", C.c_int32), ("max_outer_iters", C.c_int32),
                 ("host_workspace", C.c_void_p), ("host_workspace_bytes", C.c_size_t), ("ring_bits", C.c_int32),
-                ("host_pieces", C.c_int32), ("device_workspace", C.c_void_p), ("device_workspace_bytes", C.c_size_t)]
+                ("host_pieces", C.c_int32), ("device_workspace", C.c_void_p), ("device_workspace_bytes", C.c_size_t),
+                ("batched_init_colors", C.c_void_p)]
 
 
 class wl_stats(C.Structure):
@@ -468,12 +469,13 @@ def wl_refine_batched(n: int, row_ptr: torch.Tensor, col_idx: torch.Tensor, weig
                       max_batch_edges: int = 0, cuts=None, seed: int = 0, device_cap_bytes: int = 0, flags: int = 0,
                       max_outer_iters: int = 0, out: Optional[torch.Tensor] = None, device=None,
                       allow_limit: bool = False, host_workspace: Optional[torch.Tensor] = None,
-                      coo_batches=None) -> RefineResult:
+                      coo_batches=None, init_colors: Optional[torch.Tensor] = None) -> RefineResult:
     """Algorithm 2 over a HOST-resident CSR (pinned recommended).  cuts (optional, increasing edge positions from 0 to m)
     gives the edge partition of the first outer iteration as consecutive CSR slices; otherwise the library cuts by
     max_batch_edges; max_batch_edges <= 0 (with device_cap_bytes > 0): the library derives M_b from the cap.
     coo_batches (optional): an ARBITRARY edge partition as a list of (src int32[e], col int32[e],
     weights or None) host tensors, one triple per batch; row_ptr / col_idx / weights are then ignored (pass None).
+    init_colors (optional): HOST int32[n] initial classes (wl_options.batched_init_colors, reading Q18).
     Returns canonical colours on the original nodes (host int32[n])."""
     L = lib()
     if not torch.cuda.is_available():
@@ -492,6 +494,9 @@ def wl_refine_batched(n: int, row_ptr: torch.Tensor, col_idx: torch.Tensor, weig
             raise ValueError("host_workspace must be a contiguous host uint8 tensor (pinned: the transfers then overlap)")
     opt = wl_options(flags, 0, 0, None, 0, max_outer_iters, _ptr(host_workspace),
                      0 if host_workspace is None else host_workspace.numel())
+    if init_colors is not None:
+        _check(init_colors, torch.int32, "cpu", "init_colors", n)
+        opt.batched_init_colors = init_colors.data_ptr()
     st = wl_stats()
     nb = 0
     batches = None

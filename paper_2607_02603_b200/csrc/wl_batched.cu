@@ -219,6 +219,18 @@ __global__ void window_carry_kernel(int* __restrict__ cnt, int64_t len, int* __r
   else cnt[0] = *carry;
 }
 
+// initial classes (wl_options.batched_init_colors, reading Q18): the class of a block is the class of its nodes (every local
+// colouring refines its start, so all writers of one entry store the same value)
+__global__ void class_of_blocks_kernel(int64_t n, const int* __restrict__ block_of, const int* __restrict__ cls, int* __restrict__ cls_next) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) cls_next[block_of[i]] = cls[i];
+}
+// classes of the gathered rows of a COO batch: local node t is node order[t]
+__global__ void gather_class_kernel(int64_t nl, const int* __restrict__ order, const int* __restrict__ cls, int* __restrict__ out) {
+  int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t < nl) out[t] = cls[order[t]];
+}
+
 __global__ void compose_kernel(int64_t n0, int* __restrict__ map0, const int* __restrict__ Hc) {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i < n0) map0[i] = Hc[map0[i]];
@@ -1094,7 +1106,8 @@ struct CooStats {
 
 static int coo_first_iteration(int64_t n, int nb, const wl_edge_batch* batches, int64_t m_total, uint64_t seed, uint32_t flags,
                                const wl_options* opt, size_t cap, size_t* used_persistent, DevBuf& d_map0, HostQuot& hq,
-                               bool build_quotient, cudaStream_t st, cudaStream_t copy_st, cudaStream_t down_st, CooStats* out) {
+                               bool build_quotient, cudaStream_t st, cudaStream_t copy_st, cudaStream_t down_st, CooStats* out,
+                               const int* d_cls = nullptr) {  // d_cls: DEVICE int32[n] initial classes or NULL
   bool weighted = false;
   for (int k = 0; k < nb; ++k) weighted |= batches[k].num_edges > 0 && batches[k].weights != nullptr;
   int64_t max_e = 1;
@@ -1247,6 +1260,8 @@ static int coo_first_iteration(int64_t n, int nb, const wl_edge_batch* batches, 
   COO_ALLOC(d_lcol, sizeof(int) * (size_t)max_el);
   if (weighted) COO_ALLOC(d_lwt, sizeof(u32) * (size_t)max_el);
   COO_ALLOC(d_sbsum, sizeof(u64) * (size_t)(max_nl / kScanC + 3));
+  DevBuf d_lcls;
+  if (d_cls) COO_ALLOC(d_lcls, sizeof(int) * (size_t)max_nl);
   if (rc) return rc;
   int64_t base_id = 0;
   rc = stream_batches(all, [&](int k, int buf) -> int {
@@ -1271,7 +1286,8 @@ static int coo_first_iteration(int64_t n, int nb, const wl_edge_batch* batches, 
     lo.stream_id = (1ull << 32) | (u64)(u32)k;
     const Layout L = make_layout(nl, el);
     CoreResult cr{};
-    const int prc = refine_core(&lg, nullptr, seed, &lo, /*ranged=*/true, 0, (int)nl, n, 0, d_ws.p, L.bytes, L, st, &cr);
+    if (d_cls) { ++g_launches; gather_class_kernel<<<blocks_for(nl, 256), 256, 0, st>>>(nl, d_order.as<int>() + off[k], d_cls, d_lcls.as<int>()); }
+    const int prc = refine_core(&lg, d_cls ? d_lcls.as<int>() : nullptr, seed, &lo, /*ranged=*/true, 0, (int)nl, n, 0, d_ws.p, L.bytes, L, st, &cr);
     if (prc) return prc;
     ++g_launches; coo_merge_kernel<<<blocks_for(nl, 256), 256, 0, st>>>(nl, d_order.as<int>() + off[k], cr.colour, (int)base_id, d_H.as<int>());
     base_id += cr.k;
@@ -1495,6 +1511,12 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
     max_row_cur = longest;
   }
 
+  // initial classes (reading Q18): the class of every node of the CURRENT graph stays on the device (d_cls, below)
+  const int32_t* init_host = opt ? opt->batched_init_colors : nullptr;
+  if (init_host && !(flags & WL_FLAG_NO_VALIDATE))
+    for (int64_t i = 0; i < n; ++i)
+      if (init_host[i] < 0) return WL_EINVAL;
+
   u64* hs = host_scal();
   if (!hs) return WL_ECUDA;
   int dev_id = 0;
@@ -1552,6 +1574,15 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
   const bool map0_on_host = !coo && device_cap_bytes > 0 && (size_t)n0 * sizeof(int) * 8 > device_cap_bytes;
   HostQuot hq;  // quotient graphs of later iterations (pinned host memory)
   const int64_t rp0_edges = coo ? coo_edges : rp[n];
+  DevBuf d_cls, d_cls_next;  // initial classes of the nodes of the current graph / of its quotient (persistent: counted in `used`)
+  if (init_host) {
+    const int arc = d_cls.alloc(sizeof(int) * (size_t)n0, &used, device_cap_bytes);
+    if (arc) {
+      cleanup();
+      return arc;
+    }
+    cudaMemcpyAsync(d_cls.p, init_host, sizeof(int) * (size_t)n0, cudaMemcpyHostToDevice, st);
+  }
 
   int64_t n_t = n;
   int outer = 0;
@@ -1562,6 +1593,7 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
   const int64_t launches_at_entry = g_launches;
   int rc = WL_OK;
   bool hit_limit = false;
+  if (init_host) bytes_h2d += sizeof(int) * n0;
 
   // WL_FLAG_INHERIT_BATCHES (reading Q14b): the local refinement of the NEXT outer iteration runs on the quotient rows while
   // they are still on the device, batch = the rows emitted together; the next iteration then starts at the merge.
@@ -1587,7 +1619,7 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
     outer = 1;
     CooStats cs;
     rc = coo_first_iteration(n, num_batches, batches, coo_edges, seed, flags, opt, device_cap_bytes, &used, d_map0, hq,
-                             /*build_quotient=*/max_outer > 1, st, copy_st, down_st, &cs);
+                             /*build_quotient=*/max_outer > 1, st, copy_st, down_st, &cs, init_host ? d_cls.as<int>() : nullptr);
     edges_streamed += cs.edges_streamed;
     bytes_h2d += cs.bytes_h2d;
     bytes_d2h += cs.bytes_d2h;
@@ -1607,6 +1639,17 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
         loop_done = true;
         hit_limit = !(num_batches == 1 || cs.K == n);  // stopped by max_outer_iters only
       } else {
+        if (init_host) {  // classes of the blocks, through the composed map of iteration 1
+          rc = d_cls_next.alloc(sizeof(int) * (size_t)cs.K, &used, device_cap_bytes);
+          if (!rc) {
+            ++g_launches; class_of_blocks_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, d_map0.as<int>(), d_cls.as<int>(), d_cls_next.as<int>());
+            rc = check_cuda(cudaStreamSynchronize(st));
+          }
+          d_cls.release(&used);
+          std::swap(d_cls.p, d_cls_next.p);
+          std::swap(d_cls.bytes, d_cls_next.bytes);
+          if (rc) loop_done = true;
+        }
         rp = hq.rp[1];
         n_t = cs.K;
         weighted = true;
@@ -1771,7 +1814,7 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
       lo.stream_id = ((u64)outer << 32) | (u64)(u32)k;
       const Layout L = make_layout(nr, lg.m);
       CoreResult cr{};
-      rc = refine_core(&lg, nullptr, seed, &lo, /*ranged=*/true, (int)r0[k], (int)r1[k], n_t, e0, d_ws.p, L.bytes, L, st, &cr);
+      rc = refine_core(&lg, init_host ? d_cls.as<int>() + r0[k] : nullptr, seed, &lo, /*ranged=*/true, (int)r0[k], (int)r1[k], n_t, e0, d_ws.p, L.bytes, L, st, &cr);
       if (rc) break;
       // canonical ids inside the batch (scratch: two dead arrays of the local workspace, as wl_refine does), then Eq. 4
       char* wsb = (char*)d_ws.p;
@@ -1862,6 +1905,11 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
       break;
     }
 
+    if (init_host) {  // classes of the K blocks = of the nodes of the quotient (ready before the first piece is refined)
+      if ((rc = d_cls_next.alloc(sizeof(int) * (size_t)K, &used, device_cap_bytes))) break;
+      used_iter += d_cls_next.bytes;
+      ++g_launches; class_of_blocks_kernel<<<blocks_for(n_t, 256), 256, 0, st>>>(n_t, d_Hc.as<int>(), d_cls.as<int>(), d_cls_next.as<int>());
+    }
     // the local workspace is dead: its bytes go to the quotient pass
     cudaStreamSynchronize(st);
     d_ws.release(&used_iter);
@@ -2041,7 +2089,7 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
       lo.stream_id = ((u64)(outer + 1) << 32) | (u64)(u32)pending.index;
       const Layout L2 = make_layout(nr, pending.tot);
       CoreResult cr{};
-      int prc = refine_core(&lg, nullptr, seed, &lo, /*ranged=*/true, (int)pending.b_lo, (int)pending.b_hi, K, pending.q_off,
+      int prc = refine_core(&lg, init_host ? d_cls_next.as<int>() + pending.b_lo : nullptr, seed, &lo, /*ranged=*/true, (int)pending.b_lo, (int)pending.b_hi, K, pending.q_off,
                             d_ws2.p, L2.bytes, L2, side_st, &cr);
       if (prc) return prc;
       char* wsb = (char*)d_ws2.p;
@@ -2265,6 +2313,11 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
     rp = nrp;
     n_t = K;
     weighted = true;
+    if (init_host) {  // the quotient becomes the current graph
+      d_cls.release(&used);
+      std::swap(d_cls.p, d_cls_next.p);
+      std::swap(d_cls.bytes, d_cls_next.bytes);
+    }
     std::vector<int64_t> next_cuts;
     if (inherit) {
       next_cuts = next_edge_cuts;
@@ -2338,7 +2391,7 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
 
 // Rough device budget of batched_run for a batch cap M_b (DESIGN.md §8 "Device budget"): node arrays, two input and two
 // output buffers of 8 bytes per edge, the quotient table, the local workspace of a batch with its share of the rows.
-static double batched_budget(int64_t n, int64_t m, int64_t mb, size_t cap, bool inherit) {
+static double batched_budget(int64_t n, int64_t m, int64_t mb, size_t cap, bool inherit, bool with_init) {
   double slots = 1024;
   while (slots < 2.0 * (double)mb) slots *= 2;
   const double rows = m > 0 ? (double)n * (double)mb / (double)m + 1 : (double)n;
@@ -2349,7 +2402,8 @@ static double batched_budget(int64_t n, int64_t m, int64_t mb, size_t cap, bool 
   // batching costs more colours and iterations than the saved uploads buy (measured: 516 batches, 7 iterations, 28.1 s
   // against 136 batches, 6 iterations, 27-28 s).  Without the budget the staging simply does not fit and the pass uploads twice.
   const bool fused = !inherit && 5.0 * (double)n < 0.1 * (double)cap;
-  const double per_node = 5.0 + ((size_t)n * 32 > cap ? 0.25 : 4.0) + (inherit ? 4.0 : 0.0) + (fused ? 5.0 : 0.0);
+  const double per_node = 5.0 + ((size_t)n * 32 > cap ? 0.25 : 4.0) + (inherit ? 4.0 : 0.0) + (fused ? 5.0 : 0.0) +
+                          (with_init ? 8.0 : 0.0);  // initial classes of the current graph and of its quotient
   return per_node * (double)n + (fused ? 64.0 : 32.0) * (double)mb + 16.0 * slots + (fused ? 300.0 : 100.0) * rows + (double)(1 << 20);
 }
 
@@ -2377,7 +2431,7 @@ int wl_refine_batched(int64_t n, int32_t num_batches, const wl_edge_batch* batch
   const int64_t m = whole->m;
   int64_t mb = m > 0 ? m : 1;
   const bool inh = opt && (opt->flags & WL_FLAG_INHERIT_BATCHES);
-  while (mb > 1024 && batched_budget(n, m, mb, device_cap_bytes, inh) > 0.9 * (double)device_cap_bytes) mb = (int64_t)((double)mb * 0.8);
+  while (mb > 1024 && batched_budget(n, m, mb, device_cap_bytes, inh, opt && opt->batched_init_colors) > 0.9 * (double)device_cap_bytes) mb = (int64_t)((double)mb * 0.8);
   for (int attempt = 0; attempt < 12; ++attempt) {
     const int rc = run(mb);
     if (rc != WL_ENOMEM || mb <= 1024 || g_input_consumed) return rc;  // a consumed input cannot be read a second time

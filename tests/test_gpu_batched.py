@@ -200,6 +200,92 @@ def test_batched_coo_partitions_equal_cpu_algorithm2(name, nb, part):
     assert res2.colors.numpy().tolist() == want2.tolist()
 
 
+# ------------------------------------------------------------------ initial classes (L94 carried into Algorithm 2, reading Q18)
+@pytest.mark.parametrize("name", list(BATCH_GRAPHS))
+@pytest.mark.parametrize("nb", [1, 2, 4, 16])
+@pytest.mark.parametrize("classes", [2, 5])
+def test_batched_with_initial_classes_equals_cpu_algorithm2(name, nb, classes):
+    """wl_options.batched_init_colors in every mode of the CSR forms (fused re-cut, uploads twice, inherited batches, aggressive
+    stop): bit-exact against the CPU Algorithm 2 started from the same classes; the result is stable (Thm 2), refines the
+    classes and the coarsest stable colouring refining them, and equals it when the loop ends on one batch (L208)."""
+    g = BATCH_GRAPHS[name]()
+    n, rp, ci, wt = g.numpy()
+    cap = max(1, -(-g.m // nb))
+    init = gg.random_partition(n, classes, 100 + nb)
+    labels = (init * 3 + 1).to(torch.int32)  # arbitrary non-negative labels, not dense
+    coarsest, _, _ = oracle.refine(n, rp, ci, wt, init.numpy())
+    for flags, kw in [(0, {}), (wl.WL_FLAG_NO_FUSED_RECUT, {}), (wl.WL_FLAG_INHERIT_BATCHES, {"inherit": True}),
+                      (wl.WL_FLAG_AGGRESSIVE_STOP, {"aggressive": True})]:
+        want, k_want, outer_want, nbl_want = oracle.rbsc(n, rp, ci, wt, cap, init=init.numpy(), **kw)
+        res = wl.wl_refine_batched(n, g.row_ptr, g.col, g.weights, max_batch_edges=cap, seed=nb, flags=flags, init_colors=labels)
+        got = res.colors.numpy()
+        assert got.tolist() == want.tolist() and res.num_colors == k_want
+        assert res.stats["outer_iters"] == outer_want and res.stats["last_num_batches"] == nbl_want
+        assert oracle.is_stable(n, rp, ci, wt, got)
+        assert refines(got, init.numpy()) and refines(got, coarsest)
+        if res.stats["last_num_batches"] == 1 and not flags & wl.WL_FLAG_AGGRESSIVE_STOP:
+            assert got.tolist() == coarsest.tolist()
+    # one class = no classes
+    one = wl.wl_refine_batched(n, g.row_ptr, g.col, g.weights, max_batch_edges=cap, seed=nb,
+                               init_colors=torch.full((n,), 9, dtype=torch.int32))
+    none = wl.wl_refine_batched(n, g.row_ptr, g.col, g.weights, max_batch_edges=cap, seed=nb)
+    assert one.colors.tolist() == none.colors.tolist() and one.stats["outer_iters"] == none.stats["outer_iters"]
+
+
+@pytest.mark.parametrize("name", ["rmat10_sym", "rmat11_dir", "weighted", "twins"])
+@pytest.mark.parametrize("nb", [2, 3])
+@pytest.mark.parametrize("part", list(COO_PARTITIONS))
+def test_batched_coo_partitions_with_initial_classes(name, nb, part):
+    g = BATCH_GRAPHS[name]()
+    n, rp, ci, wt = g.numpy()
+    eb = COO_PARTITIONS[part](g, nb, 7)
+    cap = max(1, -(-g.m // nb))
+    init = gg.random_partition(n, 3, 5)
+    coarsest, _, _ = oracle.refine(n, rp, ci, wt, init.numpy())
+    want, k_want, outer_want, nbl_want = oracle.rbsc(n, rp, ci, wt, cap, first_edge_batch=eb.numpy(), num_first_batches=nb,
+                                                     init=init.numpy())
+    res = wl.wl_refine_batched(n, None, None, None, max_batch_edges=cap, seed=nb, coo_batches=gg.coo_batches(g, eb, nb),
+                               init_colors=init.to(torch.int32))
+    got = res.colors.numpy()
+    assert got.tolist() == want.tolist() and res.num_colors == k_want
+    assert res.stats["outer_iters"] == outer_want and res.stats["last_num_batches"] == nbl_want
+    assert oracle.is_stable(n, rp, ci, wt, got) and refines(got, init.numpy()) and refines(got, coarsest)
+
+
+@pytest.mark.parametrize("flags", [0, 4096])
+def test_batched_with_initial_classes_over_several_tiles(flags):
+    """A graph whose batches span several kernel tiles and a ragged tail (n = 2^15 + 77 with isolated tail nodes)."""
+    g0 = gg.rmat(15, edge_factor=8, seed=4, symmetrize=False)
+    n = g0.n + 77
+    row_ptr = torch.cat([g0.row_ptr, g0.row_ptr[-1:].repeat(77)])
+    rp, ci = row_ptr.numpy(), g0.col.numpy()
+    init = gg.random_partition(n, 6, 11)
+    cap = -(-g0.m // 7)
+    want, k_want, outer_want, nbl_want = oracle.rbsc(n, rp, ci, None, cap, init=init.numpy(), inherit=bool(flags & 4096))
+    res = wl.wl_refine_batched(n, row_ptr, g0.col, None, max_batch_edges=cap, seed=3, flags=flags, init_colors=init)
+    assert res.colors.numpy().tolist() == want.tolist() and res.num_colors == k_want
+    assert res.stats["outer_iters"] == outer_want and res.stats["last_num_batches"] == nbl_want
+    assert oracle.is_stable(n, rp, ci, None, res.colors.numpy()) and refines(res.colors.numpy(), init.numpy())
+
+
+def test_batched_initial_classes_errors_and_limits():
+    g = gg.rmat(10, seed=3, symmetrize=False)
+    n = g.n
+    bad = torch.zeros(n, dtype=torch.int32)
+    bad[n // 2] = -1
+    with pytest.raises(wl.WlError) as e:
+        wl.wl_refine_batched(n, g.row_ptr, g.col, None, max_batch_edges=g.m // 3, init_colors=bad)
+    assert e.value.code == wl.WL_EINVAL
+    # discrete classes: nothing can merge, one outer iteration
+    res = wl.wl_refine_batched(n, g.row_ptr, g.col, None, max_batch_edges=g.m // 3, init_colors=torch.arange(n, dtype=torch.int32))
+    assert res.num_colors == n and res.colors.tolist() == list(range(n)) and res.stats["outer_iters"] == 1
+    # the classes count against the device cap (8 bytes per node): a cap that holds the run without them but not with them
+    init = gg.random_partition(n, 4, 1).to(torch.int32)
+    with pytest.raises(wl.WlError) as e:
+        wl.wl_refine_batched(n, g.row_ptr, g.col, None, max_batch_edges=g.m // 3, init_colors=init, device_cap_bytes=4 * n - 1)
+    assert e.value.code == wl.WL_ENOMEM
+
+
 def test_batched_coo_errors_and_edge_cases():
     g = gg.rmat(9, seed=2, symmetrize=False)
     n = g.n
