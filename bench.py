@@ -236,7 +236,7 @@ def run_batched(args):
         del g
     torch.cuda.empty_cache()
     gen_s = time.perf_counter() - t_gen0
-    hws_bytes = wl.wl_refine_batched_host_bytes_consume(n, m) if consume else wl.wl_refine_batched_host_bytes(n, m)
+    hws_bytes = (wl.wl_refine_batched_host_bytes_consume(n, m) + wl.wl_refine_batched_host_overflow_bytes(m)) if consume else wl.wl_refine_batched_host_bytes(n, m)
     scratch_kind = "pinned"
     try:
         hws = torch.empty(hws_bytes, dtype=torch.uint8, pin_memory=True)
@@ -248,12 +248,14 @@ def run_batched(args):
             hws_bytes / 2 ** 30, (rp.numel() * 8 + col.numel() * 4) / 2 ** 30)
     out = torch.empty(n, dtype=torch.int32, pin_memory=(scratch_kind == "pinned"))
     base_flags = args.flags | (wl.WL_FLAG_CONSUME_INPUT if consume else 0)
+    # caller-owned device arena of the cap's size (wl_options.device_workspace): the timed calls allocate nothing on the device
+    arena = None if args.no_arena else torch.empty(cap, dtype=torch.uint8, device=dev)
 
     def one(flags, seed):
         torch.cuda.synchronize(dev)
         t0 = time.perf_counter()
         r = wl.wl_refine_batched(n, rp, col, None, max_batch_edges=args.batch_edges, seed=seed, device_cap_bytes=cap,
-                                 flags=flags, host_workspace=hws, out=out)
+                                 flags=flags, host_workspace=hws, out=out, device_workspace=arena)
         torch.cuda.synchronize(dev)
         return r, time.perf_counter() - t0
 
@@ -295,6 +297,7 @@ def run_batched(args):
                                    f"({'BASELINE.json configs[4]' if args.scale == 30 else 'shape of BASELINE.json configs[4]'})",
                        "n": n, "m": m, "step": "wl_refine_batched to the batched fixed point (Algorithm 2, B1-B7)",
                        "consume_input": consume, "generation_seconds": gen_s, "host_scratch": scratch_kind,
+                       "device_arena": "none (library allocates)" if arena is None else "caller-owned, %.1f GB = the cap" % (cap / 2 ** 30),
                        "pinned_host_gb": (rp.numel() * 8 + col.numel() * 4 + hws.numel() + out.numel() * 4) / 2 ** 30},
             "seconds_to_stable_coloring": sec, "outer_iters": st["outer_iters"], "num_colors": st["num_colors"],
             "reduction_power": st["num_colors"] / n, "last_num_batches": st["last_num_batches"],
@@ -609,6 +612,7 @@ def main():
     ap.add_argument("--cap-gb", type=float, default=16.0, help="batched: device memory cap")
     ap.add_argument("--consume-input", action="store_true", help="batched: WL_FLAG_CONSUME_INPUT (forced from scale 30 on)")
     ap.add_argument("--no-inherit-leg", action="store_true", help="batched: skip the second run with WL_FLAG_INHERIT_BATCHES")
+    ap.add_argument("--no-arena", action="store_true", help="batched: let the library cudaMalloc / cudaFree its device buffers")
     ap.add_argument("--batch-edges", type=int, default=0, help="batched: M_b (0: derived by the library from the device cap)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)

@@ -108,11 +108,15 @@ typedef struct wl_options {
                                it is compared; used to COUNT collisions (Lemma 1), never for production results          */
   int32_t host_pieces;      /* wl_refine_host only: number of pieces (whole rows each) the column upload is cut into so that the
                                first pass over the columns runs behind the link; <= 0: about 256 MB per piece, at most 32     */
-  void* device_workspace;   /* wl_refine_host only, optional: DEVICE scratch (256-byte aligned) that holds the uploaded graph and
+  void* device_workspace;   /* wl_refine_host, optional: DEVICE scratch (256-byte aligned) that holds the uploaded graph and
                                the refinement workspace; NULL: the library allocates its own inside the call and frees it before
                                returning (cudaFree of the 28.6 GB a scale-27 call needs costs 9-17 ms: callers that refine
                                repeatedly pass one).  Caller-owned, contents undefined before and after.                       */
-  size_t device_workspace_bytes; /* >= wl_refine_host_device_bytes(n, m, weighted, with_init); a smaller one is WL_ENOMEM      */
+  size_t device_workspace_bytes; /* >= wl_refine_host_device_bytes(n, m, weighted, with_init); a smaller one is WL_ENOMEM.
+                               wl_refine_batched, optional: a DEVICE arena all device buffers of the call are cut from (give it
+                               device_cap_bytes, or what the graph needs when there is no cap): the call then makes no cudaMalloc /
+                               cudaFree (they cost 18 ms per outer iteration and now and then 0.4 s).  A buffer that finds no free
+                               block in it is allocated with cudaMalloc as without an arena; the cap is checked as always.       */
   const int32_t* batched_init_colors; /* wl_refine_batched only, optional: HOST int32[n], arbitrary non-negative labels (equal label
                                = same class), the initial partition L94 gives Algorithm 1, carried into Algorithm 2 (L171 has none;
                                reading Q18): the local start of every batch (Eq. 3) is intersected with the classes, a block of
@@ -273,6 +277,11 @@ int wl_refine_batched(int64_t n, int32_t num_batches, const wl_edge_batch* batch
 size_t wl_refine_batched_host_bytes(int64_t n, int64_t m);
 /* the same under WL_FLAG_CONSUME_INPUT: two offset arrays, plus one weight array of m entries unless the input is weighted */
 size_t wl_refine_batched_host_bytes_consume(int64_t n, int64_t m, int weighted);
+/* optional extra: a host workspace with this many bytes MORE than the size above also holds the overflow lists of the one-byte
+ * weights (unweighted inputs); otherwise the library pins them itself in every call (cudaHostAlloc / cudaFreeHost of some tens of
+ * megabytes: 50-800 ms per call, measured at scale 26).  wl_refine_batched_host_bytes has that room already (it counts four bytes
+ * per weight); add it to wl_refine_batched_host_bytes_consume. */
+size_t wl_refine_batched_host_overflow_bytes(int64_t m);
 
 /* B2: inner-node labels of Def. 5 (L139-L145) by the method of L463.  edge_batch: DEVICE int32[m] batch id of every CSR edge
  * slot; sink_batch: DEVICE int32[n] label given to nodes without out-edges (Q9); label: DEVICE int32[n], -1 = boundary. */

@@ -32,7 +32,7 @@ WL_FLAG_TEST_SMALL_OVERFLOW = 1 << 29
 
 EXPORTS = [
     "wl_refine_workspace_bytes", "wl_refine_deep_workspace_bytes", "wl_refine_host_device_bytes", "wl_refine", "wl_refine_host", "wl_round_key", "wl_weight", "wl_spmv_round",
-    "wl_spmv_rows", "wl_relabel", "wl_canonicalize", "wl_canonicalize_static", "wl_canonicalize_static_max_nodes", "wl_refine_batched", "wl_refine_batched_host_bytes", "wl_refine_batched_host_bytes_consume", "wl_inner_labels", "wl_quotient",
+    "wl_spmv_rows", "wl_relabel", "wl_canonicalize", "wl_canonicalize_static", "wl_canonicalize_static_max_nodes", "wl_refine_batched", "wl_refine_batched_host_bytes", "wl_refine_batched_host_bytes_consume", "wl_refine_batched_host_overflow_bytes", "wl_inner_labels", "wl_quotient",
     "wl_quotient_workspace_bytes", "wl_refine_inner", "wl_refine_inner_workspace_bytes", "wl_quotient_rows",
     "wl_quotient_rows_workspace_bytes", "wl_strerror", "wl_last_cuda_error", "wl_version", "wl_kernel_launches",
 ]
@@ -120,6 +120,8 @@ def lib():
         L.wl_refine_batched_host_bytes.argtypes = [i64, i64]
         L.wl_refine_batched_host_bytes_consume.restype = sz
         L.wl_refine_batched_host_bytes_consume.argtypes = [i64, i64, C.c_int]
+        L.wl_refine_batched_host_overflow_bytes.restype = sz
+        L.wl_refine_batched_host_overflow_bytes.argtypes = [i64]
         L.wl_inner_labels.restype = C.c_int
         L.wl_inner_labels.argtypes = [i64, vp, vp, vp, vp, vp]
         L.wl_quotient.restype = C.c_int
@@ -469,13 +471,15 @@ def wl_refine_batched(n: int, row_ptr: torch.Tensor, col_idx: torch.Tensor, weig
                       max_batch_edges: int = 0, cuts=None, seed: int = 0, device_cap_bytes: int = 0, flags: int = 0,
                       max_outer_iters: int = 0, out: Optional[torch.Tensor] = None, device=None,
                       allow_limit: bool = False, host_workspace: Optional[torch.Tensor] = None,
-                      coo_batches=None, init_colors: Optional[torch.Tensor] = None) -> RefineResult:
+                      coo_batches=None, init_colors: Optional[torch.Tensor] = None,
+                      device_workspace: Optional[torch.Tensor] = None) -> RefineResult:
     """Algorithm 2 over a HOST-resident CSR (pinned recommended).  cuts (optional, increasing edge positions from 0 to m)
     gives the edge partition of the first outer iteration as consecutive CSR slices; otherwise the library cuts by
     max_batch_edges; max_batch_edges <= 0 (with device_cap_bytes > 0): the library derives M_b from the cap.
     coo_batches (optional): an ARBITRARY edge partition as a list of (src int32[e], col int32[e],
     weights or None) host tensors, one triple per batch; row_ptr / col_idx / weights are then ignored (pass None).
     init_colors (optional): HOST int32[n] initial classes (wl_options.batched_init_colors, reading Q18).
+    device_workspace (optional): a device uint8 arena the call cuts all its device buffers from (no cudaMalloc / cudaFree).
     Returns canonical colours on the original nodes (host int32[n])."""
     L = lib()
     if not torch.cuda.is_available():
@@ -497,6 +501,10 @@ def wl_refine_batched(n: int, row_ptr: torch.Tensor, col_idx: torch.Tensor, weig
     if init_colors is not None:
         _check(init_colors, torch.int32, "cpu", "init_colors", n)
         opt.batched_init_colors = init_colors.data_ptr()
+    if device_workspace is not None:
+        _check(device_workspace, torch.uint8, "cuda", "device_workspace")
+        opt.device_workspace = device_workspace.data_ptr()
+        opt.device_workspace_bytes = device_workspace.numel()
     st = wl_stats()
     nb = 0
     batches = None
@@ -543,6 +551,10 @@ def wl_refine_batched_host_bytes(n: int, m: int) -> int:
 
 def wl_refine_batched_host_bytes_consume(n: int, m: int, weighted: bool = False) -> int:
     return int(lib().wl_refine_batched_host_bytes_consume(n, m, 1 if weighted else 0))
+
+
+def wl_refine_batched_host_overflow_bytes(m: int) -> int:
+    return int(lib().wl_refine_batched_host_overflow_bytes(m))
 
 
 def wl_strerror(code: int) -> str:

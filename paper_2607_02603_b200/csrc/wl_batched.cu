@@ -21,6 +21,7 @@
 #include <cstring>
 #include <condition_variable>
 #include <functional>
+#include <map>
 #include <mutex>
 #include <thread>
 #include <vector>
@@ -69,7 +70,11 @@ class PieceWorker {
       stop_ = true;
     }
     cv_.notify_all();
+    const auto t0 = std::chrono::steady_clock::now();
     th_.join();
+    if (debug_enabled())
+      std::fprintf(stderr, "[wl_refine_batched] helper thread joined in %9.3f ms\n",
+                   std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count());
   }
   void submit(std::function<int()> f) {  // at most one task is outstanding: wait() first
     if (!th_.joinable()) th_ = std::thread([this] { loop(); });
@@ -716,16 +721,79 @@ scan32_apply_kernel(const int* __restrict__ in, int64_t n, const u64* __restrict
 // ---------------------------------------------------------------------------------------------------------------------
 // host helpers
 // ---------------------------------------------------------------------------------------------------------------------
+// wl_options.device_workspace for wl_refine_batched: the buffers of an outer iteration are sized by that iteration and given back
+// at its end, and cudaFree / cudaMalloc of the same gigabytes once per iteration cost 18 ms each time and now and then 0.4 s
+// (measured at scale 26: the whole spread between two runs of the same call; a cudaMemPool of the call's own only moves the cost
+// to its destruction).  With a caller-owned arena the call makes no allocation at all: blocks are cut from it first-fit at
+// 256-byte granularity and merged with their free neighbours when they come back.  Without one: cudaMalloc / cudaFree.
+struct DevPool {
+  char* base = nullptr;
+  size_t size = 0;
+  std::map<size_t, size_t> free_blocks;  // offset -> bytes, disjoint, never adjacent
+  std::mutex mu;
+  void init(void* arena, size_t bytes) {
+    const size_t mis = (size_t)((uintptr_t)arena & 255u);
+    const size_t skip = mis ? 256 - mis : 0;
+    if (!arena || bytes < skip + 256) return;
+    base = (char*)arena + skip;
+    size = (bytes - skip) / 256 * 256;
+    free_blocks[0] = size;
+  }
+  void* take(size_t bytes) {
+    if (!base) return nullptr;
+    const size_t need = (bytes + 255) / 256 * 256;
+    std::lock_guard<std::mutex> lock(mu);
+    for (auto it = free_blocks.begin(); it != free_blocks.end(); ++it) {
+      if (it->second < need) continue;
+      const size_t off = it->first, rest = it->second - need;
+      free_blocks.erase(it);
+      if (rest) free_blocks[off + need] = rest;
+      return base + off;
+    }
+    return nullptr;
+  }
+  void give(void* p, size_t bytes) {
+    size_t off = (size_t)((char*)p - base), len = (bytes + 255) / 256 * 256;
+    std::lock_guard<std::mutex> lock(mu);
+    auto next = free_blocks.lower_bound(off);
+    if (next != free_blocks.end() && next->first == off + len) {
+      len += next->second;
+      next = free_blocks.erase(next);
+    }
+    if (next != free_blocks.begin()) {
+      auto prev = std::prev(next);
+      if (prev->first + prev->second == off) {
+        prev->second += len;
+        return;
+      }
+    }
+    free_blocks[off] = len;
+  }
+};
+static thread_local DevPool* g_dev_pool = nullptr;  // the arena of the call running on this thread, if any
+
 struct DevBuf {
   void* p = nullptr;
   size_t bytes = 0;
-  ~DevBuf() {
-    if (p) cudaFree(p);
+  DevPool* from = nullptr;  // where p came from (NULL: cudaMalloc)
+  ~DevBuf() { free_now(); }
+  void free_now() {
+    if (!p) return;
+    if (from) {
+      cudaDeviceSynchronize();  // what cudaFree implies: nothing on any stream still uses the block when it is handed out again
+      from->give(p, bytes);
+    } else {
+      cudaFree(p);
+    }
+    p = nullptr;
+    from = nullptr;
   }
   int alloc(size_t b, size_t* used, size_t cap) {
     bytes = b ? b : 256;
     if (cap && *used + bytes > cap) return WL_ENOMEM;
-    if (cudaMalloc(&p, bytes) != cudaSuccess) {
+    if (g_dev_pool && (p = g_dev_pool->take(bytes))) from = g_dev_pool;
+    // (no arena, or no free block of that size left in it although the bytes fit the cap)
+    if (!p && cudaMalloc(&p, bytes) != cudaSuccess) {
       cudaGetLastError();
       p = nullptr;
       return WL_ENOMEM;
@@ -735,10 +803,17 @@ struct DevBuf {
   }
   void release(size_t* used) {  // give the memory back before the end of the scope
     if (!p) return;
-    cudaFree(p);
-    p = nullptr;
+    free_now();
     if (*used >= bytes) *used -= bytes;
     bytes = 0;
+  }
+  void take(DevBuf& o) {  // becomes the owner of o's block (its own, if any, is freed)
+    free_now();
+    p = o.p;
+    bytes = o.bytes;
+    from = o.from;
+    o.p = nullptr;
+    o.from = nullptr;
   }
   template <typename T>
   T* as() const { return (T*)p; }
@@ -770,7 +845,12 @@ struct HostQuot {
     std::vector<Emission> em;
     u64* ovf = nullptr;  // {position inside the emission : 32 | weight : 32}
     size_t cap = 0, used = 0;
+    bool owned = false;  // pinned by the library (else: inside the caller's workspace)
   } gen[2];
+  char* spare = nullptr;  // what the caller's workspace holds beyond the arrays above: room for the overflow lists
+  size_t spare_bytes = 0;
+  // bytes of overflow lists a workspace should hold on top of bytes_for (two generations)
+  static size_t overflow_bytes_for(int64_t m) { return 2 * align_up(sizeof(u64) * (size_t)(m / 255 + 8192)); }
   static size_t bytes_for(int64_t n, int64_t m, bool consume_col = false, bool consume_wt = false, bool compressed = false) {
     return 2 * align_up(sizeof(int64_t) * (size_t)(n + 1)) + (consume_col ? 0 : align_up(sizeof(int) * (size_t)m)) +
            (consume_wt ? 0 : align_up((compressed ? 1 : sizeof(int)) * (size_t)m));
@@ -781,16 +861,26 @@ struct HostQuot {
     Generation& G = gen[g];
     G.em.clear();
     G.used = 0;
-    if (G.ovf && G.cap < entries) {
-      cudaFreeHost(G.ovf);
+    const size_t half = spare_bytes / 2 / 256 * 256;
+    if (half >= sizeof(u64) * std::max<size_t>(1, entries)) {  // inside the caller's workspace: no cudaHostAlloc / cudaFreeHost
+      if (G.ovf && G.owned) cudaFreeHost(G.ovf);               // (they cost up to hundreds of milliseconds now and then)
+      G.ovf = (u64*)(spare + (size_t)g * half);
+      G.cap = half / sizeof(u64);
+      G.owned = false;
+      return WL_OK;
+    }
+    if (G.ovf && (G.cap < entries || !G.owned)) {
+      if (G.owned) cudaFreeHost(G.ovf);
       G.ovf = nullptr;
     }
     if (!G.ovf) {
       if (cudaHostAlloc((void**)&G.ovf, sizeof(u64) * std::max<size_t>(1, entries), cudaHostAllocDefault) != cudaSuccess) {
         cudaGetLastError();
+        G.ovf = nullptr;
         return WL_ENOMEM;
       }
       G.cap = entries;
+      G.owned = true;
     }
     return WL_OK;
   }
@@ -820,9 +910,14 @@ struct HostQuot {
       off += align_up(sizeof(int) * (size_t)m);
     }
     wt = consume_wt ? consume_wt : (u32*)(base + off);
+    if (!consume_wt) off += align_up((compressed ? 1 : sizeof(int)) * (size_t)m);
     if (compressed) {
       wt8 = (unsigned char*)wt;
       wt = nullptr;
+    }
+    if (!owned && ws_bytes > off) {  // what lies behind the arrays laid out above
+      spare = base + off;
+      spare_bytes = ws_bytes - off;
     }
     cap_nodes = n;
     cap_edges = m;
@@ -831,7 +926,7 @@ struct HostQuot {
   ~HostQuot() {
     if (owned && base) cudaFreeHost(base);
     for (Generation& G : gen)
-      if (G.ovf) cudaFreeHost(G.ovf);
+      if (G.ovf && G.owned) cudaFreeHost(G.ovf);
   }
 };
 
@@ -919,6 +1014,8 @@ size_t wl_refine_batched_host_bytes_consume(int64_t n, int64_t m, int weighted) 
   if (n < 0 || m < 0 || n > kMaxNodes) return 0;
   return HostQuot::bytes_for(n, m, true, weighted != 0, /*compressed=*/weighted == 0);
 }
+
+size_t wl_refine_batched_host_overflow_bytes(int64_t m) { return m < 0 ? 0 : HostQuot::overflow_bytes_for(m); }
 
 size_t wl_quotient_workspace_bytes(int64_t n, int64_t m) {
   if (n < 0 || m < 0 || n > kMaxNodes) return 0;
@@ -1429,6 +1526,7 @@ static thread_local bool g_input_consumed = false;  // WL_FLAG_CONSUME_INPUT: th
 static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batches, const wl_csr* whole, uint64_t seed,
                        size_t device_cap_bytes, int64_t max_batch_edges, int32_t* out_colors, wl_stats* stats,
                        const wl_options* opt, void* cuda_stream, bool allow_compress = true) {
+  const auto t_entry = std::chrono::steady_clock::now();
   if (stats) std::memset(stats, 0, sizeof(*stats));
   if (n < 0 || num_batches < 0 || max_batch_edges <= 0) return WL_EINVAL;
   if (n > kMaxNodes) return WL_ERANGE;
@@ -1521,6 +1619,16 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
   if (!hs) return WL_ECUDA;
   int dev_id = 0;
   cudaGetDevice(&dev_id);
+  // the caller's device arena, if any (declared before every DevBuf and before the helper thread: it goes last)
+  struct PoolScope {
+    DevPool pool;
+    DevPool* before;
+    PoolScope(void* arena, size_t bytes) : before(g_dev_pool) {
+      pool.init(arena, bytes);
+      g_dev_pool = pool.base ? &pool : nullptr;
+    }
+    ~PoolScope() { g_dev_pool = before; }
+  } pool_scope(opt ? opt->device_workspace : nullptr, opt ? opt->device_workspace_bytes : 0);
   PieceWorker piece_worker(dev_id);  // (declared before everything its tasks touch: it is joined last)
   cudaStream_t copy_st, down_st, side_st;  // uploads; return of quotient rows; refinement of emitted pieces (inherit)
   if (cudaStreamCreateWithFlags(&copy_st, cudaStreamNonBlocking) != cudaSuccess) return check_cuda(cudaGetLastError());
@@ -1605,6 +1713,9 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
   const bool debug = debug_enabled();
   auto wall = [] { return std::chrono::duration<double>(std::chrono::steady_clock::now().time_since_epoch()).count(); };
   double t_mark = wall();
+  if (debug)
+    std::fprintf(stderr, "[wl_refine_batched] host pass over the offsets (S0), streams, events %9.3f ms\n",
+                 std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t_entry).count());
   auto phase = [&](const char* what) {  // WL_DEBUG: host wall-clock per phase (each phase ends on a synchronised stream)
     if (!debug) return;
     cudaStreamSynchronize(st);
@@ -1646,8 +1757,7 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
             rc = check_cuda(cudaStreamSynchronize(st));
           }
           d_cls.release(&used);
-          std::swap(d_cls.p, d_cls_next.p);
-          std::swap(d_cls.bytes, d_cls_next.bytes);
+          d_cls.take(d_cls_next);
           if (rc) loop_done = true;
         }
         rp = hq.rp[1];
@@ -1706,12 +1816,8 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
 #define WL_ALLOC(buf, bytes) \
   if (!rc) rc = buf.alloc((bytes), &used_iter, device_cap_bytes);
     if (have_next) {  // made by the previous iteration's quotient pass
-      d_Hc.p = d_Hnext_keep.p;
-      d_Hc.bytes = d_Hnext_keep.bytes;
-      d_Hnext_keep.p = nullptr;
-      d_isrep.p = d_isrep_keep.p;
-      d_isrep.bytes = d_isrep_keep.bytes;
-      d_isrep_keep.p = nullptr;
+      d_Hc.take(d_Hnext_keep);
+      d_isrep.take(d_isrep_keep);
       used_iter += d_Hc.bytes + d_isrep.bytes;
       if (device_cap_bytes && used_iter > device_cap_bytes) rc = WL_ENOMEM;
     } else {
@@ -2315,8 +2421,7 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
     weighted = true;
     if (init_host) {  // the quotient becomes the current graph
       d_cls.release(&used);
-      std::swap(d_cls.p, d_cls_next.p);
-      std::swap(d_cls.bytes, d_cls_next.bytes);
+      d_cls.take(d_cls_next);
     }
     std::vector<int64_t> next_cuts;
     if (inherit) {
@@ -2341,14 +2446,8 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
     if (inherit || fuse) {
       node_cuts.swap(next_node_cuts);
       next_base_id = base_next;
-      if (d_Hnext_keep.p) cudaFree(d_Hnext_keep.p);
-      if (d_isrep_keep.p) cudaFree(d_isrep_keep.p);
-      d_Hnext_keep.p = d_Hnext.p;  // survive this iteration's buffers
-      d_Hnext_keep.bytes = d_Hnext.bytes;
-      d_Hnext.p = nullptr;
-      d_isrep_keep.p = d_isrep_next.p;
-      d_isrep_keep.bytes = d_isrep_next.bytes;
-      d_isrep_next.p = nullptr;
+      d_Hnext_keep.take(d_Hnext);  // survive this iteration's buffers
+      d_isrep_keep.take(d_isrep_next);
       have_next = true;
     }
   }
@@ -2385,6 +2484,9 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
     stats->kernel_launches = (int32_t)(g_launches - launches_at_entry);
   }
   cleanup();
+  if (debug)
+    std::fprintf(stderr, "[wl_refine_batched] result copy + clean-up %9.3f ms, whole call %9.3f ms\n", 1e3 * (wall() - t_mark),
+                 std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t_entry).count());
   if (rc == WL_OK && hit_limit) return WL_EMAXROUNDS;
   return rc;
 }
@@ -2416,6 +2518,15 @@ int wl_refine_batched(int64_t n, int32_t num_batches, const wl_edge_batch* batch
   // call start over with plain uint32 weights (impossible once the input has been consumed: WL_ENOMEM then)
   g_input_consumed = false;
   auto run = [&](int64_t mb) -> int {
+    const auto t0 = std::chrono::steady_clock::now();
+    struct Trace {
+      std::chrono::steady_clock::time_point t0;
+      ~Trace() {
+        if (debug_enabled())
+          std::fprintf(stderr, "[wl_refine_batched] back in the entry point after %9.3f ms\n",
+                       std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count());
+      }
+    } trace{t0};
     int rc = batched_run(n, num_batches, batches, whole, seed, device_cap_bytes, mb, out_colors, stats, opt, cuda_stream, true);
     if (rc == kCompressOverflow) {
       if (g_input_consumed) return WL_ENOMEM;

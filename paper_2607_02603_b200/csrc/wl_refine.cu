@@ -7,6 +7,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <vector>
 
 #include "wl_deep.cuh"
@@ -309,15 +310,31 @@ int basic_csr_check(const wl_csr* g) {
 // pinned host mirror of the device scalars (one per host thread; released when the thread ends: the batched path runs
 // refinements on a helper thread of its own per call)
 u64* host_scal() {
+  // a block goes back to a process-wide list when its thread ends and is handed to the next new thread: the batched path starts
+  // a helper thread per call, and cudaHostAlloc / cudaFreeHost cost up to hundreds of milliseconds now and then
+  struct Spare {
+    std::mutex mu;
+    std::vector<u64*> blocks;
+  };
+  static Spare* spare = new Spare;  // (never destroyed: threads may end after the statics of this library)
   struct Holder {
     u64* p = nullptr;
     ~Holder() {
-      if (p) cudaFreeHost(p);
+      if (!p) return;
+      std::lock_guard<std::mutex> lock(spare->mu);
+      spare->blocks.push_back(p);
     }
   };
   static thread_local Holder h;
   if (!h.p) {
-    if (cudaHostAlloc((void**)&h.p, sizeof(u64) * (kNumScal + 8), cudaHostAllocDefault) != cudaSuccess) h.p = nullptr;
+    {
+      std::lock_guard<std::mutex> lock(spare->mu);
+      if (!spare->blocks.empty()) {
+        h.p = spare->blocks.back();
+        spare->blocks.pop_back();
+      }
+    }
+    if (!h.p && cudaHostAlloc((void**)&h.p, sizeof(u64) * (kNumScal + 8), cudaHostAllocDefault) != cudaSuccess) h.p = nullptr;
   }
   return h.p;
 }

@@ -393,7 +393,8 @@ def test_batched_validation_reaches_cut_rows_and_host_offsets():
 
 @pytest.mark.parametrize("name", ["rmat11_dir", "weighted", "hub", "grid"])
 @pytest.mark.parametrize("flags", [0, 4096])
-def test_batched_consume_input_overwrites_the_column_array(name, flags):
+@pytest.mark.parametrize("extra", [False, True])
+def test_batched_consume_input_overwrites_the_column_array(name, flags, extra):
     """WL_FLAG_CONSUME_INPUT: the first quotient is written over the caller's column (and weight) array; the scratch holds no
     column array.  Same colouring as without the flag (bit-exact against the CPU Algorithm 2); the input array is clobbered."""
     g = BATCH_GRAPHS[name]()
@@ -403,8 +404,10 @@ def test_batched_consume_input_overwrites_the_column_array(name, flags):
     col = g.col.clone().pin_memory()
     w = None if g.weights is None else g.weights.clone()
     w32 = None if w is None else (w & 0xFFFFFFFF).to(torch.uint32).pin_memory()
-    hws = torch.empty(wl.wl_refine_batched_host_bytes_consume(n, g.m, w is not None), dtype=torch.uint8).pin_memory()
-    assert hws.numel() < wl.wl_refine_batched_host_bytes(n, g.m)
+    # extra: room for the overflow lists of the one-byte weights behind the arrays (else the library pins them itself)
+    hws_bytes = wl.wl_refine_batched_host_bytes_consume(n, g.m, w is not None)
+    assert hws_bytes < wl.wl_refine_batched_host_bytes(n, g.m)
+    hws = torch.empty(hws_bytes + (wl.wl_refine_batched_host_overflow_bytes(g.m) if extra else 0), dtype=torch.uint8).pin_memory()
     res = wl.wl_refine_batched(n, g.row_ptr.pin_memory(), col, w32, max_batch_edges=cap, seed=3,
                                flags=flags | wl.WL_FLAG_CONSUME_INPUT, host_workspace=hws)
     assert res.colors.numpy().tolist() == want.tolist() and res.stats["outer_iters"] == outer_want
@@ -438,6 +441,39 @@ def test_batched_compressed_weights_with_heavy_entries(flags, nb):
         res = wl.wl_refine_batched(n, g.row_ptr, g.col, None, max_batch_edges=cap, seed=5, flags=flags)
         assert res.colors.numpy().tolist() == want.tolist() and res.stats["outer_iters"] == outer_want
         assert oracle.is_stable(n, rp, ci, wt, res.colors.numpy())
+
+
+@pytest.mark.parametrize("flags", [0, 4096, 2048])
+def test_batched_with_a_caller_device_arena(flags):
+    """wl_options.device_workspace: every device buffer of the call is cut from the caller's arena (no cudaMalloc / cudaFree:
+    the driver's free-memory count does not move during the call); a small or misaligned arena only means that some buffers
+    are allocated as before.  Same colouring either way."""
+    g = gg.rmat(13, seed=5, symmetrize=False)
+    n = g.n
+    cap = -(-g.m // 6)
+    want = wl.wl_refine_batched(n, g.row_ptr, g.col, None, max_batch_edges=cap, seed=1, flags=flags)
+    hws = torch.empty(wl.wl_refine_batched_host_bytes(n, g.m), dtype=torch.uint8, pin_memory=True)
+    out = torch.empty(n, dtype=torch.int32, pin_memory=True)
+    arena = torch.empty(64 << 20, dtype=torch.uint8, device="cuda")
+    wl.wl_refine_batched(n, g.row_ptr, g.col, None, max_batch_edges=cap, seed=1, flags=flags, device_workspace=arena,
+                         host_workspace=hws, out=out)  # (first call: module loading and the library's pinned scalars)
+    torch.cuda.synchronize()
+    free0 = torch.cuda.mem_get_info()[0]
+    lows = []
+    for seed in (1, 2):
+        got = wl.wl_refine_batched(n, g.row_ptr, g.col, None, max_batch_edges=cap, seed=seed, flags=flags, device_workspace=arena,
+                                   host_workspace=hws, out=out)
+        lows.append(torch.cuda.mem_get_info()[0])
+        assert got.colors.tolist() == want.colors.tolist() and got.stats["outer_iters"] == want.stats["outer_iters"]
+    assert lows == [free0, free0]
+    for small in (arena[:1 << 20], arena[3:(1 << 22) + 3], arena[:100]):
+        got = wl.wl_refine_batched(n, g.row_ptr, g.col, None, max_batch_edges=cap, seed=3, flags=flags, device_workspace=small)
+        assert got.colors.tolist() == want.colors.tolist()
+    # the cap is still the cap
+    with pytest.raises(wl.WlError) as e:
+        wl.wl_refine_batched(n, g.row_ptr, g.col, None, max_batch_edges=cap, seed=1, flags=flags, device_workspace=arena,
+                             device_cap_bytes=4 * n)
+    assert e.value.code == wl.WL_ENOMEM
 
 
 def test_batched_device_cap_is_checked_for_every_allocation():

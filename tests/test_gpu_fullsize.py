@@ -125,7 +125,7 @@ def test_c5_rmat30_batched_under_16gb_sampled_stability():
     n, rp, col = gg.rmat_directed_to_host(scale, seed=3, device=dev(), pin=True, top_bits=9)
     m = col.numel()
     torch.cuda.empty_cache()
-    hws = torch.empty(wl.wl_refine_batched_host_bytes_consume(n, m), dtype=torch.uint8, pin_memory=True)
+    hws = torch.empty(wl.wl_refine_batched_host_bytes_consume(n, m) + wl.wl_refine_batched_host_overflow_bytes(m), dtype=torch.uint8, pin_memory=True)
     out = torch.empty(n, dtype=torch.int32, pin_memory=True)
     report = {"n": n, "m": m}
     for mode, flags in (("re-cut", 0), ("inherited", wl.WL_FLAG_INHERIT_BATCHES)):
