@@ -1599,13 +1599,37 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
   int64_t max_row_cur = INT64_MAX;  // longest row of the current graph, when known (it bounds the rows of its quotient, Def. 4)
   if (!coo && !(flags & WL_FLAG_NO_VALIDATE)) {
     if (rp[0] != 0) return WL_EINVAL;
-    int64_t longest = 0;
-    for (int64_t i = 0; i < n; ++i) {
-      const int64_t d = rp[i + 1] - rp[i];
-      if (d < 0) return WL_EINVAL;
-      if ((u64)d >= (1ull << 32)) return WL_ERANGE;
-      longest = std::max(longest, d);
+    // (one pass over 8 (n + 1) bytes of host memory: 72 ms on one core at n = 2^26, so it is spread over a few threads)
+    const int nth = n < (1 << 20) ? 1 : (int)std::min<unsigned>(8, std::max(1u, std::thread::hardware_concurrency()));
+    std::vector<int64_t> longest_of(nth, 0);
+    std::vector<int> bad_of(nth, 0);
+    auto scan = [&](int t) {
+      const int64_t i0 = n * t / nth, i1 = n * (t + 1) / nth;
+      int64_t longest = 0;
+      int bad = 0;
+      for (int64_t i = i0; i < i1; ++i) {
+        const int64_t d = rp[i + 1] - rp[i];
+        if (d < 0) bad |= 1;
+        else if ((u64)d >= (1ull << 32)) bad |= 2;
+        longest = std::max(longest, d);
+      }
+      longest_of[t] = longest;
+      bad_of[t] = bad;
+    };
+    {
+      std::vector<std::thread> pool;
+      for (int t = 1; t < nth; ++t) pool.emplace_back(scan, t);
+      scan(0);
+      for (std::thread& th : pool) th.join();
     }
+    int64_t longest = 0;
+    int bad = 0;
+    for (int t = 0; t < nth; ++t) {
+      longest = std::max(longest, longest_of[t]);
+      bad |= bad_of[t];
+    }
+    if (bad & 1) return WL_EINVAL;
+    if (bad & 2) return WL_ERANGE;
     max_row_cur = longest;
   }
 
