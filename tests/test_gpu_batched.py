@@ -474,6 +474,18 @@ def test_batched_with_a_caller_device_arena(flags):
         wl.wl_refine_batched(n, g.row_ptr, g.col, None, max_batch_edges=cap, seed=1, flags=flags, device_workspace=arena,
                              device_cap_bytes=4 * n)
     assert e.value.code == wl.WL_ENOMEM
+    # the other forms and options draw from the arena too: COO batches, initial classes, caller-supplied slices
+    if flags == 0:
+        eb = gg.random_edge_batches(g, 3, 7)
+        coo = gg.coo_batches(g, eb, 3)
+        a = wl.wl_refine_batched(n, None, None, None, max_batch_edges=cap, seed=1, coo_batches=coo)
+        b = wl.wl_refine_batched(n, None, None, None, max_batch_edges=cap, seed=1, coo_batches=coo, device_workspace=arena)
+        assert a.colors.tolist() == b.colors.tolist() and a.stats["outer_iters"] == b.stats["outer_iters"]
+    init = gg.random_partition(n, 4, 2)
+    a = wl.wl_refine_batched(n, g.row_ptr, g.col, None, max_batch_edges=cap, seed=1, flags=flags, init_colors=init)
+    b = wl.wl_refine_batched(n, g.row_ptr, g.col, None, max_batch_edges=cap, seed=1, flags=flags, init_colors=init,
+                             device_workspace=arena)
+    assert a.colors.tolist() == b.colors.tolist() and a.stats["outer_iters"] == b.stats["outer_iters"]
 
 
 def test_batched_device_cap_is_checked_for_every_allocation():
