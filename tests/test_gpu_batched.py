@@ -413,6 +413,15 @@ def test_batched_consume_input_overwrites_the_column_array(name, flags, extra):
     assert res.colors.numpy().tolist() == want.tolist() and res.stats["outer_iters"] == outer_want
     if outer_want >= 2 and k_want < n:
         assert not torch.equal(col, g.col)  # the quotient really went over the input
+    # the same from initial classes
+    init = gg.random_partition(n, 3, 4)
+    want_i, _, outer_i, _ = oracle.rbsc(n, rp, ci, wt, cap, inherit=bool(flags), init=init.numpy())
+    col.copy_(g.col)
+    if w32 is not None:
+        w32.copy_((w & 0xFFFFFFFF).to(torch.uint32))
+    res = wl.wl_refine_batched(n, g.row_ptr.pin_memory(), col, w32, max_batch_edges=cap, seed=3,
+                               flags=flags | wl.WL_FLAG_CONSUME_INPUT, host_workspace=hws, init_colors=init)
+    assert res.colors.numpy().tolist() == want_i.tolist() and res.stats["outer_iters"] == outer_i
 
 
 def _heavy_multigraph():
@@ -441,6 +450,18 @@ def test_batched_compressed_weights_with_heavy_entries(flags, nb):
         res = wl.wl_refine_batched(n, g.row_ptr, g.col, None, max_batch_edges=cap, seed=5, flags=flags)
         assert res.colors.numpy().tolist() == want.tolist() and res.stats["outer_iters"] == outer_want
         assert oracle.is_stable(n, rp, ci, wt, res.colors.numpy())
+        # the same with the overflow lists inside a caller's host workspace (room behind its arrays), and a workspace that is
+        # one byte short of holding them (the library then pins the lists itself)
+        need = wl.wl_refine_batched_host_bytes(n, g.m)
+        for hws_bytes in (need, need + wl.wl_refine_batched_host_overflow_bytes(g.m), need - 1):
+            hws = torch.empty(hws_bytes, dtype=torch.uint8).pin_memory()
+            res = wl.wl_refine_batched(n, g.row_ptr, g.col, None, max_batch_edges=cap, seed=5, flags=flags, host_workspace=hws)
+            assert res.colors.numpy().tolist() == want.tolist() and res.stats["outer_iters"] == outer_want
+        # and from initial classes
+        init = gg.random_partition(n, 3, nb)
+        want_i, _, outer_i, _ = oracle.rbsc(n, rp, ci, wt, cap, inherit=bool(flags & 4096), init=init.numpy())
+        res = wl.wl_refine_batched(n, g.row_ptr, g.col, None, max_batch_edges=cap, seed=5, flags=flags, init_colors=init)
+        assert res.colors.numpy().tolist() == want_i.tolist() and res.stats["outer_iters"] == outer_i
 
 
 @pytest.mark.parametrize("flags", [0, 4096, 2048])
