@@ -326,15 +326,17 @@ constexpr int kQuotLongRow = 4096;  // longer pieces are left to quot_insert_lon
 // the batches of the low-degree node ranges, 5 entries per row on average: 1.45 ms per 33 M entries at 25 % issue activity and 35
 // warps stalled on memory per issue, ncu.)
 constexpr int kQuotGroupRow = 64;
+constexpr int kQuotGroup = 8;                    // lanes per row (4: no different, measured)
+constexpr int kQuotRowsPerWarp = 32 / kQuotGroup;
 __global__ void __launch_bounds__(256)
 quot_insert_kernel(int64_t row_base, int64_t n_rows, const int64_t* __restrict__ row_ptr, int64_t clip_lo, int64_t clip_hi,
                    const int* __restrict__ col, const u32* __restrict__ wt, const int* __restrict__ Hc,
                    const int* __restrict__ rep_of_block, const unsigned char* __restrict__ isrep, Slot* __restrict__ table,
                    u64 table_mask, int* __restrict__ cnt, int* __restrict__ long_rows, u32* __restrict__ long_count) {
-  const int lane = threadIdx.x & 31, sub = lane >> 3, sl = lane & 7;
+  const int lane = threadIdx.x & 31, sub = lane / kQuotGroup, sl = lane % kQuotGroup;
   const int64_t warp = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-  const int64_t w = warp * 4 + sub;
-  if (warp * 4 >= n_rows) return;  // (whole warps only)
+  const int64_t w = warp * kQuotRowsPerWarp + sub;
+  if (warp * kQuotRowsPerWarp >= n_rows) return;  // (whole warps only)
   int b = 0;
   int64_t a = 0, e = 0;
   u64 rbase = 0, rsize = 1;
@@ -358,18 +360,18 @@ quot_insert_kernel(int64_t row_base, int64_t n_rows, const int64_t* __restrict__
   const bool big = live && e - a > kQuotGroupRow;
   int fresh = 0;
   if (live && !big)
-    for (int64_t p = a + sl; p < e; p += 8)
+    for (int64_t p = a + sl; p < e; p += kQuotGroup)
       fresh += quot_insert_at(table, table_mask, rbase, rsize, b, Hc[col[p]], wt ? (u64)wt[p] : 1ull) ? 1 : 0;
-  fresh += __shfl_xor_sync(0xffffffffu, fresh, 4);
-  fresh += __shfl_xor_sync(0xffffffffu, fresh, 2);
-  fresh += __shfl_xor_sync(0xffffffffu, fresh, 1);
+#pragma unroll
+  for (int o = kQuotGroup / 2; o > 0; o >>= 1) fresh += __shfl_xor_sync(0xffffffffu, fresh, o);
   if (sl == 0 && fresh) atomicAdd(cnt + b, fresh);
 #pragma unroll 1
-  for (int g = 0; g < 4; ++g) {  // the longer pieces of the warp's rows, one after the other, by all 32 lanes
-    if (!__shfl_sync(0xffffffffu, big ? 1 : 0, g * 8)) continue;
-    const int64_t ga = __shfl_sync(0xffffffffu, a, g * 8), ge = __shfl_sync(0xffffffffu, e, g * 8);
-    const u64 gbase = __shfl_sync(0xffffffffu, rbase, g * 8), gsize = __shfl_sync(0xffffffffu, rsize, g * 8);
-    const int gb = __shfl_sync(0xffffffffu, b, g * 8);
+  for (int g = 0; g < kQuotRowsPerWarp; ++g) {  // the longer pieces of the warp's rows, one after the other, by all 32 lanes
+    const int src = g * kQuotGroup;
+    if (!__shfl_sync(0xffffffffu, big ? 1 : 0, src)) continue;
+    const int64_t ga = __shfl_sync(0xffffffffu, a, src), ge = __shfl_sync(0xffffffffu, e, src);
+    const u64 gbase = __shfl_sync(0xffffffffu, rbase, src), gsize = __shfl_sync(0xffffffffu, rsize, src);
+    const int gb = __shfl_sync(0xffffffffu, b, src);
     int f = 0;
     for (int64_t p = ga + lane; p < ge; p += 32)
       f += quot_insert_at(table, table_mask, gbase, gsize, gb, Hc[col[p]], wt ? (u64)wt[p] : 1ull) ? 1 : 0;
@@ -976,7 +978,7 @@ static void launch_quot_insert(int64_t row_base, int64_t n_rows, const int64_t* 
                                u32* long_count, cudaStream_t st) {
   if (n_rows <= 0) return;
   cudaMemsetAsync(long_count, 0, sizeof(u32), st);
-  ++g_launches; quot_insert_kernel<<<blocks_for((n_rows + 3) / 4 * 32, 256), 256, 0, st>>>(row_base, n_rows, row_ptr, clip_lo, clip_hi, col, wt, Hc, rep_of_block, isrep, (Slot*)table, table_mask, cnt, long_rows, long_count);
+  ++g_launches; quot_insert_kernel<<<blocks_for((n_rows + kQuotRowsPerWarp - 1) / kQuotRowsPerWarp * 32, 256), 256, 0, st>>>(row_base, n_rows, row_ptr, clip_lo, clip_hi, col, wt, Hc, rep_of_block, isrep, (Slot*)table, table_mask, cnt, long_rows, long_count);
   ++g_launches; quot_insert_long_kernel<<<148 * 8, 256, 0, st>>>(row_base, row_ptr, clip_lo, clip_hi, col, wt, Hc, (Slot*)table, table_mask, cnt, long_rows, long_count);
 }
 
