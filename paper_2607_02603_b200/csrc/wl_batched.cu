@@ -326,13 +326,18 @@ constexpr int kQuotLongRow = 4096;  // longer pieces are left to quot_insert_lon
 // the batches of the low-degree node ranges, 5 entries per row on average: 1.45 ms per 33 M entries at 25 % issue activity and 35
 // warps stalled on memory per issue, ncu.)
 constexpr int kQuotGroupRow = 64;
-constexpr int kQuotGroup = 8;                    // lanes per row (4: no different, measured)
-constexpr int kQuotRowsPerWarp = 32 / kQuotGroup;
+// kQuotGroup lanes per row in batches of short rows (4: no different, measured); batches whose rows average more than
+// kQuotGroupAvg entries keep one warp per row: there the rows are few (a hub-heavy batch of 33 M entries has 10 000 of them) and
+// four rows per warp left three quarters of the warp slots empty (12-38 % warps active, 0.95-2.2 ms per batch, ncu)
+constexpr int kQuotGroupShort = 8;
+constexpr int kQuotGroupAvg = 24;
+template <int kQuotGroup>
 __global__ void __launch_bounds__(256)
 quot_insert_kernel(int64_t row_base, int64_t n_rows, const int64_t* __restrict__ row_ptr, int64_t clip_lo, int64_t clip_hi,
                    const int* __restrict__ col, const u32* __restrict__ wt, const int* __restrict__ Hc,
                    const int* __restrict__ rep_of_block, const unsigned char* __restrict__ isrep, Slot* __restrict__ table,
                    u64 table_mask, int* __restrict__ cnt, int* __restrict__ long_rows, u32* __restrict__ long_count) {
+  constexpr int kQuotRowsPerWarp = 32 / kQuotGroup;
   const int lane = threadIdx.x & 31, sub = lane / kQuotGroup, sl = lane % kQuotGroup;
   const int64_t warp = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   const int64_t w = warp * kQuotRowsPerWarp + sub;
@@ -357,7 +362,7 @@ quot_insert_kernel(int64_t row_base, int64_t n_rows, const int64_t* __restrict__
       }
     }
   }
-  const bool big = live && e - a > kQuotGroupRow;
+  const bool big = kQuotGroup < 32 && live && e - a > kQuotGroupRow;
   int fresh = 0;
   if (live && !big)
     for (int64_t p = a + sl; p < e; p += kQuotGroup)
@@ -366,7 +371,7 @@ quot_insert_kernel(int64_t row_base, int64_t n_rows, const int64_t* __restrict__
   for (int o = kQuotGroup / 2; o > 0; o >>= 1) fresh += __shfl_xor_sync(0xffffffffu, fresh, o);
   if (sl == 0 && fresh) atomicAdd(cnt + b, fresh);
 #pragma unroll 1
-  for (int g = 0; g < kQuotRowsPerWarp; ++g) {  // the longer pieces of the warp's rows, one after the other, by all 32 lanes
+  for (int g = 0; g < (kQuotGroup < 32 ? kQuotRowsPerWarp : 0); ++g) {  // the longer pieces of the warp's rows, one after the other, by all 32 lanes
     const int src = g * kQuotGroup;
     if (!__shfl_sync(0xffffffffu, big ? 1 : 0, src)) continue;
     const int64_t ga = __shfl_sync(0xffffffffu, a, src), ge = __shfl_sync(0xffffffffu, e, src);
@@ -979,10 +984,15 @@ void launch_scan32(const int* cnt, int64_t n, int64_t base_off, int64_t* out, u6
 static void launch_quot_insert(int64_t row_base, int64_t n_rows, const int64_t* row_ptr, int64_t clip_lo, int64_t clip_hi,
                                const int* col, const u32* wt, const int* Hc, const int* rep_of_block,
                                const unsigned char* isrep, u64* table, u64 table_mask, int* cnt, int* long_rows,
-                               u32* long_count, cudaStream_t st) {
+                               u32* long_count, cudaStream_t st, int64_t entries_hint) {  // entries_hint: entries of these rows, roughly
   if (n_rows <= 0) return;
   cudaMemsetAsync(long_count, 0, sizeof(u32), st);
-  ++g_launches; quot_insert_kernel<<<blocks_for((n_rows + kQuotRowsPerWarp - 1) / kQuotRowsPerWarp * 32, 256), 256, 0, st>>>(row_base, n_rows, row_ptr, clip_lo, clip_hi, col, wt, Hc, rep_of_block, isrep, (Slot*)table, table_mask, cnt, long_rows, long_count);
+  if (entries_hint > kQuotGroupAvg * n_rows) {
+    ++g_launches; quot_insert_kernel<32><<<blocks_for(n_rows * 32, 256), 256, 0, st>>>(row_base, n_rows, row_ptr, clip_lo, clip_hi, col, wt, Hc, rep_of_block, isrep, (Slot*)table, table_mask, cnt, long_rows, long_count);
+  } else {
+    constexpr int rpw = 32 / kQuotGroupShort;
+    ++g_launches; quot_insert_kernel<kQuotGroupShort><<<blocks_for((n_rows + rpw - 1) / rpw * 32, 256), 256, 0, st>>>(row_base, n_rows, row_ptr, clip_lo, clip_hi, col, wt, Hc, rep_of_block, isrep, (Slot*)table, table_mask, cnt, long_rows, long_count);
+  }
   ++g_launches; quot_insert_long_kernel<<<148 * 8, 256, 0, st>>>(row_base, row_ptr, clip_lo, clip_hi, col, wt, Hc, (Slot*)table, table_mask, cnt, long_rows, long_count);
 }
 
@@ -1096,7 +1106,7 @@ int wl_quotient(const wl_csr* g, const int32_t* colors, int64_t k, int64_t* q_ro
   cudaMemsetAsync(cursor, 0, sizeof(int) * (size_t)k, st);
   ++g_launches; block_rep_kernel<<<blocks_for(n, 256), 256, 0, st>>>(n, colors, rep_of_block);
   launch_quot_insert(0, n, g->row_ptr, 0, m, g->col_idx, g->weights, colors, rep_of_block, nullptr, table, slots - 1, cnt, long_rows,
-                     (u32*)(total + 1), st);
+                     (u32*)(total + 1), st, m);
   launch_scan32(cnt, k, 0, q_row_ptr, bsum, total, st);
   u64 h_total = 0;
   cudaMemcpyAsync(&h_total, total, sizeof(u64), cudaMemcpyDeviceToHost, st);
@@ -1199,7 +1209,7 @@ int wl_quotient_rows(const wl_csr* rows, int64_t lo, const int32_t* block_of, co
   cudaMemsetAsync(cursor, 0, sizeof(int) * (size_t)(num_blocks + 1), st);
   // the kernels index the block map by global node id and the counters by global block id
   launch_quot_insert(lo, nr, rows->row_ptr, /*clip_lo=*/INT64_MIN / 2, /*clip_hi=*/INT64_MAX / 2, rows->col_idx, rows->weights,
-                     block_of, nullptr, is_first - lo, table, slots - 1, cnt - first_block, long_rows, (u32*)(total + 1), st);
+                     block_of, nullptr, is_first - lo, table, slots - 1, cnt - first_block, long_rows, (u32*)(total + 1), st, rows->m);
   launch_scan32(cnt, num_blocks, 0, q_row_ptr, bsum, total, st);
   u64 h_total = 0;
   cudaMemcpyAsync(&h_total, total, sizeof(u64), cudaMemcpyDeviceToHost, st);
@@ -2367,7 +2377,7 @@ static int batched_run(int64_t n, int32_t num_batches, const wl_edge_batch* batc
         // rows that cross a cut arrive in pieces: the kernel clips every row to [c0, c1)
         launch_quot_insert(na[k], nz[k] - na[k], d_rp[buf].as<int64_t>(), c0, c1, d_col[buf].as<int>() - c0,
                            weighted ? d_wt[buf].as<u32>() - c0 : nullptr, d_Hc.as<int>(), nullptr, d_isrep.as<unsigned char>(),
-                           d_qtab.as<u64>(), qslots - 1, d_cnt.as<int>() - wb, d_long.as<int>(), (u32*)(d_misc.as<u64>() + 16), st);
+                           d_qtab.as<u64>(), qslots - 1, d_cnt.as<int>() - wb, d_long.as<int>(), (u32*)(d_misc.as<u64>() + 16), st, c1 - c0);
       }
       cudaEventRecord(ev_ins[buf], st);
       checkpoint("insert", k);
