@@ -71,6 +71,25 @@ def test_static_at_the_maximum_in_place_and_without_a_count():
     assert k.item() == -1
 
 
+def test_static_on_a_side_stream_two_calls_in_a_row():
+    """The call only enqueues on the stream it is given: two calls back to back on a non-default stream, the second one over the
+    first one's output (canonical ids are a fixed point of S6), read after synchronising that stream only."""
+    c = _colours(200_003, 50_000, 7)
+    t = torch.from_numpy(c).to(dev())
+    want, want_k = wl.wl_canonicalize(t)
+    torch.cuda.synchronize()
+    side = torch.cuda.Stream(dev())
+    a, b = torch.empty_like(t), torch.empty_like(t)
+    ka = torch.zeros(1, dtype=torch.int64, device=dev())
+    kb = torch.zeros(1, dtype=torch.int64, device=dev())
+    with torch.cuda.stream(side):
+        wl.wl_canonicalize_static(t, a, ka)
+        wl.wl_canonicalize_static(a, b, kb)
+    side.synchronize()
+    assert torch.equal(a, want) and torch.equal(b, want)
+    assert ka.item() == kb.item() == want_k
+
+
 def test_static_rejects_what_it_cannot_hold():
     nmax = wl.wl_canonicalize_static_max_nodes()
     t = torch.zeros(nmax + 1, dtype=torch.int32, device=dev())
