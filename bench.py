@@ -430,6 +430,8 @@ def run_cap_sweep(args):
     torch.cuda.empty_cache()
     hws = torch.empty(wl.wl_refine_batched_host_bytes(n, m), dtype=torch.uint8, pin_memory=True)
     out = torch.empty(n, dtype=torch.int32, pin_memory=True)
+    # caller-owned device arena (wl_options.device_workspace): the timed calls allocate nothing on the device
+    arena = None if args.no_arena else torch.empty(int(args.cap_gb * (1 << 30)), dtype=torch.uint8, device=dev)
     rows = []
     for cap_edges in (args.batch_edges, 4 * args.batch_edges):
         for name, flags in (("aggressive (L328)", wl.WL_FLAG_AGGRESSIVE_STOP), ("paper termination (L200)", 0),
@@ -439,7 +441,7 @@ def run_cap_sweep(args):
                 torch.cuda.synchronize(dev)
                 t0 = time.perf_counter()
                 r = wl.wl_refine_batched(n, rp, col, None, max_batch_edges=cap_edges, seed=20 + rep, flags=flags,
-                                         host_workspace=hws, out=out)
+                                         host_workspace=hws, out=out, device_workspace=arena)
                 torch.cuda.synchronize(dev)
                 dt = time.perf_counter() - t0
                 best = dt if best is None else min(best, dt)
@@ -448,7 +450,8 @@ def run_cap_sweep(args):
                          "coarsest_pct": None if single is None else 100.0 * single / n,
                          "first_num_batches": -(-m // cap_edges)})
     print(json.dumps({"metric": "cap_sweep", "unit": "table", "data": "synthetic",
-                      "config": {"workload": f"R-MAT scale {args.scale}, directed, seed 3", "n": n, "m": m}, "rows": rows}))
+                      "config": {"workload": f"R-MAT scale {args.scale}, directed, seed 3", "n": n, "m": m,
+                                 "device_arena_gb": None if arena is None else args.cap_gb}, "rows": rows}))
     return 0
 
 
